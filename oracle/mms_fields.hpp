@@ -1,0 +1,96 @@
+// oracle/mms_fields.hpp -- TEST INFRASTRUCTURE (CPU oracle). Not part of the product path.
+//
+// Exact manufactured fields Q_exact(x, t) of the systems that carry MMS forcing, as jets, and the
+// manufactured source of eq (4.1), formed for the AUGMENTED system (trackers
+// forced too, with G_exact = grad V_exact; SURVEY.md §8(c) reading A5, confirmed on the ADR row of
+// Table 2).
+//   burgers2d mms 1 : eq (SM5.1), A = mms_par[0] (Table SM3: 1.3)
+//   euler2d   mms 1 : eq (SM5.2), non-dimensional rho0 = c_s = 1 (reading A9)
+//   adr2d     mms 1 : eq (SM5.7), Table SM8
+//   swe2d     mms 1 : BASELINE.json configs[1] fields, mms_par = {A_h, A_u, h0}
+//   nsf3d     mms 1 : BASELINE.json configs[3] fields, mms_par = {U0, A_rho, rho0, p0}
+#pragma once
+#include "jets.hpp"
+#include "systems.hpp"
+
+namespace orc {
+
+constexpr double PI = 3.14159265358979323846;
+
+// Q[k] (value + first derivatives in t,x,y,z) of the exact augmented state at one point.
+// returns false if (sys, mms_id) has no manufactured solution.
+inline bool exact_state(int sys, int mms_id, const Scaling& sc, const double* mp,
+                        double t_, double x_, double y_, double z_, J1* Q) {
+    if (mms_id != 1) return false;
+    const J2 t = J2::variable(0, t_), x = J2::variable(1, x_), y = J2::variable(2, y_), z = J2::variable(3, z_);
+    const double k = 2.0 * PI;
+    switch (sys) {
+    case SYS_BURGERS2D: {
+        J2 u = mp[0] * sin(k * x) * sin(k * y) * cos(t);
+        Q[0] = lower(u);
+        return true;
+    }
+    case SYS_EULER2D: {
+        const double gamma = sc.par[0], rho0 = 1.0, cs = 1.0, p0 = rho0 * cs * cs / gamma, u0 = 3.0 * cs, v0 = 3.0 * cs;
+        J2 drho = 0.3 * rho0 * sin(k * x) * cos(k * y) * cos(t);
+        J2 du = 0.3 * cs * cos(k * x) * sin(k * y) * sin(t);
+        J2 dv = 0.3 * cs * sin(k * x) * sin(k * y) * sin(t);
+        J2 dp = cs * cs * drho + 0.2 * p0 * cos(k * x) * sin(k * y) * sin(t);
+        J2 rho = rho0 + drho, u = u0 + du, v = v0 + dv, p = p0 + dp;
+        J2 E = p / (gamma - 1.0) + 0.5 * rho * (u * u + v * v);
+        Q[0] = lower(rho); Q[1] = lower(rho * u); Q[2] = lower(rho * v); Q[3] = lower(E);
+        return true;
+    }
+    case SYS_SWE2D: {
+        const double Ah = mp[0], Au = mp[1], h0 = mp[2];
+        J2 h = h0 + Ah * sin(k * x) * cos(k * y) * cos(t);
+        J2 u = Au * cos(k * x) * sin(k * y) * cos(t);
+        J2 v = Au * sin(k * x) * sin(k * y) * sin(t);
+        Q[0] = lower(h); Q[1] = lower(h * u); Q[2] = lower(h * v);
+        return true;
+    }
+    case SYS_ADR2D: {
+        const double u0 = sc.par[0], u1 = sc.par[1];
+        J2 c = 0.5 * sin(k * (x - u0 * t)) * cos(k * (y - u1 * t)) * exp(-t) + 0.5;
+        Q[0] = lower(c);
+        Q[1] = sc.dx * diff(c, 1);
+        Q[2] = sc.dx * diff(c, 2);
+        return true;
+    }
+    case SYS_NSF3D: {
+        const double gamma = sc.par[0], mu = sc.par[1];
+        const double U0 = mp[0], Ar = mp[1], rho0 = mp[2], p0 = mp[3];
+        J2 D = exp((-3.0 * (mu / rho0) * k * k) * t);
+        J2 sx = sin(k * x), cx = cos(k * x), sy = sin(k * y), cy = cos(k * y), sz = sin(k * z), cz = cos(k * z);
+        J2 u[3] = {U0 * sx * cy * cz * D, -U0 * cx * sy * cz * D, 0.5 * U0 * cx * cy * sz * D};
+        J2 p = p0 + (rho0 * U0 * U0 / 16.0) * (cos(2.0 * k * x) + cos(2.0 * k * y)) * (cos(2.0 * k * z) + 2.0) * D * D;
+        J2 rho = rho0 * (1.0 + Ar * sx * sy * cz * cos(t));
+        J2 Tm = p / rho;
+        J2 E = p / (gamma - 1.0) + 0.5 * rho * (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);
+        Q[0] = lower(rho);
+        for (int a = 0; a < 3; ++a) Q[1 + a] = lower(rho * u[a]);
+        Q[4] = lower(E);
+        for (int a = 0; a < 3; ++a)
+            for (int b = 0; b < 3; ++b) Q[5 + 3 * a + b] = sc.dx * diff(u[a], 1 + b);
+        for (int b = 0; b < 3; ++b) Q[14 + b] = sc.dx * diff(Tm, 1 + b);
+        return true;
+    }
+    }
+    return false;
+}
+
+// Lattice manufactured source at one point:
+//   s_mms[k] = dt * d_t Q_k + dx * sum_a d_a F_k,a(Q_exact) - S_k(Q_exact)      (eq 4.1 in lattice units;
+//   F = (dt/dx) Phi and S = dt * S_phys, so this is dt * [d_t Q + div Phi - S_phys].)
+inline bool mms_source(int sys, int mms_id, const Scaling& sc, const double* mp,
+                       double t, double x, double y, double z, double* s_mms) {
+    J1 Q[MAXM], F[MAXM * 3], S[MAXM];
+    if (!exact_state(sys, mms_id, sc, mp, t, x, y, z, Q)) return false;
+    flux_source<J1>(sys, Q, sc, F, S);
+    const int m = sys_info(sys).m_total;
+    for (int k = 0; k < m; ++k)
+        s_mms[k] = sc.dt * Q[k].d[0] + sc.dx * (F[k * 3 + 0].d[1] + F[k * 3 + 1].d[2] + F[k * 3 + 2].d[3]) - S[k].v;
+    return true;
+}
+
+}  // namespace orc

@@ -1,0 +1,225 @@
+// oracle/systems.hpp -- TEST INFRASTRUCTURE (CPU oracle). Not part of the product path.
+//
+// The conservation-law systems d_t Q + div Phi = S (eq 2.1) the oracle knows,
+// each as ONE templated function returning, for a state U (conserved + tracker components):
+//     F[k][a] = lattice flux      = (dt/dx) * Phi_k,a           (eq 2.7 bracket)
+//     S[k]    = lattice source    =  dt * S_k(U)                (state-dependent part only; L298)
+// Trackers are carried in lattice units G^L = dx * grad V (exponents (p-1,q)), so
+// their flux G (x) u - I V/tau_grad and source -G/tau_grad of eq (2.3) read
+//     F_G[b][j] = G_b u_j / lambda - delta_jb V / g_tau ,  S_G = -G / g_tau ,  tau_grad = g_tau dt (L106).
+// A physical diffusivity D multiplying a tracked gradient enters as D_L = D dt/dx^2.
+// The function is templated on the scalar type so the SAME flux serves the time stepping (double)
+// and the manufactured residual of eq (4.1) (jets, see jets.hpp).
+#pragma once
+#include <cmath>
+#include "jets.hpp"
+
+namespace orc {
+
+enum SystemId { SYS_ADVECTION2D = 0, SYS_BURGERS2D = 1, SYS_SWE2D = 2, SYS_EULER2D = 3, SYS_ADR2D = 4,
+                SYS_NSF3D = 5, SYS_MHD3D = 6, SYS_COUNT = 7 };
+
+constexpr int MAXM = 32;  // max components
+
+struct SysInfo { int m_conserved, m_total, dim; };
+inline SysInfo sys_info(int sys) {
+    switch (sys) {
+        case SYS_ADVECTION2D: return {1, 1, 2};
+        case SYS_BURGERS2D:   return {1, 1, 2};
+        case SYS_SWE2D:       return {3, 3, 2};
+        case SYS_EULER2D:     return {4, 4, 2};
+        case SYS_ADR2D:       return {1, 3, 2};
+        case SYS_NSF3D:       return {5, 17, 3};
+        case SYS_MHD3D:       return {8, 11, 3};
+    }
+    return {0, 0, 0};
+}
+
+struct Scaling {
+    const double* par;  // physical parameters of the system (order: see each case)
+    double dx, dt, lam; // lam = dx/dt
+    double g_tau;       // tracker step count, tau_grad = g_tau * dt
+};
+
+// F[k*3 + a], S[k]
+template <class T>
+void flux_source(int sys, const T* U, const Scaling& sc, T* F, T* S) {
+    const double il = 1.0 / sc.lam;           // dt/dx
+    const double dL = sc.dt / (sc.dx * sc.dx); // physical diffusivity -> lattice diffusivity
+    const SysInfo si = sys_info(sys);
+    for (int k = 0; k < si.m_total; ++k) { S[k] = T(0.0); for (int a = 0; a < 3; ++a) F[k * 3 + a] = T(0.0); }
+    switch (sys) {
+    case SYS_ADVECTION2D: {
+        // linear advection, Phi = (a_x U, a_y U); par = {a_x, a_y}
+        F[0] = (sc.par[0] * il) * U[0];
+        F[1] = (sc.par[1] * il) * U[0];
+    } break;
+    case SYS_BURGERS2D: {
+        // eq (3.1)-(3.2): Phi = (u^2/2, u^2/2)
+        T h = 0.5 * U[0] * U[0];
+        F[0] = il * h;
+        F[1] = il * h;
+    } break;
+    case SYS_SWE2D: {
+        // eq (3.6), flat bottom; par = {g}
+        const double g = sc.par[0];
+        T h = U[0], hu = U[1], hv = U[2];
+        T u = hu / h, v = hv / h;
+        T P = 0.5 * g * h * h;
+        F[0 * 3 + 0] = il * hu;            F[0 * 3 + 1] = il * hv;
+        F[1 * 3 + 0] = il * (hu * u + P);  F[1 * 3 + 1] = il * (hu * v);
+        F[2 * 3 + 0] = il * (hv * u);      F[2 * 3 + 1] = il * (hv * v + P);
+    } break;
+    case SYS_EULER2D: {
+        // eq (3.4); p = (gamma-1)(E - rho|u|^2/2); par = {gamma}
+        const double gamma = sc.par[0];
+        T rho = U[0], mx = U[1], my = U[2], E = U[3];
+        T u = mx / rho, v = my / rho;
+        T p = (gamma - 1.0) * (E - 0.5 * (mx * u + my * v));
+        F[0 * 3 + 0] = il * mx;            F[0 * 3 + 1] = il * my;
+        F[1 * 3 + 0] = il * (mx * u + p);  F[1 * 3 + 1] = il * (mx * v);
+        F[2 * 3 + 0] = il * (my * u);      F[2 * 3 + 1] = il * (my * v + p);
+        F[3 * 3 + 0] = il * ((E + p) * u); F[3 * 3 + 1] = il * ((E + p) * v);
+    } break;
+    case SYS_ADR2D: {
+        // eq (3.17); SM4.7 L908-L926; par = {u_x, u_y, D, R}; U = (c, G^L_x, G^L_y)
+        const double ux = sc.par[0], uy = sc.par[1], D = sc.par[2], R = sc.par[3];
+        const double DL = D * dL;
+        T c = U[0], Gx = U[1], Gy = U[2];
+        F[0 * 3 + 0] = (ux * il) * c - DL * Gx;
+        F[0 * 3 + 1] = (uy * il) * c - DL * Gy;
+        F[1 * 3 + 0] = (ux * il) * Gx - c / sc.g_tau;  F[1 * 3 + 1] = (uy * il) * Gx;
+        F[2 * 3 + 0] = (ux * il) * Gy;                 F[2 * 3 + 1] = (uy * il) * Gy - c / sc.g_tau;
+        S[0] = sc.dt * R * c * (1.0 - c);
+        S[1] = -Gx / sc.g_tau;
+        S[2] = -Gy / sc.g_tau;
+    } break;
+    case SYS_NSF3D: {
+        // eq (3.23), with the derived-parent trackers of eq (3.27) (L495-L497):
+        // G^L_ab = dx d_b u_a (9 components, index 5+3a+b), H^L_b = dx d_b T (index 14+b), T = p/rho (R = 1).
+        // par = {gamma, mu, K}
+        const double gamma = sc.par[0], muL = sc.par[1] * dL, KL = sc.par[2] * dL;
+        T rho = U[0], E = U[4];
+        T m[3] = {U[1], U[2], U[3]};
+        T u[3] = {m[0] / rho, m[1] / rho, m[2] / rho};
+        T p = (gamma - 1.0) * (E - 0.5 * (m[0] * u[0] + m[1] * u[1] + m[2] * u[2]));
+        T Tm = p / rho;
+        const T* G = U + 5;   // G[3a+b]
+        const T* H = U + 14;  // H[b]
+        T trG = G[0] + G[4] + G[8];
+        T sig[3][3];  // lattice viscous stress  mu_L (G + G^T - 2/3 tr G I)
+        for (int a = 0; a < 3; ++a)
+            for (int b = 0; b < 3; ++b) {
+                sig[a][b] = muL * (G[3 * a + b] + G[3 * b + a]);
+                if (a == b) sig[a][b] = sig[a][b] - (2.0 / 3.0) * muL * trG;
+            }
+        for (int j = 0; j < 3; ++j) {
+            F[0 * 3 + j] = il * m[j];
+            for (int a = 0; a < 3; ++a) {
+                F[(1 + a) * 3 + j] = il * (m[a] * u[j]) - sig[a][j];
+                if (a == j) F[(1 + a) * 3 + j] = F[(1 + a) * 3 + j] + il * p;
+            }
+            F[4 * 3 + j] = il * ((E + p) * u[j]) - (sig[j][0] * u[0] + sig[j][1] * u[1] + sig[j][2] * u[2]) - KL * H[j];
+            for (int a = 0; a < 3; ++a)
+                for (int b = 0; b < 3; ++b) {
+                    F[(5 + 3 * a + b) * 3 + j] = il * (G[3 * a + b] * u[j]);
+                    if (j == b) F[(5 + 3 * a + b) * 3 + j] = F[(5 + 3 * a + b) * 3 + j] - u[a] / sc.g_tau;
+                }
+            for (int b = 0; b < 3; ++b) {
+                F[(14 + b) * 3 + j] = il * (H[b] * u[j]);
+                if (j == b) F[(14 + b) * 3 + j] = F[(14 + b) * 3 + j] - Tm / sc.g_tau;
+            }
+        }
+        for (int q = 0; q < 9; ++q) S[5 + q] = -G[q] / sc.g_tau;
+        for (int b = 0; b < 3; ++b) S[14 + b] = -H[b] / sc.g_tau;
+    } break;
+    case SYS_MHD3D: {
+        // eq (3.25), inviscid, no heat flux, no Powell source, with a current-density
+        // tracker J^L = dx curl B (index 8..10) in place of the full grad B:
+        // the resistive flux -eta grad B of the induction equation equals +eta eps_ijk J_k up to
+        // eta grad(div B); energy carries eta (J x B). par = {gamma, eta}
+        const double gamma = sc.par[0], etaL = sc.par[1] * dL;
+        T rho = U[0], E = U[4];
+        T m[3] = {U[1], U[2], U[3]};
+        T B[3] = {U[5], U[6], U[7]};
+        T J[3] = {U[8], U[9], U[10]};
+        T u[3] = {m[0] / rho, m[1] / rho, m[2] / rho};
+        T B2 = B[0] * B[0] + B[1] * B[1] + B[2] * B[2];
+        T p = (gamma - 1.0) * (E - 0.5 * (m[0] * u[0] + m[1] * u[1] + m[2] * u[2]) - 0.5 * B2);
+        T pt = p + 0.5 * B2;
+        T uB = u[0] * B[0] + u[1] * B[1] + u[2] * B[2];
+        T JxB[3] = {J[1] * B[2] - J[2] * B[1], J[2] * B[0] - J[0] * B[2], J[0] * B[1] - J[1] * B[0]};
+        for (int j = 0; j < 3; ++j) {
+            F[0 * 3 + j] = il * m[j];
+            for (int a = 0; a < 3; ++a) {
+                F[(1 + a) * 3 + j] = il * (m[a] * u[j] - B[a] * B[j]);
+                if (a == j) F[(1 + a) * 3 + j] = F[(1 + a) * 3 + j] + il * pt;
+            }
+            F[4 * 3 + j] = il * ((E + pt) * u[j] - B[j] * uB) + etaL * JxB[j];
+            for (int i = 0; i < 3; ++i) {
+                F[(5 + i) * 3 + j] = il * (B[i] * u[j] - u[i] * B[j]);
+                F[(8 + i) * 3 + j] = il * (J[i] * u[j]);
+            }
+        }
+        // + eta_L eps_ijk J_k  and  - eps_ijk B_k / g_tau   (i = component, j = flux direction)
+        const int eps[6][4] = {{0, 1, 2, +1}, {1, 2, 0, +1}, {2, 0, 1, +1}, {0, 2, 1, -1}, {2, 1, 0, -1}, {1, 0, 2, -1}};
+        for (int e = 0; e < 6; ++e) {
+            const int i = eps[e][0], j = eps[e][1], k = eps[e][2];
+            const double s = eps[e][3];
+            F[(5 + i) * 3 + j] = F[(5 + i) * 3 + j] + (s * etaL) * J[k];
+            F[(8 + i) * 3 + j] = F[(8 + i) * 3 + j] - (s / sc.g_tau) * B[k];
+        }
+        for (int i = 0; i < 3; ++i) S[8 + i] = -J[i] / sc.g_tau;
+    } break;
+    }
+}
+
+// Wave speeds for the sub-characteristic condition (eq 2.19-2.20; L329).
+// out[0] = max over axes of (|u_a| + c_a)   (per-axis ceiling seen by D2Q5/D3Q7 streaming)
+// out[1] = |u| + c                          (isotropic bound over all directions n)
+// out[2] = lattice diffusive signal speed sqrt(kappa_L/g_tau) of the tracker-parent coupling (0 if none)
+// out[0], out[1] physical (divide by lambda for lattice units); out[2] already lattice.
+inline void wave_speeds(int sys, const double* U, const Scaling& sc, double* out) {
+    const double dL = sc.dt / (sc.dx * sc.dx);
+    out[0] = out[1] = out[2] = 0.0;
+    auto set = [&](const double* u, const double* c, int D) {
+        double un = 0.0, cmax = 0.0;
+        for (int a = 0; a < D; ++a) { out[0] = std::fmax(out[0], std::fabs(u[a]) + c[a]); un += u[a] * u[a]; cmax = std::fmax(cmax, c[a]); }
+        out[1] = std::sqrt(un) + cmax;
+    };
+    switch (sys) {
+    case SYS_ADVECTION2D: { double u[2] = {sc.par[0], sc.par[1]}, c[2] = {0, 0}; set(u, c, 2); } break;
+    case SYS_BURGERS2D:   { double u[2] = {U[0], U[0]}, c[2] = {0, 0}; set(u, c, 2); } break;  // f'(u) = u per axis
+    case SYS_SWE2D:       { double cc = std::sqrt(sc.par[0] * U[0]); double u[2] = {U[1] / U[0], U[2] / U[0]}, c[2] = {cc, cc}; set(u, c, 2); } break;
+    case SYS_EULER2D: {
+        double u[2] = {U[1] / U[0], U[2] / U[0]};
+        double p = (sc.par[0] - 1.0) * (U[3] - 0.5 * U[0] * (u[0] * u[0] + u[1] * u[1]));
+        double cc = std::sqrt(sc.par[0] * p / U[0]); double c[2] = {cc, cc}; set(u, c, 2);
+    } break;
+    case SYS_ADR2D: { double u[2] = {sc.par[0], sc.par[1]}, c[2] = {0, 0}; set(u, c, 2); out[2] = std::sqrt(sc.par[2] * dL / sc.g_tau); } break;
+    case SYS_NSF3D: {
+        double u[3] = {U[1] / U[0], U[2] / U[0], U[3] / U[0]};
+        double p = (sc.par[0] - 1.0) * (U[4] - 0.5 * U[0] * (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]));
+        double cc = std::sqrt(sc.par[0] * p / U[0]); double c[3] = {cc, cc, cc}; set(u, c, 3);
+        double kap = std::fmax(4.0 * sc.par[1] * dL / (3.0 * U[0]), sc.par[2] * dL * (sc.par[0] - 1.0) / U[0]);
+        out[2] = std::sqrt(kap / sc.g_tau);
+    } break;
+    case SYS_MHD3D: {
+        double rho = U[0];
+        double u[3] = {U[1] / rho, U[2] / rho, U[3] / rho};
+        double B2 = U[5] * U[5] + U[6] * U[6] + U[7] * U[7];
+        double p = (sc.par[0] - 1.0) * (U[4] - 0.5 * rho * (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]) - 0.5 * B2);
+        double a2 = sc.par[0] * p / rho, b2 = B2 / rho;
+        double c[3];
+        for (int a = 0; a < 3; ++a) {
+            double ba2 = U[5 + a] * U[5 + a] / rho;
+            c[a] = std::sqrt(0.5 * (a2 + b2 + std::sqrt(std::fmax((a2 + b2) * (a2 + b2) - 4.0 * a2 * ba2, 0.0))));
+        }
+        set(u, c, 3);
+        out[1] = std::sqrt(u[0] * u[0] + u[1] * u[1] + u[2] * u[2]) + std::sqrt(a2 + b2);
+        out[2] = std::sqrt(sc.par[1] * dL / sc.g_tau);
+    } break;
+    }
+}
+
+}  // namespace orc

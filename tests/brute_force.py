@@ -1,0 +1,75 @@
+"""Brute-force NumPy collide-and-stream step, written directly from the moment definitions
+(eq 2.6, 2.7, 2.11 of PAPER.md) with explicit sums and np.roll -- pin P13 of SURVEY.md §8(c).
+
+Independent of `oracle/` (own lattice tables, own streaming, own fluxes).  The fluxes are typed
+from the paper's *expanded component listings* (SM4.2, SM4.3, SM4.7), i.e. a different algebraic
+form than the primitive-variable form the oracle uses.
+"""
+import numpy as np
+
+# Table SM1
+LATTICES = {
+    2: dict(c=[(0, 0, 0), (1, 0, 0), (-1, 0, 0), (0, 1, 0), (0, -1, 0)],
+            w=[1 / 3, 1 / 6, 1 / 6, 1 / 6, 1 / 6], cs2=1 / 3),
+    3: dict(c=[(0, 0, 0), (1, 0, 0), (-1, 0, 0), (0, 1, 0), (0, -1, 0), (0, 0, 1), (0, 0, -1)],
+            w=[1 / 4, 1 / 8, 1 / 8, 1 / 8, 1 / 8, 1 / 8, 1 / 8], cs2=1 / 4),
+}
+
+
+def flux_euler_listing(U, gamma):
+    """SM4.2, PAPER.md:L819 (expanded component form). U[k] arrays; returns Phi[k][a] physical."""
+    rho, m0, m1, E = U
+    P10 = E * gamma - E - gamma * m0**2 / (2 * rho) - gamma * m1**2 / (2 * rho) + 3 * m0**2 / (2 * rho) + m1**2 / (2 * rho)
+    P11 = m0 * m1 / rho
+    P21 = E * gamma - E - gamma * m0**2 / (2 * rho) - gamma * m1**2 / (2 * rho) + m0**2 / (2 * rho) + 3 * m1**2 / (2 * rho)
+    P30 = E * gamma * m0 / rho - gamma * m0**3 / (2 * rho**2) - gamma * m0 * m1**2 / (2 * rho**2) + m0**3 / (2 * rho**2) + m0 * m1**2 / (2 * rho**2)
+    P31 = E * gamma * m1 / rho - gamma * m0**2 * m1 / (2 * rho**2) - gamma * m1**3 / (2 * rho**2) + m0**2 * m1 / (2 * rho**2) + m1**3 / (2 * rho**2)
+    z = np.zeros_like(rho)
+    return [[m0, m1, z], [P10, P11, z], [P11, P21, z], [P30, P31, z]]
+
+
+def flux_swe_listing(U, g):
+    """SM4.3."""
+    h, q0, q1 = U
+    z = np.zeros_like(h)
+    return [[q0, q1, z], [g * h**2 / 2 + q0**2 / h, q0 * q1 / h, z], [q0 * q1 / h, g * h**2 / 2 + q1**2 / h, z]]
+
+
+def flux_adr_listing(U, u0, u1, D, tau_grad):
+    """SM4.7, PHYSICAL tracker G = grad c. Returns (Phi, S) physical."""
+    c, G0, G1 = U
+    z = np.zeros_like(c)
+    Phi = [[-D * G0 + c * u0, -D * G1 + c * u1, z],
+           [G0 * u0 - c / tau_grad, G0 * u1, z],
+           [G1 * u0, G1 * u1 - c / tau_grad, z]]
+    return Phi
+
+
+def step(f, dim, omega, F_lat, S_lat):
+    """One collide-and-stream step.
+    f[k][i] : arrays (nz, ny, nx);  F_lat[k][a], S_lat[k] : lattice flux / source arrays at the
+    CURRENT moments (computed by the caller from U = sum_i f).  Returns the new f.
+    """
+    L = LATTICES[dim]
+    m, Q = len(f), len(L["c"])
+    new = [[None] * Q for _ in range(m)]
+    for k in range(m):
+        Uk = sum(f[k][i] for i in range(Q))                                   # eq (2.6)
+        for i in range(Q):
+            cx, cy, cz = L["c"][i]
+            cF = cx * F_lat[k][0] + cy * F_lat[k][1] + cz * F_lat[k][2]
+            feq = L["w"][i] * (Uk + cF / L["cs2"])                            # eq (2.7)
+            post = f[k][i] - omega[k] * (f[k][i] - feq) + L["w"][i] * S_lat[k]  # eq (2.11)
+            # f(x + c_i, t + dt) = post(x): shift the array by +c_i along each axis (z, y, x order)
+            new[k][i] = np.roll(post, shift=(cz, cy, cx), axis=(0, 1, 2))
+    return new
+
+
+def moments(f):
+    return [sum(fk) for fk in f]
+
+
+def init_equilibrium(U, F_lat, dim):
+    L = LATTICES[dim]
+    return [[L["w"][i] * (U[k] + (L["c"][i][0] * F_lat[k][0] + L["c"][i][1] * F_lat[k][1] + L["c"][i][2] * F_lat[k][2]) / L["cs2"])
+             for i in range(len(L["c"]))] for k in range(len(U))]

@@ -1,0 +1,72 @@
+"""Writes tests/golden/paper_pins.json: the oracle's errors on the three Table 2 rows of the paper
+that SURVEY.md Appendix A gives full recipes for, next to the values the paper prints.
+
+Calls ONLY `oracle/` and `workloads/` (never the CUDA path).  Run from the repo root:
+    python tests/golden/make_paper_pins.py            # N = 64,128,256,512; ~10 min on 8 cores
+The N = 512 rows are the pins (Table 2); the lower-N rows are fast
+regression values for the default CPU test run (tests/test_oracle_paper_pins.py).
+"""
+import json
+import os
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+sys.path.insert(0, ROOT)
+import oracle  # noqa: E402
+import workloads as W  # noqa: E402
+
+# values printed in PAPER.md Table 2 (double precision, N = 512, t = 1): (rel Linf, rel L2)
+PAPER = {
+    "burgers": {"u": (6.1175e-04, 8.5671e-05), "cite": "PAPER.md:L518"},
+    "euler": {"E": (3.3385e-06, 1.8316e-06), "rho": (1.4401e-06, 6.8435e-07), "rhou": (3.2141e-06, 1.8745e-06),
+              "cite": "PAPER.md:L519-L522 (row labels E, rho, rho u: SURVEY.md §8(c) A8)"},
+    "adr": {"c": (2.2901e-04, 1.2680e-04), "cite": "PAPER.md:L540"},
+}
+
+
+def rel_errors(U, Ue):
+    """per component (rel Linf, rel L2), PAPER.md:L504"""
+    out = []
+    for k in range(U.shape[0]):
+        e = U[k] - Ue[k]
+        out.append((float(np.abs(e).max() / np.abs(Ue[k]).max()), float(np.sqrt((e * e).sum() / (Ue[k] * Ue[k]).sum()))))
+    return out
+
+
+def run_case(case, n):
+    w = {"burgers": W.pin_burgers, "euler": W.pin_euler, "adr": W.pin_adr}[case](n)
+    g = oracle.OracleGrid.from_workload(w)
+    g.init_from_U(w.initial_U())
+    t0 = time.time()
+    g.step(w.steps)
+    wall = time.time() - t0
+    U = g.read_U()
+    _, t = g.time()
+    e = rel_errors(U, g.exact_U(t))
+    g.close()
+    if case == "burgers":
+        fields = {"u": e[0]}
+    elif case == "euler":
+        # vector field norm = root-sum-square of the components' relative norms
+        fields = {"rho": e[0], "E": e[3],
+                  "rhou": (float(np.hypot(e[1][0], e[2][0])), float(np.hypot(e[1][1], e[2][1])))}
+    else:
+        fields = {"c": e[0]}
+    return {"n": n, "steps": w.steps, "t_final": t, "wall_s": round(wall, 1), "fields": fields}
+
+
+if __name__ == "__main__":
+    cases = sys.argv[1:] or ["burgers", "euler", "adr"]
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "paper_pins.json")
+    out = json.load(open(path)) if os.path.exists(path) else {}
+    for case in cases:
+        rows = []
+        for n in (64, 128, 256, 512):
+            r = run_case(case, n)
+            print(case, r, flush=True)
+            rows.append(r)
+        out[case] = {"paper_N512": PAPER[case], "oracle": rows}
+        json.dump(out, open(path, "w"), indent=1, sort_keys=True)

@@ -1,0 +1,363 @@
+"""Seeded synthetic workloads for the collide-and-stream path (inputs only).
+
+This module is the ONE piece shared by the CPU oracle (`oracle/`) and the CUDA
+path (`paper_2607_05668_b200/`): it produces the run description (system name,
+lattice, grid, physical parameters, grid scaling) and the initial state array
+U(x, 0) in fp64.  It holds none of the method's arithmetic: no equilibrium, no
+flux, no source, no collision, no streaming, no forcing.  The analytic fields it
+evaluates are *inputs* (the t = 0 state handed to `init_from_U`), written here in
+NumPy from the recipes in DESIGN.md §"Input recipe".
+
+Stand-in note: the paper measures on no public dataset; its workloads are smooth
+trigonometric manufactured fields on periodic unit boxes (PAPER.md:L1147-L1154,
+L499).  BASELINE.json's five configs are reproduced here as c1..c5.
+
+State layout everywhere: U[k][z][y][x], C-contiguous fp64, nz = 1 in 2D.
+Node coordinates x_j = j*dx, j = 0..n-1 (SURVEY.md §8(c) reading A1).
+Trackers are carried in lattice units, G^L = dx * grad V.
+"""
+from __future__ import annotations
+
+import math
+from dataclasses import dataclass, field, replace
+from typing import Callable, Dict, List, Optional
+
+import numpy as np
+
+TWO_PI = 2.0 * math.pi
+
+# component names per system (documentation + tests)
+COMPONENTS: Dict[str, List[str]] = {
+    "advection2d": ["U"],
+    "burgers2d": ["u"],
+    "swe2d": ["h", "hu", "hv"],
+    "euler2d": ["rho", "mx", "my", "E"],
+    "adr2d": ["c", "Gx", "Gy"],
+    "nsf3d": ["rho", "mx", "my", "mz", "E",
+              "Gxx", "Gxy", "Gxz", "Gyx", "Gyy", "Gyz", "Gzx", "Gzy", "Gzz",
+              "Hx", "Hy", "Hz"],
+    "mhd3d": ["rho", "mx", "my", "mz", "E", "Bx", "By", "Bz", "Jx", "Jy", "Jz"],
+}
+N_CONSERVED = {"advection2d": 1, "burgers2d": 1, "swe2d": 3, "euler2d": 4,
+               "adr2d": 1, "nsf3d": 5, "mhd3d": 8}
+LATTICE_OF = {"advection2d": "D2Q5", "burgers2d": "D2Q5", "swe2d": "D2Q5",
+              "euler2d": "D2Q5", "adr2d": "D2Q5", "nsf3d": "D3Q7", "mhd3d": "D3Q7"}
+# c_s^2 per lattice, Table SM1; used only by the lambda rule below.
+CS2 = {"D2Q5": 1.0 / 3.0, "D3Q7": 1.0 / 4.0}
+SIGMA = 0.6  # lambda rule: lattice wave speed = SIGMA * c_s^2 (SURVEY.md §8(c) "lambda rule")
+
+
+@dataclass
+class Workload:
+    name: str
+    system: str
+    nx: int
+    ny: int
+    nz: int
+    precision: str              # "f64" | "f32s" (reference- and equilibrium-shifted fp32)
+    dx: float
+    lam: float                  # lattice velocity lambda = dx/dt
+    params: List[float]         # physical parameters, order documented per system in DESIGN.md
+    tau_R: float                # tau_LB = 1/2 + tau_R*dt for conserved fields
+    g_tau: float                # tracker step count; 0 if tracker-free
+    U_ref: List[float]          # reference state Q0 for the shifted form
+    mms_id: int                 # 0 = no forcing, 1 = the system's manufactured solution
+    mms_params: List[float]
+    steps: int
+    s_max: float                # a-priori physical max wave speed from the declared amplitudes
+    seed: int
+    init: Callable[["Workload"], np.ndarray] = field(repr=False, default=None)
+    note: str = ""
+
+    @property
+    def lattice(self) -> str:
+        return LATTICE_OF[self.system]
+
+    @property
+    def m_total(self) -> int:
+        return len(COMPONENTS[self.system])
+
+    @property
+    def dim(self) -> int:
+        return 2 if self.lattice == "D2Q5" else 3
+
+    @property
+    def Q(self) -> int:
+        return 5 if self.lattice == "D2Q5" else 7
+
+    @property
+    def dt(self) -> float:
+        return self.dx / self.lam
+
+    @property
+    def n_nodes(self) -> int:
+        return self.nx * self.ny * self.nz
+
+    @property
+    def bytes_per_node(self) -> int:
+        """Algorithmic traffic 2*Q*m_total*sizeof (the byte model of Table 3)."""
+        return 2 * self.Q * self.m_total * (8 if self.precision == "f64" else 4)
+
+    def initial_U(self) -> np.ndarray:
+        U = self.init(self)
+        assert U.shape == (self.m_total, self.nz, self.ny, self.nx) and U.dtype == np.float64
+        return np.ascontiguousarray(U)
+
+
+def _grid(w: Workload):
+    """Node coordinates as broadcastable arrays (z, y, x), x_j = j*dx."""
+    x = (np.arange(w.nx, dtype=np.float64) * w.dx)[None, None, :]
+    y = (np.arange(w.ny, dtype=np.float64) * w.dx)[None, :, None]
+    z = (np.arange(w.nz, dtype=np.float64) * w.dx)[:, None, None]
+    return x, y, z
+
+
+def _full(w: Workload, a) -> np.ndarray:
+    return np.broadcast_to(np.asarray(a, dtype=np.float64), (w.nz, w.ny, w.nx))
+
+
+def lambda_rule(s_max: float, lattice: str) -> float:
+    return s_max / (SIGMA * CS2[lattice])
+
+
+# --------------------------------------------------------------------------- c1
+def _init_c1(w: Workload) -> np.ndarray:
+    # U = 1 + 0.1 sin(2 pi x/64) sin(2 pi y/64) + U(0,1e-3) noise; x, y = node indices (A12, A13).
+    x, y, _ = _grid(w)
+    Lx, Ly = w.nx * w.dx, w.ny * w.dx
+    U = 1.0 + 0.1 * np.sin(TWO_PI * x / Lx) * np.sin(TWO_PI * y / Ly)
+    U = _full(w, U).copy()
+    amp = w.mms_params[0] if w.mms_params else 0.0
+    if amp > 0.0:
+        rng = np.random.default_rng(w.seed)
+        U += rng.uniform(0.0, amp, size=U.shape)
+    return U[None]
+
+
+def c1_advection(n: int = 64, ny: Optional[int] = None, noise: float = 1e-3, steps: int = 200) -> Workload:
+    # velocity (0.1, 0.05) in lattice units => lambda = 1, dx = dt = 1; tau = 0.8 => tau_R = 0.3.
+    return Workload(name=f"c1_advection2d_{n}", system="advection2d", nx=n, ny=ny or n, nz=1,
+                    precision="f64", dx=1.0, lam=1.0, params=[0.1, 0.05], tau_R=0.3, g_tau=0.0,
+                    U_ref=[1.0], mms_id=0, mms_params=[noise], steps=steps,
+                    s_max=0.1, seed=56680 + 1, init=_init_c1,
+                    note="BASELINE.json configs[0]")
+
+
+# --------------------------------------------------------------------------- c2
+def _init_swe(w: Workload) -> np.ndarray:
+    A_h, A_u, h0 = w.mms_params
+    x, y, _ = _grid(w)
+    k = TWO_PI
+    # exact fields at t = 0: cos t = 1, sin t = 0
+    h = h0 + A_h * np.sin(k * x) * np.cos(k * y)
+    u = A_u * np.cos(k * x) * np.sin(k * y)
+    v = 0.0 * x * y
+    return np.stack([_full(w, h), _full(w, h * u), _full(w, h * v)]).copy()
+
+
+def c2_swe(n: int = 512, ny: Optional[int] = None, precision: str = "f64", steps: int = 1000,
+           tau_R: float = 0.5) -> Workload:
+    g, A_h, A_u, h0 = 1.0, 0.05, 0.02, 1.0
+    s_max = A_u * math.sqrt(2.0) + math.sqrt(g * (h0 + A_h))
+    return Workload(name=f"c2_swe2d_{n}", system="swe2d", nx=n, ny=ny or n, nz=1, precision=precision,
+                    dx=1.0 / n, lam=lambda_rule(s_max, "D2Q5"), params=[g], tau_R=tau_R, g_tau=0.0,
+                    U_ref=[h0, 0.0, 0.0], mms_id=1, mms_params=[A_h, A_u, h0], steps=steps,
+                    s_max=s_max, seed=56680 + 2, init=_init_swe, note="BASELINE.json configs[1]")
+
+
+# --------------------------------------------------------------------------- c3
+def _modes(rng, J=4):
+    out = []
+    while len(out) < J:
+        p, q = int(rng.integers(-3, 4)), int(rng.integers(-3, 4))
+        if p == 0 and q == 0:
+            continue
+        out.append((p, q, float(rng.uniform(0.5, 1.0)), float(rng.uniform(0.0, TWO_PI))))
+    return out
+
+
+def _init_c3(w: Workload) -> np.ndarray:
+    gamma = w.params[0]
+    A = w.mms_params[0]
+    x, y, _ = _grid(w)
+    rng = np.random.default_rng(w.seed)
+    rho0, p0 = 1.0, 1.0 / gamma
+
+    def pert():
+        acc = 0.0
+        modes = _modes(rng)
+        for (p, q, a, ph) in modes:
+            acc = acc + a * np.sin(TWO_PI * (p * x + q * y) + ph)
+        return (A / len(modes)) * acc
+
+    rho = rho0 + pert()
+    prs = p0 + pert()
+    E = prs / (gamma - 1.0)
+    zero = 0.0 * rho
+    return np.stack([_full(w, rho), _full(w, zero), _full(w, zero), _full(w, E)]).copy()
+
+
+def c3_euler(n: int = 2048, ny: Optional[int] = None, precision: str = "f32s", steps: int = 500) -> Workload:
+    gamma, A = 1.4, 1e-2
+    p0 = 1.0 / gamma
+    s_max = math.sqrt(gamma * (p0 + A) / (1.0 - A)) + A
+    return Workload(name=f"c3_euler2d_{n}", system="euler2d", nx=n, ny=ny or n, nz=1, precision=precision,
+                    dx=1.0 / n, lam=lambda_rule(s_max, "D2Q5"), params=[gamma], tau_R=5.0, g_tau=0.0,
+                    U_ref=[1.0, 0.0, 0.0, p0 / (gamma - 1.0)], mms_id=0, mms_params=[A], steps=steps,
+                    s_max=s_max, seed=56680 + 3, init=_init_c3, note="BASELINE.json configs[2]")
+
+
+# --------------------------------------------------------------------------- c4
+def nsf3d_exact_primitives_t0(w: Workload):
+    """rho, u(3), p and the analytic gradients of u and T at t = 0 (D(0) = 1, cos 0 = 1)."""
+    gamma, mu, K = w.params
+    U0, A_rho, rho0, p0 = w.mms_params
+    x, y, z = _grid(w)
+    k = TWO_PI
+    sx, cx, sy, cy, sz, cz = np.sin(k * x), np.cos(k * x), np.sin(k * y), np.cos(k * y), np.sin(k * z), np.cos(k * z)
+    c2x, s2x = np.cos(2 * k * x), np.sin(2 * k * x)
+    c2y, s2y = np.cos(2 * k * y), np.sin(2 * k * y)
+    c2z, s2z = np.cos(2 * k * z), np.sin(2 * k * z)
+    u = [U0 * sx * cy * cz, -U0 * cx * sy * cz, 0.5 * U0 * cx * cy * sz]
+    # du[a][b] = d u_a / d x_b
+    du = [[U0 * k * cx * cy * cz, -U0 * k * sx * sy * cz, -U0 * k * sx * cy * sz],
+          [U0 * k * sx * sy * cz, -U0 * k * cx * cy * cz, U0 * k * cx * sy * sz],
+          [-0.5 * U0 * k * sx * cy * sz, -0.5 * U0 * k * cx * sy * sz, 0.5 * U0 * k * cx * cy * cz]]
+    Pa = rho0 * U0 * U0 / 16.0
+    p = p0 + Pa * (c2x + c2y) * (c2z + 2.0)
+    dp = [Pa * (-2 * k * s2x) * (c2z + 2.0), Pa * (-2 * k * s2y) * (c2z + 2.0), Pa * (c2x + c2y) * (-2 * k * s2z)]
+    rho = rho0 * (1.0 + A_rho * sx * sy * cz)
+    drho = [rho0 * A_rho * k * cx * sy * cz, rho0 * A_rho * k * sx * cy * cz, -rho0 * A_rho * k * sx * sy * sz]
+    T = p / rho
+    dT = [(dp[b] - T * drho[b]) / rho for b in range(3)]
+    return rho, u, p, du, dT
+
+
+def _init_c4(w: Workload) -> np.ndarray:
+    gamma = w.params[0]
+    rho, u, p, du, dT = nsf3d_exact_primitives_t0(w)
+    E = p / (gamma - 1.0) + 0.5 * rho * (u[0] ** 2 + u[1] ** 2 + u[2] ** 2)
+    comps = [rho, rho * u[0], rho * u[1], rho * u[2], E]
+    comps += [w.dx * du[a][b] for a in range(3) for b in range(3)]
+    comps += [w.dx * dT[b] for b in range(3)]
+    return np.stack([_full(w, c) for c in comps]).copy()
+
+
+def c4_nsf3d(n: int = 256, ny: Optional[int] = None, nz: Optional[int] = None, precision: str = "f32s",
+             steps: int = 200, mms: bool = True) -> Workload:
+    gamma, Re, Pr, U0, rho0 = 1.4, 100.0, 0.71, 0.1, 1.0
+    p0 = 1.0 / gamma
+    mu = rho0 * U0 * 1.0 / Re
+    K = mu * (gamma / (gamma - 1.0)) / Pr
+    A_rho = 0.01
+    p_max = p0 + (rho0 * U0 * U0 / 16.0) * 6.0
+    s_max = U0 + math.sqrt(gamma * p_max / (rho0 * (1.0 - A_rho)))
+    return Workload(name=f"c4_nsf3d_{n}", system="nsf3d", nx=n, ny=ny or n, nz=nz or n, precision=precision,
+                    dx=1.0 / n, lam=lambda_rule(s_max, "D3Q7"), params=[gamma, mu, K], tau_R=20.0, g_tau=3.0,
+                    U_ref=[rho0, 0.0, 0.0, 0.0, p0 / (gamma - 1.0)] + [0.0] * 12,
+                    mms_id=1 if mms else 0, mms_params=[U0, A_rho, rho0, p0], steps=steps,
+                    s_max=s_max, seed=56680 + 4, init=_init_c4, note="BASELINE.json configs[3]")
+
+
+# --------------------------------------------------------------------------- c5
+def _init_c5(w: Workload) -> np.ndarray:
+    gamma, eta = w.params
+    A = w.mms_params[0]
+    x, y, z = _grid(w)
+    k = TWO_PI
+    sx, cx, sy, cy, sz, cz = np.sin(k * x), np.cos(k * x), np.sin(k * y), np.cos(k * y), np.sin(k * z), np.cos(k * z)
+    s2x, c2x = np.sin(2 * k * x), np.cos(2 * k * x)
+    rho = 1.0 + 0.0 * x * y * z
+    p = 1.0 / gamma
+    u = [-A * sy * cz, A * sx * cz, 0.5 * A * sx * sy]
+    B = [-A * sy * cz, A * s2x * cz, A * sx * sy]
+    # dB[i][j] = d B_i / d x_j ; J = curl B
+    dB = [[0.0 * x, -A * k * cy * cz, A * k * sy * sz],
+          [2 * A * k * c2x * cz, 0.0 * x, -A * k * s2x * sz],
+          [A * k * cx * sy, A * k * sx * cy, 0.0 * x]]
+    J = [dB[2][1] - dB[1][2], dB[0][2] - dB[2][0], dB[1][0] - dB[0][1]]
+    E = p / (gamma - 1.0) + 0.5 * rho * (u[0] ** 2 + u[1] ** 2 + u[2] ** 2) + 0.5 * (B[0] ** 2 + B[1] ** 2 + B[2] ** 2)
+    comps = [rho, rho * u[0], rho * u[1], rho * u[2], E, B[0], B[1], B[2]] + [w.dx * j for j in J]
+    return np.stack([_full(w, c) for c in comps]).copy()
+
+
+def c5_mhd3d(n: int = 192, ny: Optional[int] = None, nz: Optional[int] = None, precision: str = "f32s",
+             steps: int = 200) -> Workload:
+    gamma, eta, A = 1.4, 1e-3, 0.1
+    p0 = 1.0 / gamma
+    # fast magnetosonic bound: c_f^2 <= a^2 + b^2, a^2 = gamma p/rho (p rises little), |B|^2 <= 3 A^2
+    s_max = A + math.sqrt(gamma * p0 * 1.05 + 3.0 * A * A)
+    return Workload(name=f"c5_mhd3d_{n}", system="mhd3d", nx=n, ny=ny or n, nz=nz or n, precision=precision,
+                    dx=1.0 / n, lam=lambda_rule(s_max, "D3Q7"), params=[gamma, eta], tau_R=160.0, g_tau=4.0,
+                    U_ref=[1.0, 0.0, 0.0, 0.0, p0 / (gamma - 1.0)] + [0.0] * 6,
+                    mms_id=0, mms_params=[A], steps=steps, s_max=s_max, seed=56680 + 5, init=_init_c5,
+                    note="BASELINE.json configs[4]")
+
+
+# ----------------------------------------------------- paper pins (Table 2 / SM2 / SM5 recipes)
+def _init_burgers(w: Workload) -> np.ndarray:
+    A = w.mms_params[0]
+    x, y, _ = _grid(w)
+    return _full(w, A * np.sin(TWO_PI * x) * np.sin(TWO_PI * y))[None].copy()
+
+
+def pin_burgers(n: int = 512, precision: str = "f64") -> Workload:
+    # Table SM2: acoustic f = 0.2 (1/lambda = 0.2), tau_R = 0.2; SM5.2 (L1161-L1167): A = 1.3
+    f = 0.2
+    return Workload(name=f"pin_burgers2d_{n}", system="burgers2d", nx=n, ny=n, nz=1, precision=precision,
+                    dx=1.0 / n, lam=1.0 / f, params=[], tau_R=0.2, g_tau=0.0, U_ref=[0.0], mms_id=1,
+                    mms_params=[1.3], steps=int(round(n / f)), s_max=1.3, seed=0, init=_init_burgers,
+                    note="PAPER.md Table 2 L518")
+
+
+def _init_euler_mms(w: Workload) -> np.ndarray:
+    gamma = w.params[0]
+    x, y, _ = _grid(w)
+    k = TWO_PI
+    rho0, cs, M = 1.0, 1.0, 3.0
+    p0 = rho0 * cs * cs / gamma
+    rho = rho0 + 0.3 * rho0 * np.sin(k * x) * np.cos(k * y)      # cos t = 1
+    u = M * cs + 0.0 * x * y                                      # sin t = 0
+    v = M * cs + 0.0 * x * y
+    p = p0 + cs * cs * (rho - rho0)
+    E = p / (gamma - 1.0) + 0.5 * rho * (u * u + v * v)
+    return np.stack([_full(w, rho), _full(w, rho * u), _full(w, rho * v), _full(w, E)]).copy()
+
+
+def pin_euler(n: int = 512, precision: str = "f64") -> Workload:
+    # Table SM2: f = 0.05, tau_R = 0.2; SM5.3 (L1175-L1186)
+    f, gamma = 0.05, 1.4
+    return Workload(name=f"pin_euler2d_{n}", system="euler2d", nx=n, ny=n, nz=1, precision=precision,
+                    dx=1.0 / n, lam=1.0 / f, params=[gamma], tau_R=0.2, g_tau=0.0,
+                    U_ref=[1.0, 3.0, 3.0, (1.0 / gamma) / (gamma - 1.0) + 9.0], mms_id=1, mms_params=[],
+                    steps=int(round(n / f)), s_max=3.3 + math.sqrt(gamma * (1 / gamma + 0.3 + 0.2 / gamma) / 0.7),
+                    seed=0, init=_init_euler_mms, note="PAPER.md Table 2 L519-L522")
+
+
+def _init_adr(w: Workload) -> np.ndarray:
+    x, y, _ = _grid(w)
+    k = TWO_PI
+    c = 0.5 * np.sin(k * x) * np.cos(k * y) + 0.5
+    gx = 0.5 * k * np.cos(k * x) * np.cos(k * y)
+    gy = -0.5 * k * np.sin(k * x) * np.sin(k * y)
+    return np.stack([_full(w, c), _full(w, w.dx * gx), _full(w, w.dx * gy)]).copy()
+
+
+def pin_adr(n: int = 512, precision: str = "f64") -> Workload:
+    # Table SM2: diffusive f = 1.9 (dt = 1.9 dx^2), tau_R = 50, g_tau = 6; SM5.8 (L1292-L1300)
+    f = 1.9
+    dx = 1.0 / n
+    dt = f * dx * dx
+    return Workload(name=f"pin_adr2d_{n}", system="adr2d", nx=n, ny=n, nz=1, precision=precision,
+                    dx=dx, lam=dx / dt, params=[0.1, -0.1, 0.01, 1.0], tau_R=50.0, g_tau=6.0,
+                    U_ref=[0.5, 0.0, 0.0], mms_id=1, mms_params=[], steps=int(round(1.0 / dt)),
+                    s_max=0.1, seed=0, init=_init_adr, note="PAPER.md Table 2 L540")
+
+
+BASELINE_CONFIGS: Dict[str, Callable[..., Workload]] = {
+    "c1": c1_advection, "c2": c2_swe, "c3": c3_euler, "c4": c4_nsf3d, "c5": c5_mhd3d,
+}
+
+
+def relabel(w: Workload, **kw) -> Workload:
+    return replace(w, **kw)
