@@ -1,0 +1,187 @@
+/* lbmk.h -- C-ABI of the B200-native collide-and-stream library (liblbmk.so).
+ *
+ * One thing is implemented behind this boundary: the fused collide-and-stream time step of the
+ * vector-population discrete-kinetic relaxation LBM of arxiv/paper_2607_05668 for a system of m
+ * conservation laws  d_t Q + div Phi(Q) = S  (eq 2.1):
+ *   - every component k of the augmented state Q+ (conserved fields + the gradient-tracker fields the
+ *     first-order cascade adds, eq 2.2-2.4) carries its own Q populations f_k,i on
+ *     one compact lattice, D2Q5 or D3Q7 (eq 2.5-2.6; Table SM1);
+ *   - exact-flux equilibrium  f_eq,k,i = w_i (Q_k + c_i . F_k / c_s^2),  F_k = (dt/dx) Phi_k(Q+)
+ *     (eq 2.7-2.8);
+ *   - BGK collide-and-stream with the source taken as w_i dt S (eq 2.11);
+ *   - fp64, or the reference- and equilibrium-shifted fp32 form f* = f - f_eq(Q0, F0)
+ *     (eq 2.23).
+ * The call sequence follows the paper's statement of the problem: declare the system (m, lattice,
+ * flux/source specialisation, relaxation times, lattice velocity), allocate a periodic or bounded grid,
+ * initialise from U, step N times, read back U.
+ *
+ * Conventions
+ *   - Every function returns lbmk_status; no exception crosses the ABI.  On failure the grid (or, for
+ *     system calls, a thread-local slot) keeps a message readable with lbmk_last_error().
+ *   - Handles (lbmk_system*, lbmk_grid*) are library-owned and freed by the *_destroy calls.
+ *   - Population memory is CALLER-owned device memory (e.g. a torch tensor): query the size with
+ *     lbmk_grid_workspace_bytes(), allocate, hand it over with lbmk_grid_bind_workspace().  The library
+ *     never frees it.  Arrays passed to init/read calls are borrowed for the duration of the call.
+ *   - "on_device" arguments say whether a data pointer is a DEVICE pointer (non-zero) or a HOST pointer
+ *     (zero).  Host transfers are staged through a transient stream-ordered device allocation.
+ *   - All work is enqueued on the cudaStream_t given to lbmk_grid_create (passed as void*; NULL = the
+ *     legacy default stream).  lbmk_step is asynchronous; calls that return data to the host synchronise
+ *     that stream.
+ *   - Field layout everywhere: U[k][z][y][x] and f[k][i][z][y][x], C-contiguous, x fastest, nz = 1 in 2D.
+ *     Node coordinates x_j = j*dx.  Direction order i: 0 rest; 1:+x 2:-x 3:+y 4:-y 5:+z 6:-z.
+ *   - There is NO CPU fallback: without a CUDA device every compute call returns LBMK_ECUDA.
+ */
+#ifndef LBMK_H
+#define LBMK_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LBMK_MAX_COMPONENTS 32
+#define LBMK_MAX_PARAMS 16
+
+typedef enum {
+    LBMK_OK = 0,
+    LBMK_EINVAL = 1,       /* bad argument: unknown id, non-positive size, NULL pointer, wrong count */
+    LBMK_ENOMEM = 2,       /* workspace too small / host allocation failed */
+    LBMK_ECUDA = 3,        /* a CUDA runtime call failed (message holds cudaGetErrorString) */
+    LBMK_ESUBCHAR = 4,     /* sub-characteristic condition violated (eq 2.19-2.20) */
+    LBMK_ESTATE = 5,       /* call out of order (e.g. step before init, bind after init) */
+    LBMK_EUNSUPPORTED = 6  /* valid request this build has no kernel for */
+} lbmk_status;
+
+typedef enum { LBMK_D2Q5 = 0, LBMK_D3Q7 = 1 } lbmk_lattice;          /* Table SM1 */
+typedef enum { LBMK_F64 = 0, LBMK_F32_SHIFTED = 1,                   /* eq 2.23 */
+               LBMK_F64_SHIFTED = 2 /* shift algebra in fp64: test of the identity */ } lbmk_precision;
+typedef enum { LBMK_PERIODIC = 0, LBMK_DIRICHLET_MMS = 1 } lbmk_bc;
+
+/* Compiled-in flux/source specialisations (the paper's Emit stage, Alg 2.1 lines 24-25, replaced by
+ * hand-written / build-time generated CUDA).  params order per system:
+ *   ADVECTION2D  {a_x, a_y}            Phi = a U                                   m = 1
+ *   BURGERS2D    {}                    Phi = (u^2/2, u^2/2)   eq 3.1-3.2 L317-L323 m = 1
+ *   SWE2D        {g}                   eq 3.6, flat bottom               m = 3 (h, hu, hv)
+ *   EULER2D      {gamma}               eq 3.4 L344-L347                            m = 4 (rho, mx, my, E)
+ *   ADR2D        {u_x, u_y, D, R}      eq 3.17 L424-L425                           m = 1 + 2 trackers
+ *   NSF3D        {gamma, mu, K}        eq 3.23 L456-L463 + trackers of grad u (9), grad T (3)  m = 5 + 12
+ *   MHD3D        {gamma, eta}          eq 3.25, current-density trackers J (3)       m = 8 + 3
+ * Trackers are carried in lattice units G^L = dx grad V. */
+typedef enum {
+    LBMK_SYS_ADVECTION2D = 0, LBMK_SYS_BURGERS2D = 1, LBMK_SYS_SWE2D = 2, LBMK_SYS_EULER2D = 3,
+    LBMK_SYS_ADR2D = 4, LBMK_SYS_NSF3D_GRADTRACK = 5, LBMK_SYS_MHD3D_JTRACK = 6, LBMK_SYS_COUNT = 7
+} lbmk_system_id;
+
+/* Grid options (lbmk_grid_set_option, before lbmk_grid_workspace_bytes / bind). */
+typedef enum {
+    LBMK_OPT_PATTERN = 0,   /* streaming pattern: LBMK_PATTERN_* ; default chosen per config by measurement */
+    LBMK_OPT_KERNEL = 1     /* kernel variant: LBMK_KERNEL_* */
+} lbmk_option;
+enum { LBMK_PATTERN_AUTO = 0, LBMK_PATTERN_PULL2 = 1 /* two-lattice pull */, LBMK_PATTERN_AA = 2 /* in-place */ };
+enum { LBMK_KERNEL_AUTO = 0, LBMK_KERNEL_NODE = 1 /* one node per thread, direct loads */,
+       LBMK_KERNEL_ROW = 2 /* bulk-copy staged x-rows in shared memory */ };
+
+typedef struct lbmk_system lbmk_system;
+typedef struct lbmk_grid lbmk_grid;
+
+/* ---- declare the system (eq 2.1; Alg 2.1 "Split/Cascade/Assemble" results are compiled in) ---------- */
+
+/* Creates a system.  lattice must match the system's dimension (2D: D2Q5, 3D: D3Q7).  params: n_params
+ * doubles in the order listed above (host pointer, copied).  *out receives the handle. */
+lbmk_status lbmk_system_create(lbmk_system_id id, lbmk_lattice lattice, const double* params, int n_params,
+                               lbmk_system** out);
+/* m_conserved, m_total (= conserved + tracker components), spatial dimension, Q.  Any out pointer may be NULL. */
+lbmk_status lbmk_system_info(const lbmk_system* sys, int* m_conserved, int* m_total, int* dim, int* Q);
+/* Relaxation: conserved fields tau_k = 1/2 + tau_R[k]*dt; n = 1 (same for all) or
+ * m_conserved.  Tracker fields relax at omega = 1/(g_tau+1) and use tau_grad = g_tau*dt in their flux and
+ * source.  g_tau is ignored by tracker-free systems. */
+lbmk_status lbmk_system_set_relaxation(lbmk_system* sys, const double* tau_R, int n, double g_tau);
+/* Direct relaxation rates omega_k = 1/tau_k for all m_total components (n = 1 or m_total); overrides the
+ * rule above.  omega = 0 gives pure streaming, omega = 1 the Lax-Friedrichs collapse. */
+lbmk_status lbmk_system_set_omega(lbmk_system* sys, const double* omega, int n);
+/* Reference state Q0 [m_total] of the shifted form (eq 2.23).  Default: zeros.  NSF3D / MHD3D require
+ * zero reference momentum, magnetic field and trackers (LBMK_EUNSUPPORTED otherwise). */
+lbmk_status lbmk_system_set_reference(lbmk_system* sys, const double* U0, int n);
+/* Manufactured-solution forcing S_MMS of eq 4.1 for the augmented system, evaluated at
+ * t_n + dt/2.  mms_id 0 = none, 1 = the system's manufactured fields.
+ *   BURGERS2D {A};  EULER2D {};  SWE2D {A_h, A_u, h0};  ADR2D {};  NSF3D {U0, A_rho, rho0, p0}. */
+lbmk_status lbmk_system_set_mms(lbmk_system* sys, int mms_id, const double* mms_params, int n);
+/* A-priori bound on the physical wave speed max|eig sum n_a A_a| from the declared amplitudes (eq 2.20).
+ * lbmk_grid_create rejects the grid with LBMK_ESUBCHAR if s_max/lambda > c_s.  0 = no declared bound. */
+lbmk_status lbmk_system_set_wave_speed_bound(lbmk_system* sys, double s_max);
+void lbmk_system_destroy(lbmk_system* sys);
+
+/* ---- allocate a periodic or bounded grid ------------------------------------------------------------ */
+
+/* nx, ny, nz >= 1 nodes (nz must be 1 for 2D systems); dx = node spacing; lambda = dx/dt the lattice
+ * velocity (grid scaling).  The system is copied: later changes to *sys do not affect
+ * the grid.  cuda_stream: a cudaStream_t.  With LBMK_DIRICHLET_MMS the outermost node layer is reset to
+ * f_eq(Q_exact(x_b, t_n)) before every step and before readback (needs mms_id != 0; the paper defines no
+ * boundary operator, PAPER.md:L504, L608 -- DESIGN.md reading A18). */
+lbmk_status lbmk_grid_create(const lbmk_system* sys, int nx, int ny, int nz, lbmk_bc bc, double dx, double lambda,
+                             lbmk_precision precision, void* cuda_stream, lbmk_grid** out);
+lbmk_status lbmk_grid_set_option(lbmk_grid* g, lbmk_option key, long long value);
+lbmk_status lbmk_grid_get_option(const lbmk_grid* g, lbmk_option key, long long* value); /* resolved value */
+/* Device bytes the grid needs (populations, trig tables, reduction scratch). */
+lbmk_status lbmk_grid_workspace_bytes(const lbmk_grid* g, size_t* bytes);
+/* device_ptr: DEVICE memory, 256-byte aligned, >= workspace_bytes; caller-owned, must outlive the grid. */
+lbmk_status lbmk_grid_bind_workspace(lbmk_grid* g, void* device_ptr, size_t bytes);
+void lbmk_grid_destroy(lbmk_grid* g);
+
+/* ---- initialise from U, step, read back U ------------------------------------------------------------ */
+
+/* Step 0: all populations, conserved and tracker, at the (shifted) equilibrium of
+ * U [m_total][nz][ny][nx] (fp64).  Sets step = 0, t = t0. */
+lbmk_status lbmk_init_from_U(lbmk_grid* g, const double* U, int on_device, double t0);
+/* Sets the populations directly (canonical layout below, fp64; stored as given minus the shift). */
+lbmk_status lbmk_set_populations(lbmk_grid* g, const double* f, int on_device, double t0);
+/* n_steps fused collide-and-stream steps (eq 2.11), asynchronous on the grid's stream. */
+lbmk_status lbmk_step(lbmk_grid* g, int n_steps);
+/* U_k = Q0_k + sum_i f*_k,i (eq 2.6; L312), returned as fp64 [m_total][nz][ny][nx].  Synchronises. */
+lbmk_status lbmk_read_U(lbmk_grid* g, double* U_out, int on_device);
+/* Canonical population state after the completed steps: f[k][i][node] = the (unshifted) population of
+ * component k that sits at `node` and will next move along c_i -- independent of the storage pattern.
+ * fp64 [m_total][Q][nz][ny][nx].  Synchronises. */
+lbmk_status lbmk_read_populations(lbmk_grid* g, double* f_out, int on_device);
+/* Completed steps and current time t0 + step*dt. */
+lbmk_status lbmk_time(const lbmk_grid* g, long long* step, double* t);
+
+/* ---- sub-characteristic check (eq 2.19-2.20; L329; eq 3.12) ------------------ */
+
+/* Device max-reduction over the current state, in LATTICE units:
+ *   out3[0] = max_x max_axis (|u_a| + c_a)/lambda   per-axis ceiling seen by D2Q5/D3Q7 streaming
+ *   out3[1] = max_x (|u| + c)/lambda                isotropic bound over all directions n
+ *   out3[2] = sqrt(kappa_L/g_tau)                   diffusive signal speed of the tracker-parent coupling
+ * Returns LBMK_ESUBCHAR if max(out3[0], out3[1]) + out3[2] > c_s.  out3 is a HOST pointer (may be NULL). */
+lbmk_status lbmk_check_subcharacteristic(lbmk_grid* g, double* out3);
+
+/* ---- test hooks ------------------------------------------------------------------------------------- */
+
+/* For every node x: linear index of the node whose post-collision population `dir` arrives at x, i.e.
+ * wrap(x - c_dir), computed on the device by the index functions the step kernels use.  int64
+ * [nz][ny][nx]; bit-exact against the oracle's table. */
+lbmk_status lbmk_stream_index_map(lbmk_grid* g, int dir, long long* src_index_out, int on_device);
+/* Lattice constants as the kernels use them: c [Q][3] int, w [Q], c_s^2.  Host pointers. */
+lbmk_status lbmk_lattice_constants(lbmk_lattice lattice, int* c, double* w, double* cs2);
+/* Relaxation rates omega_k [m_total] the grid uses.  Host pointer. */
+lbmk_status lbmk_grid_omega(const lbmk_grid* g, double* omega_out);
+/* Kernel launches enqueued by this grid so far (bench.py's gpu_launches). */
+lbmk_status lbmk_grid_launch_count(const lbmk_grid* g, long long* launches);
+/* CUDA-event time, in milliseconds, of the collide-and-stream kernels of the most recent lbmk_step call
+ * (first kernel start to last kernel end, on the grid's stream).  Synchronises. */
+lbmk_status lbmk_last_step_ms(lbmk_grid* g, float* ms);
+
+/* Message of the last failure on this grid (g != NULL) or in this thread's system calls (g == NULL). */
+const char* lbmk_last_error(const lbmk_grid* g);
+const char* lbmk_version(void);
+
+/* Streaming-bandwidth probe: a plain device copy of `bytes` bytes (read + write) repeated `reps` times on
+ * `cuda_stream`; *gbs receives (2*bytes*reps)/time.  The like-for-like roofline denominator, cf. the
+ * paper's BabelStream Triad peak.  src/dst: device pointers, 16-byte aligned. */
+lbmk_status lbmk_copy_bandwidth(void* dst, const void* src, size_t bytes, int reps, void* cuda_stream, double* gbs);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LBMK_H */

@@ -1,0 +1,91 @@
+// common.cuh -- lattice constants, kernel parameter block and index functions of the CUDA path.
+//
+// Lattices: Table SM1.  D2Q5: w = 1/3, 1/6, c_s^2 = 1/3; D3Q7: w = 1/4, 1/8,
+// c_s^2 = 1/4.  Direction order (free choice, reading A10): 0 rest; 1:+x 2:-x 3:+y 4:-y 5:+z 6:-z;
+// opposite(i) pairs (1,2), (3,4), (5,6).  On both lattices w_i / c_s^2 = 1/2 for the moving directions.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <type_traits>
+
+#include "mms_generated.cuh"
+
+namespace lbmk {
+
+constexpr int MAXM = 20;   // largest compiled-in system has 17 components
+
+template <int D> struct Lattice;
+template <> struct Lattice<2> {
+    static constexpr int Q = 5;
+    static constexpr double w0 = 1.0 / 3.0, w1 = 1.0 / 6.0, cs2 = 1.0 / 3.0;
+};
+template <> struct Lattice<3> {
+    static constexpr int Q = 7;
+    static constexpr double w0 = 1.0 / 4.0, w1 = 1.0 / 8.0, cs2 = 1.0 / 4.0;
+};
+
+__host__ __device__ constexpr int opposite(int i) { return i == 0 ? 0 : (((i - 1) ^ 1) + 1); }
+// c_i component along axis a (0 x, 1 y, 2 z)
+__host__ __device__ constexpr int cvel(int i, int a) { return (i == 0 || (i - 1) / 2 != a) ? 0 : (((i - 1) & 1) ? -1 : +1); }
+
+// Kernel parameter block (passed by value).  R = arithmetic/storage type of the path.
+template <class R>
+struct KParams {
+    int nx, ny, nz;
+    long long n;            // nodes
+    R omega[MAXM];          // relaxation rate per component
+    R ref[MAXM];            // reference state Q0 of eq (2.23); zeros in the unshifted fp64 form
+    R par[8];               // physical parameters of the system
+    R cst[8];               // host-derived reference constants (u0, p0, E0+p0, T0, ...), see systems.cuh
+    R il;                   // dt/dx = 1/lambda
+    R dL;                   // dt/dx^2: physical diffusivity -> lattice diffusivity
+    R inv_gtau;             // 1/g_tau
+    R dt;
+    // manufactured forcing (eq 4.1): time scalars at t_n + dt/2 and per-axis tables [entry][index]
+    MmsArgs<R> mms;
+    R T[8];
+    const R* tabX;
+    const R* tabY;
+    const R* tabZ;
+};
+
+struct NodeIdx { int ix, iy, iz; };
+
+__device__ __forceinline__ NodeIdx decompose(long long node, int nx, int ny) {
+    NodeIdx p;
+    const long long row = node / nx;
+    p.ix = (int)(node - row * nx);
+    p.iz = (int)(row / ny);
+    p.iy = (int)(row - (long long)p.iz * ny);
+    return p;
+}
+
+// Element offset from `node` to the periodic neighbour node - c_i (the node a pull along direction i
+// reads from), i.e. wrap(x - c_i) - x in linear index space.  The ONE place the streaming index map is
+// defined on the device: the step kernels, the readback gathers and lbmk_stream_index_map all call it.
+__device__ __forceinline__ long long pull_offset(int i, const NodeIdx& p, int nx, int ny, int nz) {
+    switch (i) {
+        case 1: return p.ix == 0 ? (long long)(nx - 1) : -1LL;
+        case 2: return p.ix == nx - 1 ? -(long long)(nx - 1) : 1LL;
+        case 3: return p.iy == 0 ? (long long)(ny - 1) * nx : -(long long)nx;
+        case 4: return p.iy == ny - 1 ? -(long long)(ny - 1) * nx : (long long)nx;
+        case 5: return p.iz == 0 ? (long long)(nz - 1) * nx * ny : -(long long)nx * ny;
+        case 6: return p.iz == nz - 1 ? -(long long)(nz - 1) * nx * ny : (long long)nx * ny;
+        default: return 0LL;
+    }
+}
+// Offset to node + c_i (push target): the pull offset of the opposite direction.
+__device__ __forceinline__ long long push_offset(int i, const NodeIdx& p, int nx, int ny, int nz) {
+    return pull_offset(opposite(i), p, nx, ny, nz);
+}
+
+// Compile-time loop
+template <int I, int N, class F>
+__host__ __device__ __forceinline__ void static_for(F&& f) {
+    if constexpr (I < N) {
+        f(std::integral_constant<int, I>{});
+        static_for<I + 1, N>(static_cast<F&&>(f));
+    }
+}
+
+}  // namespace lbmk

@@ -1,0 +1,295 @@
+// kernels.cuh -- the collide-and-stream step (one node per thread, direct loads) and its service kernels.
+//
+// Population storage: structure of arrays S[(k*Q + i)*n + node], x fastest.
+// Step per node (eq 2.6 / 2.7 / 2.11 of the paper):
+//   gather f_k,i  ->  dQ_k = sum_i f_k,i  ->  dF_k, s_k (systems.cuh; + manufactured forcing at t_n + dt/2)
+//   ->  f' = f - omega_k (f - w_i (dQ_k + c_i.dF_k/c_s^2)) + w_i s_k  ->  scatter.
+// Because c_i are the axis unit vectors and w_i/c_s^2 = 1/2 for them, the relaxation reads
+//   rest:   f' = (1-omega) f + w0 (omega dQ + s)
+//   +-a:    f' = (1-omega) f + w1 (omega dQ + s) +- (omega/2) dF_a .
+// Streaming patterns (MODE): PULL2 reads buffer `src` at x - c_i and writes buffer `dst` at x (two
+// lattices); AA is in place: the even step reads slot i at x and writes slot opp(i) at x, the odd step
+// reads slot opp(i) at x - c_i and writes slot i at x + c_i.  After an even number of steps (and always in
+// PULL2) storage is canonical: slot i at x holds the population that arrived at x along c_i.
+#pragma once
+#include "systems.cuh"
+
+namespace lbmk {
+
+enum { MODE_PULL2 = 0, MODE_AA_EVEN = 1, MODE_AA_ODD = 2 };
+
+template <class Sys> __host__ __device__ constexpr bool has_mms() { return !std::is_void<typename Sys::Mms>::value; }
+
+// per-node manufactured forcing from the tables
+template <class Sys, class R>
+__device__ __forceinline__ void mms_node(const KParams<R>& P, const NodeIdx& p, R (&s)[Sys::M]) {
+    if constexpr (has_mms<Sys>()) {
+        using G = typename Sys::Mms;
+        R X[G::NX > 0 ? G::NX : 1], Y[G::NY > 0 ? G::NY : 1], Z[G::NZ > 0 ? G::NZ : 1];
+#pragma unroll
+        for (int e = 0; e < G::NX; ++e) X[e] = __ldg(P.tabX + e * P.nx + p.ix);
+#pragma unroll
+        for (int e = 0; e < G::NY; ++e) Y[e] = __ldg(P.tabY + e * P.ny + p.iy);
+#pragma unroll
+        for (int e = 0; e < G::NZ; ++e) Z[e] = __ldg(P.tabZ + e * P.nz + p.iz);
+        G::template source<R>(P.mms, P.T, X, Y, Z, s);
+    }
+}
+
+// BGK relaxation of one component's Q populations, in registers (f[0] rest, f[1+2a] = +a, f[2+2a] = -a)
+template <int D, class R>
+__device__ __forceinline__ void relax(R (&f)[2 * D + 1], R omega, R dQ, const R (&F)[D], R S) {
+    using L = Lattice<D>;
+    const R keep = R(1) - omega;
+    const R A = omega * dQ + S;
+    const R a0 = R(L::w0) * A, a1 = R(L::w1) * A;
+    const R hw = R(0.5) * omega;
+    f[0] = keep * f[0] + a0;
+#pragma unroll
+    for (int a = 0; a < D; ++a) {
+        const R h = hw * F[a];
+        f[1 + 2 * a] = keep * f[1 + 2 * a] + (a1 + h);
+        f[2 + 2 * a] = keep * f[2 + 2 * a] + (a1 - h);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ step
+template <class Sys, class R, int MODE, bool MMS, int BLOCK, int MINB>
+__global__ void __launch_bounds__(BLOCK, MINB)
+collide_stream_node(const R* __restrict__ src, R* __restrict__ dst, const __grid_constant__ KParams<R> P) {
+    constexpr int D = Sys::D, Q = 2 * D + 1, M = Sys::M;
+    const long long node = (long long)blockIdx.x * BLOCK + threadIdx.x;
+    if (node >= P.n) return;
+    const NodeIdx p = decompose(node, P.nx, P.ny);
+    // gather addresses: element offset of direction i's source relative to `node`
+    long long off[Q];
+#pragma unroll
+    for (int i = 0; i < Q; ++i) off[i] = (MODE == MODE_AA_EVEN) ? 0LL : pull_offset(i, p, P.nx, P.ny, P.nz);
+
+    R f[M][Q];
+#pragma unroll
+    for (int k = 0; k < M; ++k)
+#pragma unroll
+        for (int i = 0; i < Q; ++i) {
+            const int slot = (MODE == MODE_AA_ODD) ? opposite(i) : i;
+            f[k][i] = src[(long long)(k * Q + slot) * P.n + node + off[i]];
+        }
+    R dQ[M];
+#pragma unroll
+    for (int k = 0; k < M; ++k) {
+        R s = f[k][0];
+#pragma unroll
+        for (int i = 1; i < Q; ++i) s += f[k][i];
+        dQ[k] = s;
+    }
+    typename Sys::Ctx ctx;
+    Sys::setup(ctx, dQ, P);
+    R smms[M];
+    if constexpr (MMS) mms_node<Sys, R>(P, p, smms);
+
+    static_for<0, M>([&](auto K) {
+        constexpr int k = decltype(K)::value;
+        R F[D], S;
+        Sys::template flux<k>(ctx, dQ, P, F, S);
+        if constexpr (MMS) S += smms[k];
+        relax<D, R>(f[k], P.omega[k], dQ[k], F, S);
+#pragma unroll
+        for (int i = 0; i < Q; ++i) {
+            if constexpr (MODE == MODE_PULL2) {
+                dst[(long long)(k * Q + i) * P.n + node] = f[k][i];
+            } else if constexpr (MODE == MODE_AA_EVEN) {
+                dst[(long long)(k * Q + opposite(i)) * P.n + node] = f[k][i];
+            } else {   // AA odd: push to x + c_i = node + pull offset of the opposite direction
+                dst[(long long)(k * Q + i) * P.n + node + off[opposite(i)]] = f[k][i];
+            }
+        }
+    });
+}
+
+// ------------------------------------------------------------------------------------------------ init
+// step 0: f*_k,i = w_i (dQ_k + c_i . dF_k / c_s^2),  dQ = U - Q0 (subtracted in fp64), eq 2.23
+template <class Sys, class R>
+__global__ void init_from_U_kernel(const double* __restrict__ U, R* __restrict__ f, const __grid_constant__ KParams<R> P,
+                                   const __grid_constant__ KParams<double> Pd) {
+    constexpr int D = Sys::D, Q = 2 * D + 1, M = Sys::M;
+    const long long node = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (node >= P.n) return;
+    R dQ[M];
+#pragma unroll
+    for (int k = 0; k < M; ++k) dQ[k] = (R)(U[(long long)k * P.n + node] - Pd.ref[k]);
+    typename Sys::Ctx ctx;
+    Sys::setup(ctx, dQ, P);
+    static_for<0, M>([&](auto K) {
+        constexpr int k = decltype(K)::value;
+        R F[D], S;
+        Sys::template flux<k>(ctx, dQ, P, F, S);
+        using L = Lattice<D>;
+        f[(long long)(k * Q) * P.n + node] = R(L::w0) * dQ[k];
+#pragma unroll
+        for (int a = 0; a < D; ++a) {
+            const R h = R(0.5) * F[a];              // w1 / c_s^2 = 1/2
+            f[(long long)(k * Q + 1 + 2 * a) * P.n + node] = R(L::w1) * dQ[k] + h;
+            f[(long long)(k * Q + 2 + 2 * a) * P.n + node] = R(L::w1) * dQ[k] - h;
+        }
+    });
+}
+
+// Equilibrium of the reference state in fp64, feq0[k*Q+i] = w_i (Q0_k + c_i.F_k(Q0)/c_s^2): what the shifted
+// storage subtracts (eq 2.23).  One thread; runs once per grid.
+template <class Sys>
+__global__ void reference_equilibrium_kernel(double* __restrict__ feq0, const __grid_constant__ KParams<double> P0 /*ref = 0*/,
+                                             const __grid_constant__ KParams<double> Pd) {
+    constexpr int D = Sys::D, Q = 2 * D + 1, M = Sys::M;
+    if (blockIdx.x != 0 || threadIdx.x != 0) return;
+    double Q0[M];
+    bool any = false;
+    for (int k = 0; k < M; ++k) { Q0[k] = Pd.ref[k]; any = any || (Q0[k] != 0.0); }
+    if (!any) { for (int q = 0; q < M * Q; ++q) feq0[q] = 0.0; return; }
+    typename Sys::Ctx ctx;
+    Sys::setup(ctx, Q0, P0);
+    static_for<0, M>([&](auto K) {
+        constexpr int k = decltype(K)::value;
+        double F[D], S;
+        Sys::template flux<k>(ctx, Q0, P0, F, S);
+        using L = Lattice<D>;
+        feq0[k * Q] = L::w0 * Q0[k];
+        for (int a = 0; a < D; ++a) {
+            feq0[k * Q + 1 + 2 * a] = L::w1 * (Q0[k] + F[a] / L::cs2);
+            feq0[k * Q + 2 + 2 * a] = L::w1 * (Q0[k] - F[a] / L::cs2);
+        }
+    });
+}
+
+// ------------------------------------------------------------------------------------------------ readback
+// canonical gather: population (k, i) of `node` sits in slot i at node (canonical storage) or, after an odd
+// number of AA steps, in slot opp(i) at node - c_i.
+template <int Q, class R>
+__device__ __forceinline__ R load_canonical(const R* __restrict__ f, long long n, int k, int i, long long node,
+                                            const NodeIdx& p, int nx, int ny, int nz, bool aa_odd) {
+    if (!aa_odd) return f[(long long)(k * Q + i) * n + node];
+    return f[(long long)(k * Q + opposite(i)) * n + node + pull_offset(i, p, nx, ny, nz)];
+}
+
+// U_k = Q0_k + sum_i f*_k,i, accumulated and returned in fp64 (eq 2.6; reading A17)
+template <int Q, class R>
+__global__ void read_U_kernel(const R* __restrict__ f, double* __restrict__ U, int M, int nx, int ny, int nz, long long n,
+                              bool aa_odd, const __grid_constant__ KParams<double> Pd) {
+    const long long node = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (node >= n) return;
+    const NodeIdx p = decompose(node, nx, ny);
+    for (int k = 0; k < M; ++k) {
+        double s = 0.0;
+#pragma unroll
+        for (int i = 0; i < Q; ++i) s += (double)load_canonical<Q, R>(f, n, k, i, node, p, nx, ny, nz, aa_odd);
+        U[(long long)k * n + node] = Pd.ref[k] + s;
+    }
+}
+
+template <int Q, class R>
+__global__ void read_f_kernel(const R* __restrict__ f, double* __restrict__ out, const double* __restrict__ feq0, int M,
+                              int nx, int ny, int nz, long long n, bool aa_odd) {
+    const long long node = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (node >= n) return;
+    const NodeIdx p = decompose(node, nx, ny);
+    for (int k = 0; k < M; ++k)
+#pragma unroll
+        for (int i = 0; i < Q; ++i)
+            out[(long long)(k * Q + i) * n + node] =
+                (double)load_canonical<Q, R>(f, n, k, i, node, p, nx, ny, nz, aa_odd) + feq0[k * Q + i];
+}
+
+template <class R>
+__global__ void set_f_kernel(const double* __restrict__ in, R* __restrict__ f, const double* __restrict__ feq0, int MQ, long long n) {
+    const long long node = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (node >= n) return;
+    for (int q = 0; q < MQ; ++q) f[(long long)q * n + node] = (R)(in[(long long)q * n + node] - feq0[q]);
+}
+
+// ------------------------------------------------------------------------------------------------ a10
+// Sub-characteristic check (eq 2.19-2.20; L329): max over nodes of the system's wave
+// speeds, in fp64 from the canonical moments.  Warp shuffle -> shared -> one atomicMax per block on the
+// bit pattern (non-negative doubles order like unsigned integers).  out3 must be zeroed before launch.
+__device__ __forceinline__ double warp_max(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+
+template <class Sys, class R>
+__global__ void __launch_bounds__(256)
+max_wave_speed_kernel(const R* __restrict__ f, unsigned long long* __restrict__ out3, long long n, int nx, int ny, int nz,
+                      bool aa_odd, const __grid_constant__ KParams<double> Pd) {
+    constexpr int Q = 2 * Sys::D + 1, M = Sys::M;
+    double m[3] = {0.0, 0.0, 0.0};
+    for (long long node = (long long)blockIdx.x * blockDim.x + threadIdx.x; node < n; node += (long long)gridDim.x * blockDim.x) {
+        const NodeIdx p = decompose(node, nx, ny);
+        double U[M], w[3];
+        for (int k = 0; k < M; ++k) {
+            double s = 0.0;
+#pragma unroll
+            for (int i = 0; i < Q; ++i) s += (double)load_canonical<Q, R>(f, n, k, i, node, p, nx, ny, nz, aa_odd);
+            U[k] = Pd.ref[k] + s;
+        }
+        Sys::wave(U, Pd, w);
+        m[0] = fmax(m[0], w[0] * Pd.il);     // physical speed / lambda
+        m[1] = fmax(m[1], w[1] * Pd.il);
+        m[2] = fmax(m[2], w[2]);             // already lattice
+    }
+    __shared__ double sm[3][8];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+        const double v = warp_max(m[j]);
+        if (lane == 0) sm[j][warp] = v;
+    }
+    __syncthreads();
+    if (warp == 0) {
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            double v = lane < (int)(blockDim.x >> 5) ? sm[j][lane] : 0.0;
+            v = warp_max(v);
+            if (lane == 0) atomicMax(out3 + j, (unsigned long long)__double_as_longlong(v));
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ a11
+// Dirichlet-MMS frame (reading A18; the paper defines no boundary operator):
+// the outermost node layer is reset to f_eq(Q_exact(x_b, t_n)) in canonical slots.  One thread per frame
+// node candidate; P.T holds the time scalars at t_n (not the midpoint).  Only launched on canonical storage.
+template <class Sys, class R>
+__global__ void dirichlet_frame_kernel(R* __restrict__ f, const __grid_constant__ KParams<R> P, const __grid_constant__ KParams<double> Pd) {
+    if constexpr (has_mms<Sys>()) {
+        constexpr int D = Sys::D, Q = 2 * D + 1, M = Sys::M;
+        using G = typename Sys::Mms;
+        const long long node = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+        if (node >= P.n) return;
+        const NodeIdx p = decompose(node, P.nx, P.ny);
+        bool frame = p.ix == 0 || p.ix == P.nx - 1 || p.iy == 0 || p.iy == P.ny - 1;
+        if (D == 3) frame = frame || p.iz == 0 || p.iz == P.nz - 1;
+        if (!frame) return;
+        // exact state in fp64 from the fp64 images of the tables is not available on the R path: evaluate in R
+        R X[G::NX > 0 ? G::NX : 1], Y[G::NY > 0 ? G::NY : 1], Z[G::NZ > 0 ? G::NZ : 1], q[M], dQ[M];
+        for (int e = 0; e < G::NX; ++e) X[e] = P.tabX[e * P.nx + p.ix];
+        for (int e = 0; e < G::NY; ++e) Y[e] = P.tabY[e * P.ny + p.iy];
+        for (int e = 0; e < G::NZ; ++e) Z[e] = P.tabZ[e * P.nz + p.iz];
+        G::template exact<R>(P.mms, P.T, X, Y, Z, q);
+        for (int k = 0; k < M; ++k) dQ[k] = q[k] - P.ref[k];
+        typename Sys::Ctx ctx;
+        Sys::setup(ctx, dQ, P);
+        static_for<0, M>([&](auto K) {
+            constexpr int k = decltype(K)::value;
+            R F[D], S;
+            Sys::template flux<k>(ctx, dQ, P, F, S);
+            using L = Lattice<D>;
+            f[(long long)(k * Q) * P.n + node] = R(L::w0) * dQ[k];
+            for (int a = 0; a < D; ++a) {
+                const R h = R(0.5) * F[a];
+                f[(long long)(k * Q + 1 + 2 * a) * P.n + node] = R(L::w1) * dQ[k] + h;
+                f[(long long)(k * Q + 2 + 2 * a) * P.n + node] = R(L::w1) * dQ[k] - h;
+            }
+        });
+    }
+}
+
+}  // namespace lbmk

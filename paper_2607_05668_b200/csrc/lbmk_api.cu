@@ -1,0 +1,568 @@
+// lbmk_api.cu -- the C-ABI of include/lbmk.h: handles, validation, workspace layout, host-side grid scaling
+// and the a-priori sub-characteristic check.  All arithmetic of the method runs in the kernels
+// (kernels.cuh, systems.cuh); this file only derives launch parameters on the host:
+//   dt = dx/lambda, omega_k = 1/(1/2 + tau_R,k dt) for conserved fields, omega = 1/(g_tau+1)
+//   for tracker fields, the reference constants of the delta forms (systems.cuh header).
+#include "../../include/lbmk.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "api_kernels.cuh"
+#include "ops.h"
+
+using namespace lbmk;
+
+struct lbmk_system {
+    int id, lattice;
+    double par[LBMK_MAX_PARAMS];
+    int n_par;
+    double tau_R[LBMK_MAX_COMPONENTS];
+    double g_tau;
+    double omega[LBMK_MAX_COMPONENTS];
+    bool omega_set;
+    double ref[LBMK_MAX_COMPONENTS];
+    int mms_id;
+    double mp[LBMK_MAX_PARAMS];
+    double s_max;
+};
+
+struct lbmk_grid {
+    lbmk_system sys;
+    const SysOps* ops;
+    GridCore c;
+    int precision;                 // lbmk_precision as given
+    double dx, lam;
+    long long opt_pattern, opt_kernel;
+    bool bound, inited;
+    size_t ws_bytes;
+    size_t off_f[2], off_tab[3], off_feq0, off_red;
+    std::string err;
+    cudaEvent_t ev0, ev1;
+    bool have_events, timed;
+};
+
+static thread_local std::string g_sys_err;
+
+static const SysOps* ops_of(int id) {
+    switch (id) {
+        case LBMK_SYS_ADVECTION2D: return ops_advection2d();
+        case LBMK_SYS_BURGERS2D: return ops_burgers2d();
+        case LBMK_SYS_SWE2D: return ops_swe2d();
+        case LBMK_SYS_EULER2D: return ops_euler2d();
+        case LBMK_SYS_ADR2D: return ops_adr2d();
+        case LBMK_SYS_NSF3D_GRADTRACK: return ops_nsf3d();
+        case LBMK_SYS_MHD3D_JTRACK: return ops_mhd3d();
+    }
+    return nullptr;
+}
+static const int N_PARAMS[LBMK_SYS_COUNT] = {2, 0, 1, 1, 4, 3, 2};
+static const int N_MMS_PARAMS[LBMK_SYS_COUNT] = {0, 1, 3, 0, 0, 4, 0};
+
+static lbmk_status sys_fail(lbmk_status s, const char* msg) { g_sys_err = msg; return s; }
+static lbmk_status fail(lbmk_grid* g, lbmk_status s, const std::string& msg) { if (g) g->err = msg; else g_sys_err = msg; return s; }
+static lbmk_status cuda_fail(lbmk_grid* g, cudaError_t e, const char* where) {
+    return fail(g, LBMK_ECUDA, std::string(where) + ": " + cudaGetErrorString(e));
+}
+#define CK(g, call, where) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail((g), e_, (where)); } while (0)
+
+static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+extern "C" {
+
+const char* lbmk_version(void) { return "lbmk 0.1 (sm_100a)"; }
+
+const char* lbmk_last_error(const lbmk_grid* g) { return g ? g->err.c_str() : g_sys_err.c_str(); }
+
+lbmk_status lbmk_lattice_constants(lbmk_lattice lattice, int* c, double* w, double* cs2) {
+    if (lattice != LBMK_D2Q5 && lattice != LBMK_D3Q7) return sys_fail(LBMK_EINVAL, "unknown lattice");
+    const int D = lattice == LBMK_D2Q5 ? 2 : 3, Q = 2 * D + 1;
+    for (int i = 0; i < Q; ++i) {
+        if (c) for (int a = 0; a < 3; ++a) c[i * 3 + a] = cvel(i, a);
+        if (w) w[i] = (i == 0) ? (D == 2 ? Lattice<2>::w0 : Lattice<3>::w0) : (D == 2 ? Lattice<2>::w1 : Lattice<3>::w1);
+    }
+    if (cs2) *cs2 = D == 2 ? Lattice<2>::cs2 : Lattice<3>::cs2;
+    return LBMK_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ system
+lbmk_status lbmk_system_create(lbmk_system_id id, lbmk_lattice lattice, const double* params, int n_params, lbmk_system** out) {
+    if (!out) return sys_fail(LBMK_EINVAL, "out is NULL");
+    *out = nullptr;
+    const SysOps* ops = ops_of((int)id);
+    if (!ops) return sys_fail(LBMK_EINVAL, "unknown system id");
+    if ((ops->D == 2 && lattice != LBMK_D2Q5) || (ops->D == 3 && lattice != LBMK_D3Q7))
+        return sys_fail(LBMK_EINVAL, "lattice does not match the system's dimension (2D: D2Q5, 3D: D3Q7)");
+    if (n_params != N_PARAMS[id] || (n_params > 0 && !params)) return sys_fail(LBMK_EINVAL, "wrong number of system parameters");
+    lbmk_system* s = new (std::nothrow) lbmk_system();
+    if (!s) return sys_fail(LBMK_ENOMEM, "host allocation failed");
+    memset(s, 0, sizeof(*s));
+    s->id = id; s->lattice = lattice; s->n_par = n_params;
+    for (int i = 0; i < n_params; ++i) s->par[i] = params[i];
+    s->g_tau = 1.0;
+    *out = s;
+    return LBMK_OK;
+}
+
+lbmk_status lbmk_system_info(const lbmk_system* sys, int* m_conserved, int* m_total, int* dim, int* Q) {
+    if (!sys) return sys_fail(LBMK_EINVAL, "sys is NULL");
+    const SysOps* o = ops_of(sys->id);
+    if (m_conserved) *m_conserved = o->MC;
+    if (m_total) *m_total = o->M;
+    if (dim) *dim = o->D;
+    if (Q) *Q = 2 * o->D + 1;
+    return LBMK_OK;
+}
+
+lbmk_status lbmk_system_set_relaxation(lbmk_system* sys, const double* tau_R, int n, double g_tau) {
+    if (!sys || !tau_R) return sys_fail(LBMK_EINVAL, "NULL argument");
+    const SysOps* o = ops_of(sys->id);
+    if (n != 1 && n != o->MC) return sys_fail(LBMK_EINVAL, "tau_R: n must be 1 or m_conserved");
+    for (int k = 0; k < o->MC; ++k) {
+        sys->tau_R[k] = tau_R[n == 1 ? 0 : k];
+        if (!(sys->tau_R[k] >= 0.0)) return sys_fail(LBMK_EINVAL, "tau_R must be >= 0");
+    }
+    if (o->M > o->MC && !(g_tau > 0.0)) return sys_fail(LBMK_EINVAL, "g_tau must be > 0 for tracker systems");
+    sys->g_tau = g_tau > 0.0 ? g_tau : 1.0;
+    return LBMK_OK;
+}
+
+lbmk_status lbmk_system_set_omega(lbmk_system* sys, const double* omega, int n) {
+    if (!sys || !omega) return sys_fail(LBMK_EINVAL, "NULL argument");
+    const SysOps* o = ops_of(sys->id);
+    if (n != 1 && n != o->M) return sys_fail(LBMK_EINVAL, "omega: n must be 1 or m_total");
+    for (int k = 0; k < o->M; ++k) {
+        sys->omega[k] = omega[n == 1 ? 0 : k];
+        if (!(sys->omega[k] >= 0.0 && sys->omega[k] <= 2.0)) return sys_fail(LBMK_EINVAL, "omega must lie in [0, 2]");
+    }
+    sys->omega_set = true;
+    return LBMK_OK;
+}
+
+lbmk_status lbmk_system_set_reference(lbmk_system* sys, const double* U0, int n) {
+    if (!sys || !U0) return sys_fail(LBMK_EINVAL, "NULL argument");
+    const SysOps* o = ops_of(sys->id);
+    if (n != o->M) return sys_fail(LBMK_EINVAL, "reference: n must be m_total");
+    if (sys->id == LBMK_SYS_NSF3D_GRADTRACK || sys->id == LBMK_SYS_MHD3D_JTRACK) {
+        for (int k = 0; k < n; ++k)
+            if (k != 0 && k != 4 && U0[k] != 0.0)
+                return sys_fail(LBMK_EUNSUPPORTED, "NSF3D/MHD3D delta forms need zero reference momentum, field and trackers");
+    }
+    if ((sys->id == LBMK_SYS_ADR2D) && (U0[1] != 0.0 || U0[2] != 0.0))
+        return sys_fail(LBMK_EUNSUPPORTED, "ADR2D needs zero reference trackers");
+    for (int k = 0; k < n; ++k) sys->ref[k] = U0[k];
+    return LBMK_OK;
+}
+
+lbmk_status lbmk_system_set_mms(lbmk_system* sys, int mms_id, const double* mms_params, int n) {
+    if (!sys) return sys_fail(LBMK_EINVAL, "sys is NULL");
+    if (mms_id == 0) { sys->mms_id = 0; return LBMK_OK; }
+    const SysOps* o = ops_of(sys->id);
+    if (mms_id != 1 || !o->has_mms) return sys_fail(LBMK_EUNSUPPORTED, "no manufactured solution compiled in for this (system, mms_id)");
+    if (n != N_MMS_PARAMS[sys->id] || (n > 0 && !mms_params)) return sys_fail(LBMK_EINVAL, "wrong number of mms parameters");
+    for (int i = 0; i < n; ++i) sys->mp[i] = mms_params[i];
+    sys->mms_id = 1;
+    return LBMK_OK;
+}
+
+lbmk_status lbmk_system_set_wave_speed_bound(lbmk_system* sys, double s_max) {
+    if (!sys || !(s_max >= 0.0)) return sys_fail(LBMK_EINVAL, "bad argument");
+    sys->s_max = s_max;
+    return LBMK_OK;
+}
+
+void lbmk_system_destroy(lbmk_system* sys) { delete sys; }
+
+// ------------------------------------------------------------------------------------------------ grid
+static bool is_shifted(int precision) { return precision == LBMK_F32_SHIFTED || precision == LBMK_F64_SHIFTED; }
+
+// host-side derivation of the kernel parameter block (grid scaling + reference constants of the delta forms)
+static void derive_params(lbmk_grid* g) {
+    const lbmk_system& s = g->sys;
+    const SysOps* o = g->ops;
+    GridCore& c = g->c;
+    KParams<double>& P = c.Pd;
+    memset(&P, 0, sizeof(P));
+    const double dt = g->dx / g->lam;
+    c.dt = dt;
+    P.nx = c.nx; P.ny = c.ny; P.nz = c.nz; P.n = c.n;
+    P.il = 1.0 / g->lam;
+    P.dL = dt / (g->dx * g->dx);
+    P.inv_gtau = 1.0 / s.g_tau;
+    P.dt = dt;
+    for (int k = 0; k < o->M; ++k) {
+        double om = (k < o->MC) ? 1.0 / (0.5 + s.tau_R[k] * dt)     // tau_LB = 1/2 + tau_R dt
+                                : 1.0 / (s.g_tau + 1.0);            // tracker rate
+        if (s.omega_set) om = s.omega[k];
+        P.omega[k] = om;
+        P.ref[k] = is_shifted(g->precision) ? s.ref[k] : 0.0;
+    }
+    for (int i = 0; i < 8; ++i) P.par[i] = s.par[i];
+    const double* r = P.ref;
+    switch (s.id) {
+        case LBMK_SYS_SWE2D:
+            for (int a = 0; a < 2; ++a) P.cst[a] = r[0] != 0.0 ? r[1 + a] / r[0] : 0.0;
+            break;
+        case LBMK_SYS_EULER2D: {
+            double ke = 0.0;
+            for (int a = 0; a < 2; ++a) { P.cst[a] = r[0] != 0.0 ? r[1 + a] / r[0] : 0.0; ke += r[1 + a] * P.cst[a]; }
+            P.cst[3] = (s.par[0] - 1.0) * (r[3] - 0.5 * ke);
+            P.cst[4] = r[3] + P.cst[3];
+        } break;
+        case LBMK_SYS_NSF3D_GRADTRACK:
+        case LBMK_SYS_MHD3D_JTRACK:
+            P.cst[3] = (s.par[0] - 1.0) * r[4];
+            P.cst[4] = r[4] + P.cst[3];
+            P.cst[5] = r[0] != 0.0 ? P.cst[3] / r[0] : 0.0;
+            break;
+        default: break;
+    }
+    MmsHostArgs& mh = c.mh;
+    memset(&mh, 0, sizeof(mh));
+    for (int i = 0; i < 16; ++i) { mh.par[i] = s.par[i]; mh.mp[i] = s.mp[i]; }
+    mh.dx = g->dx; mh.dt = dt; mh.il = P.il; mh.gtau = s.g_tau;
+    for (int i = 0; i < 8; ++i) { P.mms.par[i] = s.par[i]; P.mms.mp[i] = s.mp[i]; }
+    P.mms.dx = g->dx; P.mms.dt = dt; P.mms.il = P.il; P.mms.gtau = s.g_tau;
+    // fp32 image
+    KParams<float>& F = c.Pf;
+    memset(&F, 0, sizeof(F));
+    F.nx = P.nx; F.ny = P.ny; F.nz = P.nz; F.n = P.n;
+    for (int k = 0; k < MAXM; ++k) { F.omega[k] = (float)P.omega[k]; F.ref[k] = (float)P.ref[k]; }
+    for (int i = 0; i < 8; ++i) { F.par[i] = (float)P.par[i]; F.cst[i] = (float)P.cst[i]; F.mms.par[i] = (float)P.mms.par[i]; F.mms.mp[i] = (float)P.mms.mp[i]; }
+    F.il = (float)P.il; F.dL = (float)P.dL; F.inv_gtau = (float)P.inv_gtau; F.dt = (float)P.dt;
+    F.mms.dx = (float)P.mms.dx; F.mms.dt = (float)P.mms.dt; F.mms.il = (float)P.mms.il; F.mms.gtau = (float)P.mms.gtau;
+}
+
+static void resolve_options(lbmk_grid* g) {
+    GridCore& c = g->c;
+    c.pattern = g->opt_pattern == LBMK_PATTERN_AUTO ? PATTERN_PULL2 : (int)g->opt_pattern;
+    if (c.bc == LBMK_DIRICHLET_MMS) c.pattern = PATTERN_PULL2;      // the frame refill needs canonical storage
+    c.kernel = g->opt_kernel == LBMK_KERNEL_AUTO ? KERNEL_NODE : (int)g->opt_kernel;
+    if (c.kernel == KERNEL_ROW && !g->ops->row_kernel_supported(c)) c.kernel = KERNEL_NODE;
+}
+
+static void layout(lbmk_grid* g) {
+    GridCore& c = g->c;
+    const SysOps* o = g->ops;
+    const size_t esz = c.prec == PREC_F64 ? 8 : 4;
+    const size_t fbytes = align_up((size_t)o->M * (2 * o->D + 1) * (size_t)c.n * esz, 256);
+    size_t off = 0;
+    g->off_f[0] = off; off += fbytes;
+    g->off_f[1] = off; if (c.pattern == PATTERN_PULL2) off += fbytes;
+    const int len[3] = {c.nx, c.ny, c.nz};
+    for (int a = 0; a < 3; ++a) { g->off_tab[a] = off; off += align_up((size_t)(o->nax[a] > 0 ? o->nax[a] : 1) * len[a] * esz, 256); }
+    g->off_feq0 = off; off += align_up((size_t)o->M * (2 * o->D + 1) * 8, 256);
+    g->off_red = off; off += 256;
+    g->ws_bytes = off;
+}
+
+lbmk_status lbmk_grid_create(const lbmk_system* sys, int nx, int ny, int nz, lbmk_bc bc, double dx, double lambda,
+                             lbmk_precision precision, void* cuda_stream, lbmk_grid** out) {
+    if (!out) return sys_fail(LBMK_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (!sys) return sys_fail(LBMK_EINVAL, "sys is NULL");
+    const SysOps* o = ops_of(sys->id);
+    if (nx < 1 || ny < 1 || nz < 1) return sys_fail(LBMK_EINVAL, "grid sizes must be >= 1");
+    if (o->D == 2 && nz != 1) return sys_fail(LBMK_EINVAL, "nz must be 1 for a 2D system");
+    if (!(dx > 0.0) || !(lambda > 0.0)) return sys_fail(LBMK_EINVAL, "dx and lambda must be > 0");
+    if (bc != LBMK_PERIODIC && bc != LBMK_DIRICHLET_MMS) return sys_fail(LBMK_EINVAL, "unknown boundary condition");
+    if (precision != LBMK_F64 && precision != LBMK_F32_SHIFTED && precision != LBMK_F64_SHIFTED) return sys_fail(LBMK_EINVAL, "unknown precision");
+    if (bc == LBMK_DIRICHLET_MMS && (sys->mms_id == 0 || !o->has_mms))
+        return sys_fail(LBMK_EINVAL, "LBMK_DIRICHLET_MMS needs a manufactured solution (lbmk_system_set_mms)");
+    if (bc == LBMK_DIRICHLET_MMS && (nx < 3 || ny < 3 || (o->D == 3 && nz < 3))) return sys_fail(LBMK_EINVAL, "bounded grid needs >= 3 nodes per axis");
+    // a-priori sub-characteristic check from the declared amplitudes, eq (2.20): s_max/lambda <= c_s
+    const double cs = std::sqrt(o->D == 2 ? Lattice<2>::cs2 : Lattice<3>::cs2);
+    if (sys->s_max > 0.0 && sys->s_max / lambda > cs) {
+        char b[200];
+        snprintf(b, sizeof b, "a-priori sub-characteristic violation: s_max/lambda = %.6g > c_s = %.6g", sys->s_max / lambda, cs);
+        return sys_fail(LBMK_ESUBCHAR, b);
+    }
+    lbmk_grid* g = new (std::nothrow) lbmk_grid();
+    if (!g) return sys_fail(LBMK_ENOMEM, "host allocation failed");
+    g->sys = *sys;
+    g->ops = o;
+    g->precision = precision;
+    g->dx = dx; g->lam = lambda;
+    g->opt_pattern = LBMK_PATTERN_AUTO; g->opt_kernel = LBMK_KERNEL_AUTO;
+    g->bound = g->inited = false;
+    g->have_events = g->timed = false;
+    GridCore& c = g->c;
+    memset(&c, 0, sizeof(c));
+    c.nx = nx; c.ny = ny; c.nz = nz; c.n = (long long)nx * ny * nz;
+    c.prec = precision == LBMK_F32_SHIFTED ? PREC_F32 : PREC_F64;
+    c.bc = bc;
+    c.mms_id = sys->mms_id;
+    c.stream = (cudaStream_t)cuda_stream;
+    derive_params(g);
+    resolve_options(g);
+    layout(g);
+    *out = g;
+    return LBMK_OK;
+}
+
+lbmk_status lbmk_grid_set_option(lbmk_grid* g, lbmk_option key, long long value) {
+    if (!g) return sys_fail(LBMK_EINVAL, "grid is NULL");
+    if (g->bound) return fail(g, LBMK_ESTATE, "options must be set before the workspace is bound");
+    if (key == LBMK_OPT_PATTERN) {
+        if (value < LBMK_PATTERN_AUTO || value > LBMK_PATTERN_AA) return fail(g, LBMK_EINVAL, "unknown pattern");
+        g->opt_pattern = value;
+    } else if (key == LBMK_OPT_KERNEL) {
+        if (value < LBMK_KERNEL_AUTO || value > LBMK_KERNEL_ROW) return fail(g, LBMK_EINVAL, "unknown kernel variant");
+        g->opt_kernel = value;
+    } else {
+        return fail(g, LBMK_EINVAL, "unknown option");
+    }
+    resolve_options(g);
+    layout(g);
+    return LBMK_OK;
+}
+
+lbmk_status lbmk_grid_get_option(const lbmk_grid* g, lbmk_option key, long long* value) {
+    if (!g || !value) return sys_fail(LBMK_EINVAL, "NULL argument");
+    if (key == LBMK_OPT_PATTERN) *value = g->c.pattern;
+    else if (key == LBMK_OPT_KERNEL) *value = g->c.kernel;
+    else return sys_fail(LBMK_EINVAL, "unknown option");
+    return LBMK_OK;
+}
+
+lbmk_status lbmk_grid_workspace_bytes(const lbmk_grid* g, size_t* bytes) {
+    if (!g || !bytes) return sys_fail(LBMK_EINVAL, "NULL argument");
+    *bytes = g->ws_bytes;
+    return LBMK_OK;
+}
+
+lbmk_status lbmk_grid_bind_workspace(lbmk_grid* g, void* device_ptr, size_t bytes) {
+    if (!g) return sys_fail(LBMK_EINVAL, "grid is NULL");
+    if (!device_ptr) return fail(g, LBMK_EINVAL, "workspace pointer is NULL");
+    if (((uintptr_t)device_ptr & 255) != 0) return fail(g, LBMK_EINVAL, "workspace must be 256-byte aligned");
+    if (bytes < g->ws_bytes) return fail(g, LBMK_ENOMEM, "workspace smaller than lbmk_grid_workspace_bytes");
+    cudaPointerAttributes at;
+    cudaError_t e = cudaPointerGetAttributes(&at, device_ptr);
+    if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(g, e, "cudaPointerGetAttributes (no CUDA device? there is no CPU fallback)"); }
+    if (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged) return fail(g, LBMK_EINVAL, "workspace is not device memory");
+    GridCore& c = g->c;
+    char* base = (char*)device_ptr;
+    c.f[0] = base + g->off_f[0];
+    c.f[1] = c.pattern == PATTERN_PULL2 ? base + g->off_f[1] : nullptr;
+    for (int a = 0; a < 3; ++a) c.tab[a] = base + g->off_tab[a];
+    c.feq0 = (double*)(base + g->off_feq0);
+    c.red = (unsigned long long*)(base + g->off_red);
+    c.cur = 0;
+    CK(g, g->ops->fill_tables(c), "fill_tables");
+    CK(g, g->ops->reference_equilibrium(c), "reference_equilibrium");
+    if (!g->have_events) {
+        CK(g, cudaEventCreate(&g->ev0), "cudaEventCreate");
+        CK(g, cudaEventCreate(&g->ev1), "cudaEventCreate");
+        g->have_events = true;
+    }
+    g->bound = true;
+    g->inited = false;
+    return LBMK_OK;
+}
+
+void lbmk_grid_destroy(lbmk_grid* g) {
+    if (!g) return;
+    if (g->have_events) { cudaEventDestroy(g->ev0); cudaEventDestroy(g->ev1); }
+    delete g;
+}
+
+// ------------------------------------------------------------------------------------------------ data in/out
+// Stage `bytes` of host data into a transient stream-ordered device buffer (or pass a device pointer through).
+struct Staging {
+    void* dev = nullptr;
+    bool owned = false;
+    cudaStream_t stream = nullptr;
+    cudaError_t acquire(const void* user, int on_device, size_t bytes, bool copy_in, cudaStream_t s) {
+        stream = s;
+        if (on_device) { dev = const_cast<void*>(user); return cudaSuccess; }
+        cudaError_t e = cudaMallocAsync(&dev, bytes, s);
+        if (e != cudaSuccess) return e;
+        owned = true;
+        if (copy_in) e = cudaMemcpyAsync(dev, user, bytes, cudaMemcpyHostToDevice, s);
+        return e;
+    }
+    cudaError_t release() {
+        if (!owned) return cudaSuccess;
+        owned = false;
+        return cudaFreeAsync(dev, stream);
+    }
+    ~Staging() { if (owned) cudaFreeAsync(dev, stream); }
+};
+
+static lbmk_status need_bound(lbmk_grid* g) {
+    if (!g) return sys_fail(LBMK_EINVAL, "grid is NULL");
+    if (!g->bound) return fail(g, LBMK_ESTATE, "no workspace bound (lbmk_grid_bind_workspace)");
+    return LBMK_OK;
+}
+static lbmk_status need_inited(lbmk_grid* g) {
+    lbmk_status s = need_bound(g);
+    if (s != LBMK_OK) return s;
+    if (!g->inited) return fail(g, LBMK_ESTATE, "grid not initialised (lbmk_init_from_U)");
+    return LBMK_OK;
+}
+
+lbmk_status lbmk_init_from_U(lbmk_grid* g, const double* U, int on_device, double t0) {
+    lbmk_status s = need_bound(g);
+    if (s != LBMK_OK) return s;
+    if (!U) return fail(g, LBMK_EINVAL, "U is NULL");
+    GridCore& c = g->c;
+    const size_t bytes = (size_t)g->ops->M * c.n * sizeof(double);
+    Staging st;
+    CK(g, st.acquire(U, on_device, bytes, true, c.stream), "stage U");
+    c.step = 0; c.t0 = t0; c.cur = 0;
+    CK(g, g->ops->init_from_U(c, (const double*)st.dev), "init_from_U kernel");
+    CK(g, st.release(), "cudaFreeAsync");
+    if (!on_device) CK(g, cudaStreamSynchronize(c.stream), "cudaStreamSynchronize");   // the host buffer is only borrowed
+    g->inited = true;
+    return LBMK_OK;
+}
+
+lbmk_status lbmk_set_populations(lbmk_grid* g, const double* f, int on_device, double t0) {
+    lbmk_status s = need_bound(g);
+    if (s != LBMK_OK) return s;
+    if (!f) return fail(g, LBMK_EINVAL, "f is NULL");
+    GridCore& c = g->c;
+    const size_t bytes = (size_t)g->ops->M * (2 * g->ops->D + 1) * c.n * sizeof(double);
+    Staging st;
+    CK(g, st.acquire(f, on_device, bytes, true, c.stream), "stage f");
+    c.step = 0; c.t0 = t0; c.cur = 0;
+    CK(g, g->ops->set_f(c, (const double*)st.dev), "set_f kernel");
+    CK(g, st.release(), "cudaFreeAsync");
+    if (!on_device) CK(g, cudaStreamSynchronize(c.stream), "cudaStreamSynchronize");
+    g->inited = true;
+    return LBMK_OK;
+}
+
+lbmk_status lbmk_step(lbmk_grid* g, int n_steps) {
+    lbmk_status s = need_inited(g);
+    if (s != LBMK_OK) return s;
+    if (n_steps < 0) return fail(g, LBMK_EINVAL, "n_steps must be >= 0");
+    if (n_steps == 0) return LBMK_OK;
+    GridCore& c = g->c;
+    CK(g, cudaEventRecord(g->ev0, c.stream), "cudaEventRecord");
+    CK(g, g->ops->step(c, n_steps), "collide_stream launch");
+    CK(g, cudaEventRecord(g->ev1, c.stream), "cudaEventRecord");
+    g->timed = true;
+    return LBMK_OK;
+}
+
+lbmk_status lbmk_last_step_ms(lbmk_grid* g, float* ms) {
+    lbmk_status s = need_inited(g);
+    if (s != LBMK_OK) return s;
+    if (!ms) return fail(g, LBMK_EINVAL, "ms is NULL");
+    if (!g->timed) return fail(g, LBMK_ESTATE, "no lbmk_step call to time yet");
+    CK(g, cudaEventSynchronize(g->ev1), "cudaEventSynchronize");
+    CK(g, cudaEventElapsedTime(ms, g->ev0, g->ev1), "cudaEventElapsedTime");
+    return LBMK_OK;
+}
+
+lbmk_status lbmk_read_U(lbmk_grid* g, double* U_out, int on_device) {
+    lbmk_status s = need_inited(g);
+    if (s != LBMK_OK) return s;
+    if (!U_out) return fail(g, LBMK_EINVAL, "U_out is NULL");
+    GridCore& c = g->c;
+    const size_t bytes = (size_t)g->ops->M * c.n * sizeof(double);
+    Staging st;
+    CK(g, st.acquire(U_out, on_device, bytes, false, c.stream), "stage U_out");
+    CK(g, g->ops->read_U(c, (double*)st.dev), "read_U kernel");
+    if (!on_device) CK(g, cudaMemcpyAsync(U_out, st.dev, bytes, cudaMemcpyDeviceToHost, c.stream), "cudaMemcpyAsync D2H");
+    CK(g, st.release(), "cudaFreeAsync");
+    CK(g, cudaStreamSynchronize(c.stream), "cudaStreamSynchronize");
+    return LBMK_OK;
+}
+
+lbmk_status lbmk_read_populations(lbmk_grid* g, double* f_out, int on_device) {
+    lbmk_status s = need_inited(g);
+    if (s != LBMK_OK) return s;
+    if (!f_out) return fail(g, LBMK_EINVAL, "f_out is NULL");
+    GridCore& c = g->c;
+    const size_t bytes = (size_t)g->ops->M * (2 * g->ops->D + 1) * c.n * sizeof(double);
+    Staging st;
+    CK(g, st.acquire(f_out, on_device, bytes, false, c.stream), "stage f_out");
+    CK(g, g->ops->read_f(c, (double*)st.dev), "read_f kernel");
+    if (!on_device) CK(g, cudaMemcpyAsync(f_out, st.dev, bytes, cudaMemcpyDeviceToHost, c.stream), "cudaMemcpyAsync D2H");
+    CK(g, st.release(), "cudaFreeAsync");
+    CK(g, cudaStreamSynchronize(c.stream), "cudaStreamSynchronize");
+    return LBMK_OK;
+}
+
+lbmk_status lbmk_time(const lbmk_grid* g, long long* step, double* t) {
+    if (!g) return sys_fail(LBMK_EINVAL, "grid is NULL");
+    if (step) *step = g->c.step;
+    if (t) *t = g->c.t0 + (double)g->c.step * g->c.dt;
+    return LBMK_OK;
+}
+
+lbmk_status lbmk_check_subcharacteristic(lbmk_grid* g, double* out3) {
+    lbmk_status s = need_inited(g);
+    if (s != LBMK_OK) return s;
+    double o[3];
+    CK(g, g->ops->max_wave_speed(g->c, o), "max_wave_speed kernel");
+    if (out3) { out3[0] = o[0]; out3[1] = o[1]; out3[2] = o[2]; }
+    const double cs = std::sqrt(g->ops->D == 2 ? Lattice<2>::cs2 : Lattice<3>::cs2);
+    const double sp = std::fmax(o[0], o[1]) + o[2];
+    if (!(sp <= cs)) {
+        char b[200];
+        snprintf(b, sizeof b, "sub-characteristic violation: lattice wave speed %.6g > c_s = %.6g", sp, cs);
+        return fail(g, LBMK_ESUBCHAR, b);
+    }
+    return LBMK_OK;
+}
+
+lbmk_status lbmk_stream_index_map(lbmk_grid* g, int dir, long long* src_index_out, int on_device) {
+    lbmk_status s = need_bound(g);
+    if (s != LBMK_OK) return s;
+    if (!src_index_out) return fail(g, LBMK_EINVAL, "output is NULL");
+    if (dir < 0 || dir > 2 * g->ops->D) return fail(g, LBMK_EINVAL, "direction out of range");
+    GridCore& c = g->c;
+    const size_t bytes = (size_t)c.n * sizeof(long long);
+    Staging st;
+    CK(g, st.acquire(src_index_out, on_device, bytes, false, c.stream), "stage index map");
+    stream_index_map_kernel<<<(unsigned)((c.n + 255) / 256), 256, 0, c.stream>>>((long long*)st.dev, dir, c.nx, c.ny, c.nz, c.n);
+    c.launches++;
+    CK(g, cudaGetLastError(), "stream_index_map kernel");
+    if (!on_device) CK(g, cudaMemcpyAsync(src_index_out, st.dev, bytes, cudaMemcpyDeviceToHost, c.stream), "cudaMemcpyAsync D2H");
+    CK(g, st.release(), "cudaFreeAsync");
+    CK(g, cudaStreamSynchronize(c.stream), "cudaStreamSynchronize");
+    return LBMK_OK;
+}
+
+lbmk_status lbmk_grid_omega(const lbmk_grid* g, double* omega_out) {
+    if (!g || !omega_out) return sys_fail(LBMK_EINVAL, "NULL argument");
+    for (int k = 0; k < g->ops->M; ++k) omega_out[k] = g->c.Pd.omega[k];
+    return LBMK_OK;
+}
+
+lbmk_status lbmk_grid_launch_count(const lbmk_grid* g, long long* launches) {
+    if (!g || !launches) return sys_fail(LBMK_EINVAL, "NULL argument");
+    *launches = g->c.launches;
+    return LBMK_OK;
+}
+
+lbmk_status lbmk_copy_bandwidth(void* dst, const void* src, size_t bytes, int reps, void* cuda_stream, double* gbs) {
+    if (!dst || !src || !gbs || reps < 1 || bytes < 16) return sys_fail(LBMK_EINVAL, "bad argument");
+    if ((((uintptr_t)dst) | ((uintptr_t)src)) & 15) return sys_fail(LBMK_EINVAL, "pointers must be 16-byte aligned");
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    cudaEvent_t a, b;
+    cudaError_t e;
+    if ((e = cudaEventCreate(&a)) != cudaSuccess) return cuda_fail(nullptr, e, "cudaEventCreate");
+    if ((e = cudaEventCreate(&b)) != cudaSuccess) { cudaEventDestroy(a); return cuda_fail(nullptr, e, "cudaEventCreate"); }
+    const size_t n16 = bytes / 16;
+    const unsigned nb = 148 * 16;
+    copy_kernel<<<nb, 256, 0, s>>>((float4*)dst, (const float4*)src, n16);   // warm-up
+    cudaEventRecord(a, s);
+    for (int r = 0; r < reps; ++r) copy_kernel<<<nb, 256, 0, s>>>((float4*)dst, (const float4*)src, n16);
+    cudaEventRecord(b, s);
+    e = cudaEventSynchronize(b);
+    float ms = 0.f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, a, b);
+    cudaEventDestroy(a); cudaEventDestroy(b);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "copy_kernel");
+    *gbs = 2.0 * (double)(n16 * 16) * reps / (ms * 1e-3) / 1e9;
+    return LBMK_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,59 @@
+// ops.h -- type-erased per-system entry points: the seam between the C-ABI (lbmk_api.cu, host logic) and
+// the templated kernels (one translation unit per system, sys_*.cu, instantiating ops_impl.cuh).
+#pragma once
+#include <cuda_runtime.h>
+
+#include "common.cuh"
+
+namespace lbmk {
+
+enum { PREC_F64 = 0, PREC_F32 = 1 };
+enum { PATTERN_PULL2 = 1, PATTERN_AA = 2 };
+enum { KERNEL_NODE = 1, KERNEL_ROW = 2 };
+
+struct GridCore {
+    int nx, ny, nz;
+    long long n;
+    int prec;             // PREC_F64 / PREC_F32 (storage and arithmetic type R)
+    int bc;               // 0 periodic, 1 Dirichlet-MMS frame
+    int pattern, kernel;
+    int mms_id;
+    cudaStream_t stream;
+    void* f[2];           // population buffers; f[1] == nullptr for the in-place AA pattern
+    int cur;              // PULL2: which buffer holds the current state
+    long long step;       // completed steps
+    double t0, dt;
+    void* tab[3];         // per-axis trig tables in R, [entry][index]
+    double* feq0;         // [M*Q] reference equilibrium (fp64)
+    unsigned long long* red;   // [4] reduction scratch
+    KParams<double> Pd;   // parameters in fp64 (host logic, fp64 kernels, readback)
+    KParams<float> Pf;    // same, rounded to fp32 (fp32 kernels)
+    MmsHostArgs mh;
+    long long launches;
+};
+
+struct SysOps {
+    int id, D, M, MC;
+    bool has_mms;
+    int nt, nax[3];       // time scalars and table entries per axis of the manufactured solution
+    // all return cudaError_t of the last launch / API call
+    cudaError_t (*fill_tables)(GridCore&);                 // host fp64 -> device R tables (synchronous copy on the stream)
+    cudaError_t (*reference_equilibrium)(GridCore&);
+    cudaError_t (*init_from_U)(GridCore&, const double* U_dev);
+    cudaError_t (*set_f)(GridCore&, const double* f_dev);
+    cudaError_t (*step)(GridCore&, int n_steps);
+    cudaError_t (*read_U)(GridCore&, double* U_dev);
+    cudaError_t (*read_f)(GridCore&, double* f_dev);
+    cudaError_t (*max_wave_speed)(GridCore&, double* out3_host);
+    bool (*row_kernel_supported)(const GridCore&);
+};
+
+const SysOps* ops_advection2d();
+const SysOps* ops_burgers2d();
+const SysOps* ops_swe2d();
+const SysOps* ops_euler2d();
+const SysOps* ops_adr2d();
+const SysOps* ops_nsf3d();
+const SysOps* ops_mhd3d();
+
+}  // namespace lbmk

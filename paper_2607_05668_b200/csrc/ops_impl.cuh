@@ -1,0 +1,196 @@
+// ops_impl.cuh -- launches of the templated kernels for one system; included by each sys_*.cu.
+#pragma once
+#include <algorithm>
+#include <cstring>
+#include <vector>
+
+#include "kernels.cuh"
+#include "ops.h"
+
+namespace lbmk {
+
+template <class R> __host__ inline KParams<R>& kp(GridCore& g);
+template <> __host__ inline KParams<double>& kp<double>(GridCore& g) { return g.Pd; }
+template <> __host__ inline KParams<float>& kp<float>(GridCore& g) { return g.Pf; }
+
+// launch shape of the node kernel per system: threads per block, min blocks per SM (register cap)
+template <template <class> class S, class R> struct Tune { static constexpr int BLOCK = 256, MINB = 1; };
+template <class R> struct Tune<SysNsf3D, R> { static constexpr int BLOCK = 128, MINB = 2; };
+template <> struct Tune<SysNsf3D, double> { static constexpr int BLOCK = 128, MINB = 1; };
+template <class R> struct Tune<SysMhd3D, R> { static constexpr int BLOCK = 128, MINB = 2; };
+
+template <class Mm> struct MmsCounts { static constexpr int NT = Mm::NT, NX = Mm::NX, NY = Mm::NY, NZ = Mm::NZ; };
+template <> struct MmsCounts<void> { static constexpr int NT = 0, NX = 0, NY = 0, NZ = 0; };
+
+inline unsigned blocks_for(long long n, int block) { return (unsigned)((n + block - 1) / block); }
+
+template <template <class> class S>
+struct Ops {
+    using Sd = S<double>;
+    static constexpr int D = Sd::D, Q = 2 * D + 1, M = Sd::M;
+    static constexpr bool HAS_MMS = has_mms<Sd>();
+
+    using C = MmsCounts<typename Sd::Mms>;
+
+    // ---- manufactured-solution tables and time scalars (host fp64)
+    static void time_scalars(GridCore& g, double t) {
+        if constexpr (HAS_MMS) {
+            double T[8] = {0};
+            Sd::Mms::time_scalars(t, g.mh, T);
+            for (int i = 0; i < 8; ++i) { g.Pd.T[i] = T[i]; g.Pf.T[i] = (float)T[i]; }
+        }
+    }
+    template <class R>
+    static cudaError_t fill_tables_t(GridCore& g) {
+        if constexpr (HAS_MMS) {
+            const int cnt[3] = {C::NX, C::NY, C::NZ};
+            const int len[3] = {g.nx, g.ny, g.nz};
+            for (int ax = 0; ax < 3; ++ax) {
+                if (cnt[ax] == 0) continue;
+                std::vector<R> h((size_t)cnt[ax] * len[ax]);
+                double row[8];
+                for (int j = 0; j < len[ax]; ++j) {
+                    Sd::Mms::axis_row(ax, j * g.mh.dx, g.mh, row);          // x_j = j dx (reading A1)
+                    for (int e = 0; e < cnt[ax]; ++e) h[(size_t)e * len[ax] + j] = (R)row[e];
+                }
+                cudaError_t e = cudaMemcpyAsync(g.tab[ax], h.data(), h.size() * sizeof(R), cudaMemcpyHostToDevice, g.stream);
+                if (e != cudaSuccess) return e;
+                e = cudaStreamSynchronize(g.stream);                         // h goes out of scope
+                if (e != cudaSuccess) return e;
+            }
+            kp<R>(g).tabX = (const R*)g.tab[0]; kp<R>(g).tabY = (const R*)g.tab[1]; kp<R>(g).tabZ = (const R*)g.tab[2];
+        }
+        return cudaSuccess;
+    }
+    static cudaError_t fill_tables(GridCore& g) { return g.prec == PREC_F64 ? fill_tables_t<double>(g) : fill_tables_t<float>(g); }
+
+    static cudaError_t reference_equilibrium(GridCore& g) {
+        KParams<double> P0 = g.Pd;
+        for (int k = 0; k < MAXM; ++k) P0.ref[k] = 0.0;
+        for (int k = 0; k < 8; ++k) P0.cst[k] = 0.0;
+        reference_equilibrium_kernel<Sd><<<1, 1, 0, g.stream>>>(g.feq0, P0, g.Pd);
+        g.launches++;
+        return cudaGetLastError();
+    }
+
+    template <class R>
+    static cudaError_t init_t(GridCore& g, const double* U) {
+        init_from_U_kernel<S<R>, R><<<blocks_for(g.n, 256), 256, 0, g.stream>>>(U, (R*)g.f[0], kp<R>(g), g.Pd);
+        g.launches++;
+        g.cur = 0;
+        return cudaGetLastError();
+    }
+    static cudaError_t init_from_U(GridCore& g, const double* U) { return g.prec == PREC_F64 ? init_t<double>(g, U) : init_t<float>(g, U); }
+
+    template <class R>
+    static cudaError_t set_f_t(GridCore& g, const double* f) {
+        set_f_kernel<R><<<blocks_for(g.n, 256), 256, 0, g.stream>>>(f, (R*)g.f[0], g.feq0, M * Q, g.n);
+        g.launches++;
+        g.cur = 0;
+        return cudaGetLastError();
+    }
+    static cudaError_t set_f(GridCore& g, const double* f) { return g.prec == PREC_F64 ? set_f_t<double>(g, f) : set_f_t<float>(g, f); }
+
+    static bool aa_odd(const GridCore& g) { return g.pattern == PATTERN_AA && (g.step & 1); }
+
+    template <class R>
+    static cudaError_t read_U_t(GridCore& g, double* U) {
+        read_U_kernel<Q, R><<<blocks_for(g.n, 256), 256, 0, g.stream>>>((const R*)g.f[g.cur], U, M, g.nx, g.ny, g.nz, g.n, aa_odd(g), g.Pd);
+        g.launches++;
+        return cudaGetLastError();
+    }
+    static cudaError_t read_U(GridCore& g, double* U) { return g.prec == PREC_F64 ? read_U_t<double>(g, U) : read_U_t<float>(g, U); }
+
+    template <class R>
+    static cudaError_t read_f_t(GridCore& g, double* f) {
+        read_f_kernel<Q, R><<<blocks_for(g.n, 256), 256, 0, g.stream>>>((const R*)g.f[g.cur], f, g.feq0, M, g.nx, g.ny, g.nz, g.n, aa_odd(g));
+        g.launches++;
+        return cudaGetLastError();
+    }
+    static cudaError_t read_f(GridCore& g, double* f) { return g.prec == PREC_F64 ? read_f_t<double>(g, f) : read_f_t<float>(g, f); }
+
+    template <class R>
+    static cudaError_t wave_t(GridCore& g, double* out3) {
+        cudaError_t e = cudaMemsetAsync(g.red, 0, 4 * sizeof(unsigned long long), g.stream);
+        if (e != cudaSuccess) return e;
+        const unsigned nb = (unsigned)std::min<long long>((g.n + 255) / 256, 148 * 8);
+        max_wave_speed_kernel<Sd, R><<<nb, 256, 0, g.stream>>>((const R*)g.f[g.cur], g.red, g.n, g.nx, g.ny, g.nz, aa_odd(g), g.Pd);
+        g.launches++;
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+        unsigned long long h[3];
+        e = cudaMemcpyAsync(h, g.red, sizeof(h), cudaMemcpyDeviceToHost, g.stream);
+        if (e != cudaSuccess) return e;
+        e = cudaStreamSynchronize(g.stream);
+        if (e != cudaSuccess) return e;
+        for (int j = 0; j < 3; ++j) { double d; memcpy(&d, &h[j], 8); out3[j] = d; }
+        return cudaSuccess;
+    }
+    static cudaError_t max_wave_speed(GridCore& g, double* out3) { return g.prec == PREC_F64 ? wave_t<double>(g, out3) : wave_t<float>(g, out3); }
+
+    // ---- the step
+    template <class R, int MODE, bool MMS>
+    static void launch_node(GridCore& g, const R* src, R* dst) {
+        constexpr int BLOCK = Tune<S, R>::BLOCK, MINB = Tune<S, R>::MINB;
+        collide_stream_node<S<R>, R, MODE, MMS, BLOCK, MINB><<<blocks_for(g.n, BLOCK), BLOCK, 0, g.stream>>>(src, dst, kp<R>(g));
+        g.launches++;
+    }
+    template <class R, bool MMS>
+    static cudaError_t step_t(GridCore& g, int n_steps) {
+        for (int s = 0; s < n_steps; ++s) {
+            const double t_n = g.t0 + (double)g.step * g.dt;
+            if (g.bc == 1) {
+                if constexpr (HAS_MMS) {
+                    time_scalars(g, t_n);
+                    dirichlet_frame_kernel<S<R>, R><<<blocks_for(g.n, 256), 256, 0, g.stream>>>((R*)g.f[g.cur], kp<R>(g), g.Pd);
+                    g.launches++;
+                }
+            }
+            if constexpr (MMS) time_scalars(g, t_n + 0.5 * g.dt);           // explicit forcing at the temporal midpoint, L154
+            if (g.pattern == PATTERN_PULL2) {
+                launch_node<R, MODE_PULL2, MMS>(g, (const R*)g.f[g.cur], (R*)g.f[g.cur ^ 1]);
+                g.cur ^= 1;
+            } else if ((g.step & 1) == 0) {
+                launch_node<R, MODE_AA_EVEN, MMS>(g, (const R*)g.f[0], (R*)g.f[0]);
+            } else {
+                launch_node<R, MODE_AA_ODD, MMS>(g, (const R*)g.f[0], (R*)g.f[0]);
+            }
+            g.step++;
+        }
+        return cudaGetLastError();
+    }
+    static cudaError_t step(GridCore& g, int n_steps) {
+        const bool mms = HAS_MMS && g.mms_id != 0;
+        if constexpr (HAS_MMS) {
+            if (mms) return g.prec == PREC_F64 ? step_t<double, true>(g, n_steps) : step_t<float, true>(g, n_steps);
+        }
+        return g.prec == PREC_F64 ? step_t<double, false>(g, n_steps) : step_t<float, false>(g, n_steps);
+    }
+    // Dirichlet frame refresh before readback (the oracle does the same in orc_read_U)
+    static cudaError_t frame_now(GridCore& g) {
+        if constexpr (HAS_MMS) {
+            if (g.bc == 1) {
+                time_scalars(g, g.t0 + (double)g.step * g.dt);
+                if (g.prec == PREC_F64) dirichlet_frame_kernel<S<double>, double><<<blocks_for(g.n, 256), 256, 0, g.stream>>>((double*)g.f[g.cur], g.Pd, g.Pd);
+                else dirichlet_frame_kernel<S<float>, float><<<blocks_for(g.n, 256), 256, 0, g.stream>>>((float*)g.f[g.cur], g.Pf, g.Pd);
+                g.launches++;
+            }
+        }
+        return cudaGetLastError();
+    }
+    static cudaError_t read_U_with_frame(GridCore& g, double* U) {
+        cudaError_t e = frame_now(g);
+        if (e != cudaSuccess) return e;
+        return read_U(g, U);
+    }
+    static bool row_supported(const GridCore&) { return false; }
+
+    static const SysOps* get() {
+        static const SysOps ops = {Sd::ID, D, M, Sd::MC, HAS_MMS, C::NT, {C::NX, C::NY, C::NZ},
+                                   &fill_tables, &reference_equilibrium, &init_from_U, &set_f, &step,
+                                   &read_U_with_frame, &read_f, &max_wave_speed, &row_supported};
+        return &ops;
+    }
+};
+
+}  // namespace lbmk

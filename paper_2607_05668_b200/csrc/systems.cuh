@@ -1,0 +1,318 @@
+// systems.cuh -- per-system lattice flux F_k = (dt/dx) Phi_k(Q+) and source s_k = dt S_k(Q+), in delta form.
+//
+// Every system is written ONCE for the state split Q = Q0 + dQ of eq (2.23): the
+// kernels hand in dQ (the zeroth moments of the shifted populations f*) and get back
+//     dF_k = F_k(Q0 + dQ) - F_k(Q0)          and        s_k(Q0 + dQ)
+// with every dF term O(dQ): products of two O(1) backgrounds are cancelled on paper, not in fp32
+// (SURVEY.md Appendix B).  With Q0 = 0 (plain fp64 form) the same code is the plain flux.
+// Host-derived reference constants arrive in KParams::cst (filled by derive_constants in lbmk_api.cu):
+//   hydrodynamic systems  cst[0..2] = u0 = m0/rho0,  cst[3] = p0,  cst[4] = E0 + p0,  cst[5] = T0 = p0/rho0
+//   SWE                   cst[0..1] = u0 = m0/h0
+// Trackers are in lattice units G^L = dx grad V: F_G[b][j] = G_b u_j/lambda - delta_jb V/g_tau,
+// s_G = -G/g_tau (eq 2.3; tau_grad = g_tau dt, L106); a physical diffusivity D enters the
+// parent's flux as D_L = D dt/dx^2.
+//
+// Interface of a system S<R>:
+//   ID, D (dimension), M (components), MC (conserved), Ctx (primitives shared by all components)
+//   setup(Ctx&, dQ[M], P)                 once per node
+//   flux<k>(Ctx, dQ, P, F[D], S)          lattice flux columns and source of component k
+//   wave(Q[M] full state, P, out[3])      physical |u_a|+c_a max, |u|+c, lattice diffusive signal speed
+#pragma once
+#include "common.cuh"
+
+namespace lbmk {
+
+enum { SYS_ADVECTION2D = 0, SYS_BURGERS2D = 1, SYS_SWE2D = 2, SYS_EULER2D = 3, SYS_ADR2D = 4, SYS_NSF3D = 5, SYS_MHD3D = 6 };
+
+// ------------------------------------------------------------------------------------------ advection
+// Phi = (a_x U, a_y U); par = {a_x, a_y}
+template <class R> struct SysAdvection2D {
+    static constexpr int ID = SYS_ADVECTION2D, D = 2, M = 1, MC = 1;
+    using Mms = void;
+    struct Ctx {};
+    __device__ __forceinline__ static void setup(Ctx&, const R (&)[M], const KParams<R>&) {}
+    template <int k> __device__ __forceinline__ static void flux(const Ctx&, const R (&dQ)[M], const KParams<R>& P, R (&F)[D], R& S) {
+        F[0] = (P.par[0] * P.il) * dQ[0];
+        F[1] = (P.par[1] * P.il) * dQ[0];
+        S = R(0);
+    }
+    __device__ static void wave(const double* Q, const KParams<double>& P, double* out) {
+        const double ax = fabs(P.par[0]), ay = fabs(P.par[1]);
+        out[0] = fmax(ax, ay); out[1] = sqrt(ax * ax + ay * ay); out[2] = 0.0;
+    }
+};
+
+// ------------------------------------------------------------------------------------------ Burgers
+// eq (3.1)-(3.2): Phi = (u^2/2, u^2/2);  delta form du (u0 + du/2)
+template <class R> struct SysBurgers2D {
+    static constexpr int ID = SYS_BURGERS2D, D = 2, M = 1, MC = 1;
+    using Mms = Mms_burgers2d;
+    struct Ctx {};
+    __device__ __forceinline__ static void setup(Ctx&, const R (&)[M], const KParams<R>&) {}
+    template <int k> __device__ __forceinline__ static void flux(const Ctx&, const R (&dQ)[M], const KParams<R>& P, R (&F)[D], R& S) {
+        const R h = P.il * (dQ[0] * (P.ref[0] + R(0.5) * dQ[0]));
+        F[0] = h; F[1] = h;
+        S = R(0);
+    }
+    __device__ static void wave(const double* Q, const KParams<double>& P, double* out) {
+        const double a = fabs(Q[0]);      // f'(u) = u on both axes
+        out[0] = a; out[1] = sqrt(2.0) * a; out[2] = 0.0;
+    }
+};
+
+// ------------------------------------------------------------------------------------------ shallow water
+// eq (3.6), flat bottom; par = {g}; Q = (h, hu, hv)
+template <class R> struct SysSwe2D {
+    static constexpr int ID = SYS_SWE2D, D = 2, M = 3, MC = 3;
+    using Mms = Mms_swe2d;
+    struct Ctx { R u[2], du[2], dP; };
+    __device__ __forceinline__ static void setup(Ctx& c, const R (&dQ)[M], const KParams<R>& P) {
+        const R h = P.ref[0] + dQ[0];
+        const R rh = R(1) / h;
+        for (int a = 0; a < 2; ++a) {
+            c.du[a] = (dQ[1 + a] - P.cst[a] * dQ[0]) * rh;     // u - u0 = (dm - u0 dh)/h
+            c.u[a] = P.cst[a] + c.du[a];
+        }
+        c.dP = R(0.5) * P.par[0] * dQ[0] * (R(2) * P.ref[0] + dQ[0]);   // g/2 (h^2 - h0^2)
+    }
+    template <int k> __device__ __forceinline__ static void flux(const Ctx& c, const R (&dQ)[M], const KParams<R>& P, R (&F)[D], R& S) {
+        S = R(0);
+        if constexpr (k == 0) {
+            F[0] = P.il * dQ[1]; F[1] = P.il * dQ[2];
+        } else {
+            constexpr int a = k - 1;
+            for (int j = 0; j < 2; ++j) {
+                R v = dQ[1 + a] * c.u[j] + P.ref[1 + a] * c.du[j];      // m_a u_j - m0_a u0_j
+                if (j == a) v += c.dP;
+                F[j] = P.il * v;
+            }
+        }
+    }
+    __device__ static void wave(const double* Q, const KParams<double>& P, double* out) {
+        const double cc = sqrt(P.par[0] * Q[0]), u = Q[1] / Q[0], v = Q[2] / Q[0];
+        out[0] = fmax(fabs(u), fabs(v)) + cc; out[1] = sqrt(u * u + v * v) + cc; out[2] = 0.0;
+    }
+};
+
+// ------------------------------------------------------------------------------------------ Euler 2D
+// eq (3.4); p = (gamma-1)(E - rho|u|^2/2); par = {gamma}; Q = (rho, mx, my, E)
+template <class R> struct SysEuler2D {
+    static constexpr int ID = SYS_EULER2D, D = 2, M = 4, MC = 4;
+    using Mms = Mms_euler2d;
+    struct Ctx { R u[2], du[2], dp; };
+    __device__ __forceinline__ static void setup(Ctx& c, const R (&dQ)[M], const KParams<R>& P) {
+        const R rho = P.ref[0] + dQ[0];
+        const R r = R(1) / rho;
+        R dke = R(0);
+        for (int a = 0; a < 2; ++a) {
+            c.du[a] = (dQ[1 + a] - P.cst[a] * dQ[0]) * r;
+            c.u[a] = P.cst[a] + c.du[a];
+            dke += dQ[1 + a] * c.u[a] + P.ref[1 + a] * c.du[a];         // m.u - m0.u0
+        }
+        c.dp = (P.par[0] - R(1)) * (dQ[3] - R(0.5) * dke);
+    }
+    template <int k> __device__ __forceinline__ static void flux(const Ctx& c, const R (&dQ)[M], const KParams<R>& P, R (&F)[D], R& S) {
+        S = R(0);
+        if constexpr (k == 0) {
+            F[0] = P.il * dQ[1]; F[1] = P.il * dQ[2];
+        } else if constexpr (k == 3) {
+            for (int j = 0; j < 2; ++j) F[j] = P.il * ((dQ[3] + c.dp) * c.u[j] + P.cst[4] * c.du[j]);
+        } else {
+            constexpr int a = k - 1;
+            for (int j = 0; j < 2; ++j) {
+                R v = dQ[1 + a] * c.u[j] + P.ref[1 + a] * c.du[j];
+                if (j == a) v += c.dp;
+                F[j] = P.il * v;
+            }
+        }
+    }
+    __device__ static void wave(const double* Q, const KParams<double>& P, double* out) {
+        const double u = Q[1] / Q[0], v = Q[2] / Q[0];
+        const double p = (P.par[0] - 1.0) * (Q[3] - 0.5 * Q[0] * (u * u + v * v));
+        const double cc = sqrt(P.par[0] * p / Q[0]);
+        out[0] = fmax(fabs(u), fabs(v)) + cc; out[1] = sqrt(u * u + v * v) + cc; out[2] = 0.0;
+    }
+};
+
+// ------------------------------------------------------------------------------------------ scalar ADR
+// eq (3.17); SM4.7 L908-L926; par = {u_x, u_y, D, R}; Q = (c, G^L_x, G^L_y)
+template <class R> struct SysAdr2D {
+    static constexpr int ID = SYS_ADR2D, D = 2, M = 3, MC = 1;
+    using Mms = Mms_adr2d;
+    struct Ctx {};
+    __device__ __forceinline__ static void setup(Ctx&, const R (&)[M], const KParams<R>&) {}
+    template <int k> __device__ __forceinline__ static void flux(const Ctx&, const R (&dQ)[M], const KParams<R>& P, R (&F)[D], R& S) {
+        const R ax = P.par[0] * P.il, ay = P.par[1] * P.il;
+        if constexpr (k == 0) {
+            const R DL = P.par[2] * P.dL;
+            F[0] = ax * dQ[0] - DL * dQ[1];
+            F[1] = ay * dQ[0] - DL * dQ[2];
+            const R c = P.ref[0] + dQ[0];
+            S = P.dt * P.par[3] * c * (R(1) - c);                       // reaction at the full state
+        } else {
+            constexpr int b = k - 1;
+            F[0] = ax * dQ[k]; F[1] = ay * dQ[k];
+            F[b] -= dQ[0] * P.inv_gtau;
+            S = -(P.ref[k] + dQ[k]) * P.inv_gtau;
+        }
+    }
+    __device__ static void wave(const double* Q, const KParams<double>& P, double* out) {
+        const double ax = fabs(P.par[0]), ay = fabs(P.par[1]);
+        out[0] = fmax(ax, ay); out[1] = sqrt(ax * ax + ay * ay);
+        out[2] = sqrt(P.par[2] * P.dL * P.inv_gtau);
+    }
+};
+
+// ------------------------------------------------------------------------------------------ NSF 3D
+// eq (3.23), with derived-parent trackers after eq (3.27) (L495-L497):
+// Q = (rho, m(3), E, G^L_ab = dx d_b u_a [index 5+3a+b], H^L_b = dx d_b T [index 14+b]), T = p/rho.
+// par = {gamma, mu, K}.  Reference: rho0, E0 free; m0 = 0, trackers 0 (checked on the host).
+//   sigma_ab = mu_L (G_ab + G_ba - 2/3 tr G delta_ab)
+//   dF_rho,j = m_j/lam;  dF_ma,j = (m_a u_j + delta_aj dp)/lam - sigma_aj
+//   dF_E,j = (E0 + p0 + dE + dp) u_j/lam - sigma_jb u_b - K_L H_j
+//   dF_Gab,j = G_ab u_j/lam - delta_jb u_a/g_tau;  dF_Hb,j = H_b u_j/lam - delta_jb (T - T0)/g_tau
+//   T - T0 = (dp - T0 drho)/rho;  s_G = -G/g_tau, s_H = -H/g_tau
+template <class R> struct SysNsf3D {
+    static constexpr int ID = SYS_NSF3D, D = 3, M = 17, MC = 5;
+    using Mms = Mms_nsf3d;
+    struct Ctx { R u[3], ul[3], dp, dT, sig[6], Hh; };   // ul = u/lambda; sig: xx yy zz xy xz yz
+    __device__ __forceinline__ static int sidx(int a, int b) { return a == b ? a : (a + b + 2); }
+    __device__ __forceinline__ static void setup(Ctx& c, const R (&dQ)[M], const KParams<R>& P) {
+        const R rho = P.ref[0] + dQ[0];
+        const R r = R(1) / rho;
+        R ke = R(0);
+        for (int a = 0; a < 3; ++a) { c.u[a] = dQ[1 + a] * r; c.ul[a] = c.u[a] * P.il; ke += dQ[1 + a] * c.u[a]; }
+        c.dp = (P.par[0] - R(1)) * (dQ[4] - R(0.5) * ke);
+        c.dT = (c.dp - P.cst[5] * dQ[0]) * r;
+        const R muL = P.par[1] * P.dL;
+        const R tr = (R(2.0 / 3.0) * muL) * (dQ[5] + dQ[9] + dQ[13]);
+        c.sig[0] = R(2) * muL * dQ[5] - tr;
+        c.sig[1] = R(2) * muL * dQ[9] - tr;
+        c.sig[2] = R(2) * muL * dQ[13] - tr;
+        c.sig[3] = muL * (dQ[5 + 1] + dQ[5 + 3]);    // xy
+        c.sig[4] = muL * (dQ[5 + 2] + dQ[5 + 6]);    // xz
+        c.sig[5] = muL * (dQ[5 + 5] + dQ[5 + 7]);    // yz
+        c.Hh = P.cst[4] + dQ[4] + c.dp;              // E0 + p0 + dE + dp
+    }
+    template <int k> __device__ __forceinline__ static void flux(const Ctx& c, const R (&dQ)[M], const KParams<R>& P, R (&F)[D], R& S) {
+        if constexpr (k == 0) {
+            for (int j = 0; j < 3; ++j) F[j] = P.il * dQ[1 + j];
+            S = R(0);
+        } else if constexpr (k <= 3) {
+            constexpr int a = k - 1;
+            for (int j = 0; j < 3; ++j) {
+                R v = dQ[1 + a] * c.ul[j] - c.sig[sidx(a, j)];
+                if (j == a) v += P.il * c.dp;
+                F[j] = v;
+            }
+            S = R(0);
+        } else if constexpr (k == 4) {
+            const R KL = P.par[2] * P.dL;
+            for (int j = 0; j < 3; ++j)
+                F[j] = c.Hh * c.ul[j] - (c.sig[sidx(j, 0)] * c.u[0] + c.sig[sidx(j, 1)] * c.u[1] + c.sig[sidx(j, 2)] * c.u[2]) - KL * dQ[14 + j];
+            S = R(0);
+        } else if constexpr (k < 14) {
+            constexpr int a = (k - 5) / 3, b = (k - 5) % 3;
+            for (int j = 0; j < 3; ++j) F[j] = dQ[k] * c.ul[j];
+            F[b] -= c.u[a] * P.inv_gtau;
+            S = -dQ[k] * P.inv_gtau;
+        } else {
+            constexpr int b = k - 14;
+            for (int j = 0; j < 3; ++j) F[j] = dQ[k] * c.ul[j];
+            F[b] -= c.dT * P.inv_gtau;
+            S = -dQ[k] * P.inv_gtau;
+        }
+    }
+    __device__ static void wave(const double* Q, const KParams<double>& P, double* out) {
+        const double u[3] = {Q[1] / Q[0], Q[2] / Q[0], Q[3] / Q[0]};
+        const double u2 = u[0] * u[0] + u[1] * u[1] + u[2] * u[2];
+        const double p = (P.par[0] - 1.0) * (Q[4] - 0.5 * Q[0] * u2);
+        const double cc = sqrt(P.par[0] * p / Q[0]);
+        out[0] = fmax(fmax(fabs(u[0]), fabs(u[1])), fabs(u[2])) + cc;
+        out[1] = sqrt(u2) + cc;
+        const double kap = fmax(4.0 * P.par[1] * P.dL / (3.0 * Q[0]), P.par[2] * P.dL * (P.par[0] - 1.0) / Q[0]);
+        out[2] = sqrt(kap * P.inv_gtau);
+    }
+};
+
+// ------------------------------------------------------------------------------------------ resistive MHD 3D
+// eq (3.25), inviscid, no heat flux, no Powell source, current-density trackers
+// J^L = dx curl B in place of the full grad B (C5).  Q = (rho, m(3), E, B(3), J^L(3)).
+// par = {gamma, eta}.  Reference: rho0, E0 free; m0 = B0 = J0 = 0 (checked on the host).
+//   p = (gamma-1)(E - rho|u|^2/2 - |B|^2/2),  p_tot = p + |B|^2/2
+//   dF_ma,j = (m_a u_j - B_a B_j + delta_aj (dp + |B|^2/2))/lam
+//   dF_E,j = ((E0 + p0 + dE + dp + |B|^2/2) u_j - B_j (u.B))/lam + eta_L (J x B)_j
+//   dF_Bi,j = (B_i u_j - u_i B_j)/lam + eta_L eps_ijk J_k;   dF_Ji,j = J_i u_j/lam - eps_ijk B_k/g_tau
+template <class R> struct SysMhd3D {
+    static constexpr int ID = SYS_MHD3D, D = 3, M = 11, MC = 8;
+    using Mms = void;
+    struct Ctx { R u[3], ul[3], dpt, Hh, uB; };
+    __device__ __forceinline__ static void setup(Ctx& c, const R (&dQ)[M], const KParams<R>& P) {
+        const R rho = P.ref[0] + dQ[0];
+        const R r = R(1) / rho;
+        R ke = R(0), B2 = R(0);
+        c.uB = R(0);
+        for (int a = 0; a < 3; ++a) {
+            c.u[a] = dQ[1 + a] * r; c.ul[a] = c.u[a] * P.il;
+            ke += dQ[1 + a] * c.u[a]; B2 += dQ[5 + a] * dQ[5 + a]; c.uB += c.u[a] * dQ[5 + a];
+        }
+        const R dp = (P.par[0] - R(1)) * (dQ[4] - R(0.5) * ke - R(0.5) * B2);
+        c.dpt = dp + R(0.5) * B2;
+        c.Hh = P.cst[4] + dQ[4] + c.dpt;
+    }
+    // eps_ijk for (i, j): k index and sign; i != j
+    __device__ __forceinline__ static constexpr int eps_k(int i, int j) { return 3 - i - j; }
+    __device__ __forceinline__ static constexpr int eps_s(int i, int j) { return ((j - i + 3) % 3 == 1) ? +1 : -1; }
+    template <int k> __device__ __forceinline__ static void flux(const Ctx& c, const R (&dQ)[M], const KParams<R>& P, R (&F)[D], R& S) {
+        const R* B = &dQ[5];
+        const R* J = &dQ[8];
+        S = R(0);
+        if constexpr (k == 0) {
+            for (int j = 0; j < 3; ++j) F[j] = P.il * dQ[1 + j];
+        } else if constexpr (k <= 3) {
+            constexpr int a = k - 1;
+            for (int j = 0; j < 3; ++j) {
+                R v = dQ[1 + a] * c.u[j] - B[a] * B[j];
+                if (j == a) v += c.dpt;
+                F[j] = P.il * v;
+            }
+        } else if constexpr (k == 4) {
+            const R etaL = P.par[1] * P.dL;
+            const R JxB[3] = {J[1] * B[2] - J[2] * B[1], J[2] * B[0] - J[0] * B[2], J[0] * B[1] - J[1] * B[0]};
+            for (int j = 0; j < 3; ++j) F[j] = P.il * (c.Hh * c.u[j] - B[j] * c.uB) + etaL * JxB[j];
+        } else if constexpr (k < 8) {
+            constexpr int i = k - 5;
+            const R etaL = P.par[1] * P.dL;
+            for (int j = 0; j < 3; ++j) {
+                if (j == i) { F[j] = R(0); continue; }                  // B_i u_i - u_i B_i = 0
+                F[j] = P.il * (B[i] * c.u[j] - c.u[i] * B[j]) + R(eps_s(i, j)) * etaL * J[eps_k(i, j)];
+            }
+        } else {
+            constexpr int i = k - 8;
+            for (int j = 0; j < 3; ++j) {
+                F[j] = J[i] * c.ul[j];
+                if (j != i) F[j] -= R(eps_s(i, j)) * P.inv_gtau * B[eps_k(i, j)];
+            }
+            S = -J[i] * P.inv_gtau;
+        }
+    }
+    __device__ static void wave(const double* Q, const KParams<double>& P, double* out) {
+        const double rho = Q[0];
+        const double u[3] = {Q[1] / rho, Q[2] / rho, Q[3] / rho};
+        const double u2 = u[0] * u[0] + u[1] * u[1] + u[2] * u[2];
+        const double B2 = Q[5] * Q[5] + Q[6] * Q[6] + Q[7] * Q[7];
+        const double p = (P.par[0] - 1.0) * (Q[4] - 0.5 * rho * u2 - 0.5 * B2);
+        const double a2 = P.par[0] * p / rho, b2 = B2 / rho;
+        double m0 = 0.0;
+        for (int a = 0; a < 3; ++a) {
+            const double ba2 = Q[5 + a] * Q[5 + a] / rho;
+            const double cf = sqrt(0.5 * (a2 + b2 + sqrt(fmax((a2 + b2) * (a2 + b2) - 4.0 * a2 * ba2, 0.0))));
+            m0 = fmax(m0, fabs(u[a]) + cf);
+        }
+        out[0] = m0;
+        out[1] = sqrt(u2) + sqrt(a2 + b2);
+        out[2] = sqrt(P.par[1] * P.dL * P.inv_gtau);
+    }
+};
+
+}  // namespace lbmk

@@ -1,0 +1,441 @@
+"""Build-time generator: manufactured-solution forcing (eq 4.1) -> CUDA/C++ source.
+
+Product-side code (the CUDA path's counterpart of the paper's "Emit" stage, Alg 2.1 lines 24-25,
+PAPER.md:L275-L277).  It shares nothing with `oracle/`: the oracle forms the same residual numerically
+with forward-mode jets; here the residual of the AUGMENTED system (trackers forced too, reading A5) is
+derived symbolically, once, and printed as straight-line code:
+
+    s_k(x, t) = dt d_t Q_k + dx sum_a d_a F_k,a(Q_exact) - S_k(Q_exact)            (lattice units)
+
+Two layers keep the expression small:
+  layer 2  the residual written for abstract primitive fields P(t,x,y,z) (rho, u, p, ...): SymPy applies
+           the product/chain rules; every Derivative(P, ...) atom becomes a scalar symbol `P_tx` etc.
+  layer 1  the closed form of each such atom from the concrete trigonometric fields.  Every sin/cos/exp
+           atom depends on ONE of t, x, y, z (after expand_trig), so it is either a per-step "time scalar"
+           (host, fp64) or an entry of a per-axis table (host, fp64, one row per node coordinate).
+Both layers are CSE'd together.  Output: `csrc/mms_generated.cuh` (device functions + host table code).
+
+Run from the repo root:   python -m paper_2607_05668_b200.gen.mms_codegen
+The generated header is committed; `__graft_entry__.build()` does not need SymPy.
+"""
+from __future__ import annotations
+
+import os
+import sys
+from typing import Callable, Dict, List, Sequence, Tuple
+
+import sympy as sp
+from sympy.printing.c import C99CodePrinter
+
+t, x, y, z = sp.symbols("t x y z", real=True)
+COORDS = (t, x, y, z)
+CNAME = {t: "t", x: "x", y: "y", z: "z"}
+# scaling symbols shared by all systems
+dx, dt, il, gtau = sp.symbols("dx dt il gtau", positive=True)   # il = dt/dx = 1/lambda
+TWO_PI = sp.Symbol("TWO_PI", positive=True)
+
+
+def par(i):
+    return sp.Symbol(f"par{i}", real=True)
+
+
+def mp(i):
+    return sp.Symbol(f"mp{i}", real=True)
+
+
+# ------------------------------------------------------------------------------------------------ systems
+# Each system: (name, dim, primitive names, concrete primitive fields, augmented state/flux/source builder)
+# builder(P: dict name -> expr, D: callable(expr, coord) -> derivative) -> (Q[m], F[m][dim], S[m])
+
+def sys_burgers2d():
+    A = mp(0)
+    k = TWO_PI
+    prim = {"u": A * sp.sin(k * x) * sp.sin(k * y) * sp.cos(t)}          # eq SM5.1
+
+    def build(P, D):
+        u = P["u"]
+        return [u], [[il * u * u / 2, il * u * u / 2]], [sp.Integer(0)]   # eq 3.1-3.2
+    return "burgers2d", 2, prim, build
+
+
+def sys_swe2d():
+    g = par(0)
+    Ah, Au, h0 = mp(0), mp(1), mp(2)
+    k = TWO_PI
+    prim = {"h": h0 + Ah * sp.sin(k * x) * sp.cos(k * y) * sp.cos(t),
+            "u": Au * sp.cos(k * x) * sp.sin(k * y) * sp.cos(t),
+            "v": Au * sp.sin(k * x) * sp.sin(k * y) * sp.sin(t)}
+
+    def build(P, D):
+        h, u, v = P["h"], P["u"], P["v"]
+        Pr = g * h * h / 2                                                # eq 3.6, flat bottom
+        Q = [h, h * u, h * v]
+        F = [[il * h * u, il * h * v],
+             [il * (h * u * u + Pr), il * h * u * v],
+             [il * h * u * v, il * (h * v * v + Pr)]]
+        return Q, F, [sp.Integer(0)] * 3
+    return "swe2d", 2, prim, build
+
+
+def sys_euler2d():
+    gamma = par(0)
+    k = TWO_PI
+    rho0, cs = sp.Integer(1), sp.Integer(1)                              # non-dimensional, reading A9
+    p0 = rho0 * cs * cs / gamma
+    drho = sp.Rational(3, 10) * rho0 * sp.sin(k * x) * sp.cos(k * y) * sp.cos(t)   # eq SM5.2
+    prim = {"rho": rho0 + drho,
+            "u": 3 * cs + sp.Rational(3, 10) * cs * sp.cos(k * x) * sp.sin(k * y) * sp.sin(t),
+            "v": 3 * cs + sp.Rational(3, 10) * cs * sp.sin(k * x) * sp.sin(k * y) * sp.sin(t),
+            "p": p0 + cs * cs * drho + sp.Rational(1, 5) * p0 * sp.cos(k * x) * sp.sin(k * y) * sp.sin(t)}
+
+    def build(P, D):
+        rho, u, v, p = P["rho"], P["u"], P["v"], P["p"]
+        E = p / (gamma - 1) + rho * (u * u + v * v) / 2
+        Q = [rho, rho * u, rho * v, E]
+        F = [[il * rho * u, il * rho * v],                                # eq 3.4
+             [il * (rho * u * u + p), il * rho * u * v],
+             [il * rho * u * v, il * (rho * v * v + p)],
+             [il * (E + p) * u, il * (E + p) * v]]
+        return Q, F, [sp.Integer(0)] * 4
+    return "euler2d", 2, prim, build
+
+
+def sys_adr2d():
+    ux, uy, Dc, R = par(0), par(1), par(2), par(3)
+    k = TWO_PI
+    prim = {"c": sp.Rational(1, 2) * sp.sin(k * (x - ux * t)) * sp.cos(k * (y - uy * t)) * sp.exp(-t)
+            + sp.Rational(1, 2)}                                          # eq SM5.7
+
+    def build(P, D):
+        c = P["c"]
+        G = [dx * D(c, x), dx * D(c, y)]                                  # lattice-unit trackers, L298
+        DL = Dc * dt / dx**2
+        Q = [c, G[0], G[1]]
+        F = [[ux * il * c - DL * G[0], uy * il * c - DL * G[1]],         # eq 3.17
+             [ux * il * G[0] - c / gtau, uy * il * G[0]],
+             [ux * il * G[1], uy * il * G[1] - c / gtau]]
+        S = [dt * R * c * (1 - c), -G[0] / gtau, -G[1] / gtau]
+        return Q, F, S
+    return "adr2d", 2, prim, build
+
+
+def sys_nsf3d():
+    gamma, mu, K = par(0), par(1), par(2)
+    U0, Ar, rho0, p0 = mp(0), mp(1), mp(2), mp(3)
+    k = TWO_PI
+    Dt = sp.exp(-3 * (mu / rho0) * k * k * t)
+    sx, cx, sy, cy, sz, cz = sp.sin(k * x), sp.cos(k * x), sp.sin(k * y), sp.cos(k * y), sp.sin(k * z), sp.cos(k * z)
+    prim = {"rho": rho0 * (1 + Ar * sx * sy * cz * sp.cos(t)),
+            "u0": U0 * sx * cy * cz * Dt,
+            "u1": -U0 * cx * sy * cz * Dt,
+            "u2": U0 / 2 * cx * cy * sz * Dt,
+            "p": p0 + (rho0 * U0 * U0 / 16) * (sp.cos(2 * k * x) + sp.cos(2 * k * y)) * (sp.cos(2 * k * z) + 2) * Dt * Dt}
+
+    def build(P, D):
+        X = (x, y, z)
+        rho, p = P["rho"], P["p"]
+        u = [P["u0"], P["u1"], P["u2"]]
+        T = p / rho
+        E = p / (gamma - 1) + rho * sum(ua * ua for ua in u) / 2
+        G = [[dx * D(u[a], X[b]) for b in range(3)] for a in range(3)]    # G_ab = dx d_b u_a
+        H = [dx * D(T, X[b]) for b in range(3)]
+        muL, KL = mu * dt / dx**2, K * dt / dx**2
+        trG = G[0][0] + G[1][1] + G[2][2]
+        sig = [[muL * (G[a][b] + G[b][a]) - (sp.Rational(2, 3) * muL * trG if a == b else 0) for b in range(3)]
+               for a in range(3)]
+        Q = [rho] + [rho * ua for ua in u] + [E] + [G[a][b] for a in range(3) for b in range(3)] + H
+        F = [[il * rho * u[j] for j in range(3)]]                         # eq 3.23
+        for a in range(3):
+            F.append([il * (rho * u[a] * u[j] + (p if a == j else 0)) - sig[a][j] for j in range(3)])
+        F.append([il * (E + p) * u[j] - sum(sig[j][b] * u[b] for b in range(3)) - KL * H[j] for j in range(3)])
+        for a in range(3):
+            for b in range(3):
+                F.append([il * G[a][b] * u[j] - (u[a] / gtau if j == b else 0) for j in range(3)])
+        for b in range(3):
+            F.append([il * H[b] * u[j] - (T / gtau if j == b else 0) for j in range(3)])
+        S = [sp.Integer(0)] * 5 + [-G[a][b] / gtau for a in range(3) for b in range(3)] + [-H[b] / gtau for b in range(3)]
+        return Q, F, S
+    return "nsf3d", 3, prim, build
+
+
+SYSTEMS = [sys_burgers2d, sys_swe2d, sys_euler2d, sys_adr2d, sys_nsf3d]
+
+
+# ------------------------------------------------------------------------------------------------ printing
+class _Printer(C99CodePrinter):
+    """C printer with R(...)-typed literals and multiplications instead of pow()."""
+
+    def __init__(self, real="R"):
+        super().__init__()
+        self.real = real
+
+    def _lit(self, s):
+        return f"{self.real}({s})" if self.real else s
+
+    def _print_Float(self, e):
+        return self._lit(repr(float(e)))
+
+    def _print_Integer(self, e):
+        return self._lit(f"{int(e)}.0")
+
+    def _print_Rational(self, e):
+        return self._lit(f"{int(e.p)}.0/{int(e.q)}.0")
+
+    def _print_Pow(self, e):
+        b, ex = e.base, e.exp
+        if ex.is_Integer and -8 <= int(ex) <= 8 and int(ex) != 0:
+            n = abs(int(ex))
+            s = "*".join([self.parenthesize(b, 60)] * n)
+            if n > 1:
+                s = f"({s})"
+            return f"({self._lit('1.0')}/{s})" if int(ex) < 0 else s
+        if ex == sp.Rational(1, 2):
+            return f"sqrt({self._print(b)})"
+        raise ValueError(f"unsupported power {e}")
+
+
+def _atom_symbol_name(f, wrt: Sequence[sp.Symbol]) -> str:
+    return f.func.__name__ + ("_" + "".join(CNAME[c] for c in wrt) if wrt else "")
+
+
+def _separate(expr):
+    """Rewrite sin/cos atoms whose argument mixes coordinates into products of single-coordinate atoms."""
+    repl = {}
+    for a in expr.atoms(sp.sin, sp.cos):
+        if len(a.free_symbols & set(COORDS)) > 1:
+            repl[a] = sp.expand_trig(a.func(sp.expand(a.args[0])))
+    return expr.xreplace(repl) if repl else expr
+
+
+def generate_system(name, dim, prim_concrete, build):
+    X = (x, y, z)[:dim]
+    prim_concrete = {k: _separate(v) for k, v in prim_concrete.items()}
+    # ---- layer 2: residual for abstract primitives
+    Pf = {k: sp.Function(k)(t, x, y, z) for k in prim_concrete}
+    Q, F, S = build(Pf, lambda e, c: sp.diff(e, c))
+    m = len(Q)
+    res = []
+    for k in range(m):
+        r = dt * sp.diff(Q[k], t) + dx * sum(sp.diff(F[k][a], X[a]) for a in range(dim)) - S[k]
+        res.append(r.doit())
+    # ---- every abstract atom (function value or derivative) -> scalar symbol
+    atom_syms: Dict[sp.Basic, sp.Symbol] = {}
+    layer1: List[Tuple[sp.Symbol, sp.Expr]] = []
+
+    def atom_to_symbol(a):
+        if a in atom_syms:
+            return atom_syms[a]
+        if isinstance(a, sp.Derivative):
+            f = a.expr
+            wrt = []
+            for v, n in a.variable_count:
+                wrt += [v] * int(n)
+            wrt.sort(key=COORDS.index)
+        else:
+            f, wrt = a, []
+        s = sp.Symbol(_atom_symbol_name(f, wrt), real=True)
+        concrete = prim_concrete[f.func.__name__]
+        for v in wrt:
+            concrete = sp.diff(concrete, v)
+        atom_syms[a] = s
+        layer1.append((s, concrete))
+        return s
+
+    def lower(e):
+        repl = {}
+        for a in e.atoms(sp.Derivative):
+            repl[a] = atom_to_symbol(a)
+        e = e.xreplace(repl)
+        repl = {}
+        for a in e.atoms(sp.core.function.AppliedUndef):
+            repl[a] = atom_to_symbol(a)
+        return e.xreplace(repl)
+
+    res_l = [lower(r) for r in res]
+    Q_l = [lower(q.doit()) for q in Q]
+    # light algebra: cancels the tracker 1/g_tau pair and the rho*u/rho quotients, keeps factored products
+    res_l = [sp.factor_terms(sp.expand(r)) for r in res_l]
+    # ---- layer 1: closed forms; classify trig/exp atoms into time scalars and per-axis table entries
+    tabs: Dict[sp.Symbol, List[sp.Expr]] = {c: [] for c in COORDS}
+    tab_syms: Dict[sp.Basic, sp.Symbol] = {}
+
+    def table_symbol(a):
+        if a in tab_syms:
+            return tab_syms[a]
+        fs = a.free_symbols & set(COORDS)
+        assert len(fs) == 1, f"atom {a} is not separable"
+        c = next(iter(fs))
+        s = sp.Symbol(f"{CNAME[c].upper()}{len(tabs[c])}", real=True)
+        tabs[c].append(a)
+        tab_syms[a] = s
+        return s
+
+    layer1_l = []
+    for s, e in layer1:
+        e = sp.expand(e)
+        repl = {a: table_symbol(a) for a in sorted(e.atoms(sp.sin, sp.cos, sp.exp), key=str)}
+        e = e.xreplace(repl)
+        assert not (e.free_symbols & set(COORDS)), f"{s}: bare coordinate left in {e}"
+        layer1_l.append((s, sp.factor_terms(e)))
+    return dict(name=name, dim=dim, m=m, layer1=layer1_l, res=res_l, Q=Q_l, tabs=tabs)
+
+
+def _used_symbols(exprs):
+    out = set()
+    for e in exprs:
+        out |= e.free_symbols
+    return out
+
+
+def _emit_body(assign: List[Tuple[sp.Symbol, sp.Expr]], outputs: List[sp.Expr], out_name: str, pr: _Printer, indent="    "):
+    """CSE the layer-1 definitions and the outputs together and print the definitions the outputs need,
+    in dependency order.  Returns (code lines, operation count, free input symbols)."""
+    l1_syms = [s for s, _ in assign]
+    exprs = [e for _, e in assign] + list(outputs)
+    repl, red = sp.cse(exprs, symbols=sp.numbered_symbols("v"), optimizations="basic")
+    defs = list(repl) + [(l1_syms[i], red[i]) for i in range(len(assign))]
+    index_of = {s: i for i, (s, _) in enumerate(defs)}
+    out_red = red[len(assign):]
+    done, ordered = set(), []
+
+    def visit(i):
+        if i in done:
+            return
+        done.add(i)
+        for d in sorted(defs[i][1].free_symbols, key=str):
+            if d in index_of:
+                visit(index_of[d])
+        ordered.append(i)
+
+    for e in out_red:
+        for d in sorted(e.free_symbols, key=str):
+            if d in index_of:
+                visit(index_of[d])
+    lines, ops, free = [], 0, set()
+    for i in ordered:
+        s, e = defs[i]
+        lines.append(f"{indent}const {pr.real} {s} = {pr.doprint(e)};")
+        ops += int(sp.count_ops(e))
+        free |= e.free_symbols
+    for k, e in enumerate(out_red):
+        lines.append(f"{indent}{out_name}[{k}] = {pr.doprint(e)};")
+        ops += int(sp.count_ops(e))
+        free |= e.free_symbols
+    free -= {defs[i][0] for i in ordered}
+    return lines, ops, free
+
+
+# ------------------------------------------------------------------------------------------------ emission
+SCALARS = {"dx": "a.dx", "dt": "a.dt", "il": "a.il", "gtau": "a.gtau", "TWO_PI": "R(6.283185307179586477)"}
+
+
+def _bind_inputs(free, real, tab_prefix=True):
+    """Declarations binding the free symbols of a body to the argument struct / table rows."""
+    out = []
+    for s in sorted(free, key=str):
+        n = str(s)
+        if n in SCALARS:
+            out.append(f"    const {real} {n} = {SCALARS[n]};")
+        elif n.startswith("par"):
+            out.append(f"    const {real} {n} = a.par[{int(n[3:])}];")
+        elif n.startswith("mp"):
+            out.append(f"    const {real} {n} = a.mp[{int(n[2:])}];")
+        elif n[0] in "TXYZ" and n[1:].isdigit():
+            out.append(f"    const {real} {n} = {n[0]}[{int(n[1:])}];")
+        else:
+            raise ValueError(f"unbound symbol {n}")
+    return out
+
+
+def _host_expr(e, coord):
+    """C++ (double) text of a table atom as a function of the scalar `c` (the coordinate or the time)."""
+    pr = _Printer(real="")
+    pr._lit = lambda s: s
+    e = e.xreplace({coord: sp.Symbol("c"), TWO_PI: sp.Symbol("6.283185307179586477")})
+    return pr.doprint(e)
+
+
+def emit_system(g) -> str:
+    name, m, dim = g["name"], g["m"], g["dim"]
+    pr = _Printer("R")
+    src_lines, src_ops, src_free = _emit_body(g["layer1"], g["res"], "s", pr)
+    q_lines, q_ops, q_free = _emit_body(g["layer1"], g["Q"], "q", pr)
+    nt, nx_, ny_, nz_ = (len(g["tabs"][c]) for c in COORDS)
+    o = []
+    o.append(f"// ---- {name}: m = {m}, dim = {dim}; forcing {src_ops} ops, exact state {q_ops} ops")
+    o.append(f"struct Mms_{name} {{")
+    o.append(f"    static constexpr int M = {m}, NT = {nt}, NX = {nx_}, NY = {ny_}, NZ = {max(nz_, 0)};")
+    # host: time scalars and axis rows
+    o.append("    // host side (fp64): per-step time scalars and per-axis table rows")
+    o.append("    static inline void time_scalars(double c, const MmsHostArgs& a, double* T) {")
+    o.append("        (void)c; (void)a; (void)T;")
+    for i, e in enumerate(g["tabs"][t]):
+        o.append(f"        T[{i}] = {_host_bind(_host_expr(e, t))};")
+    o.append("    }")
+    o.append("    static inline void axis_row(int axis, double c, const MmsHostArgs& a, double* row) {")
+    o.append("        (void)c; (void)a; (void)row;")
+    for ax, cs in enumerate((x, y, z)):
+        if not g["tabs"][cs]:
+            continue
+        o.append(f"        if (axis == {ax}) {{")
+        for i, e in enumerate(g["tabs"][cs]):
+            o.append(f"            row[{i}] = {_host_bind(_host_expr(e, cs))};")
+        o.append("        }")
+    o.append("    }")
+    # device: forcing and exact state
+    for fn, lines, free, outn in (("source", src_lines, src_free, "s"), ("exact", q_lines, q_free, "q")):
+        o.append("    template <class R>")
+        o.append(f"    static __host__ __device__ __forceinline__ void {fn}(const MmsArgs<R>& a, const R* T, const R* X, const R* Y, const R* Z, R* {outn}) {{")
+        o.append("        (void)a; (void)T; (void)X; (void)Y; (void)Z;")
+        o += ["    " + l for l in _bind_inputs(free, "R")]
+        o += ["    " + l for l in lines]
+        o.append("    }")
+    o.append("};")
+    return "\n".join(o)
+
+
+def _host_bind(text: str) -> str:
+    """par<i>/mp<i> symbols inside a host table expression -> a.par[i] / a.mp[i]."""
+    import re
+    text = re.sub(r"\bpar(\d+)\b", r"a.par[\1]", text)
+    text = re.sub(r"\bmp(\d+)\b", r"a.mp[\1]", text)
+    return text
+
+
+HEADER = """// mms_generated.cuh -- GENERATED by paper_2607_05668_b200/gen/mms_codegen.py; do not edit.
+//
+// Manufactured-solution forcing s_k = dt d_t Q_k + dx div F_k(Q_exact) - S_k(Q_exact) of eq (4.1)
+// (PAPER.md:L499-L504) for the AUGMENTED system (trackers forced too), and the exact augmented state
+// Q_exact, as straight-line code over per-step time scalars T[] and per-axis table rows X[], Y[], Z[]
+// (every trigonometric/exponential atom of the exact fields depends on one coordinate only).
+// Exact fields: Burgers eq SM5.1 (L1161), Euler eq SM5.2 (L1175-L1186), ADR eq SM5.7 (L1292); SWE and
+// NSF3D are the BASELINE.json configs[1] / configs[3] fields (DESIGN.md "Input recipe").
+#pragma once
+#include <cmath>
+
+namespace lbmk {
+
+struct MmsHostArgs { double par[16]; double mp[16]; double dx, dt, il, gtau; };
+template <class R> struct MmsArgs { R par[8]; R mp[8]; R dx, dt, il, gtau; };
+
+"""
+
+
+def main(out_path=None):
+    here = os.path.dirname(os.path.abspath(__file__))
+    out_path = out_path or os.path.join(os.path.dirname(here), "csrc", "mms_generated.cuh")
+    parts = [HEADER]
+    for mk in SYSTEMS:
+        name, dim, prim, build = mk()
+        g = generate_system(name, dim, prim, build)
+        parts.append(emit_system(g))
+        parts.append("")
+        print(f"generated {name}", file=sys.stderr)
+    parts.append("}  // namespace lbmk\n")
+    with open(out_path, "w") as fh:
+        fh.write("\n".join(parts))
+    print(out_path)
+
+
+if __name__ == "__main__":
+    main(*sys.argv[1:])

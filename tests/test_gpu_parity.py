@@ -1,0 +1,234 @@
+"""GPU parity: the CUDA path (through the C-ABI, via the thin binding) against the CPU oracle, element by
+element on the same seeded inputs.  Bars (BASELINE.json north_star): bit-exact integer index maps and pure
+streaming; max relative error <= 1e-12 in fp64; <= 2e-5 in shifted fp32 (metric: DESIGN.md reading A16).
+"""
+import numpy as np
+import pytest
+
+import oracle
+import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL64 = 1e-12
+TOL32 = 2e-5
+
+
+@pytest.fixture(scope="module")
+def P():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (run with -m 'not gpu' on CPU boxes)")
+    import paper_2607_05668_b200 as P
+    P.lib()
+    return P
+
+
+def rel_err(U, Uo):
+    """per component max|dU| / max|U_oracle| (A16); identically-zero components use the system scale."""
+    scale_sys = max(np.abs(Uo).max(), 1e-300)
+    out = []
+    for k in range(U.shape[0]):
+        s = np.abs(Uo[k]).max()
+        out.append(np.abs(U[k] - Uo[k]).max() / (s if s > 1e-12 * scale_sys else scale_sys))
+    return np.array(out)
+
+
+def small(name, **kw):
+    """A reduced-size instance of a baseline config with identical physics parameters per node spacing."""
+    return W.BASELINE_CONFIGS[name](**kw)
+
+
+def run_pair(P, w, steps, precision=None, pattern="auto", kernel="auto", shifted_oracle=False):
+    U0 = w.initial_U()
+    g = P.Grid.from_workload(w, precision=precision, pattern=pattern, kernel=kernel)
+    g.init_from_U(U0)
+    g.step(steps)
+    U = g.read_U()
+    f = g.read_populations()
+    g.close()
+    o = oracle.OracleGrid.from_workload(w, shifted=shifted_oracle)
+    o.init_from_U(U0)
+    o.step(steps)
+    Uo, fo = o.read_U(), o.read_f()
+    o.close()
+    return U, f, Uo, fo
+
+
+# ------------------------------------------------------------------------------------------- integer work
+@pytest.mark.parametrize("system,shape", [("euler2d", (1, 5, 7)), ("euler2d", (1, 64, 33)), ("mhd3d", (3, 4, 5)),
+                                          ("mhd3d", (9, 6, 34)), ("advection2d", (1, 1, 1))])
+def test_stream_index_map_bit_exact(P, system, shape):
+    nz, ny, nx = shape
+    s = P.System(system, params={"euler2d": [1.4], "mhd3d": [1.4, 1e-3], "advection2d": [0.1, 0.05]}[system], tau_R=1.0, g_tau=4.0)
+    g = P.Grid(s, nx, ny, nz, 1.0, 4.0)
+    o = oracle.OracleGrid(system, nx, ny, nz, 1.0, 4.0, params={"euler2d": [1.4], "mhd3d": [1.4, 1e-3], "advection2d": [0.1, 0.05]}[system], g_tau=4.0)
+    for d in range(s.Q):
+        a, b = g.stream_index_map(d), o.stream_index_map(d)
+        assert a.dtype == np.int64 and np.array_equal(a, b), f"direction {d}"
+    g.close(); o.close()
+
+
+@pytest.mark.parametrize("pattern", ["pull2", "aa"])
+@pytest.mark.parametrize("system,shape,steps", [("euler2d", (1, 5, 7), 9), ("euler2d", (1, 37, 130), 4), ("swe2d", (1, 6, 4), 5)])
+def test_pure_streaming_bit_exact(P, system, shape, steps, pattern):
+    """omega = 0, S = 0: N steps are pure shifts f_i(x, N) = f_i(x - N c_i, 0), bit for bit (pin P5 on the GPU)."""
+    nz, ny, nx = shape
+    par = {"euler2d": [1.4], "swe2d": [1.0]}[system]
+    rng = np.random.default_rng(7)
+    s = P.System(system, params=par, omega=0.0)
+    g = P.Grid(s, nx, ny, nz, 1.0, 4.0, pattern=pattern)
+    f0 = 1.0 + rng.random(g.shape_f)
+    g.set_populations(f0)
+    g.step(steps)
+    f = g.read_populations()
+    c, _, _ = P.lbmk_lattice_constants(0)
+    for i in range(s.Q):
+        want = np.roll(f0[:, i], shift=(steps * c[i][2], steps * c[i][1], steps * c[i][0]), axis=(1, 2, 3))
+        assert np.array_equal(f[:, i], want), f"direction {i}"
+    o = oracle.OracleGrid(system, nx, ny, nz, 1.0, 4.0, params=par, omega=0.0)
+    o.set_f(f0); o.step(steps)
+    assert np.array_equal(f, o.read_f())
+    g.close(); o.close()
+
+
+# ------------------------------------------------------------------------------------------- fp64 parity
+CASES64 = [
+    # (config, constructor kwargs, steps)
+    ("c1", dict(n=64), 200),                         # BASELINE.json configs[0], full size and duration
+    ("c1", dict(n=37, ny=23), 51),                   # ragged, odd step count
+    ("c2", dict(n=96, ny=50), 120),
+    ("c3", dict(n=80, ny=36, precision="f64"), 61),
+    ("c4", dict(n=20, ny=12, nz=9, precision="f64"), 30),
+    ("c4", dict(n=16, precision="f64", mms=False), 25),
+    ("c5", dict(n=24, ny=10, nz=7, precision="f64"), 31),
+]
+
+
+@pytest.mark.parametrize("pattern", ["pull2", "aa"])
+@pytest.mark.parametrize("name,kw,steps", CASES64)
+def test_parity_fp64(P, name, kw, steps, pattern):
+    w = small(name, **kw)
+    U, f, Uo, fo = run_pair(P, w, steps, precision="f64", pattern=pattern)
+    assert np.isfinite(U).all()
+    e = rel_err(U, Uo)
+    assert e.max() <= TOL64, f"{w.name} U rel err {e}"
+    ef = np.abs(f - fo).max() / np.abs(fo).max()
+    assert ef <= TOL64, f"{w.name} populations rel err {ef}"
+
+
+@pytest.mark.parametrize("mk,n,steps", [(W.pin_burgers, 48, 100), (W.pin_euler, 40, 150), (W.pin_adr, 32, 300)])
+def test_parity_fp64_paper_systems_with_mms(P, mk, n, steps):
+    """The three Table-2 systems (Burgers L518, Euler L519-L522, ADR L540) with their manufactured forcing."""
+    w = mk(n)
+    U, f, Uo, fo = run_pair(P, w, steps, precision="f64")
+    e = rel_err(U, Uo)
+    assert e.max() <= TOL64, f"{w.name} {e}"
+
+
+@pytest.mark.parametrize("name,kw,steps", [("c2", dict(n=64), 40), ("c3", dict(n=48, precision="f64"), 40),
+                                           ("c4", dict(n=12, precision="f64"), 20), ("c5", dict(n=12, precision="f64"), 20)])
+def test_shifted_fp64_matches_unshifted_oracle(P, name, kw, steps):
+    """eq (2.23) is an identity: the delta-form kernels in fp64 reproduce the plain fp64 oracle (pin P7 on the GPU)."""
+    w = small(name, **kw)
+    U, f, Uo, fo = run_pair(P, w, steps, precision="f64s")
+    e = rel_err(U, Uo)
+    assert e.max() <= 1e-11, f"{w.name} {e}"
+    assert np.abs(f - fo).max() / np.abs(fo).max() <= 1e-11
+
+
+def test_shifted_fp64_general_reference_momentum(P):
+    """Euler with a moving reference state u0 = v0 = 3 (the paper's SM5.3 fields): general delta form."""
+    w = W.pin_euler(40)
+    U, f, Uo, fo = run_pair(P, w, 120, precision="f64s")
+    assert rel_err(U, Uo).max() <= 1e-11
+
+
+# ------------------------------------------------------------------------------------------- shifted fp32
+CASES32 = [
+    ("c3", dict(n=128, ny=72), 500),                 # BASELINE.json configs[2] physics, full duration
+    ("c4", dict(n=32, ny=24, nz=20), 200),           # configs[3], full duration, MMS forcing on
+    ("c4", dict(n=24, mms=False), 60),
+    ("c5", dict(n=32, ny=20, nz=24), 200),           # configs[4], full duration
+    ("c2", dict(n=64, precision="f32s"), 200),
+]
+
+
+@pytest.mark.parametrize("pattern", ["pull2", "aa"])
+@pytest.mark.parametrize("name,kw,steps", CASES32)
+def test_parity_fp32_shifted(P, name, kw, steps, pattern):
+    w = small(name, **kw)
+    assert w.precision == "f32s"
+    U, f, Uo, fo = run_pair(P, w, steps, pattern=pattern)
+    assert np.isfinite(U).all()
+    e = rel_err(U, Uo)
+    assert e.max() <= TOL32, f"{w.name} U rel err {e}"
+    # stricter, reported figure: relative to the fluctuation about the reference state (A16)
+    ref = np.asarray(w.U_ref).reshape(-1, 1, 1, 1)
+    fl = np.array([np.abs(U[k] - Uo[k]).max() / max(np.abs(Uo[k] - ref[k]).max(), 1e-30) for k in range(U.shape[0])])
+    print(f"{w.name} [{pattern}] rel err max {e.max():.2e}; fluctuation-relative max {fl.max():.2e}")
+
+
+def test_fp32_uniform_reference_state_stays_exactly_zero(P):
+    """delta = 0 is a fixed point of the shifted form, exactly (pin P6 on the GPU, eq 2.23)."""
+    for name, kw in (("c3", dict(n=32)), ("c4", dict(n=8, mms=False)), ("c5", dict(n=8))):
+        w = small(name, **kw)
+        U0 = np.broadcast_to(np.asarray(w.U_ref).reshape(-1, 1, 1, 1), (w.m_total, w.nz, w.ny, w.nx)).copy()
+        g = P.Grid.from_workload(w)
+        g.init_from_U(U0)
+        g.step(7)
+        assert np.array_equal(g.read_U(), U0)
+        g.close()
+
+
+# ------------------------------------------------------------------- full size, bench launch configuration
+def _subbox_check(P, w, steps, box, origin, tol):
+    """GPU: the full-size grid of the config.  Oracle: a periodic sub-box with the same node coordinates;
+    nodes at least `steps` away from the sub-box faces have the same domain of dependence in both runs."""
+    U0 = w.initial_U()
+    g = P.Grid.from_workload(w)
+    g.init_from_U(U0)
+    g.step(steps)
+    U = g.read_U()
+    g.close()
+    bz, by, bx = box
+    oz, oy, ox = origin
+    sl = (slice(None), slice(oz, oz + bz), slice(oy, oy + by), slice(ox, ox + bx))
+    o = oracle.OracleGrid.from_workload(w, nx=bx, ny=by, nz=bz, origin=(ox, oy, oz))
+    o.init_from_U(np.ascontiguousarray(U0[sl]))
+    o.step(steps)
+    Uo = o.read_U()
+    o.close()
+    m = steps
+    inner = (slice(None), slice(m, bz - m) if w.dim == 3 else slice(None), slice(m, by - m), slice(m, bx - m))
+    Ug = U[sl][inner]
+    e = rel_err(Ug, Uo[inner])
+    assert Ug.size > 0 and e.max() <= tol, f"{w.name}: {e}"
+    return U
+
+
+def test_full_size_c2_sampled(P):
+    w = W.c2_swe()
+    _subbox_check(P, w, 12, (1, 64, 64), (0, 300, 200), TOL64)
+
+
+def test_full_size_c3_sampled_and_conservation(P):
+    w = W.c3_euler()
+    U = _subbox_check(P, w, 10, (1, 60, 72), (0, 1000, 1500), TOL32)
+    # unforced periodic run conserves the totals (pin P2 at full size)
+    U0 = w.initial_U()
+    for k in (0, 3):
+        assert abs(U[k].sum() - U0[k].sum()) / abs(U0[k].sum()) < 1e-6
+
+
+def test_full_size_c4_sampled(P):
+    w = W.c4_nsf3d()
+    _subbox_check(P, w, 6, (24, 28, 40), (100, 17, 200), TOL32)
+
+
+def test_full_size_c5_sampled_and_conservation(P):
+    w = W.c5_mhd3d()
+    U = _subbox_check(P, w, 6, (24, 28, 40), (150, 3, 90), TOL32)
+    U0 = w.initial_U()
+    for k in (0, 4):
+        assert abs(U[k].sum() - U0[k].sum()) / abs(U0[k].sum()) < 1e-6
