@@ -7,16 +7,22 @@
 // Because c_i are the axis unit vectors and w_i/c_s^2 = 1/2 for them, the relaxation reads
 //   rest:   f' = (1-omega) f + w0 (omega dQ + s)
 //   +-a:    f' = (1-omega) f + w1 (omega dQ + s) +- (omega/2) dF_a .
-// Streaming patterns (MODE): PULL2 reads buffer `src` at x - c_i and writes buffer `dst` at x (two
-// lattices); AA is in place: the even step reads slot i at x and writes slot opp(i) at x, the odd step
-// reads slot opp(i) at x - c_i and writes slot i at x + c_i.  After an even number of steps (and always in
-// PULL2) storage is canonical: slot i at x holds the population that arrived at x along c_i.
+// Streaming patterns (MODE).  Canonical state after n steps: slot i at x holds the population that arrived
+// at x along c_i (what the oracle's array holds after its stream).  Storage states (GATHER_*):
+//   two-lattice pull: the first step after init is LOCAL (read slot i at x of `src`, collide, write slot i at
+//     x of `dst`); the storage is then post-collision with the stream pending (GATHER_PULL: the canonical
+//     population (i, x) sits in slot i at x - c_i), and every further step is PULL2: read slot i at x - c_i,
+//     collide, write slot i at x.  n steps = n kernels; the last stream is done by whoever reads the state.
+//   AA is in place: the even step reads slot i at x and writes slot opp(i) at x (GATHER_AA_ODD: canonical
+//     (i, x) sits in slot opp(i) at x - c_i), the odd step reads that and writes slot i at x + c_i, which is
+//     canonical again.
 #pragma once
 #include "systems.cuh"
 
 namespace lbmk {
 
-enum { MODE_PULL2 = 0, MODE_AA_EVEN = 1, MODE_AA_ODD = 2 };
+enum { MODE_PULL2 = 0, MODE_AA_EVEN = 1, MODE_AA_ODD = 2, MODE_LOCAL = 3 };
+enum { GATHER_CANON = 0, GATHER_AA_ODD = 1, GATHER_PULL = 2 };
 
 template <class Sys> __host__ __device__ constexpr bool has_mms() { return !std::is_void<typename Sys::Mms>::value; }
 
@@ -64,7 +70,7 @@ collide_stream_node(const R* __restrict__ src, R* __restrict__ dst, const __grid
     // gather addresses: element offset of direction i's source relative to `node`
     long long off[Q];
 #pragma unroll
-    for (int i = 0; i < Q; ++i) off[i] = (MODE == MODE_AA_EVEN) ? 0LL : pull_offset(i, p, P.nx, P.ny, P.nz);
+    for (int i = 0; i < Q; ++i) off[i] = (MODE == MODE_AA_EVEN || MODE == MODE_LOCAL) ? 0LL : pull_offset(i, p, P.nx, P.ny, P.nz);
 
     R f[M][Q];
 #pragma unroll
@@ -95,7 +101,7 @@ collide_stream_node(const R* __restrict__ src, R* __restrict__ dst, const __grid
         relax<D, R>(f[k], P.omega[k], dQ[k], F, S);
 #pragma unroll
         for (int i = 0; i < Q; ++i) {
-            if constexpr (MODE == MODE_PULL2) {
+            if constexpr (MODE == MODE_PULL2 || MODE == MODE_LOCAL) {
                 dst[(long long)(k * Q + i) * P.n + node] = f[k][i];
             } else if constexpr (MODE == MODE_AA_EVEN) {
                 dst[(long long)(k * Q + opposite(i)) * P.n + node] = f[k][i];
@@ -161,33 +167,34 @@ __global__ void reference_equilibrium_kernel(double* __restrict__ feq0, const __
 }
 
 // ------------------------------------------------------------------------------------------------ readback
-// canonical gather: population (k, i) of `node` sits in slot i at node (canonical storage) or, after an odd
-// number of AA steps, in slot opp(i) at node - c_i.
+// canonical gather: population (k, i) of `node` sits in slot i at node (GATHER_CANON), in slot opp(i) at
+// node - c_i (GATHER_AA_ODD) or in slot i at node - c_i (GATHER_PULL).
 template <int Q, class R>
 __device__ __forceinline__ R load_canonical(const R* __restrict__ f, long long n, int k, int i, long long node,
-                                            const NodeIdx& p, int nx, int ny, int nz, bool aa_odd) {
-    if (!aa_odd) return f[(long long)(k * Q + i) * n + node];
-    return f[(long long)(k * Q + opposite(i)) * n + node + pull_offset(i, p, nx, ny, nz)];
+                                            const NodeIdx& p, int nx, int ny, int nz, int gather) {
+    if (gather == GATHER_CANON) return f[(long long)(k * Q + i) * n + node];
+    const int slot = gather == GATHER_AA_ODD ? opposite(i) : i;
+    return f[(long long)(k * Q + slot) * n + node + pull_offset(i, p, nx, ny, nz)];
 }
 
 // U_k = Q0_k + sum_i f*_k,i, accumulated and returned in fp64 (eq 2.6; reading A17)
 template <int Q, class R>
 __global__ void read_U_kernel(const R* __restrict__ f, double* __restrict__ U, int M, int nx, int ny, int nz, long long n,
-                              bool aa_odd, const __grid_constant__ KParams<double> Pd) {
+                              int gather, const __grid_constant__ KParams<double> Pd) {
     const long long node = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (node >= n) return;
     const NodeIdx p = decompose(node, nx, ny);
     for (int k = 0; k < M; ++k) {
         double s = 0.0;
 #pragma unroll
-        for (int i = 0; i < Q; ++i) s += (double)load_canonical<Q, R>(f, n, k, i, node, p, nx, ny, nz, aa_odd);
+        for (int i = 0; i < Q; ++i) s += (double)load_canonical<Q, R>(f, n, k, i, node, p, nx, ny, nz, gather);
         U[(long long)k * n + node] = Pd.ref[k] + s;
     }
 }
 
 template <int Q, class R>
 __global__ void read_f_kernel(const R* __restrict__ f, double* __restrict__ out, const double* __restrict__ feq0, int M,
-                              int nx, int ny, int nz, long long n, bool aa_odd) {
+                              int nx, int ny, int nz, long long n, int gather) {
     const long long node = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (node >= n) return;
     const NodeIdx p = decompose(node, nx, ny);
@@ -195,7 +202,7 @@ __global__ void read_f_kernel(const R* __restrict__ f, double* __restrict__ out,
 #pragma unroll
         for (int i = 0; i < Q; ++i)
             out[(long long)(k * Q + i) * n + node] =
-                (double)load_canonical<Q, R>(f, n, k, i, node, p, nx, ny, nz, aa_odd) + feq0[k * Q + i];
+                (double)load_canonical<Q, R>(f, n, k, i, node, p, nx, ny, nz, gather) + feq0[k * Q + i];
 }
 
 template <class R>
@@ -218,7 +225,7 @@ __device__ __forceinline__ double warp_max(double v) {
 template <class Sys, class R>
 __global__ void __launch_bounds__(256)
 max_wave_speed_kernel(const R* __restrict__ f, unsigned long long* __restrict__ out3, long long n, int nx, int ny, int nz,
-                      bool aa_odd, const __grid_constant__ KParams<double> Pd) {
+                      int gather, const __grid_constant__ KParams<double> Pd) {
     constexpr int Q = 2 * Sys::D + 1, M = Sys::M;
     double m[3] = {0.0, 0.0, 0.0};
     for (long long node = (long long)blockIdx.x * blockDim.x + threadIdx.x; node < n; node += (long long)gridDim.x * blockDim.x) {
@@ -227,7 +234,7 @@ max_wave_speed_kernel(const R* __restrict__ f, unsigned long long* __restrict__ 
         for (int k = 0; k < M; ++k) {
             double s = 0.0;
 #pragma unroll
-            for (int i = 0; i < Q; ++i) s += (double)load_canonical<Q, R>(f, n, k, i, node, p, nx, ny, nz, aa_odd);
+            for (int i = 0; i < Q; ++i) s += (double)load_canonical<Q, R>(f, n, k, i, node, p, nx, ny, nz, gather);
             U[k] = Pd.ref[k] + s;
         }
         Sys::wave(U, Pd, w);
@@ -256,9 +263,10 @@ max_wave_speed_kernel(const R* __restrict__ f, unsigned long long* __restrict__ 
 // ------------------------------------------------------------------------------------------------ a11
 // Dirichlet-MMS frame (reading A18; the paper defines no boundary operator):
 // the outermost node layer is reset to f_eq(Q_exact(x_b, t_n)) in canonical slots.  One thread per frame
-// node candidate; P.T holds the time scalars at t_n (not the midpoint).  Only launched on canonical storage.
+// node candidate; P.T holds the time scalars at t_n (not the midpoint).  Two-lattice storage only: with the
+// stream pending (GATHER_PULL) the canonical population (i, x_b) is written where the next pull finds it.
 template <class Sys, class R>
-__global__ void dirichlet_frame_kernel(R* __restrict__ f, const __grid_constant__ KParams<R> P, const __grid_constant__ KParams<double> Pd) {
+__global__ void dirichlet_frame_kernel(R* __restrict__ f, int gather, const __grid_constant__ KParams<R> P, const __grid_constant__ KParams<double> Pd) {
     if constexpr (has_mms<Sys>()) {
         constexpr int D = Sys::D, Q = 2 * D + 1, M = Sys::M;
         using G = typename Sys::Mms;
@@ -285,8 +293,10 @@ __global__ void dirichlet_frame_kernel(R* __restrict__ f, const __grid_constant_
             f[(long long)(k * Q) * P.n + node] = R(L::w0) * dQ[k];
             for (int a = 0; a < D; ++a) {
                 const R h = R(0.5) * F[a];
-                f[(long long)(k * Q + 1 + 2 * a) * P.n + node] = R(L::w1) * dQ[k] + h;
-                f[(long long)(k * Q + 2 + 2 * a) * P.n + node] = R(L::w1) * dQ[k] - h;
+                const long long op = gather == GATHER_PULL ? pull_offset(1 + 2 * a, p, P.nx, P.ny, P.nz) : 0LL;
+                const long long om = gather == GATHER_PULL ? pull_offset(2 + 2 * a, p, P.nx, P.ny, P.nz) : 0LL;
+                f[(long long)(k * Q + 1 + 2 * a) * P.n + node + op] = R(L::w1) * dQ[k] + h;
+                f[(long long)(k * Q + 2 + 2 * a) * P.n + node + om] = R(L::w1) * dQ[k] - h;
             }
         });
     }

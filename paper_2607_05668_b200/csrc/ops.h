@@ -21,6 +21,7 @@ struct GridCore {
     cudaStream_t stream;
     void* f[2];           // population buffers; f[1] == nullptr for the in-place AA pattern
     int cur;              // PULL2: which buffer holds the current state
+    int pending;          // PULL2: storage is post-collision, the stream is pending (kernels.cuh GATHER_PULL)
     long long step;       // completed steps
     double t0, dt;
     void* tab[3];         // per-axis trig tables in R, [entry][index]

@@ -78,6 +78,7 @@ struct Ops {
         init_from_U_kernel<S<R>, R><<<blocks_for(g.n, 256), 256, 0, g.stream>>>(U, (R*)g.f[0], kp<R>(g), g.Pd);
         g.launches++;
         g.cur = 0;
+        g.pending = 0;
         return cudaGetLastError();
     }
     static cudaError_t init_from_U(GridCore& g, const double* U) { return g.prec == PREC_F64 ? init_t<double>(g, U) : init_t<float>(g, U); }
@@ -87,11 +88,16 @@ struct Ops {
         set_f_kernel<R><<<blocks_for(g.n, 256), 256, 0, g.stream>>>(f, (R*)g.f[0], g.feq0, M * Q, g.n);
         g.launches++;
         g.cur = 0;
+        g.pending = 0;
         return cudaGetLastError();
     }
     static cudaError_t set_f(GridCore& g, const double* f) { return g.prec == PREC_F64 ? set_f_t<double>(g, f) : set_f_t<float>(g, f); }
 
-    static bool aa_odd(const GridCore& g) { return g.pattern == PATTERN_AA && (g.step & 1); }
+    // where the canonical population sits in the current storage (kernels.cuh GATHER_*)
+    static int aa_odd(const GridCore& g) {
+        if (g.pattern == PATTERN_AA) return (g.step & 1) ? GATHER_AA_ODD : GATHER_CANON;
+        return g.pending ? GATHER_PULL : GATHER_CANON;
+    }
 
     template <class R>
     static cudaError_t read_U_t(GridCore& g, double* U) {
@@ -142,14 +148,16 @@ struct Ops {
             if (g.bc == 1) {
                 if constexpr (HAS_MMS) {
                     time_scalars(g, t_n);
-                    dirichlet_frame_kernel<S<R>, R><<<blocks_for(g.n, 256), 256, 0, g.stream>>>((R*)g.f[g.cur], kp<R>(g), g.Pd);
+                    dirichlet_frame_kernel<S<R>, R><<<blocks_for(g.n, 256), 256, 0, g.stream>>>((R*)g.f[g.cur], aa_odd(g), kp<R>(g), g.Pd);
                     g.launches++;
                 }
             }
             if constexpr (MMS) time_scalars(g, t_n + 0.5 * g.dt);           // explicit forcing at the temporal midpoint, L154
             if (g.pattern == PATTERN_PULL2) {
-                launch_node<R, MODE_PULL2, MMS>(g, (const R*)g.f[g.cur], (R*)g.f[g.cur ^ 1]);
+                if (g.pending) launch_node<R, MODE_PULL2, MMS>(g, (const R*)g.f[g.cur], (R*)g.f[g.cur ^ 1]);
+                else launch_node<R, MODE_LOCAL, MMS>(g, (const R*)g.f[g.cur], (R*)g.f[g.cur ^ 1]);
                 g.cur ^= 1;
+                g.pending = 1;
             } else if ((g.step & 1) == 0) {
                 launch_node<R, MODE_AA_EVEN, MMS>(g, (const R*)g.f[0], (R*)g.f[0]);
             } else {
@@ -171,8 +179,8 @@ struct Ops {
         if constexpr (HAS_MMS) {
             if (g.bc == 1) {
                 time_scalars(g, g.t0 + (double)g.step * g.dt);
-                if (g.prec == PREC_F64) dirichlet_frame_kernel<S<double>, double><<<blocks_for(g.n, 256), 256, 0, g.stream>>>((double*)g.f[g.cur], g.Pd, g.Pd);
-                else dirichlet_frame_kernel<S<float>, float><<<blocks_for(g.n, 256), 256, 0, g.stream>>>((float*)g.f[g.cur], g.Pf, g.Pd);
+                if (g.prec == PREC_F64) dirichlet_frame_kernel<S<double>, double><<<blocks_for(g.n, 256), 256, 0, g.stream>>>((double*)g.f[g.cur], aa_odd(g), g.Pd, g.Pd);
+                else dirichlet_frame_kernel<S<float>, float><<<blocks_for(g.n, 256), 256, 0, g.stream>>>((float*)g.f[g.cur], aa_odd(g), g.Pf, g.Pd);
                 g.launches++;
             }
         }

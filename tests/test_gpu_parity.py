@@ -24,14 +24,7 @@ def P():
     return P
 
 
-def rel_err(U, Uo):
-    """per component max|dU| / max|U_oracle| (A16); identically-zero components use the system scale."""
-    scale_sys = max(np.abs(Uo).max(), 1e-300)
-    out = []
-    for k in range(U.shape[0]):
-        s = np.abs(Uo[k]).max()
-        out.append(np.abs(U[k] - Uo[k]).max() / (s if s > 1e-12 * scale_sys else scale_sys))
-    return np.array(out)
+from parity_metric import rel_err, plain_rel_err, fluct_rel_err   # noqa: E402  (reading A16)
 
 
 def small(name, **kw):
@@ -111,7 +104,7 @@ def test_parity_fp64(P, name, kw, steps, pattern):
     w = small(name, **kw)
     U, f, Uo, fo = run_pair(P, w, steps, precision="f64", pattern=pattern)
     assert np.isfinite(U).all()
-    e = rel_err(U, Uo)
+    e = rel_err(U, Uo, fo)
     assert e.max() <= TOL64, f"{w.name} U rel err {e}"
     ef = np.abs(f - fo).max() / np.abs(fo).max()
     assert ef <= TOL64, f"{w.name} populations rel err {ef}"
@@ -122,7 +115,7 @@ def test_parity_fp64_paper_systems_with_mms(P, mk, n, steps):
     """The three Table-2 systems (Burgers L518, Euler L519-L522, ADR L540) with their manufactured forcing."""
     w = mk(n)
     U, f, Uo, fo = run_pair(P, w, steps, precision="f64")
-    e = rel_err(U, Uo)
+    e = rel_err(U, Uo, fo)
     assert e.max() <= TOL64, f"{w.name} {e}"
 
 
@@ -132,7 +125,7 @@ def test_shifted_fp64_matches_unshifted_oracle(P, name, kw, steps):
     """eq (2.23) is an identity: the delta-form kernels in fp64 reproduce the plain fp64 oracle (pin P7 on the GPU)."""
     w = small(name, **kw)
     U, f, Uo, fo = run_pair(P, w, steps, precision="f64s")
-    e = rel_err(U, Uo)
+    e = rel_err(U, Uo, fo)
     assert e.max() <= 1e-11, f"{w.name} {e}"
     assert np.abs(f - fo).max() / np.abs(fo).max() <= 1e-11
 
@@ -141,7 +134,7 @@ def test_shifted_fp64_general_reference_momentum(P):
     """Euler with a moving reference state u0 = v0 = 3 (the paper's SM5.3 fields): general delta form."""
     w = W.pin_euler(40)
     U, f, Uo, fo = run_pair(P, w, 120, precision="f64s")
-    assert rel_err(U, Uo).max() <= 1e-11
+    assert rel_err(U, Uo, fo).max() <= 1e-11
 
 
 # ------------------------------------------------------------------------------------------- shifted fp32
@@ -161,12 +154,11 @@ def test_parity_fp32_shifted(P, name, kw, steps, pattern):
     assert w.precision == "f32s"
     U, f, Uo, fo = run_pair(P, w, steps, pattern=pattern)
     assert np.isfinite(U).all()
-    e = rel_err(U, Uo)
+    e = rel_err(U, Uo, fo)
     assert e.max() <= TOL32, f"{w.name} U rel err {e}"
     # stricter, reported figure: relative to the fluctuation about the reference state (A16)
-    ref = np.asarray(w.U_ref).reshape(-1, 1, 1, 1)
-    fl = np.array([np.abs(U[k] - Uo[k]).max() / max(np.abs(Uo[k] - ref[k]).max(), 1e-30) for k in range(U.shape[0])])
-    print(f"{w.name} [{pattern}] rel err max {e.max():.2e}; fluctuation-relative max {fl.max():.2e}")
+    fl, pl = fluct_rel_err(U, Uo, w.U_ref), plain_rel_err(U, Uo)
+    print(f"{w.name} [{pattern}] rel err max {e.max():.2e}; vs max|U_k| {pl.max():.2e}; fluctuation-relative {fl.max():.2e}")
 
 
 def test_fp32_uniform_reference_state_stays_exactly_zero(P):
@@ -197,12 +189,12 @@ def _subbox_check(P, w, steps, box, origin, tol):
     o = oracle.OracleGrid.from_workload(w, nx=bx, ny=by, nz=bz, origin=(ox, oy, oz))
     o.init_from_U(np.ascontiguousarray(U0[sl]))
     o.step(steps)
-    Uo = o.read_U()
+    Uo, fo = o.read_U(), o.read_f()
     o.close()
     m = steps
     inner = (slice(None), slice(m, bz - m) if w.dim == 3 else slice(None), slice(m, by - m), slice(m, bx - m))
     Ug = U[sl][inner]
-    e = rel_err(Ug, Uo[inner])
+    e = rel_err(Ug, Uo[inner], fo[(slice(None), slice(None)) + inner[1:]])
     assert Ug.size > 0 and e.max() <= tol, f"{w.name}: {e}"
     return U
 
