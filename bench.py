@@ -1,0 +1,415 @@
+#!/usr/bin/env python
+"""bench.py -- MLUPS and achieved HBM GB/s of the fused collide-and-stream step on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config c4] [--impl ours|reference]
+
+A "step" is one collide-and-stream pass (eq 2.11; all rows a1-a7 of SURVEY.md §8(a)) over
+the whole grid of the workload.  Default workload: BASELINE.json configs[3] ("c4": 3D compressible NSF with the
+gradient-tracking cascade, 17 components, D3Q7, 256^3 periodic, shifted fp32, manufactured forcing on) -- the
+larger of the two "3D fp32 configs" BASELINE.json's target is quoted on; it fits one GPU (8 GB per population
+copy).  Inputs are the seeded synthetic fields of workloads/ (DESIGN.md "Input recipe").
+
+One JSON line is printed by rank 0:
+  value       MLUPS over all ranks, populations resident in HBM when the timed region starts
+  e2e         the same metric through the public API with HOST buffers: lbmk_init_from_U(host U) -> K steps ->
+              lbmk_read_U(host U), copies inside the timed region
+  roofline    dominant kernel (collide_stream_*): algorithmic bytes 2*Q*m_total*sizeof per node (the byte model
+              of the paper's Table 3) / CUDA-event time per launch, against the measured
+              copy bandwidth in MEASURED_PEAKS.json
+  cpu_baseline  the CPU oracle (oracle/, plain fp64 C++) timed on this box's host cores on a bounded sample
+  all_configs   short runs of the other BASELINE.json configs (reported, not the headline)
+
+Multi-GPU (--gpus N under torchrun): "replicas only" -- every rank advances its own
+full-size grid, no data-path collective; value = sum over ranks / max-over-ranks time; scaling "weak".
+
+`--impl reference` times the oracle as it stands on host cores (rank 0 only): each step is one oracle step on a
+bounded sub-box of the same workload (same node spacing and parameters), sized so the run ends within minutes.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "MLUPS (million lattice-node updates per second) of the fused collide-and-stream step"
+UNIT = "MLUPS"
+
+# dram__bytes_read.sum + dram__bytes_write.sum per collide_stream launch from the committed `ncu --set full`
+# captures (profiles/), keyed by (config, pattern); None = not captured for this launch configuration.
+NCU_TRAFFIC_BYTES = {}
+try:
+    with open(os.path.join(ROOT, "profiles", "traffic_per_launch.json")) as _fh:
+        NCU_TRAFFIC_BYTES = json.load(_fh)
+except Exception:
+    NCU_TRAFFIC_BYTES = {}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None, help="timed LBM steps (default: the config's step count, capped at 200)")
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="c4", choices=["c1", "c2", "c3", "c4", "c5"])
+    ap.add_argument("--pattern", default="auto", choices=["auto", "pull2", "aa"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "node", "row"])
+    ap.add_argument("--n", type=int, default=None, help="override the grid edge (debug; the line then says so)")
+    ap.add_argument("--no-mms", action="store_true", help="c4 without manufactured forcing (the paper's Table 3 kernels carry none)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-all-configs", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def make_workload(name, n=None, mms=True):
+    import workloads as W
+    kw = {}
+    if n is not None:
+        kw["n"] = n
+    if name == "c4" and not mms:
+        kw["mms"] = False
+    return W.BASELINE_CONFIGS[name](**kw)
+
+
+def measured_peak():
+    """(GB/s, source) -- MEASURED_PEAKS.json (driver-written) else the profiling guide's fallback."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (torch copy, read+write bytes)"
+    except Exception:
+        return 6650.0, "fallback 6.65 TB/s (B200_PROFILING.md; MEASURED_PEAKS.json absent)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index = index
+        self.lines = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.lines.append((time.perf_counter(), ln.strip()))
+
+    def stop(self, t0=None, t1=None):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        time.sleep(0.06)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, smax, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        rows = [ln for (t, ln) in self.lines if (t0 is None or t >= t0) and (t1 is None or t <= t1 + 0.06)] or [ln for _, ln in self.lines]
+        for ln in rows:
+            p = [x.strip() for x in ln.split(",")]
+            if len(p) < 7:
+                continue
+            try:
+                sm.append(float(p[0])); smax.append(float(p[1])); pw.append(float(p[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, p[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(pw) if pw else None, "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def dist_setup(n_gpus):
+    """(rank, world, dist or None).  One process per GPU under torchrun; N = 1 needs no process group."""
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    if world == 1:
+        return 0, 1, None
+    import torch
+    import torch.distributed as dist
+    os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+    backend = "nccl" if torch.cuda.is_available() else "gloo"
+    if backend == "nccl":
+        torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    dist.init_process_group(backend=backend)
+    return rank, world, dist
+
+
+def aggregate(dist, local_ms, local_node_updates, device="cpu"):
+    """replicas-only aggregation: (max over ranks of the time, sum over ranks of the node updates)."""
+    if dist is None:
+        return local_ms, local_node_updates
+    import torch
+    t = torch.tensor([local_ms], dtype=torch.float64, device=device)
+    u = torch.tensor([float(local_node_updates)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+def time_steps(g, torch, steps, dist=None):
+    """CUDA-event time (ms) of exactly `steps` steps on the grid's stream, barrier + synchronize on both sides."""
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = g.launch_count()
+    e0.record()
+    g.step(steps)
+    e1.record()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    return e0.elapsed_time(e1), g.launch_count() - l0
+
+
+def short_run(P, torch, name, pattern):
+    """MLUPS / GB/s of one of the other configs (its full step count, 5% warm-up)."""
+    w = make_workload(name)
+    g = P.Grid.from_workload(w, pattern=pattern)
+    g.init_from_U(torch.from_numpy(w.initial_U()).cuda())
+    g.step(max(10, w.steps // 20))
+    reps = []
+    for _ in range(3):
+        ms, _ = time_steps(g, torch, w.steps)
+        reps.append(ms)
+    ms = min(reps)
+    mlups = w.n_nodes * w.steps / (ms * 1e-3) / 1e6
+    out = {"workload": w.name, "dtype": "f64" if w.precision == "f64" else "f32", "pattern": g.pattern, "steps": w.steps,
+           "ms_per_step": ms / w.steps, "MLUPS": mlups, "GBps_algorithmic": mlups * w.bytes_per_node / 1e3,
+           "state_MB": w.n_nodes * w.bytes_per_node / 2 / 1e6}
+    g.close()
+    return out
+
+
+def cpu_baseline(w, budget_s=15.0):
+    """The oracle as it stands on host cores, on a bounded sub-box of workload w (same dx, lambda, parameters)."""
+    import numpy as np
+    import oracle
+    U0 = w.initial_U()
+    # calibration box -> rate -> sample box
+    def box(nz, ny):
+        return (min(w.nz, nz) if w.dim == 3 else 1, min(w.ny, ny), w.nx)
+
+    def run(bz, by, bx, steps):
+        o = oracle.OracleGrid.from_workload(w, nx=bx, ny=by, nz=bz)
+        o.init_from_U(np.ascontiguousarray(U0[:, :bz, :by, :bx]))
+        o.step(1)
+        t = time.perf_counter()
+        o.step(steps)
+        dt = time.perf_counter() - t
+        o.close()
+        return bz * by * bx * steps / dt / 1e6, dt
+
+    bz, by, bx = box(4, 64)
+    rate, _ = run(bz, by, bx, 2)
+    target_updates = rate * 1e6 * budget_s
+    steps = 8
+    plane = w.nx * w.ny
+    if w.dim == 3:
+        bz = int(max(4, min(w.nz, target_updates / steps / plane)))
+        by = w.ny
+    else:
+        bz, by = 1, int(max(8, min(w.ny, target_updates / steps / w.nx)))
+        steps = int(max(8, min(w.steps, target_updates / (by * w.nx))))
+    mlups, dt = run(bz, by, w.nx, steps)
+    return {"value": mlups, "unit": UNIT, "cores": oracle.n_threads(), "kind": "oracle",
+            "sample": f"{steps} steps (after 1 warm-up) on a periodic {w.nx}x{by}x{bz} sub-box of {w.name} "
+                      f"(same dx, lambda, parameters, forcing); {dt:.1f} s wall"}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import numpy as np
+    import oracle
+    w = make_workload(args.config, args.n, not args.no_mms)
+    steps = args.steps if args.steps is not None else min(w.steps, 200)
+    warm = args.warmup
+    U0 = w.initial_U()
+    # calibrate on a tiny box, then size the sample so (steps + warm) oracle steps take about two minutes
+    cz, cy = (4 if w.dim == 3 else 1), min(w.ny, 64)
+    o = oracle.OracleGrid.from_workload(w, nx=w.nx, ny=cy, nz=cz)
+    o.init_from_U(np.ascontiguousarray(U0[:, :cz, :cy, :]))
+    o.step(1)
+    t = time.perf_counter(); o.step(2); rate = cz * cy * w.nx * 2 / (time.perf_counter() - t)
+    o.close()
+    per_step = rate * 120.0 / (steps + warm)
+    if w.dim == 3:
+        by = w.ny
+        bz = int(max(2, min(w.nz, per_step / (w.nx * w.ny))))
+        if bz == 2:
+            by = int(max(8, min(w.ny, per_step / (w.nx * bz))))
+    else:
+        bz, by = 1, int(max(8, min(w.ny, per_step / w.nx)))
+    o = oracle.OracleGrid.from_workload(w, nx=w.nx, ny=by, nz=bz)
+    o.init_from_U(np.ascontiguousarray(U0[:, :bz, :by, :]))
+    o.step(warm)
+    t = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t
+    o.close()
+    nodes = bz * by * w.nx
+    mlups = nodes * steps / dt / 1e6
+    sample = f"each step = one oracle step on a periodic {w.nx}x{by}x{bz} sub-box of {w.name} (same dx, lambda, parameters, forcing)"
+    line = {"impl": "reference", "metric": METRIC, "value": mlups, "unit": UNIT, "n_gpus": args.gpus, "steps": steps, "warmup": warm,
+            "ms_per_step": dt * 1e3 / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": w.name, "system": w.system, "lattice": w.lattice, "m_total": w.m_total,
+                                            "grid": [w.nx, w.ny, w.nz], "sample_grid": [w.nx, by, bz], "note": sample},
+            "cpu_baseline": {"value": mlups, "unit": UNIT, "cores": oracle.n_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": mlups, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the collide-and-stream path has no CPU fallback "
+                         "(use --impl reference for the CPU oracle)")
+    rank, world, dist = dist_setup(args.gpus)
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    import paper_2607_05668_b200 as P
+    P.lib()
+
+    w = make_workload(args.config, args.n, not args.no_mms)
+    steps = args.steps if args.steps is not None else min(w.steps, 200)
+    warm = max(args.warmup, 3)
+    dev = f"cuda:{local}"
+    U0 = w.initial_U()
+    g = P.Grid.from_workload(w, pattern=args.pattern, kernel=args.kernel, device=dev)
+    U0_dev = torch.from_numpy(U0).to(dev)
+    g.init_from_U(U0_dev)
+    speeds, status = g.max_wave_speed()                      # a10: device sub-characteristic check (untimed)
+    g.step(warm)
+    sampler = ClockSampler(local).start() if rank == 0 else None
+    # keep the sampler busy for a while before the timed region so that it has samples
+    t_wall0 = time.perf_counter()
+    reps = []
+    n_rep = 3
+    launches = 0
+    for _ in range(n_rep):
+        ms, launches = time_steps(g, torch, steps, dist)
+        reps.append(ms)
+    t_wall1 = time.perf_counter()
+    clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
+    ms_local = statistics.median(reps)
+    ms, updates = aggregate(dist, ms_local, w.n_nodes * steps, dev)
+    mlups = updates / (ms * 1e-3) / 1e6
+    finite = bool(np.isfinite(g.read_U(torch.empty(g.shape_U, dtype=torch.float64, device=dev)).sum().item()))
+
+    # e2e through the public API with host buffers (pinned), copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        U_host = torch.from_numpy(U0).pin_memory()
+        out_host = torch.empty(g.shape_U, dtype=torch.float64).pin_memory()
+        g.init_from_U(U_host); g.step(2); g.read_U(out_host)      # warm the staging pool
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        tw = time.perf_counter()
+        e0.record()
+        g.init_from_U(U_host)
+        g.step(steps)
+        g.read_U(out_host)
+        e1.record()
+        torch.cuda.synchronize()
+        wall_ms = (time.perf_counter() - tw) * 1e3
+        e_ms = max(e0.elapsed_time(e1), wall_ms)
+        e_ms, e_upd = aggregate(dist, e_ms, w.n_nodes * steps, dev)
+        nbytes = U_host.numel() * 8
+        e2e = {"value": e_upd / (e_ms * 1e-3) / 1e6, "unit": UNIT, "h2d_bytes_per_step": nbytes / steps,
+               "d2h_bytes_per_step": nbytes / steps, "ms_total": e_ms,
+               "what": f"lbmk_init_from_U(pinned host U, {nbytes / 1e6:.0f} MB) -> {steps} steps -> lbmk_read_U(pinned host)"}
+        del U_host, out_host
+    pattern, kernel = g.pattern, g.kernel
+    g.close()
+    del g, U0_dev
+    torch.cuda.empty_cache()
+
+    if rank != 0:
+        if dist is not None:
+            dist.barrier()
+            dist.destroy_process_group()
+        return 0
+
+    peak, peak_src = measured_peak()
+    bytes_per_launch = w.n_nodes * w.bytes_per_node
+    ms_launch = ms_local / steps
+    achieved = bytes_per_launch / (ms_launch * 1e-3) / 1e9
+    traffic = NCU_TRAFFIC_BYTES.get(f"{args.config}:{pattern}:{kernel}")
+    line = {
+        "metric": METRIC, "value": mlups, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warm,
+        "ms_per_step": ms / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64" if w.precision == "f64" else "f32", "data": "synthetic",
+        "config": {"workload": w.name, "system": w.system, "lattice": w.lattice, "m_conserved": None, "m_total": w.m_total,
+                   "grid": [w.nx, w.ny, w.nz], "precision": w.precision, "mms_forcing": bool(w.mms_id),
+                   "pattern": pattern, "kernel": kernel, "bytes_per_node": w.bytes_per_node,
+                   "l2": "state larger than L2 (no flush needed)" if bytes_per_launch / 2 > 2.5e8 else "state fits in L2: HBM roofline n/a",
+                   "parallelism": "replicas only" if world > 1 else "single GPU", "timing": f"median of {n_rep} x {steps} steps, CUDA events",
+                   "lattice_wave_speed": max(speeds[0], speeds[1]) + speeds[2], "finite": finite},
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": traffic, "peak_source": peak_src, "frac_of_nominal_8TBps": achieved / 8000.0,
+                     "kernel": "collide_stream (one launch per step)", "algorithmic_bytes_per_launch": bytes_per_launch},
+        "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+    }
+    line["config"].pop("m_conserved")
+    if not args.no_cpu_baseline and world == 1:
+        line["cpu_baseline"] = cpu_baseline(w)
+    if not args.no_all_configs and world == 1:
+        others = {}
+        for name in ("c1", "c2", "c3", "c4", "c5"):
+            if name == args.config:
+                continue
+            try:
+                r = short_run(P, torch, name, args.pattern)
+                r["frac_of_measured_peak"] = r["GBps_algorithmic"] / peak
+                others[name] = r
+            except Exception as e:   # reported, never hidden
+                others[name] = {"error": repr(e)}
+            torch.cuda.empty_cache()
+        line["all_configs"] = others
+    print(json.dumps(line))
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
