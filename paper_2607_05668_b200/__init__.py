@@ -31,11 +31,11 @@ LBMK_F64, LBMK_F32_SHIFTED, LBMK_F64_SHIFTED = 0, 1, 2
 LBMK_PERIODIC, LBMK_DIRICHLET_MMS = 0, 1
 LBMK_OPT_PATTERN, LBMK_OPT_KERNEL = 0, 1
 LBMK_PATTERN_AUTO, LBMK_PATTERN_PULL2, LBMK_PATTERN_AA = 0, 1, 2
-LBMK_KERNEL_AUTO, LBMK_KERNEL_NODE, LBMK_KERNEL_ROW = 0, 1, 2
+LBMK_KERNEL_AUTO, LBMK_KERNEL_NODE, LBMK_KERNEL_ROW, LBMK_KERNEL_TWOPASS = 0, 1, 2, 3
 SYSTEM_ID = {"advection2d": 0, "burgers2d": 1, "swe2d": 2, "euler2d": 3, "adr2d": 4, "nsf3d": 5, "mhd3d": 6}
 PRECISION = {"f64": LBMK_F64, "f32s": LBMK_F32_SHIFTED, "f64s": LBMK_F64_SHIFTED}
 PATTERN = {"auto": 0, "pull2": 1, "aa": 2}
-KERNEL = {"auto": 0, "node": 1, "row": 2}
+KERNEL = {"auto": 0, "node": 1, "row": 2, "twopass": 3}
 
 # every symbol include/lbmk.h declares: (restype, argtypes)
 _dp = C.POINTER(C.c_double)
@@ -317,7 +317,7 @@ class Grid:
         self.workspace = torch.empty(self.workspace_bytes, dtype=torch.uint8, device=self.device)
         lbmk_grid_bind_workspace(self.h, self.workspace.data_ptr(), self.workspace_bytes)
         self.pattern = {1: "pull2", 2: "aa"}[lbmk_grid_get_option(self.h, LBMK_OPT_PATTERN)]
-        self.kernel = {1: "node", 2: "row"}[lbmk_grid_get_option(self.h, LBMK_OPT_KERNEL)]
+        self.kernel = {1: "node", 2: "row", 3: "twopass"}[lbmk_grid_get_option(self.h, LBMK_OPT_KERNEL)]
 
     @classmethod
     def from_workload(cls, w, precision: Optional[str] = None, omega=None, declare_bound: bool = True, **kw):

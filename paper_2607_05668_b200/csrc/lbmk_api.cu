@@ -267,6 +267,7 @@ lbmk_status lbmk_grid_create(const lbmk_system* sys, int nx, int ny, int nz, lbm
     const SysOps* o = ops_of(sys->id);
     if (nx < 1 || ny < 1 || nz < 1) return sys_fail(LBMK_EINVAL, "grid sizes must be >= 1");
     if (o->D == 2 && nz != 1) return sys_fail(LBMK_EINVAL, "nz must be 1 for a 2D system");
+    if ((long long)nx * ny * nz > 0x7fffffffLL) return sys_fail(LBMK_EINVAL, "grid too large: nx*ny*nz must be < 2^31 nodes");
     if (!(dx > 0.0) || !(lambda > 0.0)) return sys_fail(LBMK_EINVAL, "dx and lambda must be > 0");
     if (bc != LBMK_PERIODIC && bc != LBMK_DIRICHLET_MMS) return sys_fail(LBMK_EINVAL, "unknown boundary condition");
     if (precision != LBMK_F64 && precision != LBMK_F32_SHIFTED && precision != LBMK_F64_SHIFTED) return sys_fail(LBMK_EINVAL, "unknown precision");
@@ -310,7 +311,7 @@ lbmk_status lbmk_grid_set_option(lbmk_grid* g, lbmk_option key, long long value)
         if (value < LBMK_PATTERN_AUTO || value > LBMK_PATTERN_AA) return fail(g, LBMK_EINVAL, "unknown pattern");
         g->opt_pattern = value;
     } else if (key == LBMK_OPT_KERNEL) {
-        if (value < LBMK_KERNEL_AUTO || value > LBMK_KERNEL_ROW) return fail(g, LBMK_EINVAL, "unknown kernel variant");
+        if (value < LBMK_KERNEL_AUTO || value > LBMK_KERNEL_TWOPASS) return fail(g, LBMK_EINVAL, "unknown kernel variant");
         g->opt_kernel = value;
     } else {
         return fail(g, LBMK_EINVAL, "unknown option");

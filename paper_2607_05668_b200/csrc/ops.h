@@ -9,7 +9,7 @@ namespace lbmk {
 
 enum { PREC_F64 = 0, PREC_F32 = 1 };
 enum { PATTERN_PULL2 = 1, PATTERN_AA = 2 };
-enum { KERNEL_NODE = 1, KERNEL_ROW = 2 };
+enum { KERNEL_NODE = 1, KERNEL_ROW = 2, KERNEL_TWOPASS = 3 };
 
 struct GridCore {
     int nx, ny, nz;

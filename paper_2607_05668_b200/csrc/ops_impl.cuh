@@ -19,6 +19,11 @@ template <class R> struct Tune<SysNsf3D, R> { static constexpr int BLOCK = 128, 
 template <> struct Tune<SysNsf3D, double> { static constexpr int BLOCK = 128, MINB = 1; };
 template <class R> struct Tune<SysMhd3D, R> { static constexpr int BLOCK = 128, MINB = 2; };
 
+// two-pass kernel: register cap via min blocks per SM
+template <template <class> class S, class R> struct Tune2 { static constexpr int BLOCK = 256, MINB = 2; };
+template <class R> struct Tune2<SysNsf3D, R> { static constexpr int BLOCK = 128, MINB = 4; };
+template <class R> struct Tune2<SysMhd3D, R> { static constexpr int BLOCK = 128, MINB = 4; };
+
 template <class Mm> struct MmsCounts { static constexpr int NT = Mm::NT, NX = Mm::NX, NY = Mm::NY, NZ = Mm::NZ; };
 template <> struct MmsCounts<void> { static constexpr int NT = 0, NX = 0, NY = 0, NZ = 0; };
 
@@ -138,7 +143,12 @@ struct Ops {
     template <class R, int MODE, bool MMS>
     static void launch_node(GridCore& g, const R* src, R* dst) {
         constexpr int BLOCK = Tune<S, R>::BLOCK, MINB = Tune<S, R>::MINB;
-        collide_stream_node<S<R>, R, MODE, MMS, BLOCK, MINB><<<blocks_for(g.n, BLOCK), BLOCK, 0, g.stream>>>(src, dst, kp<R>(g));
+        if (g.kernel == KERNEL_TWOPASS) {
+            constexpr int B2 = Tune2<S, R>::BLOCK, M2 = Tune2<S, R>::MINB;
+            collide_stream_twopass<S<R>, R, MODE, MMS, B2, M2><<<blocks_for(g.n, B2), B2, 0, g.stream>>>(src, dst, kp<R>(g));
+        } else {
+            collide_stream_node<S<R>, R, MODE, MMS, BLOCK, MINB><<<blocks_for(g.n, BLOCK), BLOCK, 0, g.stream>>>(src, dst, kp<R>(g));
+        }
         g.launches++;
     }
     template <class R, bool MMS>
