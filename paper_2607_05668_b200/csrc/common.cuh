@@ -47,6 +47,7 @@ struct KParams {
     const R* tabX;
     const R* tabY;
     const R* tabZ;
+    const R* coef;          // per-row forcing coefficients [nz*ny][Mms::NC], rewritten before every step
 };
 
 struct NodeIdx { int ix, iy, iz; };
@@ -77,6 +78,19 @@ __device__ __forceinline__ long long pull_offset(int i, const NodeIdx& p, int nx
 // Offset to node + c_i (push target): the pull offset of the opposite direction.
 __device__ __forceinline__ long long push_offset(int i, const NodeIdx& p, int nx, int ny, int nz) {
     return pull_offset(opposite(i), p, nx, ny, nz);
+}
+
+// Population storage: tiled structure of arrays.  Nodes are grouped, in linear index order, into tiles of TILE
+// consecutive nodes (x fastest, so a tile is an x-row segment); within a tile the M*Q population planes are
+// stored one after the other, TILE elements each:
+//     element(plane, node) = (node / TILE) * (M*Q*TILE) + plane * TILE + node % TILE .
+// A thread block therefore streams ONE contiguous M*Q*TILE*sizeof(R) chunk per direction (c4: 60 KB) instead
+// of M*Q segments from planes a whole grid apart, and -- the point for the step kernels -- the plane offset
+// is a compile-time constant: every access is [per-direction base pointer + immediate], with no address
+// arithmetic per population.  The last tile is padded (allocation = n_tiles * TILE nodes).
+constexpr int LOG_TILE = 7, TILE = 1 << LOG_TILE;
+__host__ __device__ __forceinline__ long long tile_off(long long node, int MQ) {
+    return (node >> LOG_TILE) * ((long long)MQ << LOG_TILE) + (node & (TILE - 1));
 }
 
 // Compile-time loop

@@ -1,6 +1,7 @@
 // kernels.cuh -- the collide-and-stream step (one node per thread, direct loads) and its service kernels.
 //
-// Population storage: structure of arrays S[(k*Q + i)*n + node], x fastest.
+// Population storage: tiled structure of arrays, element(k*Q + i, node) = tile_off(node) + (k*Q + i)*TILE
+// (common.cuh).
 // Step per node (eq 2.6 / 2.7 / 2.11 of the paper):
 //   gather f_k,i  ->  dQ_k = sum_i f_k,i  ->  dF_k, s_k (systems.cuh; + manufactured forcing at t_n + dt/2)
 //   ->  f' = f - omega_k (f - w_i (dQ_k + c_i.dF_k/c_s^2)) + w_i s_k  ->  scatter.
@@ -26,19 +27,34 @@ enum { GATHER_CANON = 0, GATHER_AA_ODD = 1, GATHER_PULL = 2 };
 
 template <class Sys> __host__ __device__ constexpr bool has_mms() { return !std::is_void<typename Sys::Mms>::value; }
 
-// per-node manufactured forcing from the tables
+// per-node manufactured forcing: the x-table entries of this node and the coefficients of its (y, z) row
+// (mms_generated.cuh source_row; the row table is filled by mms_row_coeffs_kernel before every step)
 template <class Sys, class R>
 __device__ __forceinline__ void mms_node(const KParams<R>& P, const NodeIdx& p, R (&s)[Sys::M]) {
     if constexpr (has_mms<Sys>()) {
         using G = typename Sys::Mms;
-        R X[G::NX > 0 ? G::NX : 1], Y[G::NY > 0 ? G::NY : 1], Z[G::NZ > 0 ? G::NZ : 1];
+        R X[G::NX > 0 ? G::NX : 1];
 #pragma unroll
         for (int e = 0; e < G::NX; ++e) X[e] = __ldg(P.tabX + e * P.nx + p.ix);
-#pragma unroll
-        for (int e = 0; e < G::NY; ++e) Y[e] = __ldg(P.tabY + e * P.ny + p.iy);
-#pragma unroll
-        for (int e = 0; e < G::NZ; ++e) Z[e] = __ldg(P.tabZ + e * P.nz + p.iz);
-        G::template source<R>(P.mms, P.T, X, Y, Z, s);
+        G::template source_row<R>(P.coef + (size_t)(p.iz * P.ny + p.iy) * G::NC, X, s);
+    }
+}
+
+// Row coefficients of the forcing at the time whose scalars are in T: one thread per (y, z) row, fp64 from the
+// closed forms (no tables), stored in R.  ~1e3 flops x ny*nz threads per step: negligible next to the step.
+template <class Sys, class R>
+__global__ void __launch_bounds__(128)
+mms_row_coeffs_kernel(R* __restrict__ coef, int ny, int nz, const __grid_constant__ MmsHostArgs mh,
+                      const __grid_constant__ KParams<double> Pd) {
+    if constexpr (has_mms<Sys>()) {
+        using G = typename Sys::Mms;
+        const int row = blockIdx.x * blockDim.x + threadIdx.x;
+        if (row >= ny * nz) return;
+        const int iz = row / ny, iy = row - iz * ny;
+        double Y[8], Z[8];
+        G::axis_row(1, iy * mh.dx, mh, Y);
+        if (G::NZ > 0) G::axis_row(2, iz * mh.dx, mh, Z);
+        G::template row_coeffs<double, R>(Pd.mms, Pd.T, Y, Z, coef + (size_t)row * G::NC);
     }
 }
 
@@ -67,17 +83,13 @@ collide_stream_node(const R* __restrict__ src, R* __restrict__ dst, const __grid
     const long long node = (long long)blockIdx.x * BLOCK + threadIdx.x;
     if (node >= P.n) return;
     const NodeIdx p = decompose(node, P.nx, P.ny);
-    // manufactured forcing first: its ~200 temporaries die before the populations are loaded
-    R smms[M];
-    if constexpr (MMS) mms_node<Sys, R>(P, p, smms);
-    // gather addresses: one 64-bit pointer per direction (source node of direction i), then a 32 x 32 -> 64 bit
-    // multiply-add per access for the (component, slot) plane: plane index is a compile-time constant, the
-    // plane stride n fits 32 bits (checked at grid creation), so each address is one IMAD.WIDE.U32.
-    const unsigned nn = (unsigned)P.n;
+    // gather addresses: one 64-bit pointer per direction (the source node's slot in its tile); the plane offset
+    // (k*Q + slot)*TILE is a compile-time constant, so every access is [pointer + immediate]
     const R* sp[Q];
 #pragma unroll
     for (int i = 0; i < Q; ++i)
-        sp[i] = src + node + ((MODE == MODE_AA_EVEN || MODE == MODE_LOCAL) ? 0LL : pull_offset(i, p, P.nx, P.ny, P.nz));
+        sp[i] = src + tile_off(node + ((MODE == MODE_AA_EVEN || MODE == MODE_LOCAL) ? 0LL : pull_offset(i, p, P.nx, P.ny, P.nz)), M * Q);
+    R* const dp = dst + tile_off(node, M * Q);
 
     R f[M][Q];
 #pragma unroll
@@ -85,8 +97,12 @@ collide_stream_node(const R* __restrict__ src, R* __restrict__ dst, const __grid
 #pragma unroll
         for (int i = 0; i < Q; ++i) {
             const int slot = (MODE == MODE_AA_ODD) ? opposite(i) : i;
-            f[k][i] = sp[i][(size_t)((unsigned)(k * Q + slot)) * nn];
+            f[k][i] = sp[i][(k * Q + slot) * TILE];
         }
+    // manufactured forcing while the gather is in flight: after the row/node split it is ~250 instructions on
+    // ~40 registers, independent of the populations
+    R smms[M];
+    if constexpr (MMS) mms_node<Sys, R>(P, p, smms);
     R dQ[M];
 #pragma unroll
     for (int k = 0; k < M; ++k) {
@@ -107,11 +123,11 @@ collide_stream_node(const R* __restrict__ src, R* __restrict__ dst, const __grid
 #pragma unroll
         for (int i = 0; i < Q; ++i) {
             if constexpr (MODE == MODE_PULL2 || MODE == MODE_LOCAL) {
-                (dst + node)[(size_t)((unsigned)(k * Q + i)) * nn] = f[k][i];
+                dp[(k * Q + i) * TILE] = f[k][i];
             } else if constexpr (MODE == MODE_AA_EVEN) {
-                (dst + node)[(size_t)((unsigned)(k * Q + opposite(i))) * nn] = f[k][i];
+                dp[(k * Q + opposite(i)) * TILE] = f[k][i];
             } else {   // AA odd: push to x + c_i; sp[opp(i)] - src + dst is that node (pull source of the opposite direction)
-                (dst + (sp[opposite(i)] - src))[(size_t)((unsigned)(k * Q + i)) * nn] = f[k][i];
+                (dst + (sp[opposite(i)] - src))[(k * Q + i) * TILE] = f[k][i];
             }
         }
     });
@@ -133,11 +149,11 @@ collide_stream_twopass(const R* __restrict__ src, R* __restrict__ dst, const __g
     const NodeIdx p = decompose(node, P.nx, P.ny);
     R smms[M];
     if constexpr (MMS) mms_node<Sys, R>(P, p, smms);
-    const unsigned nn = (unsigned)P.n;
     const R* sp[Q];
 #pragma unroll
     for (int i = 0; i < Q; ++i)
-        sp[i] = src + node + ((MODE == MODE_AA_EVEN || MODE == MODE_LOCAL) ? 0LL : pull_offset(i, p, P.nx, P.ny, P.nz));
+        sp[i] = src + tile_off(node + ((MODE == MODE_AA_EVEN || MODE == MODE_LOCAL) ? 0LL : pull_offset(i, p, P.nx, P.ny, P.nz)), M * Q);
+    R* const dp = dst + tile_off(node, M * Q);
     R dQ[M];
 #pragma unroll
     for (int k = 0; k < M; ++k) {
@@ -145,7 +161,7 @@ collide_stream_twopass(const R* __restrict__ src, R* __restrict__ dst, const __g
 #pragma unroll
         for (int i = 0; i < Q; ++i) {
             const int slot = (MODE == MODE_AA_ODD) ? opposite(i) : i;
-            const R v = sp[i][(size_t)((unsigned)(k * Q + slot)) * nn];
+            const R v = sp[i][(k * Q + slot) * TILE];
             s = (i == 0) ? v : s + v;                     // same summation order as the node kernel
         }
         dQ[k] = s;
@@ -161,17 +177,17 @@ collide_stream_twopass(const R* __restrict__ src, R* __restrict__ dst, const __g
 #pragma unroll
         for (int i = 0; i < Q; ++i) {
             const int slot = (MODE == MODE_AA_ODD) ? opposite(i) : i;
-            f[i] = sp[i][(size_t)((unsigned)(k * Q + slot)) * nn];
+            f[i] = sp[i][(k * Q + slot) * TILE];
         }
         relax<D, R>(f, P.omega[k], dQ[k], F, S);
 #pragma unroll
         for (int i = 0; i < Q; ++i) {
             if constexpr (MODE == MODE_PULL2 || MODE == MODE_LOCAL) {
-                (dst + node)[(size_t)((unsigned)(k * Q + i)) * nn] = f[i];
+                dp[(k * Q + i) * TILE] = f[i];
             } else if constexpr (MODE == MODE_AA_EVEN) {
-                (dst + node)[(size_t)((unsigned)(k * Q + opposite(i))) * nn] = f[i];
+                dp[(k * Q + opposite(i)) * TILE] = f[i];
             } else {
-                (dst + (sp[opposite(i)] - src))[(size_t)((unsigned)(k * Q + i)) * nn] = f[i];
+                (dst + (sp[opposite(i)] - src))[(k * Q + i) * TILE] = f[i];
             }
         }
     });
@@ -195,12 +211,12 @@ __global__ void init_from_U_kernel(const double* __restrict__ U, R* __restrict__
         R F[D], S;
         Sys::template flux<k>(ctx, dQ, P, F, S);
         using L = Lattice<D>;
-        f[(long long)(k * Q) * P.n + node] = R(L::w0) * dQ[k];
+        f[tile_off(node, M * Q) + (k * Q) * TILE] = R(L::w0) * dQ[k];
 #pragma unroll
         for (int a = 0; a < D; ++a) {
             const R h = R(0.5) * F[a];              // w1 / c_s^2 = 1/2
-            f[(long long)(k * Q + 1 + 2 * a) * P.n + node] = R(L::w1) * dQ[k] + h;
-            f[(long long)(k * Q + 2 + 2 * a) * P.n + node] = R(L::w1) * dQ[k] - h;
+            f[tile_off(node, M * Q) + (k * Q + 1 + 2 * a) * TILE] = R(L::w1) * dQ[k] + h;
+            f[tile_off(node, M * Q) + (k * Q + 2 + 2 * a) * TILE] = R(L::w1) * dQ[k] - h;
         }
     });
 }
@@ -235,11 +251,11 @@ __global__ void reference_equilibrium_kernel(double* __restrict__ feq0, const __
 // canonical gather: population (k, i) of `node` sits in slot i at node (GATHER_CANON), in slot opp(i) at
 // node - c_i (GATHER_AA_ODD) or in slot i at node - c_i (GATHER_PULL).
 template <int Q, class R>
-__device__ __forceinline__ R load_canonical(const R* __restrict__ f, long long n, int k, int i, long long node,
+__device__ __forceinline__ R load_canonical(const R* __restrict__ f, int M, int k, int i, long long node,
                                             const NodeIdx& p, int nx, int ny, int nz, int gather) {
-    if (gather == GATHER_CANON) return f[(long long)(k * Q + i) * n + node];
+    if (gather == GATHER_CANON) return f[tile_off(node, M * Q) + (k * Q + i) * TILE];
     const int slot = gather == GATHER_AA_ODD ? opposite(i) : i;
-    return f[(long long)(k * Q + slot) * n + node + pull_offset(i, p, nx, ny, nz)];
+    return f[tile_off(node + pull_offset(i, p, nx, ny, nz), M * Q) + (k * Q + slot) * TILE];
 }
 
 // U_k = Q0_k + sum_i f*_k,i, accumulated and returned in fp64 (eq 2.6; reading A17)
@@ -252,7 +268,7 @@ __global__ void read_U_kernel(const R* __restrict__ f, double* __restrict__ U, i
     for (int k = 0; k < M; ++k) {
         double s = 0.0;
 #pragma unroll
-        for (int i = 0; i < Q; ++i) s += (double)load_canonical<Q, R>(f, n, k, i, node, p, nx, ny, nz, gather);
+        for (int i = 0; i < Q; ++i) s += (double)load_canonical<Q, R>(f, M, k, i, node, p, nx, ny, nz, gather);
         U[(long long)k * n + node] = Pd.ref[k] + s;
     }
 }
@@ -267,14 +283,14 @@ __global__ void read_f_kernel(const R* __restrict__ f, double* __restrict__ out,
 #pragma unroll
         for (int i = 0; i < Q; ++i)
             out[(long long)(k * Q + i) * n + node] =
-                (double)load_canonical<Q, R>(f, n, k, i, node, p, nx, ny, nz, gather) + feq0[k * Q + i];
+                (double)load_canonical<Q, R>(f, M, k, i, node, p, nx, ny, nz, gather) + feq0[k * Q + i];
 }
 
 template <class R>
-__global__ void set_f_kernel(const double* __restrict__ in, R* __restrict__ f, const double* __restrict__ feq0, int MQ, long long n) {
+__global__ void set_f_kernel(const double* __restrict__ in, R* __restrict__ f, const double* __restrict__ feq0, int MQ, long long n) {   // in: [plane][node]
     const long long node = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (node >= n) return;
-    for (int q = 0; q < MQ; ++q) f[(long long)q * n + node] = (R)(in[(long long)q * n + node] - feq0[q]);
+    for (int q = 0; q < MQ; ++q) f[tile_off(node, MQ) + q * TILE] = (R)(in[(long long)q * n + node] - feq0[q]);
 }
 
 // ------------------------------------------------------------------------------------------------ a10
@@ -299,7 +315,7 @@ max_wave_speed_kernel(const R* __restrict__ f, unsigned long long* __restrict__ 
         for (int k = 0; k < M; ++k) {
             double s = 0.0;
 #pragma unroll
-            for (int i = 0; i < Q; ++i) s += (double)load_canonical<Q, R>(f, n, k, i, node, p, nx, ny, nz, gather);
+            for (int i = 0; i < Q; ++i) s += (double)load_canonical<Q, R>(f, M, k, i, node, p, nx, ny, nz, gather);
             U[k] = Pd.ref[k] + s;
         }
         Sys::wave(U, Pd, w);
@@ -355,13 +371,13 @@ __global__ void dirichlet_frame_kernel(R* __restrict__ f, int gather, const __gr
             R F[D], S;
             Sys::template flux<k>(ctx, dQ, P, F, S);
             using L = Lattice<D>;
-            f[(long long)(k * Q) * P.n + node] = R(L::w0) * dQ[k];
+            f[tile_off(node, M * Q) + (k * Q) * TILE] = R(L::w0) * dQ[k];
             for (int a = 0; a < D; ++a) {
                 const R h = R(0.5) * F[a];
                 const long long op = gather == GATHER_PULL ? pull_offset(1 + 2 * a, p, P.nx, P.ny, P.nz) : 0LL;
                 const long long om = gather == GATHER_PULL ? pull_offset(2 + 2 * a, p, P.nx, P.ny, P.nz) : 0LL;
-                f[(long long)(k * Q + 1 + 2 * a) * P.n + node + op] = R(L::w1) * dQ[k] + h;
-                f[(long long)(k * Q + 2 + 2 * a) * P.n + node + om] = R(L::w1) * dQ[k] - h;
+                f[tile_off(node + op, M * Q) + (k * Q + 1 + 2 * a) * TILE] = R(L::w1) * dQ[k] + h;
+                f[tile_off(node + om, M * Q) + (k * Q + 2 + 2 * a) * TILE] = R(L::w1) * dQ[k] - h;
             }
         });
     }

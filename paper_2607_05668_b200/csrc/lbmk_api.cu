@@ -39,7 +39,7 @@ struct lbmk_grid {
     long long opt_pattern, opt_kernel;
     bool bound, inited;
     size_t ws_bytes;
-    size_t off_f[2], off_tab[3], off_feq0, off_red;
+    size_t off_f[2], off_tab[3], off_coef, off_feq0, off_red;
     std::string err;
     cudaEvent_t ev0, ev1;
     bool have_events, timed;
@@ -248,12 +248,14 @@ static void layout(lbmk_grid* g) {
     GridCore& c = g->c;
     const SysOps* o = g->ops;
     const size_t esz = c.prec == PREC_F64 ? 8 : 4;
-    const size_t fbytes = align_up((size_t)o->M * (2 * o->D + 1) * (size_t)c.n * esz, 256);
+    const size_t ntiles = ((size_t)c.n + TILE - 1) / TILE;               // tiled SoA (common.cuh): last tile padded
+    const size_t fbytes = align_up((size_t)o->M * (2 * o->D + 1) * ntiles * TILE * esz, 256);
     size_t off = 0;
     g->off_f[0] = off; off += fbytes;
     g->off_f[1] = off; if (c.pattern == PATTERN_PULL2) off += fbytes;
     const int len[3] = {c.nx, c.ny, c.nz};
     for (int a = 0; a < 3; ++a) { g->off_tab[a] = off; off += align_up((size_t)(o->nax[a] > 0 ? o->nax[a] : 1) * len[a] * esz, 256); }
+    g->off_coef = off; off += align_up((size_t)(o->nc > 0 ? o->nc : 4) * c.ny * c.nz * esz, 256);
     g->off_feq0 = off; off += align_up((size_t)o->M * (2 * o->D + 1) * 8, 256);
     g->off_red = off; off += 256;
     g->ws_bytes = off;
@@ -349,6 +351,7 @@ lbmk_status lbmk_grid_bind_workspace(lbmk_grid* g, void* device_ptr, size_t byte
     c.f[0] = base + g->off_f[0];
     c.f[1] = c.pattern == PATTERN_PULL2 ? base + g->off_f[1] : nullptr;
     for (int a = 0; a < 3; ++a) c.tab[a] = base + g->off_tab[a];
+    c.coef = base + g->off_coef;
     c.feq0 = (double*)(base + g->off_feq0);
     c.red = (unsigned long long*)(base + g->off_red);
     c.cur = 0;

@@ -25,6 +25,7 @@ struct GridCore {
     long long step;       // completed steps
     double t0, dt;
     void* tab[3];         // per-axis trig tables in R, [entry][index]
+    void* coef;           // per-row forcing coefficients in R, [nz*ny][nc]
     double* feq0;         // [M*Q] reference equilibrium (fp64)
     unsigned long long* red;   // [4] reduction scratch
     KParams<double> Pd;   // parameters in fp64 (host logic, fp64 kernels, readback)
@@ -37,6 +38,7 @@ struct SysOps {
     int id, D, M, MC;
     bool has_mms;
     int nt, nax[3];       // time scalars and table entries per axis of the manufactured solution
+    int nc;               // per-row forcing coefficients (multiple of 4; 0 without manufactured solution)
     // all return cudaError_t of the last launch / API call
     cudaError_t (*fill_tables)(GridCore&);                 // host fp64 -> device R tables (synchronous copy on the stream)
     cudaError_t (*reference_equilibrium)(GridCore&);

@@ -15,7 +15,7 @@ template <> __host__ inline KParams<float>& kp<float>(GridCore& g) { return g.Pf
 
 // launch shape of the node kernel per system: threads per block, min blocks per SM (register cap)
 template <template <class> class S, class R> struct Tune { static constexpr int BLOCK = 256, MINB = 1; };
-template <class R> struct Tune<SysNsf3D, R> { static constexpr int BLOCK = 128, MINB = 2; };
+template <class R> struct Tune<SysNsf3D, R> { static constexpr int BLOCK = 128, MINB = 3; };
 template <> struct Tune<SysNsf3D, double> { static constexpr int BLOCK = 128, MINB = 1; };
 template <class R> struct Tune<SysMhd3D, R> { static constexpr int BLOCK = 128, MINB = 2; };
 
@@ -24,8 +24,8 @@ template <template <class> class S, class R> struct Tune2 { static constexpr int
 template <class R> struct Tune2<SysNsf3D, R> { static constexpr int BLOCK = 128, MINB = 4; };
 template <class R> struct Tune2<SysMhd3D, R> { static constexpr int BLOCK = 128, MINB = 4; };
 
-template <class Mm> struct MmsCounts { static constexpr int NT = Mm::NT, NX = Mm::NX, NY = Mm::NY, NZ = Mm::NZ; };
-template <> struct MmsCounts<void> { static constexpr int NT = 0, NX = 0, NY = 0, NZ = 0; };
+template <class Mm> struct MmsCounts { static constexpr int NT = Mm::NT, NX = Mm::NX, NY = Mm::NY, NZ = Mm::NZ, NC = Mm::NC; };
+template <> struct MmsCounts<void> { static constexpr int NT = 0, NX = 0, NY = 0, NZ = 0, NC = 0; };
 
 inline unsigned blocks_for(long long n, int block) { return (unsigned)((n + block - 1) / block); }
 
@@ -64,6 +64,7 @@ struct Ops {
                 if (e != cudaSuccess) return e;
             }
             kp<R>(g).tabX = (const R*)g.tab[0]; kp<R>(g).tabY = (const R*)g.tab[1]; kp<R>(g).tabZ = (const R*)g.tab[2];
+            kp<R>(g).coef = (const R*)g.coef;
         }
         return cudaSuccess;
     }
@@ -162,7 +163,12 @@ struct Ops {
                     g.launches++;
                 }
             }
-            if constexpr (MMS) time_scalars(g, t_n + 0.5 * g.dt);           // explicit forcing at the temporal midpoint, L154
+            if constexpr (MMS) {                                             // explicit forcing at the temporal midpoint, L154
+                time_scalars(g, t_n + 0.5 * g.dt);
+                const int rows = g.ny * g.nz;
+                mms_row_coeffs_kernel<S<R>, R><<<(rows + 127) / 128, 128, 0, g.stream>>>((R*)g.coef, g.ny, g.nz, g.mh, g.Pd);
+                g.launches++;
+            }
             if (g.pattern == PATTERN_PULL2) {
                 if (g.pending) launch_node<R, MODE_PULL2, MMS>(g, (const R*)g.f[g.cur], (R*)g.f[g.cur ^ 1]);
                 else launch_node<R, MODE_LOCAL, MMS>(g, (const R*)g.f[g.cur], (R*)g.f[g.cur ^ 1]);
@@ -204,7 +210,7 @@ struct Ops {
     static bool row_supported(const GridCore&) { return false; }
 
     static const SysOps* get() {
-        static const SysOps ops = {Sd::ID, D, M, Sd::MC, HAS_MMS, C::NT, {C::NX, C::NY, C::NZ},
+        static const SysOps ops = {Sd::ID, D, M, Sd::MC, HAS_MMS, C::NT, {C::NX, C::NY, C::NZ}, C::NC,
                                    &fill_tables, &reference_equilibrium, &init_from_U, &set_f, &step,
                                    &read_U_with_frame, &read_f, &max_wave_speed, &row_supported};
         return &ops;

@@ -325,6 +325,134 @@ def _emit_body(assign: List[Tuple[sp.Symbol, sp.Expr]], outputs: List[sp.Expr], 
     return lines, ops, free
 
 
+# ------------------------------------------------------------------------------------------------ row / node split
+# The step kernels run one thread block per x-row segment, so everything that does not depend on x is the
+# same for all threads of a block.  Substituting the closed forms and expanding, every forcing component is
+#     s_k(x; y, z, t) = sum_j C_kj(y, z, t) * mon_j(X0.., r..)
+# a short polynomial in the x-table entries X# and in the reciprocals r of the (x-dependent) fields that the
+# residual divides by (rho for NSF: T = p/rho), with coefficients that are per-row constants.  `row_coeffs`
+# evaluates the C_kj once per (y, z) row and step (a tiny pre-kernel, in fp64); `source_row` is what is left
+# per node: a few monomials and one FMA per term.
+def split_rows(g):
+    xs = [sp.Symbol(f"X{i}", real=True) for i in range(len(g["tabs"][x]))]
+    xset = set(xs)
+    l1 = dict(g["layer1"])
+    recips: Dict[sp.Symbol, sp.Symbol] = {}
+
+    def neg_pow(a):
+        return a.is_Pow and a.exp.is_Integer and a.exp < 0 and a.base in l1 and bool(l1[a.base].free_symbols & xset)
+
+    def to_recip(a):
+        if a.base not in recips:
+            recips[a.base] = sp.Symbol(f"r_{a.base}", real=True)
+        return recips[a.base] ** (-a.exp)
+
+    lowered = []
+    for e in g["res"]:
+        e = sp.expand(e).replace(neg_pow, to_recip)
+        lowered.append(sp.expand(e.xreplace(l1)))
+    gens = xs + [recips[b] for b in sorted(recips, key=str)]
+    coefs: List[sp.Expr] = []           # distinct per-row coefficient expressions
+    index: Dict[sp.Expr, Tuple[int, int]] = {}
+
+    def coef_ref(c):
+        """(index, sign) of coefficient expression c in the row table (shared up to sign)."""
+        c = sp.factor_terms(c)
+        if c in index:
+            return index[c]
+        if -c in index:
+            i, sg = index[-c]
+            return i, -sg
+        coefs.append(c)
+        index[c] = (len(coefs) - 1, 1)
+        return index[c]
+
+    def poly_terms(e, gs):
+        if e == 0:
+            return []
+        P = sp.Poly(e, *gs) if gs else None
+        if P is None:
+            return [((), e)]
+        return [(m, c) for m, c in zip(P.monoms(), P.coeffs())]
+
+    C = lambda i: sp.Symbol(f"C{i}", real=True)
+    node_defs: List[Tuple[sp.Symbol, sp.Expr]] = []
+    for b in sorted(recips, key=str):                       # r_b = 1 / (polynomial in X with row coefficients)
+        den = 0
+        for m, c in poly_terms(sp.expand(l1[b]), xs):
+            i, sg = coef_ref(c)
+            den += sg * C(i) * sp.Mul(*[gx ** ex for gx, ex in zip(xs, m)])
+        node_defs.append((recips[b], 1 / den))
+    outs = []
+    n_terms = 0
+    for e in lowered:
+        acc = 0
+        for m, c in poly_terms(e, gens):
+            assert not (c.free_symbols & (xset | set(recips.values()))), "coefficient depends on x"
+            i, sg = coef_ref(c)
+            acc += sg * C(i) * sp.Mul(*[gx ** ex for gx, ex in zip(gens, m)])
+            n_terms += 1
+        outs.append(acc)
+    return dict(coefs=coefs, node_defs=node_defs, outs=outs, n_terms=n_terms)
+
+
+def _emit_row_coeffs(sr, pr: _Printer, indent="        "):
+    """CSE'd straight-line code c[i] = ... for the per-row coefficients."""
+    repl, red = sp.cse(sr["coefs"], symbols=sp.numbered_symbols("u"), optimizations="basic")
+    lines, ops, free = [], 0, set()
+    for s_, e in repl:
+        lines.append(f"{indent}const {pr.real} {s_} = {pr.doprint(e)};")
+        ops += int(sp.count_ops(e)); free |= e.free_symbols
+    for i, e in enumerate(red):
+        lines.append(f"{indent}c[{i}] = (RO)({pr.doprint(e)});")
+        ops += int(sp.count_ops(e)); free |= e.free_symbols
+    free -= {s_ for s_, _ in repl}
+    return lines, ops, free
+
+
+def _emit_source_row(sr, pr: _Printer, indent="        "):
+    """Per-node code: coefficient loads in 4-wide chunks right before first use, monomials CSE'd."""
+    n_def = len(sr["node_defs"])
+    repl, red = sp.cse([e for _, e in sr["node_defs"]] + sr["outs"], symbols=sp.numbered_symbols("m"), optimizations="basic")
+    loaded = set()
+    lines, ops = [], 0
+    names = {}
+
+    def prepare(e):
+        for s_ in sorted(e.free_symbols, key=str):
+            n = str(s_)
+            if n[0] == "C" and n[1:].isdigit():
+                i = int(n[1:])
+                if i // 4 not in loaded:
+                    loaded.add(i // 4)
+                    lines.append(f"{indent}const Vec4<R> q{i // 4} = ld4(c + {4 * (i // 4)});")
+                names[s_] = sp.Symbol(f"q{i // 4}.{'xyzw'[i % 4]}", real=True)
+        return e.xreplace(names)
+
+    defs = list(repl) + [(sr["node_defs"][i][0], red[i]) for i in range(n_def)]
+    index_of = {s_: i for i, (s_, _) in enumerate(defs)}
+    done = set()
+
+    def visit(i):                                   # dependency order: r_* are inputs of CSE temps and outputs of others
+        if i in done:
+            return
+        done.add(i)
+        for d in sorted(defs[i][1].free_symbols, key=str):
+            if d in index_of:
+                visit(index_of[d])
+        s_, e = defs[i]
+        lines.append(f"{indent}const R {s_} = {pr.doprint(prepare(e))};")
+
+    for k, e in enumerate(red[n_def:]):
+        for d in sorted(e.free_symbols, key=str):
+            if d in index_of:
+                visit(index_of[d])
+        lines.append(f"{indent}s[{k}] = {pr.doprint(prepare(e))};")
+        ops += int(sp.count_ops(e))
+    ops += sum(int(sp.count_ops(defs[i][1])) for i in done)
+    return lines, ops
+
+
 # ------------------------------------------------------------------------------------------------ emission
 SCALARS = {"dx": "a.dx", "dt": "a.dt", "il": "a.il", "gtau": "a.gtau", "TWO_PI": "R(6.283185307179586477)"}
 
@@ -365,6 +493,14 @@ def emit_system(g) -> str:
     o.append(f"// ---- {name}: m = {m}, dim = {dim}; forcing {src_ops} ops, exact state {q_ops} ops")
     o.append(f"struct Mms_{name} {{")
     o.append(f"    static constexpr int M = {m}, NT = {nt}, NX = {nx_}, NY = {ny_}, NZ = {max(nz_, 0)};")
+    sr = split_rows(g)
+    nc = len(sr["coefs"])
+    ncp = (nc + 3) // 4 * 4
+    prd = _Printer("R")
+    rc_lines, rc_ops, rc_free = _emit_row_coeffs(sr, prd)
+    sn_lines, sn_ops = _emit_source_row(sr, pr)
+    o.append(f"    // row/node split of the forcing: {nc} per-row coefficients ({rc_ops} ops per row), {sr['n_terms']} terms, {sn_ops} ops per node")
+    o.append(f"    static constexpr int NC = {ncp};")
     # host: time scalars and axis rows
     o.append("    // host side (fp64): per-step time scalars and per-axis table rows")
     o.append("    static inline void time_scalars(double c, const MmsHostArgs& a, double* T) {")
@@ -372,7 +508,7 @@ def emit_system(g) -> str:
     for i, e in enumerate(g["tabs"][t]):
         o.append(f"        T[{i}] = {_host_bind(_host_expr(e, t))};")
     o.append("    }")
-    o.append("    static inline void axis_row(int axis, double c, const MmsHostArgs& a, double* row) {")
+    o.append("    static __host__ __device__ inline void axis_row(int axis, double c, const MmsHostArgs& a, double* row) {")
     o.append("        (void)c; (void)a; (void)row;")
     for ax, cs in enumerate((x, y, z)):
         if not g["tabs"][cs]:
@@ -390,6 +526,24 @@ def emit_system(g) -> str:
         o += ["    " + l for l in _bind_inputs(free, "R")]
         o += ["    " + l for l in lines]
         o.append("    }")
+    # row / node split
+    o.append("    // per-row coefficients C(y, z, t) of the forcing polynomial in the x-table entries (see gen/mms_codegen.py split_rows)")
+    o.append("    template <class R, class RO>")
+    o.append("    static __host__ __device__ __forceinline__ void row_coeffs(const MmsArgs<R>& a, const R* T, const R* Y, const R* Z, RO* c) {")
+    o.append("        (void)a; (void)T; (void)Y; (void)Z;")
+    o += ["    " + l for l in _bind_inputs(rc_free, "R")]
+    o += rc_lines
+    for i in range(nc, ncp):
+        o.append(f"        c[{i}] = (RO)0;")
+    o.append("    }")
+    o.append("    // per-node remainder: s_k = sum_j C_kj * monomial_j(X, 1/rho..); c = this row's coefficients (32-byte aligned)")
+    o.append("    template <class R>")
+    o.append("    static __device__ __forceinline__ void source_row(const R* __restrict__ c, const R* X, R* s) {")
+    o.append("        (void)c; (void)X;")
+    for i in range(nx_):
+        o.append(f"        const R X{i} = X[{i}];")
+    o += sn_lines
+    o.append("    }")
     o.append("};")
     return "\n".join(o)
 
@@ -417,6 +571,19 @@ namespace lbmk {
 
 struct MmsHostArgs { double par[16]; double mp[16]; double dx, dt, il, gtau; };
 template <class R> struct MmsArgs { R par[8]; R mp[8]; R dx, dt, il, gtau; };
+
+// four consecutive row coefficients, loaded with 128-bit read-only loads (all threads of a block read the same row)
+template <class R> struct Vec4 { R x, y, z, w; };
+#ifdef __CUDACC__
+__device__ __forceinline__ Vec4<float> ld4(const float* p) {
+    const float4 v = __ldg(reinterpret_cast<const float4*>(p));
+    return Vec4<float>{v.x, v.y, v.z, v.w};
+}
+__device__ __forceinline__ Vec4<double> ld4(const double* p) {
+    const double2 a = __ldg(reinterpret_cast<const double2*>(p)), b = __ldg(reinterpret_cast<const double2*>(p) + 1);
+    return Vec4<double>{a.x, a.y, b.x, b.y};
+}
+#endif
 
 """
 

@@ -84,7 +84,7 @@ def test_argument_validation():
 
 def test_grid_scaling_and_workspace_layout():
     """omega_k = 1/(1/2 + tau_R dt) for conserved fields (L194), 1/(g_tau + 1) for trackers (L718); workspace
-    = populations (x2 for the two-lattice pattern) + small tables."""
+    = populations (x2 for the two-lattice pattern) + small tables + the per-row forcing coefficients."""
     w = W.c4_nsf3d(16)
     s = P.System(w.system, params=w.params, tau_R=w.tau_R, g_tau=w.g_tau, U_ref=w.U_ref, mms_id=1, mms_params=w.mms_params)
     g = P.lbmk_grid_create(s.h, 16, 16, 16, 0, w.dx, w.lam, P.LBMK_F32_SHIFTED, 0)
@@ -95,7 +95,9 @@ def test_grid_scaling_and_workspace_layout():
     b2 = P.lbmk_grid_workspace_bytes(g)
     P.lbmk_grid_set_option(g, P.LBMK_OPT_PATTERN, P.LBMK_PATTERN_AA)
     b1 = P.lbmk_grid_workspace_bytes(g)
-    assert 2 * pops <= b2 < 2 * pops + 65536 and pops <= b1 < pops + 65536
+    small = 65536 + 16 * 16 * 128 * 4          # tables, reduction scratch, [ny*nz][NC <= 128] row coefficients
+    assert 2 * pops <= b2 < 2 * pops + small and pops <= b1 < pops + small
+    assert b2 - b1 == pops                     # the second lattice is the only difference
     assert P.lbmk_time(g) == (0, 0.0)
     # calls out of order are refused, not crashed
     with pytest.raises(P.LbmkError) as e:
