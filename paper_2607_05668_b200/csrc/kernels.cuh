@@ -40,21 +40,27 @@ __device__ __forceinline__ void mms_node(const KParams<R>& P, const NodeIdx& p, 
     }
 }
 
-// Row coefficients of the forcing at the time whose scalars are in T: one thread per (y, z) row, fp64 from the
-// closed forms (no tables), stored in R.  ~1e3 flops x ny*nz threads per step: negligible next to the step.
+// Row coefficients of the forcing for `nb` consecutive steps: one thread per (step, (y, z) row), fp64 from the
+// closed forms (no tables), stored in R as coef[b][row][NC].  Step b is forced at its temporal midpoint
+// t_first + b dt + dt/2.  ~1e3 flops x ny*nz threads per step: negligible next to the step,
+// and it runs on the auxiliary stream under the previous batch's steps.
 template <class Sys, class R>
 __global__ void __launch_bounds__(128)
-mms_row_coeffs_kernel(R* __restrict__ coef, int ny, int nz, const __grid_constant__ MmsHostArgs mh,
-                      const __grid_constant__ KParams<double> Pd) {
+mms_row_coeffs_kernel(R* __restrict__ coef, int ny, int nz, int nb, double t_first, double dt,
+                      const __grid_constant__ MmsHostArgs mh, const __grid_constant__ MmsArgs<double> ma) {
     if constexpr (has_mms<Sys>()) {
         using G = typename Sys::Mms;
-        const int row = blockIdx.x * blockDim.x + threadIdx.x;
-        if (row >= ny * nz) return;
+        const int rows = ny * nz;
+        const long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+        if (id >= (long long)rows * nb) return;
+        const int b = (int)(id / rows), row = (int)(id - (long long)b * rows);
         const int iz = row / ny, iy = row - iz * ny;
-        double Y[8], Z[8];
+        double T[8], Y[8], Z[8];
+        const double t_n = t_first + (double)b * dt;
+        G::time_scalars(t_n + 0.5 * dt, mh, T);
         G::axis_row(1, iy * mh.dx, mh, Y);
         if (G::NZ > 0) G::axis_row(2, iz * mh.dx, mh, Z);
-        G::template row_coeffs<double, R>(Pd.mms, Pd.T, Y, Z, coef + (size_t)row * G::NC);
+        G::template row_coeffs<double, R>(ma, T, Y, Z, coef + (size_t)id * G::NC);
     }
 }
 

@@ -255,7 +255,14 @@ static void layout(lbmk_grid* g) {
     g->off_f[1] = off; if (c.pattern == PATTERN_PULL2) off += fbytes;
     const int len[3] = {c.nx, c.ny, c.nz};
     for (int a = 0; a < 3; ++a) { g->off_tab[a] = off; off += align_up((size_t)(o->nax[a] > 0 ? o->nax[a] : 1) * len[a] * esz, 256); }
-    g->off_coef = off; off += align_up((size_t)(o->nc > 0 ? o->nc : 4) * c.ny * c.nz * esz, 256);
+    // per-row forcing coefficients: 2 buffers x coef_B steps x [ny*nz][nc]; a batch is at most ~32 MB and 64 steps
+    {
+        const size_t per_step = (size_t)(o->nc > 0 ? o->nc : 4) * c.ny * c.nz * esz;
+        size_t B = (size_t(32) << 20) / per_step;
+        c.coef_B = (int)(B < 1 ? 1 : (B > 64 ? 64 : B));
+        if (!(o->has_mms && c.mms_id != 0)) c.coef_B = 1;
+        g->off_coef = off; off += align_up(2 * (size_t)c.coef_B * per_step, 256);
+    }
     g->off_feq0 = off; off += align_up((size_t)o->M * (2 * o->D + 1) * 8, 256);
     g->off_red = off; off += 256;
     g->ws_bytes = off;
@@ -360,6 +367,12 @@ lbmk_status lbmk_grid_bind_workspace(lbmk_grid* g, void* device_ptr, size_t byte
     if (!g->have_events) {
         CK(g, cudaEventCreate(&g->ev0), "cudaEventCreate");
         CK(g, cudaEventCreate(&g->ev1), "cudaEventCreate");
+        CK(g, cudaStreamCreateWithFlags(&c.aux, cudaStreamNonBlocking), "cudaStreamCreate");
+        CK(g, cudaEventCreateWithFlags(&c.ev_entry, cudaEventDisableTiming), "cudaEventCreate");
+        for (int b = 0; b < 2; ++b) {
+            CK(g, cudaEventCreateWithFlags(&c.ev_coef[b], cudaEventDisableTiming), "cudaEventCreate");
+            CK(g, cudaEventCreateWithFlags(&c.ev_free[b], cudaEventDisableTiming), "cudaEventCreate");
+        }
         g->have_events = true;
     }
     g->bound = true;
@@ -369,7 +382,12 @@ lbmk_status lbmk_grid_bind_workspace(lbmk_grid* g, void* device_ptr, size_t byte
 
 void lbmk_grid_destroy(lbmk_grid* g) {
     if (!g) return;
-    if (g->have_events) { cudaEventDestroy(g->ev0); cudaEventDestroy(g->ev1); }
+    if (g->have_events) {
+        cudaStreamSynchronize(g->c.aux);
+        cudaEventDestroy(g->ev0); cudaEventDestroy(g->ev1); cudaEventDestroy(g->c.ev_entry);
+        for (int b = 0; b < 2; ++b) { cudaEventDestroy(g->c.ev_coef[b]); cudaEventDestroy(g->c.ev_free[b]); }
+        cudaStreamDestroy(g->c.aux);
+    }
     delete g;
 }
 

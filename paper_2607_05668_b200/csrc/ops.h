@@ -25,7 +25,11 @@ struct GridCore {
     long long step;       // completed steps
     double t0, dt;
     void* tab[3];         // per-axis trig tables in R, [entry][index]
-    void* coef;           // per-row forcing coefficients in R, [nz*ny][nc]
+    void* coef;           // per-row forcing coefficients in R: 2 buffers x [coef_B steps][nz*ny][nc]
+    int coef_B;           // steps per coefficient batch (one pre-kernel launch fills a batch)
+    cudaStream_t aux;     // the pre-kernel of batch j+1 runs here while the steps of batch j run on `stream`
+    cudaEvent_t ev_entry, ev_coef[2], ev_free[2];
+    bool coef_used[2];
     double* feq0;         // [M*Q] reference equilibrium (fp64)
     unsigned long long* red;   // [4] reduction scratch
     KParams<double> Pd;   // parameters in fp64 (host logic, fp64 kernels, readback)

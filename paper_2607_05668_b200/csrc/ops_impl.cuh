@@ -152,36 +152,76 @@ struct Ops {
         }
         g.launches++;
     }
+    // one collide-and-stream launch (plus the Dirichlet frame refill before it on bounded grids)
     template <class R, bool MMS>
-    static cudaError_t step_t(GridCore& g, int n_steps) {
-        for (int s = 0; s < n_steps; ++s) {
-            const double t_n = g.t0 + (double)g.step * g.dt;
-            if (g.bc == 1) {
-                if constexpr (HAS_MMS) {
-                    time_scalars(g, t_n);
-                    dirichlet_frame_kernel<S<R>, R><<<blocks_for(g.n, 256), 256, 0, g.stream>>>((R*)g.f[g.cur], aa_odd(g), kp<R>(g), g.Pd);
-                    g.launches++;
-                }
-            }
-            if constexpr (MMS) {                                             // explicit forcing at the temporal midpoint, L154
-                time_scalars(g, t_n + 0.5 * g.dt);
-                const int rows = g.ny * g.nz;
-                mms_row_coeffs_kernel<S<R>, R><<<(rows + 127) / 128, 128, 0, g.stream>>>((R*)g.coef, g.ny, g.nz, g.mh, g.Pd);
+    static void one_step(GridCore& g) {
+        if (g.bc == 1) {
+            if constexpr (HAS_MMS) {
+                time_scalars(g, g.t0 + (double)g.step * g.dt);
+                dirichlet_frame_kernel<S<R>, R><<<blocks_for(g.n, 256), 256, 0, g.stream>>>((R*)g.f[g.cur], aa_odd(g), kp<R>(g), g.Pd);
                 g.launches++;
             }
-            if (g.pattern == PATTERN_PULL2) {
-                if (g.pending) launch_node<R, MODE_PULL2, MMS>(g, (const R*)g.f[g.cur], (R*)g.f[g.cur ^ 1]);
-                else launch_node<R, MODE_LOCAL, MMS>(g, (const R*)g.f[g.cur], (R*)g.f[g.cur ^ 1]);
-                g.cur ^= 1;
-                g.pending = 1;
-            } else if ((g.step & 1) == 0) {
-                launch_node<R, MODE_AA_EVEN, MMS>(g, (const R*)g.f[0], (R*)g.f[0]);
-            } else {
-                launch_node<R, MODE_AA_ODD, MMS>(g, (const R*)g.f[0], (R*)g.f[0]);
-            }
-            g.step++;
         }
-        return cudaGetLastError();
+        if (g.pattern == PATTERN_PULL2) {
+            if (g.pending) launch_node<R, MODE_PULL2, MMS>(g, (const R*)g.f[g.cur], (R*)g.f[g.cur ^ 1]);
+            else launch_node<R, MODE_LOCAL, MMS>(g, (const R*)g.f[g.cur], (R*)g.f[g.cur ^ 1]);
+            g.cur ^= 1;
+            g.pending = 1;
+        } else if ((g.step & 1) == 0) {
+            launch_node<R, MODE_AA_EVEN, MMS>(g, (const R*)g.f[0], (R*)g.f[0]);
+        } else {
+            launch_node<R, MODE_AA_ODD, MMS>(g, (const R*)g.f[0], (R*)g.f[0]);
+        }
+        g.step++;
+    }
+    // row coefficients of steps [first, first + nb) into coefficient buffer `buf`, on the auxiliary stream
+    template <class R>
+    static void launch_coeffs(GridCore& g, int buf, long long first, int nb) {
+        const long long rows = (long long)g.ny * g.nz;
+        R* dst = (R*)g.coef + (size_t)buf * g.coef_B * rows * C::NC;
+        const long long threads = rows * nb;
+        mms_row_coeffs_kernel<S<R>, R><<<(unsigned)((threads + 127) / 128), 128, 0, g.aux>>>(
+            dst, g.ny, g.nz, nb, g.t0 + (double)first * g.dt, g.dt, g.mh, g.Pd.mms);
+        g.launches++;
+    }
+    template <class R, bool MMS>
+    static cudaError_t step_t(GridCore& g, int n_steps) {
+        if constexpr (!MMS) {
+            for (int s = 0; s < n_steps; ++s) one_step<R, false>(g);
+            return cudaGetLastError();
+        } else {
+            // Explicit forcing at the temporal midpoint (L154).  Its per-row coefficients are produced in batches of
+            // coef_B steps on the auxiliary stream, double-buffered: batch j+1 is computed while batch j is consumed.
+            const long long rows = (long long)g.ny * g.nz;
+            const int B = g.coef_B;
+            cudaError_t e = cudaEventRecord(g.ev_entry, g.stream);       // earlier calls may still read the buffers
+            if (e != cudaSuccess) return e;
+            e = cudaStreamWaitEvent(g.aux, g.ev_entry, 0);
+            if (e != cudaSuccess) return e;
+            int done = 0, buf = 0;
+            launch_coeffs<R>(g, 0, g.step, std::min(B, n_steps));
+            cudaEventRecord(g.ev_coef[0], g.aux);
+            g.coef_used[0] = g.coef_used[1] = false;
+            while (done < n_steps) {
+                const int cnt = std::min(B, n_steps - done);
+                if (done + cnt < n_steps) {
+                    if (g.coef_used[buf ^ 1]) cudaStreamWaitEvent(g.aux, g.ev_free[buf ^ 1], 0);
+                    launch_coeffs<R>(g, buf ^ 1, g.step + cnt, std::min(B, n_steps - done - cnt));
+                    cudaEventRecord(g.ev_coef[buf ^ 1], g.aux);
+                }
+                e = cudaStreamWaitEvent(g.stream, g.ev_coef[buf], 0);
+                if (e != cudaSuccess) return e;
+                for (int j = 0; j < cnt; ++j) {
+                    kp<R>(g).coef = (const R*)g.coef + ((size_t)buf * B + j) * rows * C::NC;
+                    one_step<R, true>(g);
+                }
+                cudaEventRecord(g.ev_free[buf], g.stream);
+                g.coef_used[buf] = true;
+                done += cnt;
+                buf ^= 1;
+            }
+            return cudaGetLastError();
+        }
     }
     static cudaError_t step(GridCore& g, int n_steps) {
         const bool mms = HAS_MMS && g.mms_id != 0;

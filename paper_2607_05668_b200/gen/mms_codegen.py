@@ -503,7 +503,7 @@ def emit_system(g) -> str:
     o.append(f"    static constexpr int NC = {ncp};")
     # host: time scalars and axis rows
     o.append("    // host side (fp64): per-step time scalars and per-axis table rows")
-    o.append("    static inline void time_scalars(double c, const MmsHostArgs& a, double* T) {")
+    o.append("    static __host__ __device__ inline void time_scalars(double c, const MmsHostArgs& a, double* T) {")
     o.append("        (void)c; (void)a; (void)T;")
     for i, e in enumerate(g["tabs"][t]):
         o.append(f"        T[{i}] = {_host_bind(_host_expr(e, t))};")

@@ -95,7 +95,7 @@ def test_grid_scaling_and_workspace_layout():
     b2 = P.lbmk_grid_workspace_bytes(g)
     P.lbmk_grid_set_option(g, P.LBMK_OPT_PATTERN, P.LBMK_PATTERN_AA)
     b1 = P.lbmk_grid_workspace_bytes(g)
-    small = 65536 + 16 * 16 * 128 * 4          # tables, reduction scratch, [ny*nz][NC <= 128] row coefficients
+    small = 65536 + 2 * 64 * 16 * 16 * 128 * 4   # tables, scratch, forcing coefficients: 2 buffers x <= 64 steps x [ny*nz][NC <= 128]
     assert 2 * pops <= b2 < 2 * pops + small and pops <= b1 < pops + small
     assert b2 - b1 == pops                     # the second lattice is the only difference
     assert P.lbmk_time(g) == (0, 0.0)
