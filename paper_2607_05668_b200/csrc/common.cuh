@@ -53,11 +53,14 @@ struct KParams {
 struct NodeIdx { int ix, iy, iz; };
 
 __device__ __forceinline__ NodeIdx decompose(long long node, int nx, int ny) {
+    // nx*ny*nz < 2^31 is checked at grid creation: 32-bit unsigned divisions (no 64-bit division subroutine)
     NodeIdx p;
-    const long long row = node / nx;
-    p.ix = (int)(node - row * nx);
-    p.iz = (int)(row / ny);
-    p.iy = (int)(row - (long long)p.iz * ny);
+    const unsigned nd = (unsigned)node;
+    const unsigned row = nd / (unsigned)nx;
+    p.ix = (int)(nd - row * (unsigned)nx);
+    const unsigned iz = row / (unsigned)ny;
+    p.iz = (int)iz;
+    p.iy = (int)(row - iz * (unsigned)ny);
     return p;
 }
 

@@ -26,19 +26,34 @@ enum { MODE_PULL2 = 0, MODE_AA_EVEN = 1, MODE_AA_ODD = 2, MODE_LOCAL = 3 };
 enum { GATHER_CANON = 0, GATHER_AA_ODD = 1, GATHER_PULL = 2 };
 
 template <class Sys> __host__ __device__ constexpr bool has_mms() { return !std::is_void<typename Sys::Mms>::value; }
+template <class Sys, bool = has_mms<Sys>()> struct MmsNC { static constexpr int value = 4; };
+template <class Sys> struct MmsNC<Sys, true> { static constexpr int value = Sys::Mms::NC; };
 
 // per-node manufactured forcing: the x-table entries of this node and the coefficients of its (y, z) row
-// (mms_generated.cuh source_row; the row table is filled by mms_row_coeffs_kernel before every step)
-template <class Sys, class R>
-__device__ __forceinline__ void mms_node(const KParams<R>& P, const NodeIdx& p, R (&s)[Sys::M]) {
+// (mms_generated.cuh source_row; the row table is filled by mms_row_coeffs_kernel).  SH: `c` is the block's
+// shared-memory copy of its row (see stage_row_coeffs), otherwise the row is read from global memory.
+template <class Sys, class R, bool SH>
+__device__ __forceinline__ void mms_node(const KParams<R>& P, const NodeIdx& p, const R* c, R (&s)[Sys::M]) {
     if constexpr (has_mms<Sys>()) {
         using G = typename Sys::Mms;
         R X[G::NX > 0 ? G::NX : 1];
 #pragma unroll
         for (int e = 0; e < G::NX; ++e) X[e] = __ldg(P.tabX + e * P.nx + p.ix);
-        G::template source_row<R>(P.coef + (size_t)(p.iz * P.ny + p.iy) * G::NC, X, s);
+        if (!SH) c = P.coef + (size_t)(p.iz * P.ny + p.iy) * G::NC;
+        G::template source_row<R, SH>(c, X, s);
     }
 }
+
+// When nx is a multiple of the block size a thread block lies inside ONE (y, z) row: its NC coefficients are
+// copied to shared memory with 16-byte cp.async issued BEFORE the population gather, so that the forcing reads
+// them with short-latency LDS.128 instead of chains of L2 round trips queued behind the gather.
+template <class R>
+__device__ __forceinline__ void cp_async16(R* smem_dst, const R* gmem_src) {
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
 // Row coefficients of the forcing for `nb` consecutive steps: one thread per (step, (y, z) row), fp64 from the
 // closed forms (no tables), stored in R as coef[b][row][NC].  Step b is forced at its temporal midpoint
@@ -87,6 +102,17 @@ __global__ void __launch_bounds__(BLOCK, MINB)
 collide_stream_node(const R* __restrict__ src, R* __restrict__ dst, const __grid_constant__ KParams<R> P) {
     constexpr int D = Sys::D, Q = 2 * D + 1, M = Sys::M;
     const long long node = (long long)blockIdx.x * BLOCK + threadIdx.x;
+    constexpr int NCs = MMS ? MmsNC<Sys>::value : 4;
+    __shared__ __align__(16) R coef_s[NCs];
+    const bool staged = MMS && (P.nx % BLOCK == 0);          // kernel-uniform; then n is a multiple of BLOCK too
+    if constexpr (MMS) {
+        if (staged) {
+            const unsigned row = (unsigned)((long long)blockIdx.x * BLOCK / P.nx);
+            constexpr int per = 16 / sizeof(R);
+            if (threadIdx.x < NCs / per) cp_async16(coef_s + per * threadIdx.x, P.coef + (size_t)row * NCs + per * threadIdx.x);
+            cp_async_commit();
+        }
+    }
     if (node >= P.n) return;
     const NodeIdx p = decompose(node, P.nx, P.ny);
     // gather addresses: one 64-bit pointer per direction (the source node's slot in its tile); the plane offset
@@ -108,7 +134,15 @@ collide_stream_node(const R* __restrict__ src, R* __restrict__ dst, const __grid
     // manufactured forcing while the gather is in flight: after the row/node split it is ~250 instructions on
     // ~40 registers, independent of the populations
     R smms[M];
-    if constexpr (MMS) mms_node<Sys, R>(P, p, smms);
+    if constexpr (MMS) {
+        if (staged) {
+            cp_async_wait_all();
+            __syncthreads();
+            mms_node<Sys, R, true>(P, p, coef_s, smms);
+        } else {
+            mms_node<Sys, R, false>(P, p, nullptr, smms);
+        }
+    }
     R dQ[M];
 #pragma unroll
     for (int k = 0; k < M; ++k) {
@@ -154,7 +188,7 @@ collide_stream_twopass(const R* __restrict__ src, R* __restrict__ dst, const __g
     if (node >= P.n) return;
     const NodeIdx p = decompose(node, P.nx, P.ny);
     R smms[M];
-    if constexpr (MMS) mms_node<Sys, R>(P, p, smms);
+    if constexpr (MMS) mms_node<Sys, R, false>(P, p, nullptr, smms);
     const R* sp[Q];
 #pragma unroll
     for (int i = 0; i < Q; ++i)

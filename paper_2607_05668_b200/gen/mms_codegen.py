@@ -425,7 +425,7 @@ def _emit_source_row(sr, pr: _Printer, indent="        "):
                 i = int(n[1:])
                 if i // 4 not in loaded:
                     loaded.add(i // 4)
-                    lines.append(f"{indent}const Vec4<R> q{i // 4} = ld4(c + {4 * (i // 4)});")
+                    lines.append(f"{indent}const Vec4<R> q{i // 4} = ld4<SH>(c + {4 * (i // 4)});")
                 names[s_] = sp.Symbol(f"q{i // 4}.{'xyzw'[i % 4]}", real=True)
         return e.xreplace(names)
 
@@ -537,7 +537,7 @@ def emit_system(g) -> str:
         o.append(f"        c[{i}] = (RO)0;")
     o.append("    }")
     o.append("    // per-node remainder: s_k = sum_j C_kj * monomial_j(X, 1/rho..); c = this row's coefficients (32-byte aligned)")
-    o.append("    template <class R>")
+    o.append("    template <class R, bool SH>")
     o.append("    static __device__ __forceinline__ void source_row(const R* __restrict__ c, const R* X, R* s) {")
     o.append("        (void)c; (void)X;")
     for i in range(nx_):
@@ -575,12 +575,14 @@ template <class R> struct MmsArgs { R par[8]; R mp[8]; R dx, dt, il, gtau; };
 // four consecutive row coefficients, loaded with 128-bit read-only loads (all threads of a block read the same row)
 template <class R> struct Vec4 { R x, y, z, w; };
 #ifdef __CUDACC__
-__device__ __forceinline__ Vec4<float> ld4(const float* p) {
-    const float4 v = __ldg(reinterpret_cast<const float4*>(p));
+// SH: p points into shared memory (plain vector load -> LDS.128); otherwise read-only global load
+template <bool SH> __device__ __forceinline__ Vec4<float> ld4(const float* p) {
+    const float4 v = SH ? *reinterpret_cast<const float4*>(p) : __ldg(reinterpret_cast<const float4*>(p));
     return Vec4<float>{v.x, v.y, v.z, v.w};
 }
-__device__ __forceinline__ Vec4<double> ld4(const double* p) {
-    const double2 a = __ldg(reinterpret_cast<const double2*>(p)), b = __ldg(reinterpret_cast<const double2*>(p) + 1);
+template <bool SH> __device__ __forceinline__ Vec4<double> ld4(const double* p) {
+    const double2* q = reinterpret_cast<const double2*>(p);
+    const double2 a = SH ? q[0] : __ldg(q), b = SH ? q[1] : __ldg(q + 1);
     return Vec4<double>{a.x, a.y, b.x, b.y};
 }
 #endif
