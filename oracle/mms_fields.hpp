@@ -9,6 +9,8 @@
 //   adr2d     mms 1 : eq (SM5.7), Table SM8
 //   swe2d     mms 1 : BASELINE.json configs[1] fields, mms_par = {A_h, A_u, h0}
 //   nsf3d     mms 1 : BASELINE.json configs[3] fields, mms_par = {U0, A_rho, rho0, p0}
+//   urf2d     mms 1 : eq (SM5.4)
+//   maxwell2d mms 1 : eq (SM5.5), PAPER.md:L1248-L1254 (k_x = 2 pi, k_y = 4 pi, A = 1/2, omega = 4)
 #pragma once
 #include "jets.hpp"
 #include "systems.hpp"
@@ -73,6 +75,19 @@ inline bool exact_state(int sys, int mms_id, const Scaling& sc, const double* mp
         for (int a = 0; a < 3; ++a)
             for (int b = 0; b < 3; ++b) Q[5 + 3 * a + b] = sc.dx * diff(u[a], 1 + b);
         for (int b = 0; b < 3; ++b) Q[14 + b] = sc.dx * diff(Tm, 1 + b);
+        return true;
+    }
+    case SYS_URF2D: {
+        Q[0] = lower(0.4 * sin(k * x) * sin(k * y) * cos(t) + 3.0);
+        Q[1] = lower(0.4 * cos(k * x) * cos(k * y) * sin(t) + 1.2);
+        Q[2] = lower(0.4 * sin(k * x) * sin(k * y) * sin(t) + 1.2);
+        return true;
+    }
+    case SYS_MAXWELL2D: {
+        const double A = 0.5, kx = 2.0 * PI, ky = 4.0 * PI, om = 4.0;
+        Q[0] = lower(A * sin(kx * x) * sin(ky * y) * cos(om * t));
+        Q[1] = lower(A * sin(kx * x) * cos(ky * y) * sin(om * t));
+        Q[2] = lower((-A * kx / ky) * cos(kx * x) * sin(ky * y) * sin(om * t));
         return true;
     }
     }

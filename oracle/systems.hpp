@@ -17,7 +17,7 @@
 namespace orc {
 
 enum SystemId { SYS_ADVECTION2D = 0, SYS_BURGERS2D = 1, SYS_SWE2D = 2, SYS_EULER2D = 3, SYS_ADR2D = 4,
-                SYS_NSF3D = 5, SYS_MHD3D = 6, SYS_COUNT = 7 };
+                SYS_NSF3D = 5, SYS_MHD3D = 6, SYS_URF2D = 7, SYS_MAXWELL2D = 8, SYS_COUNT = 9 };
 
 constexpr int MAXM = 32;  // max components
 
@@ -31,6 +31,8 @@ inline SysInfo sys_info(int sys) {
         case SYS_ADR2D:       return {1, 3, 2};
         case SYS_NSF3D:       return {5, 17, 3};
         case SYS_MHD3D:       return {8, 11, 3};
+        case SYS_URF2D:       return {3, 3, 2};
+        case SYS_MAXWELL2D:   return {3, 3, 2};
     }
     return {0, 0, 0};
 }
@@ -171,6 +173,25 @@ void flux_source(int sys, const T* U, const Scaling& sc, T* F, T* S) {
         }
         for (int i = 0; i < 3; ++i) S[8 + i] = -J[i] / sc.g_tau;
     } break;
+    case SYS_URF2D: {
+        // ideal ultrarelativistic fluid, eq (3.7)-(3.9): Q = (E, S), Phi = (S, S (x) v + p I),
+        // p = (sqrt(4E^2 - 3|S|^2) - E)/3, v = S/(E + p); natural units c = 1; no parameters
+        using std::sqrt;
+        T E = U[0], Sx = U[1], Sy = U[2];
+        T p = (sqrt(4.0 * E * E - 3.0 * (Sx * Sx + Sy * Sy)) - E) / 3.0;
+        T vx = Sx / (E + p), vy = Sy / (E + p);
+        F[0 * 3 + 0] = il * Sx;             F[0 * 3 + 1] = il * Sy;
+        F[1 * 3 + 0] = il * (Sx * vx + p);  F[1 * 3 + 1] = il * (Sx * vy);
+        F[2 * 3 + 0] = il * (Sy * vx);      F[2 * 3 + 1] = il * (Sy * vy + p);
+    } break;
+    case SYS_MAXWELL2D: {
+        // Maxwell TM mode in vacuum, eq (3.10)-(3.11): Q = (E_z, H_x, H_y); par = {c}
+        const double c = sc.par[0];
+        T Ez = U[0], Hx = U[1], Hy = U[2];
+        F[0 * 3 + 0] = (-c * il) * Hy;      F[0 * 3 + 1] = (c * il) * Hx;
+        F[1 * 3 + 0] = T(0.0);              F[1 * 3 + 1] = (c * il) * Ez;
+        F[2 * 3 + 0] = (-c * il) * Ez;      F[2 * 3 + 1] = T(0.0);
+    } break;
     }
 }
 
@@ -219,6 +240,24 @@ inline void wave_speeds(int sys, const double* U, const Scaling& sc, double* out
         out[1] = std::sqrt(u[0] * u[0] + u[1] * u[1] + u[2] * u[2]) + std::sqrt(a2 + b2);
         out[2] = std::sqrt(sc.par[1] * dL / sc.g_tau);
     } break;
+    case SYS_URF2D: {
+        // barotropic relativistic Euler with c_s^2 = 1/3: along a unit vector n the acoustic
+        // characteristic speeds are [v_n (1 - cs2) +- cs sqrt((1 - v^2)(1 - v^2 cs2 - v_n^2 (1 - cs2)))] / (1 - v^2 cs2)
+        // (relativistic velocity addition of the flow and the sound speed); the largest over all n is the
+        // collinear sum (|v| + cs)/(1 + |v| cs).
+        const double cs2 = 1.0 / 3.0, cs = std::sqrt(cs2);
+        const double p = (std::sqrt(4.0 * U[0] * U[0] - 3.0 * (U[1] * U[1] + U[2] * U[2])) - U[0]) / 3.0;
+        const double v[2] = {U[1] / (U[0] + p), U[2] / (U[0] + p)};
+        const double v2 = v[0] * v[0] + v[1] * v[1];
+        for (int a = 0; a < 2; ++a) {
+            const double vn = std::fabs(v[a]);
+            const double lam = (vn * (1.0 - cs2) + cs * std::sqrt(std::fmax((1.0 - v2) * (1.0 - v2 * cs2 - vn * vn * (1.0 - cs2)), 0.0))) / (1.0 - v2 * cs2);
+            out[0] = std::fmax(out[0], lam);
+        }
+        const double vm = std::sqrt(v2);
+        out[1] = (vm + cs) / (1.0 + vm * cs);
+    } break;
+    case SYS_MAXWELL2D: { out[0] = std::fabs(sc.par[0]); out[1] = std::fabs(sc.par[0]); } break;  // eigenvalues {+c, -c, 0}, L393
     }
 }
 

@@ -57,11 +57,13 @@ static const SysOps* ops_of(int id) {
         case LBMK_SYS_ADR2D: return ops_adr2d();
         case LBMK_SYS_NSF3D_GRADTRACK: return ops_nsf3d();
         case LBMK_SYS_MHD3D_JTRACK: return ops_mhd3d();
+        case LBMK_SYS_URF2D: return ops_urf2d();
+        case LBMK_SYS_MAXWELL2D: return ops_maxwell2d();
     }
     return nullptr;
 }
-static const int N_PARAMS[LBMK_SYS_COUNT] = {2, 0, 1, 1, 4, 3, 2};
-static const int N_MMS_PARAMS[LBMK_SYS_COUNT] = {0, 1, 3, 0, 0, 4, 0};
+static const int N_PARAMS[LBMK_SYS_COUNT] = {2, 0, 1, 1, 4, 3, 2, 0, 1};
+static const int N_MMS_PARAMS[LBMK_SYS_COUNT] = {0, 1, 3, 0, 0, 4, 0, 0, 0};
 
 static lbmk_status sys_fail(lbmk_status s, const char* msg) { g_sys_err = msg; return s; }
 static lbmk_status fail(lbmk_grid* g, lbmk_status s, const std::string& msg) { if (g) g->err = msg; else g_sys_err = msg; return s; }
@@ -212,6 +214,13 @@ static void derive_params(lbmk_grid* g) {
             for (int a = 0; a < 2; ++a) { P.cst[a] = r[0] != 0.0 ? r[1 + a] / r[0] : 0.0; ke += r[1 + a] * P.cst[a]; }
             P.cst[3] = (s.par[0] - 1.0) * (r[3] - 0.5 * ke);
             P.cst[4] = r[3] + P.cst[3];
+        } break;
+        case LBMK_SYS_URF2D: {
+            const double D0 = 4.0 * r[0] * r[0] - 3.0 * (r[1] * r[1] + r[2] * r[2]);
+            P.cst[2] = D0 > 0.0 ? std::sqrt(D0) : 0.0;
+            P.cst[4] = 2.0 * r[0] + P.cst[2];
+            P.cst[3] = (P.cst[2] - r[0]) / 3.0;
+            for (int a = 0; a < 2; ++a) P.cst[a] = P.cst[4] != 0.0 ? 3.0 * r[1 + a] / P.cst[4] : 0.0;
         } break;
         case LBMK_SYS_NSF3D_GRADTRACK:
         case LBMK_SYS_MHD3D_JTRACK:

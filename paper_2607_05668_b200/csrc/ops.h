@@ -62,5 +62,7 @@ const SysOps* ops_euler2d();
 const SysOps* ops_adr2d();
 const SysOps* ops_nsf3d();
 const SysOps* ops_mhd3d();
+const SysOps* ops_urf2d();
+const SysOps* ops_maxwell2d();
 
 }  // namespace lbmk

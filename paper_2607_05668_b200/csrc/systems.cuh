@@ -8,6 +8,7 @@
 // Host-derived reference constants arrive in KParams::cst (filled by derive_constants in lbmk_api.cu):
 //   hydrodynamic systems  cst[0..2] = u0 = m0/rho0,  cst[3] = p0,  cst[4] = E0 + p0,  cst[5] = T0 = p0/rho0
 //   SWE                   cst[0..1] = u0 = m0/h0
+//   ultrarelativistic     cst[0..1] = v0,  cst[2] = sqrt(D0),  cst[3] = p0,  cst[4] = W0 = 2 E0 + sqrt(D0)
 // Trackers are in lattice units G^L = dx grad V: F_G[b][j] = G_b u_j/lambda - delta_jb V/g_tau,
 // s_G = -G/g_tau (eq 2.3; tau_grad = g_tau dt, L106); a physical diffusivity D enters the
 // parent's flux as D_L = D dt/dx^2.
@@ -22,7 +23,8 @@
 
 namespace lbmk {
 
-enum { SYS_ADVECTION2D = 0, SYS_BURGERS2D = 1, SYS_SWE2D = 2, SYS_EULER2D = 3, SYS_ADR2D = 4, SYS_NSF3D = 5, SYS_MHD3D = 6 };
+enum { SYS_ADVECTION2D = 0, SYS_BURGERS2D = 1, SYS_SWE2D = 2, SYS_EULER2D = 3, SYS_ADR2D = 4, SYS_NSF3D = 5, SYS_MHD3D = 6,
+       SYS_URF2D = 7, SYS_MAXWELL2D = 8 };
 
 // ------------------------------------------------------------------------------------------ advection
 // Phi = (a_x U, a_y U); par = {a_x, a_y}
@@ -312,6 +314,86 @@ template <class R> struct SysMhd3D {
         out[0] = m0;
         out[1] = sqrt(u2) + sqrt(a2 + b2);
         out[2] = sqrt(P.par[1] * P.dL * P.inv_gtau);
+    }
+};
+
+// ------------------------------------------------------------------------------------------ ultrarelativistic fluid
+// eq (3.7)-(3.9): Q = (E, S_x, S_y), Phi_E = S, Phi_S = S (x) v + p I,
+// p = (sqrt(D) - E)/3, D = 4E^2 - 3|S|^2, v = S/(E + p) = 3 S/W, W = 2E + sqrt(D); c = 1, no parameters.
+// Delta form about (E0, S0): dD = 4 (2 E0 + dE) dE - 3 sum_a (2 S0a + dSa) dSa,  d sqrtD = dD/(sqrtD + sqrtD0),
+// dp = (d sqrtD - dE)/3,  dW = 2 dE + d sqrtD,  dv_b = 3 (dS_b W0 - S0b dW)/(W W0),
+// d(S_a v_b) = dS_a v_b + S0a dv_b.  With Q0 = 0 the reference constants vanish and this is the plain flux
+// (sqrtD0 = W0 = 0 is handled by taking dv = v).
+template <class R> struct SysUrf2D {
+    static constexpr int ID = SYS_URF2D, D = 2, M = 3, MC = 3;
+    using Mms = Mms_urf2d;
+    struct Ctx { R v[2], dv[2], dp; };
+    __device__ __forceinline__ static void setup(Ctx& c, const R (&dQ)[M], const KParams<R>& P) {
+        const R E0 = P.ref[0], E = E0 + dQ[0];
+        const R Sx = P.ref[1] + dQ[1], Sy = P.ref[2] + dQ[2];
+        const R sD = sqrt(R(4) * E * E - R(3) * (Sx * Sx + Sy * Sy));
+        const R W = R(2) * E + sD, iW = R(3) / W;
+        c.v[0] = Sx * iW; c.v[1] = Sy * iW;
+        const R sD0 = P.cst[2], W0 = P.cst[4];
+        if (W0 != R(0)) {
+            const R dD = R(4) * (R(2) * E0 + dQ[0]) * dQ[0] - R(3) * ((R(2) * P.ref[1] + dQ[1]) * dQ[1] + (R(2) * P.ref[2] + dQ[2]) * dQ[2]);
+            const R dsD = dD / (sD + sD0);
+            c.dp = (dsD - dQ[0]) * R(1.0 / 3.0);
+            const R dW = R(2) * dQ[0] + dsD, k = iW / W0;
+            c.dv[0] = (dQ[1] * W0 - P.ref[1] * dW) * k;
+            c.dv[1] = (dQ[2] * W0 - P.ref[2] * dW) * k;
+        } else {
+            c.dp = (sD - E) * R(1.0 / 3.0);
+            c.dv[0] = c.v[0]; c.dv[1] = c.v[1];
+        }
+    }
+    template <int k> __device__ __forceinline__ static void flux(const Ctx& c, const R (&dQ)[M], const KParams<R>& P, R (&F)[D], R& S) {
+        S = R(0);
+        if constexpr (k == 0) {
+            F[0] = P.il * dQ[1]; F[1] = P.il * dQ[2];
+        } else {
+            constexpr int a = k - 1;
+#pragma unroll
+            for (int b = 0; b < 2; ++b) {
+                R h = dQ[1 + a] * c.v[b] + P.ref[1 + a] * c.dv[b];
+                if (a == b) h += c.dp;
+                F[b] = P.il * h;
+            }
+        }
+    }
+    __device__ static void wave(const double* Q, const KParams<double>& P, double* out) {
+        const double cs2 = 1.0 / 3.0, cs = sqrt(cs2);
+        const double p = (sqrt(4.0 * Q[0] * Q[0] - 3.0 * (Q[1] * Q[1] + Q[2] * Q[2])) - Q[0]) / 3.0;
+        const double v[2] = {Q[1] / (Q[0] + p), Q[2] / (Q[0] + p)};
+        const double v2 = v[0] * v[0] + v[1] * v[1];
+        out[0] = 0.0;
+        for (int a = 0; a < 2; ++a) {
+            const double vn = fabs(v[a]);
+            out[0] = fmax(out[0], (vn * (1.0 - cs2) + cs * sqrt(fmax((1.0 - v2) * (1.0 - v2 * cs2 - vn * vn * (1.0 - cs2)), 0.0))) / (1.0 - v2 * cs2));
+        }
+        const double vm = sqrt(v2);
+        out[1] = (vm + cs) / (1.0 + vm * cs);
+        out[2] = 0.0;
+    }
+};
+
+// ------------------------------------------------------------------------------------------ Maxwell TM
+// eq (3.10)-(3.11): Q = (E_z, H_x, H_y), Phi = c ((-H_y, H_x), (0, E_z), (-E_z, 0)); par = {c}.
+// Linear: the delta form is the flux itself.
+template <class R> struct SysMaxwell2D {
+    static constexpr int ID = SYS_MAXWELL2D, D = 2, M = 3, MC = 3;
+    using Mms = Mms_maxwell2d;
+    struct Ctx {};
+    __device__ __forceinline__ static void setup(Ctx&, const R (&)[M], const KParams<R>&) {}
+    template <int k> __device__ __forceinline__ static void flux(const Ctx&, const R (&dQ)[M], const KParams<R>& P, R (&F)[D], R& S) {
+        const R cl = P.par[0] * P.il;
+        S = R(0);
+        if constexpr (k == 0) { F[0] = -cl * dQ[2]; F[1] = cl * dQ[1]; }
+        else if constexpr (k == 1) { F[0] = R(0); F[1] = cl * dQ[0]; }
+        else { F[0] = -cl * dQ[0]; F[1] = R(0); }
+    }
+    __device__ static void wave(const double*, const KParams<double>& P, double* out) {
+        out[0] = fabs(P.par[0]); out[1] = fabs(P.par[0]); out[2] = 0.0;    // eigenvalues {+c, -c, 0}
     }
 };
 

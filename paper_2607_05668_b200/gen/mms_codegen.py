@@ -158,7 +158,40 @@ def sys_nsf3d():
     return "nsf3d", 3, prim, build
 
 
-SYSTEMS = [sys_burgers2d, sys_swe2d, sys_euler2d, sys_adr2d, sys_nsf3d]
+def sys_urf2d():
+    k = TWO_PI
+    prim = {"E": sp.Rational(2, 5) * sp.sin(k * x) * sp.sin(k * y) * sp.cos(t) + 3,          # eq SM5.4
+            "Sx": sp.Rational(2, 5) * sp.cos(k * x) * sp.cos(k * y) * sp.sin(t) + sp.Rational(6, 5),
+            "Sy": sp.Rational(2, 5) * sp.sin(k * x) * sp.sin(k * y) * sp.sin(t) + sp.Rational(6, 5)}
+
+    def build(P, D):
+        E, Sx, Sy = P["E"], P["Sx"], P["Sy"]
+        p = (sp.sqrt(4 * E * E - 3 * (Sx * Sx + Sy * Sy)) - E) / 3                             # eq 3.9
+        vx, vy = Sx / (E + p), Sy / (E + p)
+        Q = [E, Sx, Sy]
+        F = [[il * Sx, il * Sy],                                                                # eq 3.8
+             [il * (Sx * vx + p), il * Sx * vy],
+             [il * Sy * vx, il * (Sy * vy + p)]]
+        return Q, F, [sp.Integer(0)] * 3
+    return "urf2d", 2, prim, build
+
+
+def sys_maxwell2d():
+    c = par(0)
+    kx, ky, om, A = TWO_PI, 2 * TWO_PI, 4, sp.Rational(1, 2)                                    # eq SM5.5
+    prim = {"Ez": A * sp.sin(kx * x) * sp.sin(ky * y) * sp.cos(om * t),
+            "Hx": A * sp.sin(kx * x) * sp.cos(ky * y) * sp.sin(om * t),
+            "Hy": -A * (kx / ky) * sp.cos(kx * x) * sp.sin(ky * y) * sp.sin(om * t)}
+
+    def build(P, D):
+        Ez, Hx, Hy = P["Ez"], P["Hx"], P["Hy"]
+        Q = [Ez, Hx, Hy]
+        F = [[-c * il * Hy, c * il * Hx], [sp.Integer(0), c * il * Ez], [-c * il * Ez, sp.Integer(0)]]   # eq 3.11
+        return Q, F, [sp.Integer(0)] * 3
+    return "maxwell2d", 2, prim, build
+
+
+SYSTEMS = [sys_burgers2d, sys_swe2d, sys_euler2d, sys_adr2d, sys_nsf3d, sys_urf2d, sys_maxwell2d]
 
 
 # ------------------------------------------------------------------------------------------------ printing
@@ -189,8 +222,13 @@ class _Printer(C99CodePrinter):
             if n > 1:
                 s = f"({s})"
             return f"({self._lit('1.0')}/{s})" if int(ex) < 0 else s
-        if ex == sp.Rational(1, 2):
-            return f"sqrt({self._print(b)})"
+        if ex.is_Rational and ex.q == 2 and abs(int(ex.p)) <= 9:                # half-integer powers via sqrt
+            n = abs(int(ex.p)) // 2
+            root = f"sqrt({self._print(b)})"
+            s = "*".join([self.parenthesize(b, 60)] * n + [root])
+            if n > 0:
+                s = f"({s})"
+            return f"({self._lit('1.0')}/{s})" if ex.p < 0 else s
         raise ValueError(f"unsupported power {e}")
 
 
@@ -334,6 +372,28 @@ def _emit_body(assign: List[Tuple[sp.Symbol, sp.Expr]], outputs: List[sp.Expr], 
 # evaluates the C_kj once per (y, z) row and step (a tiny pre-kernel, in fp64); `source_row` is what is left
 # per node: a few monomials and one FMA per term.
 def split_rows(g):
+    """Polynomial row/node split; for residuals that are not polynomial in the x-atoms (the ultrarelativistic
+    fluid's sqrt) the split degenerates to: row coefficients = the row-uniform table atoms Y#, Z#, T# themselves,
+    node code = the direct CSE'd residual reading them from the row table."""
+    try:
+        return _split_rows_poly(g)
+    except (sp.PolynomialError, AssertionError):
+        return _split_rows_direct(g)
+
+
+def _split_rows_direct(g):
+    d = dict(g["layer1"])
+    outs = [e.xreplace(d) for e in g["res"]]              # closed forms inlined; CSE'd as a whole by _emit_source_row
+    free = set()
+    for e in outs:
+        free |= e.free_symbols
+    is_x = lambda s_: str(s_)[0] == "X" and str(s_)[1:].isdigit()
+    uni = sorted([s_ for s_ in free if not is_x(s_)], key=str)   # Y#, Z#, T# atoms and the scalars (il, dt, par#, ...)
+    C = {u: sp.Symbol(f"C{i}", real=True) for i, u in enumerate(uni)}
+    return dict(coefs=uni, node_defs=[], outs=[e.xreplace(C) for e in outs], n_terms=0, direct=True)
+
+
+def _split_rows_poly(g):
     xs = [sp.Symbol(f"X{i}", real=True) for i in range(len(g["tabs"][x]))]
     xset = set(xs)
     l1 = dict(g["layer1"])

@@ -45,6 +45,24 @@ def flux_adr_listing(U, u0, u1, D, tau_grad):
     return Phi
 
 
+def flux_urf_listing(U):
+    """SM4.4, PAPER.md:L849 (ideal ultrarelativistic fluid, expanded component form)."""
+    E, S0, S1 = U
+    z = np.zeros_like(E)
+    root = np.sqrt(4 * E**2 - 3 * S0**2 - 3 * S1**2)
+    P10 = -E / 3 + 3 * S0**2 / (2 * E + root) + root / 3
+    P11 = 3 * S0 * S1 / (2 * E + root)
+    P21 = -E / 3 + 3 * S1**2 / (2 * E + root) + root / 3
+    return [[S0, S1, z], [P10, P11, z], [P11, P21, z]]
+
+
+def flux_maxwell_listing(U, c):
+    """SM4.5, PAPER.md:L861 (Maxwell TM)."""
+    Ez, Hx, Hy = U
+    z = np.zeros_like(Ez)
+    return [[-Hy * c, Hx * c, z], [z, Ez * c, z], [-Ez * c, z, z]]
+
+
 def step(f, dim, omega, F_lat, S_lat):
     """One collide-and-stream step.
     f[k][i] : arrays (nz, ny, nx);  F_lat[k][a], S_lat[k] : lattice flux / source arrays at the

@@ -1,0 +1,87 @@
+"""GPU parity of the paper systems added beyond the five BASELINE.json configs: the ideal
+ultrarelativistic fluid (eq 3.7-3.9; MMS eq SM5.4) and Maxwell TM (eq 3.10-3.11,
+L385-L391; MMS eq SM5.5), at the paper's working point (Table SM2: f = 0.2, tau_R = 0.2)."""
+import numpy as np
+import pytest
+
+import oracle
+import workloads as W
+from parity_metric import rel_err
+
+pytestmark = pytest.mark.gpu
+TOL64, TOL32 = 1e-12, 2e-5
+
+
+@pytest.fixture(scope="module")
+def P():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device")
+    import paper_2607_05668_b200 as P
+    P.lib()
+    return P
+
+
+def _pair(P, w, steps, **kw):
+    U0 = w.initial_U()
+    g = P.Grid.from_workload(w, **kw)
+    g.init_from_U(U0)
+    g.step(steps)
+    U, f, ws = g.read_U(), g.read_populations(), g.max_wave_speed()
+    g.close()
+    o = oracle.OracleGrid.from_workload(w)
+    o.init_from_U(U0)
+    o.step(steps)
+    Uo, fo, wo = o.read_U(), o.read_f(), o.max_wave_speed()
+    o.close()
+    return U, f, Uo, fo, ws, wo
+
+
+@pytest.mark.parametrize("pattern", ["pull2", "aa"])
+@pytest.mark.parametrize("mk,n,steps", [(W.pin_urf, 48, 121), (W.pin_maxwell, 40, 150), (W.pin_urf, 256, 24), (W.pin_maxwell, 256, 25)])
+@pytest.mark.parametrize("precision", ["f64", "f64s"])
+def test_parity_fp64(P, mk, n, steps, pattern, precision):
+    """n = 256 takes the staged-coefficient path (nx a multiple of the block size), the small grids the global one."""
+    w = mk(n)
+    U, f, Uo, fo, ws, wo = _pair(P, w, steps, precision=precision, pattern=pattern)
+    tol = TOL64 if precision == "f64" else 1e-11
+    assert rel_err(U, Uo, fo).max() <= tol
+    assert np.abs(f - fo).max() / np.abs(fo).max() <= tol
+    for a, b in zip(ws[0], wo):
+        assert a == pytest.approx(b, rel=1e-10, abs=1e-15)
+    assert ws[1] == 0
+
+
+@pytest.mark.parametrize("pattern", ["pull2", "aa"])
+@pytest.mark.parametrize("mk,n,steps", [(W.pin_urf, 64, 320), (W.pin_maxwell, 64, 320), (W.pin_urf, 256, 60)])
+def test_parity_fp32_shifted(P, mk, n, steps, pattern):
+    """Reference- and equilibrium-shifted fp32 (eq 2.23) to t = 1 on the 64^2 grid of the paper's study."""
+    w = mk(n, precision="f32s")
+    U, f, Uo, fo, _, _ = _pair(P, w, steps, pattern=pattern)
+    e = rel_err(U, Uo, fo)
+    assert np.isfinite(U).all() and e.max() <= TOL32, f"{w.name} {e}"
+
+
+def test_fp32_convergence_order_retained(P):
+    """north_star: "the fp32 convergence order retained": relative L2 error against the exact fields at t = 1 on
+    N = 32, 64, 128 in shifted fp32; the slope stays within 0.5 of the fp64 oracle's (paper: L567)."""
+    for mk in (W.pin_urf, W.pin_maxwell):
+        err32, err64 = [], []
+        for n in (32, 64, 128):
+            w = mk(n, precision="f32s")
+            g = P.Grid.from_workload(w)
+            g.init_from_U(w.initial_U())
+            g.step(w.steps)
+            U = g.read_U()
+            g.close()
+            o = oracle.OracleGrid.from_workload(w)
+            o.init_from_U(w.initial_U())
+            o.step(w.steps)
+            Uo, Ue = o.read_U(), o.exact_U(w.steps * w.dt)
+            o.close()
+            l2 = lambda A: float(np.sqrt(((A[0] - Ue[0]) ** 2).sum() / (Ue[0] ** 2).sum()))
+            err32.append(l2(U)); err64.append(l2(Uo))
+        ns = np.log2([32, 64, 128])
+        s32 = -np.polyfit(ns, np.log2(err32), 1)[0]
+        s64 = -np.polyfit(ns, np.log2(err64), 1)[0]
+        assert 1.7 <= s64 <= 2.51 and abs(s32 - s64) <= 0.5, (mk.__name__, s32, s64, err32, err64)

@@ -22,7 +22,7 @@ import workloads as W
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 PINS = json.load(open(os.path.join(HERE, "golden", "paper_pins.json")))
-MAKERS = {"burgers": W.pin_burgers, "euler": W.pin_euler, "adr": W.pin_adr}
+MAKERS = {"burgers": W.pin_burgers, "euler": W.pin_euler, "adr": W.pin_adr, "urf": W.pin_urf, "maxwell": W.pin_maxwell}
 
 
 def _rows(case):
@@ -70,6 +70,10 @@ def test_p8_live_n64_matches_stored_row(case):
         live = {"u": e[0]}
     elif case == "euler":
         live = {"rho": e[0], "E": e[3], "rhou": (math.hypot(e[1][0], e[2][0]), math.hypot(e[1][1], e[2][1]))}
+    elif case == "urf":
+        live = {"E": e[0], "S": (math.hypot(e[1][0], e[2][0]), math.hypot(e[1][1], e[2][1]))}
+    elif case == "maxwell":
+        live = {"Ez": e[0], "Hx": e[1], "Hy": e[2]}
     else:
         live = {"c": e[0]}
     for field, (linf, l2) in stored.items():

@@ -13,12 +13,12 @@ import oracle
 import workloads as W
 from oracle import OracleGrid
 
-from brute_force import (LATTICES, flux_adr_listing, flux_euler_listing, flux_swe_listing,
+from brute_force import (LATTICES, flux_adr_listing, flux_euler_listing, flux_maxwell_listing, flux_swe_listing, flux_urf_listing,
                          init_equilibrium, moments, step as bf_step)
 
-SYSTEMS = ["advection2d", "burgers2d", "swe2d", "euler2d", "adr2d", "nsf3d", "mhd3d"]
+SYSTEMS = ["advection2d", "burgers2d", "swe2d", "euler2d", "adr2d", "nsf3d", "mhd3d", "urf2d", "maxwell2d"]
 PARAMS = {"advection2d": [0.1, 0.05], "burgers2d": [], "swe2d": [1.0], "euler2d": [1.4],
-          "adr2d": [0.1, -0.1, 0.01, 1.0], "nsf3d": [1.4, 1e-3, 4.9e-3], "mhd3d": [1.4, 1e-3]}
+          "adr2d": [0.1, -0.1, 0.01, 1.0], "nsf3d": [1.4, 1e-3, 4.9e-3], "mhd3d": [1.4, 1e-3], "urf2d": [], "maxwell2d": [1.0]}
 
 
 def small_grid(system, **kw):
@@ -41,6 +41,8 @@ def physical_state(system, rng, shape=()):
         U[4] = rng.uniform(2.0, 3.0, size=shape)
     if system in ("advection2d", "burgers2d", "adr2d"):
         U[0] = rng.uniform(0.2, 0.9, size=shape)
+    if system == "urf2d":                       # physicality E > |S|
+        U[0] = rng.uniform(1.0, 2.0, size=shape)
     return U
 
 
@@ -265,6 +267,8 @@ MMS_CASES = {
     "adr2d": lambda: W.pin_adr(32),
     "swe2d": lambda: W.c2_swe(32),
     "nsf3d": lambda: W.c4_nsf3d(16),
+    "urf2d": lambda: W.pin_urf(32),
+    "maxwell2d": lambda: W.pin_maxwell(32),
 }
 
 
@@ -396,6 +400,62 @@ def test_p13_brute_force_adr_tracker():
     w.steps = 12
     exp = _bf_run("adr2d", w, w.steps, None)
     assert np.abs(oracle.run(w) - exp).max() < 1e-14
+
+
+def test_p13_brute_force_ultrarelativistic():
+    w = W.pin_urf(8)
+    w.mms_id = 0
+    w.steps = 12
+    exp = _bf_run("urf2d", w, w.steps, flux_urf_listing)
+    assert np.abs(oracle.run(w) - exp).max() < 1e-14
+
+
+def test_p13_brute_force_maxwell():
+    w = W.pin_maxwell(8)
+    w.mms_id = 0
+    w.steps = 12
+    U0 = w.initial_U()
+    U0[1] = 0.3 * np.roll(U0[0], 2, axis=2); U0[2] = -0.2 * np.roll(U0[0], 1, axis=1)     # non-trivial H
+    w.init = lambda _w: U0
+    exp = _bf_run("maxwell2d", w, w.steps, lambda U: flux_maxwell_listing(U, w.params[0]))
+    assert np.abs(oracle.run(w) - exp).max() < 1e-14
+
+
+def test_maxwell_wave_equation_dispersion():
+    """Eliminating H gives the scalar wave equation d_tt E_z = c^2 lap E_z: an unforced standing TM
+    mode oscillates at omega = c |k| (closed form, independent of the scheme), up to the O(dx^2) scheme error."""
+    n = 64
+    w = W.pin_maxwell(n)
+    w.mms_id = 0
+    kx, ky = 2 * np.pi, 4 * np.pi
+    om = math.hypot(kx, ky)
+    T = 2 * np.pi / om                                  # one period
+    w.steps = int(round(T / w.dt))
+    U = oracle.run(w)
+    t = w.steps * w.dt
+    x = (np.arange(n) / n)[None, :]; y = (np.arange(n) / n)[:, None]
+    Ez = 0.5 * np.sin(kx * x) * np.sin(ky * y) * np.cos(om * t)
+    assert np.abs(U[0, 0] - Ez).max() < 2e-2 * 0.5
+
+
+def test_urf_and_maxwell_wave_speeds():
+    """Closed forms: fluid at rest => sound speed 1/sqrt(3); collinear relativistic addition for a
+    moving fluid; Maxwell eigenvalues +-c (L393)."""
+    g = OracleGrid("urf2d", 4, 4, 1, dx=0.25, lam=1.0, params=[])
+    U = np.zeros((3, 1, 4, 4)); U[0] = 2.0
+    g.init_from_U(U)
+    ax, iso, _ = g.max_wave_speed()
+    assert ax == pytest.approx(1 / math.sqrt(3)) and iso == pytest.approx(1 / math.sqrt(3))
+    v = 0.5                                              # S = (4/3) Gamma^2 e v, E = (4/3) Gamma^2 e - e/3 with p = e/3
+    G2 = 1 / (1 - v * v); e = 1.7
+    U[0] = 4 / 3 * G2 * e - e / 3; U[1] = 4 / 3 * G2 * e * v
+    g.init_from_U(U)
+    ax, iso, _ = g.max_wave_speed()
+    cs = 1 / math.sqrt(3)
+    assert ax == pytest.approx((v + cs) / (1 + v * cs)) and iso == pytest.approx((v + cs) / (1 + v * cs))
+    g = OracleGrid("maxwell2d", 4, 4, 1, dx=0.25, lam=2.0, params=[0.7])
+    g.init_from_U(np.ones((3, 1, 4, 4)))
+    assert g.max_wave_speed()[:2] == (pytest.approx(0.35), pytest.approx(0.35))
 
 
 @pytest.mark.parametrize("name", ["c4", "c5"])

@@ -37,11 +37,14 @@ COMPONENTS: Dict[str, List[str]] = {
               "Gxx", "Gxy", "Gxz", "Gyx", "Gyy", "Gyz", "Gzx", "Gzy", "Gzz",
               "Hx", "Hy", "Hz"],
     "mhd3d": ["rho", "mx", "my", "mz", "E", "Bx", "By", "Bz", "Jx", "Jy", "Jz"],
+    "urf2d": ["E", "Sx", "Sy"],
+    "maxwell2d": ["Ez", "Hx", "Hy"],
 }
 N_CONSERVED = {"advection2d": 1, "burgers2d": 1, "swe2d": 3, "euler2d": 4,
-               "adr2d": 1, "nsf3d": 5, "mhd3d": 8}
+               "adr2d": 1, "nsf3d": 5, "mhd3d": 8, "urf2d": 3, "maxwell2d": 3}
 LATTICE_OF = {"advection2d": "D2Q5", "burgers2d": "D2Q5", "swe2d": "D2Q5",
-              "euler2d": "D2Q5", "adr2d": "D2Q5", "nsf3d": "D3Q7", "mhd3d": "D3Q7"}
+              "euler2d": "D2Q5", "adr2d": "D2Q5", "nsf3d": "D3Q7", "mhd3d": "D3Q7",
+              "urf2d": "D2Q5", "maxwell2d": "D2Q5"}
 # c_s^2 per lattice, Table SM1; used only by the lambda rule below.
 CS2 = {"D2Q5": 1.0 / 3.0, "D3Q7": 1.0 / 4.0}
 SIGMA = 0.6  # lambda rule: lattice wave speed = SIGMA * c_s^2 (SURVEY.md §8(c) "lambda rule")
@@ -352,6 +355,40 @@ def pin_adr(n: int = 512, precision: str = "f64") -> Workload:
                     dx=dx, lam=dx / dt, params=[0.1, -0.1, 0.01, 1.0], tau_R=50.0, g_tau=6.0,
                     U_ref=[0.5, 0.0, 0.0], mms_id=1, mms_params=[], steps=int(round(1.0 / dt)),
                     s_max=0.1, seed=0, init=_init_adr, note="PAPER.md Table 2 L540")
+
+
+def _init_urf(w: Workload) -> np.ndarray:
+    # eq (SM5.4), PAPER.md:L1229-L1235 at t = 0 (cos t = 1, sin t = 0)
+    x, y, _ = _grid(w)
+    k = TWO_PI
+    E = 0.4 * np.sin(k * x) * np.sin(k * y) + 3.0
+    S = 1.2 + 0.0 * x * y
+    return np.stack([_full(w, E), _full(w, S), _full(w, S)]).copy()
+
+
+def pin_urf(n: int = 512, precision: str = "f64") -> Workload:
+    # ideal ultrarelativistic fluid; Table SM2: acoustic f = 0.2, tau_R = 0.2 (both precisions)
+    f = 0.2
+    return Workload(name=f"pin_urf2d_{n}", system="urf2d", nx=n, ny=n, nz=1, precision=precision,
+                    dx=1.0 / n, lam=1.0 / f, params=[], tau_R=0.2, g_tau=0.0, U_ref=[3.0, 1.2, 1.2], mms_id=1,
+                    mms_params=[], steps=int(round(n / f)), s_max=1.0, seed=0, init=_init_urf,
+                    note="PAPER.md Table 2 L527-L529 (signal speeds are bounded by c = 1)")
+
+
+def _init_maxwell(w: Workload) -> np.ndarray:
+    # eq (SM5.5), PAPER.md:L1248-L1254 at t = 0: E_z = A sin(kx x) sin(ky y), H = 0
+    x, y, _ = _grid(w)
+    Ez = 0.5 * np.sin(TWO_PI * x) * np.sin(2.0 * TWO_PI * y)
+    zero = 0.0 * x * y
+    return np.stack([_full(w, Ez), _full(w, zero), _full(w, zero)]).copy()
+
+
+def pin_maxwell(n: int = 512, precision: str = "f64", f: float = 0.2) -> Workload:
+    # Maxwell TM; Table SM2: acoustic f = 0.2, tau_R = 0.2; c = 1 (Table SM6)
+    return Workload(name=f"pin_maxwell2d_{n}", system="maxwell2d", nx=n, ny=n, nz=1, precision=precision,
+                    dx=1.0 / n, lam=1.0 / f, params=[1.0], tau_R=0.2, g_tau=0.0, U_ref=[0.0, 0.0, 0.0], mms_id=1,
+                    mms_params=[], steps=int(round(n / f)), s_max=1.0, seed=0, init=_init_maxwell,
+                    note="PAPER.md Table 2 L530-L535")
 
 
 BASELINE_CONFIGS: Dict[str, Callable[..., Workload]] = {
