@@ -161,6 +161,15 @@ lbmk_status lbmk_time(const lbmk_grid* g, long long* step, double* t);
  * Returns LBMK_ESUBCHAR if max(out3[0], out3[1]) + out3[2] > c_s.  out3 is a HOST pointer (may be NULL). */
 lbmk_status lbmk_check_subcharacteristic(lbmk_grid* g, double* out3);
 
+/* ---- convergence study -------------------------------------------------------- */
+
+/* Device reductions of the current state against the manufactured solution at the current time t0 + step*dt
+ * (needs mms_id != 0, else LBMK_EUNSUPPORTED).  out: HOST pointer to [m_total][6] doubles,
+ *   out[k] = { sum_x |e|, sum_x e^2, max_x |e|, sum_x |q|, sum_x q^2, max_x |q| },  e = U_k - Q_exact,k,  q = Q_exact,k,
+ * all in fp64 (exact fields from their closed forms).  The paper's relative norms (L504) are
+ * L1 = out[0]/out[3], L2 = sqrt(out[1]/out[4]), Linf = out[2]/out[5].  Synchronises. */
+lbmk_status lbmk_error_norms(lbmk_grid* g, double* out);
+
 /* ---- test hooks ------------------------------------------------------------------------------------- */
 
 /* For every node x: linear index of the node whose post-collision population `dir` arrives at x, i.e.

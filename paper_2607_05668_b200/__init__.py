@@ -62,6 +62,7 @@ SYMBOLS = {
     "lbmk_read_populations": (C.c_int, [_vp, _vp, C.c_int]),
     "lbmk_time": (C.c_int, [_vp, C.POINTER(C.c_longlong), _dp]),
     "lbmk_check_subcharacteristic": (C.c_int, [_vp, _dp]),
+    "lbmk_error_norms": (C.c_int, [_vp, _dp]),
     "lbmk_stream_index_map": (C.c_int, [_vp, C.c_int, _vp, C.c_int]),
     "lbmk_lattice_constants": (C.c_int, [C.c_int, C.POINTER(C.c_int), _dp, _dp]),
     "lbmk_grid_omega": (C.c_int, [_vp, _dp]),
@@ -222,6 +223,12 @@ def lbmk_check_subcharacteristic(grid_h, raise_on_violation: bool = True):
     return (float(out[0]), float(out[1]), float(out[2])), st
 
 
+def lbmk_error_norms(grid_h, m_total: int) -> np.ndarray:
+    out = np.zeros((m_total, 6))
+    _check(lib().lbmk_error_norms(grid_h, out.ctypes.data_as(_dp)), grid_h)
+    return out
+
+
 def lbmk_stream_index_map(grid_h, direction: int, ptr: int, on_device: bool):
     _check(lib().lbmk_stream_index_map(grid_h, direction, _vp(ptr), int(on_device)), grid_h)
 
@@ -379,6 +386,12 @@ class Grid:
 
     def max_wave_speed(self):
         return lbmk_check_subcharacteristic(self.h, raise_on_violation=False)
+
+    def error_norms(self):
+        """Relative (L1, L2, Linf) errors per component against the manufactured solution at the current time."""
+        o = lbmk_error_norms(self.h, self.system.m_total)
+        with np.errstate(divide="ignore", invalid="ignore"):
+            return np.stack([o[:, 0] / o[:, 3], np.sqrt(o[:, 1] / o[:, 4]), o[:, 2] / o[:, 5]], axis=1)
 
     def check_subcharacteristic(self):
         return lbmk_check_subcharacteristic(self.h, raise_on_violation=True)[0]

@@ -544,6 +544,22 @@ lbmk_status lbmk_check_subcharacteristic(lbmk_grid* g, double* out3) {
     return LBMK_OK;
 }
 
+lbmk_status lbmk_error_norms(lbmk_grid* g, double* out) {
+    lbmk_status s = need_inited(g);
+    if (s != LBMK_OK) return s;
+    if (!out) return fail(g, LBMK_EINVAL, "out is NULL");
+    GridCore& c = g->c;
+    if (!g->ops->has_mms || c.mms_id == 0) return fail(g, LBMK_EUNSUPPORTED, "error norms need a manufactured solution (lbmk_system_set_mms)");
+    const size_t bytes = (size_t)g->ops->M * 6 * sizeof(double);
+    Staging st;
+    CK(g, st.acquire(out, 0, bytes, false, c.stream), "stage norms");
+    CK(g, g->ops->error_norms(c, (double*)st.dev), "error_norms kernel");
+    CK(g, cudaMemcpyAsync(out, st.dev, bytes, cudaMemcpyDeviceToHost, c.stream), "cudaMemcpyAsync D2H");
+    CK(g, cudaStreamSynchronize(c.stream), "cudaStreamSynchronize");
+    CK(g, st.release(), "cudaFreeAsync");
+    return LBMK_OK;
+}
+
 lbmk_status lbmk_stream_index_map(lbmk_grid* g, int dir, long long* src_index_out, int on_device) {
     lbmk_status s = need_bound(g);
     if (s != LBMK_OK) return s;

@@ -52,6 +52,7 @@ struct SysOps {
     cudaError_t (*read_U)(GridCore&, double* U_dev);
     cudaError_t (*read_f)(GridCore&, double* f_dev);
     cudaError_t (*max_wave_speed)(GridCore&, double* out3_host);
+    cudaError_t (*error_norms)(GridCore&, double* out_dev /*[M][6], zeroed here*/);
     bool (*row_kernel_supported)(const GridCore&);
 };
 

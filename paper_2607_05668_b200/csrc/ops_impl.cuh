@@ -247,12 +247,28 @@ struct Ops {
         if (e != cudaSuccess) return e;
         return read_U(g, U);
     }
+    template <class R>
+    static cudaError_t norms_t(GridCore& g, double* out) {
+        cudaError_t e = cudaMemsetAsync(out, 0, (size_t)M * 6 * sizeof(double), g.stream);
+        if (e != cudaSuccess) return e;
+        const unsigned nb = (unsigned)std::min<long long>((g.n + 255) / 256, 148 * 4);
+        error_norms_kernel<Sd, R><<<nb, 256, 0, g.stream>>>((const R*)g.f[g.cur], out, g.n, g.nx, g.ny, g.nz, aa_odd(g),
+                                                            g.t0 + (double)g.step * g.dt, g.mh, g.Pd);
+        g.launches++;
+        return cudaGetLastError();
+    }
+    static cudaError_t error_norms(GridCore& g, double* out) {
+        if constexpr (!HAS_MMS) return cudaErrorNotSupported;
+        cudaError_t e = frame_now(g);
+        if (e != cudaSuccess) return e;
+        return g.prec == PREC_F64 ? norms_t<double>(g, out) : norms_t<float>(g, out);
+    }
     static bool row_supported(const GridCore&) { return false; }
 
     static const SysOps* get() {
         static const SysOps ops = {Sd::ID, D, M, Sd::MC, HAS_MMS, C::NT, {C::NX, C::NY, C::NZ}, C::NC,
                                    &fill_tables, &reference_equilibrium, &init_from_U, &set_f, &step,
-                                   &read_U_with_frame, &read_f, &max_wave_speed, &row_supported};
+                                   &read_U_with_frame, &read_f, &max_wave_speed, &error_norms, &row_supported};
         return &ops;
     }
 };
