@@ -134,6 +134,26 @@ lbmk_status lbmk_grid_workspace_bytes(const lbmk_grid* g, size_t* bytes);
 lbmk_status lbmk_grid_bind_workspace(lbmk_grid* g, void* device_ptr, size_t bytes);
 void lbmk_grid_destroy(lbmk_grid* g);
 
+/* ---- sub-domains and slabs -------------------------------------------------------- */
+
+/* The grid is a sub-domain of a larger one: node (ix, iy, iz) sits at ((ix+ox) dx, (iy+oy) dx, (iz+oz) dx).  Only
+ * explicit (x, t) dependence sees it (manufactured forcing and exact fields).  Before lbmk_grid_bind_workspace. */
+lbmk_status lbmk_grid_set_origin(lbmk_grid* g, int ox, int oy, int oz);
+/* Slab mode: the slowest axis (z in 3D, y in 2D) holds one GHOST plane at each end (plane 0 and plane n-1), the
+ * planes between are the rank's own.  Forces the two-lattice pull pattern; the reductions (sub-characteristic
+ * check, error norms) skip the ghost planes; lbmk_read_U still returns all planes (ghost values are meaningless).
+ * lbmk_init_from_U must be given valid data on the ghost planes too (they are the neighbours' planes at t0).
+ * After EVERY lbmk_step(g, 1) the face-crossing populations are exchanged with the two neighbours:
+ *   lbmk_halo_pack   send_lo <- populations of the first own plane moving down, send_hi <- of the last own plane moving up
+ *   (transport: the lower neighbour's send_hi is this rank's recv_lo, the upper neighbour's send_lo its recv_hi)
+ *   lbmk_halo_unpack recv_lo -> lower ghost plane, recv_hi -> upper ghost plane.
+ * Buffers: DEVICE pointers, lbmk_halo_bytes() each, layout [m_total][plane nodes] in the grid's storage type;
+ * both calls are asynchronous on the grid's stream.  Before lbmk_grid_bind_workspace. */
+lbmk_status lbmk_grid_set_slab(lbmk_grid* g, int enable);
+lbmk_status lbmk_halo_bytes(const lbmk_grid* g, size_t* bytes);
+lbmk_status lbmk_halo_pack(lbmk_grid* g, void* send_lo, void* send_hi);
+lbmk_status lbmk_halo_unpack(lbmk_grid* g, const void* recv_lo, const void* recv_hi);
+
 /* ---- initialise from U, step, read back U ------------------------------------------------------------ */
 
 /* Step 0: all populations, conserved and tracker, at the (shifted) equilibrium of

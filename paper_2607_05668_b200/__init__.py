@@ -63,6 +63,11 @@ SYMBOLS = {
     "lbmk_time": (C.c_int, [_vp, C.POINTER(C.c_longlong), _dp]),
     "lbmk_check_subcharacteristic": (C.c_int, [_vp, _dp]),
     "lbmk_error_norms": (C.c_int, [_vp, _dp]),
+    "lbmk_grid_set_origin": (C.c_int, [_vp, C.c_int, C.c_int, C.c_int]),
+    "lbmk_grid_set_slab": (C.c_int, [_vp, C.c_int]),
+    "lbmk_halo_bytes": (C.c_int, [_vp, C.POINTER(C.c_size_t)]),
+    "lbmk_halo_pack": (C.c_int, [_vp, _vp, _vp]),
+    "lbmk_halo_unpack": (C.c_int, [_vp, _vp, _vp]),
     "lbmk_stream_index_map": (C.c_int, [_vp, C.c_int, _vp, C.c_int]),
     "lbmk_lattice_constants": (C.c_int, [C.c_int, C.POINTER(C.c_int), _dp, _dp]),
     "lbmk_grid_omega": (C.c_int, [_vp, _dp]),
@@ -223,6 +228,28 @@ def lbmk_check_subcharacteristic(grid_h, raise_on_violation: bool = True):
     return (float(out[0]), float(out[1]), float(out[2])), st
 
 
+def lbmk_grid_set_origin(grid_h, ox: int, oy: int, oz: int):
+    _check(lib().lbmk_grid_set_origin(grid_h, ox, oy, oz), grid_h)
+
+
+def lbmk_grid_set_slab(grid_h, enable: bool):
+    _check(lib().lbmk_grid_set_slab(grid_h, int(enable)), grid_h)
+
+
+def lbmk_halo_bytes(grid_h) -> int:
+    n = C.c_size_t()
+    _check(lib().lbmk_halo_bytes(grid_h, C.byref(n)), grid_h)
+    return n.value
+
+
+def lbmk_halo_pack(grid_h, send_lo: int, send_hi: int):
+    _check(lib().lbmk_halo_pack(grid_h, _vp(send_lo), _vp(send_hi)), grid_h)
+
+
+def lbmk_halo_unpack(grid_h, recv_lo: int, recv_hi: int):
+    _check(lib().lbmk_halo_unpack(grid_h, _vp(recv_lo), _vp(recv_hi)), grid_h)
+
+
 def lbmk_error_norms(grid_h, m_total: int) -> np.ndarray:
     out = np.zeros((m_total, 6))
     _check(lib().lbmk_error_norms(grid_h, out.ctypes.data_as(_dp)), grid_h)
@@ -304,7 +331,8 @@ class Grid:
     """A grid bound to a torch-owned device workspace on `device`, enqueuing on torch's current stream."""
 
     def __init__(self, system: System, nx: int, ny: int, nz: int, dx: float, lam: float, precision: str = "f64",
-                 bc: str = "periodic", pattern: str = "auto", kernel: str = "auto", device: str = "cuda:0"):
+                 bc: str = "periodic", pattern: str = "auto", kernel: str = "auto", device: str = "cuda:0",
+                 origin: Sequence[int] = (0, 0, 0), slab: bool = False):
         import torch
         if not torch.cuda.is_available():
             raise LbmkError(3, "no CUDA device: the collide-and-stream path has no CPU fallback")
@@ -316,10 +344,15 @@ class Grid:
         self.stream = torch.cuda.current_stream(self.device)
         self.h = lbmk_grid_create(system.h, nx, ny, nz, {"periodic": 0, "dirichlet_mms": 1}[bc], dx, lam,
                                   PRECISION[precision], self.stream.cuda_stream)
+        if tuple(origin) != (0, 0, 0):
+            lbmk_grid_set_origin(self.h, *[int(o) for o in origin])
+        self.slab = bool(slab)
         if pattern != "auto":
             lbmk_grid_set_option(self.h, LBMK_OPT_PATTERN, PATTERN[pattern])
         if kernel != "auto":
             lbmk_grid_set_option(self.h, LBMK_OPT_KERNEL, KERNEL[kernel])
+        if slab:
+            lbmk_grid_set_slab(self.h, True)
         self.workspace_bytes = lbmk_grid_workspace_bytes(self.h)
         self.workspace = torch.empty(self.workspace_bytes, dtype=torch.uint8, device=self.device)
         lbmk_grid_bind_workspace(self.h, self.workspace.data_ptr(), self.workspace_bytes)
@@ -330,6 +363,7 @@ class Grid:
     def from_workload(cls, w, precision: Optional[str] = None, omega=None, declare_bound: bool = True, **kw):
         s = System(w.system, params=w.params, tau_R=w.tau_R, g_tau=w.g_tau, U_ref=w.U_ref, mms_id=w.mms_id,
                    mms_params=w.mms_params if w.mms_id else (), omega=omega, s_max=w.s_max if declare_bound else 0.0)
+        kw.setdefault("origin", getattr(w, "origin", (0, 0, 0)))
         return cls(s, w.nx, w.ny, w.nz, w.dx, w.lam, precision=precision or w.precision, **kw)
 
     # shapes

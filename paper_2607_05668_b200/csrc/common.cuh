@@ -33,6 +33,8 @@ template <class R>
 struct KParams {
     int nx, ny, nz;
     long long n;            // nodes
+    int ox, oy, oz;         // node (ix, iy, iz) sits at ((ix+ox) dx, (iy+oy) dx, (iz+oz) dx): sub-domain of a larger grid
+    int ghost;              // 1: slab with one ghost plane at each end of the slowest axis (skipped by the reductions)
     R omega[MAXM];          // relaxation rate per component
     R ref[MAXM];            // reference state Q0 of eq (2.23); zeros in the unshifted fp64 form
     R par[8];               // physical parameters of the system

@@ -61,7 +61,7 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 // and it runs on the auxiliary stream under the previous batch's steps.
 template <class Sys, class R>
 __global__ void __launch_bounds__(128)
-mms_row_coeffs_kernel(R* __restrict__ coef, int ny, int nz, int nb, double t_first, double dt,
+mms_row_coeffs_kernel(R* __restrict__ coef, int ny, int nz, int oy, int oz, int nb, double t_first, double dt,
                       const __grid_constant__ MmsHostArgs mh, const __grid_constant__ MmsArgs<double> ma) {
     if constexpr (has_mms<Sys>()) {
         using G = typename Sys::Mms;
@@ -73,8 +73,8 @@ mms_row_coeffs_kernel(R* __restrict__ coef, int ny, int nz, int nb, double t_fir
         double T[8], Y[8], Z[8];
         const double t_n = t_first + (double)b * dt;
         G::time_scalars(t_n + 0.5 * dt, mh, T);
-        G::axis_row(1, iy * mh.dx, mh, Y);
-        if (G::NZ > 0) G::axis_row(2, iz * mh.dx, mh, Z);
+        G::axis_row(1, (iy + oy) * mh.dx, mh, Y);
+        if (G::NZ > 0) G::axis_row(2, (iz + oz) * mh.dx, mh, Z);
         G::template row_coeffs<double, R>(ma, T, Y, Z, coef + (size_t)id * G::NC);
     }
 }
@@ -333,6 +333,11 @@ __global__ void set_f_kernel(const double* __restrict__ in, R* __restrict__ f, c
     for (int q = 0; q < MQ; ++q) f[tile_off(node, MQ) + q * TILE] = (R)(in[(long long)q * n + node] - feq0[q]);
 }
 
+// ghost plane of a slab: first / last plane of the slowest axis
+template <int D> __device__ __forceinline__ bool is_ghost(const NodeIdx& p, int ny, int nz) {
+    return D == 3 ? (p.iz == 0 || p.iz == nz - 1) : (p.iy == 0 || p.iy == ny - 1);
+}
+
 // ------------------------------------------------------------------------------------------------ a10
 // Sub-characteristic check (eq 2.19-2.20; L329): max over nodes of the system's wave
 // speeds, in fp64 from the canonical moments.  Warp shuffle -> shared -> one atomicMax per block on the
@@ -351,6 +356,7 @@ max_wave_speed_kernel(const R* __restrict__ f, unsigned long long* __restrict__ 
     double m[3] = {0.0, 0.0, 0.0};
     for (long long node = (long long)blockIdx.x * blockDim.x + threadIdx.x; node < n; node += (long long)gridDim.x * blockDim.x) {
         const NodeIdx p = decompose(node, nx, ny);
+        if (Pd.ghost && is_ghost<Sys::D>(p, ny, nz)) continue;
         double U[M], w[3];
         for (int k = 0; k < M; ++k) {
             double s = 0.0;
@@ -407,9 +413,10 @@ error_norms_kernel(const R* __restrict__ f, double* __restrict__ out, long long 
         for (long long node = (long long)blockIdx.x * blockDim.x + threadIdx.x; node < n; node += (long long)gridDim.x * blockDim.x) {
             const NodeIdx p = decompose(node, nx, ny);
             double X[8], Y[8], Z[8], q[M];
-            G::axis_row(0, p.ix * mh.dx, mh, X);
-            G::axis_row(1, p.iy * mh.dx, mh, Y);
-            if (G::NZ > 0) G::axis_row(2, p.iz * mh.dx, mh, Z);
+            if (Pd.ghost && is_ghost<Sys::D>(p, ny, nz)) continue;
+            G::axis_row(0, (p.ix + Pd.ox) * mh.dx, mh, X);
+            G::axis_row(1, (p.iy + Pd.oy) * mh.dx, mh, Y);
+            if (G::NZ > 0) G::axis_row(2, (p.iz + Pd.oz) * mh.dx, mh, Z);
             G::template exact<double>(Pd.mms, T, X, Y, Z, q);
             for (int k = 0; k < M; ++k) {
                 double s = 0.0;

@@ -340,6 +340,77 @@ lbmk_status lbmk_grid_set_option(lbmk_grid* g, lbmk_option key, long long value)
     return LBMK_OK;
 }
 
+// ------------------------------------------------------------------------------------------------ sub-domains / slabs
+static lbmk_status need_inited(lbmk_grid* g);
+lbmk_status lbmk_grid_set_origin(lbmk_grid* g, int ox, int oy, int oz) {
+    if (!g) return sys_fail(LBMK_EINVAL, "grid is NULL");
+    if (g->bound) return fail(g, LBMK_ESTATE, "the origin must be set before the workspace is bound");
+    GridCore& c = g->c;
+    c.Pd.ox = c.Pf.ox = ox; c.Pd.oy = c.Pf.oy = oy; c.Pd.oz = c.Pf.oz = oz;
+    return LBMK_OK;
+}
+
+lbmk_status lbmk_grid_set_slab(lbmk_grid* g, int enable) {
+    if (!g) return sys_fail(LBMK_EINVAL, "grid is NULL");
+    if (g->bound) return fail(g, LBMK_ESTATE, "slab mode must be set before the workspace is bound");
+    GridCore& c = g->c;
+    if (enable) {
+        if (c.bc != LBMK_PERIODIC) return fail(g, LBMK_EUNSUPPORTED, "slabs are periodic grids");
+        if ((g->ops->D == 3 ? c.nz : c.ny) < 3) return fail(g, LBMK_EINVAL, "a slab needs >= 1 interior plane between its 2 ghost planes");
+        g->opt_pattern = LBMK_PATTERN_PULL2;            // the halo is defined on the two-lattice pull storage
+        resolve_options(g);
+        layout(g);
+    }
+    c.Pd.ghost = c.Pf.ghost = enable ? 1 : 0;
+    return LBMK_OK;
+}
+
+static long long plane_nodes_of(const lbmk_grid* g) { return g->ops->D == 3 ? (long long)g->c.nx * g->c.ny : (long long)g->c.nx; }
+static int planes_of(const lbmk_grid* g) { return g->ops->D == 3 ? g->c.nz : g->c.ny; }
+
+lbmk_status lbmk_halo_bytes(const lbmk_grid* g, size_t* bytes) {
+    if (!g || !bytes) return sys_fail(LBMK_EINVAL, "NULL argument");
+    *bytes = (size_t)g->ops->M * plane_nodes_of(g) * (g->c.prec == PREC_F64 ? 8 : 4);
+    return LBMK_OK;
+}
+
+static lbmk_status halo_move(lbmk_grid* g, void* lo, void* hi, const bool PACK) {
+    lbmk_status s = need_inited(g);
+    if (s != LBMK_OK) return s;
+    GridCore& c = g->c;
+    if (!c.Pd.ghost) return fail(g, LBMK_ESTATE, "not a slab (lbmk_grid_set_slab)");
+    if (!lo || !hi) return fail(g, LBMK_EINVAL, "halo buffer is NULL");
+    if (!c.pending) return fail(g, LBMK_ESTATE, "halo exchange is defined after at least one step (initialise the ghost planes through lbmk_init_from_U)");
+    const int D = g->ops->D, M = g->ops->M, Q = 2 * D + 1;
+    const int up = 2 * D - 1, down = 2 * D;                       // slot of +s / -s along the slowest axis
+    const long long pn = plane_nodes_of(g);
+    const int np = planes_of(g);
+    const unsigned nb = (unsigned)(((long long)M * pn + 255) / 256);
+    // pack: lo <- slot(-s) of the first interior plane, hi <- slot(+s) of the last interior plane
+    // unpack: lo -> slot(+s) of the lower ghost plane, hi -> slot(-s) of the upper ghost plane
+    const int slot_lo = PACK ? down : up, slot_hi = PACK ? up : down;
+    const long long plane_lo = PACK ? 1 : 0, plane_hi = PACK ? np - 2 : np - 1;
+    void* bufs[2] = {lo, hi};
+    const int slots[2] = {slot_lo, slot_hi};
+    const long long planes[2] = {plane_lo, plane_hi};
+    for (int e = 0; e < 2; ++e) {
+        if (c.prec == PREC_F64) {
+            if (PACK) halo_kernel<double, true><<<nb, 256, 0, c.stream>>>((double*)c.f[c.cur], (double*)bufs[e], M, Q, slots[e], planes[e] * pn, pn);
+            else halo_kernel<double, false><<<nb, 256, 0, c.stream>>>((double*)c.f[c.cur], (double*)bufs[e], M, Q, slots[e], planes[e] * pn, pn);
+        } else {
+            if (PACK) halo_kernel<float, true><<<nb, 256, 0, c.stream>>>((float*)c.f[c.cur], (float*)bufs[e], M, Q, slots[e], planes[e] * pn, pn);
+            else halo_kernel<float, false><<<nb, 256, 0, c.stream>>>((float*)c.f[c.cur], (float*)bufs[e], M, Q, slots[e], planes[e] * pn, pn);
+        }
+    }
+    c.launches += 2;
+    CK(g, cudaGetLastError(), "halo kernel");
+    return LBMK_OK;
+}
+lbmk_status lbmk_halo_pack(lbmk_grid* g, void* send_lo, void* send_hi) { return halo_move(g, send_lo, send_hi, true); }
+lbmk_status lbmk_halo_unpack(lbmk_grid* g, const void* recv_lo, const void* recv_hi) {
+    return halo_move(g, const_cast<void*>(recv_lo), const_cast<void*>(recv_hi), false);
+}
+
 lbmk_status lbmk_grid_get_option(const lbmk_grid* g, lbmk_option key, long long* value) {
     if (!g || !value) return sys_fail(LBMK_EINVAL, "NULL argument");
     if (key == LBMK_OPT_PATTERN) *value = g->c.pattern;

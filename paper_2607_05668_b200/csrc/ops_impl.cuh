@@ -50,12 +50,13 @@ struct Ops {
         if constexpr (HAS_MMS) {
             const int cnt[3] = {C::NX, C::NY, C::NZ};
             const int len[3] = {g.nx, g.ny, g.nz};
+            const int org[3] = {g.Pd.ox, g.Pd.oy, g.Pd.oz};
             for (int ax = 0; ax < 3; ++ax) {
                 if (cnt[ax] == 0) continue;
                 std::vector<R> h((size_t)cnt[ax] * len[ax]);
                 double row[8];
                 for (int j = 0; j < len[ax]; ++j) {
-                    Sd::Mms::axis_row(ax, j * g.mh.dx, g.mh, row);          // x_j = j dx (reading A1)
+                    Sd::Mms::axis_row(ax, (j + org[ax]) * g.mh.dx, g.mh, row);   // x_j = j dx (reading A1), plus the sub-domain origin
                     for (int e = 0; e < cnt[ax]; ++e) h[(size_t)e * len[ax] + j] = (R)row[e];
                 }
                 cudaError_t e = cudaMemcpyAsync(g.tab[ax], h.data(), h.size() * sizeof(R), cudaMemcpyHostToDevice, g.stream);
@@ -181,7 +182,7 @@ struct Ops {
         R* dst = (R*)g.coef + (size_t)buf * g.coef_B * rows * C::NC;
         const long long threads = rows * nb;
         mms_row_coeffs_kernel<S<R>, R><<<(unsigned)((threads + 127) / 128), 128, 0, g.aux>>>(
-            dst, g.ny, g.nz, nb, g.t0 + (double)first * g.dt, g.dt, g.mh, g.Pd.mms);
+            dst, g.ny, g.nz, g.Pd.oy, g.Pd.oz, nb, g.t0 + (double)first * g.dt, g.dt, g.mh, g.Pd.mms);
         g.launches++;
     }
     template <class R, bool MMS>

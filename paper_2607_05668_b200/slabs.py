@@ -1,0 +1,104 @@
+"""Slab decomposition of a periodic grid over ranks.
+
+The slowest axis (z in 3D, y in 2D) is cut into contiguous slabs, one per rank (one process per GPU).  Every rank
+holds its planes plus one ghost plane at each end (`lbmk_grid_set_slab`).  After every collide-and-stream step the
+only data another rank needs are the face-crossing populations of the two boundary planes (1 of Q directions per
+face and component: nx*ny*m_total scalars per face):
+
+    lbmk_halo_pack -> exchange with the two ring neighbours -> lbmk_halo_unpack
+
+`HaloRing.exchange` is the transport: `torch.distributed` point-to-point (NCCL over NVLink on GPUs, gloo on CPU in
+the tests) between ring neighbours, or plain copies when the ring has one rank.  This module only marshals buffers:
+every step of the path, including packing and unpacking, runs in the kernels behind the C-ABI.
+"""
+from __future__ import annotations
+
+from typing import List, Optional
+
+
+class HaloRing:
+    """Periodic ring of `world` ranks along the slab axis; rank r's lower neighbour is r-1, upper neighbour r+1."""
+
+    def __init__(self, rank: int = 0, world: int = 1, dist=None):
+        self.rank, self.world, self.dist = rank, world, dist
+        self.lo = (rank - 1) % world
+        self.hi = (rank + 1) % world
+        if world > 1 and dist is None:
+            raise ValueError("a ring of more than one rank needs torch.distributed")
+
+    def exchange(self, send_lo, send_hi, recv_lo, recv_hi):
+        """recv_lo <- the lower neighbour's send_hi; recv_hi <- the upper neighbour's send_lo.
+
+        world == 1: the rank is its own neighbour (periodic wrap through the ghost planes).
+        world == 2: both neighbours are the same peer; messages between one pair of ranks are matched in posting
+        order, so the receives are posted in the order the peer posts its sends (its send_lo, then its send_hi).
+        """
+        if self.world == 1:
+            recv_lo.copy_(send_hi)
+            recv_hi.copy_(send_lo)
+            return
+        d = self.dist
+        ops = [d.P2POp(d.isend, send_lo, self.lo), d.P2POp(d.isend, send_hi, self.hi),
+               d.P2POp(d.irecv, recv_hi, self.hi), d.P2POp(d.irecv, recv_lo, self.lo)]
+        for req in d.batch_isend_irecv(ops):
+            req.wait()
+
+
+class SlabGrid:
+    """One rank's slab of a periodic workload: a `Grid` in slab mode plus its four halo buffers."""
+
+    def __init__(self, P, w_global, rank: int = 0, world: int = 1, device: str = "cuda:0", precision: Optional[str] = None):
+        import torch
+        import workloads as W
+        self.torch = torch
+        self.P = P
+        self.rank, self.world = rank, world
+        self.w = W.slab_workload(w_global, rank, world)
+        self.start, self.count = W.slab_range(w_global.nz if w_global.dim == 3 else w_global.ny, world, rank)
+        self.grid = P.Grid.from_workload(self.w, precision=precision, slab=True, device=device)
+        m = self.w.m_total
+        plane = self.w.nx * (self.w.ny if self.w.dim == 3 else 1)
+        dt = torch.float64 if (precision or self.w.precision) in ("f64", "f64s") else torch.float32
+        assert P.lbmk_halo_bytes(self.grid.h) == m * plane * (8 if dt == torch.float64 else 4)
+        mk = lambda: torch.empty((m, plane), dtype=dt, device=self.grid.device)
+        self.send_lo, self.send_hi, self.recv_lo, self.recv_hi = mk(), mk(), mk(), mk()
+
+    def init(self):
+        self.grid.init_from_U(self.w.initial_U())
+
+    def pack(self):
+        self.P.lbmk_halo_pack(self.grid.h, self.send_lo.data_ptr(), self.send_hi.data_ptr())
+
+    def unpack(self):
+        self.P.lbmk_halo_unpack(self.grid.h, self.recv_lo.data_ptr(), self.recv_hi.data_ptr())
+
+    def step(self, n: int, ring: HaloRing):
+        """n steps, each followed by the halo exchange with the ring neighbours (all on torch's current stream)."""
+        for _ in range(n):
+            self.grid.step(1)
+            self.pack()
+            ring.exchange(self.send_lo, self.send_hi, self.recv_lo, self.recv_hi)
+            self.unpack()
+
+    def read_U_interior(self):
+        U = self.grid.read_U()
+        return U[:, 1:-1] if self.w.dim == 3 else U[:, :, 1:-1]
+
+    def close(self):
+        self.grid.close()
+
+
+def step_local_ring(slabs: List[SlabGrid], n: int):
+    """All slabs of a ring held by ONE process on one device (tests, and N = 1 with several slabs): every slab steps
+    once, then the buffers are routed exactly as HaloRing.exchange routes them between ranks.  No kernel of one slab
+    waits on another slab's kernel: the routing is plain stream-ordered copies."""
+    W = len(slabs)
+    for _ in range(n):
+        for s in slabs:
+            s.grid.step(1)
+            s.pack()
+        for r, s in enumerate(slabs):
+            s.recv_lo.copy_(slabs[(r - 1) % W].send_hi)
+            s.recv_hi.copy_(slabs[(r + 1) % W].send_lo)
+        for s in slabs:
+            s.unpack()

@@ -1,0 +1,88 @@
+"""Slab decomposition on the device: several slabs of one periodic grid, held by one process
+on one GPU and exchanged exactly as the ranks of a ring exchange them, reproduce the single-grid run BIT FOR BIT
+(same kernels, same arithmetic; the ghost planes and halo pack/unpack are the only difference)."""
+import numpy as np
+import pytest
+
+import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def P():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device")
+    import paper_2607_05668_b200 as P
+    P.lib()
+    return P
+
+
+# the slab axis spans the periodic unit box (n planes), so that the analytic ghost planes wrap
+CASES = [(W.c4_nsf3d, dict(n=13, ny=10), 3, 9), (W.c4_nsf3d, dict(n=128, ny=4, precision="f64"), 2, 5),
+         (W.c5_mhd3d, dict(n=9, ny=10), 4, 8), (W.c2_swe, dict(n=17), 3, 11), (W.c2_swe, dict(n=256), 2, 6),
+         (W.c3_euler, dict(n=32), 2, 10), (W.pin_adr, dict(n=16), 3, 12)]
+
+
+@pytest.mark.parametrize("mk,kw,world,steps", CASES)
+def test_slabs_reproduce_the_single_grid_bit_for_bit(P, mk, kw, world, steps):
+    from paper_2607_05668_b200.slabs import SlabGrid, step_local_ring
+    w = mk(**kw)
+    g = P.Grid.from_workload(w, pattern="pull2")
+    g.init_from_U(w.initial_U())
+    g.step(steps)
+    U = g.read_U()
+    speeds = g.max_wave_speed()[0]
+    norms = P.lbmk_error_norms(g.h, w.m_total) if w.mms_id else None      # raw sums / maxima
+    g.close()
+    slabs = [SlabGrid(P, w, r, world) for r in range(world)]
+    for s in slabs:
+        s.init()
+    step_local_ring(slabs, steps)
+    ax = 1 if w.dim == 3 else 2
+    Us = np.concatenate([s.read_U_interior() for s in slabs], axis=ax)
+    assert Us.shape == U.shape and np.array_equal(Us, U)
+    # the reductions skip the ghost planes: max over slabs = the single grid's value
+    sp = np.max([s.grid.max_wave_speed()[0] for s in slabs], axis=0)
+    assert np.allclose(sp, speeds, rtol=1e-14)
+    if norms is not None:
+        parts = [P.lbmk_error_norms(s.grid.h, w.m_total) for s in slabs]
+        for j in (0, 1, 3, 4):                               # sums add up over the slabs
+            assert np.allclose(sum(p[:, j] for p in parts), norms[:, j], rtol=1e-12, atol=1e-300)
+        for j in (2, 5):                                     # maxima: max over the slabs
+            assert np.array_equal(np.max([p[:, j] for p in parts], axis=0), norms[:, j])
+    for s in slabs:
+        s.close()
+
+
+def test_one_rank_ring_equals_periodic_grid(P):
+    """world = 1: the slab's ghost planes wrap onto the slab itself through HaloRing.exchange."""
+    from paper_2607_05668_b200.slabs import HaloRing, SlabGrid
+    w = W.c5_mhd3d(n=10, ny=8)
+    g = P.Grid.from_workload(w, pattern="pull2")
+    g.init_from_U(w.initial_U())
+    g.step(7)
+    U = g.read_U()
+    g.close()
+    s = SlabGrid(P, w, 0, 1)
+    s.init()
+    s.step(7, HaloRing(0, 1))
+    assert np.array_equal(s.read_U_interior(), U)
+    s.close()
+
+
+def test_halo_calls_are_refused_out_of_order(P):
+    w = W.c5_mhd3d(n=6)
+    g = P.Grid.from_workload(w)                              # not a slab
+    g.init_from_U(w.initial_U()); g.step(1)
+    with pytest.raises(P.LbmkError) as e:
+        P.lbmk_halo_pack(g.h, g.workspace.data_ptr(), g.workspace.data_ptr())
+    assert e.value.status == 5
+    g.close()
+    s = P.Grid.from_workload(W.slab_workload(w, 0, 2), slab=True)
+    s.init_from_U(W.slab_workload(w, 0, 2).initial_U())
+    with pytest.raises(P.LbmkError) as e:                    # before the first step: ghosts come from init
+        P.lbmk_halo_pack(s.h, s.workspace.data_ptr(), s.workspace.data_ptr())
+    assert e.value.status == 5 and s.pattern == "pull2"
+    s.close()

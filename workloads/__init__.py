@@ -71,6 +71,7 @@ class Workload:
     seed: int
     init: Callable[["Workload"], np.ndarray] = field(repr=False, default=None)
     note: str = ""
+    origin: tuple = (0, 0, 0)   # (ox, oy, oz) in nodes: this grid is a sub-domain, node j sits at (j + o) dx
 
     @property
     def lattice(self) -> str:
@@ -109,9 +110,10 @@ class Workload:
 
 def _grid(w: Workload):
     """Node coordinates as broadcastable arrays (z, y, x), x_j = j*dx."""
-    x = (np.arange(w.nx, dtype=np.float64) * w.dx)[None, None, :]
-    y = (np.arange(w.ny, dtype=np.float64) * w.dx)[None, :, None]
-    z = (np.arange(w.nz, dtype=np.float64) * w.dx)[:, None, None]
+    ox, oy, oz = w.origin
+    x = ((np.arange(w.nx, dtype=np.float64) + ox) * w.dx)[None, None, :]
+    y = ((np.arange(w.ny, dtype=np.float64) + oy) * w.dx)[None, :, None]
+    z = ((np.arange(w.nz, dtype=np.float64) + oz) * w.dx)[:, None, None]
     return x, y, z
 
 
@@ -132,6 +134,7 @@ def _init_c1(w: Workload) -> np.ndarray:
     U = _full(w, U).copy()
     amp = w.mms_params[0] if w.mms_params else 0.0
     if amp > 0.0:
+        assert tuple(w.origin) == (0, 0, 0), "the seeded noise of c1 is defined on the whole grid only"
         rng = np.random.default_rng(w.seed)
         U += rng.uniform(0.0, amp, size=U.shape)
     return U[None]
@@ -394,6 +397,24 @@ def pin_maxwell(n: int = 512, precision: str = "f64", f: float = 0.2) -> Workloa
 BASELINE_CONFIGS: Dict[str, Callable[..., Workload]] = {
     "c1": c1_advection, "c2": c2_swe, "c3": c3_euler, "c4": c4_nsf3d, "c5": c5_mhd3d,
 }
+
+
+def slab_range(n_global: int, world: int, rank: int):
+    """Contiguous, balanced split of n_global planes over `world` ranks: (first plane, plane count) of `rank`."""
+    base, rem = divmod(n_global, world)
+    return rank * base + min(rank, rem), base + (1 if rank < rem else 0)
+
+
+def slab_workload(w: Workload, rank: int, world: int) -> Workload:
+    """The sub-domain of periodic workload w that `rank` of `world` owns when the slowest axis (z in 3D, y in 2D) is
+    cut into slabs, with one ghost plane at each end: the same fields, dx, lambda and
+    parameters, evaluated on planes start-1 .. start+count (periodic fields need no index wrap)."""
+    n_glob = w.nz if w.dim == 3 else w.ny
+    start, count = slab_range(n_glob, world, rank)
+    assert count >= 1
+    if w.dim == 3:
+        return replace(w, name=f"{w.name}_slab{rank}of{world}", nz=count + 2, origin=(0, 0, start - 1))
+    return replace(w, name=f"{w.name}_slab{rank}of{world}", ny=count + 2, origin=(0, start - 1, 0))
 
 
 def relabel(w: Workload, **kw) -> Workload:
