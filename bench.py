@@ -19,8 +19,9 @@ One JSON line is printed by rank 0:
   cpu_baseline  the CPU oracle (oracle/, plain fp64 C++) timed on this box's host cores on a bounded sample
   all_configs   short runs of the other BASELINE.json configs (reported, not the headline)
 
-Multi-GPU (--gpus N under torchrun): "replicas only" -- every rank advances its own
+Multi-GPU (--gpus N under torchrun): by default "replicas only" -- every rank advances its own
 full-size grid, no data-path collective; value = sum over ranks / max-over-ranks time; scaling "weak".
+`--parallelism slabs` instead cuts ONE N-times-taller periodic grid into z-slabs with a halo exchange after every step.
 
 `--impl reference` times the oracle as it stands on host cores (rank 0 only): each step is one oracle step on a
 bounded sub-box of the same workload (same node spacing and parameters), sized so the run ends within minutes.
@@ -67,6 +68,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-all-configs", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--parallelism", default="replicas", choices=["replicas", "slabs"],
+                    help="N > 1: independent replicas (default) or z-slabs of one N-times-taller periodic grid with a halo exchange per step")
     ap.add_argument("--table3", action="store_true", help="also run the paper's Table 3 systems (4096^2, forcing off, S and D)")
     return ap.parse_args()
 
@@ -185,6 +188,38 @@ def time_steps(g, torch, steps, dist=None):
     if dist is not None:
         dist.barrier()
     return e0.elapsed_time(e1), g.launch_count() - l0
+
+
+class SlabRunner:
+    """This rank's slab of the global workload behind the interface run_ours uses for a Grid."""
+
+    def __init__(self, P, w_global, rank, world, dist, device):
+        from paper_2607_05668_b200.slabs import HaloRing, SlabGrid
+        self.slab = SlabGrid(P, w_global, rank, world, device=device)
+        self.ring = HaloRing(rank, world, dist)
+        self.grid = self.slab.grid
+        self.w = self.slab.w                                   # local workload, ghost planes included
+        self.pattern, self.kernel, self.shape_U = self.grid.pattern, self.grid.kernel, self.grid.shape_U
+        plane = self.w.nx * (self.w.ny if self.w.dim == 3 else 1)
+        self.own_nodes = plane * self.slab.count               # node updates that count: ghost planes excluded
+
+    def init_from_U(self, U):
+        self.grid.init_from_U(U)
+
+    def step(self, n):
+        self.slab.step(n, self.ring)
+
+    def read_U(self, out=None):
+        return self.grid.read_U(out)
+
+    def max_wave_speed(self):
+        return self.grid.max_wave_speed()
+
+    def launch_count(self):
+        return self.grid.launch_count()
+
+    def close(self):
+        self.slab.close()
 
 
 def short_run(P, torch, name, pattern):
@@ -342,8 +377,16 @@ def run_ours(args):
     steps = args.steps if args.steps is not None else min(w.steps, 200)
     warm = max(args.warmup, 3)
     dev = f"cuda:{local}"
-    U0 = w.initial_U()
-    g = P.Grid.from_workload(w, pattern=args.pattern, kernel=args.kernel, device=dev)
+    slabs = args.parallelism == "slabs"
+    if slabs:
+        import workloads as W
+        # weak scaling: one periodic grid `world` times taller along the slab axis, this rank owns one workload-sized slab
+        wg = W.relabel(w, **({"nz": w.nz * world} if w.dim == 3 else {"ny": w.ny * world}))
+        g = SlabRunner(P, wg, rank, world, dist, dev)
+        own_nodes, U0 = g.own_nodes, g.w.initial_U()
+    else:
+        own_nodes, U0 = w.n_nodes, w.initial_U()
+        g = P.Grid.from_workload(w, pattern=args.pattern, kernel=args.kernel, device=dev)
     U0_dev = torch.from_numpy(U0).to(dev)
     g.init_from_U(U0_dev)
     speeds, status = g.max_wave_speed()                      # a10: device sub-characteristic check (untimed)
@@ -360,7 +403,7 @@ def run_ours(args):
     t_wall1 = time.perf_counter()
     clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
     ms_local = statistics.median(reps)
-    ms, updates = aggregate(dist, ms_local, w.n_nodes * steps, dev)
+    ms, updates = aggregate(dist, ms_local, own_nodes * steps, dev)
     mlups = updates / (ms * 1e-3) / 1e6
     finite = bool(np.isfinite(g.read_U(torch.empty(g.shape_U, dtype=torch.float64, device=dev)).sum().item()))
 
@@ -383,7 +426,7 @@ def run_ours(args):
         torch.cuda.synchronize()
         wall_ms = (time.perf_counter() - tw) * 1e3
         e_ms = max(e0.elapsed_time(e1), wall_ms)
-        e_ms, e_upd = aggregate(dist, e_ms, w.n_nodes * steps, dev)
+        e_ms, e_upd = aggregate(dist, e_ms, own_nodes * steps, dev)
         nbytes = U_host.numel() * 8
         e2e = {"value": e_upd / (e_ms * 1e-3) / 1e6, "unit": UNIT, "h2d_bytes_per_step": nbytes / steps,
                "d2h_bytes_per_step": nbytes / steps, "ms_total": e_ms,
@@ -413,7 +456,7 @@ def run_ours(args):
                    "grid": [w.nx, w.ny, w.nz], "precision": w.precision, "mms_forcing": bool(w.mms_id),
                    "pattern": pattern, "kernel": kernel, "bytes_per_node": w.bytes_per_node,
                    "l2": "state larger than L2 (no flush needed)" if bytes_per_launch / 2 > 2.5e8 else "state fits in L2: HBM roofline n/a",
-                   "parallelism": "replicas only" if world > 1 else "single GPU", "timing": f"median of {n_rep} x {steps} steps, CUDA events",
+                   "parallelism": ("z-slabs, halo exchange per step" if slabs else "replicas only") if (world > 1 or slabs) else "single GPU", "timing": f"median of {n_rep} x {steps} steps, CUDA events",
                    "lattice_wave_speed": max(speeds[0], speeds[1]) + speeds[2], "finite": finite},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": traffic, "peak_source": peak_src, "frac_of_nominal_8TBps": achieved / 8000.0,
