@@ -10,6 +10,7 @@
 //   swe2d     mms 1 : BASELINE.json configs[1] fields, mms_par = {A_h, A_u, h0}
 //   nsf3d     mms 1 : BASELINE.json configs[3] fields, mms_par = {U0, A_rho, rho0, p0}
 //   urf2d     mms 1 : eq (SM5.4)
+//   allencahn2d mms 1 : eq (SM5.8); Table SM9 L1316 (gamma = 0.01, r = 1)
 //   maxwell2d mms 1 : eq (SM5.5), PAPER.md:L1248-L1254 (k_x = 2 pi, k_y = 4 pi, A = 1/2, omega = 4)
 #pragma once
 #include "jets.hpp"
@@ -81,6 +82,13 @@ inline bool exact_state(int sys, int mms_id, const Scaling& sc, const double* mp
         Q[0] = lower(0.4 * sin(k * x) * sin(k * y) * cos(t) + 3.0);
         Q[1] = lower(0.4 * cos(k * x) * cos(k * y) * sin(t) + 1.2);
         Q[2] = lower(0.4 * sin(k * x) * sin(k * y) * sin(t) + 1.2);
+        return true;
+    }
+    case SYS_ALLENCAHN2D: {
+        J2 phi = 0.7 * sin(k * x) * cos(k * y) * cos(t);          // eq (SM5.8)
+        Q[0] = lower(phi);
+        Q[1] = sc.dx * diff(phi, 1);
+        Q[2] = sc.dx * diff(phi, 2);
         return true;
     }
     case SYS_MAXWELL2D: {

@@ -17,7 +17,7 @@
 namespace orc {
 
 enum SystemId { SYS_ADVECTION2D = 0, SYS_BURGERS2D = 1, SYS_SWE2D = 2, SYS_EULER2D = 3, SYS_ADR2D = 4,
-                SYS_NSF3D = 5, SYS_MHD3D = 6, SYS_URF2D = 7, SYS_MAXWELL2D = 8, SYS_COUNT = 9 };
+                SYS_NSF3D = 5, SYS_MHD3D = 6, SYS_URF2D = 7, SYS_MAXWELL2D = 8, SYS_ALLENCAHN2D = 9, SYS_COUNT = 10 };
 
 constexpr int MAXM = 32;  // max components
 
@@ -33,6 +33,7 @@ inline SysInfo sys_info(int sys) {
         case SYS_MHD3D:       return {8, 11, 3};
         case SYS_URF2D:       return {3, 3, 2};
         case SYS_MAXWELL2D:   return {3, 3, 2};
+        case SYS_ALLENCAHN2D: return {1, 3, 2};
     }
     return {0, 0, 0};
 }
@@ -184,6 +185,19 @@ void flux_source(int sys, const T* U, const Scaling& sc, T* F, T* S) {
         F[1 * 3 + 0] = il * (Sx * vx + p);  F[1 * 3 + 1] = il * (Sx * vy);
         F[2 * 3 + 0] = il * (Sy * vx);      F[2 * 3 + 1] = il * (Sy * vy + p);
     } break;
+    case SYS_ALLENCAHN2D: {
+        // Allen-Cahn phase field, eq (3.18)-(3.19); SM4.8 L928-L945; par = {gamma, r};
+        // U = (phi, G^L_x, G^L_y), G^L = dx grad phi:  F_phi = -gamma_L G^L,  F_Gb,j = -delta_jb phi/g_tau,
+        // S_phi = dt r (phi - phi^3),  S_G = -G^L/g_tau
+        const double gL = sc.par[0] * dL, r = sc.par[1];
+        T phi = U[0], Gx = U[1], Gy = U[2];
+        F[0 * 3 + 0] = -gL * Gx;             F[0 * 3 + 1] = -gL * Gy;
+        F[1 * 3 + 0] = -(phi / sc.g_tau);    F[1 * 3 + 1] = T(0.0);
+        F[2 * 3 + 0] = T(0.0);               F[2 * 3 + 1] = -(phi / sc.g_tau);
+        S[0] = (sc.dt * r) * (phi - phi * phi * phi);
+        S[1] = -Gx / sc.g_tau;
+        S[2] = -Gy / sc.g_tau;
+    } break;
     case SYS_MAXWELL2D: {
         // Maxwell TM mode in vacuum, eq (3.10)-(3.11): Q = (E_z, H_x, H_y); par = {c}
         const double c = sc.par[0];
@@ -257,6 +271,7 @@ inline void wave_speeds(int sys, const double* U, const Scaling& sc, double* out
         const double vm = std::sqrt(v2);
         out[1] = (vm + cs) / (1.0 + vm * cs);
     } break;
+    case SYS_ALLENCAHN2D: { out[2] = std::sqrt(sc.par[0] * dL / sc.g_tau); } break;   // no advection: tracker-parent coupling only
     case SYS_MAXWELL2D: { out[0] = std::fabs(sc.par[0]); out[1] = std::fabs(sc.par[0]); } break;  // eigenvalues {+c, -c, 0}, L393
     }
 }

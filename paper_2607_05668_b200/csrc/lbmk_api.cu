@@ -59,11 +59,12 @@ static const SysOps* ops_of(int id) {
         case LBMK_SYS_MHD3D_JTRACK: return ops_mhd3d();
         case LBMK_SYS_URF2D: return ops_urf2d();
         case LBMK_SYS_MAXWELL2D: return ops_maxwell2d();
+        case LBMK_SYS_ALLENCAHN2D: return ops_allencahn2d();
     }
     return nullptr;
 }
-static const int N_PARAMS[LBMK_SYS_COUNT] = {2, 0, 1, 1, 4, 3, 2, 0, 1};
-static const int N_MMS_PARAMS[LBMK_SYS_COUNT] = {0, 1, 3, 0, 0, 4, 0, 0, 0};
+static const int N_PARAMS[LBMK_SYS_COUNT] = {2, 0, 1, 1, 4, 3, 2, 0, 1, 2};
+static const int N_MMS_PARAMS[LBMK_SYS_COUNT] = {0, 1, 3, 0, 0, 4, 0, 0, 0, 0};
 
 static lbmk_status sys_fail(lbmk_status s, const char* msg) { g_sys_err = msg; return s; }
 static lbmk_status fail(lbmk_grid* g, lbmk_status s, const std::string& msg) { if (g) g->err = msg; else g_sys_err = msg; return s; }
@@ -154,7 +155,7 @@ lbmk_status lbmk_system_set_reference(lbmk_system* sys, const double* U0, int n)
             if (k != 0 && k != 4 && U0[k] != 0.0)
                 return sys_fail(LBMK_EUNSUPPORTED, "NSF3D/MHD3D delta forms need zero reference momentum, field and trackers");
     }
-    if ((sys->id == LBMK_SYS_ADR2D) && (U0[1] != 0.0 || U0[2] != 0.0))
+    if ((sys->id == LBMK_SYS_ADR2D || sys->id == LBMK_SYS_ALLENCAHN2D) && (U0[1] != 0.0 || U0[2] != 0.0))
         return sys_fail(LBMK_EUNSUPPORTED, "ADR2D needs zero reference trackers");
     for (int k = 0; k < n; ++k) sys->ref[k] = U0[k];
     return LBMK_OK;

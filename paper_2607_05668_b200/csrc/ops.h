@@ -65,5 +65,6 @@ const SysOps* ops_nsf3d();
 const SysOps* ops_mhd3d();
 const SysOps* ops_urf2d();
 const SysOps* ops_maxwell2d();
+const SysOps* ops_allencahn2d();
 
 }  // namespace lbmk

@@ -24,7 +24,7 @@
 namespace lbmk {
 
 enum { SYS_ADVECTION2D = 0, SYS_BURGERS2D = 1, SYS_SWE2D = 2, SYS_EULER2D = 3, SYS_ADR2D = 4, SYS_NSF3D = 5, SYS_MHD3D = 6,
-       SYS_URF2D = 7, SYS_MAXWELL2D = 8 };
+       SYS_URF2D = 7, SYS_MAXWELL2D = 8, SYS_ALLENCAHN2D = 9 };
 
 // ------------------------------------------------------------------------------------------ advection
 // Phi = (a_x U, a_y U); par = {a_x, a_y}
@@ -162,6 +162,32 @@ template <class R> struct SysAdr2D {
         const double ax = fabs(P.par[0]), ay = fabs(P.par[1]);
         out[0] = fmax(ax, ay); out[1] = sqrt(ax * ax + ay * ay);
         out[2] = sqrt(P.par[2] * P.dL * P.inv_gtau);
+    }
+};
+
+// ------------------------------------------------------------------------------------------ Allen-Cahn
+// eq (3.18)-(3.19); SM4.8 L928-L945; par = {gamma, r}; Q = (phi, G^L_x, G^L_y)
+template <class R> struct SysAllenCahn2D {
+    static constexpr int ID = SYS_ALLENCAHN2D, D = 2, M = 3, MC = 1;
+    using Mms = Mms_allencahn2d;
+    struct Ctx {};
+    __device__ __forceinline__ static void setup(Ctx&, const R (&)[M], const KParams<R>&) {}
+    template <int k> __device__ __forceinline__ static void flux(const Ctx&, const R (&dQ)[M], const KParams<R>& P, R (&F)[D], R& S) {
+        if constexpr (k == 0) {
+            const R gL = P.par[0] * P.dL;
+            F[0] = -gL * dQ[1];
+            F[1] = -gL * dQ[2];
+            const R phi = P.ref[0] + dQ[0];
+            S = (P.dt * P.par[1]) * (phi - phi * phi * phi);            // bistable reaction at the full state
+        } else {
+            constexpr int b = k - 1;
+            F[0] = R(0); F[1] = R(0);
+            F[b] = -dQ[0] * P.inv_gtau;
+            S = -(P.ref[k] + dQ[k]) * P.inv_gtau;
+        }
+    }
+    __device__ static void wave(const double*, const KParams<double>& P, double* out) {
+        out[0] = 0.0; out[1] = 0.0; out[2] = sqrt(P.par[0] * P.dL * P.inv_gtau);
     }
 };
 

@@ -191,7 +191,23 @@ def sys_maxwell2d():
     return "maxwell2d", 2, prim, build
 
 
-SYSTEMS = [sys_burgers2d, sys_swe2d, sys_euler2d, sys_adr2d, sys_nsf3d, sys_urf2d, sys_maxwell2d]
+def sys_allencahn2d():
+    gam, r = par(0), par(1)
+    k = TWO_PI
+    prim = {"phi": sp.Rational(7, 10) * sp.sin(k * x) * sp.cos(k * y) * sp.cos(t)}            # eq SM5.8
+
+    def build(P, D):
+        phi = P["phi"]
+        G = [dx * D(phi, x), dx * D(phi, y)]
+        gL = gam * dt / dx**2
+        Q = [phi, G[0], G[1]]
+        F = [[-gL * G[0], -gL * G[1]], [-phi / gtau, sp.Integer(0)], [sp.Integer(0), -phi / gtau]]   # eq 3.19
+        S = [dt * r * (phi - phi**3), -G[0] / gtau, -G[1] / gtau]
+        return Q, F, S
+    return "allencahn2d", 2, prim, build
+
+
+SYSTEMS = [sys_burgers2d, sys_swe2d, sys_euler2d, sys_adr2d, sys_nsf3d, sys_urf2d, sys_maxwell2d, sys_allencahn2d]
 
 
 # ------------------------------------------------------------------------------------------------ printing

@@ -63,6 +63,15 @@ def flux_maxwell_listing(U, c):
     return [[-Hy * c, Hx * c, z], [z, Ez * c, z], [-Ez * c, z, z]]
 
 
+def flux_allencahn_listing(U, gamma, r, tau_grad):
+    """SM4.8, PHYSICAL tracker G = grad phi. Returns (Phi, S) physical."""
+    phi, G0, G1 = U
+    z = np.zeros_like(phi)
+    Phi = [[-G0 * gamma, -G1 * gamma, z], [-phi / tau_grad, z, z], [z, -phi / tau_grad, z]]
+    S = [-phi**3 * r + phi * r, -G0 / tau_grad, -G1 / tau_grad]
+    return Phi, S
+
+
 def step(f, dim, omega, F_lat, S_lat):
     """One collide-and-stream step.
     f[k][i] : arrays (nz, ny, nx);  F_lat[k][a], S_lat[k] : lattice flux / source arrays at the

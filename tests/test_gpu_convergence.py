@@ -24,7 +24,7 @@ def P():
 @pytest.mark.parametrize("mk,kw,steps", [
     (W.pin_burgers, dict(n=40), 30), (W.pin_euler, dict(n=36), 25), (W.pin_adr, dict(n=32), 40), (W.c2_swe, dict(n=48, ny=20), 21),
     (W.c4_nsf3d, dict(n=16, ny=12, nz=10, precision="f64"), 9), (W.c4_nsf3d, dict(n=16, ny=12, nz=10), 8),
-    (W.pin_urf, dict(n=32), 17), (W.pin_maxwell, dict(n=32), 16)])
+    (W.pin_urf, dict(n=32), 17), (W.pin_maxwell, dict(n=32), 16), (W.pin_allencahn, dict(n=32), 40)])
 @pytest.mark.parametrize("pattern", ["pull2", "aa"])
 def test_error_norms_match_numpy(P, mk, kw, steps, pattern):
     """Device reductions vs norms formed in NumPy from the read-back state and the ORACLE's exact fields (jets)."""
@@ -66,6 +66,7 @@ TABLE2 = [
     (W.pin_urf, {"E": ((0,), 4.3449e-06, 2.1354e-06), "S": ((1, 2), 9.6256e-06, 6.3943e-06)}, "L527-L529"),
     (W.pin_maxwell, {"Ez": ((0,), 2.9956e-05, 2.9956e-05), "Hx": ((1,), 1.0951e-04, 1.0951e-04), "Hy": ((2,), 1.1587e-05, 1.1587e-05)}, "L530-L535"),
     (W.pin_adr, {"c": ((0,), 2.2901e-04, 1.2680e-04)}, "L540"),
+    (W.pin_allencahn, {"phi": ((0,), 7.3196e-04, 7.8653e-04)}, "L542"),
 ]
 
 

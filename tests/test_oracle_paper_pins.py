@@ -22,7 +22,8 @@ import workloads as W
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 PINS = json.load(open(os.path.join(HERE, "golden", "paper_pins.json")))
-MAKERS = {"burgers": W.pin_burgers, "euler": W.pin_euler, "adr": W.pin_adr, "urf": W.pin_urf, "maxwell": W.pin_maxwell}
+MAKERS = {"burgers": W.pin_burgers, "euler": W.pin_euler, "adr": W.pin_adr, "urf": W.pin_urf, "maxwell": W.pin_maxwell,
+          "allencahn": W.pin_allencahn}
 
 
 def _rows(case):
@@ -70,6 +71,8 @@ def test_p8_live_n64_matches_stored_row(case):
         live = {"u": e[0]}
     elif case == "euler":
         live = {"rho": e[0], "E": e[3], "rhou": (math.hypot(e[1][0], e[2][0]), math.hypot(e[1][1], e[2][1]))}
+    elif case == "allencahn":
+        live = {"phi": e[0]}
     elif case == "urf":
         live = {"E": e[0], "S": (math.hypot(e[1][0], e[2][0]), math.hypot(e[1][1], e[2][1]))}
     elif case == "maxwell":

@@ -13,12 +13,12 @@ import oracle
 import workloads as W
 from oracle import OracleGrid
 
-from brute_force import (LATTICES, flux_adr_listing, flux_euler_listing, flux_maxwell_listing, flux_swe_listing, flux_urf_listing,
+from brute_force import (LATTICES, flux_adr_listing, flux_allencahn_listing, flux_euler_listing, flux_maxwell_listing, flux_swe_listing, flux_urf_listing,
                          init_equilibrium, moments, step as bf_step)
 
-SYSTEMS = ["advection2d", "burgers2d", "swe2d", "euler2d", "adr2d", "nsf3d", "mhd3d", "urf2d", "maxwell2d"]
+SYSTEMS = ["advection2d", "burgers2d", "swe2d", "euler2d", "adr2d", "nsf3d", "mhd3d", "urf2d", "maxwell2d", "allencahn2d"]
 PARAMS = {"advection2d": [0.1, 0.05], "burgers2d": [], "swe2d": [1.0], "euler2d": [1.4],
-          "adr2d": [0.1, -0.1, 0.01, 1.0], "nsf3d": [1.4, 1e-3, 4.9e-3], "mhd3d": [1.4, 1e-3], "urf2d": [], "maxwell2d": [1.0]}
+          "adr2d": [0.1, -0.1, 0.01, 1.0], "nsf3d": [1.4, 1e-3, 4.9e-3], "mhd3d": [1.4, 1e-3], "urf2d": [], "maxwell2d": [1.0], "allencahn2d": [0.01, 1.0]}
 
 
 def small_grid(system, **kw):
@@ -39,7 +39,7 @@ def physical_state(system, rng, shape=()):
         U[3] = rng.uniform(2.0, 3.0, size=shape)
     if system in ("nsf3d", "mhd3d"):
         U[4] = rng.uniform(2.0, 3.0, size=shape)
-    if system in ("advection2d", "burgers2d", "adr2d"):
+    if system in ("advection2d", "burgers2d", "adr2d", "allencahn2d"):
         U[0] = rng.uniform(0.2, 0.9, size=shape)
     if system == "urf2d":                       # physicality E > |S|
         U[0] = rng.uniform(1.0, 2.0, size=shape)
@@ -269,6 +269,7 @@ MMS_CASES = {
     "nsf3d": lambda: W.c4_nsf3d(16),
     "urf2d": lambda: W.pin_urf(32),
     "maxwell2d": lambda: W.pin_maxwell(32),
+    "allencahn2d": lambda: W.pin_allencahn(32),
 }
 
 
@@ -369,6 +370,12 @@ def _bf_run(system, w, steps, listing_flux):
             F = [[il * Phi[0][a] for a in range(3)]] + [[il * w.dx * Phi[k][a] for a in range(3)] for k in (1, 2)]
             S = [dt * (-R * Uc[0] ** 2 + R * Uc[0]), dt * (-Uc[1] / tau_grad), dt * (-Uc[2] / tau_grad)]
             return F, S
+        if system == "allencahn2d":
+            gam, r = w.params
+            tau_grad = w.g_tau * dt
+            Phi, Sp = flux_allencahn_listing([Uc[0], Uc[1] / w.dx, Uc[2] / w.dx], gam, r, tau_grad)
+            F = [[il * Phi[0][a] for a in range(3)]] + [[il * w.dx * Phi[k][a] for a in range(3)] for k in (1, 2)]
+            return F, [dt * Sp[0], dt * w.dx * Sp[1], dt * w.dx * Sp[2]]
         Phi = listing_flux(Uc)
         return [[il * Phi[k][a] for a in range(3)] for k in range(len(Uc))], [0.0 * Uc[0] for _ in Uc]
 
@@ -399,6 +406,14 @@ def test_p13_brute_force_adr_tracker():
     w.mms_id = 0
     w.steps = 12
     exp = _bf_run("adr2d", w, w.steps, None)
+    assert np.abs(oracle.run(w) - exp).max() < 1e-14
+
+
+def test_p13_brute_force_allencahn_tracker():
+    w = W.pin_allencahn(8)
+    w.mms_id = 0
+    w.steps = 12
+    exp = _bf_run("allencahn2d", w, w.steps, None)
     assert np.abs(oracle.run(w) - exp).max() < 1e-14
 
 

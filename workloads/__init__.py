@@ -39,12 +39,13 @@ COMPONENTS: Dict[str, List[str]] = {
     "mhd3d": ["rho", "mx", "my", "mz", "E", "Bx", "By", "Bz", "Jx", "Jy", "Jz"],
     "urf2d": ["E", "Sx", "Sy"],
     "maxwell2d": ["Ez", "Hx", "Hy"],
+    "allencahn2d": ["phi", "Gx", "Gy"],
 }
 N_CONSERVED = {"advection2d": 1, "burgers2d": 1, "swe2d": 3, "euler2d": 4,
-               "adr2d": 1, "nsf3d": 5, "mhd3d": 8, "urf2d": 3, "maxwell2d": 3}
+               "adr2d": 1, "nsf3d": 5, "mhd3d": 8, "urf2d": 3, "maxwell2d": 3, "allencahn2d": 1}
 LATTICE_OF = {"advection2d": "D2Q5", "burgers2d": "D2Q5", "swe2d": "D2Q5",
               "euler2d": "D2Q5", "adr2d": "D2Q5", "nsf3d": "D3Q7", "mhd3d": "D3Q7",
-              "urf2d": "D2Q5", "maxwell2d": "D2Q5"}
+              "urf2d": "D2Q5", "maxwell2d": "D2Q5", "allencahn2d": "D2Q5"}
 # c_s^2 per lattice, Table SM1; used only by the lambda rule below.
 CS2 = {"D2Q5": 1.0 / 3.0, "D3Q7": 1.0 / 4.0}
 SIGMA = 0.6  # lambda rule: lattice wave speed = SIGMA * c_s^2 (SURVEY.md §8(c) "lambda rule")
@@ -392,6 +393,27 @@ def pin_maxwell(n: int = 512, precision: str = "f64", f: float = 0.2) -> Workloa
                     dx=1.0 / n, lam=1.0 / f, params=[1.0], tau_R=0.2, g_tau=0.0, U_ref=[0.0, 0.0, 0.0], mms_id=1,
                     mms_params=[], steps=int(round(n / f)), s_max=1.0, seed=0, init=_init_maxwell,
                     note="PAPER.md Table 2 L530-L535")
+
+
+def _init_allencahn(w: Workload) -> np.ndarray:
+    # eq (SM5.8), PAPER.md:L1310 at t = 0; trackers = dx * analytic gradient
+    x, y, _ = _grid(w)
+    k = TWO_PI
+    phi = 0.7 * np.sin(k * x) * np.cos(k * y)
+    gx = 0.7 * k * np.cos(k * x) * np.cos(k * y)
+    gy = -0.7 * k * np.sin(k * x) * np.sin(k * y)
+    return np.stack([_full(w, phi), _full(w, w.dx * gx), _full(w, w.dx * gy)]).copy()
+
+
+def pin_allencahn(n: int = 512, precision: str = "f64") -> Workload:
+    # Table SM2: diffusive f = 1.9 (dt = 1.9 dx^2), tau_R = 50, g_tau = 6; Table SM9: gamma = 0.01, r = 1
+    f = 1.9
+    dx = 1.0 / n
+    dt = f * dx * dx
+    return Workload(name=f"pin_allencahn2d_{n}", system="allencahn2d", nx=n, ny=n, nz=1, precision=precision,
+                    dx=dx, lam=dx / dt, params=[0.01, 1.0], tau_R=50.0, g_tau=6.0, U_ref=[0.0, 0.0, 0.0], mms_id=1,
+                    mms_params=[], steps=int(round(1.0 / dt)), s_max=0.0, seed=0, init=_init_allencahn,
+                    note="PAPER.md Table 2 L542")
 
 
 BASELINE_CONFIGS: Dict[str, Callable[..., Workload]] = {
