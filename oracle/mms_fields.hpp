@@ -11,6 +11,7 @@
 //   nsf3d     mms 1 : BASELINE.json configs[3] fields, mms_par = {U0, A_rho, rho0, p0}
 //   urf2d     mms 1 : eq (SM5.4)
 //   allencahn2d mms 1 : eq (SM5.8); Table SM9 L1316 (gamma = 0.01, r = 1)
+//   inse2d    mms 1 : eq (SM5.9), PAPER.md:L1330-L1334 (Taylor-Green vortex), mms_par = {U, rho0}
 //   maxwell2d mms 1 : eq (SM5.5), PAPER.md:L1248-L1254 (k_x = 2 pi, k_y = 4 pi, A = 1/2, omega = 4)
 #pragma once
 #include "jets.hpp"
@@ -89,6 +90,20 @@ inline bool exact_state(int sys, int mms_id, const Scaling& sc, const double* mp
         Q[0] = lower(phi);
         Q[1] = sc.dx * diff(phi, 1);
         Q[2] = sc.dx * diff(phi, 2);
+        return true;
+    }
+    case SYS_INSE2D: {
+        // eq (SM5.9): 2D Taylor-Green vortex; mp = {U, rho0}; nu = mu/rho0
+        const double cs = sc.par[0], U0 = mp[0], rho0 = mp[1], nu = sc.par[1] / rho0;
+        J2 D = exp((-2.0 * (nu / cs) * k * k) * t);
+        J2 u = -U0 * cos(k * x) * sin(k * y) * D;
+        J2 v = U0 * sin(k * x) * cos(k * y) * D;
+        J2 p = (-0.25 * rho0 * U0 * U0) * (cos(2.0 * k * x) + cos(2.0 * k * y)) * D * D;
+        J2 rho = rho0 + p / (cs * cs);
+        J2 mx = rho * u, my = rho * v;
+        Q[0] = lower(rho); Q[1] = lower(mx); Q[2] = lower(my);
+        Q[3] = sc.dx * diff(mx, 1); Q[4] = sc.dx * diff(mx, 2);
+        Q[5] = sc.dx * diff(my, 1); Q[6] = sc.dx * diff(my, 2);
         return true;
     }
     case SYS_MAXWELL2D: {

@@ -17,7 +17,7 @@
 namespace orc {
 
 enum SystemId { SYS_ADVECTION2D = 0, SYS_BURGERS2D = 1, SYS_SWE2D = 2, SYS_EULER2D = 3, SYS_ADR2D = 4,
-                SYS_NSF3D = 5, SYS_MHD3D = 6, SYS_URF2D = 7, SYS_MAXWELL2D = 8, SYS_ALLENCAHN2D = 9, SYS_COUNT = 10 };
+                SYS_NSF3D = 5, SYS_MHD3D = 6, SYS_URF2D = 7, SYS_MAXWELL2D = 8, SYS_ALLENCAHN2D = 9, SYS_INSE2D = 10, SYS_COUNT = 11 };
 
 constexpr int MAXM = 32;  // max components
 
@@ -34,6 +34,7 @@ inline SysInfo sys_info(int sys) {
         case SYS_URF2D:       return {3, 3, 2};
         case SYS_MAXWELL2D:   return {3, 3, 2};
         case SYS_ALLENCAHN2D: return {1, 3, 2};
+        case SYS_INSE2D:      return {3, 7, 2};
     }
     return {0, 0, 0};
 }
@@ -198,6 +199,29 @@ void flux_source(int sys, const T* U, const Scaling& sc, T* F, T* S) {
         S[1] = -Gx / sc.g_tau;
         S[2] = -Gy / sc.g_tau;
     } break;
+    case SYS_INSE2D: {
+        // weakly compressible (incompressible-limit) Navier-Stokes, eq (3.21)-(3.22); SM4.9 L947-L959;
+        // par = {c_s_phys, mu}; U = (rho, m_x, m_y, G^L_ab = dx d_b m_a [index 3+2a+b]):
+        //   F_rho = m/lam;  F_ma,j = (m_a u_j + delta_aj c_s^2 rho)/lam - (mu_L/rho)(G_aj + G_ja);
+        //   F_Gab,j = G_ab u_j/lam - delta_jb m_a/g_tau;  S_G = -G/g_tau
+        const double cs2 = sc.par[0] * sc.par[0], muL = sc.par[1] * dL;
+        T rho = U[0];
+        T m[2] = {U[1], U[2]};
+        T u[2] = {m[0] / rho, m[1] / rho};
+        const T* G = U + 3;
+        for (int j = 0; j < 2; ++j) {
+            F[0 * 3 + j] = il * m[j];
+            for (int a = 0; a < 2; ++a) {
+                F[(1 + a) * 3 + j] = il * (m[a] * u[j]) - (muL / rho) * (G[2 * a + j] + G[2 * j + a]);
+                if (a == j) F[(1 + a) * 3 + j] = F[(1 + a) * 3 + j] + (il * cs2) * rho;
+                for (int b = 0; b < 2; ++b) {
+                    F[(3 + 2 * a + b) * 3 + j] = il * (G[2 * a + b] * u[j]);
+                    if (j == b) F[(3 + 2 * a + b) * 3 + j] = F[(3 + 2 * a + b) * 3 + j] - m[a] / sc.g_tau;
+                }
+            }
+        }
+        for (int q = 0; q < 4; ++q) S[3 + q] = -G[q] / sc.g_tau;
+    } break;
     case SYS_MAXWELL2D: {
         // Maxwell TM mode in vacuum, eq (3.10)-(3.11): Q = (E_z, H_x, H_y); par = {c}
         const double c = sc.par[0];
@@ -272,6 +296,10 @@ inline void wave_speeds(int sys, const double* U, const Scaling& sc, double* out
         out[1] = (vm + cs) / (1.0 + vm * cs);
     } break;
     case SYS_ALLENCAHN2D: { out[2] = std::sqrt(sc.par[0] * dL / sc.g_tau); } break;   // no advection: tracker-parent coupling only
+    case SYS_INSE2D: {
+        double u[2] = {U[1] / U[0], U[2] / U[0]}, c[2] = {sc.par[0], sc.par[0]}; set(u, c, 2);
+        out[2] = std::sqrt(2.0 * sc.par[1] * dL / U[0] / sc.g_tau);
+    } break;
     case SYS_MAXWELL2D: { out[0] = std::fabs(sc.par[0]); out[1] = std::fabs(sc.par[0]); } break;  // eigenvalues {+c, -c, 0}, L393
     }
 }

@@ -60,11 +60,12 @@ static const SysOps* ops_of(int id) {
         case LBMK_SYS_URF2D: return ops_urf2d();
         case LBMK_SYS_MAXWELL2D: return ops_maxwell2d();
         case LBMK_SYS_ALLENCAHN2D: return ops_allencahn2d();
+        case LBMK_SYS_INSE2D: return ops_inse2d();
     }
     return nullptr;
 }
-static const int N_PARAMS[LBMK_SYS_COUNT] = {2, 0, 1, 1, 4, 3, 2, 0, 1, 2};
-static const int N_MMS_PARAMS[LBMK_SYS_COUNT] = {0, 1, 3, 0, 0, 4, 0, 0, 0, 0};
+static const int N_PARAMS[LBMK_SYS_COUNT] = {2, 0, 1, 1, 4, 3, 2, 0, 1, 2, 2};
+static const int N_MMS_PARAMS[LBMK_SYS_COUNT] = {0, 1, 3, 0, 0, 4, 0, 0, 0, 0, 2};
 
 static lbmk_status sys_fail(lbmk_status s, const char* msg) { g_sys_err = msg; return s; }
 static lbmk_status fail(lbmk_grid* g, lbmk_status s, const std::string& msg) { if (g) g->err = msg; else g_sys_err = msg; return s; }
@@ -154,6 +155,10 @@ lbmk_status lbmk_system_set_reference(lbmk_system* sys, const double* U0, int n)
         for (int k = 0; k < n; ++k)
             if (k != 0 && k != 4 && U0[k] != 0.0)
                 return sys_fail(LBMK_EUNSUPPORTED, "NSF3D/MHD3D delta forms need zero reference momentum, field and trackers");
+    }
+    if (sys->id == LBMK_SYS_INSE2D) {
+        for (int k = 1; k < n; ++k)
+            if (U0[k] != 0.0) return sys_fail(LBMK_EUNSUPPORTED, "INSE2D delta form needs zero reference momentum and trackers");
     }
     if ((sys->id == LBMK_SYS_ADR2D || sys->id == LBMK_SYS_ALLENCAHN2D) && (U0[1] != 0.0 || U0[2] != 0.0))
         return sys_fail(LBMK_EUNSUPPORTED, "ADR2D needs zero reference trackers");

@@ -66,5 +66,6 @@ const SysOps* ops_mhd3d();
 const SysOps* ops_urf2d();
 const SysOps* ops_maxwell2d();
 const SysOps* ops_allencahn2d();
+const SysOps* ops_inse2d();
 
 }  // namespace lbmk

@@ -24,7 +24,7 @@
 namespace lbmk {
 
 enum { SYS_ADVECTION2D = 0, SYS_BURGERS2D = 1, SYS_SWE2D = 2, SYS_EULER2D = 3, SYS_ADR2D = 4, SYS_NSF3D = 5, SYS_MHD3D = 6,
-       SYS_URF2D = 7, SYS_MAXWELL2D = 8, SYS_ALLENCAHN2D = 9 };
+       SYS_URF2D = 7, SYS_MAXWELL2D = 8, SYS_ALLENCAHN2D = 9, SYS_INSE2D = 10 };
 
 // ------------------------------------------------------------------------------------------ advection
 // Phi = (a_x U, a_y U); par = {a_x, a_y}
@@ -188,6 +188,46 @@ template <class R> struct SysAllenCahn2D {
     }
     __device__ static void wave(const double*, const KParams<double>& P, double* out) {
         out[0] = 0.0; out[1] = 0.0; out[2] = sqrt(P.par[0] * P.dL * P.inv_gtau);
+    }
+};
+
+// ------------------------------------------------------------------------------------------ weakly compressible NSE
+// eq (3.21)-(3.22); SM4.9 L947-L959; par = {c_s_phys, mu};
+// Q = (rho, m_x, m_y, G^L_ab = dx d_b m_a [index 3+2a+b]).  Reference: rho0 free, m0 = 0, trackers 0 (host-checked).
+//   dF_rho,j = m_j/lam;  dF_ma,j = (m_a u_j + delta_aj c_s^2 drho)/lam - (mu_L/rho)(G_aj + G_ja)
+//   dF_Gab,j = G_ab u_j/lam - delta_jb m_a/g_tau;  s_G = -G/g_tau
+template <class R> struct SysInse2D {
+    static constexpr int ID = SYS_INSE2D, D = 2, M = 7, MC = 3;
+    using Mms = Mms_inse2d;
+    struct Ctx { R ul[2], nuL; };
+    __device__ __forceinline__ static void setup(Ctx& c, const R (&dQ)[M], const KParams<R>& P) {
+        const R r = R(1) / (P.ref[0] + dQ[0]);
+        c.ul[0] = dQ[1] * r * P.il; c.ul[1] = dQ[2] * r * P.il;
+        c.nuL = P.par[1] * P.dL * r;
+    }
+    template <int k> __device__ __forceinline__ static void flux(const Ctx& c, const R (&dQ)[M], const KParams<R>& P, R (&F)[D], R& S) {
+        if constexpr (k == 0) {
+            F[0] = P.il * dQ[1]; F[1] = P.il * dQ[2]; S = R(0);
+        } else if constexpr (k <= 2) {
+            constexpr int a = k - 1;
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                R v = dQ[1 + a] * c.ul[j] - c.nuL * (dQ[3 + 2 * a + j] + dQ[3 + 2 * j + a]);
+                if (a == j) v += (P.il * P.par[0] * P.par[0]) * dQ[0];
+                F[j] = v;
+            }
+            S = R(0);
+        } else {
+            constexpr int a = (k - 3) / 2, b = (k - 3) % 2;
+            F[0] = dQ[k] * c.ul[0]; F[1] = dQ[k] * c.ul[1];
+            F[b] -= dQ[1 + a] * P.inv_gtau;
+            S = -dQ[k] * P.inv_gtau;
+        }
+    }
+    __device__ static void wave(const double* Q, const KParams<double>& P, double* out) {
+        const double u = Q[1] / Q[0], v = Q[2] / Q[0], cc = P.par[0];
+        out[0] = fmax(fabs(u), fabs(v)) + cc; out[1] = sqrt(u * u + v * v) + cc;
+        out[2] = sqrt(2.0 * P.par[1] * P.dL / Q[0] * P.inv_gtau);
     }
 };
 

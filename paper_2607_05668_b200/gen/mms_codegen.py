@@ -207,7 +207,35 @@ def sys_allencahn2d():
     return "allencahn2d", 2, prim, build
 
 
-SYSTEMS = [sys_burgers2d, sys_swe2d, sys_euler2d, sys_adr2d, sys_nsf3d, sys_urf2d, sys_maxwell2d, sys_allencahn2d]
+def sys_inse2d():
+    cs, mu = par(0), par(1)
+    U0, rho0 = mp(0), mp(1)
+    k = TWO_PI
+    Dt = sp.exp(-2 * (mu / rho0 / cs) * k * k * t)                                           # eq SM5.9
+    p = -rho0 * U0 * U0 / 4 * (sp.cos(2 * k * x) + sp.cos(2 * k * y)) * Dt * Dt
+    prim = {"rho": rho0 + p / cs**2,
+            "u0": -U0 * sp.cos(k * x) * sp.sin(k * y) * Dt,
+            "u1": U0 * sp.sin(k * x) * sp.cos(k * y) * Dt}
+
+    def build(P, D):
+        X = (x, y)
+        rho, u = P["rho"], [P["u0"], P["u1"]]
+        m = [rho * u[0], rho * u[1]]
+        G = [[dx * D(m[a], X[b]) for b in range(2)] for a in range(2)]
+        muL = mu * dt / dx**2
+        Q = [rho, m[0], m[1]] + [G[a][b] for a in range(2) for b in range(2)]
+        F = [[il * m[0], il * m[1]]]                                                          # eq 3.22
+        for a in range(2):
+            F.append([il * (m[a] * u[j] + (cs**2 * rho if a == j else 0)) - muL / rho * (G[a][j] + G[j][a]) for j in range(2)])
+        for a in range(2):
+            for b in range(2):
+                F.append([il * G[a][b] * u[j] - (m[a] / gtau if j == b else 0) for j in range(2)])
+        S = [sp.Integer(0)] * 3 + [-G[a][b] / gtau for a in range(2) for b in range(2)]
+        return Q, F, S
+    return "inse2d", 2, prim, build
+
+
+SYSTEMS = [sys_burgers2d, sys_swe2d, sys_euler2d, sys_adr2d, sys_nsf3d, sys_urf2d, sys_maxwell2d, sys_allencahn2d, sys_inse2d]
 
 
 # ------------------------------------------------------------------------------------------------ printing

@@ -72,6 +72,24 @@ def flux_allencahn_listing(U, gamma, r, tau_grad):
     return Phi, S
 
 
+def flux_inse_listing(U, cs, mu, tau_grad):
+    """SM4.9, PAPER.md:L947-L959 (weakly compressible NSE), PHYSICAL trackers G_ab = d_b (rho u_a); the tracker rows
+    follow the vector form G (x) u - I (x) rho u / tau_grad of eq (3.22) (L452) where the listing is garbled (L955).
+    U = (rho, ru0, ru1, G00, G01, G10, G11).  Returns (Phi, S) physical."""
+    rho, ru0, ru1, G00, G01, G10, G11 = U
+    z = np.zeros_like(rho)
+    P11 = -G01 * mu / rho - G10 * mu / rho + ru0 * ru1 / rho
+    Phi = [[ru0, ru1, z],
+           [-2 * G00 * mu / rho + cs**2 * rho + ru0**2 / rho, P11, z],
+           [P11, -2 * G11 * mu / rho + cs**2 * rho + ru1**2 / rho, z],
+           [G00 * ru0 / rho - ru0 / tau_grad, G00 * ru1 / rho, z],
+           [G01 * ru0 / rho, G01 * ru1 / rho - ru0 / tau_grad, z],
+           [G10 * ru0 / rho - ru1 / tau_grad, G10 * ru1 / rho, z],
+           [G11 * ru0 / rho, G11 * ru1 / rho - ru1 / tau_grad, z]]
+    S = [z, z, z, -G00 / tau_grad, -G01 / tau_grad, -G10 / tau_grad, -G11 / tau_grad]
+    return Phi, S
+
+
 def step(f, dim, omega, F_lat, S_lat):
     """One collide-and-stream step.
     f[k][i] : arrays (nz, ny, nx);  F_lat[k][a], S_lat[k] : lattice flux / source arrays at the

@@ -24,7 +24,7 @@ def P():
 @pytest.mark.parametrize("mk,kw,steps", [
     (W.pin_burgers, dict(n=40), 30), (W.pin_euler, dict(n=36), 25), (W.pin_adr, dict(n=32), 40), (W.c2_swe, dict(n=48, ny=20), 21),
     (W.c4_nsf3d, dict(n=16, ny=12, nz=10, precision="f64"), 9), (W.c4_nsf3d, dict(n=16, ny=12, nz=10), 8),
-    (W.pin_urf, dict(n=32), 17), (W.pin_maxwell, dict(n=32), 16), (W.pin_allencahn, dict(n=32), 40)])
+    (W.pin_urf, dict(n=32), 17), (W.pin_maxwell, dict(n=32), 16), (W.pin_allencahn, dict(n=32), 40), (W.pin_inse, dict(n=32), 40)])
 @pytest.mark.parametrize("pattern", ["pull2", "aa"])
 def test_error_norms_match_numpy(P, mk, kw, steps, pattern):
     """Device reductions vs norms formed in NumPy from the read-back state and the ORACLE's exact fields (jets)."""
@@ -85,6 +85,25 @@ def test_paper_table2_double_rows_reproduced_on_the_gpu(P, mk, fields, cite):
         got_l2 = math.sqrt(sum(n[k][1] ** 2 for k in ks))
         print(f"{w.name} {name}: Linf {got_linf:.4e} (paper {linf:.4e})  L2 {got_l2:.4e} (paper {l2:.4e})  PAPER.md:{cite}")
         assert _sig5(got_l2, l2) and _sig5(got_linf, linf), (w.name, name, got_linf, got_l2)
+
+
+def test_paper_table2_inse_row_partially_reproduced(P):
+    """Weakly compressible NSE.  The listing of its tracker fluxes is inconsistent with eq (3.22)
+    (SM4.9 L955: Phi_{4,1}, Phi_{6,1} print rho u_0 where G (x) u gives rho u_1); the vector form is used.  It
+    reproduces the printed momentum L2 error to 3 digits; rho (an O(Ma^2) quantity, 6e-7) and the momentum Linf do
+    not match to the printed precision -- an unresolved reading, so this system's parity is UNPINNED beyond
+    P1/P3/P10/P13.  Gate: momentum L2 within 0.2 %, the rest within 50 %, values printed."""
+    w = W.pin_inse(512)
+    g = P.Grid.from_workload(w)
+    g.init_from_U(w.initial_U())
+    g.step(w.steps)
+    n = g.error_norms()
+    g.close()
+    mom_l2, mom_linf = math.hypot(n[1][1], n[2][1]), math.hypot(n[1][2], n[2][2])
+    print(f"{w.name}: rho Linf {n[0][2]:.4e} (paper 1.3419e-06) L2 {n[0][1]:.4e} (paper 6.0683e-07); "
+          f"rho u Linf {mom_linf:.4e} (paper 8.2447e-04) L2 {mom_l2:.4e} (paper 8.5394e-04)")
+    assert abs(mom_l2 - 8.5394e-04) <= 2e-3 * 8.5394e-04
+    assert abs(mom_linf - 8.2447e-04) <= 0.5 * 8.2447e-04 and abs(n[0][1] - 6.0683e-07) <= 0.5 * 6.0683e-07
 
 
 @pytest.mark.parametrize("mk,field,paper_l2", [(W.pin_urf, 0, 4.7227e-06), (W.pin_maxwell, 0, 3.0632e-05)])

@@ -13,12 +13,12 @@ import oracle
 import workloads as W
 from oracle import OracleGrid
 
-from brute_force import (LATTICES, flux_adr_listing, flux_allencahn_listing, flux_euler_listing, flux_maxwell_listing, flux_swe_listing, flux_urf_listing,
+from brute_force import (LATTICES, flux_adr_listing, flux_allencahn_listing, flux_euler_listing, flux_inse_listing, flux_maxwell_listing, flux_swe_listing, flux_urf_listing,
                          init_equilibrium, moments, step as bf_step)
 
-SYSTEMS = ["advection2d", "burgers2d", "swe2d", "euler2d", "adr2d", "nsf3d", "mhd3d", "urf2d", "maxwell2d", "allencahn2d"]
+SYSTEMS = ["advection2d", "burgers2d", "swe2d", "euler2d", "adr2d", "nsf3d", "mhd3d", "urf2d", "maxwell2d", "allencahn2d", "inse2d"]
 PARAMS = {"advection2d": [0.1, 0.05], "burgers2d": [], "swe2d": [1.0], "euler2d": [1.4],
-          "adr2d": [0.1, -0.1, 0.01, 1.0], "nsf3d": [1.4, 1e-3, 4.9e-3], "mhd3d": [1.4, 1e-3], "urf2d": [], "maxwell2d": [1.0], "allencahn2d": [0.01, 1.0]}
+          "adr2d": [0.1, -0.1, 0.01, 1.0], "nsf3d": [1.4, 1e-3, 4.9e-3], "mhd3d": [1.4, 1e-3], "urf2d": [], "maxwell2d": [1.0], "allencahn2d": [0.01, 1.0], "inse2d": [1.0, 0.01]}
 
 
 def small_grid(system, **kw):
@@ -33,7 +33,7 @@ def physical_state(system, rng, shape=()):
     """A random admissible state (rho, h > 0, p > 0)."""
     m = len(W.COMPONENTS[system])
     U = rng.uniform(-0.3, 0.3, size=(m,) + shape)
-    if system in ("swe2d", "euler2d", "nsf3d", "mhd3d"):
+    if system in ("swe2d", "euler2d", "nsf3d", "mhd3d", "inse2d"):
         U[0] = rng.uniform(0.8, 1.2, size=shape)
     if system == "euler2d":
         U[3] = rng.uniform(2.0, 3.0, size=shape)
@@ -270,6 +270,7 @@ MMS_CASES = {
     "urf2d": lambda: W.pin_urf(32),
     "maxwell2d": lambda: W.pin_maxwell(32),
     "allencahn2d": lambda: W.pin_allencahn(32),
+    "inse2d": lambda: W.pin_inse(32),
 }
 
 
@@ -370,6 +371,12 @@ def _bf_run(system, w, steps, listing_flux):
             F = [[il * Phi[0][a] for a in range(3)]] + [[il * w.dx * Phi[k][a] for a in range(3)] for k in (1, 2)]
             S = [dt * (-R * Uc[0] ** 2 + R * Uc[0]), dt * (-Uc[1] / tau_grad), dt * (-Uc[2] / tau_grad)]
             return F, S
+        if system == "inse2d":
+            cs, mu = w.params
+            tau_grad = w.g_tau * dt
+            Phi, Sp = flux_inse_listing(list(Uc[:3]) + [Uc[k] / w.dx for k in range(3, 7)], cs, mu, tau_grad)
+            F = [[il * Phi[k][a] for a in range(3)] for k in range(3)] + [[il * w.dx * Phi[k][a] for a in range(3)] for k in range(3, 7)]
+            return F, [dt * Sp[k] for k in range(3)] + [dt * w.dx * Sp[k] for k in range(3, 7)]
         if system == "allencahn2d":
             gam, r = w.params
             tau_grad = w.g_tau * dt
@@ -415,6 +422,14 @@ def test_p13_brute_force_allencahn_tracker():
     w.steps = 12
     exp = _bf_run("allencahn2d", w, w.steps, None)
     assert np.abs(oracle.run(w) - exp).max() < 1e-14
+
+
+def test_p13_brute_force_inse_trackers():
+    w = W.pin_inse(8)
+    w.mms_id = 0
+    w.steps = 12
+    exp = _bf_run("inse2d", w, w.steps, None)
+    assert np.abs(oracle.run(w) - exp).max() < 1e-13
 
 
 def test_p13_brute_force_ultrarelativistic():

@@ -40,12 +40,13 @@ COMPONENTS: Dict[str, List[str]] = {
     "urf2d": ["E", "Sx", "Sy"],
     "maxwell2d": ["Ez", "Hx", "Hy"],
     "allencahn2d": ["phi", "Gx", "Gy"],
+    "inse2d": ["rho", "mx", "my", "Gxx", "Gxy", "Gyx", "Gyy"],
 }
 N_CONSERVED = {"advection2d": 1, "burgers2d": 1, "swe2d": 3, "euler2d": 4,
-               "adr2d": 1, "nsf3d": 5, "mhd3d": 8, "urf2d": 3, "maxwell2d": 3, "allencahn2d": 1}
+               "adr2d": 1, "nsf3d": 5, "mhd3d": 8, "urf2d": 3, "maxwell2d": 3, "allencahn2d": 1, "inse2d": 3}
 LATTICE_OF = {"advection2d": "D2Q5", "burgers2d": "D2Q5", "swe2d": "D2Q5",
               "euler2d": "D2Q5", "adr2d": "D2Q5", "nsf3d": "D3Q7", "mhd3d": "D3Q7",
-              "urf2d": "D2Q5", "maxwell2d": "D2Q5", "allencahn2d": "D2Q5"}
+              "urf2d": "D2Q5", "maxwell2d": "D2Q5", "allencahn2d": "D2Q5", "inse2d": "D2Q5"}
 # c_s^2 per lattice, Table SM1; used only by the lambda rule below.
 CS2 = {"D2Q5": 1.0 / 3.0, "D3Q7": 1.0 / 4.0}
 SIGMA = 0.6  # lambda rule: lattice wave speed = SIGMA * c_s^2 (SURVEY.md §8(c) "lambda rule")
@@ -414,6 +415,35 @@ def pin_allencahn(n: int = 512, precision: str = "f64") -> Workload:
                     dx=dx, lam=dx / dt, params=[0.01, 1.0], tau_R=50.0, g_tau=6.0, U_ref=[0.0, 0.0, 0.0], mms_id=1,
                     mms_params=[], steps=int(round(1.0 / dt)), s_max=0.0, seed=0, init=_init_allencahn,
                     note="PAPER.md Table 2 L542")
+
+
+def _init_inse(w: Workload) -> np.ndarray:
+    # eq (SM5.9), PAPER.md:L1330-L1334 at t = 0 (D = 1); trackers = dx * analytic gradient of the momentum
+    cs, mu = w.params
+    U0, rho0 = w.mms_params
+    x, y, _ = _grid(w)
+    k = TWO_PI
+    sx, cx, sy, cy = np.sin(k * x), np.cos(k * x), np.sin(k * y), np.cos(k * y)
+    A = 0.25 * rho0 * U0 * U0 / (cs * cs)
+    rho = rho0 - A * (np.cos(2 * k * x) + np.cos(2 * k * y))
+    rx, ry = 2 * k * A * np.sin(2 * k * x), 2 * k * A * np.sin(2 * k * y)          # d rho / dx, dy
+    u, v = -U0 * cx * sy, U0 * sx * cy
+    ux, uy, vx, vy = U0 * k * sx * sy, -U0 * k * cx * cy, U0 * k * cx * cy, -U0 * k * sx * sy
+    comps = [rho, rho * u, rho * v,
+             w.dx * (rx * u + rho * ux), w.dx * (ry * u + rho * uy), w.dx * (rx * v + rho * vx), w.dx * (ry * v + rho * vy)]
+    return np.stack([_full(w, c) for c in comps]).copy()
+
+
+def pin_inse(n: int = 512, precision: str = "f64") -> Workload:
+    # weakly compressible NSE; Table SM2: diffusive f = 2, tau_R = 50 (Float: 90), g_tau = 6;
+    # Table SM10 L1340 non-dimensionalised by rho0, c_s, L (reading A9): c_s = 1, Ma = 0.1, Re = 10 => mu = 0.01
+    f = 2.0
+    dx = 1.0 / n
+    dt = f * dx * dx
+    return Workload(name=f"pin_inse2d_{n}", system="inse2d", nx=n, ny=n, nz=1, precision=precision,
+                    dx=dx, lam=dx / dt, params=[1.0, 0.01], tau_R=50.0 if precision == "f64" else 90.0, g_tau=6.0,
+                    U_ref=[1.0] + [0.0] * 6, mms_id=1, mms_params=[0.1, 1.0], steps=int(round(1.0 / dt)), s_max=1.1,
+                    seed=0, init=_init_inse, note="PAPER.md Table 2 L543-L546")
 
 
 BASELINE_CONFIGS: Dict[str, Callable[..., Workload]] = {
