@@ -241,7 +241,7 @@ def short_run(P, torch, name, pattern):
     return out
 
 
-# The paper's Table 3 rows (PAPER.md:L577-L592) that have a compiled-in system here: bulk collide-and-stream without
+# The paper's Table 3 rows (PAPER.md:L577-L594) that have a compiled-in system here: bulk collide-and-stream without
 # manufactured forcing, single (shifted fp32) and double precision, on a saturating grid.  Paper columns: MLUPS and
 # % of its 680 GB/s BabelStream peak on an RTX A5000 (context only -- another GPU, other kernels).
 TABLE3 = [  # (label, workload maker name, paper S (MLUPS, %), paper D (MLUPS, %))
@@ -252,6 +252,7 @@ TABLE3 = [  # (label, workload maker name, paper S (MLUPS, %), paper D (MLUPS, %
     ("maxwell", "pin_maxwell", (5269, 93.0), (2634, 93.0)),
     ("adr", "pin_adr", (5405, 95.4), (1673, 59.0)),
     ("allen-cahn", "pin_allencahn", (5487, 96.8), (1918, 67.7)),
+    ("incompressible-nse", "pin_inse", (2328, 95.8), (662, 54.6)),
 ]
 
 
