@@ -14,7 +14,7 @@ template <> __host__ inline KParams<double>& kp<double>(GridCore& g) { return g.
 template <> __host__ inline KParams<float>& kp<float>(GridCore& g) { return g.Pf; }
 
 // launch shape of the node kernel per system: threads per block, min blocks per SM (register cap)
-template <template <class> class S, class R> struct Tune { static constexpr int BLOCK = 256, MINB = 1; };
+template <template <class> class S, class R> struct Tune { static constexpr int BLOCK = 128, MINB = 1; };
 template <class R> struct Tune<SysNsf3D, R> { static constexpr int BLOCK = 128, MINB = 3; };
 template <> struct Tune<SysNsf3D, double> { static constexpr int BLOCK = 128, MINB = 1; };
 template <class R> struct Tune<SysMhd3D, R> { static constexpr int BLOCK = 128, MINB = 2; };
