@@ -15,9 +15,9 @@ template <> __host__ inline KParams<float>& kp<float>(GridCore& g) { return g.Pf
 
 // launch shape of the node kernel per system: threads per block, min blocks per SM (register cap)
 template <template <class> class S, class R> struct Tune { static constexpr int BLOCK = 128, MINB = 1; };
-template <class R> struct Tune<SysNsf3D, R> { static constexpr int BLOCK = 128, MINB = 3; };
+template <class R> struct Tune<SysNsf3D, R> { static constexpr int BLOCK = 64, MINB = 6; };
 template <> struct Tune<SysNsf3D, double> { static constexpr int BLOCK = 128, MINB = 1; };
-template <class R> struct Tune<SysMhd3D, R> { static constexpr int BLOCK = 128, MINB = 2; };
+template <class R> struct Tune<SysMhd3D, R> { static constexpr int BLOCK = 64, MINB = 4; };
 
 // two-pass kernel: register cap via min blocks per SM
 template <template <class> class S, class R> struct Tune2 { static constexpr int BLOCK = 256, MINB = 2; };
