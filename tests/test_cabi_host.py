@@ -75,6 +75,12 @@ def test_argument_validation():
         P.lbmk_system_set_mms(s.h, 1, [0.1])                                    # wrong mms parameter count
     with pytest.raises(P.LbmkError):
         P.lbmk_grid_create(s.h, 8, 8, 0, 0, 0.1, 5.0, P.LBMK_F64, 0)
+    with pytest.raises(P.LbmkError) as e:
+        P.lbmk_grid_create(s.h, 2048, 1024, 1024, 0, 0.1, 5.0, P.LBMK_F32_SHIFTED, 0)   # 2^31 nodes: above the maximum
+    assert e.value.status == 1
+    g = P.lbmk_grid_create(s.h, 2047, 1024, 1024, 0, 0.1, 5.0, P.LBMK_F32_SHIFTED, 0)    # largest accepted size class
+    assert P.lbmk_grid_workspace_bytes(g) > 2 * 17 * 7 * 2047 * 1024 * 1024 * 4          # > 2 TB: size_t arithmetic, no overflow
+    P.lbmk_grid_destroy(g)
     e2 = P.System("euler2d", params=[1.4], tau_R=1.0)
     with pytest.raises(P.LbmkError):
         P.lbmk_grid_create(e2.h, 8, 8, 2, 0, 0.1, 5.0, P.LBMK_F64, 0)           # nz != 1 in 2D

@@ -116,3 +116,17 @@ def test_staged_row_coefficients_parity(P, mk, kw, steps, tol, pattern):
     U1 = g.read_U()
     g.close()
     assert np.array_equal(U1, U)
+
+
+# ------------------------------------------------------------------------ degenerate grids
+@pytest.mark.parametrize("name,kw", [("c3", dict(n=1, ny=1, precision="f64")), ("c3", dict(n=1, ny=9, precision="f64")),
+                                     ("c3", dict(n=7, ny=1)), ("c5", dict(n=1, ny=1, nz=1, precision="f64")),
+                                     ("c5", dict(n=1, ny=3, nz=2)), ("c4", dict(n=2, ny=1, nz=1, precision="f64")),
+                                     ("c1", dict(n=1, ny=2))])
+@pytest.mark.parametrize("pattern", ["pull2", "aa"])
+def test_degenerate_grids_parity(P, name, kw, pattern):
+    """One-node axes: every neighbour along such an axis is the node itself (periodic wrap onto itself)."""
+    w = W.BASELINE_CONFIGS[name](**kw)
+    U, Uo, fo, _, _ = _pair(P, w, 7, pattern=pattern)
+    tol = TOL64 if w.precision == "f64" else TOL32
+    assert np.isfinite(U).all() and rel_err(U, Uo, fo).max() <= tol
