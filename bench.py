@@ -253,6 +253,7 @@ TABLE3 = [  # (label, workload maker name, paper S (MLUPS, %), paper D (MLUPS, %
     ("adr", "pin_adr", (5405, 95.4), (1673, 59.0)),
     ("allen-cahn", "pin_allencahn", (5487, 96.8), (1918, 67.7)),
     ("incompressible-nse", "pin_inse", (2328, 95.8), (662, 54.6)),
+    ("elasticity", "pin_elasticity", (2536, 89.5), (641, 45.2)),
 ]
 
 

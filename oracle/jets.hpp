@@ -41,6 +41,7 @@ inline J1 operator*(const J1& a, double c) { return a * J1(c); }
 inline J1 operator*(double c, const J1& a) { return J1(c) * a; }
 inline J1 operator/(const J1& a, double c) { return a / J1(c); }
 inline J1 operator/(double c, const J1& a) { return J1(c) / a; }
+inline J1 log(const J1& a) { J1 r; r.v = std::log(a.v); for (int i = 0; i < NV; ++i) r.d[i] = a.d[i] / a.v; return r; }
 inline J1 sqrt(const J1& a) { J1 r; r.v = std::sqrt(a.v); for (int i = 0; i < NV; ++i) r.d[i] = a.d[i] / (2.0 * r.v); return r; }
 
 struct J2 {

@@ -12,6 +12,7 @@
 //   urf2d     mms 1 : eq (SM5.4)
 //   allencahn2d mms 1 : eq (SM5.8); Table SM9 L1316 (gamma = 0.01, r = 1)
 //   inse2d    mms 1 : eq (SM5.9), PAPER.md:L1330-L1334 (Taylor-Green vortex), mms_par = {U, rho0}
+//   elasticity2d mms 1 : eq (SM5.6)
 //   maxwell2d mms 1 : eq (SM5.5), PAPER.md:L1248-L1254 (k_x = 2 pi, k_y = 4 pi, A = 1/2, omega = 4)
 #pragma once
 #include "jets.hpp"
@@ -104,6 +105,16 @@ inline bool exact_state(int sys, int mms_id, const Scaling& sc, const double* mp
         Q[0] = lower(rho); Q[1] = lower(mx); Q[2] = lower(my);
         Q[3] = sc.dx * diff(mx, 1); Q[4] = sc.dx * diff(mx, 2);
         Q[5] = sc.dx * diff(my, 1); Q[6] = sc.dx * diff(my, 2);
+        return true;
+    }
+    case SYS_ELASTICITY2D: {
+        // eq (SM5.6): displacement potential w, F = I + grad w, v = d_t w; A = 0.06
+        const double A = 0.06, rho0 = sc.par[0];
+        J2 w0 = A * (sin(k * x) * sin(k * y) * cos(t) + 0.5 * sin(k * x) * cos(k * y) * sin(t) + 0.25 * cos(k * (x + y)) * cos(t));
+        J2 w1 = A * (cos(k * x) * cos(k * y) * sin(t) + 0.5 * cos(k * x) * sin(k * y) * cos(t) + 0.25 * sin(k * (x - y)) * sin(t));
+        Q[0] = 1.0 + diff(w0, 1); Q[1] = diff(w0, 2);
+        Q[2] = diff(w1, 1);       Q[3] = 1.0 + diff(w1, 2);
+        Q[4] = rho0 * diff(w0, 0); Q[5] = rho0 * diff(w1, 0);
         return true;
     }
     case SYS_MAXWELL2D: {

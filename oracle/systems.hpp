@@ -17,7 +17,7 @@
 namespace orc {
 
 enum SystemId { SYS_ADVECTION2D = 0, SYS_BURGERS2D = 1, SYS_SWE2D = 2, SYS_EULER2D = 3, SYS_ADR2D = 4,
-                SYS_NSF3D = 5, SYS_MHD3D = 6, SYS_URF2D = 7, SYS_MAXWELL2D = 8, SYS_ALLENCAHN2D = 9, SYS_INSE2D = 10, SYS_COUNT = 11 };
+                SYS_NSF3D = 5, SYS_MHD3D = 6, SYS_URF2D = 7, SYS_MAXWELL2D = 8, SYS_ALLENCAHN2D = 9, SYS_INSE2D = 10, SYS_ELASTICITY2D = 11, SYS_COUNT = 12 };
 
 constexpr int MAXM = 32;  // max components
 
@@ -35,6 +35,7 @@ inline SysInfo sys_info(int sys) {
         case SYS_MAXWELL2D:   return {3, 3, 2};
         case SYS_ALLENCAHN2D: return {1, 3, 2};
         case SYS_INSE2D:      return {3, 7, 2};
+        case SYS_ELASTICITY2D: return {6, 6, 2};
     }
     return {0, 0, 0};
 }
@@ -222,6 +223,26 @@ void flux_source(int sys, const T* U, const Scaling& sc, T* F, T* S) {
         }
         for (int q = 0; q < 4; ++q) S[3 + q] = -G[q] / sc.g_tau;
     } break;
+    case SYS_ELASTICITY2D: {
+        // nonlinear finite-strain elasticity, total-Lagrangian, eq (3.13)-(3.15), PAPER.md:L402-L414:
+        // Q = (F_00, F_01, F_10, F_11, rho0 v_0, rho0 v_1);  d_t F_ij - d_j v_i = 0;  d_t (rho0 v_i) - d_k P_ik = 0;
+        // compressible neo-Hookean P = mu_s (F - F^-T) + lambda_s ln(J) F^-T, J = det F; par = {rho0, mu_s, lambda_s}
+        using std::log;
+        const double rho0 = sc.par[0], mus = sc.par[1], las = sc.par[2];
+        T F00 = U[0], F01 = U[1], F10 = U[2], F11 = U[3];
+        T v0 = U[4] / rho0, v1 = U[5] / rho0;
+        T J = F00 * F11 - F01 * F10;
+        T iT00 = F11 / J, iT01 = -(F10 / J), iT10 = -(F01 / J), iT11 = F00 / J;     // F^-T
+        T lJ = las * log(J);
+        T P00 = mus * (F00 - iT00) + lJ * iT00, P01 = mus * (F01 - iT01) + lJ * iT01;
+        T P10 = mus * (F10 - iT10) + lJ * iT10, P11 = mus * (F11 - iT11) + lJ * iT11;
+        F[0 * 3 + 0] = -(il * v0);  F[0 * 3 + 1] = T(0.0);        // F_00: d_0 v_0
+        F[1 * 3 + 0] = T(0.0);      F[1 * 3 + 1] = -(il * v0);    // F_01: d_1 v_0
+        F[2 * 3 + 0] = -(il * v1);  F[2 * 3 + 1] = T(0.0);        // F_10: d_0 v_1
+        F[3 * 3 + 0] = T(0.0);      F[3 * 3 + 1] = -(il * v1);    // F_11: d_1 v_1
+        F[4 * 3 + 0] = -(il * P00); F[4 * 3 + 1] = -(il * P01);
+        F[5 * 3 + 0] = -(il * P10); F[5 * 3 + 1] = -(il * P11);
+    } break;
     case SYS_MAXWELL2D: {
         // Maxwell TM mode in vacuum, eq (3.10)-(3.11): Q = (E_z, H_x, H_y); par = {c}
         const double c = sc.par[0];
@@ -299,6 +320,11 @@ inline void wave_speeds(int sys, const double* U, const Scaling& sc, double* out
     case SYS_INSE2D: {
         double u[2] = {U[1] / U[0], U[2] / U[0]}, c[2] = {sc.par[0], sc.par[0]}; set(u, c, 2);
         out[2] = std::sqrt(2.0 * sc.par[1] * dL / U[0] / sc.g_tau);
+    } break;
+    case SYS_ELASTICITY2D: {
+        // linearised about the rest configuration: longitudinal speed sqrt((lambda_s + 2 mu_s)/rho0) (the fastest wave)
+        const double cp = std::sqrt((sc.par[2] + 2.0 * sc.par[1]) / sc.par[0]);
+        out[0] = cp; out[1] = cp;
     } break;
     case SYS_MAXWELL2D: { out[0] = std::fabs(sc.par[0]); out[1] = std::fabs(sc.par[0]); } break;  // eigenvalues {+c, -c, 0}, L393
     }

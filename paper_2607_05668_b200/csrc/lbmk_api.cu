@@ -61,11 +61,12 @@ static const SysOps* ops_of(int id) {
         case LBMK_SYS_MAXWELL2D: return ops_maxwell2d();
         case LBMK_SYS_ALLENCAHN2D: return ops_allencahn2d();
         case LBMK_SYS_INSE2D: return ops_inse2d();
+        case LBMK_SYS_ELASTICITY2D: return ops_elasticity2d();
     }
     return nullptr;
 }
-static const int N_PARAMS[LBMK_SYS_COUNT] = {2, 0, 1, 1, 4, 3, 2, 0, 1, 2, 2};
-static const int N_MMS_PARAMS[LBMK_SYS_COUNT] = {0, 1, 3, 0, 0, 4, 0, 0, 0, 0, 2};
+static const int N_PARAMS[LBMK_SYS_COUNT] = {2, 0, 1, 1, 4, 3, 2, 0, 1, 2, 2, 3};
+static const int N_MMS_PARAMS[LBMK_SYS_COUNT] = {0, 1, 3, 0, 0, 4, 0, 0, 0, 0, 2, 0};
 
 static lbmk_status sys_fail(lbmk_status s, const char* msg) { g_sys_err = msg; return s; }
 static lbmk_status fail(lbmk_grid* g, lbmk_status s, const std::string& msg) { if (g) g->err = msg; else g_sys_err = msg; return s; }
@@ -155,6 +156,12 @@ lbmk_status lbmk_system_set_reference(lbmk_system* sys, const double* U0, int n)
         for (int k = 0; k < n; ++k)
             if (k != 0 && k != 4 && U0[k] != 0.0)
                 return sys_fail(LBMK_EUNSUPPORTED, "NSF3D/MHD3D delta forms need zero reference momentum, field and trackers");
+    }
+    if (sys->id == LBMK_SYS_ELASTICITY2D) {
+        const double rest[6] = {1, 0, 0, 1, 0, 0};
+        bool zero = true, is_rest = true;
+        for (int k = 0; k < 6; ++k) { zero = zero && U0[k] == 0.0; is_rest = is_rest && U0[k] == rest[k]; }
+        if (!zero && !is_rest) return sys_fail(LBMK_EUNSUPPORTED, "ELASTICITY2D reference state must be the rest configuration F = I, v = 0");
     }
     if (sys->id == LBMK_SYS_INSE2D) {
         for (int k = 1; k < n; ++k)

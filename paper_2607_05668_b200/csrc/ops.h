@@ -67,5 +67,6 @@ const SysOps* ops_urf2d();
 const SysOps* ops_maxwell2d();
 const SysOps* ops_allencahn2d();
 const SysOps* ops_inse2d();
+const SysOps* ops_elasticity2d();
 
 }  // namespace lbmk

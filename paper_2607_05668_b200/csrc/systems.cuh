@@ -24,7 +24,7 @@
 namespace lbmk {
 
 enum { SYS_ADVECTION2D = 0, SYS_BURGERS2D = 1, SYS_SWE2D = 2, SYS_EULER2D = 3, SYS_ADR2D = 4, SYS_NSF3D = 5, SYS_MHD3D = 6,
-       SYS_URF2D = 7, SYS_MAXWELL2D = 8, SYS_ALLENCAHN2D = 9, SYS_INSE2D = 10 };
+       SYS_URF2D = 7, SYS_MAXWELL2D = 8, SYS_ALLENCAHN2D = 9, SYS_INSE2D = 10, SYS_ELASTICITY2D = 11 };
 
 // ------------------------------------------------------------------------------------------ advection
 // Phi = (a_x U, a_y U); par = {a_x, a_y}
@@ -228,6 +228,46 @@ template <class R> struct SysInse2D {
         const double u = Q[1] / Q[0], v = Q[2] / Q[0], cc = P.par[0];
         out[0] = fmax(fabs(u), fabs(v)) + cc; out[1] = sqrt(u * u + v * v) + cc;
         out[2] = sqrt(2.0 * P.par[1] * P.dL / Q[0] * P.inv_gtau);
+    }
+};
+
+// ------------------------------------------------------------------------------------------ finite-strain elasticity
+// eq (3.13)-(3.15); SM4.6 L865-L897: Q = (F_00, F_01, F_10, F_11, rho0 v_0, rho0 v_1);
+// d_t F_ij - d_j v_i = 0, d_t (rho0 v_i) - d_k P_ik = 0, P = mu_s (F - F^-T) + lambda_s ln(J) F^-T; par = {rho0, mu_s, lambda_s}.
+// Reference: the rest configuration F = I, v = 0 (P(I) = 0) or none.  With d = F - I:
+//   dJ = d00 + d11 + d00 d11 - d01 d10,  F^-T = [[1+d11, -d10], [-d01, 1+d00]]/J,  I - F^-T = [[dJ-d11, d10], [d01, dJ-d00]]/J,
+//   P = mu_s (d + (I - F^-T)) + lambda_s log1p(dJ) F^-T   -- every term O(d).
+template <class R> struct SysElasticity2D {
+    static constexpr int ID = SYS_ELASTICITY2D, D = 2, M = 6, MC = 6;
+    using Mms = Mms_elasticity2d;
+    struct Ctx { R P[2][2], vl[2]; };
+    __device__ __forceinline__ static void setup(Ctx& c, const R (&dQ)[M], const KParams<R>& P) {
+        const R d00 = (P.ref[0] - R(1)) + dQ[0], d01 = P.ref[1] + dQ[1], d10 = P.ref[2] + dQ[2], d11 = (P.ref[3] - R(1)) + dQ[3];
+        const R dJ = d00 + d11 + d00 * d11 - d01 * d10;
+        const R iJ = R(1) / (R(1) + dJ);
+        const R lJ = P.par[2] * log1p(dJ), mu = P.par[1];
+        const R T00 = (R(1) + d11) * iJ, T01 = -d10 * iJ, T10 = -d01 * iJ, T11 = (R(1) + d00) * iJ;    // F^-T
+        c.P[0][0] = mu * (d00 + (dJ - d11) * iJ) + lJ * T00;
+        c.P[0][1] = mu * (d01 + d10 * iJ) + lJ * T01;
+        c.P[1][0] = mu * (d10 + d01 * iJ) + lJ * T10;
+        c.P[1][1] = mu * (d11 + (dJ - d00) * iJ) + lJ * T11;
+        const R ir = P.il / P.par[0];
+        c.vl[0] = (P.ref[4] + dQ[4]) * ir; c.vl[1] = (P.ref[5] + dQ[5]) * ir;
+    }
+    template <int k> __device__ __forceinline__ static void flux(const Ctx& c, const R (&)[M], const KParams<R>& P, R (&F)[D], R& S) {
+        S = R(0);
+        if constexpr (k < 4) {
+            constexpr int i = k / 2, j = k % 2;
+            F[0] = R(0); F[1] = R(0);
+            F[j] = -c.vl[i];
+        } else {
+            constexpr int i = k - 4;
+            F[0] = -P.il * c.P[i][0]; F[1] = -P.il * c.P[i][1];
+        }
+    }
+    __device__ static void wave(const double*, const KParams<double>& P, double* out) {
+        const double cp = sqrt((P.par[2] + 2.0 * P.par[1]) / P.par[0]);      // rest-state longitudinal speed
+        out[0] = cp; out[1] = cp; out[2] = 0.0;
     }
 };
 

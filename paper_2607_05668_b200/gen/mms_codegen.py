@@ -235,7 +235,30 @@ def sys_inse2d():
     return "inse2d", 2, prim, build
 
 
-SYSTEMS = [sys_burgers2d, sys_swe2d, sys_euler2d, sys_adr2d, sys_nsf3d, sys_urf2d, sys_maxwell2d, sys_allencahn2d, sys_inse2d]
+def sys_elasticity2d():
+    rho0, mus, las = par(0), par(1), par(2)
+    k = TWO_PI
+    A = sp.Rational(3, 50)                                                                    # eq SM5.6
+    w0 = A * (sp.sin(k * x) * sp.sin(k * y) * sp.cos(t) + sp.sin(k * x) * sp.cos(k * y) * sp.sin(t) / 2 + sp.cos(k * (x + y)) * sp.cos(t) / 4)
+    w1 = A * (sp.cos(k * x) * sp.cos(k * y) * sp.sin(t) + sp.cos(k * x) * sp.sin(k * y) * sp.cos(t) / 2 + sp.sin(k * (x - y)) * sp.sin(t) / 4)
+    prim = {"F00": 1 + sp.diff(w0, x), "F01": sp.diff(w0, y), "F10": sp.diff(w1, x), "F11": 1 + sp.diff(w1, y),
+            "v0": sp.diff(w0, t), "v1": sp.diff(w1, t)}
+
+    def build(P, D):
+        F = [[P["F00"], P["F01"]], [P["F10"], P["F11"]]]
+        v = [P["v0"], P["v1"]]
+        J = F[0][0] * F[1][1] - F[0][1] * F[1][0]
+        FiT = [[F[1][1] / J, -F[1][0] / J], [-F[0][1] / J, F[0][0] / J]]
+        Pk = [[mus * (F[i][j] - FiT[i][j]) + las * sp.log(J) * FiT[i][j] for j in range(2)] for i in range(2)]   # eq 3.14
+        Q = [F[0][0], F[0][1], F[1][0], F[1][1], rho0 * v[0], rho0 * v[1]]
+        Fl = [[-il * v[0], sp.Integer(0)], [sp.Integer(0), -il * v[0]], [-il * v[1], sp.Integer(0)], [sp.Integer(0), -il * v[1]],
+              [-il * Pk[0][0], -il * Pk[0][1]], [-il * Pk[1][0], -il * Pk[1][1]]]                # eq 3.15
+        return Q, Fl, [sp.Integer(0)] * 6
+    return "elasticity2d", 2, prim, build
+
+
+SYSTEMS = [sys_burgers2d, sys_swe2d, sys_euler2d, sys_adr2d, sys_nsf3d, sys_urf2d, sys_maxwell2d, sys_allencahn2d, sys_inse2d,
+           sys_elasticity2d]
 
 
 # ------------------------------------------------------------------------------------------------ printing

@@ -90,6 +90,20 @@ def flux_inse_listing(U, cs, mu, tau_grad):
     return Phi, S
 
 
+def flux_elasticity_listing(U, rho0, mu_s, lambda_s):
+    """SM4.6, PAPER.md:L871-L895 (state (F_00, F_01, F_10, F_11, v_0, v_1), shared subexpressions chi_0..chi_8)."""
+    F00, F01, F10, F11, v0, v1 = U
+    z = np.zeros_like(F00)
+    chi0, chi1, chi2 = -v0, -v1, mu_s / rho0
+    chi3, chi4 = F00 * F11, F01 * F10
+    chi5 = 1 / (chi3 * rho0 - chi4 * rho0)
+    chi6 = np.log(chi3 - chi4)
+    chi7, chi8 = chi5 * chi6 * lambda_s, chi5 * mu_s
+    return [[chi0, z, z], [z, chi0, z], [chi1, z, z], [z, chi1, z],
+            [-F00 * chi2 + F11 * chi5 * mu_s - F11 * chi7, -F01 * chi2 + F10 * chi5 * chi6 * lambda_s - F10 * chi8, z],
+            [F01 * chi5 * chi6 * lambda_s - F01 * chi8 - F10 * chi2, F00 * chi5 * mu_s - F00 * chi7 - F11 * chi2, z]]
+
+
 def step(f, dim, omega, F_lat, S_lat):
     """One collide-and-stream step.
     f[k][i] : arrays (nz, ny, nx);  F_lat[k][a], S_lat[k] : lattice flux / source arrays at the

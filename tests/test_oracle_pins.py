@@ -13,12 +13,12 @@ import oracle
 import workloads as W
 from oracle import OracleGrid
 
-from brute_force import (LATTICES, flux_adr_listing, flux_allencahn_listing, flux_euler_listing, flux_inse_listing, flux_maxwell_listing, flux_swe_listing, flux_urf_listing,
+from brute_force import (LATTICES, flux_adr_listing, flux_allencahn_listing, flux_elasticity_listing, flux_euler_listing, flux_inse_listing, flux_maxwell_listing, flux_swe_listing, flux_urf_listing,
                          init_equilibrium, moments, step as bf_step)
 
-SYSTEMS = ["advection2d", "burgers2d", "swe2d", "euler2d", "adr2d", "nsf3d", "mhd3d", "urf2d", "maxwell2d", "allencahn2d", "inse2d"]
+SYSTEMS = ["advection2d", "burgers2d", "swe2d", "euler2d", "adr2d", "nsf3d", "mhd3d", "urf2d", "maxwell2d", "allencahn2d", "inse2d", "elasticity2d"]
 PARAMS = {"advection2d": [0.1, 0.05], "burgers2d": [], "swe2d": [1.0], "euler2d": [1.4],
-          "adr2d": [0.1, -0.1, 0.01, 1.0], "nsf3d": [1.4, 1e-3, 4.9e-3], "mhd3d": [1.4, 1e-3], "urf2d": [], "maxwell2d": [1.0], "allencahn2d": [0.01, 1.0], "inse2d": [1.0, 0.01]}
+          "adr2d": [0.1, -0.1, 0.01, 1.0], "nsf3d": [1.4, 1e-3, 4.9e-3], "mhd3d": [1.4, 1e-3], "urf2d": [], "maxwell2d": [1.0], "allencahn2d": [0.01, 1.0], "inse2d": [1.0, 0.01], "elasticity2d": [1.3, 1.0, 2.0]}
 
 
 def small_grid(system, **kw):
@@ -41,6 +41,9 @@ def physical_state(system, rng, shape=()):
         U[4] = rng.uniform(2.0, 3.0, size=shape)
     if system in ("advection2d", "burgers2d", "adr2d", "allencahn2d"):
         U[0] = rng.uniform(0.2, 0.9, size=shape)
+    if system == "elasticity2d":                # det F > 0: F near the identity
+        U[0] = U[0] + 1.0
+        U[3] = U[3] + 1.0
     if system == "urf2d":                       # physicality E > |S|
         U[0] = rng.uniform(1.0, 2.0, size=shape)
     return U
@@ -271,6 +274,7 @@ MMS_CASES = {
     "maxwell2d": lambda: W.pin_maxwell(32),
     "allencahn2d": lambda: W.pin_allencahn(32),
     "inse2d": lambda: W.pin_inse(32),
+    "elasticity2d": lambda: W.pin_elasticity(32),
 }
 
 
@@ -371,6 +375,11 @@ def _bf_run(system, w, steps, listing_flux):
             F = [[il * Phi[0][a] for a in range(3)]] + [[il * w.dx * Phi[k][a] for a in range(3)] for k in (1, 2)]
             S = [dt * (-R * Uc[0] ** 2 + R * Uc[0]), dt * (-Uc[1] / tau_grad), dt * (-Uc[2] / tau_grad)]
             return F, S
+        if system == "elasticity2d":
+            rho0, mus, las = w.params
+            Phi = flux_elasticity_listing(list(Uc[:4]) + [Uc[4] / rho0, Uc[5] / rho0], rho0, mus, las)
+            F = [[il * Phi[k][a] for a in range(3)] for k in range(4)] + [[il * rho0 * Phi[k][a] for a in range(3)] for k in (4, 5)]
+            return F, [0.0 * Uc[0] for _ in Uc]
         if system == "inse2d":
             cs, mu = w.params
             tau_grad = w.g_tau * dt
@@ -430,6 +439,17 @@ def test_p13_brute_force_inse_trackers():
     w.steps = 12
     exp = _bf_run("inse2d", w, w.steps, None)
     assert np.abs(oracle.run(w) - exp).max() < 1e-13
+
+
+def test_p13_brute_force_elasticity():
+    w = W.pin_elasticity(8)
+    w.params = [1.3, 1.0, 2.0]                       # rho0 != 1: the listing carries v, the state rho0 v
+    w.mms_id = 0
+    w.steps = 12
+    U0 = w.initial_U(); U0[4:] *= 1.3
+    w.init = lambda _w: U0
+    exp = _bf_run("elasticity2d", w, w.steps, None)
+    assert np.abs(oracle.run(w) - exp).max() < 1e-14
 
 
 def test_p13_brute_force_ultrarelativistic():

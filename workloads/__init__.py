@@ -41,12 +41,13 @@ COMPONENTS: Dict[str, List[str]] = {
     "maxwell2d": ["Ez", "Hx", "Hy"],
     "allencahn2d": ["phi", "Gx", "Gy"],
     "inse2d": ["rho", "mx", "my", "Gxx", "Gxy", "Gyx", "Gyy"],
+    "elasticity2d": ["F00", "F01", "F10", "F11", "m0", "m1"],
 }
 N_CONSERVED = {"advection2d": 1, "burgers2d": 1, "swe2d": 3, "euler2d": 4,
-               "adr2d": 1, "nsf3d": 5, "mhd3d": 8, "urf2d": 3, "maxwell2d": 3, "allencahn2d": 1, "inse2d": 3}
+               "adr2d": 1, "nsf3d": 5, "mhd3d": 8, "urf2d": 3, "maxwell2d": 3, "allencahn2d": 1, "inse2d": 3, "elasticity2d": 6}
 LATTICE_OF = {"advection2d": "D2Q5", "burgers2d": "D2Q5", "swe2d": "D2Q5",
               "euler2d": "D2Q5", "adr2d": "D2Q5", "nsf3d": "D3Q7", "mhd3d": "D3Q7",
-              "urf2d": "D2Q5", "maxwell2d": "D2Q5", "allencahn2d": "D2Q5", "inse2d": "D2Q5"}
+              "urf2d": "D2Q5", "maxwell2d": "D2Q5", "allencahn2d": "D2Q5", "inse2d": "D2Q5", "elasticity2d": "D2Q5"}
 # c_s^2 per lattice, Table SM1; used only by the lambda rule below.
 CS2 = {"D2Q5": 1.0 / 3.0, "D3Q7": 1.0 / 4.0}
 SIGMA = 0.6  # lambda rule: lattice wave speed = SIGMA * c_s^2 (SURVEY.md §8(c) "lambda rule")
@@ -444,6 +445,37 @@ def pin_inse(n: int = 512, precision: str = "f64") -> Workload:
                     dx=dx, lam=dx / dt, params=[1.0, 0.01], tau_R=50.0 if precision == "f64" else 90.0, g_tau=6.0,
                     U_ref=[1.0] + [0.0] * 6, mms_id=1, mms_params=[0.1, 1.0], steps=int(round(1.0 / dt)), s_max=1.1,
                     seed=0, init=_init_inse, note="PAPER.md Table 2 L543-L546")
+
+
+def _init_elasticity(w: Workload) -> np.ndarray:
+    # eq (SM5.6), PAPER.md:L1271-L1272 at t = 0: F = I + grad w, rho0 v = rho0 d_t w
+    rho0 = w.params[0]
+    A = 0.06
+    x, y, _ = _grid(w)
+    k = TWO_PI
+    sx, cx, sy, cy = np.sin(k * x), np.cos(k * x), np.sin(k * y), np.cos(k * y)
+    spp, cmm = np.sin(k * (x + y)), np.cos(k * (x - y))
+    # w0 = A (sx sy cos t + sx cy sin t / 2 + cos(k(x+y)) cos t / 4);  w1 = A (cx cy sin t + cx sy cos t / 2 + sin(k(x-y)) sin t / 4)
+    F00 = 1.0 + A * k * (cx * sy - 0.25 * spp)
+    F01 = A * k * (sx * cy - 0.25 * spp)
+    F10 = A * k * (-0.5 * sx * sy)
+    F11 = 1.0 + A * k * (0.5 * cx * cy)
+    v0 = A * 0.5 * sx * cy
+    v1 = A * (cx * cy + 0.25 * np.sin(k * (x - y))) + 0.0 * cmm
+    return np.stack([_full(w, c) for c in (F00, F01, F10, F11, rho0 * v0, rho0 * v1)]).copy()
+
+
+def pin_elasticity(n: int = 512, precision: str = "f64", scale: str = "p") -> Workload:
+    # Table SM2: acoustic f = 0.1, tau_R = 0.2 (Float: f = 0.15, tau_R = 2); Table SM7 L1280 (aluminium-like:
+    # rho0 = 2700, mu_s = 2.6e10, lambda_s = 5.2e10) non-dimensionalised by rho0 and a velocity scale (reading A23):
+    # "shear": c = sqrt(mu_s/rho0) -> mu_s = 1, lambda_s = 2;  "p": c = sqrt((lambda_s + 2 mu_s)/rho0) -> 0.25, 0.5
+    f, tau_R = (0.1, 0.2) if precision in ("f64", "f64s") else (0.15, 2.0)
+    mus, las = (1.0, 2.0) if scale == "shear" else (0.25, 0.5)
+    cp = math.sqrt(las + 2.0 * mus)
+    return Workload(name=f"pin_elasticity2d_{n}", system="elasticity2d", nx=n, ny=n, nz=1, precision=precision,
+                    dx=1.0 / n, lam=1.0 / f, params=[1.0, mus, las], tau_R=tau_R, g_tau=0.0,
+                    U_ref=[1.0, 0.0, 0.0, 1.0, 0.0, 0.0], mms_id=1, mms_params=[], steps=int(round(n / f)), s_max=1.3 * cp,
+                    seed=0, init=_init_elasticity, note="PAPER.md Table 2 L536-L539")
 
 
 BASELINE_CONFIGS: Dict[str, Callable[..., Workload]] = {
