@@ -25,6 +25,7 @@ PAPER = {
               "cite": "PAPER.md:L519-L522 (row labels E, rho, rho u: SURVEY.md §8(c) A8)"},
     "adr": {"c": (2.2901e-04, 1.2680e-04), "cite": "PAPER.md:L540"},
     "allencahn": {"phi": (7.3196e-04, 7.8653e-04), "cite": "PAPER.md:L542"},
+    "elasticity": {"F": (3.1874e-05, 2.8940e-05), "v": (6.4804e-05, 4.5664e-05), "cite": "PAPER.md:L536-L539"},
     "urf": {"E": (4.3449e-06, 2.1354e-06), "S": (9.6256e-06, 6.3943e-06), "cite": "PAPER.md:L527-L529"},
     "maxwell": {"Ez": (2.9956e-05, 2.9956e-05), "Hx": (1.0951e-04, 1.0951e-04), "Hy": (1.1587e-05, 1.1587e-05),
                 "cite": "PAPER.md:L530-L535"},
@@ -42,7 +43,7 @@ def rel_errors(U, Ue):
 
 def run_case(case, n):
     w = {"burgers": W.pin_burgers, "euler": W.pin_euler, "adr": W.pin_adr, "urf": W.pin_urf, "maxwell": W.pin_maxwell,
-         "allencahn": W.pin_allencahn}[case](n)
+         "allencahn": W.pin_allencahn, "elasticity": W.pin_elasticity}[case](n)
     g = oracle.OracleGrid.from_workload(w)
     g.init_from_U(w.initial_U())
     t0 = time.time()
@@ -60,6 +61,9 @@ def run_case(case, n):
                   "rhou": (float(np.hypot(e[1][0], e[2][0])), float(np.hypot(e[1][1], e[2][1])))}
     elif case == "allencahn":
         fields = {"phi": e[0]}
+    elif case == "elasticity":
+        rss = lambda ks, j: float(np.sqrt(sum(e[k][j] ** 2 for k in ks)))
+        fields = {"F": (rss(range(4), 0), rss(range(4), 1)), "v": (rss((4, 5), 0), rss((4, 5), 1))}
     elif case == "urf":
         fields = {"E": e[0], "S": (float(np.hypot(e[1][0], e[2][0])), float(np.hypot(e[1][1], e[2][1])))}
     elif case == "maxwell":
@@ -70,7 +74,7 @@ def run_case(case, n):
 
 
 if __name__ == "__main__":
-    cases = sys.argv[1:] or ["burgers", "euler", "adr", "urf", "maxwell", "allencahn"]
+    cases = sys.argv[1:] or ["burgers", "euler", "adr", "urf", "maxwell", "allencahn", "elasticity"]
     path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "paper_pins.json")
     out = json.load(open(path)) if os.path.exists(path) else {}
     for case in cases:

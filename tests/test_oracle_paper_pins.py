@@ -23,7 +23,7 @@ import workloads as W
 HERE = os.path.dirname(os.path.abspath(__file__))
 PINS = json.load(open(os.path.join(HERE, "golden", "paper_pins.json")))
 MAKERS = {"burgers": W.pin_burgers, "euler": W.pin_euler, "adr": W.pin_adr, "urf": W.pin_urf, "maxwell": W.pin_maxwell,
-          "allencahn": W.pin_allencahn}
+          "allencahn": W.pin_allencahn, "elasticity": W.pin_elasticity}
 
 
 def _rows(case):
@@ -73,6 +73,9 @@ def test_p8_live_n64_matches_stored_row(case):
         live = {"rho": e[0], "E": e[3], "rhou": (math.hypot(e[1][0], e[2][0]), math.hypot(e[1][1], e[2][1]))}
     elif case == "allencahn":
         live = {"phi": e[0]}
+    elif case == "elasticity":
+        rss = lambda ks, j: math.sqrt(sum(e[k][j] ** 2 for k in ks))
+        live = {"F": (rss(range(4), 0), rss(range(4), 1)), "v": (rss((4, 5), 0), rss((4, 5), 1))}
     elif case == "urf":
         live = {"E": e[0], "S": (math.hypot(e[1][0], e[2][0]), math.hypot(e[1][1], e[2][1]))}
     elif case == "maxwell":
