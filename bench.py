@@ -62,7 +62,7 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="c4", choices=["c1", "c2", "c3", "c4", "c5"])
     ap.add_argument("--pattern", default="auto", choices=["auto", "pull2", "aa"])
-    ap.add_argument("--kernel", default="auto", choices=["auto", "node", "row", "twopass"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "node", "twopass"])
     ap.add_argument("--n", type=int, default=None, help="override the grid edge (debug; the line then says so)")
     ap.add_argument("--no-mms", action="store_true", help="c4 without manufactured forcing (the paper's Table 3 kernels carry none)")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -87,7 +87,8 @@ typedef enum {
 } lbmk_option;
 enum { LBMK_PATTERN_AUTO = 0, LBMK_PATTERN_PULL2 = 1 /* two-lattice pull */, LBMK_PATTERN_AA = 2 /* in-place */ };
 enum { LBMK_KERNEL_AUTO = 0, LBMK_KERNEL_NODE = 1 /* one node per thread, direct loads */,
-       LBMK_KERNEL_ROW = 2 /* bulk-copy staged x-rows in shared memory */,
+       LBMK_KERNEL_ROW = 2 /* reserved: shared-memory / TMA staged x-rows; not built (direct loads already move exactly the
+                              algorithmic bytes at the copy peak) -- selecting it returns LBMK_EUNSUPPORTED */,
        LBMK_KERNEL_TWOPASS = 3 /* one node per thread, moments first, populations re-read for the relaxation */ };
 
 typedef struct lbmk_system lbmk_system;

@@ -344,6 +344,7 @@ lbmk_status lbmk_grid_set_option(lbmk_grid* g, lbmk_option key, long long value)
         g->opt_pattern = value;
     } else if (key == LBMK_OPT_KERNEL) {
         if (value < LBMK_KERNEL_AUTO || value > LBMK_KERNEL_TWOPASS) return fail(g, LBMK_EINVAL, "unknown kernel variant");
+        if (value == LBMK_KERNEL_ROW) return fail(g, LBMK_EUNSUPPORTED, "LBMK_KERNEL_ROW is reserved: no staged-row kernel in this build");
         g->opt_kernel = value;
     } else {
         return fail(g, LBMK_EINVAL, "unknown option");

@@ -111,6 +111,9 @@ def test_grid_scaling_and_workspace_layout():
     assert e.value.status == 5
     with pytest.raises(P.LbmkError):
         P.lbmk_grid_bind_workspace(g, 0, b1)
+    with pytest.raises(P.LbmkError) as e:                      # reserved kernel variant: refused, never silently replaced
+        P.lbmk_grid_set_option(g, P.LBMK_OPT_KERNEL, P.LBMK_KERNEL_ROW)
+    assert e.value.status == 6
     P.lbmk_grid_destroy(g)
 
 
