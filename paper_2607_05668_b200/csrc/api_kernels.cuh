@@ -29,7 +29,13 @@ __global__ void halo_kernel(R* __restrict__ f, R* __restrict__ buf, int M, int Q
 
 // plain streaming copy: the roofline denominator probe (cf. the paper's BabelStream peak)
 __global__ void __launch_bounds__(256) copy_kernel(float4* __restrict__ dst, const float4* __restrict__ src, size_t n16) {
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += (size_t)gridDim.x * blockDim.x) dst[i] = src[i];
+    // one 16 KB chunk per block: 4 independent 128-bit loads per thread in flight, then 4 stores
+    const size_t base = (size_t)blockIdx.x * 1024 + threadIdx.x;
+    float4 v[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) if (base + 256 * j < n16) v[j] = src[base + 256 * j];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) if (base + 256 * j < n16) dst[base + 256 * j] = v[j];
 }
 
 }  // namespace lbmk

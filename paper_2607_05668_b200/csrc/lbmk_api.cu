@@ -684,7 +684,7 @@ lbmk_status lbmk_copy_bandwidth(void* dst, const void* src, size_t bytes, int re
     if ((e = cudaEventCreate(&a)) != cudaSuccess) return cuda_fail(nullptr, e, "cudaEventCreate");
     if ((e = cudaEventCreate(&b)) != cudaSuccess) { cudaEventDestroy(a); return cuda_fail(nullptr, e, "cudaEventCreate"); }
     const size_t n16 = bytes / 16;
-    const unsigned nb = 148 * 16;
+    const unsigned nb = (unsigned)((n16 + 1023) / 1024);
     copy_kernel<<<nb, 256, 0, s>>>((float4*)dst, (const float4*)src, n16);   // warm-up
     cudaEventRecord(a, s);
     for (int r = 0; r < reps; ++r) copy_kernel<<<nb, 256, 0, s>>>((float4*)dst, (const float4*)src, n16);
