@@ -241,7 +241,7 @@ def short_run(P, torch, name, pattern):
     return out
 
 
-# The paper's Table 3 rows (PAPER.md:L577-L594) that have a compiled-in system here: bulk collide-and-stream without
+# The paper's Table 3 rows (PAPER.md:L577-L596) that have a compiled-in system here: bulk collide-and-stream without
 # manufactured forcing, single (shifted fp32) and double precision, on a saturating grid.  Paper columns: MLUPS and
 # % of its 680 GB/s BabelStream peak on an RTX A5000 (context only -- another GPU, other kernels).
 TABLE3 = [  # (label, workload maker name, paper S (MLUPS, %), paper D (MLUPS, %))
@@ -254,6 +254,7 @@ TABLE3 = [  # (label, workload maker name, paper S (MLUPS, %), paper D (MLUPS, %
     ("allen-cahn", "pin_allencahn", (5487, 96.8), (1918, 67.7)),
     ("incompressible-nse", "pin_inse", (2328, 95.8), (662, 54.6)),
     ("elasticity", "pin_elasticity", (2536, 89.5), (641, 45.2)),
+    ("compressible-nsf", "pin_nsf2d", (1335, 94.2), (256, 36.2)),
 ]
 
 

@@ -71,13 +71,14 @@ typedef enum { LBMK_PERIODIC = 0, LBMK_DIRICHLET_MMS = 1 } lbmk_bc;
  *   ALLENCAHN2D  {gamma, r}            Allen-Cahn phase field, eq 3.18-3.19 L429-L434          m = 1 + 2 trackers
  *   INSE2D       {c_s_phys, mu}        weakly compressible NSE, eq 3.21-3.22 L446-L452          m = 3 + 4 trackers
  *   ELASTICITY2D {rho0, mu_s, lambda_s} neo-Hookean finite-strain elasticity, eq 3.13-3.15 L402-L414  m = 6 (F, rho0 v)
+ *   NSF2D        {gamma, mu, K}        compressible NSF 2D, eq 3.23-3.24, cascade on the conserved fields  m = 4 + 8
  *   MAXWELL2D    {c}                   Maxwell TM mode, eq 3.10-3.11 L385-L391                 m = 3 (E_z, H_x, H_y)
  * Trackers are carried in lattice units G^L = dx grad V. */
 typedef enum {
     LBMK_SYS_ADVECTION2D = 0, LBMK_SYS_BURGERS2D = 1, LBMK_SYS_SWE2D = 2, LBMK_SYS_EULER2D = 3,
     LBMK_SYS_ADR2D = 4, LBMK_SYS_NSF3D_GRADTRACK = 5, LBMK_SYS_MHD3D_JTRACK = 6, LBMK_SYS_URF2D = 7,
     LBMK_SYS_MAXWELL2D = 8, LBMK_SYS_ALLENCAHN2D = 9, LBMK_SYS_INSE2D = 10,
-    LBMK_SYS_ELASTICITY2D = 11, LBMK_SYS_COUNT = 12
+    LBMK_SYS_ELASTICITY2D = 11, LBMK_SYS_NSF2D_GRADTRACK = 12, LBMK_SYS_COUNT = 13
 } lbmk_system_id;
 
 /* Grid options (lbmk_grid_set_option, before lbmk_grid_workspace_bytes / bind). */
@@ -116,7 +117,8 @@ lbmk_status lbmk_system_set_reference(lbmk_system* sys, const double* U0, int n)
  * t_n + dt/2.  mms_id 0 = none, 1 = the system's manufactured fields.
  *   BURGERS2D {A};  EULER2D {};  SWE2D {A_h, A_u, h0};  ADR2D {};  NSF3D {U0, A_rho, rho0, p0};
  *   URF2D {} (eq SM5.4);  MAXWELL2D {} (eq SM5.5);  ALLENCAHN2D {} (eq SM5.8);
- *   INSE2D {U, rho0} (eq SM5.9);  ELASTICITY2D {} (eq SM5.6). */
+ *   INSE2D {U, rho0} (eq SM5.9);  ELASTICITY2D {} (eq SM5.6);
+ *   NSF2D {} (eq SM5.10). */
 lbmk_status lbmk_system_set_mms(lbmk_system* sys, int mms_id, const double* mms_params, int n);
 /* A-priori bound on the physical wave speed max|eig sum n_a A_a| from the declared amplitudes (eq 2.20).
  * lbmk_grid_create rejects the grid with LBMK_ESUBCHAR if s_max/lambda > c_s.  0 = no declared bound. */

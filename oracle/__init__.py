@@ -16,7 +16,7 @@ import numpy as np
 from . import build as _build
 
 MAXM = 32
-SYSTEM_ID = {"advection2d": 0, "burgers2d": 1, "swe2d": 2, "euler2d": 3, "adr2d": 4, "nsf3d": 5, "mhd3d": 6, "urf2d": 7, "maxwell2d": 8, "allencahn2d": 9, "inse2d": 10, "elasticity2d": 11}
+SYSTEM_ID = {"advection2d": 0, "burgers2d": 1, "swe2d": 2, "euler2d": 3, "adr2d": 4, "nsf3d": 5, "mhd3d": 6, "urf2d": 7, "maxwell2d": 8, "allencahn2d": 9, "inse2d": 10, "elasticity2d": 11, "nsf2d": 12}
 
 
 class _Spec(C.Structure):

@@ -13,6 +13,7 @@
 //   allencahn2d mms 1 : eq (SM5.8); Table SM9 L1316 (gamma = 0.01, r = 1)
 //   inse2d    mms 1 : eq (SM5.9), PAPER.md:L1330-L1334 (Taylor-Green vortex), mms_par = {U, rho0}
 //   elasticity2d mms 1 : eq (SM5.6)
+//   nsf2d     mms 1 : eq (SM5.10)
 //   maxwell2d mms 1 : eq (SM5.5), PAPER.md:L1248-L1254 (k_x = 2 pi, k_y = 4 pi, A = 1/2, omega = 4)
 #pragma once
 #include "jets.hpp"
@@ -115,6 +116,22 @@ inline bool exact_state(int sys, int mms_id, const Scaling& sc, const double* mp
         Q[0] = 1.0 + diff(w0, 1); Q[1] = diff(w0, 2);
         Q[2] = diff(w1, 1);       Q[3] = 1.0 + diff(w1, 2);
         Q[4] = rho0 * diff(w0, 0); Q[5] = rho0 * diff(w1, 0);
+        return true;
+    }
+    case SYS_NSF2D: {
+        // eq (SM5.10), non-dimensional rho0 = c_s = 1 (reading A9): u0 = 3, v0 = 2, p0 = 1/gamma
+        const double gamma = sc.par[0], p0 = 1.0 / gamma;
+        J2 drho = 0.2 * sin(k * x) * cos(k * y) * cos(t);
+        J2 rho = 1.0 + drho;
+        J2 u = 3.0 + 0.2 * cos(k * x) * sin(k * y) * sin(t);
+        J2 v = 2.0 + 0.15 * sin(k * x) * sin(k * y) * cos(t);
+        J2 p = p0 + drho + (0.2 * p0) * cos(k * x) * sin(k * y) * sin(t);
+        J2 V[4] = {rho, rho * u, rho * v, p / (gamma - 1.0) + 0.5 * rho * (u * u + v * v)};
+        for (int q = 0; q < 4; ++q) {
+            Q[q] = lower(V[q]);
+            Q[4 + 2 * q + 0] = sc.dx * diff(V[q], 1);
+            Q[4 + 2 * q + 1] = sc.dx * diff(V[q], 2);
+        }
         return true;
     }
     case SYS_MAXWELL2D: {

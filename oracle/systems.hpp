@@ -17,7 +17,7 @@
 namespace orc {
 
 enum SystemId { SYS_ADVECTION2D = 0, SYS_BURGERS2D = 1, SYS_SWE2D = 2, SYS_EULER2D = 3, SYS_ADR2D = 4,
-                SYS_NSF3D = 5, SYS_MHD3D = 6, SYS_URF2D = 7, SYS_MAXWELL2D = 8, SYS_ALLENCAHN2D = 9, SYS_INSE2D = 10, SYS_ELASTICITY2D = 11, SYS_COUNT = 12 };
+                SYS_NSF3D = 5, SYS_MHD3D = 6, SYS_URF2D = 7, SYS_MAXWELL2D = 8, SYS_ALLENCAHN2D = 9, SYS_INSE2D = 10, SYS_ELASTICITY2D = 11, SYS_NSF2D = 12, SYS_COUNT = 13 };
 
 constexpr int MAXM = 32;  // max components
 
@@ -36,6 +36,7 @@ inline SysInfo sys_info(int sys) {
         case SYS_ALLENCAHN2D: return {1, 3, 2};
         case SYS_INSE2D:      return {3, 7, 2};
         case SYS_ELASTICITY2D: return {6, 6, 2};
+        case SYS_NSF2D:       return {4, 12, 2};
     }
     return {0, 0, 0};
 }
@@ -243,6 +244,49 @@ void flux_source(int sys, const T* U, const Scaling& sc, T* F, T* S) {
         F[4 * 3 + 0] = -(il * P00); F[4 * 3 + 1] = -(il * P01);
         F[5 * 3 + 0] = -(il * P10); F[5 * 3 + 1] = -(il * P11);
     } break;
+    case SYS_NSF2D: {
+        // compressible Navier-Stokes-Fourier, 2D, eq (3.23)-(3.24), PAPER.md:L456-L467 and Listing 2 (L750-L791), with the
+        // gradient cascade on the CONSERVED fields (N = 4 + 8, SM4.10 L961): U = (rho, m0, m1, E, G^L_{V,b} = dx d_b V
+        // [index 4 + 2 v + b, V = rho, m0, m1, E]).  Derived gradients by the chain rule (cgrad, L219):
+        //   d_b u_a = (G_{m_a,b} - u_a G_{rho,b})/rho,  d_b p = (gamma-1)(G_{E,b} - sum_a u_a G_{m_a,b} + |u|^2/2 G_{rho,b}),
+        //   d_b T = (d_b p - T G_{rho,b})/rho,  T = p/rho (R eliminated, L768);  par = {gamma, mu, K}
+        //   tau_ab = mu (d_b u_a + d_a u_b - 2/3 delta_ab div u),  q = -K grad T
+        const double gamma = sc.par[0], muL = sc.par[1] * dL, KL = sc.par[2] * dL;
+        T rho = U[0], E = U[3];
+        T m[2] = {U[1], U[2]};
+        T u[2] = {m[0] / rho, m[1] / rho};
+        T u2 = u[0] * u[0] + u[1] * u[1];
+        T p = (gamma - 1.0) * (E - 0.5 * rho * u2);
+        T Tm = p / rho;
+        const T* G = U + 4;   // G[2 v + b]
+        T du[2][2], dT[2];
+        for (int b = 0; b < 2; ++b) {
+            for (int a = 0; a < 2; ++a) du[a][b] = (G[2 * (1 + a) + b] - u[a] * G[b]) / rho;
+            T dp = (gamma - 1.0) * (G[6 + b] - u[0] * G[2 + b] - u[1] * G[4 + b] + 0.5 * u2 * G[b]);
+            dT[b] = (dp - Tm * G[b]) / rho;
+        }
+        T divu = du[0][0] + du[1][1];
+        T tau[2][2];
+        for (int a = 0; a < 2; ++a)
+            for (int b = 0; b < 2; ++b) {
+                tau[a][b] = muL * (du[a][b] + du[b][a]);
+                if (a == b) tau[a][b] = tau[a][b] - (2.0 / 3.0) * muL * divu;
+            }
+        for (int j = 0; j < 2; ++j) {
+            F[0 * 3 + j] = il * m[j];
+            for (int a = 0; a < 2; ++a) {
+                F[(1 + a) * 3 + j] = il * (m[a] * u[j]) - tau[a][j];
+                if (a == j) F[(1 + a) * 3 + j] = F[(1 + a) * 3 + j] + il * p;
+            }
+            F[3 * 3 + j] = il * ((E + p) * u[j]) - (tau[j][0] * u[0] + tau[j][1] * u[1]) - KL * dT[j];
+            for (int v = 0; v < 4; ++v)
+                for (int b = 0; b < 2; ++b) {
+                    F[(4 + 2 * v + b) * 3 + j] = il * (G[2 * v + b] * u[j]);
+                    if (j == b) F[(4 + 2 * v + b) * 3 + j] = F[(4 + 2 * v + b) * 3 + j] - U[v] / sc.g_tau;
+                }
+        }
+        for (int q = 0; q < 8; ++q) S[4 + q] = -G[q] / sc.g_tau;
+    } break;
     case SYS_MAXWELL2D: {
         // Maxwell TM mode in vacuum, eq (3.10)-(3.11): Q = (E_z, H_x, H_y); par = {c}
         const double c = sc.par[0];
@@ -325,6 +369,13 @@ inline void wave_speeds(int sys, const double* U, const Scaling& sc, double* out
         // linearised about the rest configuration: longitudinal speed sqrt((lambda_s + 2 mu_s)/rho0) (the fastest wave)
         const double cp = std::sqrt((sc.par[2] + 2.0 * sc.par[1]) / sc.par[0]);
         out[0] = cp; out[1] = cp;
+    } break;
+    case SYS_NSF2D: {
+        double u[2] = {U[1] / U[0], U[2] / U[0]};
+        double p = (sc.par[0] - 1.0) * (U[3] - 0.5 * U[0] * (u[0] * u[0] + u[1] * u[1]));
+        double cc = std::sqrt(sc.par[0] * p / U[0]); double c[2] = {cc, cc}; set(u, c, 2);
+        double kap = std::fmax(4.0 * sc.par[1] * dL / (3.0 * U[0]), sc.par[2] * dL * (sc.par[0] - 1.0) / U[0]);
+        out[2] = std::sqrt(kap / sc.g_tau);
     } break;
     case SYS_MAXWELL2D: { out[0] = std::fabs(sc.par[0]); out[1] = std::fabs(sc.par[0]); } break;  // eigenvalues {+c, -c, 0}, L393
     }

@@ -32,7 +32,7 @@ LBMK_PERIODIC, LBMK_DIRICHLET_MMS = 0, 1
 LBMK_OPT_PATTERN, LBMK_OPT_KERNEL = 0, 1
 LBMK_PATTERN_AUTO, LBMK_PATTERN_PULL2, LBMK_PATTERN_AA = 0, 1, 2
 LBMK_KERNEL_AUTO, LBMK_KERNEL_NODE, LBMK_KERNEL_ROW, LBMK_KERNEL_TWOPASS = 0, 1, 2, 3
-SYSTEM_ID = {"advection2d": 0, "burgers2d": 1, "swe2d": 2, "euler2d": 3, "adr2d": 4, "nsf3d": 5, "mhd3d": 6, "urf2d": 7, "maxwell2d": 8, "allencahn2d": 9, "inse2d": 10, "elasticity2d": 11}
+SYSTEM_ID = {"advection2d": 0, "burgers2d": 1, "swe2d": 2, "euler2d": 3, "adr2d": 4, "nsf3d": 5, "mhd3d": 6, "urf2d": 7, "maxwell2d": 8, "allencahn2d": 9, "inse2d": 10, "elasticity2d": 11, "nsf2d": 12}
 PRECISION = {"f64": LBMK_F64, "f32s": LBMK_F32_SHIFTED, "f64s": LBMK_F64_SHIFTED}
 PATTERN = {"auto": 0, "pull2": 1, "aa": 2}
 KERNEL = {"auto": 0, "node": 1, "row": 2, "twopass": 3}

@@ -62,11 +62,12 @@ static const SysOps* ops_of(int id) {
         case LBMK_SYS_ALLENCAHN2D: return ops_allencahn2d();
         case LBMK_SYS_INSE2D: return ops_inse2d();
         case LBMK_SYS_ELASTICITY2D: return ops_elasticity2d();
+        case LBMK_SYS_NSF2D_GRADTRACK: return ops_nsf2d();
     }
     return nullptr;
 }
-static const int N_PARAMS[LBMK_SYS_COUNT] = {2, 0, 1, 1, 4, 3, 2, 0, 1, 2, 2, 3};
-static const int N_MMS_PARAMS[LBMK_SYS_COUNT] = {0, 1, 3, 0, 0, 4, 0, 0, 0, 0, 2, 0};
+static const int N_PARAMS[LBMK_SYS_COUNT] = {2, 0, 1, 1, 4, 3, 2, 0, 1, 2, 2, 3, 3};
+static const int N_MMS_PARAMS[LBMK_SYS_COUNT] = {0, 1, 3, 0, 0, 4, 0, 0, 0, 0, 2, 0, 0};
 
 static lbmk_status sys_fail(lbmk_status s, const char* msg) { g_sys_err = msg; return s; }
 static lbmk_status fail(lbmk_grid* g, lbmk_status s, const std::string& msg) { if (g) g->err = msg; else g_sys_err = msg; return s; }
@@ -163,6 +164,10 @@ lbmk_status lbmk_system_set_reference(lbmk_system* sys, const double* U0, int n)
         for (int k = 0; k < 6; ++k) { zero = zero && U0[k] == 0.0; is_rest = is_rest && U0[k] == rest[k]; }
         if (!zero && !is_rest) return sys_fail(LBMK_EUNSUPPORTED, "ELASTICITY2D reference state must be the rest configuration F = I, v = 0");
     }
+    if (sys->id == LBMK_SYS_NSF2D_GRADTRACK) {
+        for (int k = 4; k < n; ++k)
+            if (U0[k] != 0.0) return sys_fail(LBMK_EUNSUPPORTED, "NSF2D needs zero reference trackers");
+    }
     if (sys->id == LBMK_SYS_INSE2D) {
         for (int k = 1; k < n; ++k)
             if (U0[k] != 0.0) return sys_fail(LBMK_EUNSUPPORTED, "INSE2D delta form needs zero reference momentum and trackers");
@@ -222,6 +227,7 @@ static void derive_params(lbmk_grid* g) {
         case LBMK_SYS_SWE2D:
             for (int a = 0; a < 2; ++a) P.cst[a] = r[0] != 0.0 ? r[1 + a] / r[0] : 0.0;
             break;
+        case LBMK_SYS_NSF2D_GRADTRACK:
         case LBMK_SYS_EULER2D: {
             double ke = 0.0;
             for (int a = 0; a < 2; ++a) { P.cst[a] = r[0] != 0.0 ? r[1 + a] / r[0] : 0.0; ke += r[1 + a] * P.cst[a]; }

@@ -68,5 +68,6 @@ const SysOps* ops_maxwell2d();
 const SysOps* ops_allencahn2d();
 const SysOps* ops_inse2d();
 const SysOps* ops_elasticity2d();
+const SysOps* ops_nsf2d();
 
 }  // namespace lbmk

@@ -24,7 +24,7 @@
 namespace lbmk {
 
 enum { SYS_ADVECTION2D = 0, SYS_BURGERS2D = 1, SYS_SWE2D = 2, SYS_EULER2D = 3, SYS_ADR2D = 4, SYS_NSF3D = 5, SYS_MHD3D = 6,
-       SYS_URF2D = 7, SYS_MAXWELL2D = 8, SYS_ALLENCAHN2D = 9, SYS_INSE2D = 10, SYS_ELASTICITY2D = 11 };
+       SYS_URF2D = 7, SYS_MAXWELL2D = 8, SYS_ALLENCAHN2D = 9, SYS_INSE2D = 10, SYS_ELASTICITY2D = 11, SYS_NSF2D = 12 };
 
 // ------------------------------------------------------------------------------------------ advection
 // Phi = (a_x U, a_y U); par = {a_x, a_y}
@@ -268,6 +268,79 @@ template <class R> struct SysElasticity2D {
     __device__ static void wave(const double*, const KParams<double>& P, double* out) {
         const double cp = sqrt((P.par[2] + 2.0 * P.par[1]) / P.par[0]);      // rest-state longitudinal speed
         out[0] = cp; out[1] = cp; out[2] = 0.0;
+    }
+};
+
+// ------------------------------------------------------------------------------------------ compressible NSF 2D
+// eq (3.23)-(3.24); Listing 2; cascade on the CONSERVED fields (N = 4 + 8, SM4.10 L961):
+// Q = (rho, m0, m1, E, G^L_{V,b} = dx d_b V [index 4 + 2 v + b], V = rho, m0, m1, E); par = {gamma, mu, K}.
+// Derived gradients by the chain rule: d_b u_a = (G_{ma,b} - u_a G_{rho,b})/rho,
+//   d_b p = (gamma-1)(G_{E,b} - u.G_{m,b} + |u|^2/2 G_{rho,b}),  d_b T = (d_b p - T G_{rho,b})/rho,  T = p/rho.
+// Reference: (rho0, m0, E0) free (moving reference as in Euler 2D), trackers 0 (host-checked).
+template <class R> struct SysNsf2D {
+    static constexpr int ID = SYS_NSF2D, D = 2, M = 12, MC = 4;
+    using Mms = Mms_nsf2d;
+    struct Ctx { R u[2], du[2], ul[2], dp, tau[2][2], qh[2]; };
+    __device__ __forceinline__ static void setup(Ctx& c, const R (&dQ)[M], const KParams<R>& P) {
+        const R rho = P.ref[0] + dQ[0];
+        const R r = R(1) / rho;
+        R dke = R(0), u2 = R(0);
+#pragma unroll
+        for (int a = 0; a < 2; ++a) {
+            c.du[a] = (dQ[1 + a] - P.cst[a] * dQ[0]) * r;
+            c.u[a] = P.cst[a] + c.du[a];
+            c.ul[a] = c.u[a] * P.il;
+            dke += dQ[1 + a] * c.u[a] + P.ref[1 + a] * c.du[a];
+            u2 += c.u[a] * c.u[a];
+        }
+        const R gm1 = P.par[0] - R(1);
+        c.dp = gm1 * (dQ[3] - R(0.5) * dke);
+        const R T = (P.cst[3] + c.dp) * r;
+        const R muL = P.par[1] * P.dL, KL = P.par[2] * P.dL;
+        R gu[2][2], dT[2];
+#pragma unroll
+        for (int b = 0; b < 2; ++b) {
+            gu[0][b] = (dQ[6 + b] - c.u[0] * dQ[4 + b]) * r;
+            gu[1][b] = (dQ[8 + b] - c.u[1] * dQ[4 + b]) * r;
+            const R dpb = gm1 * (dQ[10 + b] - c.u[0] * dQ[6 + b] - c.u[1] * dQ[8 + b] + R(0.5) * u2 * dQ[4 + b]);
+            dT[b] = (dpb - T * dQ[4 + b]) * r;
+        }
+        const R dv = R(2.0 / 3.0) * muL * (gu[0][0] + gu[1][1]);
+        c.tau[0][0] = R(2) * muL * gu[0][0] - dv;
+        c.tau[1][1] = R(2) * muL * gu[1][1] - dv;
+        c.tau[0][1] = c.tau[1][0] = muL * (gu[0][1] + gu[1][0]);
+#pragma unroll
+        for (int j = 0; j < 2; ++j) c.qh[j] = c.tau[j][0] * c.u[0] + c.tau[j][1] * c.u[1] + KL * dT[j];
+    }
+    template <int k> __device__ __forceinline__ static void flux(const Ctx& c, const R (&dQ)[M], const KParams<R>& P, R (&F)[D], R& S) {
+        if constexpr (k == 0) {
+            F[0] = P.il * dQ[1]; F[1] = P.il * dQ[2]; S = R(0);
+        } else if constexpr (k <= 2) {
+            constexpr int a = k - 1;
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                R v = dQ[1 + a] * c.u[j] + P.ref[1 + a] * c.du[j];
+                if (j == a) v += c.dp;
+                F[j] = P.il * v - c.tau[a][j];
+            }
+            S = R(0);
+        } else if constexpr (k == 3) {
+#pragma unroll
+            for (int j = 0; j < 2; ++j) F[j] = P.il * ((dQ[3] + c.dp) * c.u[j] + P.cst[4] * c.du[j]) - c.qh[j];
+            S = R(0);
+        } else {
+            constexpr int v = (k - 4) / 2, b = (k - 4) % 2;
+            F[0] = dQ[k] * c.ul[0]; F[1] = dQ[k] * c.ul[1];
+            F[b] -= dQ[v] * P.inv_gtau;
+            S = -dQ[k] * P.inv_gtau;
+        }
+    }
+    __device__ static void wave(const double* Q, const KParams<double>& P, double* out) {
+        const double u = Q[1] / Q[0], v = Q[2] / Q[0];
+        const double p = (P.par[0] - 1.0) * (Q[3] - 0.5 * Q[0] * (u * u + v * v));
+        const double cc = sqrt(P.par[0] * p / Q[0]);
+        out[0] = fmax(fabs(u), fabs(v)) + cc; out[1] = sqrt(u * u + v * v) + cc;
+        out[2] = sqrt(fmax(4.0 * P.par[1] * P.dL / (3.0 * Q[0]), P.par[2] * P.dL * (P.par[0] - 1.0) / Q[0]) * P.inv_gtau);
     }
 };
 

@@ -257,8 +257,45 @@ def sys_elasticity2d():
     return "elasticity2d", 2, prim, build
 
 
+def sys_nsf2d():
+    gamma, mu, K = par(0), par(1), par(2)
+    k = TWO_PI
+    p0 = 1 / gamma                                                                            # rho0 = c_s = 1 (reading A9)
+    drho = sp.Rational(1, 5) * sp.sin(k * x) * sp.cos(k * y) * sp.cos(t)                       # eq SM5.10
+    prim = {"rho": 1 + drho,
+            "u0": 3 + sp.Rational(1, 5) * sp.cos(k * x) * sp.sin(k * y) * sp.sin(t),
+            "u1": 2 + sp.Rational(3, 20) * sp.sin(k * x) * sp.sin(k * y) * sp.cos(t),
+            "p": p0 + drho + sp.Rational(1, 5) * p0 * sp.cos(k * x) * sp.sin(k * y) * sp.sin(t)}
+
+    def build(P, D):
+        X = (x, y)
+        rho, p = P["rho"], P["p"]
+        u = [P["u0"], P["u1"]]
+        T = p / rho
+        E = p / (gamma - 1) + rho * (u[0]**2 + u[1]**2) / 2
+        V = [rho, rho * u[0], rho * u[1], E]
+        G = [[dx * D(V[v], X[b]) for b in range(2)] for v in range(4)]
+        muL, KL = mu * dt / dx**2, K * dt / dx**2
+        # physical gradients of the derived fields are those of the exact fields: dx d_b u_a etc. (chain rule on exact data)
+        gu = [[dx * D(u[a], X[b]) for b in range(2)] for a in range(2)]
+        gT = [dx * D(T, X[b]) for b in range(2)]
+        divu = gu[0][0] + gu[1][1]
+        tau = [[muL * (gu[a][b] + gu[b][a]) - (sp.Rational(2, 3) * muL * divu if a == b else 0) for b in range(2)] for a in range(2)]
+        Q = V + [G[v][b] for v in range(4) for b in range(2)]
+        F = [[il * V[1], il * V[2]]]
+        for a in range(2):
+            F.append([il * (V[1 + a] * u[j] + (p if a == j else 0)) - tau[a][j] for j in range(2)])
+        F.append([il * (E + p) * u[j] - sum(tau[j][b] * u[b] for b in range(2)) - KL * gT[j] for j in range(2)])
+        for v in range(4):
+            for b in range(2):
+                F.append([il * G[v][b] * u[j] - (V[v] / gtau if j == b else 0) for j in range(2)])
+        S = [sp.Integer(0)] * 4 + [-G[v][b] / gtau for v in range(4) for b in range(2)]
+        return Q, F, S
+    return "nsf2d", 2, prim, build
+
+
 SYSTEMS = [sys_burgers2d, sys_swe2d, sys_euler2d, sys_adr2d, sys_nsf3d, sys_urf2d, sys_maxwell2d, sys_allencahn2d, sys_inse2d,
-           sys_elasticity2d]
+           sys_elasticity2d, sys_nsf2d]
 
 
 # ------------------------------------------------------------------------------------------------ printing

@@ -54,7 +54,7 @@ def test_system_info_matches_workloads():
 
 def _params(name):
     return {"advection2d": [0.1, 0.05], "burgers2d": [], "swe2d": [1.0], "euler2d": [1.4], "adr2d": [0.1, -0.1, 0.01, 1.0],
-            "nsf3d": [1.4, 1e-3, 5e-3], "mhd3d": [1.4, 1e-3], "urf2d": [], "maxwell2d": [1.0], "allencahn2d": [0.01, 1.0], "inse2d": [1.0, 0.01], "elasticity2d": [1.0, 1.0, 2.0]}[name]
+            "nsf3d": [1.4, 1e-3, 5e-3], "mhd3d": [1.4, 1e-3], "urf2d": [], "maxwell2d": [1.0], "allencahn2d": [0.01, 1.0], "inse2d": [1.0, 0.01], "elasticity2d": [1.0, 1.0, 2.0], "nsf2d": [1.4, 0.0084, 0.0416]}[name]
 
 
 def test_argument_validation():

@@ -24,7 +24,7 @@ def P():
 @pytest.mark.parametrize("mk,kw,steps", [
     (W.pin_burgers, dict(n=40), 30), (W.pin_euler, dict(n=36), 25), (W.pin_adr, dict(n=32), 40), (W.c2_swe, dict(n=48, ny=20), 21),
     (W.c4_nsf3d, dict(n=16, ny=12, nz=10, precision="f64"), 9), (W.c4_nsf3d, dict(n=16, ny=12, nz=10), 8),
-    (W.pin_urf, dict(n=32), 17), (W.pin_maxwell, dict(n=32), 16), (W.pin_allencahn, dict(n=32), 40), (W.pin_inse, dict(n=32), 40), (W.pin_elasticity, dict(n=32), 40)])
+    (W.pin_urf, dict(n=32), 17), (W.pin_maxwell, dict(n=32), 16), (W.pin_allencahn, dict(n=32), 40), (W.pin_inse, dict(n=32), 40), (W.pin_elasticity, dict(n=32), 40), (W.pin_nsf2d, dict(n=32), 40)])
 @pytest.mark.parametrize("pattern", ["pull2", "aa"])
 def test_error_norms_match_numpy(P, mk, kw, steps, pattern):
     """Device reductions vs norms formed in NumPy from the read-back state and the ORACLE's exact fields (jets)."""
@@ -105,6 +105,26 @@ def test_paper_table2_inse_row_partially_reproduced(P):
           f"rho u Linf {mom_linf:.4e} (paper 8.2447e-04) L2 {mom_l2:.4e} (paper 8.5394e-04)")
     assert abs(mom_l2 - 8.5394e-04) <= 2e-3 * 8.5394e-04
     assert abs(mom_linf - 8.2447e-04) <= 0.5 * 8.2447e-04 and abs(n[0][1] - 6.0683e-07) <= 0.5 * 6.0683e-07
+
+
+def test_paper_table2_nsf2d_row_magnitude_only(P):
+    """Compressible NSF 2D, the paper's running example (Listing 2; Table 2).  Its component
+    listing is garbled (L971), so the system is built from eq (3.23)-(3.24) with the chain-rule cascade on the conserved
+    fields.  At the printed working point (f = 2, tau_R = 60, g_tau = 6) the GPU run converges at second order and lands
+    at 1.8-2.1x the printed errors; scans of f, tau_R, g_tau and the viscosity scale do not close the gap (the scheme is
+    at its stability edge: tau_R < 60 or g_tau = 3 blow up) -- reading A24, UNPINNED beyond P1/P3/P10.  Gate: factor 2.5."""
+    w = W.pin_nsf2d(512)
+    g = P.Grid.from_workload(w)
+    g.init_from_U(w.initial_U())
+    g.step(w.steps)
+    n = g.error_norms()
+    g.close()
+    got = {"rho": (n[0][2], n[0][1]), "rhou": (math.hypot(n[1][2], n[2][2]), math.hypot(n[1][1], n[2][1])), "E": (n[3][2], n[3][1])}
+    paper = {"rho": (7.3384e-05, 3.7592e-05), "rhou": (1.1775e-04, 6.8579e-05), "E": (8.3354e-05, 4.5785e-05)}
+    for k in got:
+        print(f"{w.name} {k}: Linf {got[k][0]:.4e} (paper {paper[k][0]:.4e})  L2 {got[k][1]:.4e} (paper {paper[k][1]:.4e})")
+        for a, b in zip(got[k], paper[k]):
+            assert b / 2.5 <= a <= b * 2.5
 
 
 @pytest.mark.parametrize("mk,field,paper_l2", [(W.pin_urf, 0, 4.7227e-06), (W.pin_maxwell, 0, 3.0632e-05)])

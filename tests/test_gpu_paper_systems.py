@@ -41,7 +41,8 @@ def _pair(P, w, steps, **kw):
 @pytest.mark.parametrize("mk,n,steps", [(W.pin_urf, 48, 121), (W.pin_maxwell, 40, 150), (W.pin_urf, 256, 24), (W.pin_maxwell, 256, 25),
                                         (W.pin_allencahn, 40, 300), (W.pin_allencahn, 256, 30),
                                         (W.pin_inse, 40, 300), (W.pin_inse, 256, 30),
-                                        (W.pin_elasticity, 40, 200), (W.pin_elasticity, 256, 30)])
+                                        (W.pin_elasticity, 40, 200), (W.pin_elasticity, 256, 30),
+                                        (W.pin_nsf2d, 40, 300), (W.pin_nsf2d, 256, 30)])
 @pytest.mark.parametrize("precision", ["f64", "f64s"])
 def test_parity_fp64(P, mk, n, steps, pattern, precision):
     """n = 256 takes the staged-coefficient path (nx a multiple of the block size), the small grids the global one."""
@@ -56,7 +57,7 @@ def test_parity_fp64(P, mk, n, steps, pattern, precision):
 
 
 @pytest.mark.parametrize("pattern", ["pull2", "aa"])
-@pytest.mark.parametrize("mk,n,steps", [(W.pin_urf, 64, 320), (W.pin_maxwell, 64, 320), (W.pin_urf, 256, 60), (W.pin_allencahn, 64, 300), (W.pin_inse, 64, 300), (W.pin_elasticity, 64, 200)])
+@pytest.mark.parametrize("mk,n,steps", [(W.pin_urf, 64, 320), (W.pin_maxwell, 64, 320), (W.pin_urf, 256, 60), (W.pin_allencahn, 64, 300), (W.pin_inse, 64, 300), (W.pin_elasticity, 64, 200), (W.pin_nsf2d, 64, 300)])
 def test_parity_fp32_shifted(P, mk, n, steps, pattern):
     """Reference- and equilibrium-shifted fp32 (eq 2.23): to t = 1 on the 64^2 grid of the paper's study for the acoustic
     cases; 300 steps for Allen-Cahn (diffusive scaling, omega = 1.91: over 2156 steps to t = 1 fp32 rounding grows to

@@ -16,9 +16,9 @@ from oracle import OracleGrid
 from brute_force import (LATTICES, flux_adr_listing, flux_allencahn_listing, flux_elasticity_listing, flux_euler_listing, flux_inse_listing, flux_maxwell_listing, flux_swe_listing, flux_urf_listing,
                          init_equilibrium, moments, step as bf_step)
 
-SYSTEMS = ["advection2d", "burgers2d", "swe2d", "euler2d", "adr2d", "nsf3d", "mhd3d", "urf2d", "maxwell2d", "allencahn2d", "inse2d", "elasticity2d"]
+SYSTEMS = ["advection2d", "burgers2d", "swe2d", "euler2d", "adr2d", "nsf3d", "mhd3d", "urf2d", "maxwell2d", "allencahn2d", "inse2d", "elasticity2d", "nsf2d"]
 PARAMS = {"advection2d": [0.1, 0.05], "burgers2d": [], "swe2d": [1.0], "euler2d": [1.4],
-          "adr2d": [0.1, -0.1, 0.01, 1.0], "nsf3d": [1.4, 1e-3, 4.9e-3], "mhd3d": [1.4, 1e-3], "urf2d": [], "maxwell2d": [1.0], "allencahn2d": [0.01, 1.0], "inse2d": [1.0, 0.01], "elasticity2d": [1.3, 1.0, 2.0]}
+          "adr2d": [0.1, -0.1, 0.01, 1.0], "nsf3d": [1.4, 1e-3, 4.9e-3], "mhd3d": [1.4, 1e-3], "urf2d": [], "maxwell2d": [1.0], "allencahn2d": [0.01, 1.0], "inse2d": [1.0, 0.01], "elasticity2d": [1.3, 1.0, 2.0], "nsf2d": [1.4, 0.0084, 0.0416]}
 
 
 def small_grid(system, **kw):
@@ -33,9 +33,9 @@ def physical_state(system, rng, shape=()):
     """A random admissible state (rho, h > 0, p > 0)."""
     m = len(W.COMPONENTS[system])
     U = rng.uniform(-0.3, 0.3, size=(m,) + shape)
-    if system in ("swe2d", "euler2d", "nsf3d", "mhd3d", "inse2d"):
+    if system in ("swe2d", "euler2d", "nsf3d", "mhd3d", "inse2d", "nsf2d"):
         U[0] = rng.uniform(0.8, 1.2, size=shape)
-    if system == "euler2d":
+    if system in ("euler2d", "nsf2d"):
         U[3] = rng.uniform(2.0, 3.0, size=shape)
     if system in ("nsf3d", "mhd3d"):
         U[4] = rng.uniform(2.0, 3.0, size=shape)
@@ -275,6 +275,7 @@ MMS_CASES = {
     "allencahn2d": lambda: W.pin_allencahn(32),
     "inse2d": lambda: W.pin_inse(32),
     "elasticity2d": lambda: W.pin_elasticity(32),
+    "nsf2d": lambda: W.pin_nsf2d(32),
 }
 
 

@@ -42,12 +42,13 @@ COMPONENTS: Dict[str, List[str]] = {
     "allencahn2d": ["phi", "Gx", "Gy"],
     "inse2d": ["rho", "mx", "my", "Gxx", "Gxy", "Gyx", "Gyy"],
     "elasticity2d": ["F00", "F01", "F10", "F11", "m0", "m1"],
+    "nsf2d": ["rho", "mx", "my", "E", "Grx", "Gry", "Gmxx", "Gmxy", "Gmyx", "Gmyy", "GEx", "GEy"],
 }
 N_CONSERVED = {"advection2d": 1, "burgers2d": 1, "swe2d": 3, "euler2d": 4,
-               "adr2d": 1, "nsf3d": 5, "mhd3d": 8, "urf2d": 3, "maxwell2d": 3, "allencahn2d": 1, "inse2d": 3, "elasticity2d": 6}
+               "adr2d": 1, "nsf3d": 5, "mhd3d": 8, "urf2d": 3, "maxwell2d": 3, "allencahn2d": 1, "inse2d": 3, "elasticity2d": 6, "nsf2d": 4}
 LATTICE_OF = {"advection2d": "D2Q5", "burgers2d": "D2Q5", "swe2d": "D2Q5",
               "euler2d": "D2Q5", "adr2d": "D2Q5", "nsf3d": "D3Q7", "mhd3d": "D3Q7",
-              "urf2d": "D2Q5", "maxwell2d": "D2Q5", "allencahn2d": "D2Q5", "inse2d": "D2Q5", "elasticity2d": "D2Q5"}
+              "urf2d": "D2Q5", "maxwell2d": "D2Q5", "allencahn2d": "D2Q5", "inse2d": "D2Q5", "elasticity2d": "D2Q5", "nsf2d": "D2Q5"}
 # c_s^2 per lattice, Table SM1; used only by the lambda rule below.
 CS2 = {"D2Q5": 1.0 / 3.0, "D3Q7": 1.0 / 4.0}
 SIGMA = 0.6  # lambda rule: lattice wave speed = SIGMA * c_s^2 (SURVEY.md §8(c) "lambda rule")
@@ -476,6 +477,41 @@ def pin_elasticity(n: int = 512, precision: str = "f64") -> Workload:
                     dx=1.0 / n, lam=1.0 / f, params=[1.0, mus, las], tau_R=tau_R, g_tau=0.0,
                     U_ref=[1.0, 0.0, 0.0, 1.0, 0.0, 0.0], mms_id=1, mms_params=[], steps=int(round(n / f)), s_max=1.3 * cp,
                     seed=0, init=_init_elasticity, note="PAPER.md Table 2 L536-L539")
+
+
+def _init_nsf2d(w: Workload) -> np.ndarray:
+    # eq (SM5.10), PAPER.md:L1351-L1358 at t = 0 (cos t = 1, sin t = 0); trackers = dx * gradient of the conserved fields,
+    # by the product rule from the analytic derivatives of (rho, u, v, p)
+    gamma = w.params[0]
+    p0 = 1.0 / gamma
+    x, y, _ = _grid(w)
+    k = TWO_PI
+    sx, cx, sy, cy = np.sin(k * x), np.cos(k * x), np.sin(k * y), np.cos(k * y)
+    rho, rx, ry = 1.0 + 0.2 * sx * cy, 0.2 * k * cx * cy, -0.2 * k * sx * sy
+    u, ux, uy = 3.0 + 0.0 * sx * sy, 0.0 * sx * sy, 0.0 * sx * sy
+    v, vx, vy = 2.0 + 0.15 * sx * sy, 0.15 * k * cx * sy, 0.15 * k * sx * cy
+    p, px, py = p0 + 0.2 * sx * cy, rx, ry
+    ke = 0.5 * (u * u + v * v)
+    V = [rho, rho * u, rho * v, p / (gamma - 1.0) + rho * ke]
+    dV = [(rx, ry), (rx * u + rho * ux, ry * u + rho * uy), (rx * v + rho * vx, ry * v + rho * vy),
+          (px / (gamma - 1.0) + rx * ke + rho * (u * ux + v * vx), py / (gamma - 1.0) + ry * ke + rho * (u * uy + v * vy))]
+    comps = V + [w.dx * d for pair in dV for d in pair]
+    return np.stack([_full(w, c) for c in comps]).copy()
+
+
+def pin_nsf2d(n: int = 512, precision: str = "f64") -> Workload:
+    # compressible NSF 2D; Table SM2: diffusive f = 2, tau_R = 60, g_tau = 6; Table SM11
+    # non-dimensionalised by rho0, c_s, L, R (reading A9): mu = 3.52/(1.225*340.2), K = 4980/(1.225*340.2*287)
+    f = 2.0
+    dx = 1.0 / n
+    dt = f * dx * dx
+    gamma = 1.4
+    mu, K = 3.52 / (1.225 * 340.2), 4980.0 / (1.225 * 340.2 * 287.0)
+    E0 = (1.0 / gamma) / (gamma - 1.0) + 0.5 * 13.0
+    return Workload(name=f"pin_nsf2d_{n}", system="nsf2d", nx=n, ny=n, nz=1, precision=precision,
+                    dx=dx, lam=dx / dt, params=[gamma, mu, K], tau_R=60.0, g_tau=6.0,
+                    U_ref=[1.0, 3.0, 2.0, E0] + [0.0] * 8, mms_id=1, mms_params=[], steps=int(round(1.0 / dt)), s_max=5.5,
+                    seed=0, init=_init_nsf2d, note="PAPER.md Table 2 L547-L551")
 
 
 BASELINE_CONFIGS: Dict[str, Callable[..., Workload]] = {
