@@ -18,6 +18,8 @@ One JSON line is printed by rank 0:
               copy bandwidth in MEASURED_PEAKS.json
   cpu_baseline  the CPU oracle (oracle/, plain fp64 C++) timed on this box's host cores on a bounded sample
   all_configs   short runs of the other BASELINE.json configs (reported, not the headline)
+  paper_table3_systems  the paper's Table 3 systems compiled in here (4096^2, forcing off, S and D) next to the paper's
+                RTX A5000 numbers (context); skipped with --no-table3 / --no-all-configs
 
 Multi-GPU (--gpus N under torchrun): by default "replicas only" -- every rank advances its own
 full-size grid, no data-path collective; value = sum over ranks / max-over-ranks time; scaling "weak".
@@ -70,7 +72,8 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--parallelism", default="replicas", choices=["replicas", "slabs"],
                     help="N > 1: independent replicas (default) or z-slabs of one N-times-taller periodic grid with a halo exchange per step")
-    ap.add_argument("--table3", action="store_true", help="also run the paper's Table 3 systems (4096^2, forcing off, S and D)")
+    ap.add_argument("--table3", action="store_true", help="(default on) also run the paper's Table 3 systems (4096^2, forcing off, S and D)")
+    ap.add_argument("--no-table3", action="store_true")
     return ap.parse_args()
 
 
@@ -493,7 +496,7 @@ def run_ours(args):
                 others[name] = {"error": repr(e)}
             torch.cuda.empty_cache()
         line["all_configs"] = others
-    if args.table3 and world == 1:
+    if not args.no_table3 and not args.no_all_configs and world == 1 or args.table3 and world == 1:
         line["paper_table3_systems"] = table3_runs(P, torch, peak)
     print(json.dumps(line))
     if dist is not None:
