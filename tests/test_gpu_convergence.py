@@ -127,6 +127,40 @@ def test_paper_table2_nsf2d_row_magnitude_only(P):
             assert b / 2.5 <= a <= b * 2.5
 
 
+# printed EOCs (Table 2, Double): field -> (components, Linf EOC, L2 EOC); "negative least-squares log-log slope
+# over all simulated resolutions" (L514), N = 64, 128, 256, 512 (L499)
+TABLE2_EOC = [
+    (W.pin_burgers, {"u": ((0,), 1.46, 1.87)}),
+    (W.pin_euler, {"rho": ((0,), 1.98, 1.99), "E": ((3,), 2.01, 2.00), "rhou": ((1, 2), 2.00, 2.00)}),
+    (W.pin_urf, {"E": ((0,), 2.00, 2.00), "S": ((1, 2), 2.00, 2.00)}),
+    (W.pin_maxwell, {"Ez": ((0,), 1.95, 1.95), "Hx": ((1,), 2.00, 2.00), "Hy": ((2,), 2.02, 2.02)}),
+    (W.pin_elasticity, {"F": ((0, 1, 2, 3), 2.00, 2.00), "v": ((4, 5), 2.01, 1.99)}),
+    (W.pin_adr, {"c": ((0,), 2.50, 2.49)}),
+    (W.pin_allencahn, {"phi": ((0,), 2.50, 2.51)}),
+]
+
+
+@pytest.mark.parametrize("mk,fields", TABLE2_EOC)
+def test_paper_table2_eoc_reproduced_on_the_gpu(P, mk, fields):
+    """The refinement study itself on the device: four resolutions to t = 1 in fp64, LSQ slope of log2(error) vs
+    log2(N) -- equal to the printed experimental orders of convergence to their 2 decimals."""
+    ns = (64, 128, 256, 512)
+    norms = []
+    for n in ns:
+        w = mk(n)
+        g = P.Grid.from_workload(w)
+        g.init_from_U(w.initial_U())
+        g.step(w.steps)
+        norms.append(g.error_norms())
+        g.close()
+    for name, (ks, eoc_inf, eoc_2) in fields.items():
+        for j, want in ((2, eoc_inf), (1, eoc_2)):
+            err = [math.sqrt(sum(e[k][j] ** 2 for k in ks)) for e in norms]
+            slope = -np.polyfit(np.log2(ns), np.log2(err), 1)[0]
+            print(f"{mk.__name__} {name} {'Linf' if j == 2 else 'L2'} EOC {slope:.3f} (paper {want:.2f})")
+            assert abs(slope - want) <= 0.0151, (mk.__name__, name, j, slope, want)
+
+
 @pytest.mark.parametrize("mk,field,paper_l2", [(W.pin_urf, 0, 4.7227e-06), (W.pin_maxwell, 0, 3.0632e-05)])
 def test_paper_table2_float_rows_same_magnitude(P, mk, field, paper_l2):
     """Float rows (same f, tau_R as double for these two systems, Table SM2): rounding differs between
