@@ -314,8 +314,9 @@ def _init_burgers(w: Workload) -> np.ndarray:
 def pin_burgers(n: int = 512, precision: str = "f64") -> Workload:
     # Table SM2: acoustic f = 0.2 (1/lambda = 0.2), tau_R = 0.2; SM5.2 (L1161-L1167): A = 1.3
     f = 0.2
+    tau_R = 0.2 if precision in ("f64", "f64s") else 2.0          # Table SM2: Double 0.2, Float 2
     return Workload(name=f"pin_burgers2d_{n}", system="burgers2d", nx=n, ny=n, nz=1, precision=precision,
-                    dx=1.0 / n, lam=1.0 / f, params=[], tau_R=0.2, g_tau=0.0, U_ref=[0.0], mms_id=1,
+                    dx=1.0 / n, lam=1.0 / f, params=[], tau_R=tau_R, g_tau=0.0, U_ref=[0.0], mms_id=1,
                     mms_params=[1.3], steps=int(round(n / f)), s_max=1.3, seed=0, init=_init_burgers,
                     note="PAPER.md Table 2 L518")
 
@@ -337,8 +338,9 @@ def _init_euler_mms(w: Workload) -> np.ndarray:
 def pin_euler(n: int = 512, precision: str = "f64") -> Workload:
     # Table SM2: f = 0.05, tau_R = 0.2; SM5.3 (L1175-L1186)
     f, gamma = 0.05, 1.4
+    tau_R = 0.2 if precision in ("f64", "f64s") else 5.0          # Table SM2: Double 0.2, Float 5
     return Workload(name=f"pin_euler2d_{n}", system="euler2d", nx=n, ny=n, nz=1, precision=precision,
-                    dx=1.0 / n, lam=1.0 / f, params=[gamma], tau_R=0.2, g_tau=0.0,
+                    dx=1.0 / n, lam=1.0 / f, params=[gamma], tau_R=tau_R, g_tau=0.0,
                     U_ref=[1.0, 3.0, 3.0, (1.0 / gamma) / (gamma - 1.0) + 9.0], mms_id=1, mms_params=[],
                     steps=int(round(n / f)), s_max=3.3 + math.sqrt(gamma * (1 / gamma + 0.3 + 0.2 / gamma) / 0.7),
                     seed=0, init=_init_euler_mms, note="PAPER.md Table 2 L519-L522")
