@@ -86,6 +86,49 @@ def test_mhd3d_flux_matches_independent_vector_form():
         assert np.abs(F - Fn).max() < 1e-13 and np.abs(S - Sn).max() < 1e-13
 
 
+def nsf2d_flux_numpy(U, gamma, mu, K, dx, dt, g_tau):
+    """Compressible NSF 2D with the cascade on the conserved fields (eq 3.23-3.24, Listing 2): gradients of the derived
+    fields u, T from the tracked gradients of (rho, m, E) by the chain rule, written here with Jacobian matrices."""
+    lam, dL = dx / dt, dt / dx**2
+    rho, m, E = U[0], U[1:3], U[3]
+    GV = U[4:12].reshape(4, 2) / dx                      # physical gradients d_b V, V = rho, m0, m1, E
+    u = m / rho
+    p = (gamma - 1) * (E - 0.5 * (m @ m) / rho)
+    T = p / rho
+    # Jacobians of u and T with respect to (rho, m0, m1, E)
+    dudV = np.array([[-u[0] / rho, 1 / rho, 0, 0], [-u[1] / rho, 0, 1 / rho, 0]])
+    dpdV = (gamma - 1) * np.array([0.5 * (u @ u), -u[0], -u[1], 1.0])
+    dTdV = dpdV / rho - np.array([T / rho, 0, 0, 0])
+    gu = dudV @ GV                                       # gu[a][b] = d_b u_a
+    gT = dTdV @ GV
+    tau = mu * (gu + gu.T - (2.0 / 3.0) * np.trace(gu) * np.eye(2))
+    q = -K * gT
+    Phi = np.zeros((12, 2))
+    Phi[0] = m
+    Phi[1:3] = np.outer(m, u) + p * np.eye(2) - tau
+    Phi[3] = (E + p) * u - tau @ u + q
+    F = Phi * dt / dx
+    S = np.zeros(12)
+    V = U[:4]
+    for v in range(4):
+        for b in range(2):
+            F[4 + 2 * v + b] = U[4 + 2 * v + b] * u / lam
+            F[4 + 2 * v + b, b] -= V[v] / g_tau
+    S[4:] = -U[4:] / g_tau
+    return F, S
+
+
+def test_nsf2d_flux_matches_independent_vector_form():
+    rng = np.random.default_rng(7)
+    gamma, mu, K, dx, lam, g_tau = 1.4, 8e-3, 4e-2, 1.0 / 32, 16.0, 6.0
+    g = OracleGrid("nsf2d", 4, 4, 1, dx=dx, lam=lam, params=[gamma, mu, K], g_tau=g_tau)
+    for _ in range(20):
+        U = rng.uniform(-0.3, 0.3, 12); U[0] = rng.uniform(0.8, 1.3); U[3] = rng.uniform(2.0, 3.0)
+        F, S = g.flux_source(U)
+        Fn, Sn = nsf2d_flux_numpy(U, gamma, mu, K, dx, dx / lam, g_tau)
+        assert np.abs(F[:, :2] - Fn).max() < 1e-13 and np.abs(S - Sn).max() < 1e-13
+
+
 def test_mhd3d_alfven_wave_speed():
     """Textbook closed form: a small transverse perturbation of a uniform field B0 e_x travels at v_A = B0/sqrt(rho)
     with dv = -dB/sqrt(rho) (ideal MHD, eta = 0).  Checks the signs of B (x) B in the momentum flux and of the
