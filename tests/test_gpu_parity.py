@@ -224,3 +224,38 @@ def test_full_size_c5_sampled_and_conservation(P):
     U0 = w.initial_U()
     for k in (0, 4):
         assert abs(U[k].sum() - U0[k].sum()) / abs(U0[k].sum()) < 1e-6
+
+
+# ------------------------------------------------------------------- full size AND full duration (properties)
+@pytest.mark.parametrize("name,cons", [("c3", (0, 3)), ("c5", (0, 4))])
+def test_full_size_full_duration_properties(P, name, cons):
+    """BASELINE.json configs[2] / configs[4] at their full grid and step count in the bench launch configuration:
+    properties that hold at any size -- finite state, conserved totals on the periodic domain (pin P2; momentum and B
+    have zero mean), sub-characteristic condition still met at the end."""
+    w = W.BASELINE_CONFIGS[name]()
+    U0 = w.initial_U()
+    g = P.Grid.from_workload(w)
+    g.init_from_U(U0)
+    g.step(w.steps)
+    U = g.read_U()
+    speeds, status = g.max_wave_speed()
+    g.close()
+    assert np.isfinite(U).all() and status == 0
+    for k in cons:
+        assert abs(U[k].sum() - U0[k].sum()) / abs(U0[k].sum()) < 2e-6
+    for k in range(1, w.dim + 1):                              # total momentum stays zero (relative to rho c per node)
+        assert abs(U[k].mean()) < 1e-6
+
+
+def test_full_size_full_duration_c4_error_against_manufactured_solution(P):
+    """configs[3], 256^3, 200 steps, forcing on: the relative L2 error against the manufactured solution stays at the
+    scheme's truncation level (the same run on the 64^3 oracle gives the reference magnitude, O(dx^2) smaller here)."""
+    w = W.c4_nsf3d()
+    g = P.Grid.from_workload(w)
+    g.init_from_U(w.initial_U())
+    g.step(w.steps)
+    e = g.error_norms()
+    g.close()
+    assert np.isfinite(e[:5]).all()
+    assert e[0][1] < 1e-5 and e[4][1] < 1e-5                   # rho, E relative L2
+    assert max(e[k][2] for k in (1, 2, 3)) < 5e-3              # momentum relative Linf (fp32, 200 steps)
