@@ -130,3 +130,36 @@ def test_degenerate_grids_parity(P, name, kw, pattern):
     U, Uo, fo, _, _ = _pair(P, w, 7, pattern=pattern)
     tol = TOL64 if w.precision == "f64" else TOL32
     assert np.isfinite(U).all() and rel_err(U, Uo, fo).max() <= tol
+
+
+# ------------------------------------------------------------------------ out-of-bounds guard (no sanitizer on this pool)
+@pytest.mark.parametrize("mk,kw", [(W.c1_advection, dict(n=37, ny=23)), (W.c4_nsf3d, dict(n=5, ny=4, nz=3)), (W.c4_nsf3d, dict(n=130, ny=3, nz=2)),
+                                   (W.c5_mhd3d, dict(n=9, ny=2, nz=5)), (W.c2_swe, dict(n=257, ny=3)), (W.pin_nsf2d, dict(n=19))])
+@pytest.mark.parametrize("pattern", ["pull2", "aa"])
+def test_workspace_guards_stay_untouched(P, mk, kw, pattern):
+    """The workspace is bound inside a larger buffer filled with a sentinel; after init, steps (ragged last tile, wraps
+    on every axis, forcing tables), reductions and readbacks the guard bands before and after it are unchanged."""
+    import torch
+    w = mk(**kw)
+    s = P.System(w.system, params=w.params, tau_R=w.tau_R, g_tau=w.g_tau, U_ref=w.U_ref, mms_id=w.mms_id,
+                 mms_params=w.mms_params if w.mms_id else ())
+    prec = {"f64": P.LBMK_F64, "f32s": P.LBMK_F32_SHIFTED}[w.precision]
+    g = P.lbmk_grid_create(s.h, w.nx, w.ny, w.nz, 0, w.dx, w.lam, prec, torch.cuda.current_stream().cuda_stream)
+    P.lbmk_grid_set_option(g, P.LBMK_OPT_PATTERN, P.PATTERN[pattern])
+    nbytes = P.lbmk_grid_workspace_bytes(g)
+    G = 1 << 16
+    buf = torch.full((nbytes + 2 * G + 256,), 0xA5, dtype=torch.uint8, device="cuda")
+    off = (-buf.data_ptr()) % 256 + G
+    P.lbmk_grid_bind_workspace(g, buf.data_ptr() + off, nbytes)
+    U0 = torch.from_numpy(w.initial_U()).cuda()
+    out = torch.empty_like(U0)
+    P.lbmk_init_from_U(g, U0.data_ptr(), True)
+    for n in (1, 2, 5):
+        P.lbmk_step(g, n)
+        P.lbmk_read_U(g, out.data_ptr(), True)
+        P.lbmk_check_subcharacteristic(g, raise_on_violation=False)
+    torch.cuda.synchronize()
+    assert bool((buf[:off] == 0xA5).all()) and bool((buf[off + nbytes:] == 0xA5).all())
+    assert bool(torch.isfinite(out).all())
+    P.lbmk_grid_destroy(g)
+    s.close()
