@@ -24,6 +24,17 @@ template <> struct Lattice<3> {
     static constexpr double w0 = 1.0 / 4.0, w1 = 1.0 / 8.0, cs2 = 1.0 / 4.0;
 };
 
+// Weights in the arithmetic type R.  The moving weight is w1 rounded to R; the rest weight is taken as 1 - 2D*w1 IN R, so
+// that the weights sum to exactly 1 in the arithmetic the kernels run in.  In fp32 on D2Q5, float(1/3) + 4*float(1/6) =
+// 1 + 3e-8: with the plainly rounded w0 every collision would multiply the (shifted) zeroth moment by 1 + omega*3e-8 -- a
+// systematic drift, linear in the step count (3e-3 of the fluctuation after 1.4e5 steps), not rounding noise.  1 - 4*w1 is
+// exact (Sterbenz), differs from 1/3 by 2e-8 (inside fp32 rounding of the oracle's value) and conserves exactly.  D3Q7's
+// 1/4, 1/8 and the fp64 path (1/3 + 4/6 == 1 in double rounding) are unaffected.
+template <int D, class R> __host__ __device__ constexpr R weight1() { return R(Lattice<D>::w1); }
+template <int D, class R> __host__ __device__ constexpr R weight0() {
+    return std::is_same<R, float>::value ? R(1) - R(2 * D) * R(Lattice<D>::w1) : R(Lattice<D>::w0);
+}
+
 __host__ __device__ constexpr int opposite(int i) { return i == 0 ? 0 : (((i - 1) ^ 1) + 1); }
 // c_i component along axis a (0 x, 1 y, 2 z)
 __host__ __device__ constexpr int cvel(int i, int a) { return (i == 0 || (i - 1) / 2 != a) ? 0 : (((i - 1) & 1) ? -1 : +1); }

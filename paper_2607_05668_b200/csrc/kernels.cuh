@@ -85,7 +85,7 @@ __device__ __forceinline__ void relax(R (&f)[2 * D + 1], R omega, R dQ, const R 
     using L = Lattice<D>;
     const R keep = R(1) - omega;
     const R A = omega * dQ + S;
-    const R a0 = R(L::w0) * A, a1 = R(L::w1) * A;
+    const R a0 = weight0<D, R>() * A, a1 = weight1<D, R>() * A;
     const R hw = R(0.5) * omega;
     f[0] = keep * f[0] + a0;
 #pragma unroll
@@ -251,7 +251,7 @@ __global__ void init_from_U_kernel(const double* __restrict__ U, R* __restrict__
         R F[D], S;
         Sys::template flux<k>(ctx, dQ, P, F, S);
         using L = Lattice<D>;
-        f[tile_off(node, M * Q) + (k * Q) * TILE] = R(L::w0) * dQ[k];
+        f[tile_off(node, M * Q) + (k * Q) * TILE] = weight0<D, R>() * dQ[k];
 #pragma unroll
         for (int a = 0; a < D; ++a) {
             const R h = R(0.5) * F[a];              // w1 / c_s^2 = 1/2
@@ -478,7 +478,7 @@ __global__ void dirichlet_frame_kernel(R* __restrict__ f, int gather, const __gr
             R F[D], S;
             Sys::template flux<k>(ctx, dQ, P, F, S);
             using L = Lattice<D>;
-            f[tile_off(node, M * Q) + (k * Q) * TILE] = R(L::w0) * dQ[k];
+            f[tile_off(node, M * Q) + (k * Q) * TILE] = weight0<D, R>() * dQ[k];
             for (int a = 0; a < D; ++a) {
                 const R h = R(0.5) * F[a];
                 const long long op = gather == GATHER_PULL ? pull_offset(1 + 2 * a, p, P.nx, P.ny, P.nz) : 0LL;

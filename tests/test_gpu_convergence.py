@@ -161,10 +161,27 @@ def test_paper_table2_eoc_reproduced_on_the_gpu(P, mk, fields):
             assert abs(slope - want) <= 0.0151, (mk.__name__, name, j, slope, want)
 
 
+def test_fp32_tracks_fp64_over_a_long_diffusive_run(P):
+    """ADR to t = 1 at N = 256 (34 493 steps at omega = 1.994) in shifted fp32 against the same run in fp64.  With the
+    plainly rounded D2Q5 weights (float(1/3) + 4 float(1/6) = 1 + 3e-8) the zeroth moment drifts linearly in the step
+    count (3e-3 at N = 512); with the rest weight taken as 1 - 4 w1 in fp32 (csrc/common.cuh weight0) it does not."""
+    res = {}
+    for prec in ("f32s", "f64"):
+        w = W.pin_adr(256, precision=prec)
+        g = P.Grid.from_workload(w)
+        g.init_from_U(w.initial_U())
+        g.step(w.steps)
+        res[prec] = g.read_U()[0]
+        g.close()
+    d = np.abs(res["f32s"] - res["f64"]).max() / np.abs(res["f64"]).max()
+    print(f"ADR N=256, 34493 steps: fp32 vs fp64 max rel diff {d:.3e}")
+    assert d < 3e-4
+
+
 @pytest.mark.parametrize("mk,field,paper_l2", [(W.pin_urf, 0, 4.7227e-06), (W.pin_maxwell, 0, 3.0632e-05)])
 def test_paper_table2_float_rows_same_magnitude(P, mk, field, paper_l2):
     """Float rows (same f, tau_R as double for these two systems, Table SM2): rounding differs between
-    implementations, so only the magnitude is gated (factor 2); the value is printed."""
+    implementations, so only the magnitude is gated (at most 2x, at least 1/4 of the printed Float value); the value is printed."""
     w = mk(512, precision="f32s")
     g = P.Grid.from_workload(w)
     g.init_from_U(w.initial_U())
@@ -172,4 +189,4 @@ def test_paper_table2_float_rows_same_magnitude(P, mk, field, paper_l2):
     l2 = g.error_norms()[field][1]
     g.close()
     print(f"{w.name} shifted fp32: rel L2 {l2:.4e} (paper Float {paper_l2:.4e})")
-    assert paper_l2 / 2 <= l2 <= paper_l2 * 2
+    assert paper_l2 / 4 <= l2 <= paper_l2 * 2
