@@ -96,10 +96,17 @@ __device__ __forceinline__ void relax(R (&f)[2 * D + 1], R omega, R dQ, const R 
     }
 }
 
+// Pointer qualifiers of the step kernels: the two-lattice modes read one buffer and write the other, so both carry
+// __restrict__ (loads may use the non-coherent path and move freely across the stores); the in-place AA modes are
+// launched with src == dst, where __restrict__ would be a false promise -- plain pointers there.
+template <class R, int MODE> struct StepPtr { using Src = const R* __restrict__; using Dst = R* __restrict__; };
+template <class R> struct StepPtr<R, 1 /*MODE_AA_EVEN*/> { using Src = const R*; using Dst = R*; };
+template <class R> struct StepPtr<R, 2 /*MODE_AA_ODD*/> { using Src = const R*; using Dst = R*; };
+
 // ------------------------------------------------------------------------------------------------ step
 template <class Sys, class R, int MODE, bool MMS, int BLOCK, int MINB>
 __global__ void __launch_bounds__(BLOCK, MINB)
-collide_stream_node(const R* __restrict__ src, R* __restrict__ dst, const __grid_constant__ KParams<R> P) {
+collide_stream_node(typename StepPtr<R, MODE>::Src src, typename StepPtr<R, MODE>::Dst dst, const __grid_constant__ KParams<R> P) {
     constexpr int D = Sys::D, Q = 2 * D + 1, M = Sys::M;
     const long long node = (long long)blockIdx.x * BLOCK + threadIdx.x;
     constexpr int NCs = MMS ? MmsNC<Sys>::value : 4;
@@ -181,7 +188,7 @@ collide_stream_node(const R* __restrict__ src, R* __restrict__ dst, const __grid
 // unchanged) and writes f'.  ~3x fewer live registers than the node kernel -> 2-3x the resident warps.
 template <class Sys, class R, int MODE, bool MMS, int BLOCK, int MINB>
 __global__ void __launch_bounds__(BLOCK, MINB)
-collide_stream_twopass(const R* __restrict__ src, R* __restrict__ dst, const __grid_constant__ KParams<R> P) {
+collide_stream_twopass(typename StepPtr<R, MODE>::Src src, typename StepPtr<R, MODE>::Dst dst, const __grid_constant__ KParams<R> P) {
     constexpr int D = Sys::D, Q = 2 * D + 1, M = Sys::M;
     using L = Lattice<D>;
     const long long node = (long long)blockIdx.x * BLOCK + threadIdx.x;
@@ -347,6 +354,9 @@ __device__ __forceinline__ double warp_max(double v) {
     for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
     return v;
 }
+// max that does not lose a blown-up state: fmax() returns the non-NaN operand, so a NaN candidate is turned into +inf
+// (which the shuffle / atomicMax-on-the-bit-pattern reductions then carry to the host, where it fails `<= c_s`).
+__device__ __forceinline__ double max_nan_inf(double m, double v) { return (v == v) ? fmax(m, v) : (double)INFINITY; }
 
 template <class Sys, class R>
 __global__ void __launch_bounds__(256)
@@ -365,9 +375,9 @@ max_wave_speed_kernel(const R* __restrict__ f, unsigned long long* __restrict__ 
             U[k] = Pd.ref[k] + s;
         }
         Sys::wave(U, Pd, w);
-        m[0] = fmax(m[0], w[0] * Pd.il);     // physical speed / lambda
-        m[1] = fmax(m[1], w[1] * Pd.il);
-        m[2] = fmax(m[2], w[2]);             // already lattice
+        m[0] = max_nan_inf(m[0], w[0] * Pd.il);     // physical speed / lambda
+        m[1] = max_nan_inf(m[1], w[1] * Pd.il);
+        m[2] = max_nan_inf(m[2], w[2]);             // already lattice
     }
     __shared__ double sm[3][8];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -423,8 +433,8 @@ error_norms_kernel(const R* __restrict__ f, double* __restrict__ out, long long 
 #pragma unroll
                 for (int i = 0; i < Q; ++i) s += (double)load_canonical<Q, R>(f, M, k, i, node, p, nx, ny, nz, gather);
                 const double e = fabs(Pd.ref[k] + s - q[k]), a = fabs(q[k]);
-                acc[k][0] += e; acc[k][1] += e * e; acc[k][2] = fmax(acc[k][2], e);
-                acc[k][3] += a; acc[k][4] += a * a; acc[k][5] = fmax(acc[k][5], a);
+                acc[k][0] += e; acc[k][1] += e * e; acc[k][2] = max_nan_inf(acc[k][2], e);
+                acc[k][3] += a; acc[k][4] += a * a; acc[k][5] = max_nan_inf(acc[k][5], a);
             }
         }
         __shared__ double sm[8];

@@ -20,3 +20,21 @@ def pytest_collection_modifyitems(config, items):
     for it in items:
         if "slow" in it.keywords:
             it.add_marker(skip)
+
+
+def pytest_sessionfinish(session, exitstatus):
+    """GPU sessions: write the per-component parity figures the A16 gate recorded (tests/parity_metric.py) to
+    gpurun_out/parity_table.{json,md} -- the folder that comes back from the GPU box."""
+    try:
+        import json
+        import parity_metric as pm
+    except Exception:
+        return
+    if not pm.ROWS:
+        return
+    out = os.path.join(ROOT, "gpurun_out")
+    os.makedirs(out, exist_ok=True)
+    with open(os.path.join(out, "parity_table.json"), "w") as fh:
+        json.dump(pm.ROWS, fh, indent=0)
+    with open(os.path.join(out, "parity_table.md"), "w") as fh:
+        fh.write(pm.table_markdown(pm.ROWS))

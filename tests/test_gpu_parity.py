@@ -24,7 +24,7 @@ def P():
     return P
 
 
-from parity_metric import rel_err, plain_rel_err, fluct_rel_err   # noqa: E402  (reading A16)
+from parity_metric import gate   # noqa: E402  (the A16 gate: SURVEY.md §8(c) A16, tests/parity_metric.py)
 
 
 def small(name, **kw):
@@ -103,9 +103,7 @@ CASES64 = [
 def test_parity_fp64(P, name, kw, steps, pattern):
     w = small(name, **kw)
     U, f, Uo, fo = run_pair(P, w, steps, precision="f64", pattern=pattern)
-    assert np.isfinite(U).all()
-    e = rel_err(U, Uo, fo)
-    assert e.max() <= TOL64, f"{w.name} U rel err {e}"
+    gate(U, Uo, fo, "f64", f"{w.name}[{pattern}]", U_ref=w.U_ref, steps=steps)
     ef = np.abs(f - fo).max() / np.abs(fo).max()
     assert ef <= TOL64, f"{w.name} populations rel err {ef}"
 
@@ -115,8 +113,7 @@ def test_parity_fp64_paper_systems_with_mms(P, mk, n, steps):
     """The three Table-2 systems (Burgers L518, Euler L519-L522, ADR L540) with their manufactured forcing."""
     w = mk(n)
     U, f, Uo, fo = run_pair(P, w, steps, precision="f64")
-    e = rel_err(U, Uo, fo)
-    assert e.max() <= TOL64, f"{w.name} {e}"
+    gate(U, Uo, fo, "f64", w.name, U_ref=w.U_ref, steps=steps)
 
 
 @pytest.mark.parametrize("name,kw,steps", [("c2", dict(n=64), 40), ("c3", dict(n=48, precision="f64"), 40),
@@ -125,8 +122,7 @@ def test_shifted_fp64_matches_unshifted_oracle(P, name, kw, steps):
     """eq (2.23) is an identity: the delta-form kernels in fp64 reproduce the plain fp64 oracle (pin P7 on the GPU)."""
     w = small(name, **kw)
     U, f, Uo, fo = run_pair(P, w, steps, precision="f64s")
-    e = rel_err(U, Uo, fo)
-    assert e.max() <= 1e-11, f"{w.name} {e}"
+    gate(U, Uo, fo, "f64s", w.name, U_ref=w.U_ref, tol=1e-11, steps=steps)
     assert np.abs(f - fo).max() / np.abs(fo).max() <= 1e-11
 
 
@@ -134,7 +130,7 @@ def test_shifted_fp64_general_reference_momentum(P):
     """Euler with a moving reference state u0 = v0 = 3 (the paper's SM5.3 fields): general delta form."""
     w = W.pin_euler(40)
     U, f, Uo, fo = run_pair(P, w, 120, precision="f64s")
-    assert rel_err(U, Uo, fo).max() <= 1e-11
+    gate(U, Uo, fo, "f64s", w.name + "[moving reference]", U_ref=w.U_ref, tol=1e-11, steps=120)
 
 
 # ------------------------------------------------------------------------------------------- shifted fp32
@@ -153,12 +149,7 @@ def test_parity_fp32_shifted(P, name, kw, steps, pattern):
     w = small(name, **kw)
     assert w.precision == "f32s"
     U, f, Uo, fo = run_pair(P, w, steps, pattern=pattern)
-    assert np.isfinite(U).all()
-    e = rel_err(U, Uo, fo)
-    assert e.max() <= TOL32, f"{w.name} U rel err {e}"
-    # stricter, reported figure: relative to the fluctuation about the reference state (A16)
-    fl, pl = fluct_rel_err(U, Uo, w.U_ref), plain_rel_err(U, Uo)
-    print(f"{w.name} [{pattern}] rel err max {e.max():.2e}; vs max|U_k| {pl.max():.2e}; fluctuation-relative {fl.max():.2e}")
+    gate(U, Uo, fo, "f32s", f"{w.name}[{pattern}]", U_ref=w.U_ref, steps=steps)
 
 
 def test_fp32_uniform_reference_state_stays_exactly_zero(P):
@@ -194,8 +185,9 @@ def _subbox_check(P, w, steps, box, origin, tol):
     m = steps
     inner = (slice(None), slice(m, bz - m) if w.dim == 3 else slice(None), slice(m, by - m), slice(m, bx - m))
     Ug = U[sl][inner]
-    e = rel_err(Ug, Uo[inner], fo[(slice(None), slice(None)) + inner[1:]])
-    assert Ug.size > 0 and e.max() <= tol, f"{w.name}: {e}"
+    assert Ug.size > 0
+    gate(Ug, Uo[inner], fo[(slice(None), slice(None)) + inner[1:]], w.precision, f"{w.name}[full size, sub-box]", U_ref=w.U_ref,
+         tol=tol, steps=steps, strict=False)       # 6-12 steps: some components have not left zero yet (parity_metric.py)
     return U
 
 
