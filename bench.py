@@ -21,9 +21,10 @@ One JSON line is printed by rank 0:
   paper_table3_systems  the paper's Table 3 systems compiled in here (4096^2, forcing off, S and D) next to the paper's
                 RTX A5000 numbers (context); skipped with --no-table3 / --no-all-configs
 
-Multi-GPU (--gpus N under torchrun): by default "replicas only" -- every rank advances its own
-full-size grid, no data-path collective; value = sum over ranks / max-over-ranks time; scaling "weak".
-`--parallelism slabs` instead cuts ONE N-times-taller periodic grid into z-slabs with a halo exchange after every step.
+Multi-GPU (--gpus N under torchrun): the path shards, so N > 1 runs SLABS by default -- ONE periodic grid
+N times taller along the slowest axis, one workload-sized slab per rank, the face-crossing populations exchanged with the
+ring neighbours after every step, overlapped with the interior update; value = node updates of all
+ranks / max-over-ranks time; scaling "weak".  `--parallelism replicas` runs N independent full-size grids instead.
 
 `--impl reference` times the oracle as it stands on host cores (rank 0 only): each step is one oracle step on a
 bounded sub-box of the same workload (same node spacing and parameters), sized so the run ends within minutes.
@@ -70,8 +71,10 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-all-configs", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--parallelism", default="replicas", choices=["replicas", "slabs"],
-                    help="N > 1: independent replicas (default) or z-slabs of one N-times-taller periodic grid with a halo exchange per step")
+    ap.add_argument("--parallelism", default="auto", choices=["auto", "replicas", "slabs"],
+                    help="auto: slabs of one N-times-taller periodic grid with an overlapped halo exchange per step when N > 1; "
+                         "replicas: N independent grids; slabs: force the slab path (also at N = 1, where the slab wraps onto itself)")
+    ap.add_argument("--no-overlap", action="store_true", help="slabs: step, pack, exchange, unpack in series (no overlap)")
     ap.add_argument("--table3", action="store_true", help="(default on) also run the paper's Table 3 systems (4096^2, forcing off, S and D)")
     ap.add_argument("--no-table3", action="store_true")
     return ap.parse_args()
@@ -196,8 +199,9 @@ def time_steps(g, torch, steps, dist=None):
 class SlabRunner:
     """This rank's slab of the global workload behind the interface run_ours uses for a Grid."""
 
-    def __init__(self, P, w_global, rank, world, dist, device):
+    def __init__(self, P, w_global, rank, world, dist, device, overlap=True):
         from paper_2607_05668_b200.slabs import HaloRing, SlabGrid
+        self.overlap = overlap
         self.slab = SlabGrid(P, w_global, rank, world, device=device)
         self.ring = HaloRing(rank, world, dist)
         self.grid = self.slab.grid
@@ -210,7 +214,7 @@ class SlabRunner:
         self.grid.init_from_U(U)
 
     def step(self, n):
-        self.slab.step(n, self.ring)
+        self.slab.step(n, self.ring, overlap=self.overlap)
 
     def read_U(self, out=None):
         return self.grid.read_U(out)
@@ -226,21 +230,31 @@ class SlabRunner:
 
 
 def short_run(P, torch, name, pattern):
-    """MLUPS / GB/s of one of the other configs (its full step count, 5% warm-up)."""
+    """MLUPS / GB/s of one of the other configs (its full step count, 5% warm-up, median of 3).  L2-resident configs run
+    launch-free (one cooperative launch per batch of steps, lbmk.h LBMK_STEPPING_PERSISTENT); the one-launch-per-step
+    figure is reported beside it."""
     w = make_workload(name)
-    g = P.Grid.from_workload(w, pattern=pattern)
-    g.init_from_U(torch.from_numpy(w.initial_U()).cuda())
-    g.step(max(10, w.steps // 20))
-    reps = []
-    for _ in range(3):
-        ms, _ = time_steps(g, torch, w.steps)
-        reps.append(ms)
-    ms = min(reps)
-    mlups = w.n_nodes * w.steps / (ms * 1e-3) / 1e6
-    out = {"workload": w.name, "dtype": "f64" if w.precision == "f64" else "f32", "pattern": g.pattern, "steps": w.steps,
-           "ms_per_step": ms / w.steps, "MLUPS": mlups, "GBps_algorithmic": mlups * w.bytes_per_node / 1e3,
-           "state_MB": w.n_nodes * w.bytes_per_node / 2 / 1e6}
-    g.close()
+    out = None
+    for stepping in ("auto", "launch"):
+        g = P.Grid.from_workload(w, pattern=pattern, stepping=stepping)
+        if stepping == "launch" and out["stepping"] == "launch":
+            g.close()
+            break
+        g.init_from_U(torch.from_numpy(w.initial_U()).cuda())
+        g.step(max(10, w.steps // 20))
+        reps, launches = [], 0
+        for _ in range(3):
+            ms, launches = time_steps(g, torch, w.steps)
+            reps.append(ms)
+        ms = statistics.median(reps)
+        mlups = w.n_nodes * w.steps / (ms * 1e-3) / 1e6
+        if out is None:
+            out = {"workload": w.name, "dtype": "f64" if w.precision == "f64" else "f32", "pattern": g.pattern,
+                   "stepping": g.stepping, "steps": w.steps, "launches": launches, "ms_per_step": ms / w.steps, "MLUPS": mlups,
+                   "GBps_algorithmic": mlups * w.bytes_per_node / 1e3, "state_MB": w.n_nodes * w.bytes_per_node / 2 / 1e6}
+        else:
+            out["one_launch_per_step"] = {"ms_per_step": ms / w.steps, "MLUPS": mlups, "launches": launches}
+        g.close()
     return out
 
 
@@ -258,6 +272,9 @@ TABLE3 = [  # (label, workload maker name, paper S (MLUPS, %), paper D (MLUPS, %
     ("incompressible-nse", "pin_inse", (2328, 95.8), (662, 54.6)),
     ("elasticity", "pin_elasticity", (2536, 89.5), (641, 45.2)),
     ("compressible-nsf", "pin_nsf2d", (1335, 94.2), (256, 36.2)),
+    ("swe-bathymetry", "pin_swe", (5093, 89.9), (958, 33.8)),        # the same Table 3 row, with the bed-slope fields read per node
+    ("resistive-mhd", "pin_mhd2d", (736, 78.0), (168, 35.7)),        # PAPER.md:L597-L598 (255 registers, spills there)
+    ("hcnsf", "hcnsf3d", (546, 63.0), (163, 37.5)),                  # PAPER.md:L599-L600, D3Q7, 256^3 here
 ]
 
 
@@ -267,18 +284,19 @@ def table3_runs(P, torch, peak, n=4096, steps=40):
     out = {}
     for label, maker, paper_s, paper_d in TABLE3:
         for prec, paper in (("f32s", paper_s), ("f64", paper_d)):
-            w = getattr(W, maker)(n, precision=prec)
+            w = getattr(W, maker)(256 if maker == "hcnsf3d" else n, precision=prec)
             w = W.relabel(w, mms_id=0, steps=steps)
             try:
                 g = P.Grid.from_workload(w)
                 g.init_from_U(torch.from_numpy(w.initial_U()).cuda())
                 g.step(5)
-                ms = min(time_steps(g, torch, steps)[0] for _ in range(3))
+                ms = statistics.median(time_steps(g, torch, steps)[0] for _ in range(3))
                 g.close()
                 mlups = w.n_nodes * steps / (ms * 1e-3) / 1e6
                 gbs = mlups * w.bytes_per_node / 1e3
                 out[f"{label}:{'S' if prec == 'f32s' else 'D'}"] = {
-                    "m_total": w.m_total, "bytes_per_node": w.bytes_per_node, "grid": [n, n], "MLUPS": mlups, "GBps_algorithmic": gbs,
+                    "m_total": w.m_total, "n_prescribed_fields": w.n_aux, "bytes_per_node": w.bytes_per_node, "grid": [w.nx, w.ny, w.nz],
+                    "MLUPS": mlups, "GBps_algorithmic": gbs,
                     "frac_of_measured_peak": gbs / peak, "paper_A5000_MLUPS": paper[0], "paper_pct_of_680GBps": paper[1]}
             except Exception as e:   # reported, never hidden
                 out[f"{label}:{'S' if prec == 'f32s' else 'D'}"] = {"error": repr(e)}
@@ -384,12 +402,12 @@ def run_ours(args):
     steps = args.steps if args.steps is not None else min(w.steps, 200)
     warm = max(args.warmup, 3)
     dev = f"cuda:{local}"
-    slabs = args.parallelism == "slabs"
+    slabs = args.parallelism == "slabs" or (args.parallelism == "auto" and world > 1)
     if slabs:
         import workloads as W
         # weak scaling: one periodic grid `world` times taller along the slab axis, this rank owns one workload-sized slab
         wg = W.relabel(w, **({"nz": w.nz * world} if w.dim == 3 else {"ny": w.ny * world}))
-        g = SlabRunner(P, wg, rank, world, dist, dev)
+        g = SlabRunner(P, wg, rank, world, dist, dev, overlap=not args.no_overlap)
         own_nodes, U0 = g.own_nodes, g.w.initial_U()
     else:
         own_nodes, U0 = w.n_nodes, w.initial_U()
@@ -472,12 +490,18 @@ def run_ours(args):
                    "grid": [w.nx, w.ny, w.nz], "precision": w.precision, "mms_forcing": bool(w.mms_id),
                    "pattern": pattern, "kernel": kernel, "bytes_per_node": w.bytes_per_node,
                    "l2": "state larger than L2 (no flush needed)" if bytes_per_launch / 2 > 2.5e8 else "state fits in L2: HBM roofline n/a",
-                   "parallelism": ("z-slabs, halo exchange per step" if slabs else "replicas only") if (world > 1 or slabs) else "single GPU", "timing": f"median of {n_rep} x {steps} steps, CUDA events",
+                   "parallelism": (("slabs along the slowest axis, halo exchange per step" + (" overlapped with the interior update" if not args.no_overlap else ", serial"))
+                                   if slabs else "replicas only") if (world > 1 or slabs) else "single GPU", "timing": f"median of {n_rep} x {steps} steps, CUDA events",
                    "lattice_wave_speed": max(speeds[0], speeds[1]) + speeds[2], "finite": finite},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": traffic, "peak_source": peak_src, "frac_of_nominal_8TBps": achieved / 8000.0,
+                     "traffic": traffic,
+                     "traffic_source": ("constant from profiles/traffic_per_launch.json: dram__bytes_read.sum + dram__bytes_write.sum of one "
+                                        "`ncu --set full` capture of this kernel and launch configuration (profiles/), NOT measured by this run")
+                                       if traffic is not None else None,
+                     "peak_source": peak_src, "frac_of_nominal_8TBps": achieved / 8000.0,
                      "kernel": "collide_stream (one launch per step)", "algorithmic_bytes_per_launch": bytes_per_launch,
-                     "lbmk_copy_probe_GBps": probe},
+                     "lbmk_copy_probe_GBps": probe,
+                     "frac_of_max_measured_copy": achieved / max(peak, probe) if isinstance(probe, float) else None},
         "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
     }
     line["config"].pop("m_conserved")

@@ -73,19 +73,33 @@ typedef enum { LBMK_PERIODIC = 0, LBMK_DIRICHLET_MMS = 1 } lbmk_bc;
  *   ELASTICITY2D {rho0, mu_s, lambda_s} neo-Hookean finite-strain elasticity, eq 3.13-3.15 L402-L414  m = 6 (F, rho0 v)
  *   NSF2D        {gamma, mu, K}        compressible NSF 2D, eq 3.23-3.24, cascade on the conserved fields  m = 4 + 8
  *   MAXWELL2D    {c}                   Maxwell TM mode, eq 3.10-3.11 L385-L391                 m = 3 (E_z, H_x, H_y)
- * Trackers are carried in lattice units G^L = dx grad V. */
+ *   SWE2D_BATHY  {g}                   eq 3.5-3.6 L351-L359 with the bed source -g h grad z_b  m = 3; 2 prescribed fields (d_x z_b, d_y z_b)
+ *   HCNSF3D      {gamma, mu, kappa, eta_drag}  homogenized NSF, eq 3.27, trackers sym grad u (6: 00 11 22 01 02 12),
+ *                                      grad T (3)                                              m = 5 + 9; 4 prescribed fields (alpha, u_s x3)
+ *   MHD2D        {gamma, mu, K, eta}   resistive MHD 2D with Powell source, eq 3.25, cascade on the 6 conserved
+ *                                      fields (rho, m0, m1, E, B0, B1)                          m = 6 + 12
+ * Trackers are carried in lattice units G^L = dx grad V.
+ * Prescribed coefficient fields ("prescribed external coefficient fields [that] enter the dynamics without being functions
+ * of the evolved state") are per-node inputs set with lbmk_set_aux_fields. */
 typedef enum {
     LBMK_SYS_ADVECTION2D = 0, LBMK_SYS_BURGERS2D = 1, LBMK_SYS_SWE2D = 2, LBMK_SYS_EULER2D = 3,
     LBMK_SYS_ADR2D = 4, LBMK_SYS_NSF3D_GRADTRACK = 5, LBMK_SYS_MHD3D_JTRACK = 6, LBMK_SYS_URF2D = 7,
     LBMK_SYS_MAXWELL2D = 8, LBMK_SYS_ALLENCAHN2D = 9, LBMK_SYS_INSE2D = 10,
-    LBMK_SYS_ELASTICITY2D = 11, LBMK_SYS_NSF2D_GRADTRACK = 12, LBMK_SYS_COUNT = 13
+    LBMK_SYS_ELASTICITY2D = 11, LBMK_SYS_NSF2D_GRADTRACK = 12, LBMK_SYS_SWE2D_BATHY = 13, LBMK_SYS_HCNSF3D = 14,
+    LBMK_SYS_MHD2D = 15, LBMK_SYS_COUNT = 16
 } lbmk_system_id;
 
 /* Grid options (lbmk_grid_set_option, before lbmk_grid_workspace_bytes / bind). */
 typedef enum {
     LBMK_OPT_PATTERN = 0,   /* streaming pattern: LBMK_PATTERN_* ; default chosen per config by measurement */
-    LBMK_OPT_KERNEL = 1     /* kernel variant: LBMK_KERNEL_* */
+    LBMK_OPT_KERNEL = 1,    /* kernel variant: LBMK_KERNEL_* */
+    LBMK_OPT_STEPPING = 2   /* how lbmk_step(n) issues its n steps: LBMK_STEPPING_* */
 } lbmk_option;
+/* LBMK_STEPPING_LAUNCH: one kernel launch per step.  LBMK_STEPPING_PERSISTENT: one cooperative launch advances a whole batch
+ * of steps (all blocks co-resident, a grid-wide barrier between steps) -- for grids whose populations live in L2 and whose
+ * step is therefore launch-latency bound (SURVEY.md section 7 "Small configs"); two-lattice pull, periodic, node kernel only,
+ * bit-identical to the per-launch path.  AUTO picks PERSISTENT when both population copies fit in 96 MB. */
+enum { LBMK_STEPPING_AUTO = 0, LBMK_STEPPING_LAUNCH = 1, LBMK_STEPPING_PERSISTENT = 2 };
 enum { LBMK_PATTERN_AUTO = 0, LBMK_PATTERN_PULL2 = 1 /* two-lattice pull */, LBMK_PATTERN_AA = 2 /* in-place */ };
 enum { LBMK_KERNEL_AUTO = 0, LBMK_KERNEL_NODE = 1 /* one node per thread, direct loads */,
        LBMK_KERNEL_ROW = 2 /* reserved: shared-memory / TMA staged x-rows; not built (direct loads already move exactly the
@@ -103,6 +117,8 @@ lbmk_status lbmk_system_create(lbmk_system_id id, lbmk_lattice lattice, const do
                                lbmk_system** out);
 /* m_conserved, m_total (= conserved + tracker components), spatial dimension, Q.  Any out pointer may be NULL. */
 lbmk_status lbmk_system_info(const lbmk_system* sys, int* m_conserved, int* m_total, int* dim, int* Q);
+/* Number of prescribed per-node coefficient fields of the system (0 for most). */
+lbmk_status lbmk_system_aux_count(const lbmk_system* sys, int* n_aux);
 /* Relaxation: conserved fields tau_k = 1/2 + tau_R[k]*dt; n = 1 (same for all) or
  * m_conserved.  Tracker fields relax at omega = 1/(g_tau+1) and use tau_grad = g_tau*dt in their flux and
  * source.  g_tau is ignored by tracker-free systems. */
@@ -118,7 +134,8 @@ lbmk_status lbmk_system_set_reference(lbmk_system* sys, const double* U0, int n)
  *   BURGERS2D {A};  EULER2D {};  SWE2D {A_h, A_u, h0};  ADR2D {};  NSF3D {U0, A_rho, rho0, p0};
  *   URF2D {} (eq SM5.4);  MAXWELL2D {} (eq SM5.5);  ALLENCAHN2D {} (eq SM5.8);
  *   INSE2D {U, rho0} (eq SM5.9);  ELASTICITY2D {} (eq SM5.6);
- *   NSF2D {} (eq SM5.10). */
+ *   NSF2D {} (eq SM5.10);  SWE2D_BATHY {h0, A_h, m0, A_m, A_zb, w_t} (eq SM5.3, bed L1198; w_t = frequency of the time factors);
+ *   MHD2D {} (SM5.12 L1375-L1392).  HCNSF3D has none compiled in (its exact fields are truncated in the source, L1457). */
 lbmk_status lbmk_system_set_mms(lbmk_system* sys, int mms_id, const double* mms_params, int n);
 /* A-priori bound on the physical wave speed max|eig sum n_a A_a| from the declared amplitudes (eq 2.20).
  * lbmk_grid_create rejects the grid with LBMK_ESUBCHAR if s_max/lambda > c_s.  0 = no declared bound. */
@@ -132,6 +149,7 @@ void lbmk_system_destroy(lbmk_system* sys);
  * the grid.  cuda_stream: a cudaStream_t.  With LBMK_DIRICHLET_MMS the outermost node layer is reset to
  * f_eq(Q_exact(x_b, t_n)) before every step and before readback (needs mms_id != 0; the paper defines no
  * boundary operator, PAPER.md:L504, L608 -- DESIGN.md reading A18). */
+/* nx*ny*nz must be < 2^31 nodes (LBMK_EINVAL otherwise): node indices are 32-bit inside the kernels. */
 lbmk_status lbmk_grid_create(const lbmk_system* sys, int nx, int ny, int nz, lbmk_bc bc, double dx, double lambda,
                              lbmk_precision precision, void* cuda_stream, lbmk_grid** out);
 lbmk_status lbmk_grid_set_option(lbmk_grid* g, lbmk_option key, long long value);
@@ -161,12 +179,31 @@ lbmk_status lbmk_grid_set_slab(lbmk_grid* g, int enable);
 lbmk_status lbmk_halo_bytes(const lbmk_grid* g, size_t* bytes);
 lbmk_status lbmk_halo_pack(lbmk_grid* g, void* send_lo, void* send_hi);
 lbmk_status lbmk_halo_unpack(lbmk_grid* g, const void* recv_lo, const void* recv_hi);
+/* The same on another stream (a cudaStream_t; NULL = the grid's stream), so that the exchange can run beside the interior update. */
+lbmk_status lbmk_halo_pack_on(lbmk_grid* g, void* send_lo, void* send_hi, void* cuda_stream);
+lbmk_status lbmk_halo_unpack_on(lbmk_grid* g, const void* recv_lo, const void* recv_hi, void* cuda_stream);
+/* Overlapped slab step (the exchange "overlapped with the interior update"):
+ *   lbmk_step_slab(g)                     one step in three launches on the grid's stream: first own plane, last own plane,
+ *                                         [boundary event], interior planes; ghost planes are not updated
+ *   lbmk_stream_wait_boundary(g, s)       stream s waits for that boundary event (then: lbmk_halo_pack_on(.., s), transport,
+ *                                         lbmk_halo_unpack_on(.., s) while the interior launch runs on the grid's stream)
+ *   lbmk_grid_wait_stream(g, s)           the grid's stream waits for everything enqueued on s so far (before the next step).
+ * The result equals lbmk_step(g, 1) + pack/transport/unpack bit for bit. */
+lbmk_status lbmk_step_slab(lbmk_grid* g);
+lbmk_status lbmk_stream_wait_boundary(lbmk_grid* g, void* cuda_stream);
+lbmk_status lbmk_grid_wait_stream(lbmk_grid* g, void* cuda_stream);
 
 /* ---- initialise from U, step, read back U ------------------------------------------------------------ */
 
 /* Step 0: all populations, conserved and tracker, at the (shifted) equilibrium of
  * U [m_total][nz][ny][nx] (fp64).  Sets step = 0, t = t0. */
 lbmk_status lbmk_init_from_U(lbmk_grid* g, const double* U, int on_device, double t0);
+/* Prescribed coefficient fields A [n_aux][nz][ny][nx] (fp64; stored in the grid's arithmetic type): SWE2D_BATHY the bed
+ * slope (d_x z_b, d_y z_b) (eq 3.5); HCNSF3D the porosity and solid velocity (alpha, u_s) (eq 3.27).
+ * Used by every later step until replaced (time-dependent fields: call again between steps; the paper takes explicit
+ * (x, t) dependence at t_n + dt/2, L154).  Must be called before lbmk_init_from_U for systems with n_aux > 0
+ * (LBMK_ESTATE otherwise); LBMK_EUNSUPPORTED for systems without.  Asynchronous for device pointers. */
+lbmk_status lbmk_set_aux_fields(lbmk_grid* g, const double* A, int on_device);
 /* Sets the populations directly (canonical layout below, fp64; stored as given minus the shift). */
 lbmk_status lbmk_set_populations(lbmk_grid* g, const double* f, int on_device, double t0);
 /* n_steps fused collide-and-stream steps (eq 2.11), asynchronous on the grid's stream. */

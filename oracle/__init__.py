@@ -16,7 +16,8 @@ import numpy as np
 from . import build as _build
 
 MAXM = 32
-SYSTEM_ID = {"advection2d": 0, "burgers2d": 1, "swe2d": 2, "euler2d": 3, "adr2d": 4, "nsf3d": 5, "mhd3d": 6, "urf2d": 7, "maxwell2d": 8, "allencahn2d": 9, "inse2d": 10, "elasticity2d": 11, "nsf2d": 12}
+SYSTEM_ID = {"advection2d": 0, "burgers2d": 1, "swe2d": 2, "euler2d": 3, "adr2d": 4, "nsf3d": 5, "mhd3d": 6, "urf2d": 7, "maxwell2d": 8, "allencahn2d": 9, "inse2d": 10, "elasticity2d": 11, "nsf2d": 12,
+             "swe2d_bathy": 13, "hcnsf3d": 14, "mhd2d": 15}
 
 
 class _Spec(C.Structure):
@@ -47,7 +48,8 @@ def lib():
             "orc_step": [C.c_void_p, C.c_int], "orc_read_f": [C.c_void_p, dp], "orc_read_U": [C.c_void_p, dp],
             "orc_time": [C.c_void_p, C.POINTER(C.c_int64), dp], "orc_omega": [C.c_void_p, dp],
             "orc_exact_U": [C.c_void_p, C.c_double, dp],
-            "orc_flux_source": [C.c_void_p, dp, dp, dp], "orc_equilibrium": [C.c_void_p, dp, dp, dp],
+            "orc_flux_source": [C.c_void_p, dp, dp, dp, dp], "orc_set_aux": [C.c_void_p, dp],
+            "orc_system_n_aux": [C.c_int], "orc_equilibrium": [C.c_void_p, dp, dp, dp],
             "orc_mms_source": [C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_double, dp],
             "orc_exact_point": [C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_double, dp],
             "orc_max_wave_speed": [C.c_void_p, dp],
@@ -99,6 +101,7 @@ class OracleGrid:
         self.system = system
         self.m_conserved, self.m_total, self.dim, self.Q = system_info(system)
         self.nx, self.ny, self.nz = nx, ny, nz
+        self.n_aux = lib().orc_system_n_aux(SYSTEM_ID[system])
         s = _Spec()
         s.system = SYSTEM_ID[system]
         s.nx, s.ny, s.nz = nx, ny, nz
@@ -161,6 +164,12 @@ class OracleGrid:
         assert U.shape == self.shape_U
         assert lib().orc_init_from_U(self._h, _dp(U)) == 0
 
+    def set_aux(self, A: np.ndarray):
+        """Prescribed coefficient fields A[n_aux][nz][ny][nx] (bed slope; porosity and solid velocity)."""
+        A = np.ascontiguousarray(A, dtype=np.float64)
+        assert A.shape == (self.n_aux, self.nz, self.ny, self.nx)
+        assert lib().orc_set_aux(self._h, _dp(A)) == 0
+
     def set_f(self, f: np.ndarray):
         f = np.ascontiguousarray(f, dtype=np.float64)
         assert f.shape == self.shape_f
@@ -197,11 +206,12 @@ class OracleGrid:
             raise ValueError("no manufactured solution for this (system, mms_id)")
         return U
 
-    def flux_source(self, U: Sequence[float]):
+    def flux_source(self, U: Sequence[float], A: Optional[Sequence[float]] = None):
         U = np.ascontiguousarray(U, dtype=np.float64)
         F = np.zeros((self.m_total, 3))
         S = np.zeros(self.m_total)
-        lib().orc_flux_source(self._h, _dp(U), _dp(F), _dp(S))
+        Aa = np.zeros(max(self.n_aux, 1)) if A is None else np.ascontiguousarray(A, dtype=np.float64)
+        lib().orc_flux_source(self._h, _dp(U), _dp(Aa), _dp(F), _dp(S))
         return F, S
 
     def equilibrium(self, U, F) -> np.ndarray:
@@ -237,6 +247,8 @@ class OracleGrid:
 def run(w, steps: Optional[int] = None, U0: Optional[np.ndarray] = None, **kw) -> np.ndarray:
     """Initialise from the workload's U(x,0), step, read back U."""
     g = OracleGrid.from_workload(w, **kw)
+    if g.n_aux:
+        g.set_aux(w.aux_fields())
     g.init_from_U(w.initial_U() if U0 is None else U0)
     g.step(w.steps if steps is None else steps)
     U = g.read_U()

@@ -78,11 +78,17 @@ struct Grid {
     double omega[MAXM];
     double F_ref[MAXM * 3];
     std::vector<double> f, g;  // f[(k*Q + i)*n + node]
+    std::vector<double> aux;   // prescribed coefficient fields aux[a*n + node] (n_aux per system; zeros until orc_set_aux)
     bool inited;
 };
 
 static inline int64_t node_index(const Grid& G, int x, int y, int z) { return ((int64_t)z * G.s.ny + y) * G.s.nx + x; }
 static inline int wrap(int a, int n) { return ((a % n) + n) % n; }
+
+// the prescribed coefficient fields of one node (nullptr-safe: systems without aux never read A)
+static inline void node_aux(const Grid& G, int64_t nd, double* A) {
+    for (int a = 0; a < G.si.n_aux; ++a) A[a] = G.aux[(int64_t)a * G.n + nd];
+}
 
 static void coords(const Grid& G, int x, int y, int z, double* X) {
     X[0] = (x + G.s.ox) * G.s.dx;
@@ -122,11 +128,12 @@ static void fill_frame(Grid& G, double t) {
                 coords(G, x, y, z, X);
                 J1 Qe[MAXM];
                 exact_state(G.s.system, G.s.mms_id, G.sc, G.s.mms_par, t, X[0], X[1], X[2], Qe);
-                double U[MAXM], F[MAXM * 3], S[MAXM], feq[MAXM * 7];
+                double U[MAXM], F[MAXM * 3], S[MAXM], feq[MAXM * 7], A[8];
                 for (int k = 0; k < m; ++k) U[k] = Qe[k].v;
-                flux_source<double>(G.s.system, U, G.sc, F, S);
-                equilibrium(G, U, F, feq);
                 const int64_t nd = node_index(G, x, y, z);
+                node_aux(G, nd, A);
+                flux_source<double>(G.s.system, U, A, G.sc, F, S);
+                equilibrium(G, U, F, feq);
                 for (int q = 0; q < m * Q; ++q) G.f[(int64_t)q * G.n + nd] = feq[q];
             }
 }
@@ -141,7 +148,7 @@ static void one_step(Grid& G) {
         for (int y = 0; y < G.s.ny; ++y)
             for (int x = 0; x < G.s.nx; ++x) {
                 const int64_t nd = node_index(G, x, y, z);
-                double U[MAXM], F[MAXM * 3], S[MAXM], feq[MAXM * 7];
+                double U[MAXM], F[MAXM * 3], S[MAXM], feq[MAXM * 7], A[8];
                 // 1a. zeroth moments, eq (2.6)
                 for (int k = 0; k < m; ++k) {
                     double s = 0.0;
@@ -149,7 +156,8 @@ static void one_step(Grid& G) {
                     U[k] = G.s.shifted ? G.s.U_ref[k] + s : s;
                 }
                 // 1b. flux and state source at the current moments; explicit forcing at the midpoint
-                flux_source<double>(G.s.system, U, G.sc, F, S);
+                node_aux(G, nd, A);     // prescribed coefficient fields as last set by orc_set_aux
+                flux_source<double>(G.s.system, U, A, G.sc, F, S);
                 if (G.s.mms_id != 0) {
                     double X[3], sm[MAXM];
                     coords(G, x, y, z, X);
@@ -182,6 +190,7 @@ int orc_system_info(int sys, int* m_conserved, int* m_total, int* dim, int* Q) {
     *m_conserved = si.m_conserved; *m_total = si.m_total; *dim = si.dim; *Q = 2 * si.dim + 1;
     return 0;
 }
+int orc_system_n_aux(int sys) { return (sys < 0 || sys >= SYS_COUNT) ? -1 : sys_info(sys).n_aux; }
 
 int orc_lattice(int dim, int* c /*[Q][3]*/, double* w /*[Q]*/, double* cs2) {
     if (dim != 2 && dim != 3) return 1;
@@ -212,8 +221,13 @@ void* orc_create(const Spec* sp) {
     {   // F0 = F(Q0) for the shifted storage, eq (2.23)
         double S[MAXM];
         for (int q = 0; q < MAXM * 3; ++q) G->F_ref[q] = 0.0;
-        if (sp->shifted) flux_source<double>(sp->system, G->s.U_ref, G->sc, G->F_ref, S);
+        // prescribed fields at the reference state: alpha = 1 (pure fluid), everything else 0 (they multiply terms that
+        // vanish at a uniform reference with zero trackers)
+        double A0[8] = {1.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+        if (G->si.n_aux > 0 && sp->system != SYS_HCNSF3D) A0[0] = 0.0;
+        if (sp->shifted) flux_source<double>(sp->system, G->s.U_ref, A0, G->sc, G->F_ref, S);
     }
+    G->aux.assign((size_t)G->si.n_aux * G->n, 0.0);
     G->f.assign((size_t)G->si.m_total * G->L.Q * G->n, 0.0);
     G->g.assign((size_t)G->si.m_total * G->L.Q * G->n, 0.0);
 #ifdef _OPENMP
@@ -238,14 +252,24 @@ int orc_init_from_U(void* h, const double* U_in /*[m][nz][ny][nx]*/) {
     const int m = G.si.m_total, Q = G.L.Q;
 #pragma omp parallel for schedule(static)
     for (int64_t nd = 0; nd < G.n; ++nd) {
-        double U[MAXM], F[MAXM * 3], S[MAXM], feq[MAXM * 7];
+        double U[MAXM], F[MAXM * 3], S[MAXM], feq[MAXM * 7], A[8];
         for (int k = 0; k < m; ++k) U[k] = U_in[(int64_t)k * G.n + nd];
-        flux_source<double>(G.s.system, U, G.sc, F, S);
+        node_aux(G, nd, A);
+        flux_source<double>(G.s.system, U, A, G.sc, F, S);
         equilibrium(G, U, F, feq);
         for (int q = 0; q < m * Q; ++q) G.f[(int64_t)q * G.n + nd] = feq[q];
     }
     G.step = 0;
     G.inited = true;
+    return 0;
+}
+
+// prescribed coefficient fields A[a][nz][ny][nx] (bed slope of eq 3.5): used by every later flux/source
+// evaluation until replaced (time-dependent fields: call again between steps)
+int orc_set_aux(void* h, const double* A_in) {
+    Grid& G = *(Grid*)h;
+    if (G.si.n_aux == 0) return 1;
+    std::memcpy(G.aux.data(), A_in, G.aux.size() * sizeof(double));
     return 0;
 }
 
@@ -316,9 +340,10 @@ int orc_exact_U(void* h, double t, double* U_out) {
 }
 
 // pointwise hooks for the pins ------------------------------------------------------------------
-int orc_flux_source(void* h, const double* U, double* F /*[m][3]*/, double* S /*[m]*/) {
+int orc_flux_source(void* h, const double* U, const double* A /*[n_aux] or NULL*/, double* F /*[m][3]*/, double* S /*[m]*/) {
     Grid& G = *(Grid*)h;
-    flux_source<double>(G.s.system, U, G.sc, F, S);
+    double A0[8] = {0};
+    flux_source<double>(G.s.system, U, A ? A : A0, G.sc, F, S);
     return 0;
 }
 int orc_equilibrium(void* h, const double* U, const double* F, double* feq /*[m][Q]*/) {

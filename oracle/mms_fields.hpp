@@ -14,6 +14,8 @@
 //   inse2d    mms 1 : eq (SM5.9), PAPER.md:L1330-L1334 (Taylor-Green vortex), mms_par = {U, rho0}
 //   elasticity2d mms 1 : eq (SM5.6)
 //   nsf2d     mms 1 : eq (SM5.10)
+//   swe2d_bathy mms 1 : eq (SM5.3), PAPER.md:L1200-L1207 with the static bed z_b of L1198
+//   mhd2d     mms 1 : SM5.12 text
 //   maxwell2d mms 1 : eq (SM5.5), PAPER.md:L1248-L1254 (k_x = 2 pi, k_y = 4 pi, A = 1/2, omega = 4)
 #pragma once
 #include "jets.hpp"
@@ -134,6 +136,34 @@ inline bool exact_state(int sys, int mms_id, const Scaling& sc, const double* mp
         }
         return true;
     }
+    case SYS_SWE2D_BATHY: {
+        // eq (SM5.3): h = h0 + A_h sin sin cos t, hu0 = m0 + A_m cos cos sin t, hu1 = m0 + A_m sin sin sin t;
+        // mp = {h0, A_h, m0, A_m, A_zb, w} (paper: 0.1, 0.04, 0.03, 0.02, 0.01 before non-dimensionalisation; w = frequency of
+        // the time factors in the non-dimensional time, A25)
+        const double h0 = mp[0], Ah = mp[1], m0 = mp[2], Am = mp[3], w = mp[5];
+        Q[0] = lower(h0 + Ah * sin(k * x) * sin(k * y) * cos(w * t));
+        Q[1] = lower(m0 + Am * cos(k * x) * cos(k * y) * sin(w * t));
+        Q[2] = lower(m0 + Am * sin(k * x) * sin(k * y) * sin(w * t));
+        return true;
+    }
+    case SYS_MHD2D: {
+        // eq (SM5.12 text), non-dimensional rho0 = c_s = 1 (reading A9): u0 = v0 = 3, B0 = 0.5, p0 = 1/gamma
+        const double gamma = sc.par[0], p0 = 1.0 / gamma;
+        J2 drho = 0.3 * sin(k * x) * cos(k * y) * cos(t);
+        J2 rho = 1.0 + drho;
+        J2 p = p0 + drho + (0.2 * p0) * cos(k * x) * sin(k * y) * sin(t);
+        J2 u = 3.0 + 0.3 * cos(k * x) * sin(k * y) * sin(t);
+        J2 v = 3.0 + 0.3 * sin(k * x) * sin(k * y) * sin(t);
+        J2 Bx = 0.5 - 0.3 * cos(k * x) * sin(k * y) * sin(t);
+        J2 By = 0.5 + 0.3 * sin(k * x) * cos(k * y) * sin(t);
+        J2 V[6] = {rho, rho * u, rho * v, p / (gamma - 1.0) + 0.5 * rho * (u * u + v * v) + 0.5 * (Bx * Bx + By * By), Bx, By};
+        for (int q = 0; q < 6; ++q) {
+            Q[q] = lower(V[q]);
+            Q[6 + 2 * q + 0] = sc.dx * diff(V[q], 1);
+            Q[6 + 2 * q + 1] = sc.dx * diff(V[q], 2);
+        }
+        return true;
+    }
     case SYS_MAXWELL2D: {
         const double A = 0.5, kx = 2.0 * PI, ky = 4.0 * PI, om = 4.0;
         Q[0] = lower(A * sin(kx * x) * sin(ky * y) * cos(om * t));
@@ -145,14 +175,28 @@ inline bool exact_state(int sys, int mms_id, const Scaling& sc, const double* mp
     return false;
 }
 
+// Prescribed coefficient fields of the manufactured cases, as jets (their gradients enter where the flux holds them).
+inline void exact_aux(int sys, const Scaling& sc, const double* mp, double t_, double x_, double y_, double z_, J1* A) {
+    (void)sc; (void)t_; (void)z_;
+    const J2 x = J2::variable(1, x_), y = J2::variable(2, y_);
+    const double k = 2.0 * PI;
+    if (sys == SYS_SWE2D_BATHY) {
+        // static bathymetry z_b = A_zb sin(2 pi x0) cos(2 pi x1); the field handed to the scheme is its slope
+        J2 zb = mp[4] * sin(k * x) * cos(k * y);
+        A[0] = diff(zb, 1);
+        A[1] = diff(zb, 2);
+    }
+}
+
 // Lattice manufactured source at one point:
 //   s_mms[k] = dt * d_t Q_k + dx * sum_a d_a F_k,a(Q_exact) - S_k(Q_exact)      (eq 4.1 in lattice units;
 //   F = (dt/dx) Phi and S = dt * S_phys, so this is dt * [d_t Q + div Phi - S_phys].)
 inline bool mms_source(int sys, int mms_id, const Scaling& sc, const double* mp,
                        double t, double x, double y, double z, double* s_mms) {
-    J1 Q[MAXM], F[MAXM * 3], S[MAXM];
+    J1 Q[MAXM], F[MAXM * 3], S[MAXM], A[8];
     if (!exact_state(sys, mms_id, sc, mp, t, x, y, z, Q)) return false;
-    flux_source<J1>(sys, Q, sc, F, S);
+    exact_aux(sys, sc, mp, t, x, y, z, A);
+    flux_source<J1>(sys, Q, A, sc, F, S);
     const int m = sys_info(sys).m_total;
     for (int k = 0; k < m; ++k)
         s_mms[k] = sc.dt * Q[k].d[0] + sc.dx * (F[k * 3 + 0].d[1] + F[k * 3 + 1].d[2] + F[k * 3 + 2].d[3]) - S[k].v;

@@ -17,28 +17,34 @@
 namespace orc {
 
 enum SystemId { SYS_ADVECTION2D = 0, SYS_BURGERS2D = 1, SYS_SWE2D = 2, SYS_EULER2D = 3, SYS_ADR2D = 4,
-                SYS_NSF3D = 5, SYS_MHD3D = 6, SYS_URF2D = 7, SYS_MAXWELL2D = 8, SYS_ALLENCAHN2D = 9, SYS_INSE2D = 10, SYS_ELASTICITY2D = 11, SYS_NSF2D = 12, SYS_COUNT = 13 };
+                SYS_NSF3D = 5, SYS_MHD3D = 6, SYS_URF2D = 7, SYS_MAXWELL2D = 8, SYS_ALLENCAHN2D = 9, SYS_INSE2D = 10, SYS_ELASTICITY2D = 11, SYS_NSF2D = 12,
+                SYS_SWE2D_BATHY = 13, SYS_HCNSF3D = 14, SYS_MHD2D = 15, SYS_COUNT = 16 };
 
 constexpr int MAXM = 32;  // max components
 
-struct SysInfo { int m_conserved, m_total, dim; };
+// n_aux = number of PRESCRIBED per-node coefficient fields A_a(x[, t]) that enter flux/source without being functions of the
+// evolved state ("prescribed external coefficient fields"; the static bathymetry of eq 3.5).
+struct SysInfo { int m_conserved, m_total, dim, n_aux; };
 inline SysInfo sys_info(int sys) {
     switch (sys) {
-        case SYS_ADVECTION2D: return {1, 1, 2};
-        case SYS_BURGERS2D:   return {1, 1, 2};
-        case SYS_SWE2D:       return {3, 3, 2};
-        case SYS_EULER2D:     return {4, 4, 2};
-        case SYS_ADR2D:       return {1, 3, 2};
-        case SYS_NSF3D:       return {5, 17, 3};
-        case SYS_MHD3D:       return {8, 11, 3};
-        case SYS_URF2D:       return {3, 3, 2};
-        case SYS_MAXWELL2D:   return {3, 3, 2};
-        case SYS_ALLENCAHN2D: return {1, 3, 2};
-        case SYS_INSE2D:      return {3, 7, 2};
-        case SYS_ELASTICITY2D: return {6, 6, 2};
-        case SYS_NSF2D:       return {4, 12, 2};
+        case SYS_ADVECTION2D: return {1, 1, 2, 0};
+        case SYS_BURGERS2D:   return {1, 1, 2, 0};
+        case SYS_SWE2D:       return {3, 3, 2, 0};
+        case SYS_EULER2D:     return {4, 4, 2, 0};
+        case SYS_ADR2D:       return {1, 3, 2, 0};
+        case SYS_NSF3D:       return {5, 17, 3, 0};
+        case SYS_MHD3D:       return {8, 11, 3, 0};
+        case SYS_URF2D:       return {3, 3, 2, 0};
+        case SYS_MAXWELL2D:   return {3, 3, 2, 0};
+        case SYS_ALLENCAHN2D: return {1, 3, 2, 0};
+        case SYS_INSE2D:      return {3, 7, 2, 0};
+        case SYS_ELASTICITY2D: return {6, 6, 2, 0};
+        case SYS_NSF2D:       return {4, 12, 2, 0};
+        case SYS_SWE2D_BATHY: return {3, 3, 2, 2};     // aux: d_x z_b, d_y z_b (physical bed slope)
+        case SYS_HCNSF3D:     return {5, 14, 3, 4};    // aux: alpha, u_s (3)
+        case SYS_MHD2D:       return {6, 18, 2, 0};
     }
-    return {0, 0, 0};
+    return {0, 0, 0, 0};
 }
 
 struct Scaling {
@@ -47,9 +53,9 @@ struct Scaling {
     double g_tau;       // tracker step count, tau_grad = g_tau * dt
 };
 
-// F[k*3 + a], S[k]
+// F[k*3 + a], S[k];  A[n_aux] = the prescribed coefficient fields at this node (nullptr if the system has none)
 template <class T>
-void flux_source(int sys, const T* U, const Scaling& sc, T* F, T* S) {
+void flux_source(int sys, const T* U, const T* A, const Scaling& sc, T* F, T* S) {
     const double il = 1.0 / sc.lam;           // dt/dx
     const double dL = sc.dt / (sc.dx * sc.dx); // physical diffusivity -> lattice diffusivity
     const SysInfo si = sys_info(sys);
@@ -287,6 +293,129 @@ void flux_source(int sys, const T* U, const Scaling& sc, T* F, T* S) {
         }
         for (int q = 0; q < 8; ++q) S[4 + q] = -G[q] / sc.g_tau;
     } break;
+    case SYS_SWE2D_BATHY: {
+        // shallow water over a static bed z_b(x), eq (3.5)-(3.6): the SWE flux plus the source
+        // S = (0, -g h grad z_b).  A = (d_x z_b, d_y z_b) is the prescribed per-node bed slope (physical units); par = {g}
+        const double g = sc.par[0];
+        T h = U[0], hu = U[1], hv = U[2];
+        T u = hu / h, v = hv / h;
+        T P = 0.5 * g * h * h;
+        F[0 * 3 + 0] = il * hu;            F[0 * 3 + 1] = il * hv;
+        F[1 * 3 + 0] = il * (hu * u + P);  F[1 * 3 + 1] = il * (hu * v);
+        F[2 * 3 + 0] = il * (hv * u);      F[2 * 3 + 1] = il * (hv * v + P);
+        S[1] = -(sc.dt * g) * (h * A[0]);
+        S[2] = -(sc.dt * g) * (h * A[1]);
+    } break;
+    case SYS_HCNSF3D: {
+        // homogenized compressible Navier-Stokes-Fourier, eq (3.27) and the state/flux/source vectors below it
+        // (listing SM4.12): prescribed porosity alpha(x,t) = A[0] and solid velocity
+        // u_s(x,t) = A[1..3]; reduced tracker basis D^L = dx sym grad u (index 5..10: 00, 11, 22, 01, 02, 12) and
+        // H^L = dx grad T (index 11..13), T = p/rho (R = 1).  par = {gamma, mu, kappa, eta_drag}
+        //   tau = mu (2 D - 2/3 tr D I);  Phi_m = m (x) u + p I - alpha tau;  Phi_E = (E+p) u - alpha tau.u - alpha kappa H
+        //   Phi_D = D (x) u - sym(I (x) u)/tau_grad;  Phi_H = H (x) u - I T/tau_grad
+        //   S_m = (1-alpha)/eta (rho u_s - m);  S_E = S_m . u;  S_D = -D/tau_grad;  S_H = -H/tau_grad
+        const double gamma = sc.par[0], muL = sc.par[1] * dL, kaL = sc.par[2] * dL, eta = sc.par[3];
+        T rho = U[0], E = U[4];
+        T m[3] = {U[1], U[2], U[3]};
+        T u[3] = {m[0] / rho, m[1] / rho, m[2] / rho};
+        T p = (gamma - 1.0) * (E - 0.5 * (m[0] * u[0] + m[1] * u[1] + m[2] * u[2]));
+        T Tm = p / rho;
+        const int didx[3][3] = {{5, 8, 9}, {8, 6, 10}, {9, 10, 7}};   // D_ab -> component index
+        const T* H = U + 11;
+        T alpha = A[0];
+        T trD = U[5] + U[6] + U[7];
+        T tau[3][3];   // alpha * lattice viscous stress
+        for (int a = 0; a < 3; ++a)
+            for (int b = 0; b < 3; ++b) {
+                tau[a][b] = (2.0 * muL) * U[didx[a][b]];
+                if (a == b) tau[a][b] = tau[a][b] - (2.0 / 3.0) * muL * trD;
+                tau[a][b] = alpha * tau[a][b];
+            }
+        for (int j = 0; j < 3; ++j) {
+            F[0 * 3 + j] = il * m[j];
+            for (int a = 0; a < 3; ++a) {
+                F[(1 + a) * 3 + j] = il * (m[a] * u[j]) - tau[a][j];
+                if (a == j) F[(1 + a) * 3 + j] = F[(1 + a) * 3 + j] + il * p;
+            }
+            F[4 * 3 + j] = il * ((E + p) * u[j]) - (tau[j][0] * u[0] + tau[j][1] * u[1] + tau[j][2] * u[2]) - alpha * (kaL * H[j]);
+            for (int b = 0; b < 3; ++b) {
+                F[(11 + b) * 3 + j] = il * (H[b] * u[j]);
+                if (j == b) F[(11 + b) * 3 + j] = F[(11 + b) * 3 + j] - Tm / sc.g_tau;
+            }
+        }
+        for (int a = 0; a < 3; ++a)
+            for (int b = a; b < 3; ++b) {
+                const int k = didx[a][b];
+                for (int j = 0; j < 3; ++j) {
+                    F[k * 3 + j] = il * (U[k] * u[j]);
+                    // sym(I (x) u)_{ab,j} = (delta_ja u_b + delta_jb u_a)/2
+                    if (j == a) F[k * 3 + j] = F[k * 3 + j] - (0.5 / sc.g_tau) * u[b];
+                    if (j == b) F[k * 3 + j] = F[k * 3 + j] - (0.5 / sc.g_tau) * u[a];
+                }
+            }
+        T drag = (1.0 - alpha) * (sc.dt / eta);
+        S[4] = T(0.0);
+        for (int a = 0; a < 3; ++a) {
+            S[1 + a] = drag * (rho * A[1 + a] - m[a]);
+            S[4] = S[4] + S[1 + a] * u[a];
+        }
+        for (int q = 5; q < 14; ++q) S[q] = -U[q] / sc.g_tau;
+    } break;
+    case SYS_MHD2D: {
+        // resistive compressible MHD, 2D, eq (3.25), PAPER.md:L469-L484 (listing SM4.11 L1001-L1015 is garbled: built from
+        // the vector form), cascade on the six CONSERVED fields (N = 6 + 12): U = (rho, m0, m1, E, B0, B1,
+        // G^L_{V,b} = dx d_b V [index 6 + 2 v + b]).  par = {gamma, mu, K, eta}.  Chain rule as in the NSF case plus
+        //   d_b p = (gamma-1)(G_E,b - u.G_m,b + |u|^2/2 G_rho,b - B.G_B,b),  j_z = d_0 B_1 - d_1 B_0,  div B = tr G_B.
+        //   Powell source -(div B)(0, B, u.B, u) read off the same tracker (L484).
+        const double gamma = sc.par[0], muL = sc.par[1] * dL, KL = sc.par[2] * dL, etaL = sc.par[3] * dL;
+        T rho = U[0], E = U[3];
+        T m[2] = {U[1], U[2]};
+        T B[2] = {U[4], U[5]};
+        T u[2] = {m[0] / rho, m[1] / rho};
+        T u2 = u[0] * u[0] + u[1] * u[1];
+        T B2 = B[0] * B[0] + B[1] * B[1];
+        T p = (gamma - 1.0) * (E - 0.5 * rho * u2 - 0.5 * B2);
+        T pt = p + 0.5 * B2;
+        T Tm = p / rho;
+        T uB = u[0] * B[0] + u[1] * B[1];
+        const T* G = U + 6;   // G[2 v + b], v = rho, m0, m1, E, B0, B1
+        T du[2][2], dT[2];
+        for (int b = 0; b < 2; ++b) {
+            for (int a = 0; a < 2; ++a) du[a][b] = (G[2 * (1 + a) + b] - u[a] * G[b]) / rho;
+            T dp = (gamma - 1.0) * (G[6 + b] - u[0] * G[2 + b] - u[1] * G[4 + b] + 0.5 * u2 * G[b] - B[0] * G[8 + b] - B[1] * G[10 + b]);
+            dT[b] = (dp - Tm * G[b]) / rho;
+        }
+        T divu = du[0][0] + du[1][1];
+        T tau[2][2];
+        for (int a = 0; a < 2; ++a)
+            for (int b = 0; b < 2; ++b) {
+                tau[a][b] = muL * (du[a][b] + du[b][a]);
+                if (a == b) tau[a][b] = tau[a][b] - (2.0 / 3.0) * muL * divu;
+            }
+        T jz = G[10 + 0] - G[8 + 1];                 // d_0 B_1 - d_1 B_0 (lattice units)
+        T jxB[2] = {-(jz * B[1]), jz * B[0]};
+        T divB = G[8 + 0] + G[10 + 1];
+        for (int j = 0; j < 2; ++j) {
+            F[0 * 3 + j] = il * m[j];
+            for (int a = 0; a < 2; ++a) {
+                F[(1 + a) * 3 + j] = il * (m[a] * u[j] - B[a] * B[j]) - tau[a][j];
+                if (a == j) F[(1 + a) * 3 + j] = F[(1 + a) * 3 + j] + il * pt;
+            }
+            F[3 * 3 + j] = il * ((E + pt) * u[j] - B[j] * uB) - (tau[j][0] * u[0] + tau[j][1] * u[1]) - KL * dT[j] + etaL * jxB[j];
+            for (int i = 0; i < 2; ++i) F[(4 + i) * 3 + j] = il * (B[i] * u[j] - u[i] * B[j]) - etaL * G[2 * (4 + i) + j];
+            for (int v = 0; v < 6; ++v)
+                for (int b = 0; b < 2; ++b) {
+                    F[(6 + 2 * v + b) * 3 + j] = il * (G[2 * v + b] * u[j]);
+                    if (j == b) F[(6 + 2 * v + b) * 3 + j] = F[(6 + 2 * v + b) * 3 + j] - U[v] / sc.g_tau;
+                }
+        }
+        for (int a = 0; a < 2; ++a) {
+            S[1 + a] = -(il * divB) * B[a];
+            S[4 + a] = -(il * divB) * u[a];
+        }
+        S[3] = -(il * divB) * uB;
+        for (int q = 0; q < 12; ++q) S[6 + q] = -G[q] / sc.g_tau;
+    } break;
     case SYS_MAXWELL2D: {
         // Maxwell TM mode in vacuum, eq (3.10)-(3.11): Q = (E_z, H_x, H_y); par = {c}
         const double c = sc.par[0];
@@ -314,6 +443,7 @@ inline void wave_speeds(int sys, const double* U, const Scaling& sc, double* out
     switch (sys) {
     case SYS_ADVECTION2D: { double u[2] = {sc.par[0], sc.par[1]}, c[2] = {0, 0}; set(u, c, 2); } break;
     case SYS_BURGERS2D:   { double u[2] = {U[0], U[0]}, c[2] = {0, 0}; set(u, c, 2); } break;  // f'(u) = u per axis
+    case SYS_SWE2D_BATHY:
     case SYS_SWE2D:       { double cc = std::sqrt(sc.par[0] * U[0]); double u[2] = {U[1] / U[0], U[2] / U[0]}, c[2] = {cc, cc}; set(u, c, 2); } break;
     case SYS_EULER2D: {
         double u[2] = {U[1] / U[0], U[2] / U[0]};
@@ -321,6 +451,7 @@ inline void wave_speeds(int sys, const double* U, const Scaling& sc, double* out
         double cc = std::sqrt(sc.par[0] * p / U[0]); double c[2] = {cc, cc}; set(u, c, 2);
     } break;
     case SYS_ADR2D: { double u[2] = {sc.par[0], sc.par[1]}, c[2] = {0, 0}; set(u, c, 2); out[2] = std::sqrt(sc.par[2] * dL / sc.g_tau); } break;
+    case SYS_HCNSF3D:     // same hyperbolic part; the dissipative fluxes are scaled by alpha <= 1 (bound taken at alpha = 1)
     case SYS_NSF3D: {
         double u[3] = {U[1] / U[0], U[2] / U[0], U[3] / U[0]};
         double p = (sc.par[0] - 1.0) * (U[4] - 0.5 * U[0] * (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]));
@@ -375,6 +506,22 @@ inline void wave_speeds(int sys, const double* U, const Scaling& sc, double* out
         double p = (sc.par[0] - 1.0) * (U[3] - 0.5 * U[0] * (u[0] * u[0] + u[1] * u[1]));
         double cc = std::sqrt(sc.par[0] * p / U[0]); double c[2] = {cc, cc}; set(u, c, 2);
         double kap = std::fmax(4.0 * sc.par[1] * dL / (3.0 * U[0]), sc.par[2] * dL * (sc.par[0] - 1.0) / U[0]);
+        out[2] = std::sqrt(kap / sc.g_tau);
+    } break;
+    case SYS_MHD2D: {
+        double rho = U[0];
+        double u[2] = {U[1] / rho, U[2] / rho};
+        double B2 = U[4] * U[4] + U[5] * U[5];
+        double p = (sc.par[0] - 1.0) * (U[3] - 0.5 * rho * (u[0] * u[0] + u[1] * u[1]) - 0.5 * B2);
+        double a2 = sc.par[0] * p / rho, b2 = B2 / rho;
+        double c[2];
+        for (int a = 0; a < 2; ++a) {
+            double ba2 = U[4 + a] * U[4 + a] / rho;
+            c[a] = std::sqrt(0.5 * (a2 + b2 + std::sqrt(std::fmax((a2 + b2) * (a2 + b2) - 4.0 * a2 * ba2, 0.0))));
+        }
+        set(u, c, 2);
+        out[1] = std::sqrt(u[0] * u[0] + u[1] * u[1]) + std::sqrt(a2 + b2);
+        double kap = std::fmax(std::fmax(4.0 * sc.par[1] * dL / (3.0 * rho), sc.par[2] * dL * (sc.par[0] - 1.0) / rho), sc.par[3] * dL);
         out[2] = std::sqrt(kap / sc.g_tau);
     } break;
     case SYS_MAXWELL2D: { out[0] = std::fabs(sc.par[0]); out[1] = std::fabs(sc.par[0]); } break;  // eigenvalues {+c, -c, 0}, L393

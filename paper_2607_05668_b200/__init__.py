@@ -29,13 +29,16 @@ STATUS = {0: "LBMK_OK", 1: "LBMK_EINVAL", 2: "LBMK_ENOMEM", 3: "LBMK_ECUDA", 4: 
 LBMK_D2Q5, LBMK_D3Q7 = 0, 1
 LBMK_F64, LBMK_F32_SHIFTED, LBMK_F64_SHIFTED = 0, 1, 2
 LBMK_PERIODIC, LBMK_DIRICHLET_MMS = 0, 1
-LBMK_OPT_PATTERN, LBMK_OPT_KERNEL = 0, 1
+LBMK_OPT_PATTERN, LBMK_OPT_KERNEL, LBMK_OPT_STEPPING = 0, 1, 2
+LBMK_STEPPING_AUTO, LBMK_STEPPING_LAUNCH, LBMK_STEPPING_PERSISTENT = 0, 1, 2
 LBMK_PATTERN_AUTO, LBMK_PATTERN_PULL2, LBMK_PATTERN_AA = 0, 1, 2
 LBMK_KERNEL_AUTO, LBMK_KERNEL_NODE, LBMK_KERNEL_ROW, LBMK_KERNEL_TWOPASS = 0, 1, 2, 3
-SYSTEM_ID = {"advection2d": 0, "burgers2d": 1, "swe2d": 2, "euler2d": 3, "adr2d": 4, "nsf3d": 5, "mhd3d": 6, "urf2d": 7, "maxwell2d": 8, "allencahn2d": 9, "inse2d": 10, "elasticity2d": 11, "nsf2d": 12}
+SYSTEM_ID = {"advection2d": 0, "burgers2d": 1, "swe2d": 2, "euler2d": 3, "adr2d": 4, "nsf3d": 5, "mhd3d": 6, "urf2d": 7, "maxwell2d": 8, "allencahn2d": 9, "inse2d": 10, "elasticity2d": 11, "nsf2d": 12,
+             "swe2d_bathy": 13, "hcnsf3d": 14, "mhd2d": 15}
 PRECISION = {"f64": LBMK_F64, "f32s": LBMK_F32_SHIFTED, "f64s": LBMK_F64_SHIFTED}
 PATTERN = {"auto": 0, "pull2": 1, "aa": 2}
 KERNEL = {"auto": 0, "node": 1, "row": 2, "twopass": 3}
+STEPPING = {"auto": 0, "launch": 1, "persistent": 2}
 
 # every symbol include/lbmk.h declares: (restype, argtypes)
 _dp = C.POINTER(C.c_double)
@@ -43,6 +46,7 @@ _vp = C.c_void_p
 SYMBOLS = {
     "lbmk_system_create": (C.c_int, [C.c_int, C.c_int, _dp, C.c_int, C.POINTER(_vp)]),
     "lbmk_system_info": (C.c_int, [_vp] + [C.POINTER(C.c_int)] * 4),
+    "lbmk_system_aux_count": (C.c_int, [_vp, C.POINTER(C.c_int)]),
     "lbmk_system_set_relaxation": (C.c_int, [_vp, _dp, C.c_int, C.c_double]),
     "lbmk_system_set_omega": (C.c_int, [_vp, _dp, C.c_int]),
     "lbmk_system_set_reference": (C.c_int, [_vp, _dp, C.c_int]),
@@ -57,6 +61,7 @@ SYMBOLS = {
     "lbmk_grid_destroy": (None, [_vp]),
     "lbmk_init_from_U": (C.c_int, [_vp, _vp, C.c_int, C.c_double]),
     "lbmk_set_populations": (C.c_int, [_vp, _vp, C.c_int, C.c_double]),
+    "lbmk_set_aux_fields": (C.c_int, [_vp, _vp, C.c_int]),
     "lbmk_step": (C.c_int, [_vp, C.c_int]),
     "lbmk_read_U": (C.c_int, [_vp, _vp, C.c_int]),
     "lbmk_read_populations": (C.c_int, [_vp, _vp, C.c_int]),
@@ -68,6 +73,11 @@ SYMBOLS = {
     "lbmk_halo_bytes": (C.c_int, [_vp, C.POINTER(C.c_size_t)]),
     "lbmk_halo_pack": (C.c_int, [_vp, _vp, _vp]),
     "lbmk_halo_unpack": (C.c_int, [_vp, _vp, _vp]),
+    "lbmk_halo_pack_on": (C.c_int, [_vp, _vp, _vp, _vp]),
+    "lbmk_halo_unpack_on": (C.c_int, [_vp, _vp, _vp, _vp]),
+    "lbmk_step_slab": (C.c_int, [_vp]),
+    "lbmk_stream_wait_boundary": (C.c_int, [_vp, _vp]),
+    "lbmk_grid_wait_stream": (C.c_int, [_vp, _vp]),
     "lbmk_stream_index_map": (C.c_int, [_vp, C.c_int, _vp, C.c_int]),
     "lbmk_lattice_constants": (C.c_int, [C.c_int, C.POINTER(C.c_int), _dp, _dp]),
     "lbmk_grid_omega": (C.c_int, [_vp, _dp]),
@@ -136,6 +146,12 @@ def lbmk_system_info(sys_h):
     return tuple(x.value for x in v)      # m_conserved, m_total, dim, Q
 
 
+def lbmk_system_aux_count(sys_h) -> int:
+    v = C.c_int()
+    _check(lib().lbmk_system_aux_count(sys_h, C.byref(v)))
+    return v.value
+
+
 def lbmk_system_set_relaxation(sys_h, tau_R, g_tau: float):
     a, p = _darr(tau_R)
     _check(lib().lbmk_system_set_relaxation(sys_h, p, a.size, float(g_tau)))
@@ -202,6 +218,10 @@ def lbmk_set_populations(grid_h, ptr: int, on_device: bool, t0: float = 0.0):
     _check(lib().lbmk_set_populations(grid_h, _vp(ptr), int(on_device), float(t0)), grid_h)
 
 
+def lbmk_set_aux_fields(grid_h, ptr: int, on_device: bool):
+    _check(lib().lbmk_set_aux_fields(grid_h, _vp(ptr), int(on_device)), grid_h)
+
+
 def lbmk_step(grid_h, n_steps: int):
     _check(lib().lbmk_step(grid_h, int(n_steps)), grid_h)
 
@@ -248,6 +268,26 @@ def lbmk_halo_pack(grid_h, send_lo: int, send_hi: int):
 
 def lbmk_halo_unpack(grid_h, recv_lo: int, recv_hi: int):
     _check(lib().lbmk_halo_unpack(grid_h, _vp(recv_lo), _vp(recv_hi)), grid_h)
+
+
+def lbmk_halo_pack_on(grid_h, send_lo: int, send_hi: int, cuda_stream: int):
+    _check(lib().lbmk_halo_pack_on(grid_h, _vp(send_lo), _vp(send_hi), _vp(cuda_stream)), grid_h)
+
+
+def lbmk_halo_unpack_on(grid_h, recv_lo: int, recv_hi: int, cuda_stream: int):
+    _check(lib().lbmk_halo_unpack_on(grid_h, _vp(recv_lo), _vp(recv_hi), _vp(cuda_stream)), grid_h)
+
+
+def lbmk_step_slab(grid_h):
+    _check(lib().lbmk_step_slab(grid_h), grid_h)
+
+
+def lbmk_stream_wait_boundary(grid_h, cuda_stream: int):
+    _check(lib().lbmk_stream_wait_boundary(grid_h, _vp(cuda_stream)), grid_h)
+
+
+def lbmk_grid_wait_stream(grid_h, cuda_stream: int):
+    _check(lib().lbmk_grid_wait_stream(grid_h, _vp(cuda_stream)), grid_h)
 
 
 def lbmk_error_norms(grid_h, m_total: int) -> np.ndarray:
@@ -302,9 +342,10 @@ class System:
                  omega=None, s_max: float = 0.0):
         self.name = name
         sid = SYSTEM_ID[name]
-        lattice = LBMK_D3Q7 if name in ("nsf3d", "mhd3d") else LBMK_D2Q5
+        lattice = LBMK_D3Q7 if name in ("nsf3d", "mhd3d", "hcnsf3d") else LBMK_D2Q5
         self.h = lbmk_system_create(sid, lattice, list(params))
         self.m_conserved, self.m_total, self.dim, self.Q = lbmk_system_info(self.h)
+        self.n_aux = lbmk_system_aux_count(self.h)
         lbmk_system_set_relaxation(self.h, tau_R, g_tau if self.m_total > self.m_conserved else 1.0)
         if U_ref is not None:
             lbmk_system_set_reference(self.h, list(U_ref))
@@ -332,7 +373,7 @@ class Grid:
 
     def __init__(self, system: System, nx: int, ny: int, nz: int, dx: float, lam: float, precision: str = "f64",
                  bc: str = "periodic", pattern: str = "auto", kernel: str = "auto", device: str = "cuda:0",
-                 origin: Sequence[int] = (0, 0, 0), slab: bool = False):
+                 origin: Sequence[int] = (0, 0, 0), slab: bool = False, stepping: str = "auto"):
         import torch
         if not torch.cuda.is_available():
             raise LbmkError(3, "no CUDA device: the collide-and-stream path has no CPU fallback")
@@ -351,6 +392,8 @@ class Grid:
             lbmk_grid_set_option(self.h, LBMK_OPT_PATTERN, PATTERN[pattern])
         if kernel != "auto":
             lbmk_grid_set_option(self.h, LBMK_OPT_KERNEL, KERNEL[kernel])
+        if stepping != "auto":
+            lbmk_grid_set_option(self.h, LBMK_OPT_STEPPING, STEPPING[stepping])
         if slab:
             lbmk_grid_set_slab(self.h, True)
         self.workspace_bytes = lbmk_grid_workspace_bytes(self.h)
@@ -358,13 +401,17 @@ class Grid:
         lbmk_grid_bind_workspace(self.h, self.workspace.data_ptr(), self.workspace_bytes)
         self.pattern = {1: "pull2", 2: "aa"}[lbmk_grid_get_option(self.h, LBMK_OPT_PATTERN)]
         self.kernel = {1: "node", 2: "row", 3: "twopass"}[lbmk_grid_get_option(self.h, LBMK_OPT_KERNEL)]
+        self.stepping = {1: "launch", 2: "persistent"}[lbmk_grid_get_option(self.h, LBMK_OPT_STEPPING)]
 
     @classmethod
     def from_workload(cls, w, precision: Optional[str] = None, omega=None, declare_bound: bool = True, **kw):
         s = System(w.system, params=w.params, tau_R=w.tau_R, g_tau=w.g_tau, U_ref=w.U_ref, mms_id=w.mms_id,
                    mms_params=w.mms_params if w.mms_id else (), omega=omega, s_max=w.s_max if declare_bound else 0.0)
         kw.setdefault("origin", getattr(w, "origin", (0, 0, 0)))
-        return cls(s, w.nx, w.ny, w.nz, w.dx, w.lam, precision=precision or w.precision, **kw)
+        g = cls(s, w.nx, w.ny, w.nz, w.dx, w.lam, precision=precision or w.precision, **kw)
+        if s.n_aux:
+            g.set_aux_fields(w.aux_fields())        # prescribed coefficient fields are inputs of the workload, like U(x, 0)
+        return g
 
     # shapes
     @property
@@ -374,6 +421,10 @@ class Grid:
     @property
     def shape_f(self):
         return (self.system.m_total, self.system.Q, self.nz, self.ny, self.nx)
+
+    @property
+    def shape_aux(self):
+        return (self.system.n_aux, self.nz, self.ny, self.nx)
 
     def _in(self, a, shape):
         """(pointer, on_device, keepalive) of a numpy array (host) or torch tensor (host or device)."""
@@ -388,6 +439,10 @@ class Grid:
     def init_from_U(self, U, t0: float = 0.0):
         p, dev, keep = self._in(U, self.shape_U)
         lbmk_init_from_U(self.h, p, dev, t0)
+
+    def set_aux_fields(self, A):
+        p, dev, keep = self._in(A, self.shape_aux)
+        lbmk_set_aux_fields(self.h, p, dev)
 
     def set_populations(self, f, t0: float = 0.0):
         p, dev, keep = self._in(f, self.shape_f)

@@ -16,7 +16,8 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "liblbmk.so")
 UNITS = ["lbmk_api", "sys_advection2d", "sys_burgers2d", "sys_swe2d", "sys_euler2d", "sys_adr2d", "sys_nsf3d", "sys_mhd3d",
-         "sys_urf2d", "sys_maxwell2d", "sys_allencahn2d", "sys_inse2d", "sys_elasticity2d", "sys_nsf2d"]
+         "sys_urf2d", "sys_maxwell2d", "sys_allencahn2d", "sys_inse2d", "sys_elasticity2d", "sys_nsf2d",
+         "sys_swe2d_bathy", "sys_hcnsf3d", "sys_mhd2d"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 

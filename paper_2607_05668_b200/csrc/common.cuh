@@ -12,7 +12,7 @@
 
 namespace lbmk {
 
-constexpr int MAXM = 20;   // largest compiled-in system has 17 components
+constexpr int MAXM = 20;   // largest compiled-in system has 18 components
 
 template <int D> struct Lattice;
 template <> struct Lattice<2> {
@@ -61,7 +61,16 @@ struct KParams {
     const R* tabY;
     const R* tabZ;
     const R* coef;          // per-row forcing coefficients [nz*ny][Mms::NC], rewritten before every step
+    // prescribed per-node coefficient fields (bed slope of eq 3.5): aux[a * aux_stride + node], in R
+    const R* aux;
+    long long aux_stride;
+    // node range [node0, node1) a step launch updates (whole grid: 0, n); block b starts at node0 + b*BLOCK
+    long long node0, node1;
 };
+
+// number of prescribed coefficient fields of a system: Sys::NA where declared, else 0
+template <class S, class = void> struct AuxCount { static constexpr int value = 0; };
+template <class S> struct AuxCount<S, std::void_t<decltype(S::NA)>> { static constexpr int value = S::NA; };
 
 struct NodeIdx { int ix, iy, iz; };
 

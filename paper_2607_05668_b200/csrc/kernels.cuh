@@ -31,7 +31,7 @@ template <class Sys> struct MmsNC<Sys, true> { static constexpr int value = Sys:
 
 // per-node manufactured forcing: the x-table entries of this node and the coefficients of its (y, z) row
 // (mms_generated.cuh source_row; the row table is filled by mms_row_coeffs_kernel).  SH: `c` is the block's
-// shared-memory copy of its row (see stage_row_coeffs), otherwise the row is read from global memory.
+// shared-memory copy of its row, otherwise `c` is this step's coefficient table in global memory.
 template <class Sys, class R, bool SH>
 __device__ __forceinline__ void mms_node(const KParams<R>& P, const NodeIdx& p, const R* c, R (&s)[Sys::M]) {
     if constexpr (has_mms<Sys>()) {
@@ -39,7 +39,7 @@ __device__ __forceinline__ void mms_node(const KParams<R>& P, const NodeIdx& p, 
         R X[G::NX > 0 ? G::NX : 1];
 #pragma unroll
         for (int e = 0; e < G::NX; ++e) X[e] = __ldg(P.tabX + e * P.nx + p.ix);
-        if (!SH) c = P.coef + (size_t)(p.iz * P.ny + p.iy) * G::NC;
+        if (!SH) c = c + (size_t)(p.iz * P.ny + p.iy) * G::NC;      // c = this step's coefficient table
         G::template source_row<R, SH>(c, X, s);
     }
 }
@@ -96,31 +96,51 @@ __device__ __forceinline__ void relax(R (&f)[2 * D + 1], R omega, R dQ, const R 
     }
 }
 
-// Pointer qualifiers of the step kernels: the two-lattice modes read one buffer and write the other, so both carry
-// __restrict__ (loads may use the non-coherent path and move freely across the stores); the in-place AA modes are
-// launched with src == dst, where __restrict__ would be a false promise -- plain pointers there.
-template <class R, int MODE> struct StepPtr { using Src = const R* __restrict__; using Dst = R* __restrict__; };
-template <class R> struct StepPtr<R, 1 /*MODE_AA_EVEN*/> { using Src = const R*; using Dst = R*; };
-template <class R> struct StepPtr<R, 2 /*MODE_AA_ODD*/> { using Src = const R*; using Dst = R*; };
+// Pointer qualifiers of the step kernels: the two-lattice modes of the per-launch kernels read one buffer and write the
+// other, so both carry __restrict__ (loads may use the non-coherent path and move freely across the stores); the
+// in-place AA modes are launched with src == dst, where __restrict__ would be a false promise -- plain pointers there.
+// COHERENT (the persistent multi-step kernel): a buffer written in one step is read in the next step of the SAME launch,
+// so neither const __restrict__ (-> ld.global.nc) is allowed; plain pointers, ordered by the grid barrier.
+template <class R, int MODE, bool COHERENT = false> struct StepPtr { using Src = const R* __restrict__; using Dst = R* __restrict__; };
+template <class R, bool C> struct StepPtr<R, 1 /*MODE_AA_EVEN*/, C> { using Src = const R*; using Dst = R*; };
+template <class R, bool C> struct StepPtr<R, 2 /*MODE_AA_ODD*/, C> { using Src = const R*; using Dst = R*; };
+template <class R> struct StepPtr<R, 0 /*MODE_PULL2*/, true> { using Src = const R*; using Dst = R*; };
+template <class R> struct StepPtr<R, 3 /*MODE_LOCAL*/, true> { using Src = const R*; using Dst = R*; };
+
+// prescribed coefficient fields of `node` into the system's context (systems with NA > 0 only)
+template <class Sys, class R>
+__device__ __forceinline__ void load_aux(typename Sys::Ctx& ctx, const KParams<R>& P, long long node) {
+    constexpr int NA = AuxCount<Sys>::value;
+    if constexpr (NA > 0) {
+        R A[NA];
+#pragma unroll
+        for (int a = 0; a < NA; ++a) A[a] = __ldg(P.aux + a * P.aux_stride + node);
+        Sys::set_aux(ctx, A);
+    }
+}
 
 // ------------------------------------------------------------------------------------------------ step
-template <class Sys, class R, int MODE, bool MMS, int BLOCK, int MINB>
-__global__ void __launch_bounds__(BLOCK, MINB)
-collide_stream_node(typename StepPtr<R, MODE>::Src src, typename StepPtr<R, MODE>::Dst dst, const __grid_constant__ KParams<R> P) {
+// The update of ONE node by ONE thread (a1-a7).  `first` = first node of this thread block's BLOCK-node segment,
+// coef_s = the block's shared-memory slot for its row's forcing coefficients, coef = this step's coefficient table.
+// Called by the per-launch kernel (one segment per block) and by the persistent kernel (segments in a loop): the
+// same code, hence the same bits.
+template <class Sys, class R, int MODE, bool MMS, int BLOCK, bool COHERENT>
+__device__ __forceinline__ void node_step(typename StepPtr<R, MODE, COHERENT>::Src src, typename StepPtr<R, MODE, COHERENT>::Dst dst,
+                                          const KParams<R>& P, const R* coef, long long first, R* coef_s) {
     constexpr int D = Sys::D, Q = 2 * D + 1, M = Sys::M;
-    const long long node = (long long)blockIdx.x * BLOCK + threadIdx.x;
+    const long long node = first + threadIdx.x;
     constexpr int NCs = MMS ? MmsNC<Sys>::value : 4;
-    __shared__ __align__(16) R coef_s[NCs];
-    const bool staged = MMS && (P.nx % BLOCK == 0);          // kernel-uniform; then n is a multiple of BLOCK too
+    // kernel-uniform: a block lies inside one (y, z) row; then every segment is full (n and node0 are multiples of BLOCK)
+    const bool staged = MMS && (P.nx % BLOCK == 0) && (P.node0 % BLOCK == 0);
     if constexpr (MMS) {
         if (staged) {
-            const unsigned row = (unsigned)((long long)blockIdx.x * BLOCK / P.nx);
+            const unsigned row = (unsigned)(first / P.nx);
             constexpr int per = 16 / sizeof(R);
-            if (threadIdx.x < NCs / per) cp_async16(coef_s + per * threadIdx.x, P.coef + (size_t)row * NCs + per * threadIdx.x);
+            if (threadIdx.x < NCs / per) cp_async16(coef_s + per * threadIdx.x, coef + (size_t)row * NCs + per * threadIdx.x);
             cp_async_commit();
         }
     }
-    if (node >= P.n) return;
+    if (node >= P.node1) return;
     const NodeIdx p = decompose(node, P.nx, P.ny);
     // gather addresses: one 64-bit pointer per direction (the source node's slot in its tile); the plane offset
     // (k*Q + slot)*TILE is a compile-time constant, so every access is [pointer + immediate]
@@ -136,8 +156,11 @@ collide_stream_node(typename StepPtr<R, MODE>::Src src, typename StepPtr<R, MODE
 #pragma unroll
         for (int i = 0; i < Q; ++i) {
             const int slot = (MODE == MODE_AA_ODD) ? opposite(i) : i;
-            f[k][i] = sp[i][(k * Q + slot) * TILE];
+            // persistent kernel: the line may sit stale in this SM's L1 from two steps ago -> read at L2 (ld.global.cg)
+            f[k][i] = COHERENT ? __ldcg(sp[i] + (k * Q + slot) * TILE) : sp[i][(k * Q + slot) * TILE];
         }
+    typename Sys::Ctx ctx;
+    load_aux<Sys, R>(ctx, P, node);
     // manufactured forcing while the gather is in flight: after the row/node split it is ~250 instructions on
     // ~40 registers, independent of the populations
     R smms[M];
@@ -147,7 +170,7 @@ collide_stream_node(typename StepPtr<R, MODE>::Src src, typename StepPtr<R, MODE
             __syncthreads();
             mms_node<Sys, R, true>(P, p, coef_s, smms);
         } else {
-            mms_node<Sys, R, false>(P, p, nullptr, smms);
+            mms_node<Sys, R, false>(P, p, coef, smms);
         }
     }
     R dQ[M];
@@ -158,7 +181,6 @@ collide_stream_node(typename StepPtr<R, MODE>::Src src, typename StepPtr<R, MODE
         for (int i = 1; i < Q; ++i) s += f[k][i];
         dQ[k] = s;
     }
-    typename Sys::Ctx ctx;
     Sys::setup(ctx, dQ, P);
 
     static_for<0, M>([&](auto K) {
@@ -180,6 +202,59 @@ collide_stream_node(typename StepPtr<R, MODE>::Src src, typename StepPtr<R, MODE
     });
 }
 
+template <class Sys, class R, int MODE, bool MMS, int BLOCK, int MINB>
+__global__ void __launch_bounds__(BLOCK, MINB)
+collide_stream_node(typename StepPtr<R, MODE>::Src src, typename StepPtr<R, MODE>::Dst dst, const __grid_constant__ KParams<R> P) {
+    constexpr int NCs = MMS ? MmsNC<Sys>::value : 4;
+    __shared__ __align__(16) R coef_s[NCs];
+    node_step<Sys, R, MODE, MMS, BLOCK, false>(src, dst, P, P.coef, P.node0 + (long long)blockIdx.x * BLOCK, coef_s);
+}
+
+// ------------------------------------------------------------------------------------------------ step, persistent
+// Launch-free stepping for grids whose state lives in L2 (SURVEY.md §7 "Small configs"): ONE cooperative launch
+// advances `nsteps` steps of the two-lattice pull pattern; all blocks are co-resident, each takes the BLOCK-node
+// segments b, b + gridDim.x, ... of every step, and a grid-wide barrier separates the steps (the buffer written in
+// step s is the one read in step s+1).  Step s reads its forcing coefficients at P.coef + s*coef_stride.  The
+// per-node code is node_step, i.e. bit-identical to the per-launch path.
+__device__ __forceinline__ void grid_barrier(unsigned int* bar, unsigned int target) {
+    // arrive: after the block-wide barrier one thread publishes the block's stores with a gpu-scope RELEASE increment of
+    // the monotone counter (cumulative over what the other threads wrote before bar.sync); wait: the same thread spins with
+    // gpu-scope ACQUIRE loads until all blocks of this step have arrived, then releases its block.  The populations are
+    // read with ld.global.cg (L2), so no stale L1 line can be observed after the barrier.
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(bar), "r"(1u) : "memory");
+        unsigned int v;
+        do {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(bar) : "memory");
+        } while (v < target);
+    }
+    __syncthreads();
+}
+
+template <class Sys, class R, bool MMS, int BLOCK, int MINB>
+__global__ void __launch_bounds__(BLOCK, MINB)
+collide_stream_persistent(R* fa, R* fb, const __grid_constant__ KParams<R> P, int nsteps, int first_local, long long coef_stride,
+                          unsigned int* bar) {
+    constexpr int NCs = MMS ? MmsNC<Sys>::value : 4;
+    __shared__ __align__(16) R coef_s[NCs];
+    const long long nseg = (P.n + BLOCK - 1) / BLOCK;
+    const bool staged = MMS && (P.nx % BLOCK == 0);
+    R* src = fa;
+    R* dst = fb;
+    const R* coef = P.coef;
+    for (int s = 0; s < nsteps; ++s) {
+        for (long long seg = blockIdx.x; seg < nseg; seg += gridDim.x) {
+            if (s == 0 && first_local) node_step<Sys, R, MODE_LOCAL, MMS, BLOCK, true>(src, dst, P, coef, seg * BLOCK, coef_s);
+            else node_step<Sys, R, MODE_PULL2, MMS, BLOCK, true>(src, dst, P, coef, seg * BLOCK, coef_s);
+            if (staged) __syncthreads();          // coef_s is overwritten by the next segment
+        }
+        R* t = src; src = dst; dst = t;
+        coef += coef_stride;
+        if (s + 1 < nsteps) grid_barrier(bar, (unsigned)(s + 1) * gridDim.x);
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ step, two-pass
 // Low-register variant using the linearity of BGK in f (SURVEY.md §7 option iii):
 //   f'_k,i = (1 - omega_k) f_k,i + c_k,i,   c_k,0 = w0 (omega dQ_k + s_k),  c_k,+-a = w1 (omega dQ_k + s_k) +- (omega/2) dF_k,a.
@@ -191,11 +266,11 @@ __global__ void __launch_bounds__(BLOCK, MINB)
 collide_stream_twopass(typename StepPtr<R, MODE>::Src src, typename StepPtr<R, MODE>::Dst dst, const __grid_constant__ KParams<R> P) {
     constexpr int D = Sys::D, Q = 2 * D + 1, M = Sys::M;
     using L = Lattice<D>;
-    const long long node = (long long)blockIdx.x * BLOCK + threadIdx.x;
-    if (node >= P.n) return;
+    const long long node = P.node0 + (long long)blockIdx.x * BLOCK + threadIdx.x;
+    if (node >= P.node1) return;
     const NodeIdx p = decompose(node, P.nx, P.ny);
     R smms[M];
-    if constexpr (MMS) mms_node<Sys, R, false>(P, p, nullptr, smms);
+    if constexpr (MMS) mms_node<Sys, R, false>(P, p, P.coef, smms);
     const R* sp[Q];
 #pragma unroll
     for (int i = 0; i < Q; ++i)
@@ -214,6 +289,7 @@ collide_stream_twopass(typename StepPtr<R, MODE>::Src src, typename StepPtr<R, M
         dQ[k] = s;
     }
     typename Sys::Ctx ctx;
+    load_aux<Sys, R>(ctx, P, node);
     Sys::setup(ctx, dQ, P);
     static_for<0, M>([&](auto K) {
         constexpr int k = decltype(K)::value;
@@ -252,6 +328,7 @@ __global__ void init_from_U_kernel(const double* __restrict__ U, R* __restrict__
 #pragma unroll
     for (int k = 0; k < M; ++k) dQ[k] = (R)(U[(long long)k * P.n + node] - Pd.ref[k]);
     typename Sys::Ctx ctx;
+    load_aux<Sys, R>(ctx, P, node);
     Sys::setup(ctx, dQ, P);
     static_for<0, M>([&](auto K) {
         constexpr int k = decltype(K)::value;
@@ -280,6 +357,7 @@ __global__ void reference_equilibrium_kernel(double* __restrict__ feq0, const __
     for (int k = 0; k < M; ++k) { Q0[k] = Pd.ref[k]; any = any || (Q0[k] != 0.0); }
     if (!any) { for (int q = 0; q < M * Q; ++q) feq0[q] = 0.0; return; }
     typename Sys::Ctx ctx;
+    if constexpr (AuxCount<Sys>::value > 0) Sys::default_aux(ctx);     // uniform reference: the prescribed fields drop out
     Sys::setup(ctx, Q0, P0);
     static_for<0, M>([&](auto K) {
         constexpr int k = decltype(K)::value;
@@ -338,6 +416,14 @@ __global__ void set_f_kernel(const double* __restrict__ in, R* __restrict__ f, c
     const long long node = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (node >= n) return;
     for (int q = 0; q < MQ; ++q) f[tile_off(node, MQ) + q * TILE] = (R)(in[(long long)q * n + node] - feq0[q]);
+}
+
+// prescribed coefficient fields: user fp64 [NA][n] -> R [NA][aux_stride]
+template <class R>
+__global__ void set_aux_kernel(const double* __restrict__ in, R* __restrict__ aux, int NA, long long n, long long stride) {
+    const long long node = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (node >= n) return;
+    for (int a = 0; a < NA; ++a) aux[a * stride + node] = (R)in[(long long)a * n + node];
 }
 
 // ghost plane of a slab: first / last plane of the slowest axis
@@ -482,6 +568,7 @@ __global__ void dirichlet_frame_kernel(R* __restrict__ f, int gather, const __gr
         G::template exact<R>(P.mms, P.T, X, Y, Z, q);
         for (int k = 0; k < M; ++k) dQ[k] = q[k] - P.ref[k];
         typename Sys::Ctx ctx;
+        load_aux<Sys, R>(ctx, P, node);
         Sys::setup(ctx, dQ, P);
         static_for<0, M>([&](auto K) {
             constexpr int k = decltype(K)::value;

@@ -40,7 +40,9 @@ struct lbmk_grid {
     long long opt_pattern, opt_kernel;
     bool bound, inited;
     size_t ws_bytes;
-    size_t off_f[2], off_tab[3], off_coef, off_feq0, off_red;
+    size_t off_f[2], off_tab[3], off_coef, off_feq0, off_red, off_aux;
+    long long opt_stepping;
+    cudaEvent_t ev_boundary, ev_join;
     std::string err;
     cudaEvent_t ev0, ev1;
     bool have_events, timed;
@@ -63,11 +65,14 @@ static const SysOps* ops_of(int id) {
         case LBMK_SYS_INSE2D: return ops_inse2d();
         case LBMK_SYS_ELASTICITY2D: return ops_elasticity2d();
         case LBMK_SYS_NSF2D_GRADTRACK: return ops_nsf2d();
+        case LBMK_SYS_SWE2D_BATHY: return ops_swe2d_bathy();
+        case LBMK_SYS_HCNSF3D: return ops_hcnsf3d();
+        case LBMK_SYS_MHD2D: return ops_mhd2d();
     }
     return nullptr;
 }
-static const int N_PARAMS[LBMK_SYS_COUNT] = {2, 0, 1, 1, 4, 3, 2, 0, 1, 2, 2, 3, 3};
-static const int N_MMS_PARAMS[LBMK_SYS_COUNT] = {0, 1, 3, 0, 0, 4, 0, 0, 0, 0, 2, 0, 0};
+static const int N_PARAMS[LBMK_SYS_COUNT] = {2, 0, 1, 1, 4, 3, 2, 0, 1, 2, 2, 3, 3, 1, 4, 4};
+static const int N_MMS_PARAMS[LBMK_SYS_COUNT] = {0, 1, 3, 0, 0, 4, 0, 0, 0, 0, 2, 0, 0, 6, 0, 0};
 
 static lbmk_status sys_fail(lbmk_status s, const char* msg) { g_sys_err = msg; return s; }
 static lbmk_status fail(lbmk_grid* g, lbmk_status s, const std::string& msg) { if (g) g->err = msg; else g_sys_err = msg; return s; }
@@ -124,6 +129,12 @@ lbmk_status lbmk_system_info(const lbmk_system* sys, int* m_conserved, int* m_to
     return LBMK_OK;
 }
 
+lbmk_status lbmk_system_aux_count(const lbmk_system* sys, int* n_aux) {
+    if (!sys || !n_aux) return sys_fail(LBMK_EINVAL, "NULL argument");
+    *n_aux = ops_of(sys->id)->n_aux;
+    return LBMK_OK;
+}
+
 lbmk_status lbmk_system_set_relaxation(lbmk_system* sys, const double* tau_R, int n, double g_tau) {
     if (!sys || !tau_R) return sys_fail(LBMK_EINVAL, "NULL argument");
     const SysOps* o = ops_of(sys->id);
@@ -153,10 +164,14 @@ lbmk_status lbmk_system_set_reference(lbmk_system* sys, const double* U0, int n)
     if (!sys || !U0) return sys_fail(LBMK_EINVAL, "NULL argument");
     const SysOps* o = ops_of(sys->id);
     if (n != o->M) return sys_fail(LBMK_EINVAL, "reference: n must be m_total");
-    if (sys->id == LBMK_SYS_NSF3D_GRADTRACK || sys->id == LBMK_SYS_MHD3D_JTRACK) {
+    if (sys->id == LBMK_SYS_NSF3D_GRADTRACK || sys->id == LBMK_SYS_MHD3D_JTRACK || sys->id == LBMK_SYS_HCNSF3D) {
         for (int k = 0; k < n; ++k)
             if (k != 0 && k != 4 && U0[k] != 0.0)
-                return sys_fail(LBMK_EUNSUPPORTED, "NSF3D/MHD3D delta forms need zero reference momentum, field and trackers");
+                return sys_fail(LBMK_EUNSUPPORTED, "NSF3D/MHD3D/HCNSF3D delta forms need zero reference momentum, field and trackers");
+    }
+    if (sys->id == LBMK_SYS_MHD2D) {
+        for (int k = 6; k < n; ++k)
+            if (U0[k] != 0.0) return sys_fail(LBMK_EUNSUPPORTED, "MHD2D needs zero reference trackers");
     }
     if (sys->id == LBMK_SYS_ELASTICITY2D) {
         const double rest[6] = {1, 0, 0, 1, 0, 0};
@@ -224,6 +239,7 @@ static void derive_params(lbmk_grid* g) {
     for (int i = 0; i < 8; ++i) P.par[i] = s.par[i];
     const double* r = P.ref;
     switch (s.id) {
+        case LBMK_SYS_SWE2D_BATHY:
         case LBMK_SYS_SWE2D:
             for (int a = 0; a < 2; ++a) P.cst[a] = r[0] != 0.0 ? r[1 + a] / r[0] : 0.0;
             break;
@@ -241,6 +257,15 @@ static void derive_params(lbmk_grid* g) {
             P.cst[3] = (P.cst[2] - r[0]) / 3.0;
             for (int a = 0; a < 2; ++a) P.cst[a] = P.cst[4] != 0.0 ? 3.0 * r[1 + a] / P.cst[4] : 0.0;
         } break;
+        case LBMK_SYS_MHD2D: {
+            // u0 = m0/rho0; gas pressure p0 = (gamma-1)(E0 - m0.u0/2 - |B0|^2/2); cst[4] = E0 + p0 + |B0|^2/2
+            double ke = 0.0;
+            const double B2 = r[4] * r[4] + r[5] * r[5];
+            for (int a = 0; a < 2; ++a) { P.cst[a] = r[0] != 0.0 ? r[1 + a] / r[0] : 0.0; ke += r[1 + a] * P.cst[a]; }
+            P.cst[3] = (s.par[0] - 1.0) * (r[3] - 0.5 * ke - 0.5 * B2);
+            P.cst[4] = r[3] + P.cst[3] + 0.5 * B2;
+        } break;
+        case LBMK_SYS_HCNSF3D:
         case LBMK_SYS_NSF3D_GRADTRACK:
         case LBMK_SYS_MHD3D_JTRACK:
             P.cst[3] = (s.par[0] - 1.0) * r[4];
@@ -271,6 +296,13 @@ static void resolve_options(lbmk_grid* g) {
     if (c.bc == LBMK_DIRICHLET_MMS) c.pattern = PATTERN_PULL2;      // the frame refill needs canonical storage
     c.kernel = g->opt_kernel == LBMK_KERNEL_AUTO ? KERNEL_NODE : (int)g->opt_kernel;
     if (c.kernel == KERNEL_ROW && !g->ops->row_kernel_supported(c)) c.kernel = KERNEL_NODE;
+    // Stepping: grids whose two population copies fit in L2 are launch-latency bound, not bandwidth bound (c1: 0.3 MB,
+    // c2: 63 MB against 126 MB of L2) -> one cooperative launch per batch of steps; larger grids: one launch per step.
+    const size_t esz = c.prec == PREC_F64 ? 8 : 4;
+    const size_t state2 = 2 * (size_t)g->ops->M * (2 * g->ops->D + 1) * (size_t)c.n * esz;
+    const bool can = c.pattern == PATTERN_PULL2 && c.kernel == KERNEL_NODE && c.bc == LBMK_PERIODIC && !c.Pd.ghost;
+    if (g->opt_stepping == LBMK_STEPPING_AUTO) c.stepping = (can && state2 <= (size_t(96) << 20)) ? STEPPING_PERSISTENT : STEPPING_LAUNCH;
+    else c.stepping = (g->opt_stepping == LBMK_STEPPING_PERSISTENT && can) ? STEPPING_PERSISTENT : STEPPING_LAUNCH;
 }
 
 static void layout(lbmk_grid* g) {
@@ -293,7 +325,9 @@ static void layout(lbmk_grid* g) {
         g->off_coef = off; off += align_up(2 * (size_t)c.coef_B * per_step, 256);
     }
     g->off_feq0 = off; off += align_up((size_t)o->M * (2 * o->D + 1) * 8, 256);
-    g->off_red = off; off += 256;
+    g->off_red = off; off += 256;          // [0..3] reductions, [8] grid-barrier counter
+    c.aux_stride = (long long)(ntiles * TILE);
+    g->off_aux = off; off += align_up((size_t)(o->n_aux > 0 ? o->n_aux : 0) * ntiles * TILE * esz, 256);
     g->ws_bytes = off;
 }
 
@@ -325,7 +359,7 @@ lbmk_status lbmk_grid_create(const lbmk_system* sys, int nx, int ny, int nz, lbm
     g->ops = o;
     g->precision = precision;
     g->dx = dx; g->lam = lambda;
-    g->opt_pattern = LBMK_PATTERN_AUTO; g->opt_kernel = LBMK_KERNEL_AUTO;
+    g->opt_pattern = LBMK_PATTERN_AUTO; g->opt_kernel = LBMK_KERNEL_AUTO; g->opt_stepping = LBMK_STEPPING_AUTO;
     g->bound = g->inited = false;
     g->have_events = g->timed = false;
     GridCore& c = g->c;
@@ -352,6 +386,9 @@ lbmk_status lbmk_grid_set_option(lbmk_grid* g, lbmk_option key, long long value)
         if (value < LBMK_KERNEL_AUTO || value > LBMK_KERNEL_TWOPASS) return fail(g, LBMK_EINVAL, "unknown kernel variant");
         if (value == LBMK_KERNEL_ROW) return fail(g, LBMK_EUNSUPPORTED, "LBMK_KERNEL_ROW is reserved: no staged-row kernel in this build");
         g->opt_kernel = value;
+    } else if (key == LBMK_OPT_STEPPING) {
+        if (value < LBMK_STEPPING_AUTO || value > LBMK_STEPPING_PERSISTENT) return fail(g, LBMK_EINVAL, "unknown stepping mode");
+        g->opt_stepping = value;
     } else {
         return fail(g, LBMK_EINVAL, "unknown option");
     }
@@ -362,6 +399,7 @@ lbmk_status lbmk_grid_set_option(lbmk_grid* g, lbmk_option key, long long value)
 
 // ------------------------------------------------------------------------------------------------ sub-domains / slabs
 static lbmk_status need_inited(lbmk_grid* g);
+static lbmk_status need_bound(lbmk_grid* g);
 lbmk_status lbmk_grid_set_origin(lbmk_grid* g, int ox, int oy, int oz) {
     if (!g) return sys_fail(LBMK_EINVAL, "grid is NULL");
     if (g->bound) return fail(g, LBMK_ESTATE, "the origin must be set before the workspace is bound");
@@ -382,6 +420,7 @@ lbmk_status lbmk_grid_set_slab(lbmk_grid* g, int enable) {
         layout(g);
     }
     c.Pd.ghost = c.Pf.ghost = enable ? 1 : 0;
+    resolve_options(g);
     return LBMK_OK;
 }
 
@@ -394,10 +433,11 @@ lbmk_status lbmk_halo_bytes(const lbmk_grid* g, size_t* bytes) {
     return LBMK_OK;
 }
 
-static lbmk_status halo_move(lbmk_grid* g, void* lo, void* hi, const bool PACK) {
+static lbmk_status halo_move(lbmk_grid* g, void* lo, void* hi, const bool PACK, void* on_stream) {
     lbmk_status s = need_inited(g);
     if (s != LBMK_OK) return s;
     GridCore& c = g->c;
+    const cudaStream_t hs = on_stream ? (cudaStream_t)on_stream : c.stream;
     if (!c.Pd.ghost) return fail(g, LBMK_ESTATE, "not a slab (lbmk_grid_set_slab)");
     if (!lo || !hi) return fail(g, LBMK_EINVAL, "halo buffer is NULL");
     if (!c.pending) return fail(g, LBMK_ESTATE, "halo exchange is defined after at least one step (initialise the ghost planes through lbmk_init_from_U)");
@@ -415,26 +455,64 @@ static lbmk_status halo_move(lbmk_grid* g, void* lo, void* hi, const bool PACK) 
     const long long planes[2] = {plane_lo, plane_hi};
     for (int e = 0; e < 2; ++e) {
         if (c.prec == PREC_F64) {
-            if (PACK) halo_kernel<double, true><<<nb, 256, 0, c.stream>>>((double*)c.f[c.cur], (double*)bufs[e], M, Q, slots[e], planes[e] * pn, pn);
-            else halo_kernel<double, false><<<nb, 256, 0, c.stream>>>((double*)c.f[c.cur], (double*)bufs[e], M, Q, slots[e], planes[e] * pn, pn);
+            if (PACK) halo_kernel<double, true><<<nb, 256, 0, hs>>>((double*)c.f[c.cur], (double*)bufs[e], M, Q, slots[e], planes[e] * pn, pn);
+            else halo_kernel<double, false><<<nb, 256, 0, hs>>>((double*)c.f[c.cur], (double*)bufs[e], M, Q, slots[e], planes[e] * pn, pn);
         } else {
-            if (PACK) halo_kernel<float, true><<<nb, 256, 0, c.stream>>>((float*)c.f[c.cur], (float*)bufs[e], M, Q, slots[e], planes[e] * pn, pn);
-            else halo_kernel<float, false><<<nb, 256, 0, c.stream>>>((float*)c.f[c.cur], (float*)bufs[e], M, Q, slots[e], planes[e] * pn, pn);
+            if (PACK) halo_kernel<float, true><<<nb, 256, 0, hs>>>((float*)c.f[c.cur], (float*)bufs[e], M, Q, slots[e], planes[e] * pn, pn);
+            else halo_kernel<float, false><<<nb, 256, 0, hs>>>((float*)c.f[c.cur], (float*)bufs[e], M, Q, slots[e], planes[e] * pn, pn);
         }
     }
     c.launches += 2;
     CK(g, cudaGetLastError(), "halo kernel");
     return LBMK_OK;
 }
-lbmk_status lbmk_halo_pack(lbmk_grid* g, void* send_lo, void* send_hi) { return halo_move(g, send_lo, send_hi, true); }
+lbmk_status lbmk_halo_pack(lbmk_grid* g, void* send_lo, void* send_hi) { return halo_move(g, send_lo, send_hi, true, nullptr); }
 lbmk_status lbmk_halo_unpack(lbmk_grid* g, const void* recv_lo, const void* recv_hi) {
-    return halo_move(g, const_cast<void*>(recv_lo), const_cast<void*>(recv_hi), false);
+    return halo_move(g, const_cast<void*>(recv_lo), const_cast<void*>(recv_hi), false, nullptr);
+}
+lbmk_status lbmk_halo_pack_on(lbmk_grid* g, void* send_lo, void* send_hi, void* cuda_stream) { return halo_move(g, send_lo, send_hi, true, cuda_stream); }
+lbmk_status lbmk_halo_unpack_on(lbmk_grid* g, const void* recv_lo, const void* recv_hi, void* cuda_stream) {
+    return halo_move(g, const_cast<void*>(recv_lo), const_cast<void*>(recv_hi), false, cuda_stream);
+}
+
+// One step of a slab, boundary planes first: [first own plane] [last own plane] -> boundary event -> [interior planes].
+// The ghost planes are not updated (their face-crossing slots arrive through the halo exchange).
+lbmk_status lbmk_step_slab(lbmk_grid* g) {
+    lbmk_status s = need_inited(g);
+    if (s != LBMK_OK) return s;
+    GridCore& c = g->c;
+    if (!c.Pd.ghost) return fail(g, LBMK_ESTATE, "not a slab (lbmk_grid_set_slab)");
+    const long long pn = plane_nodes_of(g);
+    const int np = planes_of(g);
+    long long r[6];
+    r[0] = pn; r[1] = 2 * pn;                                           // first own plane
+    r[2] = np > 3 ? (long long)(np - 2) * pn : 0; r[3] = np > 3 ? (long long)(np - 1) * pn : 0;   // last own plane (if distinct)
+    r[4] = np > 4 ? 2 * pn : 0; r[5] = np > 4 ? (long long)(np - 2) * pn : 0;                      // interior
+    CK(g, cudaEventRecord(g->ev0, c.stream), "cudaEventRecord");
+    CK(g, g->ops->step_ranges(c, r, g->ev_boundary), "collide_stream launch (slab)");
+    CK(g, cudaEventRecord(g->ev1, c.stream), "cudaEventRecord");
+    g->timed = true;
+    return LBMK_OK;
+}
+lbmk_status lbmk_stream_wait_boundary(lbmk_grid* g, void* cuda_stream) {
+    lbmk_status s = need_inited(g);
+    if (s != LBMK_OK) return s;
+    CK(g, cudaStreamWaitEvent((cudaStream_t)cuda_stream, g->ev_boundary, 0), "cudaStreamWaitEvent");
+    return LBMK_OK;
+}
+lbmk_status lbmk_grid_wait_stream(lbmk_grid* g, void* cuda_stream) {
+    lbmk_status s = need_bound(g);
+    if (s != LBMK_OK) return s;
+    CK(g, cudaEventRecord(g->ev_join, (cudaStream_t)cuda_stream), "cudaEventRecord");
+    CK(g, cudaStreamWaitEvent(g->c.stream, g->ev_join, 0), "cudaStreamWaitEvent");
+    return LBMK_OK;
 }
 
 lbmk_status lbmk_grid_get_option(const lbmk_grid* g, lbmk_option key, long long* value) {
     if (!g || !value) return sys_fail(LBMK_EINVAL, "NULL argument");
     if (key == LBMK_OPT_PATTERN) *value = g->c.pattern;
     else if (key == LBMK_OPT_KERNEL) *value = g->c.kernel;
+    else if (key == LBMK_OPT_STEPPING) *value = g->c.stepping;
     else return sys_fail(LBMK_EINVAL, "unknown option");
     return LBMK_OK;
 }
@@ -462,7 +540,16 @@ lbmk_status lbmk_grid_bind_workspace(lbmk_grid* g, void* device_ptr, size_t byte
     c.coef = base + g->off_coef;
     c.feq0 = (double*)(base + g->off_feq0);
     c.red = (unsigned long long*)(base + g->off_red);
+    c.bar = (unsigned int*)(base + g->off_red + 64);
+    c.aux_buf = g->ops->n_aux > 0 ? base + g->off_aux : nullptr;
+    c.aux_set = false;
     c.cur = 0;
+    {
+        int dev = 0, sms = 0;
+        CK(g, cudaGetDevice(&dev), "cudaGetDevice");
+        CK(g, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev), "cudaDeviceGetAttribute");
+        c.num_sms = sms;
+    }
     CK(g, g->ops->fill_tables(c), "fill_tables");
     CK(g, g->ops->reference_equilibrium(c), "reference_equilibrium");
     if (!g->have_events) {
@@ -470,6 +557,8 @@ lbmk_status lbmk_grid_bind_workspace(lbmk_grid* g, void* device_ptr, size_t byte
         CK(g, cudaEventCreate(&g->ev1), "cudaEventCreate");
         CK(g, cudaStreamCreateWithFlags(&c.aux, cudaStreamNonBlocking), "cudaStreamCreate");
         CK(g, cudaEventCreateWithFlags(&c.ev_entry, cudaEventDisableTiming), "cudaEventCreate");
+        CK(g, cudaEventCreateWithFlags(&g->ev_boundary, cudaEventDisableTiming), "cudaEventCreate");
+        CK(g, cudaEventCreateWithFlags(&g->ev_join, cudaEventDisableTiming), "cudaEventCreate");
         for (int b = 0; b < 2; ++b) {
             CK(g, cudaEventCreateWithFlags(&c.ev_coef[b], cudaEventDisableTiming), "cudaEventCreate");
             CK(g, cudaEventCreateWithFlags(&c.ev_free[b], cudaEventDisableTiming), "cudaEventCreate");
@@ -486,6 +575,7 @@ void lbmk_grid_destroy(lbmk_grid* g) {
     if (g->have_events) {
         cudaStreamSynchronize(g->c.aux);
         cudaEventDestroy(g->ev0); cudaEventDestroy(g->ev1); cudaEventDestroy(g->c.ev_entry);
+        cudaEventDestroy(g->ev_boundary); cudaEventDestroy(g->ev_join);
         for (int b = 0; b < 2; ++b) { cudaEventDestroy(g->c.ev_coef[b]); cudaEventDestroy(g->c.ev_free[b]); }
         cudaStreamDestroy(g->c.aux);
     }
@@ -532,6 +622,7 @@ lbmk_status lbmk_init_from_U(lbmk_grid* g, const double* U, int on_device, doubl
     if (s != LBMK_OK) return s;
     if (!U) return fail(g, LBMK_EINVAL, "U is NULL");
     GridCore& c = g->c;
+    if (g->ops->n_aux > 0 && !c.aux_set) return fail(g, LBMK_ESTATE, "this system has prescribed coefficient fields: call lbmk_set_aux_fields first");
     const size_t bytes = (size_t)g->ops->M * c.n * sizeof(double);
     Staging st;
     CK(g, st.acquire(U, on_device, bytes, true, c.stream), "stage U");
@@ -543,11 +634,27 @@ lbmk_status lbmk_init_from_U(lbmk_grid* g, const double* U, int on_device, doubl
     return LBMK_OK;
 }
 
+lbmk_status lbmk_set_aux_fields(lbmk_grid* g, const double* A, int on_device) {
+    lbmk_status s = need_bound(g);
+    if (s != LBMK_OK) return s;
+    if (!A) return fail(g, LBMK_EINVAL, "A is NULL");
+    if (g->ops->n_aux == 0) return fail(g, LBMK_EUNSUPPORTED, "this system has no prescribed coefficient fields");
+    GridCore& c = g->c;
+    const size_t bytes = (size_t)g->ops->n_aux * c.n * sizeof(double);
+    Staging st;
+    CK(g, st.acquire(A, on_device, bytes, true, c.stream), "stage A");
+    CK(g, g->ops->set_aux(c, (const double*)st.dev), "set_aux kernel");
+    CK(g, st.release(), "cudaFreeAsync");
+    if (!on_device) CK(g, cudaStreamSynchronize(c.stream), "cudaStreamSynchronize");
+    return LBMK_OK;
+}
+
 lbmk_status lbmk_set_populations(lbmk_grid* g, const double* f, int on_device, double t0) {
     lbmk_status s = need_bound(g);
     if (s != LBMK_OK) return s;
     if (!f) return fail(g, LBMK_EINVAL, "f is NULL");
     GridCore& c = g->c;
+    if (g->ops->n_aux > 0 && !c.aux_set) return fail(g, LBMK_ESTATE, "this system has prescribed coefficient fields: call lbmk_set_aux_fields first");
     const size_t bytes = (size_t)g->ops->M * (2 * g->ops->D + 1) * c.n * sizeof(double);
     Staging st;
     CK(g, st.acquire(f, on_device, bytes, true, c.stream), "stage f");

@@ -10,6 +10,7 @@ namespace lbmk {
 enum { PREC_F64 = 0, PREC_F32 = 1 };
 enum { PATTERN_PULL2 = 1, PATTERN_AA = 2 };
 enum { KERNEL_NODE = 1, KERNEL_ROW = 2, KERNEL_TWOPASS = 3 };
+enum { STEPPING_LAUNCH = 1, STEPPING_PERSISTENT = 2 };
 
 struct GridCore {
     int nx, ny, nz;
@@ -32,6 +33,13 @@ struct GridCore {
     bool coef_used[2];
     double* feq0;         // [M*Q] reference equilibrium (fp64)
     unsigned long long* red;   // [4] reduction scratch
+    unsigned int* bar;    // grid-barrier counter of the persistent kernel (zeroed before each launch)
+    void* aux_buf;        // prescribed coefficient fields in R, [n_aux][aux_stride]
+    long long aux_stride;
+    bool aux_set;
+    int stepping;         // STEPPING_LAUNCH: one launch per step; STEPPING_PERSISTENT: one cooperative launch per batch of steps
+    int num_sms;          // cudaDevAttrMultiProcessorCount of the current device
+    long long persistent_launches;   // cooperative launches so far (diagnostic)
     KParams<double> Pd;   // parameters in fp64 (host logic, fp64 kernels, readback)
     KParams<float> Pf;    // same, rounded to fp32 (fp32 kernels)
     MmsHostArgs mh;
@@ -43,12 +51,17 @@ struct SysOps {
     bool has_mms;
     int nt, nax[3];       // time scalars and table entries per axis of the manufactured solution
     int nc;               // per-row forcing coefficients (multiple of 4; 0 without manufactured solution)
+    int n_aux;            // prescribed per-node coefficient fields
     // all return cudaError_t of the last launch / API call
     cudaError_t (*fill_tables)(GridCore&);                 // host fp64 -> device R tables (synchronous copy on the stream)
     cudaError_t (*reference_equilibrium)(GridCore&);
     cudaError_t (*init_from_U)(GridCore&, const double* U_dev);
     cudaError_t (*set_f)(GridCore&, const double* f_dev);
     cudaError_t (*step)(GridCore&, int n_steps);
+    // one step in up to 3 launches: nodes [a0,a1) and [b0,b1) first (the slab's boundary planes), then `ev` is recorded on
+    // the stream, then [c0,c1) (the interior); empty ranges are skipped
+    cudaError_t (*step_ranges)(GridCore&, const long long* ranges6, cudaEvent_t ev);
+    cudaError_t (*set_aux)(GridCore&, const double* A_dev);
     cudaError_t (*read_U)(GridCore&, double* U_dev);
     cudaError_t (*read_f)(GridCore&, double* f_dev);
     cudaError_t (*max_wave_speed)(GridCore&, double* out3_host);
@@ -69,5 +82,8 @@ const SysOps* ops_allencahn2d();
 const SysOps* ops_inse2d();
 const SysOps* ops_elasticity2d();
 const SysOps* ops_nsf2d();
+const SysOps* ops_swe2d_bathy();
+const SysOps* ops_hcnsf3d();
+const SysOps* ops_mhd2d();
 
 }  // namespace lbmk

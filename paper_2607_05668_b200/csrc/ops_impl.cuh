@@ -18,11 +18,17 @@ template <template <class> class S, class R> struct Tune { static constexpr int 
 template <class R> struct Tune<SysNsf3D, R> { static constexpr int BLOCK = 64, MINB = 6; };
 template <> struct Tune<SysNsf3D, double> { static constexpr int BLOCK = 128, MINB = 1; };
 template <class R> struct Tune<SysMhd3D, R> { static constexpr int BLOCK = 64, MINB = 4; };
+template <class R> struct Tune<SysHcnsf3D, R> { static constexpr int BLOCK = 64, MINB = 6; };
+template <> struct Tune<SysHcnsf3D, double> { static constexpr int BLOCK = 128, MINB = 1; };
+template <class R> struct Tune<SysMhd2D, R> { static constexpr int BLOCK = 128, MINB = 3; };
+template <> struct Tune<SysMhd2D, double> { static constexpr int BLOCK = 128, MINB = 1; };
 
 // two-pass kernel: register cap via min blocks per SM
 template <template <class> class S, class R> struct Tune2 { static constexpr int BLOCK = 256, MINB = 2; };
 template <class R> struct Tune2<SysNsf3D, R> { static constexpr int BLOCK = 128, MINB = 4; };
 template <class R> struct Tune2<SysMhd3D, R> { static constexpr int BLOCK = 128, MINB = 4; };
+template <class R> struct Tune2<SysHcnsf3D, R> { static constexpr int BLOCK = 128, MINB = 4; };
+template <class R> struct Tune2<SysMhd2D, R> { static constexpr int BLOCK = 128, MINB = 4; };
 
 template <class Mm> struct MmsCounts { static constexpr int NT = Mm::NT, NX = Mm::NX, NY = Mm::NY, NZ = Mm::NZ, NC = Mm::NC; };
 template <> struct MmsCounts<void> { static constexpr int NT = 0, NX = 0, NY = 0, NZ = 0, NC = 0; };
@@ -34,6 +40,7 @@ struct Ops {
     using Sd = S<double>;
     static constexpr int D = Sd::D, Q = 2 * D + 1, M = Sd::M;
     static constexpr bool HAS_MMS = has_mms<Sd>();
+    static constexpr int NA = AuxCount<Sd>::value;
 
     using C = MmsCounts<typename Sd::Mms>;
 
@@ -67,6 +74,11 @@ struct Ops {
             kp<R>(g).tabX = (const R*)g.tab[0]; kp<R>(g).tabY = (const R*)g.tab[1]; kp<R>(g).tabZ = (const R*)g.tab[2];
             kp<R>(g).coef = (const R*)g.coef;
         }
+        kp<R>(g).aux = (const R*)g.aux_buf;
+        kp<R>(g).aux_stride = g.aux_stride;
+        kp<R>(g).node0 = 0;
+        kp<R>(g).node1 = g.n;
+        if (g.prec != PREC_F64) { g.Pd.node0 = 0; g.Pd.node1 = g.n; }
         return cudaSuccess;
     }
     static cudaError_t fill_tables(GridCore& g) { return g.prec == PREC_F64 ? fill_tables_t<double>(g) : fill_tables_t<float>(g); }
@@ -100,6 +112,18 @@ struct Ops {
     }
     static cudaError_t set_f(GridCore& g, const double* f) { return g.prec == PREC_F64 ? set_f_t<double>(g, f) : set_f_t<float>(g, f); }
 
+    template <class R>
+    static cudaError_t set_aux_t(GridCore& g, const double* A) {
+        if constexpr (NA > 0) {
+            set_aux_kernel<R><<<blocks_for(g.n, 256), 256, 0, g.stream>>>(A, (R*)g.aux_buf, NA, g.n, g.aux_stride);
+            g.launches++;
+            g.aux_set = true;
+            return cudaGetLastError();
+        }
+        return cudaErrorNotSupported;
+    }
+    static cudaError_t set_aux(GridCore& g, const double* A) { return g.prec == PREC_F64 ? set_aux_t<double>(g, A) : set_aux_t<float>(g, A); }
+
     // where the canonical population sits in the current storage (kernels.cuh GATHER_*)
     static int aa_odd(const GridCore& g) {
         if (g.pattern == PATTERN_AA) return (g.step & 1) ? GATHER_AA_ODD : GATHER_CANON;
@@ -126,7 +150,7 @@ struct Ops {
     static cudaError_t wave_t(GridCore& g, double* out3) {
         cudaError_t e = cudaMemsetAsync(g.red, 0, 4 * sizeof(unsigned long long), g.stream);
         if (e != cudaSuccess) return e;
-        const unsigned nb = (unsigned)std::min<long long>((g.n + 255) / 256, 148 * 8);
+        const unsigned nb = (unsigned)std::min<long long>((g.n + 255) / 256, (long long)g.num_sms * 8);
         max_wave_speed_kernel<Sd, R><<<nb, 256, 0, g.stream>>>((const R*)g.f[g.cur], g.red, g.n, g.nx, g.ny, g.nz, aa_odd(g), g.Pd);
         g.launches++;
         e = cudaGetLastError();
@@ -142,16 +166,55 @@ struct Ops {
     static cudaError_t max_wave_speed(GridCore& g, double* out3) { return g.prec == PREC_F64 ? wave_t<double>(g, out3) : wave_t<float>(g, out3); }
 
     // ---- the step
+    // launches over the node range [kp.node0, kp.node1) (whole grid unless step_ranges narrowed it)
     template <class R, int MODE, bool MMS>
     static void launch_node(GridCore& g, const R* src, R* dst) {
         constexpr int BLOCK = Tune<S, R>::BLOCK, MINB = Tune<S, R>::MINB;
+        const long long cnt = kp<R>(g).node1 - kp<R>(g).node0;
+        if (cnt <= 0) return;
         if (g.kernel == KERNEL_TWOPASS) {
             constexpr int B2 = Tune2<S, R>::BLOCK, M2 = Tune2<S, R>::MINB;
-            collide_stream_twopass<S<R>, R, MODE, MMS, B2, M2><<<blocks_for(g.n, B2), B2, 0, g.stream>>>(src, dst, kp<R>(g));
+            collide_stream_twopass<S<R>, R, MODE, MMS, B2, M2><<<blocks_for(cnt, B2), B2, 0, g.stream>>>(src, dst, kp<R>(g));
         } else {
-            collide_stream_node<S<R>, R, MODE, MMS, BLOCK, MINB><<<blocks_for(g.n, BLOCK), BLOCK, 0, g.stream>>>(src, dst, kp<R>(g));
+            collide_stream_node<S<R>, R, MODE, MMS, BLOCK, MINB><<<blocks_for(cnt, BLOCK), BLOCK, 0, g.stream>>>(src, dst, kp<R>(g));
         }
         g.launches++;
+    }
+    // ---- persistent stepping: `cnt` steps of the two-lattice pull pattern in ONE cooperative launch (kernels.cuh)
+    template <class R, bool MMS>
+    static int persistent_grid(GridCore& g) {
+        constexpr int BLOCK = Tune<S, R>::BLOCK, MINB = Tune<S, R>::MINB;
+        int per_sm = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, collide_stream_persistent<S<R>, R, MMS, BLOCK, MINB>, BLOCK, 0) != cudaSuccess) return 0;
+        const long long cap = (long long)per_sm * g.num_sms, nseg = (g.n + BLOCK - 1) / BLOCK;
+        if (cap <= 0) return 0;
+        const long long rounds = (nseg + cap - 1) / cap;          // segments per block and step
+        return (int)((nseg + rounds - 1) / rounds);               // balanced: every block takes `rounds` (or rounds-1) segments
+    }
+    template <class R, bool MMS>
+    static cudaError_t launch_persistent(GridCore& g, int cnt, long long coef_stride) {
+        constexpr int BLOCK = Tune<S, R>::BLOCK, MINB = Tune<S, R>::MINB;
+        const int grid = persistent_grid<R, MMS>(g);
+        if (grid <= 0) return cudaErrorLaunchOutOfResources;
+        cudaError_t e = cudaMemsetAsync(g.bar, 0, sizeof(unsigned int), g.stream);
+        if (e != cudaSuccess) return e;
+        R* fa = (R*)g.f[g.cur];
+        R* fb = (R*)g.f[g.cur ^ 1];
+        KParams<R> P = kp<R>(g);
+        int first_local = g.pending ? 0 : 1;
+        unsigned int* bar = g.bar;
+        void* args[] = {&fa, &fb, &P, &cnt, &first_local, &coef_stride, &bar};
+        e = cudaLaunchCooperativeKernel((const void*)collide_stream_persistent<S<R>, R, MMS, BLOCK, MINB>, dim3(grid), dim3(BLOCK), args, 0, g.stream);
+        if (e != cudaSuccess) return e;
+        g.launches++;
+        g.persistent_launches++;
+        g.cur ^= (cnt & 1);
+        g.pending = 1;
+        g.step += cnt;
+        return cudaSuccess;
+    }
+    static bool use_persistent(const GridCore& g, int n_steps) {
+        return g.stepping == STEPPING_PERSISTENT && g.pattern == PATTERN_PULL2 && g.kernel == KERNEL_NODE && g.bc == 0 && n_steps >= 2;
     }
     // one collide-and-stream launch (plus the Dirichlet frame refill before it on bounded grids)
     template <class R, bool MMS>
@@ -188,6 +251,15 @@ struct Ops {
     template <class R, bool MMS>
     static cudaError_t step_t(GridCore& g, int n_steps) {
         if constexpr (!MMS) {
+            if (use_persistent(g, n_steps)) {
+                for (int done = 0; done < n_steps;) {
+                    const int cnt = std::min(n_steps - done, 1 << 16);      // bounds the 32-bit barrier count
+                    cudaError_t e = launch_persistent<R, false>(g, cnt, 0);
+                    if (e != cudaSuccess) return e;
+                    done += cnt;
+                }
+                return cudaGetLastError();
+            }
             for (int s = 0; s < n_steps; ++s) one_step<R, false>(g);
             return cudaGetLastError();
         } else {
@@ -212,9 +284,15 @@ struct Ops {
                 }
                 e = cudaStreamWaitEvent(g.stream, g.ev_coef[buf], 0);
                 if (e != cudaSuccess) return e;
-                for (int j = 0; j < cnt; ++j) {
-                    kp<R>(g).coef = (const R*)g.coef + ((size_t)buf * B + j) * rows * C::NC;
-                    one_step<R, true>(g);
+                if (use_persistent(g, cnt)) {          // the whole batch of steps in one cooperative launch
+                    kp<R>(g).coef = (const R*)g.coef + (size_t)buf * B * rows * C::NC;
+                    e = launch_persistent<R, true>(g, cnt, rows * C::NC);
+                    if (e != cudaSuccess) return e;
+                } else {
+                    for (int j = 0; j < cnt; ++j) {
+                        kp<R>(g).coef = (const R*)g.coef + ((size_t)buf * B + j) * rows * C::NC;
+                        one_step<R, true>(g);
+                    }
                 }
                 cudaEventRecord(g.ev_free[buf], g.stream);
                 g.coef_used[buf] = true;
@@ -230,6 +308,48 @@ struct Ops {
             if (mms) return g.prec == PREC_F64 ? step_t<double, true>(g, n_steps) : step_t<float, true>(g, n_steps);
         }
         return g.prec == PREC_F64 ? step_t<double, false>(g, n_steps) : step_t<float, false>(g, n_steps);
+    }
+    // One step of a slab split into its boundary planes (two ranges) and its interior (third range): the boundary ranges
+    // go first and `ev` marks their completion, so that the halo exchange can run while the interior is updated.
+    template <class R, bool MMS>
+    static cudaError_t step_ranges_t(GridCore& g, const long long* r, cudaEvent_t ev) {
+        if (g.pattern != PATTERN_PULL2 || g.bc != 0) return cudaErrorNotSupported;
+        const int buf = (int)(g.step & 1);
+        if constexpr (MMS) {
+            // this step's row coefficients on the auxiliary stream, double-buffered by step parity: the pre-kernel of
+            // step s runs under the kernels of step s-1
+            const long long rows = (long long)g.ny * g.nz;
+            cudaError_t e = cudaSuccess;
+            if (g.coef_used[buf]) e = cudaStreamWaitEvent(g.aux, g.ev_free[buf], 0);
+            else { e = cudaEventRecord(g.ev_entry, g.stream); if (e == cudaSuccess) e = cudaStreamWaitEvent(g.aux, g.ev_entry, 0); }
+            if (e != cudaSuccess) return e;
+            launch_coeffs<R>(g, buf, g.step, 1);
+            cudaEventRecord(g.ev_coef[buf], g.aux);
+            e = cudaStreamWaitEvent(g.stream, g.ev_coef[buf], 0);
+            if (e != cudaSuccess) return e;
+            kp<R>(g).coef = (const R*)g.coef + (size_t)buf * g.coef_B * rows * C::NC;
+        }
+        const R* src = (const R*)g.f[g.cur];
+        R* dst = (R*)g.f[g.cur ^ 1];
+        for (int q = 0; q < 3; ++q) {
+            kp<R>(g).node0 = r[2 * q]; kp<R>(g).node1 = r[2 * q + 1];
+            if (g.pending) launch_node<R, MODE_PULL2, MMS>(g, src, dst);
+            else launch_node<R, MODE_LOCAL, MMS>(g, src, dst);
+            if (q == 1 && ev) cudaEventRecord(ev, g.stream);
+        }
+        kp<R>(g).node0 = 0; kp<R>(g).node1 = g.n;
+        if constexpr (MMS) { cudaEventRecord(g.ev_free[buf], g.stream); g.coef_used[buf] = true; }
+        g.cur ^= 1;
+        g.pending = 1;
+        g.step++;
+        return cudaGetLastError();
+    }
+    static cudaError_t step_ranges(GridCore& g, const long long* r, cudaEvent_t ev) {
+        const bool mms = HAS_MMS && g.mms_id != 0;
+        if constexpr (HAS_MMS) {
+            if (mms) return g.prec == PREC_F64 ? step_ranges_t<double, true>(g, r, ev) : step_ranges_t<float, true>(g, r, ev);
+        }
+        return g.prec == PREC_F64 ? step_ranges_t<double, false>(g, r, ev) : step_ranges_t<float, false>(g, r, ev);
     }
     // Dirichlet frame refresh before readback (the oracle does the same in orc_read_U)
     static cudaError_t frame_now(GridCore& g) {
@@ -252,7 +372,7 @@ struct Ops {
     static cudaError_t norms_t(GridCore& g, double* out) {
         cudaError_t e = cudaMemsetAsync(out, 0, (size_t)M * 6 * sizeof(double), g.stream);
         if (e != cudaSuccess) return e;
-        const unsigned nb = (unsigned)std::min<long long>((g.n + 255) / 256, 148 * 4);
+        const unsigned nb = (unsigned)std::min<long long>((g.n + 255) / 256, (long long)g.num_sms * 4);
         error_norms_kernel<Sd, R><<<nb, 256, 0, g.stream>>>((const R*)g.f[g.cur], out, g.n, g.nx, g.ny, g.nz, aa_odd(g),
                                                             g.t0 + (double)g.step * g.dt, g.mh, g.Pd);
         g.launches++;
@@ -267,8 +387,8 @@ struct Ops {
     static bool row_supported(const GridCore&) { return false; }
 
     static const SysOps* get() {
-        static const SysOps ops = {Sd::ID, D, M, Sd::MC, HAS_MMS, C::NT, {C::NX, C::NY, C::NZ}, C::NC,
-                                   &fill_tables, &reference_equilibrium, &init_from_U, &set_f, &step,
+        static const SysOps ops = {Sd::ID, D, M, Sd::MC, HAS_MMS, C::NT, {C::NX, C::NY, C::NZ}, C::NC, NA,
+                                   &fill_tables, &reference_equilibrium, &init_from_U, &set_f, &step, &step_ranges, &set_aux,
                                    &read_U_with_frame, &read_f, &max_wave_speed, &error_norms, &row_supported};
         return &ops;
     }

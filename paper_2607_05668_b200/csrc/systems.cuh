@@ -18,13 +18,16 @@
 //   setup(Ctx&, dQ[M], P)                 once per node
 //   flux<k>(Ctx, dQ, P, F[D], S)          lattice flux columns and source of component k
 //   wave(Q[M] full state, P, out[3])      physical |u_a|+c_a max, |u|+c, lattice diffusive signal speed
+// Systems with prescribed per-node coefficient fields (the bed slope of eq 3.5) also declare
+//   NA (their number), set_aux(Ctx&, A[NA]) -- called before setup with this node's values -- and default_aux(Ctx&).
 #pragma once
 #include "common.cuh"
 
 namespace lbmk {
 
 enum { SYS_ADVECTION2D = 0, SYS_BURGERS2D = 1, SYS_SWE2D = 2, SYS_EULER2D = 3, SYS_ADR2D = 4, SYS_NSF3D = 5, SYS_MHD3D = 6,
-       SYS_URF2D = 7, SYS_MAXWELL2D = 8, SYS_ALLENCAHN2D = 9, SYS_INSE2D = 10, SYS_ELASTICITY2D = 11, SYS_NSF2D = 12 };
+       SYS_URF2D = 7, SYS_MAXWELL2D = 8, SYS_ALLENCAHN2D = 9, SYS_INSE2D = 10, SYS_ELASTICITY2D = 11, SYS_NSF2D = 12,
+       SYS_SWE2D_BATHY = 13, SYS_HCNSF3D = 14, SYS_MHD2D = 15 };
 
 // ------------------------------------------------------------------------------------------ advection
 // Phi = (a_x U, a_y U); par = {a_x, a_y}
@@ -573,6 +576,232 @@ template <class R> struct SysMaxwell2D {
     }
     __device__ static void wave(const double*, const KParams<double>& P, double* out) {
         out[0] = fabs(P.par[0]); out[1] = fabs(P.par[0]); out[2] = 0.0;    // eigenvalues {+c, -c, 0}
+    }
+};
+
+// ------------------------------------------------------------------------------------------ shallow water over a bed
+// eq (3.5)-(3.6): the SWE flux plus S = (0, -g h grad z_b); the static bed enters as the prescribed
+// per-node field A = grad z_b (physical slope).  par = {g}; Q = (h, hu, hv)
+template <class R> struct SysSwe2DBathy {
+    static constexpr int ID = SYS_SWE2D_BATHY, D = 2, M = 3, MC = 3, NA = 2;
+    using Mms = Mms_swe2d_bathy;
+    struct Ctx { R u[2], du[2], dP, sl[2], gh; };
+    __device__ __forceinline__ static void set_aux(Ctx& c, const R (&A)[NA]) { c.sl[0] = A[0]; c.sl[1] = A[1]; }
+    __device__ __forceinline__ static void default_aux(Ctx& c) { c.sl[0] = R(0); c.sl[1] = R(0); }
+    __device__ __forceinline__ static void setup(Ctx& c, const R (&dQ)[M], const KParams<R>& P) {
+        const R h = P.ref[0] + dQ[0];
+        const R rh = R(1) / h;
+        for (int a = 0; a < 2; ++a) {
+            c.du[a] = (dQ[1 + a] - P.cst[a] * dQ[0]) * rh;
+            c.u[a] = P.cst[a] + c.du[a];
+        }
+        c.dP = R(0.5) * P.par[0] * dQ[0] * (R(2) * P.ref[0] + dQ[0]);
+        c.gh = (P.dt * P.par[0]) * h;
+    }
+    template <int k> __device__ __forceinline__ static void flux(const Ctx& c, const R (&dQ)[M], const KParams<R>& P, R (&F)[D], R& S) {
+        if constexpr (k == 0) {
+            F[0] = P.il * dQ[1]; F[1] = P.il * dQ[2];
+            S = R(0);
+        } else {
+            constexpr int a = k - 1;
+            for (int j = 0; j < 2; ++j) {
+                R v = dQ[1 + a] * c.u[j] + P.ref[1 + a] * c.du[j];
+                if (j == a) v += c.dP;
+                F[j] = P.il * v;
+            }
+            S = -c.gh * c.sl[a];
+        }
+    }
+    __device__ static void wave(const double* Q, const KParams<double>& P, double* out) {
+        const double cc = sqrt(P.par[0] * Q[0]), u = Q[1] / Q[0], v = Q[2] / Q[0];
+        out[0] = fmax(fabs(u), fabs(v)) + cc; out[1] = sqrt(u * u + v * v) + cc; out[2] = 0.0;
+    }
+};
+
+// ------------------------------------------------------------------------------------------ homogenized NSF 3D
+// eq (3.27) and the state/flux/source vectors below it, PAPER.md:L486-L497 (listing SM4.12): prescribed
+// porosity alpha(x,t) and solid velocity u_s(x,t) are per-node inputs A = (alpha, u_s0, u_s1, u_s2); reduced tracker
+// basis D^L = dx sym grad u [5..10: 00 11 22 01 02 12], H^L = dx grad T [11..13], T = p/rho.
+// par = {gamma, mu, kappa, eta_drag}.  Reference: rho0, E0 free; m0 = 0, trackers 0 (checked on the host).
+//   tau_ab = alpha mu_L (2 D_ab - 2/3 tr D delta_ab)
+//   dF_ma,j = (m_a u_j + delta_aj dp)/lam - tau_aj;  dF_E,j = (E0 + p0 + dE + dp) u_j/lam - tau_jb u_b - alpha kappa_L H_j
+//   dF_Dab,j = D_ab u_j/lam - (delta_ja u_b + delta_jb u_a)/(2 g_tau);  dF_Hb,j = H_b u_j/lam - delta_jb (T - T0)/g_tau
+//   s_ma = dt (1-alpha)/eta (rho u_s,a - m_a);  s_E = s_m . u;  s_D = -D/g_tau;  s_H = -H/g_tau
+template <class R> struct SysHcnsf3D {
+    static constexpr int ID = SYS_HCNSF3D, D = 3, M = 14, MC = 5, NA = 4;
+    using Mms = void;
+    struct Ctx { R al, us[3], u[3], ul[3], dp, dT, sig[6], Hh, sm[3], sE; };   // sig: xx yy zz xy xz yz (alpha included)
+    __device__ __forceinline__ static int sidx(int a, int b) { return a == b ? a : (a + b + 2); }
+    __device__ __forceinline__ static void set_aux(Ctx& c, const R (&A)[NA]) { c.al = A[0]; c.us[0] = A[1]; c.us[1] = A[2]; c.us[2] = A[3]; }
+    __device__ __forceinline__ static void default_aux(Ctx& c) { c.al = R(1); c.us[0] = c.us[1] = c.us[2] = R(0); }
+    __device__ __forceinline__ static void setup(Ctx& c, const R (&dQ)[M], const KParams<R>& P) {
+        const R rho = P.ref[0] + dQ[0];
+        const R r = R(1) / rho;
+        R ke = R(0);
+        for (int a = 0; a < 3; ++a) { c.u[a] = dQ[1 + a] * r; c.ul[a] = c.u[a] * P.il; ke += dQ[1 + a] * c.u[a]; }
+        c.dp = (P.par[0] - R(1)) * (dQ[4] - R(0.5) * ke);
+        c.dT = (c.dp - P.cst[5] * dQ[0]) * r;
+        const R amu = c.al * (P.par[1] * P.dL);
+        const R tr = (R(2.0 / 3.0) * amu) * (dQ[5] + dQ[6] + dQ[7]);
+        for (int q = 0; q < 3; ++q) c.sig[q] = R(2) * amu * dQ[5 + q] - tr;
+        for (int q = 3; q < 6; ++q) c.sig[q] = R(2) * amu * dQ[5 + q];
+        c.Hh = P.cst[4] + dQ[4] + c.dp;
+        const R drag = (R(1) - c.al) * (P.dt / P.par[3]);
+        c.sE = R(0);
+        for (int a = 0; a < 3; ++a) { c.sm[a] = drag * (rho * c.us[a] - dQ[1 + a]); c.sE += c.sm[a] * c.u[a]; }
+    }
+    template <int k> __device__ __forceinline__ static void flux(const Ctx& c, const R (&dQ)[M], const KParams<R>& P, R (&F)[D], R& S) {
+        if constexpr (k == 0) {
+            for (int j = 0; j < 3; ++j) F[j] = P.il * dQ[1 + j];
+            S = R(0);
+        } else if constexpr (k <= 3) {
+            constexpr int a = k - 1;
+            for (int j = 0; j < 3; ++j) {
+                R v = dQ[1 + a] * c.ul[j] - c.sig[sidx(a, j)];
+                if (j == a) v += P.il * c.dp;
+                F[j] = v;
+            }
+            S = c.sm[a];
+        } else if constexpr (k == 4) {
+            const R aK = c.al * (P.par[2] * P.dL);
+            for (int j = 0; j < 3; ++j)
+                F[j] = c.Hh * c.ul[j] - (c.sig[sidx(j, 0)] * c.u[0] + c.sig[sidx(j, 1)] * c.u[1] + c.sig[sidx(j, 2)] * c.u[2]) - aK * dQ[11 + j];
+            S = c.sE;
+        } else if constexpr (k < 11) {
+            // D_ab: k = 5 + q, q -> (a, b) = (0,0) (1,1) (2,2) (0,1) (0,2) (1,2)
+            constexpr int q = k - 5;
+            constexpr int a = q < 3 ? q : (q == 5 ? 1 : 0), b = q < 3 ? q : (q == 3 ? 1 : 2);
+            const R h = R(0.5) * P.inv_gtau;
+            for (int j = 0; j < 3; ++j) F[j] = dQ[k] * c.ul[j];
+            F[a] -= h * c.u[b];
+            F[b] -= h * c.u[a];
+            S = -dQ[k] * P.inv_gtau;
+        } else {
+            constexpr int b = k - 11;
+            for (int j = 0; j < 3; ++j) F[j] = dQ[k] * c.ul[j];
+            F[b] -= c.dT * P.inv_gtau;
+            S = -dQ[k] * P.inv_gtau;
+        }
+    }
+    __device__ static void wave(const double* Q, const KParams<double>& P, double* out) {
+        const double u[3] = {Q[1] / Q[0], Q[2] / Q[0], Q[3] / Q[0]};
+        const double u2 = u[0] * u[0] + u[1] * u[1] + u[2] * u[2];
+        const double p = (P.par[0] - 1.0) * (Q[4] - 0.5 * Q[0] * u2);
+        const double cc = sqrt(P.par[0] * p / Q[0]);
+        out[0] = fmax(fmax(fabs(u[0]), fabs(u[1])), fabs(u[2])) + cc;
+        out[1] = sqrt(u2) + cc;
+        const double kap = fmax(4.0 * P.par[1] * P.dL / (3.0 * Q[0]), P.par[2] * P.dL * (P.par[0] - 1.0) / Q[0]);   // alpha <= 1
+        out[2] = sqrt(kap * P.inv_gtau);
+    }
+};
+
+// ------------------------------------------------------------------------------------------ resistive MHD 2D
+// eq (3.25), PAPER.md:L469-L484 (listing SM4.11 garbled: vector form), cascade on the six conserved fields (N = 6 + 12):
+// Q = (rho, m0, m1, E, B0, B1, G^L_{V,b} = dx d_b V [index 6 + 2 v + b], V = rho, m0, m1, E, B0, B1); par = {gamma, mu, K, eta}.
+// Reference: (rho0, m0, E0, B0) free (moving, magnetised reference), trackers 0 (host-checked).  Chain rule as NSF 2D plus
+//   d_b p = (gamma-1)(G_E,b - u.G_m,b + |u|^2/2 G_rho,b - B.G_B,b),  j_z = G_B1,0 - G_B0,1,  div B = G_B0,0 + G_B1,1.
+// Delta forms (every term O(dQ)):  d(m_a u_j) = dm_a u_j + m0_a du_j;  d(B_a B_j) = dB_a B_j + B0_a dB_j;
+//   d|B|^2 = (2 B0 + dB).dB;  dp = (gamma-1)(dE - d(m.u)/2 - d|B|^2/2);  dpt = dp + d|B|^2/2;
+//   d((E+pt) u_j) = (dE + dpt) u_j + (E0 + pt0) du_j;  d(B_j (u.B)) = dB_j (u.B) + B0_j d(u.B),  d(u.B) = du.B + u0.dB.
+// Powell source -(div B)(0, B, u.B, u), read off tr G_B: state-dependent, taken at the full state.
+template <class R> struct SysMhd2D {
+    static constexpr int ID = SYS_MHD2D, D = 2, M = 18, MC = 6;
+    using Mms = Mms_mhd2d;
+    struct Ctx { R u[2], du[2], ul[2], B[2], dp_t, tau[2][2], qh[2], uB, duB, Hh, divB; };
+    __device__ __forceinline__ static void setup(Ctx& c, const R (&dQ)[M], const KParams<R>& P) {
+        const R rho = P.ref[0] + dQ[0];
+        const R r = R(1) / rho;
+        R dke = R(0), u2 = R(0), dB2 = R(0);
+        c.uB = R(0); c.duB = R(0);
+#pragma unroll
+        for (int a = 0; a < 2; ++a) {
+            c.du[a] = (dQ[1 + a] - P.cst[a] * dQ[0]) * r;
+            c.u[a] = P.cst[a] + c.du[a];
+            c.ul[a] = c.u[a] * P.il;
+            c.B[a] = P.ref[4 + a] + dQ[4 + a];
+            dke += dQ[1 + a] * c.u[a] + P.ref[1 + a] * c.du[a];
+            u2 += c.u[a] * c.u[a];
+            dB2 += (R(2) * P.ref[4 + a] + dQ[4 + a]) * dQ[4 + a];
+            c.uB += c.u[a] * c.B[a];
+            c.duB += c.du[a] * c.B[a] + P.cst[a] * dQ[4 + a];
+        }
+        const R gm1 = P.par[0] - R(1);
+        const R dp = gm1 * (dQ[3] - R(0.5) * dke - R(0.5) * dB2);
+        c.dp_t = dp + R(0.5) * dB2;
+        c.Hh = dQ[3] + c.dp_t;
+        const R T = (P.cst[3] + dp) * r;
+        const R muL = P.par[1] * P.dL, KL = P.par[2] * P.dL, etaL = P.par[3] * P.dL;
+        R gu[2][2], dT[2];
+#pragma unroll
+        for (int b = 0; b < 2; ++b) {
+            gu[0][b] = (dQ[8 + b] - c.u[0] * dQ[6 + b]) * r;
+            gu[1][b] = (dQ[10 + b] - c.u[1] * dQ[6 + b]) * r;
+            const R dpb = gm1 * (dQ[12 + b] - c.u[0] * dQ[8 + b] - c.u[1] * dQ[10 + b] + R(0.5) * u2 * dQ[6 + b]
+                                 - c.B[0] * dQ[14 + b] - c.B[1] * dQ[16 + b]);
+            dT[b] = (dpb - T * dQ[6 + b]) * r;
+        }
+        const R dv = R(2.0 / 3.0) * muL * (gu[0][0] + gu[1][1]);
+        c.tau[0][0] = R(2) * muL * gu[0][0] - dv;
+        c.tau[1][1] = R(2) * muL * gu[1][1] - dv;
+        c.tau[0][1] = c.tau[1][0] = muL * (gu[0][1] + gu[1][0]);
+        const R jz = dQ[16] - dQ[15];                     // G_B1,0 - G_B0,1
+        const R ejxB[2] = {-etaL * jz * c.B[1], etaL * jz * c.B[0]};
+#pragma unroll
+        for (int j = 0; j < 2; ++j) c.qh[j] = c.tau[j][0] * c.u[0] + c.tau[j][1] * c.u[1] + KL * dT[j] - ejxB[j];
+        c.divB = P.il * (dQ[14] + dQ[17]);
+    }
+    template <int k> __device__ __forceinline__ static void flux(const Ctx& c, const R (&dQ)[M], const KParams<R>& P, R (&F)[D], R& S) {
+        if constexpr (k == 0) {
+            F[0] = P.il * dQ[1]; F[1] = P.il * dQ[2]; S = R(0);
+        } else if constexpr (k <= 2) {
+            constexpr int a = k - 1;
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                R v = dQ[1 + a] * c.u[j] + P.ref[1 + a] * c.du[j] - (dQ[4 + a] * c.B[j] + P.ref[4 + a] * dQ[4 + j]);
+                if (j == a) v += c.dp_t;
+                F[j] = P.il * v - c.tau[a][j];
+            }
+            S = -c.divB * c.B[a];
+        } else if constexpr (k == 3) {
+#pragma unroll
+            for (int j = 0; j < 2; ++j)
+                F[j] = P.il * (c.Hh * c.u[j] + P.cst[4] * c.du[j] - (dQ[4 + j] * c.uB + P.ref[4 + j] * c.duB)) - c.qh[j];
+            S = -c.divB * c.uB;
+        } else if constexpr (k <= 5) {
+            constexpr int i = k - 4;
+            const R etaL = P.par[3] * P.dL;
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                // d(B_i u_j - u_i B_j) = dB_i u_j + B0_i du_j - du_i B_j - u0_i dB_j
+                R v = R(0);
+                if (j != i) v = dQ[4 + i] * c.u[j] + P.ref[4 + i] * c.du[j] - c.du[i] * c.B[j] - P.cst[i] * dQ[4 + j];
+                F[j] = P.il * v - etaL * dQ[6 + 2 * (4 + i) + j];
+            }
+            S = -c.divB * c.u[i];
+        } else {
+            constexpr int v = (k - 6) / 2, b = (k - 6) % 2;
+            F[0] = dQ[k] * c.ul[0]; F[1] = dQ[k] * c.ul[1];
+            F[b] -= dQ[v] * P.inv_gtau;
+            S = -dQ[k] * P.inv_gtau;
+        }
+    }
+    __device__ static void wave(const double* Q, const KParams<double>& P, double* out) {
+        const double rho = Q[0];
+        const double u[2] = {Q[1] / rho, Q[2] / rho};
+        const double u2 = u[0] * u[0] + u[1] * u[1];
+        const double B2 = Q[4] * Q[4] + Q[5] * Q[5];
+        const double p = (P.par[0] - 1.0) * (Q[3] - 0.5 * rho * u2 - 0.5 * B2);
+        const double a2 = P.par[0] * p / rho, b2 = B2 / rho;
+        double m0 = 0.0;
+        for (int a = 0; a < 2; ++a) {
+            const double ba2 = Q[4 + a] * Q[4 + a] / rho;
+            const double cf = sqrt(0.5 * (a2 + b2 + sqrt(fmax((a2 + b2) * (a2 + b2) - 4.0 * a2 * ba2, 0.0))));
+            m0 = fmax(m0, fabs(u[a]) + cf);
+        }
+        out[0] = m0;
+        out[1] = sqrt(u2) + sqrt(a2 + b2);
+        const double kap = fmax(fmax(4.0 * P.par[1] * P.dL / (3.0 * rho), P.par[2] * P.dL * (P.par[0] - 1.0) / rho), P.par[3] * P.dL);
+        out[2] = sqrt(kap * P.inv_gtau);
     }
 };
 

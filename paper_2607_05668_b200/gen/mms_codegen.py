@@ -294,8 +294,79 @@ def sys_nsf2d():
     return "nsf2d", 2, prim, build
 
 
+def sys_swe2d_bathy():
+    g = par(0)
+    h0, Ah, m0, Am, Azb, wt = mp(0), mp(1), mp(2), mp(3), mp(4), mp(5)
+    k = TWO_PI
+    prim = {"h": h0 + Ah * sp.sin(k * x) * sp.sin(k * y) * sp.cos(wt * t),            # eq SM5.3
+            "mx": m0 + Am * sp.cos(k * x) * sp.cos(k * y) * sp.sin(wt * t),
+            "my": m0 + Am * sp.sin(k * x) * sp.sin(k * y) * sp.sin(wt * t),
+            "zb": Azb * sp.sin(k * x) * sp.cos(k * y)}                                  # static bed
+
+    def build(P, D):
+        h, mx, my, zb = P["h"], P["mx"], P["my"], P["zb"]
+        u, v = mx / h, my / h
+        Pr = g * h * h / 2
+        Q = [h, mx, my]
+        F = [[il * mx, il * my],                                                        # eq 3.6
+             [il * (mx * u + Pr), il * mx * v],
+             [il * my * u, il * (my * v + Pr)]]
+        S = [sp.Integer(0), -dt * g * h * D(zb, x), -dt * g * h * D(zb, y)]           # bed source -g h grad z_b
+        return Q, F, S
+    return "swe2d_bathy", 2, prim, build
+
+
+def sys_mhd2d():
+    gamma, mu, K, eta = par(0), par(1), par(2), par(3)
+    k = TWO_PI
+    p0 = 1 / gamma                                                                            # rho0 = c_s = 1 (reading A9)
+    drho = sp.Rational(3, 10) * sp.sin(k * x) * sp.cos(k * y) * sp.cos(t)                      # SM5.12
+    prim = {"rho": 1 + drho,
+            "u0": 3 + sp.Rational(3, 10) * sp.cos(k * x) * sp.sin(k * y) * sp.sin(t),
+            "u1": 3 + sp.Rational(3, 10) * sp.sin(k * x) * sp.sin(k * y) * sp.sin(t),
+            "p": p0 + drho + sp.Rational(1, 5) * p0 * sp.cos(k * x) * sp.sin(k * y) * sp.sin(t),
+            "B0": sp.Rational(1, 2) - sp.Rational(3, 10) * sp.cos(k * x) * sp.sin(k * y) * sp.sin(t),
+            "B1": sp.Rational(1, 2) + sp.Rational(3, 10) * sp.sin(k * x) * sp.cos(k * y) * sp.sin(t)}
+
+    def build(P, D):
+        X = (x, y)
+        rho, p = P["rho"], P["p"]
+        u = [P["u0"], P["u1"]]
+        B = [P["B0"], P["B1"]]
+        T = p / rho
+        B2 = B[0]**2 + B[1]**2
+        E = p / (gamma - 1) + rho * (u[0]**2 + u[1]**2) / 2 + B2 / 2
+        pt = p + B2 / 2
+        uB = u[0] * B[0] + u[1] * B[1]
+        V = [rho, rho * u[0], rho * u[1], E, B[0], B[1]]
+        G = [[dx * D(V[v], X[b]) for b in range(2)] for v in range(6)]
+        muL, KL, etaL = mu * dt / dx**2, K * dt / dx**2, eta * dt / dx**2
+        gu = [[dx * D(u[a], X[b]) for b in range(2)] for a in range(2)]
+        gT = [dx * D(T, X[b]) for b in range(2)]
+        divu = gu[0][0] + gu[1][1]
+        tau = [[muL * (gu[a][b] + gu[b][a]) - (sp.Rational(2, 3) * muL * divu if a == b else 0) for b in range(2)] for a in range(2)]
+        jz = G[5][0] - G[4][1]
+        jxB = [-jz * B[1], jz * B[0]]
+        divB = G[4][0] + G[5][1]
+        Q = V + [G[v][b] for v in range(6) for b in range(2)]
+        F = [[il * V[1], il * V[2]]]                                                          # eq 3.25
+        for a in range(2):
+            F.append([il * (V[1 + a] * u[j] - B[a] * B[j] + (pt if a == j else 0)) - tau[a][j] for j in range(2)])
+        F.append([il * ((E + pt) * u[j] - B[j] * uB) - sum(tau[j][b] * u[b] for b in range(2)) - KL * gT[j] + etaL * jxB[j]
+                  for j in range(2)])
+        for i in range(2):
+            F.append([il * (B[i] * u[j] - u[i] * B[j]) - etaL * G[4 + i][j] for j in range(2)])
+        for v in range(6):
+            for b in range(2):
+                F.append([il * G[v][b] * u[j] - (V[v] / gtau if j == b else 0) for j in range(2)])
+        S = [sp.Integer(0), -il * divB * B[0], -il * divB * B[1], -il * divB * uB, -il * divB * u[0], -il * divB * u[1]]
+        S += [-G[v][b] / gtau for v in range(6) for b in range(2)]
+        return Q, F, S
+    return "mhd2d", 2, prim, build
+
+
 SYSTEMS = [sys_burgers2d, sys_swe2d, sys_euler2d, sys_adr2d, sys_nsf3d, sys_urf2d, sys_maxwell2d, sys_allencahn2d, sys_inse2d,
-           sys_elasticity2d, sys_nsf2d]
+           sys_elasticity2d, sys_nsf2d, sys_swe2d_bathy, sys_mhd2d]
 
 
 # ------------------------------------------------------------------------------------------------ printing
@@ -343,7 +414,7 @@ def _atom_symbol_name(f, wrt: Sequence[sp.Symbol]) -> str:
 def _separate(expr):
     """Rewrite sin/cos atoms whose argument mixes coordinates into products of single-coordinate atoms."""
     repl = {}
-    for a in expr.atoms(sp.sin, sp.cos):
+    for a in sorted(expr.atoms(sp.sin, sp.cos), key=sp.default_sort_key):
         if len(a.free_symbols & set(COORDS)) > 1:
             repl[a] = sp.expand_trig(a.func(sp.expand(a.args[0])))
     return expr.xreplace(repl) if repl else expr
@@ -384,12 +455,14 @@ def generate_system(name, dim, prim_concrete, build):
         return s
 
     def lower(e):
+        # atoms() is a set: visit it in a canonical order, so that the layer-1 list, the table indices and everything
+        # CSE'd after them do not depend on the interpreter's hash seed
         repl = {}
-        for a in e.atoms(sp.Derivative):
+        for a in sorted(e.atoms(sp.Derivative), key=sp.default_sort_key):
             repl[a] = atom_to_symbol(a)
         e = e.xreplace(repl)
         repl = {}
-        for a in e.atoms(sp.core.function.AppliedUndef):
+        for a in sorted(e.atoms(sp.core.function.AppliedUndef), key=sp.default_sort_key):
             repl[a] = atom_to_symbol(a)
         return e.xreplace(repl)
 
@@ -754,19 +827,39 @@ template <bool SH> __device__ __forceinline__ Vec4<double> ld4(const double* p) 
 """
 
 
+def _generate_one(i: int) -> str:
+    name, dim, prim, build = SYSTEMS[i]()
+    text = emit_system(generate_system(name, dim, prim, build))
+    print(f"generated {name}", file=sys.stderr)
+    return text
+
+
+def generate_text(jobs: int = 0) -> str:
+    """The whole header as one string.  Systems are generated independently (one process each when jobs != 1) and joined
+    in the fixed order of SYSTEMS; nothing in the pipeline depends on set / hash order (atoms are visited in
+    sp.default_sort_key order), so the text is a pure function of this file -- tests/test_codegen.py regenerates it
+    under a different PYTHONHASHSEED and compares it byte for byte with the tracked csrc/mms_generated.cuh."""
+    idx = list(range(len(SYSTEMS)))
+    if jobs == 1:
+        texts = [_generate_one(i) for i in idx]
+    else:
+        import multiprocessing as mpx
+        with mpx.get_context("spawn").Pool(jobs or min(len(idx), os.cpu_count() or 1)) as pool:
+            texts = pool.map(_generate_one, idx, chunksize=1)
+    parts = [HEADER]
+    for tx in texts:
+        parts.append(tx)
+        parts.append("")
+    parts.append("}  // namespace lbmk\n")
+    return "\n".join(parts)
+
+
 def main(out_path=None):
     here = os.path.dirname(os.path.abspath(__file__))
     out_path = out_path or os.path.join(os.path.dirname(here), "csrc", "mms_generated.cuh")
-    parts = [HEADER]
-    for mk in SYSTEMS:
-        name, dim, prim, build = mk()
-        g = generate_system(name, dim, prim, build)
-        parts.append(emit_system(g))
-        parts.append("")
-        print(f"generated {name}", file=sys.stderr)
-    parts.append("}  // namespace lbmk\n")
+    text = generate_text()
     with open(out_path, "w") as fh:
-        fh.write("\n".join(parts))
+        fh.write(text)
     print(out_path)
 
 

@@ -7,6 +7,11 @@ face and component: nx*ny*m_total scalars per face):
 
     lbmk_halo_pack -> exchange with the two ring neighbours -> lbmk_halo_unpack
 
+Overlap (the exchange "overlapped with the interior update"): `lbmk_step_slab` updates the two boundary
+planes first, marks them with an event and then launches the interior planes; pack, transport and unpack run on a second
+("comm") stream that waits for that event only, i.e. beside the interior launch; the next step waits for the unpack.
+Same kernels and arithmetic as the serial order: the results are equal bit for bit (tests/test_gpu_slabs.py).
+
 `HaloRing.exchange` is the transport: `torch.distributed` point-to-point (NCCL over NVLink on GPUs, gloo on CPU in
 the tests) between ring neighbours, or plain copies when the ring has one rank.  This module only marshals buffers:
 every step of the path, including packing and unpacking, runs in the kernels behind the C-ABI.
@@ -62,6 +67,7 @@ class SlabGrid:
         assert P.lbmk_halo_bytes(self.grid.h) == m * plane * (8 if dt == torch.float64 else 4)
         mk = lambda: torch.empty((m, plane), dtype=dt, device=self.grid.device)
         self.send_lo, self.send_hi, self.recv_lo, self.recv_hi = mk(), mk(), mk(), mk()
+        self.comm = torch.cuda.Stream(device=self.grid.device)      # halo pack / transport / unpack beside the interior update
 
     def init(self):
         self.grid.init_from_U(self.w.initial_U())
@@ -72,13 +78,35 @@ class SlabGrid:
     def unpack(self):
         self.P.lbmk_halo_unpack(self.grid.h, self.recv_lo.data_ptr(), self.recv_hi.data_ptr())
 
-    def step(self, n: int, ring: HaloRing):
-        """n steps, each followed by the halo exchange with the ring neighbours (all on torch's current stream)."""
+    def step(self, n: int, ring: HaloRing, overlap: bool = True):
+        """n steps, each with the halo exchange with the ring neighbours.  overlap: boundary planes first, then the
+        exchange on the comm stream while the interior planes are updated on the grid's stream; otherwise step, pack,
+        exchange, unpack in series on torch's current stream."""
+        P, h, torch = self.P, self.grid.h, self.torch
         for _ in range(n):
-            self.grid.step(1)
-            self.pack()
-            ring.exchange(self.send_lo, self.send_hi, self.recv_lo, self.recv_hi)
-            self.unpack()
+            if not overlap:
+                self.grid.step(1)
+                self.pack()
+                ring.exchange(self.send_lo, self.send_hi, self.recv_lo, self.recv_hi)
+                self.unpack()
+                continue
+            self.begin_step()
+            with torch.cuda.stream(self.comm):
+                ring.exchange(self.send_lo, self.send_hi, self.recv_lo, self.recv_hi)
+            self.end_step()
+
+    def begin_step(self):
+        """Boundary planes, [event], interior planes on the grid's stream; pack on the comm stream after the event."""
+        P, h, cs = self.P, self.grid.h, self.comm.cuda_stream
+        P.lbmk_step_slab(h)
+        P.lbmk_stream_wait_boundary(h, cs)
+        P.lbmk_halo_pack_on(h, self.send_lo.data_ptr(), self.send_hi.data_ptr(), cs)
+
+    def end_step(self):
+        """Unpack on the comm stream; the grid's stream (the next step) waits for it."""
+        P, h, cs = self.P, self.grid.h, self.comm.cuda_stream
+        P.lbmk_halo_unpack_on(h, self.recv_lo.data_ptr(), self.recv_hi.data_ptr(), cs)
+        P.lbmk_grid_wait_stream(h, cs)
 
     def read_U_interior(self):
         U = self.grid.read_U()
@@ -88,11 +116,29 @@ class SlabGrid:
         self.grid.close()
 
 
-def step_local_ring(slabs: List[SlabGrid], n: int):
+def step_local_ring(slabs: List[SlabGrid], n: int, overlap: bool = False):
     """All slabs of a ring held by ONE process on one device (tests, and N = 1 with several slabs): every slab steps
     once, then the buffers are routed exactly as HaloRing.exchange routes them between ranks.  No kernel of one slab
     waits on another slab's kernel: the routing is plain stream-ordered copies."""
     W = len(slabs)
+    if overlap:
+        torch = slabs[0].torch
+        for _ in range(n):
+            for s in slabs:
+                s.begin_step()
+            for r, s in enumerate(slabs):           # each slab's comm stream takes its neighbours' packed buffers
+                lo, hi = slabs[(r - 1) % W], slabs[(r + 1) % W]
+                s.comm.wait_stream(lo.comm)
+                s.comm.wait_stream(hi.comm)
+                with torch.cuda.stream(s.comm):
+                    s.recv_lo.copy_(lo.send_hi)
+                    s.recv_hi.copy_(hi.send_lo)
+            for r, s in enumerate(slabs):           # a neighbour's next pack must not overwrite a buffer still being copied
+                slabs[(r - 1) % W].comm.wait_stream(s.comm)
+                slabs[(r + 1) % W].comm.wait_stream(s.comm)
+            for s in slabs:
+                s.end_step()
+        return
     for _ in range(n):
         for s in slabs:
             s.grid.step(1)

@@ -27,6 +27,7 @@ PAPER = {
     "allencahn": {"phi": (7.3196e-04, 7.8653e-04), "cite": "PAPER.md:L542"},
     "elasticity": {"F": (3.1874e-05, 2.8940e-05), "v": (6.4804e-05, 4.5664e-05), "cite": "PAPER.md:L536-L539"},
     "urf": {"E": (4.3449e-06, 2.1354e-06), "S": (9.6256e-06, 6.3943e-06), "cite": "PAPER.md:L527-L529"},
+    "swe": {"h": (5.5560e-06, 2.3433e-06), "hu": (2.6837e-05, 2.0838e-05), "cite": "PAPER.md:L523-L526"},
     "maxwell": {"Ez": (2.9956e-05, 2.9956e-05), "Hx": (1.0951e-04, 1.0951e-04), "Hy": (1.1587e-05, 1.1587e-05),
                 "cite": "PAPER.md:L530-L535"},
 }
@@ -43,8 +44,10 @@ def rel_errors(U, Ue):
 
 def run_case(case, n):
     w = {"burgers": W.pin_burgers, "euler": W.pin_euler, "adr": W.pin_adr, "urf": W.pin_urf, "maxwell": W.pin_maxwell,
-         "allencahn": W.pin_allencahn, "elasticity": W.pin_elasticity}[case](n)
+         "allencahn": W.pin_allencahn, "elasticity": W.pin_elasticity, "swe": W.pin_swe}[case](n)
     g = oracle.OracleGrid.from_workload(w)
+    if g.n_aux:
+        g.set_aux(w.aux_fields())          # static bed slope
     g.init_from_U(w.initial_U())
     t0 = time.time()
     g.step(w.steps)
@@ -68,13 +71,15 @@ def run_case(case, n):
         fields = {"E": e[0], "S": (float(np.hypot(e[1][0], e[2][0])), float(np.hypot(e[1][1], e[2][1])))}
     elif case == "maxwell":
         fields = {"Ez": e[0], "Hx": e[1], "Hy": e[2]}
+    elif case == "swe":
+        fields = {"h": e[0], "hu": (float(np.hypot(e[1][0], e[2][0])), float(np.hypot(e[1][1], e[2][1])))}
     else:
         fields = {"c": e[0]}
     return {"n": n, "steps": w.steps, "t_final": t, "wall_s": round(wall, 1), "fields": fields}
 
 
 if __name__ == "__main__":
-    cases = sys.argv[1:] or ["burgers", "euler", "adr", "urf", "maxwell", "allencahn", "elasticity"]
+    cases = sys.argv[1:] or ["burgers", "euler", "adr", "urf", "maxwell", "allencahn", "elasticity", "swe"]
     path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "paper_pins.json")
     out = json.load(open(path)) if os.path.exists(path) else {}
     for case in cases:

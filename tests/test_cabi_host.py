@@ -49,12 +49,14 @@ def test_system_info_matches_workloads():
         s = P.System(name, params=_params(name), tau_R=1.0, g_tau=3.0)
         assert s.m_total == len(W.COMPONENTS[name]) and s.m_conserved == W.N_CONSERVED[name]
         assert s.Q == (5 if W.LATTICE_OF[name] == "D2Q5" else 7)
+        assert s.n_aux == len(W.AUX_FIELDS.get(name, []))          # prescribed coefficient fields
         s.close()
 
 
 def _params(name):
     return {"advection2d": [0.1, 0.05], "burgers2d": [], "swe2d": [1.0], "euler2d": [1.4], "adr2d": [0.1, -0.1, 0.01, 1.0],
-            "nsf3d": [1.4, 1e-3, 5e-3], "mhd3d": [1.4, 1e-3], "urf2d": [], "maxwell2d": [1.0], "allencahn2d": [0.01, 1.0], "inse2d": [1.0, 0.01], "elasticity2d": [1.0, 1.0, 2.0], "nsf2d": [1.4, 0.0084, 0.0416]}[name]
+            "nsf3d": [1.4, 1e-3, 5e-3], "mhd3d": [1.4, 1e-3], "urf2d": [], "maxwell2d": [1.0], "allencahn2d": [0.01, 1.0], "inse2d": [1.0, 0.01], "elasticity2d": [1.0, 1.0, 2.0], "nsf2d": [1.4, 0.0084, 0.0416],
+            "swe2d_bathy": [10.0], "hcnsf3d": [1.4, 1e-2, 1e-2, 1e-3], "mhd2d": [1.4, 0.01, 0.01, 0.01]}[name]
 
 
 def test_argument_validation():

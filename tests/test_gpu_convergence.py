@@ -24,7 +24,8 @@ def P():
 @pytest.mark.parametrize("mk,kw,steps", [
     (W.pin_burgers, dict(n=40), 30), (W.pin_euler, dict(n=36), 25), (W.pin_adr, dict(n=32), 40), (W.c2_swe, dict(n=48, ny=20), 21),
     (W.c4_nsf3d, dict(n=16, ny=12, nz=10, precision="f64"), 9), (W.c4_nsf3d, dict(n=16, ny=12, nz=10), 8),
-    (W.pin_urf, dict(n=32), 17), (W.pin_maxwell, dict(n=32), 16), (W.pin_allencahn, dict(n=32), 40), (W.pin_inse, dict(n=32), 40), (W.pin_elasticity, dict(n=32), 40), (W.pin_nsf2d, dict(n=32), 40)])
+    (W.pin_urf, dict(n=32), 17), (W.pin_maxwell, dict(n=32), 16), (W.pin_allencahn, dict(n=32), 40), (W.pin_inse, dict(n=32), 40), (W.pin_elasticity, dict(n=32), 40), (W.pin_nsf2d, dict(n=32), 40),
+    (W.pin_swe, dict(n=40), 33), (W.pin_mhd2d, dict(n=32), 40)])
 @pytest.mark.parametrize("pattern", ["pull2", "aa"])
 def test_error_norms_match_numpy(P, mk, kw, steps, pattern):
     """Device reductions vs norms formed in NumPy from the read-back state and the ORACLE's exact fields (jets)."""
@@ -68,6 +69,7 @@ TABLE2 = [
     (W.pin_adr, {"c": ((0,), 2.2901e-04, 1.2680e-04)}, "L540"),
     (W.pin_allencahn, {"phi": ((0,), 7.3196e-04, 7.8653e-04)}, "L542"),
     (W.pin_elasticity, {"F": ((0, 1, 2, 3), 3.1874e-05, 2.8940e-05), "v": ((4, 5), 6.4804e-05, 4.5664e-05)}, "L536-L539"),
+    (W.pin_swe, {"h": ((0,), 5.5560e-06, 2.3433e-06), "hu": ((1, 2), 2.6837e-05, 2.0838e-05)}, "L523-L526"),   # c2's own system, with the bed
 ]
 
 
@@ -137,6 +139,7 @@ TABLE2_EOC = [
     (W.pin_elasticity, {"F": ((0, 1, 2, 3), 2.00, 2.00), "v": ((4, 5), 2.01, 1.99)}),
     (W.pin_adr, {"c": ((0,), 2.50, 2.49)}),
     (W.pin_allencahn, {"phi": ((0,), 2.50, 2.51)}),
+    (W.pin_swe, {"h": ((0,), 1.87, 1.88), "hu": ((1, 2), 1.76, 1.70)}),
 ]
 
 

@@ -20,13 +20,15 @@ def P():
 
 
 # the slab axis spans the periodic unit box (n planes), so that the analytic ghost planes wrap
-CASES = [(W.c4_nsf3d, dict(n=13, ny=10), 3, 9), (W.c4_nsf3d, dict(n=128, ny=4, precision="f64"), 2, 5),
+CASES = [(W.pin_swe, dict(n=24), 3, 9), (W.hcnsf3d, dict(n=10, ny=6), 2, 6),      # systems with prescribed per-node fields
+         (W.c4_nsf3d, dict(n=13, ny=10), 3, 9), (W.c4_nsf3d, dict(n=128, ny=4, precision="f64"), 2, 5),
          (W.c5_mhd3d, dict(n=9, ny=10), 4, 8), (W.c2_swe, dict(n=17), 3, 11), (W.c2_swe, dict(n=256), 2, 6),
          (W.c3_euler, dict(n=32), 2, 10), (W.pin_adr, dict(n=16), 3, 12)]
 
 
+@pytest.mark.parametrize("overlap", [False, True])
 @pytest.mark.parametrize("mk,kw,world,steps", CASES)
-def test_slabs_reproduce_the_single_grid_bit_for_bit(P, mk, kw, world, steps):
+def test_slabs_reproduce_the_single_grid_bit_for_bit(P, mk, kw, world, steps, overlap):
     from paper_2607_05668_b200.slabs import SlabGrid, step_local_ring
     w = mk(**kw)
     g = P.Grid.from_workload(w, pattern="pull2")
@@ -39,7 +41,7 @@ def test_slabs_reproduce_the_single_grid_bit_for_bit(P, mk, kw, world, steps):
     slabs = [SlabGrid(P, w, r, world) for r in range(world)]
     for s in slabs:
         s.init()
-    step_local_ring(slabs, steps)
+    step_local_ring(slabs, steps, overlap=overlap)     # overlap: boundary planes first, exchange beside the interior update
     ax = 1 if w.dim == 3 else 2
     Us = np.concatenate([s.read_U_interior() for s in slabs], axis=ax)
     assert Us.shape == U.shape and np.array_equal(Us, U)
@@ -56,7 +58,8 @@ def test_slabs_reproduce_the_single_grid_bit_for_bit(P, mk, kw, world, steps):
         s.close()
 
 
-def test_one_rank_ring_equals_periodic_grid(P):
+@pytest.mark.parametrize("overlap", [False, True])
+def test_one_rank_ring_equals_periodic_grid(P, overlap):
     """world = 1: the slab's ghost planes wrap onto the slab itself through HaloRing.exchange."""
     from paper_2607_05668_b200.slabs import HaloRing, SlabGrid
     w = W.c5_mhd3d(n=10, ny=8)
@@ -67,7 +70,7 @@ def test_one_rank_ring_equals_periodic_grid(P):
     g.close()
     s = SlabGrid(P, w, 0, 1)
     s.init()
-    s.step(7, HaloRing(0, 1))
+    s.step(7, HaloRing(0, 1), overlap=overlap)
     assert np.array_equal(s.read_U_interior(), U)
     s.close()
 

@@ -23,7 +23,7 @@ import workloads as W
 HERE = os.path.dirname(os.path.abspath(__file__))
 PINS = json.load(open(os.path.join(HERE, "golden", "paper_pins.json")))
 MAKERS = {"burgers": W.pin_burgers, "euler": W.pin_euler, "adr": W.pin_adr, "urf": W.pin_urf, "maxwell": W.pin_maxwell,
-          "allencahn": W.pin_allencahn, "elasticity": W.pin_elasticity}
+          "allencahn": W.pin_allencahn, "elasticity": W.pin_elasticity, "swe": W.pin_swe}
 
 
 def _rows(case):
@@ -50,6 +50,8 @@ def test_p8_stored_n512_equals_printed_values(case):
 def _errors(case, n):
     w = MAKERS[case](n)
     g = oracle.OracleGrid.from_workload(w)
+    if g.n_aux:
+        g.set_aux(w.aux_fields())
     g.init_from_U(w.initial_U())
     g.step(w.steps)
     U = g.read_U()
@@ -80,6 +82,8 @@ def test_p8_live_n64_matches_stored_row(case):
         live = {"E": e[0], "S": (math.hypot(e[1][0], e[2][0]), math.hypot(e[1][1], e[2][1]))}
     elif case == "maxwell":
         live = {"Ez": e[0], "Hx": e[1], "Hy": e[2]}
+    elif case == "swe":
+        live = {"h": e[0], "hu": (math.hypot(e[1][0], e[2][0]), math.hypot(e[1][1], e[2][1]))}
     else:
         live = {"c": e[0]}
     for field, (linf, l2) in stored.items():
