@@ -63,11 +63,14 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=None, help="timed LBM steps (default: the config's step count, capped at 200)")
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="c4", choices=["c1", "c2", "c3", "c4", "c5"])
+    ap.add_argument("--config", default="c4", choices=["c1", "c2", "c3", "c4", "c5", "hcnsf", "mhd2d", "swe_bathy"],
+                    help="c1..c5: BASELINE.json configs; hcnsf (256^3), mhd2d, swe_bathy (4096^2): the paper's Table 3 systems added in "
+                         "round 2, shifted fp32 (profiling targets, not headline workloads)")
     ap.add_argument("--pattern", default="auto", choices=["auto", "pull2", "aa"])
     ap.add_argument("--kernel", default="auto", choices=["auto", "node", "twopass"])
     ap.add_argument("--n", type=int, default=None, help="override the grid edge (debug; the line then says so)")
-    ap.add_argument("--no-mms", action="store_true", help="c4 without manufactured forcing (the paper's Table 3 kernels carry none)")
+    ap.add_argument("--no-mms", action="store_true", help="without manufactured forcing (the paper's Table 3 kernels carry none)")
+    ap.add_argument("--stepping", default="auto", choices=["auto", "launch", "persistent"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-all-configs", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -87,7 +90,14 @@ def make_workload(name, n=None, mms=True):
         kw["n"] = n
     if name == "c4" and not mms:
         kw["mms"] = False
-    return W.BASELINE_CONFIGS[name](**kw)
+    if name in W.BASELINE_CONFIGS:
+        w = W.BASELINE_CONFIGS[name](**kw)
+    else:
+        mk, n0 = {"hcnsf": (W.hcnsf3d, 256), "mhd2d": (W.pin_mhd2d, 4096), "swe_bathy": (W.pin_swe, 4096)}[name]
+        w = W.relabel(mk(n or n0, precision="f32s"), steps=200)
+    if not mms and w.mms_id:
+        w = W.relabel(w, mms_id=0)
+    return w
 
 
 def measured_peak():
@@ -411,7 +421,7 @@ def run_ours(args):
         own_nodes, U0 = g.own_nodes, g.w.initial_U()
     else:
         own_nodes, U0 = w.n_nodes, w.initial_U()
-        g = P.Grid.from_workload(w, pattern=args.pattern, kernel=args.kernel, device=dev)
+        g = P.Grid.from_workload(w, pattern=args.pattern, kernel=args.kernel, stepping=args.stepping, device=dev)
     U0_dev = torch.from_numpy(U0).to(dev)
     g.init_from_U(U0_dev)
     speeds, status = g.max_wave_speed()                      # a10: device sub-characteristic check (untimed)
