@@ -70,7 +70,7 @@ def parse_args():
     ap.add_argument("--kernel", default="auto", choices=["auto", "node", "twopass"])
     ap.add_argument("--n", type=int, default=None, help="override the grid edge (debug; the line then says so)")
     ap.add_argument("--no-mms", action="store_true", help="without manufactured forcing (the paper's Table 3 kernels carry none)")
-    ap.add_argument("--stepping", default="auto", choices=["auto", "launch", "persistent"])
+    ap.add_argument("--stepping", default="auto", choices=["auto", "launch", "persistent", "cluster"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-all-configs", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")

@@ -71,6 +71,9 @@ struct KParams {
 // number of prescribed coefficient fields of a system: Sys::NA where declared, else 0
 template <class S, class = void> struct AuxCount { static constexpr int value = 0; };
 template <class S> struct AuxCount<S, std::void_t<decltype(S::NA)>> { static constexpr int value = S::NA; };
+// systems whose flux entries are single products (Sys::LINEAR): their results do not depend on which kernel computed them
+template <class S, class = void> struct IsLinear { static constexpr bool value = false; };
+template <class S> struct IsLinear<S, std::void_t<decltype(S::LINEAR)>> { static constexpr bool value = S::LINEAR; };
 
 struct NodeIdx { int ix, iy, iz; };
 

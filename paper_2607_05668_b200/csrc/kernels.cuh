@@ -18,6 +18,8 @@
 //     (i, x) sits in slot opp(i) at x - c_i), the odd step reads that and writes slot i at x + c_i, which is
 //     canonical again.
 #pragma once
+#include <cooperative_groups.h>
+
 #include "systems.cuh"
 
 namespace lbmk {
@@ -119,6 +121,32 @@ __device__ __forceinline__ void load_aux(typename Sys::Ctx& ctx, const KParams<R
     }
 }
 
+// a3-a6 of ONE node, in registers: moments, system algebra, equilibrium + BGK relaxation component by component; `store(K, f_k)`
+// is called with the Q post-collision populations of component k as soon as they exist (so their registers die early).
+// Shared by every step kernel -- one definition of the arithmetic, hence identical bits whatever the storage.
+template <class Sys, class R, bool MMS, class Store>
+__device__ __forceinline__ void collide_core(R (&f)[Sys::M][2 * Sys::D + 1], typename Sys::Ctx& ctx, const KParams<R>& P,
+                                             const R (&smms)[Sys::M], Store&& store) {
+    constexpr int D = Sys::D, Q = 2 * D + 1, M = Sys::M;
+    R dQ[M];
+#pragma unroll
+    for (int k = 0; k < M; ++k) {
+        R s = f[k][0];
+#pragma unroll
+        for (int i = 1; i < Q; ++i) s += f[k][i];
+        dQ[k] = s;
+    }
+    Sys::setup(ctx, dQ, P);
+    static_for<0, M>([&](auto K) {
+        constexpr int k = decltype(K)::value;
+        R F[D], S;
+        Sys::template flux<k>(ctx, dQ, P, F, S);
+        if constexpr (MMS) S += smms[k];
+        relax<D, R>(f[k], P.omega[k], dQ[k], F, S);
+        store(K, f[k]);
+    });
+}
+
 // ------------------------------------------------------------------------------------------------ step
 // The update of ONE node by ONE thread (a1-a7).  `first` = first node of this thread block's BLOCK-node segment,
 // coef_s = the block's shared-memory slot for its row's forcing coefficients, coef = this step's coefficient table.
@@ -173,30 +201,16 @@ __device__ __forceinline__ void node_step(typename StepPtr<R, MODE, COHERENT>::S
             mms_node<Sys, R, false>(P, p, coef, smms);
         }
     }
-    R dQ[M];
-#pragma unroll
-    for (int k = 0; k < M; ++k) {
-        R s = f[k][0];
-#pragma unroll
-        for (int i = 1; i < Q; ++i) s += f[k][i];
-        dQ[k] = s;
-    }
-    Sys::setup(ctx, dQ, P);
-
-    static_for<0, M>([&](auto K) {
+    collide_core<Sys, R, MMS>(f, ctx, P, smms, [&](auto K, const R* fk) {
         constexpr int k = decltype(K)::value;
-        R F[D], S;
-        Sys::template flux<k>(ctx, dQ, P, F, S);
-        if constexpr (MMS) S += smms[k];
-        relax<D, R>(f[k], P.omega[k], dQ[k], F, S);
 #pragma unroll
         for (int i = 0; i < Q; ++i) {
             if constexpr (MODE == MODE_PULL2 || MODE == MODE_LOCAL) {
-                dp[(k * Q + i) * TILE] = f[k][i];
+                dp[(k * Q + i) * TILE] = fk[i];
             } else if constexpr (MODE == MODE_AA_EVEN) {
-                dp[(k * Q + opposite(i)) * TILE] = f[k][i];
+                dp[(k * Q + opposite(i)) * TILE] = fk[i];
             } else {   // AA odd: push to x + c_i; sp[opp(i)] - src + dst is that node (pull source of the opposite direction)
-                (dst + (sp[opposite(i)] - src))[(k * Q + i) * TILE] = f[k][i];
+                (dst + (sp[opposite(i)] - src))[(k * Q + i) * TILE] = fk[i];
             }
         }
     });
@@ -252,6 +266,71 @@ collide_stream_persistent(R* fa, R* fb, const __grid_constant__ KParams<R> P, in
         R* t = src; src = dst; dst = t;
         coef += coef_stride;
         if (s + 1 < nsteps) grid_barrier(bar, (unsigned)(s + 1) * gridDim.x);
+    }
+}
+
+
+// ------------------------------------------------------------------------------------------------ step, cluster-resident
+// Grids of a few thousand nodes (configs[0]: 64 x 64) do not even fill L2 lines worth a barrier through L2: ONE thread-block
+// cluster of up to 8 CTAs holds the whole population state in DISTRIBUTED SHARED MEMORY, one node per thread.  Step 0 gathers
+// from global memory (as the per-launch kernel would), the steps between go shared -> shared through two buffers per CTA -- a
+// pull across a CTA boundary is a DSMEM load from the owner CTA's buffer -- with one hardware cluster barrier per step, and the
+// last step stores to global memory in the usual post-collision form.  Arithmetic: collide_core, i.e. the same bits.
+// smem per CTA: R[2][M*Q][npc] (npc = nodes per CTA = blockDim.x).  No forcing, no prescribed fields (small tracker-free
+// systems); everything else falls back to collide_stream_persistent.
+template <class Sys, class R>
+__global__ void __launch_bounds__(1024, 1)
+collide_stream_cluster(const R* __restrict__ gsrc, R* __restrict__ gdst, const __grid_constant__ KParams<R> P, int nsteps, int first_local) {
+    namespace cg = cooperative_groups;
+    constexpr int D = Sys::D, Q = 2 * D + 1, M = Sys::M;
+    cg::cluster_group cluster = cg::this_cluster();
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    R* const sm = reinterpret_cast<R*>(smem_raw);
+    const int npc = (int)blockDim.x;
+    const int rank = (int)cluster.block_rank();
+    const long long node = (long long)rank * npc + threadIdx.x;
+    const bool active = node < P.n;
+    const long long bufsz = (long long)M * Q * npc;
+    // where this node pulls direction i from, in buffer 0 of the owner CTA (buffer 1: + bufsz); fixed for the whole launch
+    const R* sp0[Q];
+    long long goff[Q];
+    NodeIdx p = {0, 0, 0};
+    if (active) {
+        p = decompose(node, P.nx, P.ny);
+#pragma unroll
+        for (int i = 0; i < Q; ++i) {
+            const long long sn = node + pull_offset(i, p, P.nx, P.ny, P.nz);
+            const int owner = (int)(sn / npc), loc = (int)(sn - (long long)owner * npc);
+            const R* base = owner == rank ? sm : cluster.map_shared_rank(sm, owner);
+            sp0[i] = base + (long long)i * npc + loc;                     // + k*Q*npc per component
+            goff[i] = tile_off(first_local ? node : sn, M * Q);
+        }
+    }
+    cluster.sync();                                                       // every CTA of the cluster is resident before any DSMEM access
+    R smms[M];
+    for (int s = 0; s < nsteps; ++s) {
+        if (active) {
+            R f[M][Q];
+            const long long rd = ((s - 1) & 1) * bufsz;                   // step s >= 1 reads what step s-1 wrote
+#pragma unroll
+            for (int k = 0; k < M; ++k)
+#pragma unroll
+                for (int i = 0; i < Q; ++i)
+                    f[k][i] = s == 0 ? gsrc[goff[i] + (k * Q + i) * TILE] : sp0[i][rd + (long long)(k * Q) * npc];
+            typename Sys::Ctx ctx;
+            const bool last = s == nsteps - 1;
+            R* const wr = sm + (s & 1) * bufsz + threadIdx.x;
+            R* const gp = gdst + tile_off(node, M * Q);
+            collide_core<Sys, R, false>(f, ctx, P, smms, [&](auto K, const R* fk) {
+                constexpr int k = decltype(K)::value;
+#pragma unroll
+                for (int i = 0; i < Q; ++i) {
+                    if (last) gp[(k * Q + i) * TILE] = fk[i];
+                    else wr[(long long)(k * Q + i) * npc] = fk[i];
+                }
+            });
+        }
+        cluster.sync();                  // release/acquire at cluster scope: the shared-memory stores are visible to the DSMEM loads
     }
 }
 

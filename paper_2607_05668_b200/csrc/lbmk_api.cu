@@ -301,7 +301,10 @@ static void resolve_options(lbmk_grid* g) {
     const size_t esz = c.prec == PREC_F64 ? 8 : 4;
     const size_t state2 = 2 * (size_t)g->ops->M * (2 * g->ops->D + 1) * (size_t)c.n * esz;
     const bool can = c.pattern == PATTERN_PULL2 && c.kernel == KERNEL_NODE && c.bc == LBMK_PERIODIC && !c.Pd.ghost;
-    if (g->opt_stepping == LBMK_STEPPING_AUTO) c.stepping = (can && state2 <= (size_t(96) << 20)) ? STEPPING_PERSISTENT : STEPPING_LAUNCH;
+    const bool cl = can && g->ops->cluster_supported(c);
+    if (g->opt_stepping == LBMK_STEPPING_AUTO)
+        c.stepping = (cl && g->ops->linear) ? STEPPING_CLUSTER : (can && state2 <= (size_t(96) << 20)) ? STEPPING_PERSISTENT : STEPPING_LAUNCH;
+    else if (g->opt_stepping == LBMK_STEPPING_CLUSTER) c.stepping = cl ? STEPPING_CLUSTER : (can ? STEPPING_PERSISTENT : STEPPING_LAUNCH);
     else c.stepping = (g->opt_stepping == LBMK_STEPPING_PERSISTENT && can) ? STEPPING_PERSISTENT : STEPPING_LAUNCH;
 }
 
@@ -387,7 +390,7 @@ lbmk_status lbmk_grid_set_option(lbmk_grid* g, lbmk_option key, long long value)
         if (value == LBMK_KERNEL_ROW) return fail(g, LBMK_EUNSUPPORTED, "LBMK_KERNEL_ROW is reserved: no staged-row kernel in this build");
         g->opt_kernel = value;
     } else if (key == LBMK_OPT_STEPPING) {
-        if (value < LBMK_STEPPING_AUTO || value > LBMK_STEPPING_PERSISTENT) return fail(g, LBMK_EINVAL, "unknown stepping mode");
+        if (value < LBMK_STEPPING_AUTO || value > LBMK_STEPPING_CLUSTER) return fail(g, LBMK_EINVAL, "unknown stepping mode");
         g->opt_stepping = value;
     } else {
         return fail(g, LBMK_EINVAL, "unknown option");

@@ -10,7 +10,7 @@ namespace lbmk {
 enum { PREC_F64 = 0, PREC_F32 = 1 };
 enum { PATTERN_PULL2 = 1, PATTERN_AA = 2 };
 enum { KERNEL_NODE = 1, KERNEL_ROW = 2, KERNEL_TWOPASS = 3 };
-enum { STEPPING_LAUNCH = 1, STEPPING_PERSISTENT = 2 };
+enum { STEPPING_LAUNCH = 1, STEPPING_PERSISTENT = 2, STEPPING_CLUSTER = 3 };
 
 struct GridCore {
     int nx, ny, nz;
@@ -52,6 +52,7 @@ struct SysOps {
     int nt, nax[3];       // time scalars and table entries per axis of the manufactured solution
     int nc;               // per-row forcing coefficients (multiple of 4; 0 without manufactured solution)
     int n_aux;            // prescribed per-node coefficient fields
+    bool linear;          // single-product flux entries: bits independent of the kernel (AUTO may then pick the cluster kernel)
     // all return cudaError_t of the last launch / API call
     cudaError_t (*fill_tables)(GridCore&);                 // host fp64 -> device R tables (synchronous copy on the stream)
     cudaError_t (*reference_equilibrium)(GridCore&);
@@ -67,6 +68,7 @@ struct SysOps {
     cudaError_t (*max_wave_speed)(GridCore&, double* out3_host);
     cudaError_t (*error_norms)(GridCore&, double* out_dev /*[M][6], zeroed here*/);
     bool (*row_kernel_supported)(const GridCore&);
+    bool (*cluster_supported)(const GridCore&);     // the grid fits the cluster-resident kernel (kernels.cuh collide_stream_cluster)
 };
 
 const SysOps* ops_advection2d();

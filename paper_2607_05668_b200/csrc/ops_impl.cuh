@@ -23,6 +23,16 @@ template <> struct Tune<SysHcnsf3D, double> { static constexpr int BLOCK = 128, 
 template <class R> struct Tune<SysMhd2D, R> { static constexpr int BLOCK = 128, MINB = 3; };
 template <> struct Tune<SysMhd2D, double> { static constexpr int BLOCK = 128, MINB = 1; };
 
+// launch shape of the persistent kernel (L2-resident grids: latency-bound, so occupancy matters more than for the
+// bandwidth-bound per-launch kernel)
+#ifndef LBMK_P_BLOCK
+#define LBMK_P_BLOCK 128
+#endif
+#ifndef LBMK_P_MINB
+#define LBMK_P_MINB 1
+#endif
+template <template <class> class S, class R> struct TuneP { static constexpr int BLOCK = Tune<S, R>::BLOCK == 64 ? 64 : LBMK_P_BLOCK, MINB = Tune<S, R>::BLOCK == 64 ? Tune<S, R>::MINB : LBMK_P_MINB; };
+
 // two-pass kernel: register cap via min blocks per SM
 template <template <class> class S, class R> struct Tune2 { static constexpr int BLOCK = 256, MINB = 2; };
 template <class R> struct Tune2<SysNsf3D, R> { static constexpr int BLOCK = 128, MINB = 4; };
@@ -183,7 +193,7 @@ struct Ops {
     // ---- persistent stepping: `cnt` steps of the two-lattice pull pattern in ONE cooperative launch (kernels.cuh)
     template <class R, bool MMS>
     static int persistent_grid(GridCore& g) {
-        constexpr int BLOCK = Tune<S, R>::BLOCK, MINB = Tune<S, R>::MINB;
+        constexpr int BLOCK = TuneP<S, R>::BLOCK, MINB = TuneP<S, R>::MINB;
         int per_sm = 0;
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, collide_stream_persistent<S<R>, R, MMS, BLOCK, MINB>, BLOCK, 0) != cudaSuccess) return 0;
         const long long cap = (long long)per_sm * g.num_sms, nseg = (g.n + BLOCK - 1) / BLOCK;
@@ -193,7 +203,7 @@ struct Ops {
     }
     template <class R, bool MMS>
     static cudaError_t launch_persistent(GridCore& g, int cnt, long long coef_stride) {
-        constexpr int BLOCK = Tune<S, R>::BLOCK, MINB = Tune<S, R>::MINB;
+        constexpr int BLOCK = TuneP<S, R>::BLOCK, MINB = TuneP<S, R>::MINB;
         const int grid = persistent_grid<R, MMS>(g);
         if (grid <= 0) return cudaErrorLaunchOutOfResources;
         cudaError_t e = cudaMemsetAsync(g.bar, 0, sizeof(unsigned int), g.stream);
@@ -213,8 +223,42 @@ struct Ops {
         g.step += cnt;
         return cudaSuccess;
     }
+    // ---- cluster-resident stepping for tiny grids: state in distributed shared memory of one cluster (kernels.cuh)
+    static constexpr int CLUSTER = 8;
+    template <class R>
+    static int cluster_npc(const GridCore& g) {        // threads (= nodes) per CTA, or 0 if the grid does not qualify
+        if (HAS_MMS && g.mms_id != 0) return 0;
+        if (NA > 0 || M * Q > 40 || g.n > (long long)CLUSTER * 1024 || g.n < 64) return 0;   // small tracker-free systems (<= 64 registers at 1024 threads)
+        const int npc = (int)(((g.n + CLUSTER - 1) / CLUSTER + 31) / 32 * 32);
+        const size_t smem = 2 * (size_t)M * Q * npc * sizeof(R);
+        return smem <= (size_t)200 * 1024 ? npc : 0;
+    }
+    template <class R>
+    static cudaError_t launch_cluster(GridCore& g, int cnt, int npc) {
+        const size_t smem = 2 * (size_t)M * Q * npc * sizeof(R);
+        auto kern = collide_stream_cluster<S<R>, R>;
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(CLUSTER); cfg.blockDim = dim3(npc); cfg.dynamicSmemBytes = smem; cfg.stream = g.stream;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = CLUSTER; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        const R* src = (const R*)g.f[g.cur];
+        R* dst = (R*)g.f[g.cur ^ 1];
+        e = cudaLaunchKernelEx(&cfg, kern, src, dst, kp<R>(g), cnt, g.pending ? 0 : 1);
+        if (e != cudaSuccess) return e;
+        g.launches++;
+        g.persistent_launches++;
+        g.cur ^= 1;                       // whatever cnt: the result is in the other buffer
+        g.pending = 1;
+        g.step += cnt;
+        return cudaSuccess;
+    }
+    static bool cluster_supported(const GridCore& g) { return (g.prec == PREC_F64 ? cluster_npc<double>(g) : cluster_npc<float>(g)) > 0; }
     static bool use_persistent(const GridCore& g, int n_steps) {
-        return g.stepping == STEPPING_PERSISTENT && g.pattern == PATTERN_PULL2 && g.kernel == KERNEL_NODE && g.bc == 0 && n_steps >= 2;
+        return (g.stepping == STEPPING_PERSISTENT || g.stepping == STEPPING_CLUSTER) && g.pattern == PATTERN_PULL2 && g.kernel == KERNEL_NODE && g.bc == 0 && n_steps >= 2;
     }
     // one collide-and-stream launch (plus the Dirichlet frame refill before it on bounded grids)
     template <class R, bool MMS>
@@ -252,6 +296,7 @@ struct Ops {
     static cudaError_t step_t(GridCore& g, int n_steps) {
         if constexpr (!MMS) {
             if (use_persistent(g, n_steps)) {
+                if (g.stepping == STEPPING_CLUSTER) return launch_cluster<R>(g, n_steps, cluster_npc<R>(g));
                 for (int done = 0; done < n_steps;) {
                     const int cnt = std::min(n_steps - done, 1 << 16);      // bounds the 32-bit barrier count
                     cudaError_t e = launch_persistent<R, false>(g, cnt, 0);
@@ -387,9 +432,9 @@ struct Ops {
     static bool row_supported(const GridCore&) { return false; }
 
     static const SysOps* get() {
-        static const SysOps ops = {Sd::ID, D, M, Sd::MC, HAS_MMS, C::NT, {C::NX, C::NY, C::NZ}, C::NC, NA,
+        static const SysOps ops = {Sd::ID, D, M, Sd::MC, HAS_MMS, C::NT, {C::NX, C::NY, C::NZ}, C::NC, NA, IsLinear<Sd>::value,
                                    &fill_tables, &reference_equilibrium, &init_from_U, &set_f, &step, &step_ranges, &set_aux,
-                                   &read_U_with_frame, &read_f, &max_wave_speed, &error_norms, &row_supported};
+                                   &read_U_with_frame, &read_f, &max_wave_speed, &error_norms, &row_supported, &cluster_supported};
         return &ops;
     }
 };

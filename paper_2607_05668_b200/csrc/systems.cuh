@@ -33,6 +33,7 @@ enum { SYS_ADVECTION2D = 0, SYS_BURGERS2D = 1, SYS_SWE2D = 2, SYS_EULER2D = 3, S
 // Phi = (a_x U, a_y U); par = {a_x, a_y}
 template <class R> struct SysAdvection2D {
     static constexpr int ID = SYS_ADVECTION2D, D = 2, M = 1, MC = 1;
+    static constexpr bool LINEAR = true;     // flux = one product per entry: no FMA-contraction freedom, every kernel gives the same bits
     using Mms = void;
     struct Ctx {};
     __device__ __forceinline__ static void setup(Ctx&, const R (&)[M], const KParams<R>&) {}
@@ -564,6 +565,7 @@ template <class R> struct SysUrf2D {
 // Linear: the delta form is the flux itself.
 template <class R> struct SysMaxwell2D {
     static constexpr int ID = SYS_MAXWELL2D, D = 2, M = 3, MC = 3;
+    static constexpr bool LINEAR = true;
     using Mms = Mms_maxwell2d;
     struct Ctx {};
     __device__ __forceinline__ static void setup(Ctx&, const R (&)[M], const KParams<R>&) {}

@@ -63,6 +63,8 @@ PERSIST = [
     (W.c4_nsf3d, dict(n=64, ny=6, nz=5), 30, None),                 # 17 fields, fp32, forcing on, staged (nx = block)
     (W.c5_mhd3d, dict(n=24, ny=10, nz=7, precision="f64"), 31, None),
     (W.pin_swe, dict(n=40), 50, None),                              # prescribed per-node fields
+    (lambda: W.relabel(W.pin_burgers(88), mms_id=0), dict(), 40, [3, 37]),     # 7744 nodes, no forcing: the largest cluster-resident class (npc = 992)
+    (lambda: W.relabel(W.c2_swe(72, ny=50), mms_id=0), dict(), 45, [2, 43]),  # SWE without forcing: cluster-resident, fp64, nonlinear
 ]
 
 
@@ -78,10 +80,25 @@ def test_persistent_stepping_is_bit_identical_to_per_launch(P, mk, kw, steps, ch
     assert l2 < l1                                                  # fewer launches is the point
     Uo, fo = oracle_run(w, steps)
     gate(U2, Uo, fo, w.precision, f"{w.name}[persistent]", U_ref=w.U_ref, steps=steps, strict=False)
+    # cluster-resident kernel (state in distributed shared memory): same arithmetic (collide_core), FMA contraction decided per
+    # kernel by nvcc -> equal to rounding in general, bit for bit for the linear system of configs[0]
+    U3, f3, (mode3, l3) = gpu_run(P, w, steps, chunks, pattern="pull2", stepping="cluster")
+    if mode3 == "cluster":
+        assert l3 <= l2
+        if w.system == "advection2d":
+            assert np.array_equal(f1, f3)
+        d = np.abs(f3 - f1).max() / np.abs(f1).max()
+        assert d <= (2e-7 if w.precision == "f32s" else 1e-13), d
+        gate(U3, Uo, fo, w.precision, f"{w.name}[cluster]", U_ref=w.U_ref, steps=steps, strict=False)
+    else:
+        assert mode3 == "persistent" and np.array_equal(f1, f3)     # does not qualify: falls back
 
 
 def test_persistent_is_the_default_for_l2_resident_grids_only(P):
-    small = P.Grid.from_workload(W.c2_swe(64))
+    tiny = P.Grid.from_workload(W.c1_advection())                   # configs[0]: 4096 nodes, no forcing -> one cluster, DSMEM-resident
+    assert tiny.stepping == "cluster"
+    tiny.close()
+    small = P.Grid.from_workload(W.c2_swe(64))                      # forcing on -> cooperative persistent kernel
     assert small.stepping == "persistent"
     small.close()
     aa = P.Grid.from_workload(W.c2_swe(64), pattern="aa")           # in-place pattern: per-launch only
