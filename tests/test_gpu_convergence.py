@@ -193,3 +193,83 @@ def test_paper_table2_float_rows_same_magnitude(P, mk, field, paper_l2):
     g.close()
     print(f"{w.name} shifted fp32: rel L2 {l2:.4e} (paper Float {paper_l2:.4e})")
     assert paper_l2 / 4 <= l2 <= paper_l2 * 2
+
+
+# ------------------------------------------------------------------------------------------------ fp32 order retained (north_star)
+def _l2_by_field(n, fields):
+    return {name: math.sqrt(sum(n[k][1] ** 2 for k in ks)) for name, ks in fields.items()}
+
+
+@pytest.mark.parametrize("mk,fields,paper_float_eoc", [
+    (W.pin_euler, {"rho": (0,), "rhou": (1, 2), "E": (3,)}, {"rho": 1.65, "rhou": 1.62, "E": 1.73}),        # PAPER.md:L519-L522 Float rows
+    (W.pin_swe, {"h": (0,), "hu": (1, 2)}, {"h": 1.95, "hu": 1.83}),                                         # PAPER.md:L523-L526 Float rows
+])
+def test_fp32_convergence_order_retained_on_the_config_systems(P, mk, fields, paper_float_eoc):
+    """north_star: "<= 2e-5 in shifted fp32, with the fp32 convergence order retained".  The refinement study of the systems of
+    configs[2] (Euler) and configs[1] (shallow water, here over the paper's bed) in shifted fp32 at the paper's Float knobs
+    (Table SM2) against the SAME study in fp64 at the same knobs: N = 64 ... 512 to t = 1, LSQ L2 slope.  The fp32
+    slope stays within 0.5 of the fp64 one (float keeps the order down to a 1e-5 - 1e-4 floor) and within
+    0.35 of the Float EOC the paper prints."""
+    ns = (64, 128, 256, 512)
+    slopes = {}
+    for prec in ("f32s", "f64"):
+        errs = []
+        for n in ns:
+            w = mk(n, precision="f32s")                     # Float knobs for both precisions
+            g = P.Grid.from_workload(w, precision=prec)
+            g.init_from_U(w.initial_U())
+            g.step(w.steps)
+            errs.append(_l2_by_field(g.error_norms(), fields))
+            g.close()
+        slopes[prec] = {f: -np.polyfit(np.log2(ns), np.log2([e[f] for e in errs]), 1)[0] for f in fields}
+        print(mk.__name__, prec, {f: round(s, 3) for f, s in slopes[prec].items()}, "errors at N=512:", {f: f"{errs[-1][f]:.3e}" for f in fields})
+    for f in fields:
+        assert abs(slopes["f32s"][f] - slopes["f64"][f]) <= 0.5, (f, slopes)
+        assert slopes["f32s"][f] >= 1.2, (f, slopes)
+        assert abs(slopes["f32s"][f] - paper_float_eoc[f]) <= 0.35, (f, slopes["f32s"][f], paper_float_eoc[f])
+
+
+def test_fp32_convergence_order_retained_on_c4(P):
+    """configs[3] (NSF 3D + 12 trackers, forcing on) refined N = 32, 64, 128, 256 to the time the config reaches after its 200
+    steps at 256^3, in shifted fp32 and in fp64: the L2 slopes of the five conserved fields agree within 0.5 and the fp32
+    ones stay above 1.2 (the errors are 1e-5 - 1e-3 here, above the fp32 floor)."""
+    ns = (32, 64, 128, 256)
+    slopes = {}
+    for prec in ("f32s", "f64"):
+        errs = []
+        for n in ns:
+            w = W.c4_nsf3d(n, precision=prec)
+            g = P.Grid.from_workload(w)
+            g.init_from_U(w.initial_U())
+            g.step(200 * n // 256)
+            errs.append(g.error_norms()[:5, 1])
+            g.close()
+        errs = np.array(errs)
+        slopes[prec] = [-np.polyfit(np.log2(ns), np.log2(errs[:, k]), 1)[0] for k in range(5)]
+        print("c4", prec, np.round(slopes[prec], 3), "L2 errors at 256^3:", errs[-1])
+    for k in range(5):
+        assert abs(slopes["f32s"][k] - slopes["f64"][k]) <= 0.5 and slopes["f32s"][k] >= 1.2, (k, slopes)
+
+
+def test_paper_table2_mhd2d_row_within_ten_percent(P):
+    """Resistive MHD 2D (knobs L743; fields SM5.12 L1375-L1392).  Built from the vector form (listing SM4.11
+    is garbled); the legible listing entries are pinned by P13.  At the printed working point the GPU run is second order and
+    lands within 8 % of all eight printed errors (E within 0.7 %), but not on their digits: reading A27, UNPINNED to Table 2
+    (a scan of tau_R, g_tau, f and the three diffusivities does not hit all eight at once).  Gate: within 10 %; EOCs of L2
+    within 0.15 of the printed ones."""
+    paper = {"rho": ((0,), 2.7365e-04, 1.6299e-04, 1.75), "rhou": ((1, 2), 4.6103e-04, 2.4482e-04, 1.88),
+             "E": ((3,), 3.6516e-04, 2.1223e-04, 1.96), "B": ((4, 5), 2.4829e-04, 1.6277e-04, 2.22)}
+    ns, norms = (64, 128, 256, 512), []
+    for n in ns:
+        w = W.pin_mhd2d(n)
+        g = P.Grid.from_workload(w)
+        g.init_from_U(w.initial_U())
+        g.step(w.steps)
+        norms.append(g.error_norms())
+        g.close()
+    for name, (ks, linf, l2, eoc) in paper.items():
+        got_linf = math.sqrt(sum(norms[-1][k][2] ** 2 for k in ks))
+        got_l2 = [math.sqrt(sum(e[k][1] ** 2 for k in ks)) for e in norms]
+        slope = -np.polyfit(np.log2(ns), np.log2(got_l2), 1)[0]
+        print(f"mhd2d {name}: Linf {got_linf:.4e} (paper {linf:.4e})  L2 {got_l2[-1]:.4e} (paper {l2:.4e})  L2 EOC {slope:.2f} (paper {eoc:.2f})")
+        assert abs(got_linf / linf - 1) <= 0.10 and abs(got_l2[-1] / l2 - 1) <= 0.10 and abs(slope - eoc) <= 0.15
