@@ -67,7 +67,9 @@ class SlabGrid:
         assert P.lbmk_halo_bytes(self.grid.h) == m * plane * (8 if dt == torch.float64 else 4)
         mk = lambda: torch.empty((m, plane), dtype=dt, device=self.grid.device)
         self.send_lo, self.send_hi, self.recv_lo, self.recv_hi = mk(), mk(), mk(), mk()
-        self.comm = torch.cuda.Stream(device=self.grid.device)      # halo pack / transport / unpack beside the interior update
+        # halo pack / transport / unpack run on this stream, beside the interior update (None on a CPU stand-in grid: the
+        # gloo test of the call order, tests/test_slabs_host.py)
+        self.comm = torch.cuda.Stream(device=self.grid.device) if torch.device(self.grid.device).type == "cuda" else None
 
     def init(self):
         self.grid.init_from_U(self.w.initial_U())
@@ -91,20 +93,23 @@ class SlabGrid:
                 self.unpack()
                 continue
             self.begin_step()
-            with torch.cuda.stream(self.comm):
+            if self.comm is not None:
+                with torch.cuda.stream(self.comm):
+                    ring.exchange(self.send_lo, self.send_hi, self.recv_lo, self.recv_hi)
+            else:
                 ring.exchange(self.send_lo, self.send_hi, self.recv_lo, self.recv_hi)
             self.end_step()
 
     def begin_step(self):
         """Boundary planes, [event], interior planes on the grid's stream; pack on the comm stream after the event."""
-        P, h, cs = self.P, self.grid.h, self.comm.cuda_stream
+        P, h, cs = self.P, self.grid.h, (self.comm.cuda_stream if self.comm is not None else 0)
         P.lbmk_step_slab(h)
         P.lbmk_stream_wait_boundary(h, cs)
         P.lbmk_halo_pack_on(h, self.send_lo.data_ptr(), self.send_hi.data_ptr(), cs)
 
     def end_step(self):
         """Unpack on the comm stream; the grid's stream (the next step) waits for it."""
-        P, h, cs = self.P, self.grid.h, self.comm.cuda_stream
+        P, h, cs = self.P, self.grid.h, (self.comm.cuda_stream if self.comm is not None else 0)
         P.lbmk_halo_unpack_on(h, self.recv_lo.data_ptr(), self.recv_hi.data_ptr(), cs)
         P.lbmk_grid_wait_stream(h, cs)
 

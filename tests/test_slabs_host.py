@@ -92,3 +92,108 @@ def test_single_rank_ring_wraps_onto_itself():
     a, b, rl, rh = torch.ones(2, 3), 2 * torch.ones(2, 3), torch.zeros(2, 3), torch.zeros(2, 3)
     HaloRing(0, 1).exchange(a, b, rl, rh)
     assert (rl == 2).all() and (rh == 1).all()
+
+
+# ------------------------------------------------------------------------------------------------ SlabGrid.step end to end over gloo
+# A CPU stand-in for the binding: the same calls SlabGrid makes (lbmk_step_slab, lbmk_stream_wait_boundary, lbmk_halo_pack[_on],
+# lbmk_halo_unpack[_on], lbmk_grid_wait_stream, Grid.step) acting on a D2Q5 PURE-STREAMING state of integer tags in NumPy, with the
+# library's halo protocol (send_lo = slot(-y) of the first own plane, send_hi = slot(+y) of the last own plane; recv_lo ->
+# slot(+y) of the lower ghost plane, recv_hi -> slot(-y) of the upper ghost plane).  It records the call order.  What is tested is
+# slabs.py: the order of calls in SlabGrid.step (overlapped and serial) and the routing between two ranks.
+SLAB_WORKER = r"""
+import json, os, sys
+sys.path.insert(0, {root!r})
+import numpy as np, torch, torch.distributed as dist
+import workloads as W
+from paper_2607_05668_b200.slabs import HaloRing, SlabGrid
+
+C = [(0, 0), (1, 0), (-1, 0), (0, 1), (0, -1)]          # (cx, cy), direction order of include/lbmk.h
+
+class FakeGrid:
+    def __init__(self, w):
+        self.w, self.h, self.device, self.log = w, self, torch.device("cpu"), []
+        self.f = None
+    def init_from_U(self, U):
+        # tag populations: f_i = 10 * U + i (U carries the global node tag)
+        self.f = np.stack([10.0 * U[0, 0] + i for i in range(5)])
+    def _stream(self, rows):
+        new = self.f.copy()
+        for i, (cx, cy) in enumerate(C):
+            src = np.roll(self.f[i], cx, axis=1)             # periodic in x inside the slab
+            for y in rows:
+                new[i, y] = src[y - cy]
+        return new
+    def step(self, n):
+        assert n == 1
+        self.log.append("step")
+        self.f = self._stream(range(1, self.f.shape[1] - 1))
+
+class FakeP:
+    class Grid:
+        @staticmethod
+        def from_workload(w, precision=None, slab=False, device="cpu"):
+            assert slab
+            return FakeGrid(w)
+    @staticmethod
+    def lbmk_halo_bytes(g): return 1 * g.w.nx * 8
+    @staticmethod
+    def lbmk_step_slab(g):
+        g.log.append("step_slab"); g.f = g._stream(range(1, g.f.shape[1] - 1))
+    @staticmethod
+    def lbmk_stream_wait_boundary(g, s): g.log.append("wait_boundary")
+    @staticmethod
+    def lbmk_grid_wait_stream(g, s): g.log.append("grid_wait_comm")
+    @staticmethod
+    def _pack(g, lo, hi):
+        lo.copy_(torch.from_numpy(g.f[4, 1][None].copy())); hi.copy_(torch.from_numpy(g.f[3, -2][None].copy()))
+    @staticmethod
+    def _unpack(g, lo, hi):
+        g.f[3, 0] = lo.numpy()[0]; g.f[4, -1] = hi.numpy()[0]
+
+dist.init_process_group(backend="gloo")
+rank, world = dist.get_rank(), dist.get_world_size()
+nx, ny, steps = 6, 8, 5
+tags = np.arange(nx * ny, dtype=np.float64).reshape(1, 1, ny, nx)
+wg = W.relabel(W.c1_advection(nx, ny=ny), init=lambda w: tags[:, :, [(j + w.origin[1]) % ny for j in range(w.ny)], :].copy())
+results = {{}}
+for overlap in (True, False):
+    s = SlabGrid(FakeP, wg, rank, world, device="cpu", precision="f64")
+    # the binding hands device pointers; the stand-in needs the tensors themselves
+    FakeP.lbmk_halo_pack = staticmethod(lambda g, a, b, s=s: (g.log.append("pack"), FakeP._pack(g, s.send_lo, s.send_hi)))
+    FakeP.lbmk_halo_pack_on = staticmethod(lambda g, a, b, st, s=s: (g.log.append("pack_on"), FakeP._pack(g, s.send_lo, s.send_hi)))
+    FakeP.lbmk_halo_unpack = staticmethod(lambda g, a, b, s=s: (g.log.append("unpack"), FakeP._unpack(g, s.recv_lo, s.recv_hi)))
+    FakeP.lbmk_halo_unpack_on = staticmethod(lambda g, a, b, st, s=s: (g.log.append("unpack_on"), FakeP._unpack(g, s.recv_lo, s.recv_hi)))
+    s.init()
+    s.step(steps, HaloRing(rank, world, dist), overlap=overlap)
+    results[str(overlap)] = dict(own=s.grid.f[:, 1:-1].tolist(), start=s.start, count=s.count, log=s.grid.log)
+dist.barrier()
+print(json.dumps(dict(rank=rank, res=results)))
+dist.destroy_process_group()
+"""
+
+
+def test_slab_grid_step_over_gloo_world_2():
+    """Two ranks, 5 steps, overlapped and serial: the slabs' own planes equal the global periodic streaming of the tags, and each
+    step issues its calls in the documented order (boundary event before the pack; unpack before the grid's stream goes on)."""
+    world, nx, ny, steps = 2, 6, 8, 5
+    port = _free_port()
+    procs = []
+    for r in range(world):
+        env = dict(os.environ, RANK=str(r), LOCAL_RANK=str(r), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1",
+                   MASTER_PORT=str(port), CUDA_VISIBLE_DEVICES="")
+        procs.append(subprocess.Popen([sys.executable, "-c", SLAB_WORKER.format(root=ROOT)], env=env,
+                                      stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True))
+    tags = np.arange(nx * ny, dtype=np.float64).reshape(ny, nx)
+    C = [(0, 0), (1, 0), (-1, 0), (0, 1), (0, -1)]
+    want = np.stack([np.roll(10.0 * tags + i, shift=(steps * cy, steps * cx), axis=(0, 1)) for i, (cx, cy) in enumerate(C)])
+    for p in procs:
+        o, e = p.communicate(timeout=240)
+        assert p.returncode == 0, e[-3000:]
+        d = json.loads(o.strip().splitlines()[-1])
+        for overlap in ("True", "False"):
+            r = d["res"][overlap]
+            own = np.array(r["own"])
+            assert np.array_equal(own, want[:, r["start"]:r["start"] + r["count"]]), (d["rank"], overlap)
+            per_step = (["step_slab", "wait_boundary", "pack_on", "unpack_on", "grid_wait_comm"] if overlap == "True"
+                        else ["step", "pack", "unpack"])
+            assert r["log"] == per_step * steps
