@@ -143,6 +143,16 @@ lbmk_status lbmk_system_set_reference(lbmk_system* sys, const double* U0, int n)
  *   NSF2D {} (eq SM5.10);  SWE2D_BATHY {h0, A_h, m0, A_m, A_zb, w_t} (eq SM5.3, bed L1198; w_t = frequency of the time factors);
  *   MHD2D {} (SM5.12 L1375-L1392).  HCNSF3D has none compiled in (its exact fields are truncated in the source, L1457). */
 lbmk_status lbmk_system_set_mms(lbmk_system* sys, int mms_id, const double* mms_params, int n);
+/* Collision operator.  LBMK_COLLISION_BGK (default) is eq 2.11, the operator the paper analyses and runs.  LBMK_COLLISION_TRT is
+ * the two-relaxation-time operator the paper names as consuming the same equilibria unchanged, in its textbook
+ * form: with ibar opposite to i and f+- = (f_i +- f_ibar)/2,
+ *     f' = f_i - omega_plus (f+ - f_eq+) - omega_minus (f- - f_eq-) + w_i dt S,
+ * omega_minus = the component's rate omega_k (f_eq- = w_i c_i.F/c_s^2 carries the flux, so the relaxation diffusion of eq 2.17 is
+ * unchanged) and omega_plus from the magic parameter Lambda = (1/omega_plus - 1/2)(1/omega_minus - 1/2) (`magic` > 0; 1/4 is the
+ * usual choice).  TRT runs on the two-lattice pull pattern with the node kernel, one launch per step (other options resolve
+ * to these).  Not a paper result: pinned by textbook properties, tests/test_trt.py. */
+enum { LBMK_COLLISION_BGK = 0, LBMK_COLLISION_TRT = 1 };
+lbmk_status lbmk_system_set_collision(lbmk_system* sys, int collision, double magic);
 /* A-priori bound on the physical wave speed max|eig sum n_a A_a| from the declared amplitudes (eq 2.20).
  * lbmk_grid_create rejects the grid with LBMK_ESUBCHAR if s_max/lambda > c_s.  0 = no declared bound. */
 lbmk_status lbmk_system_set_wave_speed_bound(lbmk_system* sys, double s_max);
@@ -251,6 +261,8 @@ lbmk_status lbmk_stream_index_map(lbmk_grid* g, int dir, long long* src_index_ou
 lbmk_status lbmk_lattice_constants(lbmk_lattice lattice, int* c, double* w, double* cs2);
 /* Relaxation rates omega_k [m_total] the grid uses.  Host pointer. */
 lbmk_status lbmk_grid_omega(const lbmk_grid* g, double* omega_out);
+/* TRT: rates omega_plus,k [m_total] of the symmetric parts (equal to omega_k for BGK).  Host pointer. */
+lbmk_status lbmk_grid_omega_plus(const lbmk_grid* g, double* omega_out);
 /* Kernel launches enqueued by this grid so far (bench.py's gpu_launches). */
 lbmk_status lbmk_grid_launch_count(const lbmk_grid* g, long long* launches);
 /* CUDA-event time, in milliseconds, of the collide-and-stream kernels of the most recent lbmk_step call

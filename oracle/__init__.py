@@ -28,6 +28,7 @@ class _Spec(C.Structure):
         ("dx", C.c_double), ("lam", C.c_double), ("g_tau", C.c_double), ("t0", C.c_double),
         ("par", C.c_double * 16), ("mms_par", C.c_double * 16),
         ("tau_R", C.c_double * MAXM), ("omega", C.c_double * MAXM), ("U_ref", C.c_double * MAXM),
+        ("collision", C.c_int32), ("pad2_", C.c_int32), ("trt_magic", C.c_double),
     ]
 
 
@@ -46,7 +47,7 @@ def lib():
         for name, args in {
             "orc_init_from_U": [C.c_void_p, dp], "orc_set_f": [C.c_void_p, dp],
             "orc_step": [C.c_void_p, C.c_int], "orc_read_f": [C.c_void_p, dp], "orc_read_U": [C.c_void_p, dp],
-            "orc_time": [C.c_void_p, C.POINTER(C.c_int64), dp], "orc_omega": [C.c_void_p, dp],
+            "orc_time": [C.c_void_p, C.POINTER(C.c_int64), dp], "orc_omega": [C.c_void_p, dp], "orc_omega_plus": [C.c_void_p, dp],
             "orc_exact_U": [C.c_void_p, C.c_double, dp],
             "orc_flux_source": [C.c_void_p, dp, dp, dp, dp], "orc_set_aux": [C.c_void_p, dp],
             "orc_system_n_aux": [C.c_int], "orc_equilibrium": [C.c_void_p, dp, dp, dp],
@@ -97,7 +98,7 @@ class OracleGrid:
                  mms_id: int = 0, mms_params: Sequence[float] = (), bc: str = "periodic",
                  shifted: bool = False, U_ref: Optional[Sequence[float]] = None,
                  omega: Optional[Sequence[float]] = None, origin=(0, 0, 0), t0: float = 0.0,
-                 n_threads: int = 0):
+                 n_threads: int = 0, collision: str = "bgk", trt_magic: float = 0.25):
         self.system = system
         self.m_conserved, self.m_total, self.dim, self.Q = system_info(system)
         self.nx, self.ny, self.nz = nx, ny, nz
@@ -109,6 +110,8 @@ class OracleGrid:
         s.shifted = int(bool(shifted))
         s.mms_id = mms_id
         s.n_threads = n_threads
+        s.collision = {"bgk": 0, "trt": 1}[collision]
+        s.trt_magic = trt_magic
         s.ox, s.oy, s.oz = origin
         s.dx, s.lam, s.g_tau, s.t0 = dx, lam, g_tau, t0
         for i, v in enumerate(params):
@@ -198,6 +201,11 @@ class OracleGrid:
     def omega(self) -> np.ndarray:
         o = np.empty(self.m_total)
         lib().orc_omega(self._h, _dp(o))
+        return o
+
+    def omega_plus(self) -> np.ndarray:
+        o = np.empty(self.m_total)
+        lib().orc_omega_plus(self._h, _dp(o))
         return o
 
     def exact_U(self, t: float) -> np.ndarray:

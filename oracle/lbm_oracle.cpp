@@ -66,6 +66,9 @@ struct Spec {  // mirrored field by field in oracle/__init__.py (ctypes)
     double tau_R[MAXM];  // per conserved component
     double omega[MAXM];  // >= 0 overrides the derived rate of component k (tests: omega = 0, 1)
     double U_ref[MAXM];  // Q0 for the shifted form
+    int32_t collision;   // 0 BGK (eq 2.11, the operator the paper runs); 1 two-relaxation-time (PAPER.md:L154 names it; textbook form below)
+    int32_t pad2_;
+    double trt_magic;    // Lambda = (1/omega_plus - 1/2)(1/omega_minus - 1/2)
 };
 
 struct Grid {
@@ -76,6 +79,7 @@ struct Grid {
     int64_t n;       // nodes
     int64_t step;
     double omega[MAXM];
+    double omega_plus[MAXM];   // TRT: rate of the symmetric parts; omega[] is then the rate of the antisymmetric (flux-carrying) parts
     double F_ref[MAXM * 3];
     std::vector<double> f, g;  // f[(k*Q + i)*n + node]
     std::vector<double> aux;   // prescribed coefficient fields aux[a*n + node] (n_aux per system; zeros until orc_set_aux)
@@ -169,7 +173,19 @@ static void one_step(Grid& G) {
                 for (int k = 0; k < m; ++k)
                     for (int i = 0; i < Q; ++i) {
                         const double fi = G.f[(int64_t)(k * Q + i) * G.n + nd];
-                        const double fpost = fi - G.omega[k] * (fi - feq[k * Q + i]) + L.w[i] * S[k];
+                        double fpost = fi - G.omega[k] * (fi - feq[k * Q + i]) + L.w[i] * S[k];
+                        if (G.s.collision == 1) {
+                            // two-relaxation-time operator (textbook form; the paper names it at L154 as consuming the same
+                            // equilibria): with ibar the direction opposite to i,  f+- = (f_i +- f_ibar)/2  and likewise f_eq+-,
+                            //   f' = f_i - omega_plus (f+ - f_eq+) - omega_minus (f- - f_eq-) + w_i s_k .
+                            // f_eq- = w_i c_i.F/c_s^2 carries the flux, so omega_minus = omega_k keeps the relaxation diffusion of
+                            // eq (2.17); omega_plus follows from the magic parameter Lambda.
+                            const int ib = (i == 0) ? 0 : (((i - 1) ^ 1) + 1);
+                            const double fb = G.f[(int64_t)(k * Q + ib) * G.n + nd];
+                            const double fp = 0.5 * (fi + fb), fm = 0.5 * (fi - fb);
+                            const double ep = 0.5 * (feq[k * Q + i] + feq[k * Q + ib]), em = 0.5 * (feq[k * Q + i] - feq[k * Q + ib]);
+                            fpost = fi - G.omega_plus[k] * (fp - ep) - G.omega[k] * (fm - em) + L.w[i] * S[k];
+                        }
                         const int xd = wrap(x + L.c[i][0], G.s.nx), yd = wrap(y + L.c[i][1], G.s.ny), zd = wrap(z + L.c[i][2], G.s.nz);
                         G.g[(int64_t)(k * Q + i) * G.n + node_index(G, xd, yd, zd)] = fpost;
                     }
@@ -217,6 +233,9 @@ void* orc_create(const Spec* sp) {
                                             : 1.0 / (sp->g_tau + 1.0);                 // tracker rate, L718
         if (sp->omega[k] >= 0.0) om = sp->omega[k];
         G->omega[k] = om;
+        // Lambda = (1/omega_plus - 1/2)(1/omega_minus - 1/2); omega_minus = 2 (no relaxation diffusion) leaves omega_plus free: 1
+        const double tm = 1.0 / om - 0.5;
+        G->omega_plus[k] = (sp->collision == 1 && om > 0.0) ? (tm > 0.0 ? 1.0 / (0.5 + sp->trt_magic / tm) : 1.0) : om;
     }
     {   // F0 = F(Q0) for the shifted storage, eq (2.23)
         double S[MAXM];
@@ -318,6 +337,11 @@ int orc_time(void* h, int64_t* step, double* t) {
 int orc_omega(void* h, double* omega_out) {
     Grid& G = *(Grid*)h;
     for (int k = 0; k < G.si.m_total; ++k) omega_out[k] = G.omega[k];
+    return 0;
+}
+int orc_omega_plus(void* h, double* omega_out) {
+    Grid& G = *(Grid*)h;
+    for (int k = 0; k < G.si.m_total; ++k) omega_out[k] = G.omega_plus[k];
     return 0;
 }
 

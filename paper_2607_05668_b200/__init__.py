@@ -52,6 +52,8 @@ SYMBOLS = {
     "lbmk_system_set_reference": (C.c_int, [_vp, _dp, C.c_int]),
     "lbmk_system_set_mms": (C.c_int, [_vp, C.c_int, _dp, C.c_int]),
     "lbmk_system_set_wave_speed_bound": (C.c_int, [_vp, C.c_double]),
+    "lbmk_system_set_collision": (C.c_int, [_vp, C.c_int, C.c_double]),
+    "lbmk_grid_omega_plus": (C.c_int, [_vp, _dp]),
     "lbmk_system_destroy": (None, [_vp]),
     "lbmk_grid_create": (C.c_int, [_vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int, _vp, C.POINTER(_vp)]),
     "lbmk_grid_set_option": (C.c_int, [_vp, C.c_int, C.c_longlong]),
@@ -170,6 +172,16 @@ def lbmk_system_set_reference(sys_h, U0):
 def lbmk_system_set_mms(sys_h, mms_id: int, mms_params: Sequence[float]):
     a, p = _darr(list(mms_params) if len(mms_params) else [0.0])
     _check(lib().lbmk_system_set_mms(sys_h, int(mms_id), p, len(mms_params)))
+
+
+def lbmk_system_set_collision(sys_h, collision: int, magic: float = 0.25):
+    _check(lib().lbmk_system_set_collision(sys_h, int(collision), float(magic)))
+
+
+def lbmk_grid_omega_plus(grid_h, m_total: int):
+    o = np.zeros(m_total)
+    _check(lib().lbmk_grid_omega_plus(grid_h, o.ctypes.data_as(_dp)), grid_h)
+    return o
 
 
 def lbmk_system_set_wave_speed_bound(sys_h, s_max: float):
@@ -339,7 +351,7 @@ class System:
 
     def __init__(self, name: str, params: Sequence[float] = (), tau_R=0.0, g_tau: float = 0.0,
                  U_ref: Optional[Sequence[float]] = None, mms_id: int = 0, mms_params: Sequence[float] = (),
-                 omega=None, s_max: float = 0.0):
+                 omega=None, s_max: float = 0.0, collision: str = "bgk", trt_magic: float = 0.25):
         self.name = name
         sid = SYSTEM_ID[name]
         lattice = LBMK_D3Q7 if name in ("nsf3d", "mhd3d", "hcnsf3d") else LBMK_D2Q5
@@ -355,6 +367,8 @@ class System:
             lbmk_system_set_omega(self.h, omega)
         if s_max:
             lbmk_system_set_wave_speed_bound(self.h, s_max)
+        if collision != "bgk":
+            lbmk_system_set_collision(self.h, {"bgk": 0, "trt": 1}[collision], trt_magic)
 
     def close(self):
         if getattr(self, "h", None):
@@ -404,9 +418,11 @@ class Grid:
         self.stepping = {1: "launch", 2: "persistent", 3: "cluster"}[lbmk_grid_get_option(self.h, LBMK_OPT_STEPPING)]
 
     @classmethod
-    def from_workload(cls, w, precision: Optional[str] = None, omega=None, declare_bound: bool = True, **kw):
+    def from_workload(cls, w, precision: Optional[str] = None, omega=None, declare_bound: bool = True, collision: str = "bgk",
+                      trt_magic: float = 0.25, **kw):
         s = System(w.system, params=w.params, tau_R=w.tau_R, g_tau=w.g_tau, U_ref=w.U_ref, mms_id=w.mms_id,
-                   mms_params=w.mms_params if w.mms_id else (), omega=omega, s_max=w.s_max if declare_bound else 0.0)
+                   mms_params=w.mms_params if w.mms_id else (), omega=omega, s_max=w.s_max if declare_bound else 0.0,
+                   collision=collision, trt_magic=trt_magic)
         kw.setdefault("origin", getattr(w, "origin", (0, 0, 0)))
         g = cls(s, w.nx, w.ny, w.nz, w.dx, w.lam, precision=precision or w.precision, **kw)
         if s.n_aux:

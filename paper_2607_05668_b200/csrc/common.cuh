@@ -46,7 +46,8 @@ struct KParams {
     long long n;            // nodes
     int ox, oy, oz;         // node (ix, iy, iz) sits at ((ix+ox) dx, (iy+oy) dx, (iz+oz) dx): sub-domain of a larger grid
     int ghost;              // 1: slab with one ghost plane at each end of the slowest axis (skipped by the reductions)
-    R omega[MAXM];          // relaxation rate per component
+    R omega[MAXM];          // relaxation rate per component; TRT: rate of the antisymmetric parts
+    R omega_p[MAXM];        // TRT only: rate of the symmetric parts (from the magic parameter)
     R ref[MAXM];            // reference state Q0 of eq (2.23); zeros in the unshifted fp64 form
     R par[8];               // physical parameters of the system
     R cst[8];               // host-derived reference constants (u0, p0, E0+p0, T0, ...), see systems.cuh

@@ -98,6 +98,25 @@ __device__ __forceinline__ void relax(R (&f)[2 * D + 1], R omega, R dQ, const R 
     }
 }
 
+// Two-relaxation-time relaxation (PAPER.md:L154 names TRT as an operator that consumes the same equilibria; textbook form):
+// symmetric parts s = (f_+a + f_-a)/2 relax to w1 dQ at omega_p, antisymmetric parts d = (f_+a - f_-a)/2 relax to
+// w1 c.F/c_s^2 = F_a/2 at omega (the flux-carrying rate, so the relaxation diffusion of eq 2.17 is unchanged); source as in BGK.
+template <int D, class R>
+__device__ __forceinline__ void relax_trt(R (&f)[2 * D + 1], R omega_p, R omega_m, R dQ, const R (&F)[D], R S) {
+    const R keep_p = R(1) - omega_p, keep_m = R(1) - omega_m;
+    const R A = omega_p * dQ + S;
+    const R a0 = weight0<D, R>() * A, a1 = weight1<D, R>() * A;
+    const R hw = R(0.5) * omega_m;
+    f[0] = keep_p * f[0] + a0;
+#pragma unroll
+    for (int a = 0; a < D; ++a) {
+        const R s = R(0.5) * (f[1 + 2 * a] + f[2 + 2 * a]), d = R(0.5) * (f[1 + 2 * a] - f[2 + 2 * a]);
+        const R s1 = keep_p * s + a1, d1 = keep_m * d + hw * F[a];
+        f[1 + 2 * a] = s1 + d1;
+        f[2 + 2 * a] = s1 - d1;
+    }
+}
+
 // Pointer qualifiers of the step kernels: the two-lattice modes of the per-launch kernels read one buffer and write the
 // other, so both carry __restrict__ (loads may use the non-coherent path and move freely across the stores); the
 // in-place AA modes are launched with src == dst, where __restrict__ would be a false promise -- plain pointers there.
@@ -124,7 +143,7 @@ __device__ __forceinline__ void load_aux(typename Sys::Ctx& ctx, const KParams<R
 // a3-a6 of ONE node, in registers: moments, system algebra, equilibrium + BGK relaxation component by component; `store(K, f_k)`
 // is called with the Q post-collision populations of component k as soon as they exist (so their registers die early).
 // Shared by every step kernel -- one definition of the arithmetic, hence identical bits whatever the storage.
-template <class Sys, class R, bool MMS, class Store>
+template <class Sys, class R, bool MMS, bool TRT = false, class Store>
 __device__ __forceinline__ void collide_core(R (&f)[Sys::M][2 * Sys::D + 1], typename Sys::Ctx& ctx, const KParams<R>& P,
                                              const R (&smms)[Sys::M], Store&& store) {
     constexpr int D = Sys::D, Q = 2 * D + 1, M = Sys::M;
@@ -142,7 +161,8 @@ __device__ __forceinline__ void collide_core(R (&f)[Sys::M][2 * Sys::D + 1], typ
         R F[D], S;
         Sys::template flux<k>(ctx, dQ, P, F, S);
         if constexpr (MMS) S += smms[k];
-        relax<D, R>(f[k], P.omega[k], dQ[k], F, S);
+        if constexpr (TRT) relax_trt<D, R>(f[k], P.omega_p[k], P.omega[k], dQ[k], F, S);
+        else relax<D, R>(f[k], P.omega[k], dQ[k], F, S);
         store(K, f[k]);
     });
 }
@@ -152,7 +172,7 @@ __device__ __forceinline__ void collide_core(R (&f)[Sys::M][2 * Sys::D + 1], typ
 // coef_s = the block's shared-memory slot for its row's forcing coefficients, coef = this step's coefficient table.
 // Called by the per-launch kernel (one segment per block) and by the persistent kernel (segments in a loop): the
 // same code, hence the same bits.
-template <class Sys, class R, int MODE, bool MMS, int BLOCK, bool COHERENT>
+template <class Sys, class R, int MODE, bool MMS, int BLOCK, bool COHERENT, bool TRT = false>
 __device__ __forceinline__ void node_step(typename StepPtr<R, MODE, COHERENT>::Src src, typename StepPtr<R, MODE, COHERENT>::Dst dst,
                                           const KParams<R>& P, const R* coef, long long first, R* coef_s) {
     constexpr int D = Sys::D, Q = 2 * D + 1, M = Sys::M;
@@ -201,7 +221,7 @@ __device__ __forceinline__ void node_step(typename StepPtr<R, MODE, COHERENT>::S
             mms_node<Sys, R, false>(P, p, coef, smms);
         }
     }
-    collide_core<Sys, R, MMS>(f, ctx, P, smms, [&](auto K, const R* fk) {
+    collide_core<Sys, R, MMS, TRT>(f, ctx, P, smms, [&](auto K, const R* fk) {
         constexpr int k = decltype(K)::value;
 #pragma unroll
         for (int i = 0; i < Q; ++i) {
@@ -216,12 +236,12 @@ __device__ __forceinline__ void node_step(typename StepPtr<R, MODE, COHERENT>::S
     });
 }
 
-template <class Sys, class R, int MODE, bool MMS, int BLOCK, int MINB>
+template <class Sys, class R, int MODE, bool MMS, int BLOCK, int MINB, bool TRT = false>
 __global__ void __launch_bounds__(BLOCK, MINB)
 collide_stream_node(typename StepPtr<R, MODE>::Src src, typename StepPtr<R, MODE>::Dst dst, const __grid_constant__ KParams<R> P) {
     constexpr int NCs = MMS ? MmsNC<Sys>::value : 4;
     __shared__ __align__(16) R coef_s[NCs];
-    node_step<Sys, R, MODE, MMS, BLOCK, false>(src, dst, P, P.coef, P.node0 + (long long)blockIdx.x * BLOCK, coef_s);
+    node_step<Sys, R, MODE, MMS, BLOCK, false, TRT>(src, dst, P, P.coef, P.node0 + (long long)blockIdx.x * BLOCK, coef_s);
 }
 
 // ------------------------------------------------------------------------------------------------ step, persistent

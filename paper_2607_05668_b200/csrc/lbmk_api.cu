@@ -29,6 +29,8 @@ struct lbmk_system {
     int mms_id;
     double mp[LBMK_MAX_PARAMS];
     double s_max;
+    int collision;
+    double trt_magic;
 };
 
 struct lbmk_grid {
@@ -204,6 +206,15 @@ lbmk_status lbmk_system_set_mms(lbmk_system* sys, int mms_id, const double* mms_
     return LBMK_OK;
 }
 
+lbmk_status lbmk_system_set_collision(lbmk_system* sys, int collision, double magic) {
+    if (!sys) return sys_fail(LBMK_EINVAL, "sys is NULL");
+    if (collision != LBMK_COLLISION_BGK && collision != LBMK_COLLISION_TRT) return sys_fail(LBMK_EINVAL, "unknown collision operator");
+    if (collision == LBMK_COLLISION_TRT && !(magic > 0.0)) return sys_fail(LBMK_EINVAL, "TRT magic parameter must be > 0");
+    sys->collision = collision;
+    sys->trt_magic = magic;
+    return LBMK_OK;
+}
+
 lbmk_status lbmk_system_set_wave_speed_bound(lbmk_system* sys, double s_max) {
     if (!sys || !(s_max >= 0.0)) return sys_fail(LBMK_EINVAL, "bad argument");
     sys->s_max = s_max;
@@ -234,6 +245,9 @@ static void derive_params(lbmk_grid* g) {
                                 : 1.0 / (s.g_tau + 1.0);            // tracker rate
         if (s.omega_set) om = s.omega[k];
         P.omega[k] = om;
+        // TRT: Lambda = (1/omega_p - 1/2)(1/omega - 1/2); omega = 2 leaves omega_p free (1); omega = 0 (no collision) keeps 0
+        const double tm = om > 0.0 ? 1.0 / om - 0.5 : 0.0;
+        P.omega_p[k] = (s.collision == LBMK_COLLISION_TRT && om > 0.0) ? (tm > 0.0 ? 1.0 / (0.5 + s.trt_magic / tm) : 1.0) : om;
         P.ref[k] = is_shifted(g->precision) ? s.ref[k] : 0.0;
     }
     for (int i = 0; i < 8; ++i) P.par[i] = s.par[i];
@@ -284,7 +298,7 @@ static void derive_params(lbmk_grid* g) {
     KParams<float>& F = c.Pf;
     memset(&F, 0, sizeof(F));
     F.nx = P.nx; F.ny = P.ny; F.nz = P.nz; F.n = P.n;
-    for (int k = 0; k < MAXM; ++k) { F.omega[k] = (float)P.omega[k]; F.ref[k] = (float)P.ref[k]; }
+    for (int k = 0; k < MAXM; ++k) { F.omega[k] = (float)P.omega[k]; F.omega_p[k] = (float)P.omega_p[k]; F.ref[k] = (float)P.ref[k]; }
     for (int i = 0; i < 8; ++i) { F.par[i] = (float)P.par[i]; F.cst[i] = (float)P.cst[i]; F.mms.par[i] = (float)P.mms.par[i]; F.mms.mp[i] = (float)P.mms.mp[i]; }
     F.il = (float)P.il; F.dL = (float)P.dL; F.inv_gtau = (float)P.inv_gtau; F.dt = (float)P.dt;
     F.mms.dx = (float)P.mms.dx; F.mms.dt = (float)P.mms.dt; F.mms.il = (float)P.mms.il; F.mms.gtau = (float)P.mms.gtau;
@@ -295,12 +309,14 @@ static void resolve_options(lbmk_grid* g) {
     c.pattern = g->opt_pattern == LBMK_PATTERN_AUTO ? PATTERN_PULL2 : (int)g->opt_pattern;
     if (c.bc == LBMK_DIRICHLET_MMS) c.pattern = PATTERN_PULL2;      // the frame refill needs canonical storage
     c.kernel = g->opt_kernel == LBMK_KERNEL_AUTO ? KERNEL_NODE : (int)g->opt_kernel;
+    c.collision = g->sys.collision;
+    if (c.collision == LBMK_COLLISION_TRT) { c.pattern = PATTERN_PULL2; c.kernel = KERNEL_NODE; }   // the variants TRT is compiled for
     if (c.kernel == KERNEL_ROW && !g->ops->row_kernel_supported(c)) c.kernel = KERNEL_NODE;
     // Stepping: grids whose two population copies fit in L2 are launch-latency bound, not bandwidth bound (c1: 0.3 MB,
     // c2: 63 MB against 126 MB of L2) -> one cooperative launch per batch of steps; larger grids: one launch per step.
     const size_t esz = c.prec == PREC_F64 ? 8 : 4;
     const size_t state2 = 2 * (size_t)g->ops->M * (2 * g->ops->D + 1) * (size_t)c.n * esz;
-    const bool can = c.pattern == PATTERN_PULL2 && c.kernel == KERNEL_NODE && c.bc == LBMK_PERIODIC && !c.Pd.ghost;
+    const bool can = c.pattern == PATTERN_PULL2 && c.kernel == KERNEL_NODE && c.bc == LBMK_PERIODIC && !c.Pd.ghost && c.collision == LBMK_COLLISION_BGK;
     const bool cl = can && g->ops->cluster_supported(c);
     if (g->opt_stepping == LBMK_STEPPING_AUTO)
         c.stepping = (cl && g->ops->linear) ? STEPPING_CLUSTER : (can && state2 <= (size_t(96) << 20)) ? STEPPING_PERSISTENT : STEPPING_LAUNCH;
@@ -782,6 +798,12 @@ lbmk_status lbmk_stream_index_map(lbmk_grid* g, int dir, long long* src_index_ou
 lbmk_status lbmk_grid_omega(const lbmk_grid* g, double* omega_out) {
     if (!g || !omega_out) return sys_fail(LBMK_EINVAL, "NULL argument");
     for (int k = 0; k < g->ops->M; ++k) omega_out[k] = g->c.Pd.omega[k];
+    return LBMK_OK;
+}
+
+lbmk_status lbmk_grid_omega_plus(const lbmk_grid* g, double* omega_out) {
+    if (!g || !omega_out) return sys_fail(LBMK_EINVAL, "NULL argument");
+    for (int k = 0; k < g->ops->M; ++k) omega_out[k] = g->c.Pd.omega_p[k];
     return LBMK_OK;
 }
 

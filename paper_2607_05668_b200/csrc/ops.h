@@ -37,6 +37,7 @@ struct GridCore {
     void* aux_buf;        // prescribed coefficient fields in R, [n_aux][aux_stride]
     long long aux_stride;
     bool aux_set;
+    int collision;        // 0 BGK, 1 TRT (two-lattice pull, node kernel, one launch per step)
     int stepping;         // STEPPING_LAUNCH: one launch per step; STEPPING_PERSISTENT: one cooperative launch per batch of steps
     int num_sms;          // cudaDevAttrMultiProcessorCount of the current device
     long long persistent_launches;   // cooperative launches so far (diagnostic)

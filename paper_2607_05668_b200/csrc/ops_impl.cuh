@@ -182,7 +182,10 @@ struct Ops {
         constexpr int BLOCK = Tune<S, R>::BLOCK, MINB = Tune<S, R>::MINB;
         const long long cnt = kp<R>(g).node1 - kp<R>(g).node0;
         if (cnt <= 0) return;
-        if (g.kernel == KERNEL_TWOPASS) {
+        if (g.collision == 1) {           // TRT: two-lattice modes of the node kernel only (checked at grid creation)
+            if constexpr (MODE == MODE_PULL2 || MODE == MODE_LOCAL)
+                collide_stream_node<S<R>, R, MODE, MMS, BLOCK, MINB, true><<<blocks_for(cnt, BLOCK), BLOCK, 0, g.stream>>>(src, dst, kp<R>(g));
+        } else if (g.kernel == KERNEL_TWOPASS) {
             constexpr int B2 = Tune2<S, R>::BLOCK, M2 = Tune2<S, R>::MINB;
             collide_stream_twopass<S<R>, R, MODE, MMS, B2, M2><<<blocks_for(cnt, B2), B2, 0, g.stream>>>(src, dst, kp<R>(g));
         } else {

@@ -1,0 +1,107 @@
+"""Two-relaxation-time collision (PAPER.md:L154 names TRT as an operator that consumes the compiler's equilibria unchanged; the
+paper itself runs BGK only, so there are no printed values: these are textbook pins).
+CPU: the oracle's TRT against (1) BGK when omega_plus = omega_minus, (2) the exact per-wavevector amplification matrix of the TRT
+collision for linear advection, built here from the definition (FFT -> 5x5 matrix power -> inverse FFT, as pin P4 does for
+BGK), (3) conservation, (4) the relaxation diffusion, which depends on omega_minus only (eq 2.17-2.18 with tau -> 1/omega_minus).
+GPU: the CUDA path against the oracle, element by element."""
+import numpy as np
+import pytest
+
+import oracle
+import workloads as W
+
+
+def _run(w, steps, **kw):
+    g = oracle.OracleGrid.from_workload(w, **kw)
+    if g.n_aux:
+        g.set_aux(w.aux_fields())
+    g.init_from_U(w.initial_U())
+    g.step(steps)
+    U, f = g.read_U(), g.read_f()
+    op, om = g.omega_plus(), g.omega()
+    g.close()
+    return U, f, op, om
+
+
+@pytest.mark.parametrize("mk,kw", [(W.c3_euler, dict(n=16)), (W.c2_swe, dict(n=16)), (W.c4_nsf3d, dict(n=8, precision="f64")), (W.pin_adr, dict(n=16))])
+def test_trt_with_equal_rates_is_bgk(mk, kw):
+    w = mk(**kw)
+    Ub, fb, _, om = _run(w, 15)
+    # per-component magic values are not settable; take a system-wide rate so that one Lambda makes omega_plus = omega_minus
+    o1 = float(om[0])
+    Ub, fb, _, _ = _run(w, 15, omega=o1)
+    Ut, ft, op, om = _run(w, 15, omega=o1, collision="trt", trt_magic=(1.0 / o1 - 0.5) ** 2)
+    assert np.allclose(op, om, rtol=1e-14)
+    assert np.abs(ft - fb).max() <= 1e-14 * np.abs(fb).max()
+
+
+def _trt_fourier_exact(U0, a, om_m, om_p, steps):
+    """Linear advection on D2Q5: per wavevector f^(t+1) = diag(e^{-i k.c_i}) [I - om_p P+ (I - E) - om_m P- (I - E)] f^(t), E_ij = feq
+    projector w_i (1 + c_i.a/c_s^2), P+- = (I +- R)/2 with R the swap of opposite directions."""
+    c = np.array([(0, 0), (1, 0), (-1, 0), (0, 1), (0, -1)], dtype=float)
+    wt = np.array([1 / 3, 1 / 6, 1 / 6, 1 / 6, 1 / 6])
+    cs2 = 1 / 3
+    ny, nx = U0.shape
+    E = np.outer(wt * (1 + c @ a / cs2), np.ones(5))
+    R = np.eye(5)[[0, 2, 1, 4, 3]]
+    Pp, Pm = (np.eye(5) + R) / 2, (np.eye(5) - R) / 2
+    Cmat = np.eye(5) - om_p * Pp @ (np.eye(5) - E) - om_m * Pm @ (np.eye(5) - E)
+    f0 = np.stack([wt[i] * (1 + c[i] @ a / cs2) * U0 for i in range(5)])
+    fh = np.fft.fft2(f0, axes=(1, 2))
+    kx = 2 * np.pi * np.fft.fftfreq(nx)[None, :]
+    ky = 2 * np.pi * np.fft.fftfreq(ny)[:, None]
+    out = np.zeros_like(fh)
+    for iy in range(ny):
+        for ix in range(nx):
+            ph = np.exp(-1j * (c[:, 0] * kx[0, ix] + c[:, 1] * ky[iy, 0]))
+            G = np.diag(ph) @ Cmat
+            out[:, iy, ix] = np.linalg.matrix_power(G, steps) @ fh[:, iy, ix]
+    return np.fft.ifft2(out, axes=(1, 2)).real.sum(0)
+
+
+@pytest.mark.parametrize("magic", [0.25, 3.0 / 16.0, 1.0])
+def test_trt_linear_advection_matches_the_exact_amplification_matrix(magic):
+    w = W.c1_advection(24, ny=16)
+    U, f, op, om = _run(w, 40, collision="trt", trt_magic=magic)
+    assert op[0] == pytest.approx(1.0 / (0.5 + magic / (1.0 / om[0] - 0.5)), rel=1e-14) and abs(op[0] - om[0]) > 1e-3
+    want = _trt_fourier_exact(w.initial_U()[0, 0], np.array(w.params), om[0], op[0], 40)
+    assert np.abs(U[0, 0] - want).max() < 2e-14
+
+
+def test_trt_conserves_totals_and_keeps_the_relaxation_diffusion():
+    """Sum_x U is conserved; the decay of a plane wave is set by omega_minus alone to leading order: the continuous closed form of
+    pin P4 (rate (1/omega_minus - 1/2) k^2 (2 c_s^2 - (a_x -+ a_y)^2) on the two diagonal plane waves) holds for any Lambda."""
+    w = W.c1_advection(64, noise=0.0)
+    U0 = w.initial_U()
+    for magic in (0.25, 0.05):
+        U, _, op, om = _run(w, 200, collision="trt", trt_magic=magic)
+        assert abs(U.sum() - U0.sum()) < 1e-9 * abs(U0.sum())
+        Ub, _, _, _ = _run(w, 200)
+        amp_t, amp_b = np.abs(U - 1.0).max(), np.abs(Ub - 1.0).max()
+        assert amp_t == pytest.approx(amp_b, rel=2e-3)          # same decay as BGK at the same omega_minus; differences are O(k^4)
+
+
+# ------------------------------------------------------------------------------------------------ GPU parity
+@pytest.mark.gpu
+@pytest.mark.parametrize("mk,kw,steps,prec", [(W.c1_advection, dict(n=37, ny=23), 51, "f64"), (W.c2_swe, dict(n=96, ny=50), 80, "f64"),
+                                              (W.c3_euler, dict(n=128, ny=72), 300, "f32s"), (W.c4_nsf3d, dict(n=32, ny=24, nz=20), 200, "f32s"),
+                                              (W.c5_mhd3d, dict(n=24, ny=10, nz=7), 60, "f64"), (W.pin_mhd2d, dict(n=40), 100, "f64")])
+def test_trt_gpu_matches_the_oracle(mk, kw, steps, prec):
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device")
+    import paper_2607_05668_b200 as P
+    from parity_metric import gate
+    w = mk(**kw)
+    g = P.Grid.from_workload(w, precision=prec, collision="trt", trt_magic=0.25, pattern="aa", stepping="persistent")   # resolve to pull2 / launch
+    assert (g.pattern, g.kernel, g.stepping) == ("pull2", "node", "launch")
+    g.init_from_U(w.initial_U())
+    g.step(steps)
+    U = g.read_U()
+    opg = P.lbmk_grid_omega_plus(g.h, w.m_total)
+    g.close()
+    Uo, fo, op, om = _run(w, steps, collision="trt", trt_magic=0.25)
+    assert np.allclose(opg, op, rtol=1e-14) and np.abs(op - om).max() > 1e-3
+    gate(U, Uo, fo, prec, f"{w.name}[trt]", U_ref=w.U_ref, steps=steps)
+    Ub = oracle.run(w, steps=steps)
+    assert np.abs(Uo - Ub).max() > 1e-9 * np.abs(Ub).max()       # a different operator, not BGK again
