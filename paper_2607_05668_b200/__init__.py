@@ -81,6 +81,8 @@ SYMBOLS = {
     "lbmk_stream_wait_boundary": (C.c_int, [_vp, _vp]),
     "lbmk_grid_wait_stream": (C.c_int, [_vp, _vp]),
     "lbmk_stream_index_map": (C.c_int, [_vp, C.c_int, _vp, C.c_int]),
+    "lbmk_generated_flux": (C.c_int, [C.c_int, _dp, _dp, _dp, C.c_int, C.c_double, C.c_double, C.c_double, _dp, _dp]),
+    "lbmk_flux_selfcheck": (C.c_int, [_vp, _dp]),
     "lbmk_lattice_constants": (C.c_int, [C.c_int, C.POINTER(C.c_int), _dp, _dp]),
     "lbmk_grid_omega": (C.c_int, [_vp, _dp]),
     "lbmk_grid_launch_count": (C.c_int, [_vp, C.POINTER(C.c_longlong)]),
@@ -310,6 +312,22 @@ def lbmk_error_norms(grid_h, m_total: int) -> np.ndarray:
 
 def lbmk_stream_index_map(grid_h, direction: int, ptr: int, on_device: bool):
     _check(lib().lbmk_stream_index_map(grid_h, direction, _vp(ptr), int(on_device)), grid_h)
+
+
+def lbmk_generated_flux(system_id: int, U, A, params, dx: float, lam: float, g_tau: float, m_total: int):
+    Ua, Up = _darr(U)
+    Aa, Ap = _darr(A if A is not None and len(A) else [0.0])
+    Pa, Pp = _darr(list(params) if len(params) else [0.0])
+    F, S = np.zeros((m_total, 3)), np.zeros(m_total)
+    _check(lib().lbmk_generated_flux(system_id, Up, Ap, Pp, len(params), float(dx), float(lam), float(g_tau),
+                                     F.ctypes.data_as(_dp), S.ctypes.data_as(_dp)))
+    return F, S
+
+
+def lbmk_flux_selfcheck(grid_h) -> float:
+    v = C.c_double()
+    _check(lib().lbmk_flux_selfcheck(grid_h, C.byref(v)), grid_h)
+    return v.value
 
 
 def lbmk_lattice_constants(lattice: int):

@@ -643,6 +643,52 @@ error_norms_kernel(const R* __restrict__ f, double* __restrict__ out, long long 
     }
 }
 
+// ------------------------------------------------------------------------------------------------ flux self-check
+// Every node of the current state: the hand-written delta form (Sys<double>: dF = F(Q0 + dQ) - F(Q0), s(Q0 + dQ)) against the
+// generated plain form (Gen: F(U), s(U); gen/cascade.py), in fp64.  out[0] = max over nodes and components of
+// |dF_hand - (F_gen(U) - F_gen(Q0))| and |s_hand - s_gen| relative to the node's largest |F_gen|, |s_gen| entry.
+template <class Sys, class Gen, class R>
+__global__ void __launch_bounds__(128)
+flux_selfcheck_kernel(const R* __restrict__ f, const R* __restrict__ aux, long long aux_stride, unsigned long long* __restrict__ out,
+                      long long n, int nx, int ny, int nz, int gather, const __grid_constant__ KParams<double> Pd,
+                      const __grid_constant__ GenArgs<double> ga) {
+    constexpr int D = Sys::D, Q = 2 * D + 1, M = Sys::M, NA = AuxCount<Sys>::value;
+    double worst = 0.0;
+    double F0[M * D], S0[M], Q0[M], A[NA > 0 ? NA : 1];
+    for (long long node = (long long)blockIdx.x * blockDim.x + threadIdx.x; node < n; node += (long long)gridDim.x * blockDim.x) {
+        const NodeIdx p = decompose(node, nx, ny);
+        double U[M], dQ[M];
+        for (int k = 0; k < M; ++k) {
+            double s = 0.0;
+#pragma unroll
+            for (int i = 0; i < Q; ++i) s += (double)load_canonical<Q, R>(f, M, k, i, node, p, nx, ny, nz, gather);
+            dQ[k] = s; Q0[k] = Pd.ref[k]; U[k] = Pd.ref[k] + s;
+        }
+        for (int a = 0; a < NA; ++a) A[a] = (double)aux[a * aux_stride + node];
+        typename Sys::Ctx ctx;
+        if constexpr (NA > 0) { double Aa[NA > 0 ? NA : 1]; for (int a = 0; a < NA; ++a) Aa[a] = A[a]; Sys::set_aux(ctx, Aa); }
+        Sys::setup(ctx, dQ, Pd);
+        double Fg[M * D], Sg[M];
+        Gen::template flux<double>(U, A, ga, Fg, Sg);
+        bool shifted = false;
+        for (int k = 0; k < M; ++k) shifted = shifted || Q0[k] != 0.0;
+        if (shifted) Gen::template flux<double>(Q0, A, ga, F0, S0);
+        else for (int q = 0; q < M * D; ++q) F0[q] = 0.0;
+        double scale = 1e-300;
+        for (int q = 0; q < M * D; ++q) scale = fmax(scale, fabs(Fg[q]));
+        for (int k = 0; k < M; ++k) scale = fmax(scale, fabs(Sg[k]));
+        static_for<0, M>([&](auto K) {
+            constexpr int k = decltype(K)::value;
+            double F[D], S;
+            Sys::template flux<k>(ctx, dQ, Pd, F, S);
+            for (int a = 0; a < D; ++a) worst = max_nan_inf(worst, fabs(F[a] - (Fg[k * D + a] - F0[k * D + a])) / scale);
+            worst = max_nan_inf(worst, fabs(S - Sg[k]) / scale);
+        });
+    }
+    worst = warp_max(worst);
+    if ((threadIdx.x & 31) == 0) atomicMax(out, (unsigned long long)__double_as_longlong(worst));
+}
+
 // ------------------------------------------------------------------------------------------------ a11
 // Dirichlet-MMS frame (reading A18; the paper defines no boundary operator):
 // the outermost node layer is reset to f_eq(Q_exact(x_b, t_n)) in canonical slots.  One thread per frame

@@ -13,6 +13,7 @@
 #include <string>
 
 #include "api_kernels.cuh"
+#include "cascade_generated.cuh"
 #include "ops.h"
 
 using namespace lbmk;
@@ -84,6 +85,15 @@ static lbmk_status cuda_fail(lbmk_grid* g, cudaError_t e, const char* where) {
 #define CK(g, call, where) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail((g), e_, (where)); } while (0)
 
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// evaluation of one emitted system (gen/cascade.py -> cascade_generated.cuh) on the host
+template <class Gen>
+static void gen_eval(const double* U, const double* A, const GenArgs<double>& ga, double* F3, double* S) {
+    double F[LBMK_MAX_COMPONENTS * 3], A0[8] = {0};
+    Gen::template flux<double>(U, A ? A : A0, ga, F, S);
+    for (int k = 0; k < Gen::M; ++k)
+        for (int a = 0; a < 3; ++a) F3[k * 3 + a] = a < Gen::D ? F[k * Gen::D + a] : 0.0;
+}
 
 extern "C" {
 
@@ -774,6 +784,39 @@ lbmk_status lbmk_error_norms(lbmk_grid* g, double* out) {
     CK(g, cudaMemcpyAsync(out, st.dev, bytes, cudaMemcpyDeviceToHost, c.stream), "cudaMemcpyAsync D2H");
     CK(g, cudaStreamSynchronize(c.stream), "cudaStreamSynchronize");
     CK(g, st.release(), "cudaFreeAsync");
+    return LBMK_OK;
+}
+
+// ---- generated augmented systems (gen/cascade.py -> cascade_generated.cuh)
+lbmk_status lbmk_generated_flux(lbmk_system_id id, const double* U, const double* A, const double* params, int n_params,
+                                double dx, double lambda, double g_tau, double* F_out, double* S_out) {
+    if (!U || !F_out || !S_out) return sys_fail(LBMK_EINVAL, "NULL argument");
+    if (id < 0 || id >= LBMK_SYS_COUNT || n_params != N_PARAMS[id] || (n_params > 0 && !params)) return sys_fail(LBMK_EINVAL, "unknown system or wrong parameter count");
+    if (!(dx > 0.0) || !(lambda > 0.0) || !(g_tau > 0.0)) return sys_fail(LBMK_EINVAL, "dx, lambda, g_tau must be > 0");
+    GenArgs<double> ga;
+    memset(&ga, 0, sizeof ga);
+    for (int i = 0; i < n_params; ++i) ga.par[i] = params[i];
+    ga.dx = dx; ga.dt = dx / lambda; ga.gtau = g_tau;
+    switch (id) {
+        case LBMK_SYS_EULER2D: gen_eval<Gen_euler2d>(U, A, ga, F_out, S_out); break;
+        case LBMK_SYS_SWE2D_BATHY: gen_eval<Gen_swe2d_bathy>(U, A, ga, F_out, S_out); break;
+        case LBMK_SYS_ADR2D: gen_eval<Gen_adr2d>(U, A, ga, F_out, S_out); break;
+        case LBMK_SYS_ALLENCAHN2D: gen_eval<Gen_allencahn2d>(U, A, ga, F_out, S_out); break;
+        case LBMK_SYS_INSE2D: gen_eval<Gen_inse2d>(U, A, ga, F_out, S_out); break;
+        case LBMK_SYS_NSF2D_GRADTRACK: gen_eval<Gen_nsf2d>(U, A, ga, F_out, S_out); break;
+        case LBMK_SYS_MHD2D: gen_eval<Gen_mhd2d>(U, A, ga, F_out, S_out); break;
+        case LBMK_SYS_NSF3D_GRADTRACK: gen_eval<Gen_nsf3d>(U, A, ga, F_out, S_out); break;
+        default: return sys_fail(LBMK_EUNSUPPORTED, "no generated augmented system for this id (gen/cascade.py)");
+    }
+    return LBMK_OK;
+}
+
+lbmk_status lbmk_flux_selfcheck(lbmk_grid* g, double* max_rel_diff) {
+    lbmk_status s = need_inited(g);
+    if (s != LBMK_OK) return s;
+    if (!max_rel_diff) return fail(g, LBMK_EINVAL, "output is NULL");
+    if (!g->ops->has_generated) return fail(g, LBMK_EUNSUPPORTED, "no generated augmented system for this system (gen/cascade.py)");
+    CK(g, g->ops->flux_selfcheck(g->c, g->sys.g_tau, max_rel_diff), "flux_selfcheck kernel");
     return LBMK_OK;
 }
 

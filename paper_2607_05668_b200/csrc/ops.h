@@ -69,7 +69,9 @@ struct SysOps {
     cudaError_t (*max_wave_speed)(GridCore&, double* out3_host);
     cudaError_t (*error_norms)(GridCore&, double* out_dev /*[M][6], zeroed here*/);
     bool (*row_kernel_supported)(const GridCore&);
-    bool (*cluster_supported)(const GridCore&);     // the grid fits the cluster-resident kernel (kernels.cuh collide_stream_cluster)
+    bool (*cluster_supported)(const GridCore&);
+    bool has_generated;   // gen/cascade.py emits this system: lbmk_flux_selfcheck is available
+    cudaError_t (*flux_selfcheck)(GridCore&, double g_tau, double* out_host);     // the grid fits the cluster-resident kernel (kernels.cuh collide_stream_cluster)
 };
 
 const SysOps* ops_advection2d();

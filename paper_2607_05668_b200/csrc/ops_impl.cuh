@@ -432,12 +432,41 @@ struct Ops {
         if (e != cudaSuccess) return e;
         return g.prec == PREC_F64 ? norms_t<double>(g, out) : norms_t<float>(g, out);
     }
+    using Gen = typename GenOf<S>::type;
+    static constexpr bool HAS_GEN = !std::is_void<Gen>::value;
+    template <class R>
+    static cudaError_t selfcheck_t(GridCore& g, double g_tau, double* out_host) {
+        if constexpr (HAS_GEN) {
+            cudaError_t e = cudaMemsetAsync(g.red, 0, sizeof(unsigned long long), g.stream);
+            if (e != cudaSuccess) return e;
+            GenArgs<double> ga;
+            for (int i = 0; i < 8; ++i) ga.par[i] = g.Pd.par[i];
+            ga.dx = g.mh.dx; ga.dt = g.dt; ga.gtau = g_tau;
+            const unsigned nb = (unsigned)std::min<long long>((g.n + 127) / 128, (long long)g.num_sms * 8);
+            flux_selfcheck_kernel<Sd, Gen, R><<<nb, 128, 0, g.stream>>>((const R*)g.f[g.cur], (const R*)g.aux_buf, g.aux_stride, g.red, g.n,
+                                                                        g.nx, g.ny, g.nz, aa_odd(g), g.Pd, ga);
+            g.launches++;
+            e = cudaGetLastError();
+            if (e != cudaSuccess) return e;
+            unsigned long long h = 0;
+            e = cudaMemcpyAsync(&h, g.red, sizeof(h), cudaMemcpyDeviceToHost, g.stream);
+            if (e != cudaSuccess) return e;
+            e = cudaStreamSynchronize(g.stream);
+            if (e != cudaSuccess) return e;
+            memcpy(out_host, &h, 8);
+            return cudaSuccess;
+        }
+        return cudaErrorNotSupported;
+    }
+    static cudaError_t flux_selfcheck(GridCore& g, double g_tau, double* out_host) {
+        return g.prec == PREC_F64 ? selfcheck_t<double>(g, g_tau, out_host) : selfcheck_t<float>(g, g_tau, out_host);
+    }
     static bool row_supported(const GridCore&) { return false; }
 
     static const SysOps* get() {
         static const SysOps ops = {Sd::ID, D, M, Sd::MC, HAS_MMS, C::NT, {C::NX, C::NY, C::NZ}, C::NC, NA, IsLinear<Sd>::value,
                                    &fill_tables, &reference_equilibrium, &init_from_U, &set_f, &step, &step_ranges, &set_aux,
-                                   &read_U_with_frame, &read_f, &max_wave_speed, &error_norms, &row_supported, &cluster_supported};
+                                   &read_U_with_frame, &read_f, &max_wave_speed, &error_norms, &row_supported, &cluster_supported, HAS_GEN, &flux_selfcheck};
         return &ops;
     }
 };

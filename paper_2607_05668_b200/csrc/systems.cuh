@@ -21,6 +21,7 @@
 // Systems with prescribed per-node coefficient fields (the bed slope of eq 3.5) also declare
 //   NA (their number), set_aux(Ctx&, A[NA]) -- called before setup with this node's values -- and default_aux(Ctx&).
 #pragma once
+#include "cascade_generated.cuh"
 #include "common.cuh"
 
 namespace lbmk {
@@ -806,5 +807,18 @@ template <class R> struct SysMhd2D {
         out[2] = sqrt(kap * P.inv_gtau);
     }
 };
+
+// ------------------------------------------------------------------------------------------ generated counterparts
+// The plain lattice flux/source that gen/cascade.py DERIVES (Alg 2.1 Split/Cascade/Assemble/Emit) for the same system, where one
+// is emitted: what lbmk_flux_selfcheck compares the hand-written delta form against.
+template <template <class> class S> struct GenOf { using type = void; };
+template <> struct GenOf<SysEuler2D> { using type = Gen_euler2d; };
+template <> struct GenOf<SysSwe2DBathy> { using type = Gen_swe2d_bathy; };
+template <> struct GenOf<SysAdr2D> { using type = Gen_adr2d; };
+template <> struct GenOf<SysAllenCahn2D> { using type = Gen_allencahn2d; };
+template <> struct GenOf<SysInse2D> { using type = Gen_inse2d; };
+template <> struct GenOf<SysNsf2D> { using type = Gen_nsf2d; };
+template <> struct GenOf<SysMhd2D> { using type = Gen_mhd2d; };
+template <> struct GenOf<SysNsf3D> { using type = Gen_nsf3d; };
 
 }  // namespace lbmk

@@ -199,3 +199,30 @@ def test_mhd2d_subcharacteristic_reduction_matches_the_oracle(P):
     o = oracle.OracleGrid.from_workload(w); o.init_from_U(w.initial_U()); o.step(30)
     so = o.max_wave_speed(); o.close()
     assert status == 0 and np.allclose(sp, so, rtol=1e-11)
+
+
+# ------------------------------------------------------------------------------------------- generated vs hand-written flux
+@pytest.mark.parametrize("mk,kw,prec,steps", [
+    (W.pin_euler, dict(n=48), "f64s", 40), (W.pin_swe, dict(n=40), "f64", 30), (W.pin_adr, dict(n=32), "f64s", 60),
+    (W.pin_allencahn, dict(n=32), "f64", 60), (W.pin_inse, dict(n=32), "f64s", 60), (W.pin_nsf2d, dict(n=40), "f64s", 80),
+    (W.pin_mhd2d, dict(n=40), "f64s", 80), (W.c4_nsf3d, dict(n=16, ny=12, nz=10), "f64s", 30), (W.c4_nsf3d, dict(n=16, ny=12, nz=10), "f32s", 30)])
+def test_hand_written_delta_forms_equal_the_generated_augmented_systems(P, mk, kw, prec, steps):
+    """SURVEY section 8(f) item 2: gen/cascade.py DERIVES the augmented system (Alg 2.1 Split/Cascade/Assemble/Emit, PAPER.md:L221-L278);
+    lbmk_flux_selfcheck evaluates, on every node of a live state, the hand-written delta-form flux/source the step kernels use and
+    the emitted plain form, both in fp64: they agree to rounding (reference state subtracted analytically vs numerically)."""
+    w = mk(**kw)
+    g = P.Grid.from_workload(w, precision=prec)
+    g.init_from_U(w.initial_U())
+    g.step(steps)
+    d = P.lbmk_flux_selfcheck(g.h)
+    g.close()
+    assert 0.0 <= d <= 5e-12, d
+
+
+def test_flux_selfcheck_needs_a_generated_system(P):
+    w = W.pin_urf(16)
+    g = P.Grid.from_workload(w); g.init_from_U(w.initial_U())
+    with pytest.raises(P.LbmkError) as e:
+        P.lbmk_flux_selfcheck(g.h)
+    assert e.value.status == 6
+    g.close()
