@@ -117,9 +117,9 @@ def test_a11_dirichlet_mms_frame_parity(P, mk, kw, steps, tol):
 
 # ------------------------------------------------------------------------ staged forcing coefficients
 @pytest.mark.parametrize("mk,kw,steps,tol", [
-    (W.c4_nsf3d, dict(n=128, ny=6, nz=5), 12, TOL32),                       # BLOCK = 128, fp32 shifted
+    (W.c4_nsf3d, dict(n=128, ny=6, nz=5), 12, TOL32),                       # nx = 2 blocks of 64 (c4 fp32 launch shape): staged, fp32 shifted
     (W.c4_nsf3d, dict(n=256, ny=4, nz=3, precision="f64"), 6, TOL64),
-    (W.c2_swe, dict(n=256, ny=12), 40, TOL64),                              # BLOCK = 256, fp64
+    (W.c2_swe, dict(n=256, ny=12), 40, TOL64),                              # nx = 2 blocks of 128 (2D launch shape): staged, fp64
     (W.c2_swe, dict(n=512, ny=9, precision="f32s"), 40, TOL32),
     (W.pin_burgers, dict(n=256), 20, TOL64)])
 @pytest.mark.parametrize("pattern", ["pull2", "aa"])
@@ -152,11 +152,13 @@ def test_degenerate_grids_parity(P, name, kw, pattern):
 
 # ------------------------------------------------------------------------ out-of-bounds guard (no sanitizer on this pool)
 @pytest.mark.parametrize("mk,kw", [(W.c1_advection, dict(n=37, ny=23)), (W.c4_nsf3d, dict(n=5, ny=4, nz=3)), (W.c4_nsf3d, dict(n=130, ny=3, nz=2)),
-                                   (W.c5_mhd3d, dict(n=9, ny=2, nz=5)), (W.c2_swe, dict(n=257, ny=3)), (W.pin_nsf2d, dict(n=19))])
-@pytest.mark.parametrize("pattern", ["pull2", "aa"])
-def test_workspace_guards_stay_untouched(P, mk, kw, pattern):
+                                   (W.c5_mhd3d, dict(n=9, ny=2, nz=5)), (W.c2_swe, dict(n=257, ny=3)), (W.pin_nsf2d, dict(n=19)),
+                                   (W.pin_swe, dict(n=21)), (W.hcnsf3d, dict(n=7, ny=5, nz=3)), (W.pin_mhd2d, dict(n=13))])
+@pytest.mark.parametrize("pattern,stepping", [("pull2", "launch"), ("aa", "launch"), ("pull2", "persistent"), ("pull2", "cluster")])
+def test_workspace_guards_stay_untouched(P, mk, kw, pattern, stepping):
     """The workspace is bound inside a larger buffer filled with a sentinel; after init, steps (ragged last tile, wraps
-    on every axis, forcing tables), reductions and readbacks the guard bands before and after it are unchanged."""
+    on every axis, forcing tables, prescribed fields; per-launch, persistent and cluster-resident stepping), reductions,
+    readbacks and the flux self-check the guard bands before and after it are unchanged (compute-sanitizer is closed on this pool)."""
     import torch
     w = mk(**kw)
     s = P.System(w.system, params=w.params, tau_R=w.tau_R, g_tau=w.g_tau, U_ref=w.U_ref, mms_id=w.mms_id,
@@ -164,6 +166,7 @@ def test_workspace_guards_stay_untouched(P, mk, kw, pattern):
     prec = {"f64": P.LBMK_F64, "f32s": P.LBMK_F32_SHIFTED}[w.precision]
     g = P.lbmk_grid_create(s.h, w.nx, w.ny, w.nz, 0, w.dx, w.lam, prec, torch.cuda.current_stream().cuda_stream)
     P.lbmk_grid_set_option(g, P.LBMK_OPT_PATTERN, P.PATTERN[pattern])
+    P.lbmk_grid_set_option(g, P.LBMK_OPT_STEPPING, P.STEPPING[stepping])
     nbytes = P.lbmk_grid_workspace_bytes(g)
     G = 1 << 16
     buf = torch.full((nbytes + 2 * G + 256,), 0xA5, dtype=torch.uint8, device="cuda")
@@ -171,11 +174,16 @@ def test_workspace_guards_stay_untouched(P, mk, kw, pattern):
     P.lbmk_grid_bind_workspace(g, buf.data_ptr() + off, nbytes)
     U0 = torch.from_numpy(w.initial_U()).cuda()
     out = torch.empty_like(U0)
+    if w.n_aux:
+        A = torch.from_numpy(w.aux_fields()).cuda()
+        P.lbmk_set_aux_fields(g, A.data_ptr(), True)
     P.lbmk_init_from_U(g, U0.data_ptr(), True)
     for n in (1, 2, 5):
         P.lbmk_step(g, n)
         P.lbmk_read_U(g, out.data_ptr(), True)
         P.lbmk_check_subcharacteristic(g, raise_on_violation=False)
+    if w.system in ("swe2d_bathy", "mhd2d", "nsf2d"):
+        P.lbmk_flux_selfcheck(g)
     torch.cuda.synchronize()
     assert bool((buf[:off] == 0xA5).all()) and bool((buf[off + nbytes:] == 0xA5).all())
     assert bool(torch.isfinite(out).all())
