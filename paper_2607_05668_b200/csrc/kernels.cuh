@@ -354,6 +354,47 @@ collide_stream_cluster(const R* __restrict__ gsrc, R* __restrict__ gdst, const _
     }
 }
 
+// ------------------------------------------------------------------------------------------------ step, several nodes per thread
+// Single-field systems (Burgers, advection: 5 populations per node) do not keep enough loads in flight with one node per
+// thread to cover the HBM latency (64 warps x 5 loads x 128 B = 41 KB per SM against ~37 KB needed by Little's law: 94 % of the
+// copy peak).  Here a thread gathers NPT nodes (BLOCK apart, so every warp access stays one full 128-byte line) before it
+// collides any of them: NPT x the memory-level parallelism, same collide_core.  Two-lattice modes, no forcing, no prescribed fields.
+template <class Sys, class R, int MODE, int BLOCK, int NPT>
+__global__ void __launch_bounds__(BLOCK)
+collide_stream_multi(typename StepPtr<R, MODE>::Src src, typename StepPtr<R, MODE>::Dst dst, const __grid_constant__ KParams<R> P) {
+    constexpr int D = Sys::D, Q = 2 * D + 1, M = Sys::M;
+    static_assert(MODE == MODE_PULL2 || MODE == MODE_LOCAL, "two-lattice modes only");
+    const long long first = P.node0 + (long long)blockIdx.x * (BLOCK * NPT) + threadIdx.x;
+    R f[NPT][M][Q];
+#pragma unroll
+    for (int j = 0; j < NPT; ++j) {
+        const long long node = first + (long long)j * BLOCK;
+        if (node < P.node1) {
+            const NodeIdx p = decompose(node, P.nx, P.ny);
+#pragma unroll
+            for (int i = 0; i < Q; ++i) {
+                const R* sp = src + tile_off(node + (MODE == MODE_LOCAL ? 0LL : pull_offset(i, p, P.nx, P.ny, P.nz)), M * Q);
+#pragma unroll
+                for (int k = 0; k < M; ++k) f[j][k][i] = sp[(k * Q + i) * TILE];
+            }
+        }
+    }
+    R smms[M];
+#pragma unroll
+    for (int j = 0; j < NPT; ++j) {
+        const long long node = first + (long long)j * BLOCK;
+        if (node < P.node1) {
+            typename Sys::Ctx ctx;
+            R* const dp = dst + tile_off(node, M * Q);
+            collide_core<Sys, R, false>(f[j], ctx, P, smms, [&](auto K, const R* fk) {
+                constexpr int k = decltype(K)::value;
+#pragma unroll
+                for (int i = 0; i < Q; ++i) dp[(k * Q + i) * TILE] = fk[i];
+            });
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ step, two-pass
 // Low-register variant using the linearity of BGK in f (SURVEY.md §7 option iii):
 //   f'_k,i = (1 - omega_k) f_k,i + c_k,i,   c_k,0 = w0 (omega dQ_k + s_k),  c_k,+-a = w1 (omega dQ_k + s_k) +- (omega/2) dF_k,a.

@@ -226,3 +226,14 @@ def test_flux_selfcheck_needs_a_generated_system(P):
         P.lbmk_flux_selfcheck(g.h)
     assert e.value.status == 6
     g.close()
+
+
+def test_multi_node_kernel_for_single_field_fp32_is_bit_identical(P):
+    """Single-field fp32 systems on grids of >= 128*4*SMs nodes step with 4 nodes per thread (collide_stream_multi): same bits as the
+    one-node-per-thread code (the persistent kernel runs node_step), same parity against the oracle; ragged tail, odd sizes."""
+    w = W.relabel(W.pin_burgers(301, precision="f32s"), ny=277, mms_id=0)          # 83 377 nodes, not a multiple of anything
+    U1, f1, (m1, l1) = gpu_run(P, w, 9, [1, 8], pattern="pull2", stepping="launch")
+    U2, f2, (m2, l2) = gpu_run(P, w, 9, [1, 8], pattern="pull2", stepping="persistent")
+    assert (m1, m2) == ("launch", "persistent") and np.array_equal(f1, f2)
+    Uo, fo = oracle_run(w, 9)
+    gate(U1, Uo, fo, "f32s", f"{w.name}[multi]", U_ref=w.U_ref, steps=9, strict=False)
