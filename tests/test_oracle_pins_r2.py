@@ -13,6 +13,8 @@ oracle formula: each compares the oracle's TIME STEPPING (or its flux through a 
        (|u.n| + c for Euler / NSF / weakly compressible NSE / SWE over a bed / MHD 2D fast speed); the tracker-parent
        signal speed out[2] equals the spectral radius of the augmented Jacobian for the purely diffusive pairs, and the sum
        used by the check bounds the spectral radius of the full augmented Jacobian.
+  P21  configs[2] (Euler free evolution): the same workload recipe at amplitude 1e-6 against the closed-form LINEAR acoustics of its
+       own seeded fields (standing pressure waves, steady entropy part), second-order approach under refinement.
   P11  on the configs themselves: c2 at N = 64, 128, 256 and the fp64 build of c4 at N = 16, 32, 64, to a fixed time:
        L2 slope in the paper's band 1.7-2.5.
 """
@@ -274,3 +276,39 @@ def test_p11_c4_refinement_order_fp64():
     for k in range(5):
         slope = -np.polyfit(np.log2(ns), np.log2([e[k] for e in errs]), 1)[0]
         assert 1.7 <= slope <= 2.5, (k, slope, [e[k] for e in errs])
+
+
+# ------------------------------------------------------------------------------------------------ P21 config 3 against linear acoustics
+def test_p21_c3_free_evolution_matches_linear_acoustics_at_small_amplitude():
+    """configs[2] (Euler, u = 0, seeded smooth density / pressure perturbations) has no closed form at its amplitude 1e-2, but its
+    linearisation has: with c^2 = gamma p0/rho0 = 1 every Fourier mode of the pressure is a standing wave dp_k(t) = dp_k(0) cos(c|k|t),
+    the density follows as drho_k(t) = drho_k(0) + (cos(c|k|t) - 1) dp_k(0)/c^2 (the entropy part stays), the momentum is
+    m_k(t) = -i k dp_k(0) sin(c|k|t)/(c|k|).  The oracle run of the SAME workload recipe at amplitude 1e-6 (nonlinear terms 1e-12)
+    must follow it up to the scheme's own O(dx^2) + relaxation-diffusion error; run at two resolutions, the deviation falls."""
+    devs = []
+    for n in (64, 128):
+        w = W.c3_euler(n, precision="f64")
+        w.mms_params = [1e-6]                                   # amplitude of the seeded perturbations
+        w.tau_R = 0.2
+        U0 = w.initial_U()
+        steps = int(round(0.3 / w.dt))
+        U = oracle.run(w, steps=steps, U0=U0)
+        t = steps * w.dt
+        gamma = w.params[0]
+        rho0, p0 = 1.0, 1.0 / gamma
+        drho0 = U0[0, 0] - rho0
+        dp0 = (gamma - 1.0) * U0[3, 0] - p0
+        kx = 2 * np.pi * np.fft.fftfreq(n, d=w.dx)[None, :]
+        ky = 2 * np.pi * np.fft.fftfreq(n, d=w.dx)[:, None]
+        kk = np.sqrt(kx ** 2 + ky ** 2)
+        ph = np.fft.fft2(dp0)
+        cos_, sin_over = np.cos(kk * t), np.where(kk > 0, np.sin(kk * t) / np.where(kk > 0, kk, 1.0), t)
+        dp_t = np.fft.ifft2(ph * cos_).real
+        drho_t = drho0 + np.fft.ifft2(ph * (cos_ - 1.0)).real
+        mx_t = np.fft.ifft2(-1j * kx * ph * sin_over).real
+        u = U[1, 0] / U[0, 0]
+        p = (gamma - 1.0) * (U[3, 0] - 0.5 * U[0, 0] * (u ** 2 + (U[2, 0] / U[0, 0]) ** 2))
+        amp = np.abs(dp0).max()
+        dev = max(np.abs(p - p0 - dp_t).max(), np.abs(U[0, 0] - rho0 - drho_t).max(), np.abs(U[1, 0] - mx_t).max()) / amp
+        devs.append(dev)
+    assert devs[1] < 0.02 and devs[1] < 0.45 * devs[0], devs      # second-order approach to the linear solution
