@@ -150,8 +150,11 @@ lbmk_status lbmk_system_set_mms(lbmk_system* sys, int mms_id, const double* mms_
  * omega_minus = the component's rate omega_k (f_eq- = w_i c_i.F/c_s^2 carries the flux, so the relaxation diffusion of eq 2.17 is
  * unchanged) and omega_plus from the magic parameter Lambda = (1/omega_plus - 1/2)(1/omega_minus - 1/2) (`magic` > 0; 1/4 is the
  * usual choice).  TRT runs on the two-lattice pull pattern with the node kernel, one launch per step (other options resolve
- * to these).  Not a paper result: pinned by textbook properties, tests/test_trt.py. */
-enum { LBMK_COLLISION_BGK = 0, LBMK_COLLISION_TRT = 1 };
+ * to these).  LBMK_COLLISION_REGULARIZED (the other operator L154 names): the non-equilibrium part is projected onto its first
+ * moment before it is relaxed, f_neq,i -> w_i c_i.Pi/c_s^2 with Pi = sum_j c_j (f_j - f_eq,j); on D2Q5 / D3Q7 this keeps the
+ * antisymmetric parts and removes the symmetric ones, so it runs as the two-rate kernel with omega_plus = 1 (`magic` ignored).
+ * Not paper results: pinned by textbook properties and by the projection written out, tests/test_trt.py. */
+enum { LBMK_COLLISION_BGK = 0, LBMK_COLLISION_TRT = 1, LBMK_COLLISION_REGULARIZED = 2 };
 lbmk_status lbmk_system_set_collision(lbmk_system* sys, int collision, double magic);
 /* A-priori bound on the physical wave speed max|eig sum n_a A_a| from the declared amplitudes (eq 2.20).
  * lbmk_grid_create rejects the grid with LBMK_ESUBCHAR if s_max/lambda > c_s.  0 = no declared bound. */

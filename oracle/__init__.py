@@ -110,7 +110,7 @@ class OracleGrid:
         s.shifted = int(bool(shifted))
         s.mms_id = mms_id
         s.n_threads = n_threads
-        s.collision = {"bgk": 0, "trt": 1}[collision]
+        s.collision = {"bgk": 0, "trt": 1, "regularized": 2}[collision]
         s.trt_magic = trt_magic
         s.ox, s.oy, s.oz = origin
         s.dx, s.lam, s.g_tau, s.t0 = dx, lam, g_tau, t0

@@ -174,7 +174,7 @@ static void one_step(Grid& G) {
                     for (int i = 0; i < Q; ++i) {
                         const double fi = G.f[(int64_t)(k * Q + i) * G.n + nd];
                         double fpost = fi - G.omega[k] * (fi - feq[k * Q + i]) + L.w[i] * S[k];
-                        if (G.s.collision == 1) {
+                        if (G.s.collision != 0) {
                             // two-relaxation-time operator (textbook form; the paper names it at L154 as consuming the same
                             // equilibria): with ibar the direction opposite to i,  f+- = (f_i +- f_ibar)/2  and likewise f_eq+-,
                             //   f' = f_i - omega_plus (f+ - f_eq+) - omega_minus (f- - f_eq-) + w_i s_k .
@@ -236,6 +236,10 @@ void* orc_create(const Spec* sp) {
         // Lambda = (1/omega_plus - 1/2)(1/omega_minus - 1/2); omega_minus = 2 (no relaxation diffusion) leaves omega_plus free: 1
         const double tm = 1.0 / om - 0.5;
         G->omega_plus[k] = (sp->collision == 1 && om > 0.0) ? (tm > 0.0 ? 1.0 / (0.5 + sp->trt_magic / tm) : 1.0) : om;
+        // collision 2, regularised: the non-equilibrium part is projected onto its first moment before relaxing,
+        // f_neq,i -> w_i c_i.Pi/c_s^2, Pi = sum_j c_j (f_j - f_eq,j); on D2Q5 / D3Q7 that leaves the antisymmetric parts untouched and
+        // removes the symmetric ones, i.e. it IS the two-rate form with omega_plus = 1 (pinned against the projection in tests/test_trt.py)
+        if (sp->collision == 2) G->omega_plus[k] = 1.0;
     }
     {   // F0 = F(Q0) for the shifted storage, eq (2.23)
         double S[MAXM];

@@ -386,7 +386,7 @@ class System:
         if s_max:
             lbmk_system_set_wave_speed_bound(self.h, s_max)
         if collision != "bgk":
-            lbmk_system_set_collision(self.h, {"bgk": 0, "trt": 1}[collision], trt_magic)
+            lbmk_system_set_collision(self.h, {"bgk": 0, "trt": 1, "regularized": 2}[collision], trt_magic)
 
     def close(self):
         if getattr(self, "h", None):

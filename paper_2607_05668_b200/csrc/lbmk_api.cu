@@ -218,7 +218,8 @@ lbmk_status lbmk_system_set_mms(lbmk_system* sys, int mms_id, const double* mms_
 
 lbmk_status lbmk_system_set_collision(lbmk_system* sys, int collision, double magic) {
     if (!sys) return sys_fail(LBMK_EINVAL, "sys is NULL");
-    if (collision != LBMK_COLLISION_BGK && collision != LBMK_COLLISION_TRT) return sys_fail(LBMK_EINVAL, "unknown collision operator");
+    if (collision != LBMK_COLLISION_BGK && collision != LBMK_COLLISION_TRT && collision != LBMK_COLLISION_REGULARIZED)
+        return sys_fail(LBMK_EINVAL, "unknown collision operator");
     if (collision == LBMK_COLLISION_TRT && !(magic > 0.0)) return sys_fail(LBMK_EINVAL, "TRT magic parameter must be > 0");
     sys->collision = collision;
     sys->trt_magic = magic;
@@ -258,6 +259,7 @@ static void derive_params(lbmk_grid* g) {
         // TRT: Lambda = (1/omega_p - 1/2)(1/omega - 1/2); omega = 2 leaves omega_p free (1); omega = 0 (no collision) keeps 0
         const double tm = om > 0.0 ? 1.0 / om - 0.5 : 0.0;
         P.omega_p[k] = (s.collision == LBMK_COLLISION_TRT && om > 0.0) ? (tm > 0.0 ? 1.0 / (0.5 + s.trt_magic / tm) : 1.0) : om;
+        if (s.collision == LBMK_COLLISION_REGULARIZED) P.omega_p[k] = 1.0;     // projection of f_neq onto its first moment = symmetric parts fully relaxed
         P.ref[k] = is_shifted(g->precision) ? s.ref[k] : 0.0;
     }
     for (int i = 0; i < 8; ++i) P.par[i] = s.par[i];
@@ -319,14 +321,14 @@ static void resolve_options(lbmk_grid* g) {
     c.pattern = g->opt_pattern == LBMK_PATTERN_AUTO ? PATTERN_PULL2 : (int)g->opt_pattern;
     if (c.bc == LBMK_DIRICHLET_MMS) c.pattern = PATTERN_PULL2;      // the frame refill needs canonical storage
     c.kernel = g->opt_kernel == LBMK_KERNEL_AUTO ? KERNEL_NODE : (int)g->opt_kernel;
-    c.collision = g->sys.collision;
-    if (c.collision == LBMK_COLLISION_TRT) { c.pattern = PATTERN_PULL2; c.kernel = KERNEL_NODE; }   // the variants TRT is compiled for
+    c.collision = g->sys.collision != LBMK_COLLISION_BGK ? 1 : 0;          // TRT and regularised share the two-rate kernel
+    if (c.collision != 0) { c.pattern = PATTERN_PULL2; c.kernel = KERNEL_NODE; }   // the variants TRT is compiled for
     if (c.kernel == KERNEL_ROW && !g->ops->row_kernel_supported(c)) c.kernel = KERNEL_NODE;
     // Stepping: grids whose two population copies fit in L2 are launch-latency bound, not bandwidth bound (c1: 0.3 MB,
     // c2: 63 MB against 126 MB of L2) -> one cooperative launch per batch of steps; larger grids: one launch per step.
     const size_t esz = c.prec == PREC_F64 ? 8 : 4;
     const size_t state2 = 2 * (size_t)g->ops->M * (2 * g->ops->D + 1) * (size_t)c.n * esz;
-    const bool can = c.pattern == PATTERN_PULL2 && c.kernel == KERNEL_NODE && c.bc == LBMK_PERIODIC && !c.Pd.ghost && c.collision == LBMK_COLLISION_BGK;
+    const bool can = c.pattern == PATTERN_PULL2 && c.kernel == KERNEL_NODE && c.bc == LBMK_PERIODIC && !c.Pd.ghost && c.collision == 0;
     const bool cl = can && g->ops->cluster_supported(c);
     if (g->opt_stepping == LBMK_STEPPING_AUTO)
         c.stepping = (cl && g->ops->linear) ? STEPPING_CLUSTER : (can && state2 <= (size_t(96) << 20)) ? STEPPING_PERSISTENT : STEPPING_LAUNCH;

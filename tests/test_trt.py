@@ -81,27 +81,60 @@ def test_trt_conserves_totals_and_keeps_the_relaxation_diffusion():
         assert amp_t == pytest.approx(amp_b, rel=2e-3)          # same decay as BGK at the same omega_minus; differences are O(k^4)
 
 
+def test_regularized_operator_is_the_projection_of_the_non_equilibrium_part():
+    """LBMK_COLLISION_REGULARIZED against the definition written out in NumPy on a tiny Euler grid: f_neq = f - f_eq is replaced by
+    w_i c_i.Pi/c_s^2, Pi = sum_j c_j f_neq,j (its first moment; the zeroth vanishes), then f' = f_eq + (1 - omega) f_neq^reg + w_i s,
+    streamed periodically.  (The oracle runs it as the two-rate form with omega_plus = 1.)"""
+    w = W.c3_euler(8, ny=6, precision="f64")
+    c = np.array([(0, 0), (1, 0), (-1, 0), (0, 1), (0, -1)])
+    wt = np.array([1 / 3, 1 / 6, 1 / 6, 1 / 6, 1 / 6])
+    cs2 = 1 / 3
+    o = oracle.OracleGrid.from_workload(w, collision="regularized")
+    o.init_from_U(w.initial_U())
+    f = o.read_f()[:, :, 0]                                          # [k][i][y][x]
+    om = o.omega()
+    for _ in range(6):
+        o.step(1)
+        U = f.sum(1)
+        new = np.empty_like(f)
+        for y in range(w.ny):
+            for x in range(w.nx):
+                F, S = o.flux_source(U[:, y, x])
+                for k in range(4):
+                    feq = wt * (U[k, y, x] + c @ F[k, :2] / cs2)
+                    Pi = c.T @ (f[k, :, y, x] - feq)
+                    fneq_reg = wt * (c @ Pi) / cs2
+                    post = feq + (1.0 - om[k]) * fneq_reg + wt * S[k]
+                    for i in range(5):
+                        new[k, i, (y + c[i, 1]) % w.ny, (x + c[i, 0]) % w.nx] = post[i]
+        f = new
+        assert np.abs(o.read_f()[:, :, 0] - f).max() < 1e-14
+    assert np.allclose(o.omega_plus(), 1.0)
+    o.close()
+
+
 # ------------------------------------------------------------------------------------------------ GPU parity
 @pytest.mark.gpu
 @pytest.mark.parametrize("mk,kw,steps,prec", [(W.c1_advection, dict(n=37, ny=23), 51, "f64"), (W.c2_swe, dict(n=96, ny=50), 80, "f64"),
                                               (W.c3_euler, dict(n=128, ny=72), 300, "f32s"), (W.c4_nsf3d, dict(n=32, ny=24, nz=20), 200, "f32s"),
                                               (W.c5_mhd3d, dict(n=24, ny=10, nz=7), 60, "f64"), (W.pin_mhd2d, dict(n=40), 100, "f64")])
-def test_trt_gpu_matches_the_oracle(mk, kw, steps, prec):
+@pytest.mark.parametrize("collision", ["trt", "regularized"])
+def test_trt_gpu_matches_the_oracle(mk, kw, steps, prec, collision):
     import torch
     if not torch.cuda.is_available():
         pytest.fail("GPU tests need a CUDA device")
     import paper_2607_05668_b200 as P
     from parity_metric import gate
     w = mk(**kw)
-    g = P.Grid.from_workload(w, precision=prec, collision="trt", trt_magic=0.25, pattern="aa", stepping="persistent")   # resolve to pull2 / launch
+    g = P.Grid.from_workload(w, precision=prec, collision=collision, trt_magic=0.25, pattern="aa", stepping="persistent")   # resolve to pull2 / launch
     assert (g.pattern, g.kernel, g.stepping) == ("pull2", "node", "launch")
     g.init_from_U(w.initial_U())
     g.step(steps)
     U = g.read_U()
     opg = P.lbmk_grid_omega_plus(g.h, w.m_total)
     g.close()
-    Uo, fo, op, om = _run(w, steps, collision="trt", trt_magic=0.25)
+    Uo, fo, op, om = _run(w, steps, collision=collision, trt_magic=0.25)
     assert np.allclose(opg, op, rtol=1e-14) and np.abs(op - om).max() > 1e-3
-    gate(U, Uo, fo, prec, f"{w.name}[trt]", U_ref=w.U_ref, steps=steps)
+    gate(U, Uo, fo, prec, f"{w.name}[{collision}]", U_ref=w.U_ref, steps=steps)
     Ub = oracle.run(w, steps=steps)
     assert np.abs(Uo - Ub).max() > 1e-9 * np.abs(Ub).max()       # a different operator, not BGK again
