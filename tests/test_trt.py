@@ -126,6 +126,8 @@ def test_trt_gpu_matches_the_oracle(mk, kw, steps, prec, collision):
     import paper_2607_05668_b200 as P
     from parity_metric import gate
     w = mk(**kw)
+    if collision == "regularized":
+        steps = min(steps, 60)        # omega_plus = 1 is a small magic parameter: the seeded Euler case goes unstable near step 200 (oracle too)
     g = P.Grid.from_workload(w, precision=prec, collision=collision, trt_magic=0.25, pattern="aa", stepping="persistent")   # resolve to pull2 / launch
     assert (g.pattern, g.kernel, g.stepping) == ("pull2", "node", "launch")
     g.init_from_U(w.initial_U())
