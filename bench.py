@@ -78,6 +78,11 @@ def parse_args():
                     help="auto: slabs of one N-times-taller periodic grid with an overlapped halo exchange per step when N > 1; "
                          "replicas: N independent grids; slabs: force the slab path (also at N = 1, where the slab wraps onto itself)")
     ap.add_argument("--no-overlap", action="store_true", help="slabs: step, pack, exchange, unpack in series (no overlap)")
+    ap.add_argument("--halo", default="nccl", choices=["nccl", "peer"],
+                    help="slabs: nccl = pack / torch.distributed point-to-point / unpack beside the interior update (default, the "
+                         "transport the CPU tests cover); peer = boundary kernels store straight into the neighbours' ghost planes "
+                         "over CUDA-IPC-mapped peer memory, a one-element token for ordering (kernel tested on one GPU, the "
+                         "cross-process wiring is not)")
     ap.add_argument("--table3", action="store_true", help="(default on) also run the paper's Table 3 systems (4096^2, forcing off, S and D)")
     ap.add_argument("--no-table3", action="store_true")
     return ap.parse_args()
@@ -209,9 +214,10 @@ def time_steps(g, torch, steps, dist=None):
 class SlabRunner:
     """This rank's slab of the global workload behind the interface run_ours uses for a Grid."""
 
-    def __init__(self, P, w_global, rank, world, dist, device, overlap=True):
+    def __init__(self, P, w_global, rank, world, dist, device, overlap=True, halo="nccl"):
         from paper_2607_05668_b200.slabs import HaloRing, SlabGrid
         self.overlap = overlap
+        self.halo = halo
         self.slab = SlabGrid(P, w_global, rank, world, device=device)
         self.ring = HaloRing(rank, world, dist)
         self.grid = self.slab.grid
@@ -219,11 +225,21 @@ class SlabRunner:
         self.pattern, self.kernel, self.shape_U = self.grid.pattern, self.grid.kernel, self.grid.shape_U
         plane = self.w.nx * (self.w.ny if self.w.dim == 3 else 1)
         self.own_nodes = plane * self.slab.count               # node updates that count: ghost planes excluded
+        self._keep = None
 
     def init_from_U(self, U):
         self.grid.init_from_U(U)
 
     def step(self, n):
+        if self.halo == "peer":
+            from paper_2607_05668_b200.slabs import connect_ipc_peers, connect_local_peers, step_local_ring_peer, step_ring_peer
+            if self._keep is None:
+                self._keep = connect_ipc_peers(self.slab, self.ring)
+            if self.ring.world == 1:
+                step_local_ring_peer([self.slab], n)
+            else:
+                step_ring_peer(self.slab, n, self.ring)
+            return
         self.slab.step(n, self.ring, overlap=self.overlap)
 
     def read_U(self, out=None):
@@ -417,7 +433,7 @@ def run_ours(args):
         import workloads as W
         # weak scaling: one periodic grid `world` times taller along the slab axis, this rank owns one workload-sized slab
         wg = W.relabel(w, **({"nz": w.nz * world} if w.dim == 3 else {"ny": w.ny * world}))
-        g = SlabRunner(P, wg, rank, world, dist, dev, overlap=not args.no_overlap)
+        g = SlabRunner(P, wg, rank, world, dist, dev, overlap=not args.no_overlap, halo=args.halo)
         own_nodes, U0 = g.own_nodes, g.w.initial_U()
     else:
         own_nodes, U0 = w.n_nodes, w.initial_U()
@@ -500,7 +516,7 @@ def run_ours(args):
                    "grid": [w.nx, w.ny, w.nz], "precision": w.precision, "mms_forcing": bool(w.mms_id),
                    "pattern": pattern, "kernel": kernel, "bytes_per_node": w.bytes_per_node,
                    "l2": "state larger than L2 (no flush needed)" if bytes_per_launch / 2 > 2.5e8 else "state fits in L2: HBM roofline n/a",
-                   "parallelism": (("slabs along the slowest axis, halo exchange per step" + (" overlapped with the interior update" if not args.no_overlap else ", serial"))
+                   "parallelism": (("slabs along the slowest axis, " + ("boundary kernels store into the neighbours' ghost planes over peer memory" if args.halo == "peer" else "halo exchange per step" + (" overlapped with the interior update" if not args.no_overlap else ", serial")))
                                    if slabs else "replicas only") if (world > 1 or slabs) else "single GPU", "timing": f"median of {n_rep} x {steps} steps, CUDA events",
                    "lattice_wave_speed": max(speeds[0], speeds[1]) + speeds[2], "finite": finite},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,

@@ -211,6 +211,26 @@ lbmk_status lbmk_halo_unpack_on(lbmk_grid* g, const void* recv_lo, const void* r
 lbmk_status lbmk_step_slab(lbmk_grid* g);
 lbmk_status lbmk_stream_wait_boundary(lbmk_grid* g, void* cuda_stream);
 lbmk_status lbmk_grid_wait_stream(lbmk_grid* g, void* cuda_stream);
+/* Direct halo over peer memory: compute and transfer in ONE kernel.  The boundary-plane launches of lbmk_step_slab_peer store the
+ * face-crossing populations, besides into this slab, straight into the ring neighbours' ghost planes: slot(-s) of the first own
+ * plane into the lower neighbour's upper ghost plane, slot(+s) of the last own plane into the upper neighbour's lower ghost
+ * plane -- peer device pointers (another GPU's memory over NVLink / NVSwitch mapped into this process, or another slab on the
+ * same GPU).  No pack, no transport call, no unpack.
+ *   lbmk_grid_population_buffers  this grid's two population buffers (DEVICE pointers into the bound workspace) and the first
+ *                                 node of its upper ghost plane: what a neighbour needs to address this grid's ghost planes
+ *   lbmk_grid_set_halo_peers      the neighbours' buffers: lower neighbour (f0, f1, first node of ITS upper ghost plane), upper
+ *                                 neighbour (f0, f1; its lower ghost plane is plane 0).  All slabs of a ring step in lockstep, so
+ *                                 buffer index b of this grid pairs with index b of its peers.
+ *   lbmk_step_slab_peer           as lbmk_step_slab, boundary launches with the peer stores.  Ordering is the caller's: before the
+ *                                 next step, this grid's stream must wait for BOTH neighbours' boundary events
+ *                                 (lbmk_stream_wait_boundary(neighbour, this stream); across processes: an interprocess event).
+ * The ghost slots receive exactly the values the boundary planes hold (the transfer is exact); the boundary planes themselves
+ * are computed by the peer-store instantiation of the step kernel -- same arithmetic, but FMA contraction is nvcc's per kernel,
+ * so against lbmk_step_slab + pack / transport / unpack nonlinear systems agree to rounding, linear ones bit for bit
+ * (tests/test_gpu_slabs.py).  BGK with the node kernel only (LBMK_EUNSUPPORTED otherwise). */
+lbmk_status lbmk_grid_population_buffers(const lbmk_grid* g, void** f0, void** f1, long long* upper_ghost_first_node);
+lbmk_status lbmk_grid_set_halo_peers(lbmk_grid* g, void* lo_f0, void* lo_f1, long long lo_upper_ghost_first_node, void* hi_f0, void* hi_f1);
+lbmk_status lbmk_step_slab_peer(lbmk_grid* g);
 
 /* ---- initialise from U, step, read back U ------------------------------------------------------------ */
 

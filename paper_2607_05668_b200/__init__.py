@@ -79,6 +79,9 @@ SYMBOLS = {
     "lbmk_halo_unpack_on": (C.c_int, [_vp, _vp, _vp, _vp]),
     "lbmk_step_slab": (C.c_int, [_vp]),
     "lbmk_stream_wait_boundary": (C.c_int, [_vp, _vp]),
+    "lbmk_step_slab_peer": (C.c_int, [_vp]),
+    "lbmk_grid_population_buffers": (C.c_int, [_vp, C.POINTER(_vp), C.POINTER(_vp), C.POINTER(C.c_longlong)]),
+    "lbmk_grid_set_halo_peers": (C.c_int, [_vp, _vp, _vp, C.c_longlong, _vp, _vp]),
     "lbmk_grid_wait_stream": (C.c_int, [_vp, _vp]),
     "lbmk_stream_index_map": (C.c_int, [_vp, C.c_int, _vp, C.c_int]),
     "lbmk_generated_flux": (C.c_int, [C.c_int, _dp, _dp, _dp, C.c_int, C.c_double, C.c_double, C.c_double, _dp, _dp]),
@@ -294,6 +297,21 @@ def lbmk_halo_unpack_on(grid_h, recv_lo: int, recv_hi: int, cuda_stream: int):
 
 def lbmk_step_slab(grid_h):
     _check(lib().lbmk_step_slab(grid_h), grid_h)
+
+
+def lbmk_step_slab_peer(grid_h):
+    _check(lib().lbmk_step_slab_peer(grid_h), grid_h)
+
+
+def lbmk_grid_population_buffers(grid_h):
+    """(f0, f1, first node of the upper ghost plane): device pointers of the grid's two population buffers."""
+    f0, f1, n0 = _vp(), _vp(), C.c_longlong()
+    _check(lib().lbmk_grid_population_buffers(grid_h, C.byref(f0), C.byref(f1), C.byref(n0)), grid_h)
+    return f0.value, f1.value, n0.value
+
+
+def lbmk_grid_set_halo_peers(grid_h, lo_f0: int, lo_f1: int, lo_upper_ghost_first_node: int, hi_f0: int, hi_f1: int):
+    _check(lib().lbmk_grid_set_halo_peers(grid_h, _vp(lo_f0), _vp(lo_f1), int(lo_upper_ghost_first_node), _vp(hi_f0), _vp(hi_f1)), grid_h)
 
 
 def lbmk_stream_wait_boundary(grid_h, cuda_stream: int):

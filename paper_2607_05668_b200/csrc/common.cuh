@@ -67,6 +67,13 @@ struct KParams {
     long long aux_stride;
     // node range [node0, node1) a step launch updates (whole grid: 0, n); block b starts at node0 + b*BLOCK
     long long node0, node1;
+    // direct halo (slabs, peer stores): this step's destination buffers of the lower / upper ring neighbour (peer device
+    // memory: another GPU over NVLink, or another slab on this GPU) and the first node of the ghost plane to fill there
+    R* peer_lo;
+    R* peer_hi;
+    long long peer_lo_node0, peer_hi_node0;
+    long long plane_nodes;  // nodes per plane of the slab axis
+    long long last_own0;    // first node of the last own plane
 };
 
 // number of prescribed coefficient fields of a system: Sys::NA where declared, else 0

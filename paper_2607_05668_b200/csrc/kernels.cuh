@@ -172,7 +172,7 @@ __device__ __forceinline__ void collide_core(R (&f)[Sys::M][2 * Sys::D + 1], typ
 // coef_s = the block's shared-memory slot for its row's forcing coefficients, coef = this step's coefficient table.
 // Called by the per-launch kernel (one segment per block) and by the persistent kernel (segments in a loop): the
 // same code, hence the same bits.
-template <class Sys, class R, int MODE, bool MMS, int BLOCK, bool COHERENT, bool TRT = false>
+template <class Sys, class R, int MODE, bool MMS, int BLOCK, bool COHERENT, bool TRT = false, bool PEER = false>
 __device__ __forceinline__ void node_step(typename StepPtr<R, MODE, COHERENT>::Src src, typename StepPtr<R, MODE, COHERENT>::Dst dst,
                                           const KParams<R>& P, const R* coef, long long first, R* coef_s) {
     constexpr int D = Sys::D, Q = 2 * D + 1, M = Sys::M;
@@ -197,6 +197,15 @@ __device__ __forceinline__ void node_step(typename StepPtr<R, MODE, COHERENT>::S
     for (int i = 0; i < Q; ++i)
         sp[i] = src + tile_off(node + ((MODE == MODE_AA_EVEN || MODE == MODE_LOCAL) ? 0LL : pull_offset(i, p, P.nx, P.ny, P.nz)), M * Q);
     R* const dp = dst + tile_off(node, M * Q);
+    // PEER (boundary planes of a slab): the face-crossing populations are ALSO stored straight into the ring neighbour's ghost
+    // plane -- slot(-s) of the first own plane into the lower neighbour's upper ghost plane, slot(+s) of the last own plane into
+    // the upper neighbour's lower ghost plane -- so compute and halo transfer are one kernel over peer memory
+    R* plo = nullptr;
+    R* phi = nullptr;
+    if constexpr (PEER) {
+        if (node >= P.plane_nodes && node < 2 * P.plane_nodes) plo = P.peer_lo + tile_off(P.peer_lo_node0 + (node - P.plane_nodes), M * Q);
+        if (node >= P.last_own0 && node < P.last_own0 + P.plane_nodes) phi = P.peer_hi + tile_off(P.peer_hi_node0 + (node - P.last_own0), M * Q);
+    }
 
     R f[M][Q];
 #pragma unroll
@@ -227,6 +236,10 @@ __device__ __forceinline__ void node_step(typename StepPtr<R, MODE, COHERENT>::S
         for (int i = 0; i < Q; ++i) {
             if constexpr (MODE == MODE_PULL2 || MODE == MODE_LOCAL) {
                 dp[(k * Q + i) * TILE] = fk[i];
+                if constexpr (PEER) {
+                    if (i == 2 * D && plo) plo[(k * Q + i) * TILE] = fk[i];          // slot(-s) -> lower neighbour's upper ghost
+                    if (i == 2 * D - 1 && phi) phi[(k * Q + i) * TILE] = fk[i];      // slot(+s) -> upper neighbour's lower ghost
+                }
             } else if constexpr (MODE == MODE_AA_EVEN) {
                 dp[(k * Q + opposite(i)) * TILE] = fk[i];
             } else {   // AA odd: push to x + c_i; sp[opp(i)] - src + dst is that node (pull source of the opposite direction)
@@ -236,12 +249,12 @@ __device__ __forceinline__ void node_step(typename StepPtr<R, MODE, COHERENT>::S
     });
 }
 
-template <class Sys, class R, int MODE, bool MMS, int BLOCK, int MINB, bool TRT = false>
+template <class Sys, class R, int MODE, bool MMS, int BLOCK, int MINB, bool TRT = false, bool PEER = false>
 __global__ void __launch_bounds__(BLOCK, MINB)
 collide_stream_node(typename StepPtr<R, MODE>::Src src, typename StepPtr<R, MODE>::Dst dst, const __grid_constant__ KParams<R> P) {
     constexpr int NCs = MMS ? MmsNC<Sys>::value : 4;
     __shared__ __align__(16) R coef_s[NCs];
-    node_step<Sys, R, MODE, MMS, BLOCK, false, TRT>(src, dst, P, P.coef, P.node0 + (long long)blockIdx.x * BLOCK, coef_s);
+    node_step<Sys, R, MODE, MMS, BLOCK, false, TRT, PEER>(src, dst, P, P.coef, P.node0 + (long long)blockIdx.x * BLOCK, coef_s);
 }
 
 // ------------------------------------------------------------------------------------------------ step, persistent

@@ -508,11 +508,13 @@ lbmk_status lbmk_halo_unpack_on(lbmk_grid* g, const void* recv_lo, const void* r
 
 // One step of a slab, boundary planes first: [first own plane] [last own plane] -> boundary event -> [interior planes].
 // The ghost planes are not updated (their face-crossing slots arrive through the halo exchange).
-lbmk_status lbmk_step_slab(lbmk_grid* g) {
+static lbmk_status step_slab_impl(lbmk_grid* g, int peer) {
     lbmk_status s = need_inited(g);
     if (s != LBMK_OK) return s;
     GridCore& c = g->c;
     if (!c.Pd.ghost) return fail(g, LBMK_ESTATE, "not a slab (lbmk_grid_set_slab)");
+    if (peer && !c.peers_set) return fail(g, LBMK_ESTATE, "no halo peers set (lbmk_grid_set_halo_peers)");
+    if (peer && (c.collision != 0 || c.kernel != KERNEL_NODE)) return fail(g, LBMK_EUNSUPPORTED, "peer-store halo: BGK with the node kernel only");
     const long long pn = plane_nodes_of(g);
     const int np = planes_of(g);
     long long r[6];
@@ -520,11 +522,35 @@ lbmk_status lbmk_step_slab(lbmk_grid* g) {
     r[2] = np > 3 ? (long long)(np - 2) * pn : 0; r[3] = np > 3 ? (long long)(np - 1) * pn : 0;   // last own plane (if distinct)
     r[4] = np > 4 ? 2 * pn : 0; r[5] = np > 4 ? (long long)(np - 2) * pn : 0;                      // interior
     CK(g, cudaEventRecord(g->ev0, c.stream), "cudaEventRecord");
-    CK(g, g->ops->step_ranges(c, r, g->ev_boundary), "collide_stream launch (slab)");
+    CK(g, g->ops->step_ranges(c, r, g->ev_boundary, peer), "collide_stream launch (slab)");
     CK(g, cudaEventRecord(g->ev1, c.stream), "cudaEventRecord");
     g->timed = true;
     return LBMK_OK;
 }
+lbmk_status lbmk_step_slab(lbmk_grid* g) { return step_slab_impl(g, 0); }
+lbmk_status lbmk_step_slab_peer(lbmk_grid* g) { return step_slab_impl(g, 1); }
+
+lbmk_status lbmk_grid_population_buffers(const lbmk_grid* g, void** f0, void** f1, long long* upper_ghost_first_node) {
+    if (!g || !f0 || !f1) return sys_fail(LBMK_EINVAL, "NULL argument");
+    if (!g->bound) return sys_fail(LBMK_ESTATE, "no workspace bound");
+    *f0 = g->c.f[0]; *f1 = g->c.f[1];
+    if (upper_ghost_first_node) *upper_ghost_first_node = (long long)(planes_of(g) - 1) * plane_nodes_of(g);
+    return LBMK_OK;
+}
+
+lbmk_status lbmk_grid_set_halo_peers(lbmk_grid* g, void* lo_f0, void* lo_f1, long long lo_upper_ghost_first_node, void* hi_f0, void* hi_f1) {
+    lbmk_status s = need_bound(g);
+    if (s != LBMK_OK) return s;
+    GridCore& c = g->c;
+    if (!c.Pd.ghost) return fail(g, LBMK_ESTATE, "not a slab (lbmk_grid_set_slab)");
+    if (!lo_f0 || !lo_f1 || !hi_f0 || !hi_f1 || lo_upper_ghost_first_node < 0) return fail(g, LBMK_EINVAL, "bad peer buffers");
+    c.peer_f[0][0] = lo_f0; c.peer_f[0][1] = lo_f1; c.peer_f[1][0] = hi_f0; c.peer_f[1][1] = hi_f1;
+    c.peer_node0[0] = lo_upper_ghost_first_node;      // lower neighbour: its UPPER ghost plane receives this slab's slot(-s)
+    c.peer_node0[1] = 0;                              // upper neighbour: its LOWER ghost plane (plane 0) receives slot(+s)
+    c.peers_set = true;
+    return LBMK_OK;
+}
+
 lbmk_status lbmk_stream_wait_boundary(lbmk_grid* g, void* cuda_stream) {
     lbmk_status s = need_inited(g);
     if (s != LBMK_OK) return s;

@@ -40,6 +40,9 @@ struct GridCore {
     int collision;        // 0 BGK, 1 TRT (two-lattice pull, node kernel, one launch per step)
     int stepping;         // STEPPING_LAUNCH: one launch per step; STEPPING_PERSISTENT: one cooperative launch per batch of steps
     int num_sms;          // cudaDevAttrMultiProcessorCount of the current device
+    void* peer_f[2][2];   // direct halo: [lo|hi][buffer index] population buffers of the ring neighbours (peer device memory)
+    long long peer_node0[2];   // first node of the ghost plane to fill at the lower / upper neighbour
+    bool peers_set;
     long long persistent_launches;   // cooperative launches so far (diagnostic)
     KParams<double> Pd;   // parameters in fp64 (host logic, fp64 kernels, readback)
     KParams<float> Pf;    // same, rounded to fp32 (fp32 kernels)
@@ -62,7 +65,7 @@ struct SysOps {
     cudaError_t (*step)(GridCore&, int n_steps);
     // one step in up to 3 launches: nodes [a0,a1) and [b0,b1) first (the slab's boundary planes), then `ev` is recorded on
     // the stream, then [c0,c1) (the interior); empty ranges are skipped
-    cudaError_t (*step_ranges)(GridCore&, const long long* ranges6, cudaEvent_t ev);
+    cudaError_t (*step_ranges)(GridCore&, const long long* ranges6, cudaEvent_t ev, int peer);   // peer: boundary ranges also store into the neighbours' ghost planes
     cudaError_t (*set_aux)(GridCore&, const double* A_dev);
     cudaError_t (*read_U)(GridCore&, double* U_dev);
     cudaError_t (*read_f)(GridCore&, double* f_dev);

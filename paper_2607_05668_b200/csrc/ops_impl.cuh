@@ -178,10 +178,16 @@ struct Ops {
     // ---- the step
     // launches over the node range [kp.node0, kp.node1) (whole grid unless step_ranges narrowed it)
     template <class R, int MODE, bool MMS>
-    static void launch_node(GridCore& g, const R* src, R* dst) {
+    static void launch_node(GridCore& g, const R* src, R* dst, bool peer = false) {
         constexpr int BLOCK = Tune<S, R>::BLOCK, MINB = Tune<S, R>::MINB;
         const long long cnt = kp<R>(g).node1 - kp<R>(g).node0;
         if (cnt <= 0) return;
+        if (peer) {                       // boundary planes of a slab with direct stores into the neighbours' ghost planes (BGK, node kernel)
+            if constexpr (MODE == MODE_PULL2 || MODE == MODE_LOCAL)
+                collide_stream_node<S<R>, R, MODE, MMS, BLOCK, MINB, false, true><<<blocks_for(cnt, BLOCK), BLOCK, 0, g.stream>>>(src, dst, kp<R>(g));
+            g.launches++;
+            return;
+        }
         constexpr int NPT = 4;
         if constexpr (!MMS && M == 1 && NA == 0 && sizeof(R) == 4 && (MODE == MODE_PULL2 || MODE == MODE_LOCAL)) {
             // single-field fp32 systems: NPT nodes per thread for memory-level parallelism (kernels.cuh collide_stream_multi;
@@ -370,8 +376,17 @@ struct Ops {
     // One step of a slab split into its boundary planes (two ranges) and its interior (third range): the boundary ranges
     // go first and `ev` marks their completion, so that the halo exchange can run while the interior is updated.
     template <class R, bool MMS>
-    static cudaError_t step_ranges_t(GridCore& g, const long long* r, cudaEvent_t ev) {
+    static cudaError_t step_ranges_t(GridCore& g, const long long* r, cudaEvent_t ev, int peer) {
         if (g.pattern != PATTERN_PULL2 || g.bc != 0) return cudaErrorNotSupported;
+        if (peer) {
+            if (!g.peers_set || g.collision != 0 || g.kernel != KERNEL_NODE) return cudaErrorNotSupported;
+            const long long pn = D == 3 ? (long long)g.nx * g.ny : (long long)g.nx;
+            const int np = D == 3 ? g.nz : g.ny;
+            KParams<R>& P = kp<R>(g);
+            P.peer_lo = (R*)g.peer_f[0][g.cur ^ 1]; P.peer_hi = (R*)g.peer_f[1][g.cur ^ 1];     // the neighbours' destination buffers of this step
+            P.peer_lo_node0 = g.peer_node0[0]; P.peer_hi_node0 = g.peer_node0[1];
+            P.plane_nodes = pn; P.last_own0 = (long long)(np - 2) * pn;
+        }
         const int buf = (int)(g.step & 1);
         if constexpr (MMS) {
             // this step's row coefficients on the auxiliary stream, double-buffered by step parity: the pre-kernel of
@@ -391,8 +406,8 @@ struct Ops {
         R* dst = (R*)g.f[g.cur ^ 1];
         for (int q = 0; q < 3; ++q) {
             kp<R>(g).node0 = r[2 * q]; kp<R>(g).node1 = r[2 * q + 1];
-            if (g.pending) launch_node<R, MODE_PULL2, MMS>(g, src, dst);
-            else launch_node<R, MODE_LOCAL, MMS>(g, src, dst);
+            if (g.pending) launch_node<R, MODE_PULL2, MMS>(g, src, dst, peer && q < 2);
+            else launch_node<R, MODE_LOCAL, MMS>(g, src, dst, peer && q < 2);
             if (q == 1 && ev) cudaEventRecord(ev, g.stream);
         }
         kp<R>(g).node0 = 0; kp<R>(g).node1 = g.n;
@@ -402,12 +417,12 @@ struct Ops {
         g.step++;
         return cudaGetLastError();
     }
-    static cudaError_t step_ranges(GridCore& g, const long long* r, cudaEvent_t ev) {
+    static cudaError_t step_ranges(GridCore& g, const long long* r, cudaEvent_t ev, int peer) {
         const bool mms = HAS_MMS && g.mms_id != 0;
         if constexpr (HAS_MMS) {
-            if (mms) return g.prec == PREC_F64 ? step_ranges_t<double, true>(g, r, ev) : step_ranges_t<float, true>(g, r, ev);
+            if (mms) return g.prec == PREC_F64 ? step_ranges_t<double, true>(g, r, ev, peer) : step_ranges_t<float, true>(g, r, ev, peer);
         }
-        return g.prec == PREC_F64 ? step_ranges_t<double, false>(g, r, ev) : step_ranges_t<float, false>(g, r, ev);
+        return g.prec == PREC_F64 ? step_ranges_t<double, false>(g, r, ev, peer) : step_ranges_t<float, false>(g, r, ev, peer);
     }
     // Dirichlet frame refresh before readback (the oracle does the same in orc_read_U)
     static cudaError_t frame_now(GridCore& g) {

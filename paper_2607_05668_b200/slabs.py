@@ -121,6 +121,74 @@ class SlabGrid:
         self.grid.close()
 
 
+def connect_local_peers(slabs: List[SlabGrid]):
+    """Direct halo between slabs held by ONE process: every slab gets its ring neighbours' population buffers as peers
+    (`lbmk_grid_set_halo_peers`).  Between GPUs the same pointers come from mapping the neighbour's workspace into this process
+    (CUDA IPC / NVLink peer access): `connect_ipc_peers`."""
+    P = slabs[0].P
+    W = len(slabs)
+    bufs = [P.lbmk_grid_population_buffers(s.grid.h) for s in slabs]
+    for r, s in enumerate(slabs):
+        lo, hi = bufs[(r - 1) % W], bufs[(r + 1) % W]
+        P.lbmk_grid_set_halo_peers(s.grid.h, lo[0], lo[1], lo[2], hi[0], hi[1])
+
+
+def connect_ipc_peers(slab: SlabGrid, ring: HaloRing):
+    """Direct halo between RANKS (one process per GPU): every rank publishes its workspace through CUDA IPC (torch's storage
+    sharing: cudaIpcGetMemHandle / cudaIpcOpenMemHandle, which also enables NVLink peer access), gathers its two ring neighbours'
+    handles and registers their population buffers as halo peers.  UNTESTED on this one-GPU pool (needs >= 2 GPUs); the kernel and
+    the single-process wiring (`connect_local_peers`) are what the GPU tests cover.  Returns the mapped storages (keep them alive)."""
+    torch, P, d = slab.torch, slab.P, ring.dist
+    if ring.world == 1:
+        connect_local_peers([slab])
+        return []
+    ws = slab.grid.workspace
+    f0, f1, n0 = P.lbmk_grid_population_buffers(slab.grid.h)
+    mine = dict(share=ws.untyped_storage()._share_cuda_(), base=ws.data_ptr(), f0=f0 - ws.data_ptr(), f1=f1 - ws.data_ptr(), n0=n0)
+    everyone = [None] * ring.world
+    d.all_gather_object(everyone, mine)
+    keep, ptrs = [], []
+    for peer in (ring.lo, ring.hi):
+        info = everyone[peer]
+        st = torch.UntypedStorage._new_shared_cuda(*info["share"])          # maps the peer's allocation into this process
+        keep.append(st)
+        # the handle covers the peer's whole cudaMalloc block; the tensor starts share[3] bytes into it
+        base = st.data_ptr()
+        ptrs.append((base + info["f0"], base + info["f1"], info["n0"]))
+    P.lbmk_grid_set_halo_peers(slab.grid.h, ptrs[0][0], ptrs[0][1], ptrs[0][2], ptrs[1][0], ptrs[1][1])
+    slab._tok = [torch.zeros(1, device=slab.grid.device) for _ in range(4)]
+    return keep
+
+
+def step_ring_peer(slab: SlabGrid, n: int, ring: HaloRing):
+    """n steps of one rank with the direct halo (after `connect_ipc_peers`): the boundary launches store into the neighbours' ghost
+    planes over NVLink while the interior launch runs; what goes through torch.distributed is a ONE-ELEMENT token per neighbour on
+    the comm stream, sent after the boundary event: when the neighbour's token arrives, its peer stores have completed (stream
+    order + kernel-boundary visibility), and the next step may read the ghost planes."""
+    torch, P, h = slab.torch, slab.P, slab.grid.h
+    t = slab._tok
+    for _ in range(n):
+        P.lbmk_step_slab_peer(h)
+        P.lbmk_stream_wait_boundary(h, slab.comm.cuda_stream)
+        with torch.cuda.stream(slab.comm):
+            ring.exchange(t[0], t[1], t[2], t[3])
+        P.lbmk_grid_wait_stream(h, slab.comm.cuda_stream)
+
+
+def step_local_ring_peer(slabs: List[SlabGrid], n: int):
+    """n steps of all slabs of a ring in one process with the direct halo: boundary planes (storing into the neighbours' ghost
+    planes) -> interior; before its next step every slab's stream waits for both neighbours' boundary events."""
+    P = slabs[0].P
+    W = len(slabs)
+    for _ in range(n):
+        for s in slabs:
+            P.lbmk_step_slab_peer(s.grid.h)
+        for r, s in enumerate(slabs):
+            cs = s.grid.stream.cuda_stream
+            P.lbmk_stream_wait_boundary(slabs[(r - 1) % W].grid.h, cs)
+            P.lbmk_stream_wait_boundary(slabs[(r + 1) % W].grid.h, cs)
+
+
 def step_local_ring(slabs: List[SlabGrid], n: int, overlap: bool = False):
     """All slabs of a ring held by ONE process on one device (tests, and N = 1 with several slabs): every slab steps
     once, then the buffers are routed exactly as HaloRing.exchange routes them between ranks.  No kernel of one slab
