@@ -104,3 +104,31 @@ def test_halo_calls_are_refused_out_of_order(P):
     assert e.value.status == 5 and s.pattern == "pull2"
     s.close()
 
+
+
+def test_peer_halo_calls_are_refused_out_of_order(P):
+    w = W.c5_mhd3d(n=6)
+    ws = W.slab_workload(w, 0, 2)
+    s = P.Grid.from_workload(ws, slab=True)
+    s.init_from_U(ws.initial_U())
+    with pytest.raises(P.LbmkError) as e:                    # no peers registered
+        P.lbmk_step_slab_peer(s.h)
+    assert e.value.status == 5
+    f0, f1, n0 = P.lbmk_grid_population_buffers(s.h)
+    assert f0 and f1 and f1 != f0 and n0 == (ws.nz - 1) * ws.nx * ws.ny
+    with pytest.raises(P.LbmkError):
+        P.lbmk_grid_set_halo_peers(s.h, 0, f1, n0, f0, f1)   # NULL peer buffer
+    s.close()
+    t = P.Grid.from_workload(ws, slab=True, collision="trt")
+    t.init_from_U(ws.initial_U())
+    f0, f1, n0 = P.lbmk_grid_population_buffers(t.h)
+    P.lbmk_grid_set_halo_peers(t.h, f0, f1, n0, f0, f1)
+    with pytest.raises(P.LbmkError) as e:                    # the peer-store instantiation exists for BGK only
+        P.lbmk_step_slab_peer(t.h)
+    assert e.value.status == 6
+    t.close()
+    g = P.Grid.from_workload(w)
+    with pytest.raises(P.LbmkError) as e:                    # not a slab
+        P.lbmk_grid_set_halo_peers(g.h, f0, f1, 0, f0, f1)
+    assert e.value.status == 5
+    g.close()
