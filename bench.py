@@ -68,7 +68,7 @@ def parse_args():
                          "round 2, shifted fp32 (profiling targets, not headline workloads)")
     ap.add_argument("--pattern", default="auto", choices=["auto", "pull2", "aa"])
     ap.add_argument("--kernel", default="auto", choices=["auto", "node", "twopass"])
-    ap.add_argument("--n", type=int, default=None, help="override the grid edge (debug; the line then says so)")
+    ap.add_argument("--n", "--edge", dest="n", type=int, default=None, help="override the grid edge (debug; the line then says so; --edge under torchrun, whose parser claims --n)")
     ap.add_argument("--no-mms", action="store_true", help="without manufactured forcing (the paper's Table 3 kernels carry none)")
     ap.add_argument("--stepping", default="auto", choices=["auto", "launch", "persistent", "cluster"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -83,6 +83,10 @@ def parse_args():
                          "transport the CPU tests cover); peer = boundary kernels store straight into the neighbours' ghost planes "
                          "over CUDA-IPC-mapped peer memory, a one-element token for ordering (kernel tested on one GPU, the "
                          "cross-process wiring is not)")
+    ap.add_argument("--backend", default="auto", choices=["auto", "nccl", "gloo"],
+                    help="torch.distributed backend for N > 1 (auto: nccl); gloo + --one-device runs the N-rank path on ONE GPU (a dry "
+                         "run of the multi-rank code path on pools with one GPU per call: halo buffers staged through the host)")
+    ap.add_argument("--one-device", action="store_true", help="all ranks use cuda:0 (with --backend gloo)")
     ap.add_argument("--table3", action="store_true", help="(default on) also run the paper's Table 3 systems (4096^2, forcing off, S and D)")
     ap.add_argument("--no-table3", action="store_true")
     return ap.parse_args()
@@ -166,7 +170,7 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def dist_setup(n_gpus):
+def dist_setup(n_gpus, backend="auto", one_device=False):
     """(rank, world, dist or None).  One process per GPU under torchrun; N = 1 needs no process group."""
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -175,9 +179,10 @@ def dist_setup(n_gpus):
     import torch
     import torch.distributed as dist
     os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-    backend = "nccl" if torch.cuda.is_available() else "gloo"
-    if backend == "nccl":
-        torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    if backend == "auto":
+        backend = "nccl" if torch.cuda.is_available() else "gloo"
+    if torch.cuda.is_available():
+        torch.cuda.set_device(0 if one_device else int(os.environ.get("LOCAL_RANK", "0")))
     dist.init_process_group(backend=backend)
     return rank, world, dist
 
@@ -187,6 +192,8 @@ def aggregate(dist, local_ms, local_node_updates, device="cpu"):
     if dist is None:
         return local_ms, local_node_updates
     import torch
+    if dist.get_backend() == "gloo":
+        device = "cpu"
     t = torch.tensor([local_ms], dtype=torch.float64, device=device)
     u = torch.tensor([float(local_node_updates)], dtype=torch.float64, device=device)
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -418,8 +425,8 @@ def run_ours(args):
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device -- the collide-and-stream path has no CPU fallback "
                          "(use --impl reference for the CPU oracle)")
-    rank, world, dist = dist_setup(args.gpus)
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    rank, world, dist = dist_setup(args.gpus, args.backend, args.one_device)
+    local = 0 if args.one_device else int(os.environ.get("LOCAL_RANK", "0"))
     torch.cuda.set_device(local)
     import paper_2607_05668_b200 as P
     P.lib()
@@ -507,7 +514,7 @@ def run_ours(args):
     bytes_per_launch = w.n_nodes * w.bytes_per_node
     ms_launch = ms_local / steps
     achieved = bytes_per_launch / (ms_launch * 1e-3) / 1e9
-    traffic = NCU_TRAFFIC_BYTES.get(f"{args.config}:{pattern}:{kernel}")
+    traffic = NCU_TRAFFIC_BYTES.get(f"{args.config}:{pattern}:{kernel}") if args.n is None else None    # captured at the full size only
     line = {
         "metric": METRIC, "value": mlups, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warm,
         "ms_per_step": ms / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,

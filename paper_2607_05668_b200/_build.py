@@ -6,6 +6,8 @@ One translation unit per system (sys_*.cu) plus the API (lbmk_api.cu), compiled 
 from __future__ import annotations
 
 import concurrent.futures as cf
+import fcntl
+import hashlib
 import os
 import shutil
 import subprocess
@@ -35,11 +37,25 @@ def _deps():
     return out
 
 
+STAMP = LIB + ".stamp"     # content hash of the sources the library was built from; travels with the .so (git-ignored like it)
+
+
+def _source_hash() -> str:
+    h = hashlib.sha256(" ".join(NVCC_FLAGS).encode())
+    for p in sorted(_deps()):
+        h.update(os.path.basename(p).encode())
+        with open(p, "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()
+
+
 def needs_build() -> bool:
-    if not os.path.exists(LIB):
+    """By CONTENT, not by mtime: a snapshot copied to another box (gpurun) keeps no meaningful mtimes, and rebuilding there would
+    cost a minute per process and race between the ranks of a torchrun launch."""
+    if not os.path.exists(LIB) or not os.path.exists(STAMP):
         return True
-    t = os.path.getmtime(LIB)
-    return any(os.path.getmtime(p) > t for p in _deps())
+    with open(STAMP) as fh:
+        return fh.read().strip() != _source_hash()
 
 
 def _compile(unit: str) -> str:
@@ -58,13 +74,20 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not needs_build():
         return LIB
     os.makedirs(OBJ, exist_ok=True)
-    with cf.ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as ex:
-        objs = list(ex.map(_compile, UNITS))
-    cmd = [_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB + ".tmp"] + objs
-    if verbose:
-        print(" ".join(cmd))
-    subprocess.run(cmd, check=True)
-    os.replace(LIB + ".tmp", LIB)
+    with open(os.path.join(OBJ, ".lock"), "w") as lock:          # one builder at a time (ranks of one launch, parallel test workers)
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        if not force and not needs_build():                       # another process built it while this one waited
+            return LIB
+        with cf.ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as ex:
+            objs = list(ex.map(_compile, UNITS))
+        tmp = f"{LIB}.{os.getpid()}.tmp"
+        cmd = [_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", tmp] + objs
+        if verbose:
+            print(" ".join(cmd))
+        subprocess.run(cmd, check=True)
+        os.replace(tmp, LIB)
+        with open(STAMP, "w") as fh:
+            fh.write(_source_hash() + "\n")
     return LIB
 
 

@@ -43,6 +43,15 @@ class HaloRing:
             recv_hi.copy_(send_lo)
             return
         d = self.dist
+        if send_lo.is_cuda and d.get_backend() == "gloo":
+            # gloo moves host memory only: stage through the host (the two-ranks-on-one-GPU test; NCCL takes the device buffers)
+            h = [send_lo.cpu(), send_hi.cpu(), recv_hi.cpu(), recv_lo.cpu()]
+            ops = [d.P2POp(d.isend, h[0], self.lo), d.P2POp(d.isend, h[1], self.hi),
+                   d.P2POp(d.irecv, h[2], self.hi), d.P2POp(d.irecv, h[3], self.lo)]
+            for req in d.batch_isend_irecv(ops):
+                req.wait()
+            recv_hi.copy_(h[2]); recv_lo.copy_(h[3])
+            return
         ops = [d.P2POp(d.isend, send_lo, self.lo), d.P2POp(d.isend, send_hi, self.hi),
                d.P2POp(d.irecv, recv_hi, self.hi), d.P2POp(d.irecv, recv_lo, self.lo)]
         for req in d.batch_isend_irecv(ops):
@@ -136,8 +145,9 @@ def connect_local_peers(slabs: List[SlabGrid]):
 def connect_ipc_peers(slab: SlabGrid, ring: HaloRing):
     """Direct halo between RANKS (one process per GPU): every rank publishes its workspace through CUDA IPC (torch's storage
     sharing: cudaIpcGetMemHandle / cudaIpcOpenMemHandle, which also enables NVLink peer access), gathers its two ring neighbours'
-    handles and registers their population buffers as halo peers.  UNTESTED on this one-GPU pool (needs >= 2 GPUs); the kernel and
-    the single-process wiring (`connect_local_peers`) are what the GPU tests cover.  Returns the mapped storages (keep them alive)."""
+    handles and registers their population buffers as halo peers.  Tested between two PROCESSES sharing one GPU
+    (tests/test_gpu_slabs.py: same-device IPC mapping, gloo for the token); across GPUs (NVLink peer mapping, NCCL token) it is the
+    same calls but has not run on this one-GPU pool.  Returns the mapped storages (keep them alive)."""
     torch, P, d = slab.torch, slab.P, ring.dist
     if ring.world == 1:
         connect_local_peers([slab])

@@ -132,3 +132,69 @@ def test_peer_halo_calls_are_refused_out_of_order(P):
         P.lbmk_grid_set_halo_peers(g.h, f0, f1, 0, f0, f1)
     assert e.value.status == 5
     g.close()
+
+
+TWO_RANK_WORKER = r"""
+import json, os, sys
+sys.path.insert(0, {root!r})
+import numpy as np, torch, torch.distributed as dist
+import paper_2607_05668_b200 as P, workloads as W
+from paper_2607_05668_b200.slabs import HaloRing, SlabGrid, connect_ipc_peers, step_ring_peer
+dist.init_process_group(backend="gloo")               # NCCL refuses two ranks on one GPU; gloo moves the same CUDA buffers
+rank, world = dist.get_rank(), dist.get_world_size()
+w = W.c5_mhd3d(n=10, ny=8)
+out = {{}}
+for overlap in (True, False):
+    s = SlabGrid(P, w, rank, world, device="cuda:0")
+    s.init()
+    s.step(6, HaloRing(rank, world, dist), overlap=overlap)
+    out[str(overlap)] = s.read_U_interior().tolist()
+    s.close()
+# direct halo: each rank maps the other's workspace through CUDA IPC and its boundary kernels store into the other's ghost planes
+s = SlabGrid(P, w, rank, world, device="cuda:0")
+s.init()
+ring = HaloRing(rank, world, dist)
+keep = connect_ipc_peers(s, ring)
+step_ring_peer(s, 6, ring)
+out["peer"] = s.read_U_interior().tolist()
+dist.barrier()
+del keep
+s.close()
+dist.barrier()
+print(json.dumps(dict(rank=rank, start=s.start, count=s.count, out=out)))
+dist.destroy_process_group()
+"""
+
+
+def test_two_ranks_on_one_gpu_over_gloo_reproduce_the_single_grid(P):
+    """The multi-process path end to end with real kernels: two RANKS (processes), one slab each, both on this one GPU, the halo
+    buffers moved by torch.distributed point-to-point (gloo here, because NCCL needs one GPU per rank; the calls are the ones the
+    NCCL run makes).  No kernel of one rank waits on a kernel of the other: ordering is host-side.  Overlapped and serial, and
+    the direct halo: the ranks map each other's workspace through CUDA IPC (`connect_ipc_peers`) and the boundary kernels store
+    into the other PROCESS's ghost planes, a one-element token per neighbour for ordering (`step_ring_peer`)."""
+    import json, os, socket, subprocess, sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    w = W.c5_mhd3d(n=10, ny=8)
+    g = P.Grid.from_workload(w, pattern="pull2")
+    g.init_from_U(w.initial_U()); g.step(6)
+    U = g.read_U(); g.close()
+    sk = socket.socket(); sk.bind(("127.0.0.1", 0)); port = sk.getsockname()[1]; sk.close()
+    procs = []
+    for r in range(2):
+        env = dict(os.environ, RANK=str(r), LOCAL_RANK=str(r), WORLD_SIZE="2", MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+        procs.append(subprocess.Popen([sys.executable, "-c", TWO_RANK_WORKER.format(root=root)], env=env,
+                                      stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True))
+    for p in procs:
+        try:
+            o, e = p.communicate(timeout=240)
+        except subprocess.TimeoutExpired:
+            for q in procs:
+                q.kill()
+            raise
+        assert p.returncode == 0, e[-3000:]
+        d = json.loads(o.strip().splitlines()[-1])
+        for overlap in ("True", "False"):
+            own = np.array(d["out"][overlap])
+            assert np.array_equal(own, U[:, d["start"]:d["start"] + d["count"]]), (d["rank"], overlap)
+        own = np.array(d["out"]["peer"])              # CUDA-IPC peer stores between the two processes: equal to rounding (fp32 here)
+        assert np.abs(own - U[:, d["start"]:d["start"] + d["count"]]).max() <= 1e-6 * np.abs(U).max(), d["rank"]
