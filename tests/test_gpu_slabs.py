@@ -198,3 +198,23 @@ def test_two_ranks_on_one_gpu_over_gloo_reproduce_the_single_grid(P):
             assert np.array_equal(own, U[:, d["start"]:d["start"] + d["count"]]), (d["rank"], overlap)
         own = np.array(d["out"]["peer"])              # CUDA-IPC peer stores between the two processes: equal to rounding (fp32 here)
         assert np.abs(own - U[:, d["start"]:d["start"] + d["count"]]).max() <= 1e-6 * np.abs(U).max(), d["rank"]
+
+
+@pytest.mark.parametrize("halo", ["nccl", "peer"])
+def test_bench_multi_rank_path_dry_run_on_one_gpu(P, halo):
+    """`bench.py --gpus 2` as the driver launches it (torch.distributed.run, one process per rank), but with both ranks on this one
+    GPU and gloo as transport: the slab default for N > 1, max-over-ranks timing, sum-over-ranks node updates, rank 0 prints ONE
+    JSON line.  A dry run of the code path, not a measurement."""
+    import json, os, socket, subprocess, sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    sk = socket.socket(); sk.bind(("127.0.0.1", 0)); port = sk.getsockname()[1]; sk.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.join(root, "bench.py"), "--gpus", "2", "--steps", "6", "--warmup", "3",
+           "--backend", "gloo", "--one-device", "--edge", "32", "--halo", halo, "--no-cpu-baseline"]
+    r = subprocess.run(cmd, capture_output=True, text=True, timeout=400, cwd=root)
+    assert r.returncode == 0, r.stderr[-3000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["steps"] == 6 and d["scaling"] == "weak" and d["config"]["finite"] is True
+    assert d["config"]["parallelism"].startswith("slabs") and d["value"] > 0 and d["gpu_launches"] >= 6
