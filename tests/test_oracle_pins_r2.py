@@ -15,6 +15,9 @@ oracle formula: each compares the oracle's TIME STEPPING (or its flux through a 
        used by the check bounds the spectral radius of the full augmented Jacobian.
   P21  configs[2] (Euler free evolution): the same workload recipe at amplitude 1e-6 against the closed-form LINEAR acoustics of its
        own seeded fields (standing pressure waves, steady entropy part), second-order approach under refinement.
+  P22  dynamics of the systems added in round 2: chain-rule viscous shear decay nu k^2 and thermal-mode decay kappa k^2 of NSF 2D (the
+       paper's running example) and MHD 2D; MHD 2D resistive decay eta k^2; HCNSF drag towards the solid velocity (exact
+       discrete closed form) and porosity-scaled viscous decay alpha nu k^2 (the halves of the symmetric tracker).
   P11  on the configs themselves: c2 at N = 64, 128, 256 and the fp64 build of c4 at N = 16, 32, 64, to a fixed time:
        L2 slope in the paper's band 1.7-2.5.
 """
@@ -312,3 +315,141 @@ def test_p21_c3_free_evolution_matches_linear_acoustics_at_small_amplitude():
         dev = max(np.abs(p - p0 - dp_t).max(), np.abs(U[0, 0] - rho0 - drho_t).max(), np.abs(U[1, 0] - mx_t).max()) / amp
         devs.append(dev)
     assert devs[1] < 0.02 and devs[1] < 0.45 * devs[0], devs      # second-order approach to the linear solution
+
+
+# ------------------------------------------------------------------------------------------------ P22: dynamics of the round-2 systems
+def _decay_rate(w, U0, steps, comp, shape_fn, x):
+    g = oracle.OracleGrid.from_workload(w)
+    if g.n_aux:
+        g.set_aux(w.aux_fields(0.0))
+    g.init_from_U(U0)
+    s1 = steps // 4
+    g.step(s1)
+    a1 = 2.0 * np.abs((shape_fn(g.read_U()) * np.sin(K2PI * x)).mean())
+    g.step(steps - s1)
+    a2 = 2.0 * np.abs((shape_fn(g.read_U()) * np.sin(K2PI * x)).mean())
+    g.close()
+    return math.log(a1 / a2) / ((steps - s1) * w.dt)
+
+
+def _chain_rule_system_state(system, n, dx, gamma, uy=None, rho=None, By=None):
+    """nsf2d / mhd2d state on an (n, 2) grid varying in x: conserved fields + trackers = dx * analytic x-gradients of them."""
+    x = np.arange(n) * dx
+    one = np.ones((2, 1))
+    rho = np.ones(n) if rho is None else rho
+    uy = np.zeros(n) if uy is None else uy
+    By = np.zeros(n) if By is None else By
+    p0 = 1.0 / gamma
+    E = p0 / (gamma - 1.0) + 0.5 * rho * uy ** 2 + 0.5 * By ** 2
+    d = lambda a: np.real(np.fft.ifft(1j * 2 * np.pi * np.fft.fftfreq(n, d=dx) * np.fft.fft(a)))   # spectral d/dx (periodic, exact for these modes)
+    cons = [rho, 0 * x, rho * uy, E] + ([0 * x, By] if system == "mhd2d" else [])
+    M = (4 + 8) if system == "nsf2d" else (6 + 12)
+    U = np.zeros((M, 1, 2, n))
+    for k, c in enumerate(cons):
+        U[k, 0] = c * one
+        U[len(cons) + 2 * k, 0] = dx * d(c) * one              # G_{V,0} = dx d_x V ; G_{V,1} = 0
+    return U, x
+
+
+@pytest.mark.parametrize("system", ["nsf2d", "mhd2d"])
+def test_p22_chain_rule_viscous_shear_decay(system):
+    """u_y = A sin kx decays at nu k^2 (rate with mu minus rate without): the viscous stress reconstructed by the CHAIN RULE from
+    the conserved-field trackers -- sign, mu_L scaling, the 1/rho factors."""
+    n, A, gamma, mu = 128, 1e-3, 1.4, 5e-3
+    mk = W.pin_nsf2d if system == "nsf2d" else W.pin_mhd2d
+    rates = []
+    for m_ in (0.0, mu):
+        w = W.relabel(mk(n), ny=2, mms_id=0, params=[gamma, m_, 0.0] + ([0.0] if system == "mhd2d" else []),
+                      lam=8.0, tau_R=20.0, g_tau=3.0, U_ref=[0.0] * (12 if system == "nsf2d" else 18))
+        U0, x = _chain_rule_system_state(system, n, w.dx, gamma, uy=A * np.sin(K2PI * np.arange(n) * w.dx))
+        rates.append(_decay_rate(w, U0, 1600, 2, lambda U: U[2, 0, 0] / U[0, 0, 0], x))
+    assert rates[1] - rates[0] == pytest.approx(mu * K2PI ** 2, rel=0.05)
+
+
+@pytest.mark.parametrize("system", ["nsf2d", "mhd2d"])
+def test_p22_chain_rule_thermal_mode_decay(system):
+    """Isobaric entropy mode decays at kappa k^2, kappa = K (gamma-1)/(gamma rho0): the heat flux -K grad T with grad T reconstructed by
+    the chain rule from G_rho, G_m, G_E (and G_B)."""
+    n, eps, gamma, K = 128, 1e-3, 1.4, 2e-2
+    mk = W.pin_nsf2d if system == "nsf2d" else W.pin_mhd2d
+    rates = []
+    for K_ in (0.0, K):
+        w = W.relabel(mk(n), ny=2, mms_id=0, params=[gamma, 0.0, K_] + ([0.0] if system == "mhd2d" else []),
+                      lam=8.0, tau_R=20.0, g_tau=3.0, U_ref=[0.0] * (12 if system == "nsf2d" else 18))
+        xs = np.arange(n) * w.dx
+        U0, x = _chain_rule_system_state(system, n, w.dx, gamma, rho=1.0 - eps * np.sin(K2PI * xs))
+
+        def entropy(U):
+            rho = U[0, 0, 0]
+            p = (gamma - 1.0) * (U[3, 0, 0] - 0.5 * (U[1, 0, 0] ** 2 + U[2, 0, 0] ** 2) / rho)
+            return np.log(gamma * p) - gamma * np.log(rho)
+        rates.append(_decay_rate(w, U0, 1600, 0, entropy, x))
+    assert rates[1] - rates[0] == pytest.approx(K * (gamma - 1.0) / gamma * K2PI ** 2, rel=0.05)
+
+
+def test_p22_mhd2d_resistive_decay():
+    """B_y = A sin kx decays at eta k^2: the resistive flux -eta G_B of the induction equation of the 2D system (eq 3.25)."""
+    n, A, gamma, eta = 128, 1e-3, 1.4, 5e-3
+    rates = []
+    for e_ in (0.0, eta):
+        w = W.relabel(W.pin_mhd2d(n), ny=2, mms_id=0, params=[gamma, 0.0, 0.0, e_], lam=8.0, tau_R=20.0, g_tau=3.0, U_ref=[0.0] * 18)
+        U0, x = _chain_rule_system_state("mhd2d", n, w.dx, gamma, By=A * np.sin(K2PI * np.arange(n) * w.dx))
+        rates.append(_decay_rate(w, U0, 1600, 5, lambda U: U[5, 0, 0], x))
+    assert rates[1] - rates[0] == pytest.approx(eta * K2PI ** 2, rel=0.05)
+
+
+def test_p22_hcnsf_drag_relaxes_towards_the_solid_velocity_exactly():
+    """Uniform state, uniform prescribed fields: the only active term is the drag (1-alpha)/eta (rho u_s - rho u) (eq 3.27).
+    The scheme adds dt S to the zeroth moment each step, so m_n = rho u_s + (m_0 - rho u_s)(1 - dt (1-alpha)/eta)^n EXACTLY; the
+    energy follows dE = sum of dt S_m . u.  alpha = 1 switches the drag off."""
+    w = W.hcnsf3d(4, precision="f64")
+    gamma, mu, kap, eta = w.params
+    for alpha in (1.0, 0.35):
+        us = np.array([0.2, -0.1, 0.05])
+        A = np.zeros((4, 4, 4, 4)); A[0] = alpha
+        for a in range(3):
+            A[1 + a] = us[a]
+        U0 = np.zeros((14, 4, 4, 4))
+        rho, u0 = 1.1, np.array([0.3, 0.1, -0.2])
+        U0[0] = rho
+        for a in range(3):
+            U0[1 + a] = rho * u0[a]
+        U0[4] = 1.0 / (gamma - 1.0) + 0.5 * rho * (u0 ** 2).sum()
+        g = oracle.OracleGrid.from_workload(w)
+        g.set_aux(A); g.init_from_U(U0); g.step(25)
+        U = g.read_U(); g.close()
+        q = 1.0 - w.dt * (1.0 - alpha) / eta
+        want_m = rho * us + (rho * u0 - rho * us) * q ** 25
+        assert np.allclose(U[1:4, 0, 0, 0], want_m, rtol=1e-12, atol=1e-15)
+        assert np.allclose(U[0], rho, rtol=1e-14) and np.abs(U[5:]).max() < 1e-15        # no density change, trackers stay zero
+        E, m = U0[4, 0, 0, 0], rho * u0.copy()
+        for _ in range(25):                                                               # dE = dt S_m . u, step by step
+            S = w.dt * (1.0 - alpha) / eta * (rho * us - m)
+            E += (S * m / rho).sum(); m = m + S
+        assert U[4, 0, 0, 0] == pytest.approx(E, rel=1e-13)
+
+
+def test_p22_hcnsf_porosity_scales_the_viscous_decay():
+    """u_y = A sin kx with uniform alpha and no drag (u_s = u would need eta -> inf: the drag is removed by alpha-independent choice
+    eta = 1e30): decay rate(alpha, mu) - rate(alpha, 0) = alpha nu k^2 -- the factor alpha on tau, and the halves of the symmetric
+    tracker sym(I (x) u)/tau_grad (a missing 1/2 would give half / twice the rate)."""
+    n, A, gamma, mu = 128, 1e-3, 1.4, 5e-3
+    for alpha in (1.0, 0.5):
+        rates = []
+        for m_ in (0.0, mu):
+            w = W.relabel(W.hcnsf3d(n, ny=2, nz=2, precision="f64"), params=[gamma, m_, 0.0, 1e30], lam=8.0, tau_R=20.0, g_tau=3.0, U_ref=[0.0] * 14)
+            x = np.arange(n) * w.dx
+            one = np.ones((2, 2, 1))
+            U0 = np.zeros((14, 2, 2, n))
+            uy = A * np.sin(K2PI * x)
+            U0[0] = 1.0; U0[2] = uy * one
+            U0[4] = ((1.0 / gamma) / (gamma - 1.0) + 0.5 * uy ** 2) * one
+            U0[8] = w.dx * 0.5 * A * K2PI * np.cos(K2PI * x) * one            # D_xy = (d_x u_y + d_y u_x)/2
+            Aux = np.zeros((4, 2, 2, n)); Aux[0] = alpha
+            g = oracle.OracleGrid.from_workload(w)
+            g.set_aux(Aux); g.init_from_U(U0)
+            g.step(400); a1 = 2.0 * np.abs((g.read_U()[2, 0, 0] * np.sin(K2PI * x)).mean())
+            g.step(1200); a2 = 2.0 * np.abs((g.read_U()[2, 0, 0] * np.sin(K2PI * x)).mean())
+            g.close()
+            rates.append(math.log(a1 / a2) / (1200 * w.dt))
+        assert rates[1] - rates[0] == pytest.approx(alpha * mu * K2PI ** 2, rel=0.05)
