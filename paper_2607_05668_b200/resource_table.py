@@ -19,20 +19,20 @@ import sys
 from . import _build
 
 HEADLINE = [  # (label, unit, regex on the demangled-ish mangled name)
-    ("c4 NSF3D f32, pull, forcing on", "sys_nsf3d", r"collide_stream_nodeINS_8SysNsf3DIfEEfLi0ELb1ELi64ELi6ELb0E"),
-    ("c4 NSF3D f32, pull, forcing off", "sys_nsf3d", r"collide_stream_nodeINS_8SysNsf3DIfEEfLi0ELb0ELi64ELi6ELb0E"),
-    ("c5 MHD3D f32, pull", "sys_mhd3d", r"collide_stream_nodeINS_8SysMhd3DIfEEfLi0ELb0ELi64ELi4ELb0E"),
-    ("c3 Euler2D f32, pull", "sys_euler2d", r"collide_stream_nodeINS_10SysEuler2DIfEEfLi0ELb0ELi128ELi1ELb0E"),
-    ("HCNSF f32, pull", "sys_hcnsf3d", r"collide_stream_nodeINS_10SysHcnsf3DIfEEfLi0ELb0ELi64ELi6ELb0E"),
-    ("HCNSF f64, pull", "sys_hcnsf3d", r"collide_stream_nodeINS_10SysHcnsf3DIdEEdLi0ELb0ELi128ELi1ELb0E"),
-    ("MHD2D f32, pull, forcing off", "sys_mhd2d", r"collide_stream_nodeINS_8SysMhd2DIfEEfLi0ELb0ELi128ELi3ELb0E"),
-    ("MHD2D f32, pull, forcing on", "sys_mhd2d", r"collide_stream_nodeINS_8SysMhd2DIfEEfLi0ELb1ELi128ELi3ELb0E"),
-    ("MHD2D f64, pull, forcing off", "sys_mhd2d", r"collide_stream_nodeINS_8SysMhd2DIdEEdLi0ELb0ELi128ELi1ELb0E"),
-    ("c2 SWE f64, pull, forcing on (per launch)", "sys_swe2d", r"collide_stream_nodeINS_8SysSwe2DIdEEdLi0ELb1ELi128ELi1ELb0E"),
+    ("c4 NSF3D f32, pull, forcing on", "sys_nsf3d", r"collide_stream_nodeINS_8SysNsf3DIfEEfLi0ELb1ELi64ELi6ELb0ELb0E"),
+    ("c4 NSF3D f32, pull, forcing off", "sys_nsf3d", r"collide_stream_nodeINS_8SysNsf3DIfEEfLi0ELb0ELi64ELi6ELb0ELb0E"),
+    ("c5 MHD3D f32, pull", "sys_mhd3d", r"collide_stream_nodeINS_8SysMhd3DIfEEfLi0ELb0ELi64ELi4ELb0ELb0E"),
+    ("c3 Euler2D f32, pull", "sys_euler2d", r"collide_stream_nodeINS_10SysEuler2DIfEEfLi0ELb0ELi128ELi1ELb0ELb0E"),
+    ("HCNSF f32, pull", "sys_hcnsf3d", r"collide_stream_nodeINS_10SysHcnsf3DIfEEfLi0ELb0ELi64ELi6ELb0ELb0E"),
+    ("HCNSF f64, pull", "sys_hcnsf3d", r"collide_stream_nodeINS_10SysHcnsf3DIdEEdLi0ELb0ELi128ELi1ELb0ELb0E"),
+    ("MHD2D f32, pull, forcing off", "sys_mhd2d", r"collide_stream_nodeINS_8SysMhd2DIfEEfLi0ELb0ELi128ELi3ELb0ELb0E"),
+    ("MHD2D f32, pull, forcing on", "sys_mhd2d", r"collide_stream_nodeINS_8SysMhd2DIfEEfLi0ELb1ELi128ELi3ELb0ELb0E"),
+    ("MHD2D f64, pull, forcing off", "sys_mhd2d", r"collide_stream_nodeINS_8SysMhd2DIdEEdLi0ELb0ELi128ELi1ELb0ELb0E"),
+    ("c2 SWE f64, pull, forcing on (per launch)", "sys_swe2d", r"collide_stream_nodeINS_8SysSwe2DIdEEdLi0ELb1ELi128ELi1ELb0ELb0E"),
     ("c2 SWE f64, persistent, forcing on", "sys_swe2d", r"collide_stream_persistentINS_8SysSwe2DIdEEdLb1E"),
     ("c1 advection f64, cluster-resident", "sys_advection2d", r"collide_stream_clusterINS_14SysAdvection2DIdEEdEE"),
     ("c1 advection f64, persistent", "sys_advection2d", r"collide_stream_persistentINS_14SysAdvection2DIdEEdLb0E"),
-    ("c4 NSF3D f32, TRT, forcing on", "sys_nsf3d", r"collide_stream_nodeINS_8SysNsf3DIfEEfLi0ELb1ELi64ELi6ELb1E"),
+    ("c4 NSF3D f32, TRT, forcing on", "sys_nsf3d", r"collide_stream_nodeINS_8SysNsf3DIfEEfLi0ELb1ELi64ELi6ELb1ELb0E"),
 ]
 
 
