@@ -10,6 +10,17 @@
 // A physical diffusivity D multiplying a tracked gradient enters as D_L = D dt/dx^2.
 // The function is templated on the scalar type so the SAME flux serves the time stepping (double)
 // and the manufactured residual of eq (4.1) (jets, see jets.hpp).
+//
+// What pins each system (tests/, -m "not gpu") -- and what does not:
+//   pinned to the paper's PRINTED Table 2 errors (5 digits, N = 512): Burgers, Euler, SWE over a bed (swe2d_bathy), ultrarelativistic
+//     fluid, Maxwell TM, elasticity, ADR, Allen-Cahn;
+//   pinned by closed-form dynamics / exact solutions: advection (P4 exact Fourier), NSF3D (P16-P18), MHD3D (P15, P19), NSF2D and
+//     MHD2D (P22 chain-rule viscous / thermal / resistive decay), HCNSF (P22 exact drag, porosity-scaled viscosity), Euler's
+//     config-3 fields (P21 linear acoustics); all systems: P1, P3, P13 (brute force from the paper's listings), P20 (wave speeds);
+//   PARITY UNPINNED to Table 2 digits: INSE2D (reading A22: momentum L2 to 3 digits only), NSF2D (A24: 1.8-2.1x the printed errors),
+//     MHD2D (A27: within 8 %, printed EOCs reproduced), HCNSF (A26: no manufactured forcing -- exact fields cut off in the source);
+//   PARITY UNPINNED beyond the pins above: the free NONLINEAR evolution of config 5 (MHD3D) and of config 3 at its full amplitude
+//     (no closed form); the TRT / regularised collision operators have textbook pins only (the paper runs BGK).
 #pragma once
 #include <cmath>
 #include "jets.hpp"
