@@ -281,11 +281,12 @@ lbmk_status lbmk_error_norms(lbmk_grid* g, double* out);
  * [nz][ny][nx]; bit-exact against the oracle's table. */
 lbmk_status lbmk_stream_index_map(lbmk_grid* g, int dir, long long* src_index_out, int on_device);
 /* Build-time generator check (Alg 2.1).  gen/cascade.py derives the augmented
- * system (trackers, chain rule, lattice scaling) of EULER2D, SWE2D_BATHY, ADR2D, ALLENCAHN2D, INSE2D, NSF2D, MHD2D and NSF3D from
- * the declared conservation laws and emits csrc/cascade_generated.cuh.
+ * system (trackers, chain rule, lattice scaling) of every system of this library from the declared conservation laws and emits
+ * csrc/cascade_generated.cuh -- conserved-field trackers + chain rule (ADR, Allen-Cahn, INSE, NSF 2D, MHD 2D), derived-parent
+ * trackers (NSF 3D), combination trackers (HCNSF's symmetric gradient, MHD 3D's curl), and the tracker-free systems.
  *   lbmk_generated_flux   evaluates the emitted code on the HOST (no GPU needed) at one state: U [m_total], A [n_aux] or NULL,
  *                         params as for lbmk_system_create; F_out [m_total][3] lattice flux (dt/dx) Phi, S_out [m_total] lattice
- *                         source dt S, trackers in lattice units.  LBMK_EUNSUPPORTED for the other systems.
+ *                         source dt S, trackers in lattice units.
  *   lbmk_flux_selfcheck   on the device, for every node of the grid's current state: the hand-written delta-form flux/source the
  *                         step kernels use against the emitted plain form, in fp64; *max_rel_diff = the largest difference
  *                         relative to the node's largest flux/source entry (rounding level when the two derivations agree). */

@@ -834,6 +834,14 @@ lbmk_status lbmk_generated_flux(lbmk_system_id id, const double* U, const double
         case LBMK_SYS_NSF2D_GRADTRACK: gen_eval<Gen_nsf2d>(U, A, ga, F_out, S_out); break;
         case LBMK_SYS_MHD2D: gen_eval<Gen_mhd2d>(U, A, ga, F_out, S_out); break;
         case LBMK_SYS_NSF3D_GRADTRACK: gen_eval<Gen_nsf3d>(U, A, ga, F_out, S_out); break;
+        case LBMK_SYS_ADVECTION2D: gen_eval<Gen_advection2d>(U, A, ga, F_out, S_out); break;
+        case LBMK_SYS_BURGERS2D: gen_eval<Gen_burgers2d>(U, A, ga, F_out, S_out); break;
+        case LBMK_SYS_SWE2D: gen_eval<Gen_swe2d>(U, A, ga, F_out, S_out); break;
+        case LBMK_SYS_URF2D: gen_eval<Gen_urf2d>(U, A, ga, F_out, S_out); break;
+        case LBMK_SYS_MAXWELL2D: gen_eval<Gen_maxwell2d>(U, A, ga, F_out, S_out); break;
+        case LBMK_SYS_ELASTICITY2D: gen_eval<Gen_elasticity2d>(U, A, ga, F_out, S_out); break;
+        case LBMK_SYS_HCNSF3D: gen_eval<Gen_hcnsf3d>(U, A, ga, F_out, S_out); break;
+        case LBMK_SYS_MHD3D_JTRACK: gen_eval<Gen_mhd3d>(U, A, ga, F_out, S_out); break;
         default: return sys_fail(LBMK_EUNSUPPORTED, "no generated augmented system for this id (gen/cascade.py)");
     }
     return LBMK_OK;

@@ -820,5 +820,13 @@ template <> struct GenOf<SysInse2D> { using type = Gen_inse2d; };
 template <> struct GenOf<SysNsf2D> { using type = Gen_nsf2d; };
 template <> struct GenOf<SysMhd2D> { using type = Gen_mhd2d; };
 template <> struct GenOf<SysNsf3D> { using type = Gen_nsf3d; };
+template <> struct GenOf<SysAdvection2D> { using type = Gen_advection2d; };
+template <> struct GenOf<SysBurgers2D> { using type = Gen_burgers2d; };
+template <> struct GenOf<SysSwe2D> { using type = Gen_swe2d; };
+template <> struct GenOf<SysUrf2D> { using type = Gen_urf2d; };
+template <> struct GenOf<SysMaxwell2D> { using type = Gen_maxwell2d; };
+template <> struct GenOf<SysElasticity2D> { using type = Gen_elasticity2d; };
+template <> struct GenOf<SysHcnsf3D> { using type = Gen_hcnsf3d; };
+template <> struct GenOf<SysMhd3D> { using type = Gen_mhd3d; };
 
 }  // namespace lbmk

@@ -46,6 +46,7 @@ class Laws:
         self.source: List[sp.Expr] = []
         self.velocity: List[sp.Expr] = [sp.Integer(0)] * dim      # advecting velocity of the trackers (eq 2.3)
         self.tracked: Dict[sp.Expr, str] = {}                    # derived parents transported directly (`track`)
+        self.custom: List[Tuple[str, List[sp.Expr]]] = []        # trackers of a LINEAR COMBINATION of gradients (`track_combination`)
 
     def grad(self, e) -> List[sp.Expr]:
         return [D_(e, sp.Integer(a)) for a in range(self.dim)]
@@ -53,6 +54,14 @@ class Laws:
     def track(self, name: str, e: sp.Expr):
         """Declare a derived parent whose gradient gets its own tracker (eq 3.27's reduced basis tracks u and T directly)."""
         self.tracked[sp.sympify(e)] = name
+
+    def track_combination(self, name: str, injection: Sequence[sp.Expr]) -> sp.Symbol:
+        """A tracker of a linear combination of first derivatives, T = sum_j d_j (injection_j): flux T (x) u - injection/tau_grad, source
+        -T/tau_grad (eq 2.3 applied to the combination).  HCNSF's reduced basis tracks sym grad u this way (Phi = G_u (x) u -
+        sym(I (x) u)/tau_grad); config 5 tracks the current density J = curl B."""
+        g = sp.Symbol(f"G_{name}", real=True)
+        self.custom.append((g, [sp.sympify(c) for c in injection]))
+        return g
 
     def add(self, flux_rows: Sequence[Sequence[sp.Expr]], sources: Sequence[sp.Expr]):
         assert len(flux_rows) == len(self.V) == len(sources)
@@ -105,6 +114,10 @@ def cascade(laws: Laws) -> Augmented:
                 rep = sum(sp.diff(arg, v) * D_(v, sp.Integer(ax)) for v in laws.V + list(tracker_of.values()) if arg.has(v))
             e = e.xreplace({a: rep})
 
+    for g, inj in laws.custom:                          # declared combination trackers (their symbols already appear in the fluxes)
+        names.append(str(g)); Q.append(g); parents.append((g, -1))
+        Phi.append([g * u[j] - inj[j] / tau for j in range(laws.dim)])
+        S.append(-g / tau)
     k = 0
     while k < len(Q):                                   # rows appended by register() are resolved too (nested cascades)
         Phi[k] = [resolve(sp.sympify(c)) for c in Phi[k]]
@@ -252,7 +265,114 @@ def nsf3d():
     return L
 
 
-SYSTEMS: List[Callable[[], Laws]] = [euler2d, swe2d_bathy, adr2d, allencahn2d, inse2d, nsf2d, mhd2d, nsf3d]
+def advection2d():
+    L = Laws("advection2d", 2, ["U"], ["ax", "ay"])
+    L.add([[L.par[0] * L.V[0], L.par[1] * L.V[0]]], [0])
+    return L
+
+
+def burgers2d():
+    L = Laws("burgers2d", 2, ["u"], [])
+    u, = L.V
+    L.add([[u * u / 2, u * u / 2]], [0])                                                                                       # eq 3.1-3.2
+    return L
+
+
+def swe2d():
+    L = Laws("swe2d", 2, ["h", "q0", "q1"], ["g"])
+    h, q0, q1 = L.V
+    g, = L.par
+    P = g * h * h / 2
+    L.add([[q0, q1], [q0 * q0 / h + P, q0 * q1 / h], [q1 * q0 / h, q1 * q1 / h + P]], [0, 0, 0])                                  # eq 3.6, flat bed
+    return L
+
+
+def urf2d():
+    L = Laws("urf2d", 2, ["E", "S0", "S1"], [])
+    E, S0, S1 = L.V
+    p = (sp.sqrt(4 * E * E - 3 * (S0 * S0 + S1 * S1)) - E) / 3                                                                    # eq 3.9
+    v = [S0 / (E + p), S1 / (E + p)]
+    L.add([[S0, S1], [S0 * v[0] + p, S0 * v[1]], [S1 * v[0], S1 * v[1] + p]], [0, 0, 0])                                          # eq 3.8
+    return L
+
+
+def maxwell2d():
+    L = Laws("maxwell2d", 2, ["Ez", "Hx", "Hy"], ["c"])
+    Ez, Hx, Hy = L.V
+    c, = L.par
+    L.add([[-c * Hy, c * Hx], [0, c * Ez], [-c * Ez, 0]], [0, 0, 0])                                                              # eq 3.11
+    return L
+
+
+def elasticity2d():
+    L = Laws("elasticity2d", 2, ["F00", "F01", "F10", "F11", "m0", "m1"], ["rho0", "mus", "las"])
+    F00, F01, F10, F11, m0, m1 = L.V
+    rho0, mus, las = L.par
+    F = [[F00, F01], [F10, F11]]
+    v = [m0 / rho0, m1 / rho0]
+    J = F00 * F11 - F01 * F10
+    FiT = [[F11 / J, -F10 / J], [-F01 / J, F00 / J]]
+    Pk = [[mus * (F[i][j] - FiT[i][j]) + las * sp.log(J) * FiT[i][j] for j in range(2)] for i in range(2)]                        # eq 3.14
+    L.add([[-v[0], 0], [0, -v[0]], [-v[1], 0], [0, -v[1]], [-Pk[0][0], -Pk[0][1]], [-Pk[1][0], -Pk[1][1]]], [0] * 6)            # eq 3.15
+    return L
+
+
+def hcnsf3d():
+    L = Laws("hcnsf3d", 3, ["rho", "m0", "m1", "m2", "E"], ["gamma", "mu", "kappa", "eta"], aux=["alpha", "us0", "us1", "us2"])
+    rho, m0, m1, m2, E = L.V
+    g, mu, kappa, eta = L.par
+    al, us = L.aux[0], L.aux[1:]
+    m = [m0, m1, m2]
+    u = [mi / rho for mi in m]
+    L.velocity = u
+    p = (g - 1) * (E - rho * sum(ui**2 for ui in u) / 2)
+    T = p / rho
+    L.track("T", T)
+    # reduced basis: the SYMMETRIC velocity gradient, six trackers D_ab = (d_b u_a + d_a u_b)/2
+    pairs = [(0, 0), (1, 1), (2, 2), (0, 1), (0, 2), (1, 2)]
+    Dsym = {}
+    for a, b in pairs:
+        inj = [(u[b] if j == a else 0) / 2 + (u[a] if j == b else 0) / 2 for j in range(3)]
+        Dsym[(a, b)] = Dsym[(b, a)] = L.track_combination(f"D{a}{b}", inj)
+    tr = Dsym[(0, 0)] + Dsym[(1, 1)] + Dsym[(2, 2)]
+    tau = [[mu * (2 * Dsym[(a, b)] - (sp.Rational(2, 3) * tr if a == b else 0)) for b in range(3)] for a in range(3)]
+    gT = L.grad(T)
+    rows = [m]
+    for a in range(3):
+        rows.append([m[a] * u[j] + (p if a == j else 0) - al * tau[a][j] for j in range(3)])
+    rows.append([(E + p) * u[j] - al * sum(tau[j][b] * u[b] for b in range(3)) - al * kappa * gT[j] for j in range(3)])         # eq 3.27
+    drag = [(1 - al) / eta * (rho * us[a] - m[a]) for a in range(3)]
+    L.add(rows, [0] + drag + [sum(drag[a] * u[a] for a in range(3))])
+    return L
+
+
+def mhd3d():
+    L = Laws("mhd3d", 3, ["rho", "m0", "m1", "m2", "E", "B0", "B1", "B2"], ["gamma", "eta"])
+    rho, m0, m1, m2, E, B0, B1, B2 = L.V
+    g, eta = L.par
+    m, B = [m0, m1, m2], [B0, B1, B2]
+    u = [mi / rho for mi in m]
+    L.velocity = u
+    Bsq = sum(b * b for b in B)
+    p = (g - 1) * (E - rho * sum(ui**2 for ui in u) / 2 - Bsq / 2)
+    pt = p + Bsq / 2
+    uB = sum(u[a] * B[a] for a in range(3))
+    eps = sp.LeviCivita
+    # current density J_i = eps_ijk d_j B_k as a combination tracker: injection_j = eps_ijk B_k (C5)
+    Jt = [L.track_combination(f"J{i}", [sum(eps(i, j, k) * B[k] for k in range(3)) for j in range(3)]) for i in range(3)]
+    JxB = [Jt[1] * B[2] - Jt[2] * B[1], Jt[2] * B[0] - Jt[0] * B[2], Jt[0] * B[1] - Jt[1] * B[0]]
+    rows = [m]
+    for a in range(3):
+        rows.append([m[a] * u[j] - B[a] * B[j] + (pt if a == j else 0) for j in range(3)])
+    rows.append([(E + pt) * u[j] - B[j] * uB + eta * JxB[j] for j in range(3)])
+    for i in range(3):
+        rows.append([B[i] * u[j] - u[i] * B[j] + eta * sum(eps(i, j, k) * Jt[k] for k in range(3)) for j in range(3)])
+    L.add(rows, [0] * 8)
+    return L
+
+
+SYSTEMS: List[Callable[[], Laws]] = [euler2d, swe2d_bathy, adr2d, allencahn2d, inse2d, nsf2d, mhd2d, nsf3d,
+                                     advection2d, burgers2d, swe2d, urf2d, maxwell2d, elasticity2d, hcnsf3d, mhd3d]
 
 # order of the augmented components in csrc/systems.cuh / oracle (trackers listed parent by parent, axis fastest)
 ORDER = {
@@ -264,6 +384,10 @@ ORDER = {
     "nsf2d": ["rho", "m0", "m1", "E"] + [f"G_{v}_{b}" for v in ("rho", "m0", "m1", "E") for b in range(2)],
     "mhd2d": ["rho", "m0", "m1", "E", "B0", "B1"] + [f"G_{v}_{b}" for v in ("rho", "m0", "m1", "E", "B0", "B1") for b in range(2)],
     "nsf3d": ["rho", "m0", "m1", "m2", "E"] + [f"G_u{a}_{b}" for a in range(3) for b in range(3)] + [f"G_T_{b}" for b in range(3)],
+    "advection2d": ["U"], "burgers2d": ["u"], "swe2d": ["h", "q0", "q1"], "urf2d": ["E", "S0", "S1"], "maxwell2d": ["Ez", "Hx", "Hy"],
+    "elasticity2d": ["F00", "F01", "F10", "F11", "m0", "m1"],
+    "hcnsf3d": ["rho", "m0", "m1", "m2", "E", "G_D00", "G_D11", "G_D22", "G_D01", "G_D02", "G_D12", "G_T_0", "G_T_1", "G_T_2"],
+    "mhd3d": ["rho", "m0", "m1", "m2", "E", "B0", "B1", "B2", "G_J0", "G_J1", "G_J2"],
 }
 
 

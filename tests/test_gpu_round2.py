@@ -205,7 +205,11 @@ def test_mhd2d_subcharacteristic_reduction_matches_the_oracle(P):
 @pytest.mark.parametrize("mk,kw,prec,steps", [
     (W.pin_euler, dict(n=48), "f64s", 40), (W.pin_swe, dict(n=40), "f64", 30), (W.pin_adr, dict(n=32), "f64s", 60),
     (W.pin_allencahn, dict(n=32), "f64", 60), (W.pin_inse, dict(n=32), "f64s", 60), (W.pin_nsf2d, dict(n=40), "f64s", 80),
-    (W.pin_mhd2d, dict(n=40), "f64s", 80), (W.c4_nsf3d, dict(n=16, ny=12, nz=10), "f64s", 30), (W.c4_nsf3d, dict(n=16, ny=12, nz=10), "f32s", 30)])
+    (W.pin_mhd2d, dict(n=40), "f64s", 80), (W.c4_nsf3d, dict(n=16, ny=12, nz=10), "f64s", 30), (W.c4_nsf3d, dict(n=16, ny=12, nz=10), "f32s", 30),
+    (W.c1_advection, dict(n=40, ny=24), "f64", 10), (W.pin_burgers, dict(n=32), "f64", 30), (W.c2_swe, dict(n=40, ny=28), "f64s", 30),
+    (W.pin_urf, dict(n=32), "f64", 30), (W.pin_maxwell, dict(n=32), "f64", 30), (W.pin_elasticity, dict(n=32), "f64s", 30),
+    (W.hcnsf3d, dict(n=16, ny=12, nz=10), "f64s", 20), (W.hcnsf3d, dict(n=16, ny=12, nz=10), "f32s", 20),
+    (W.c5_mhd3d, dict(n=16, ny=12, nz=10), "f64s", 20), (W.c5_mhd3d, dict(n=16, ny=12, nz=10), "f32s", 20)])
 def test_hand_written_delta_forms_equal_the_generated_augmented_systems(P, mk, kw, prec, steps):
     """SURVEY section 8(f) item 2: gen/cascade.py DERIVES the augmented system (Alg 2.1 Split/Cascade/Assemble/Emit, PAPER.md:L221-L278);
     lbmk_flux_selfcheck evaluates, on every node of a live state, the hand-written delta-form flux/source the step kernels use and
@@ -219,13 +223,19 @@ def test_hand_written_delta_forms_equal_the_generated_augmented_systems(P, mk, k
     assert 0.0 <= d <= 5e-12, d
 
 
-def test_flux_selfcheck_needs_a_generated_system(P):
-    w = W.pin_urf(16)
-    g = P.Grid.from_workload(w); g.init_from_U(w.initial_U())
-    with pytest.raises(P.LbmkError) as e:
-        P.lbmk_flux_selfcheck(g.h)
-    assert e.value.status == 6
-    g.close()
+def test_every_system_has_a_generated_form(P):
+    """All 16 systems of the library carry the emitted plain form next to their hand-written delta form."""
+    for name in P.SYSTEM_ID:
+        mk = {"advection2d": W.c1_advection, "burgers2d": W.pin_burgers, "swe2d": W.c2_swe, "euler2d": W.pin_euler, "adr2d": W.pin_adr,
+              "nsf3d": W.c4_nsf3d, "mhd3d": W.c5_mhd3d, "urf2d": W.pin_urf, "maxwell2d": W.pin_maxwell, "allencahn2d": W.pin_allencahn,
+              "inse2d": W.pin_inse, "elasticity2d": W.pin_elasticity, "nsf2d": W.pin_nsf2d, "swe2d_bathy": W.pin_swe,
+              "hcnsf3d": W.hcnsf3d, "mhd2d": W.pin_mhd2d}[name]
+        w = mk(n=16 if name in ("nsf3d", "mhd3d", "hcnsf3d") else 32)
+        assert w.system == name
+        g = P.Grid.from_workload(w); g.init_from_U(w.initial_U()); g.step(3)
+        d = P.lbmk_flux_selfcheck(g.h)
+        g.close()
+        assert 0.0 <= d <= (5e-12 if w.precision == "f64" else 5e-5), (name, d)
 
 
 def test_multi_node_kernel_for_single_field_fp32_is_bit_identical(P):

@@ -182,8 +182,7 @@ def test_workspace_guards_stay_untouched(P, mk, kw, pattern, stepping):
         P.lbmk_step(g, n)
         P.lbmk_read_U(g, out.data_ptr(), True)
         P.lbmk_check_subcharacteristic(g, raise_on_violation=False)
-    if w.system in ("swe2d_bathy", "mhd2d", "nsf2d"):
-        P.lbmk_flux_selfcheck(g)
+    P.lbmk_flux_selfcheck(g)
     torch.cuda.synchronize()
     assert bool((buf[:off] == 0xA5).all()) and bool((buf[off + nbytes:] == 0xA5).all())
     assert bool(torch.isfinite(out).all())
