@@ -12,6 +12,10 @@
 
 namespace lbmk {
 
+constexpr int PERSISTENT_MAX_BLOCKS = 2048;   // "steps done" flags of the persistent kernel: one per block,
+constexpr int FLAG_STRIDE = 32;              // each in its own 128-byte line (32 words apart)
+
+
 constexpr int MAXM = 20;   // largest compiled-in system has 18 components
 
 template <int D> struct Lattice;

@@ -30,6 +30,10 @@ enum { GATHER_CANON = 0, GATHER_AA_ODD = 1, GATHER_PULL = 2 };
 template <class Sys> __host__ __device__ constexpr bool has_mms() { return !std::is_void<typename Sys::Mms>::value; }
 template <class Sys, bool = has_mms<Sys>()> struct MmsNC { static constexpr int value = 4; };
 template <class Sys> struct MmsNC<Sys, true> { static constexpr int value = Sys::Mms::NC; };
+// Row coefficients are staged in shared memory (cp.async + one bar.sync per segment) only when there are enough of them to
+// pay for the barrier: measured on c2 (12 coefficients) the warp-uniform global loads are 0.6 us per step faster, on c4 (108)
+// the staged copy wins.
+constexpr int STAGE_MIN_NC = 48;
 
 // per-node manufactured forcing: the x-table entries of this node and the coefficients of its (y, z) row
 // (mms_generated.cuh source_row; the row table is filled by mms_row_coeffs_kernel).  SH: `c` is the block's
@@ -179,7 +183,7 @@ __device__ __forceinline__ void node_step(typename StepPtr<R, MODE, COHERENT>::S
     const long long node = first + threadIdx.x;
     constexpr int NCs = MMS ? MmsNC<Sys>::value : 4;
     // kernel-uniform: a block lies inside one (y, z) row; then every segment is full (n and node0 are multiples of BLOCK)
-    const bool staged = MMS && (P.nx % BLOCK == 0) && (P.node0 % BLOCK == 0);
+    const bool staged = MMS && NCs >= STAGE_MIN_NC && (P.nx % BLOCK == 0) && (P.node0 % BLOCK == 0);
     if constexpr (MMS) {
         if (staged) {
             const unsigned row = (unsigned)(first / P.nx);
@@ -259,22 +263,34 @@ collide_stream_node(typename StepPtr<R, MODE>::Src src, typename StepPtr<R, MODE
 
 // ------------------------------------------------------------------------------------------------ step, persistent
 // Launch-free stepping for grids whose state lives in L2 (SURVEY.md §7 "Small configs"): ONE cooperative launch
-// advances `nsteps` steps of the two-lattice pull pattern; all blocks are co-resident, each takes the BLOCK-node
-// segments b, b + gridDim.x, ... of every step, and a grid-wide barrier separates the steps (the buffer written in
-// step s is the one read in step s+1).  Step s reads its forcing coefficients at P.coef + s*coef_stride.  The
-// per-node code is node_step, i.e. bit-identical to the per-launch path.
-__device__ __forceinline__ void grid_barrier(unsigned int* bar, unsigned int target) {
-    // arrive: after the block-wide barrier one thread publishes the block's stores with a gpu-scope RELEASE increment of
-    // the monotone counter (cumulative over what the other threads wrote before bar.sync); wait: the same thread spins with
-    // gpu-scope ACQUIRE loads until all blocks of this step have arrived, then releases its block.  The populations are
-    // read with ld.global.cg (L2), so no stale L1 line can be observed after the barrier.
+// advances `nsteps` steps of the two-lattice pull pattern; all blocks are co-resident.  Block b owns the CONTIGUOUS
+// node range [b*rounds*BLOCK, (b+1)*rounds*BLOCK) in every step, so what it reads in step s+1 was written in step s by
+// the blocks whose ranges lie within one stencil reach (nx nodes in 2D, nx*ny in 3D, cyclically) of its own -- a cyclic
+// run of `ndep` blocks starting at `dep0`.  Steps are therefore separated by POINT-TO-POINT flags, not by a grid-wide
+// barrier: a block publishes "step s done" in flag[b] and waits only for the flags of its dependency run; the same
+// condition covers the write-after-read hazard of the two buffers (a block overwrites in step s+1 what its neighbours
+// read in step s).  No global drain: neighbouring blocks may be one step apart.  Step s reads its forcing coefficients
+// at P.coef + s*coef_stride.  The per-node code is node_step, i.e. bit-identical to the per-launch path.
+// One flag per 128-byte line (FLAG_STRIDE words apart): with 32 flags in a line the pollers of 32 blocks queue at one L2
+// sector in front of the stores they wait for (measured on c2: 11.0 us per step packed, 7.8 us one per line).
+__device__ __forceinline__ void flags_publish(unsigned int* flag, unsigned int value) {
+    // after the block-wide barrier one thread publishes the block's stores with a gpu-scope RELEASE store (cumulative over
+    // what the other threads wrote before bar.sync)
     __syncthreads();
-    if (threadIdx.x == 0) {
-        asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(bar), "r"(1u) : "memory");
-        unsigned int v;
-        do {
-            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(bar) : "memory");
-        } while (v < target);
+    if (threadIdx.x == 0) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(flag), "r"(value) : "memory");
+}
+__device__ __forceinline__ void flags_wait(const unsigned int* flags, int dep0, int ndep, int nblocks, unsigned int target) {
+    // the first warp polls the dependency run, one flag per lane, with gpu-scope ACQUIRE loads; the populations are then
+    // read with ld.global.cg (L2), so no stale L1 line can be observed
+    if (threadIdx.x < 32) {
+        for (int j = (int)threadIdx.x; j < ndep; j += 32) {
+            int d = dep0 + j;
+            if (d >= nblocks) d -= nblocks;
+            unsigned int v;
+            do {
+                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(flags + (size_t)d * FLAG_STRIDE) : "memory");
+            } while (v < target);
+        }
     }
     __syncthreads();
 }
@@ -282,23 +298,39 @@ __device__ __forceinline__ void grid_barrier(unsigned int* bar, unsigned int tar
 template <class Sys, class R, bool MMS, int BLOCK, int MINB>
 __global__ void __launch_bounds__(BLOCK, MINB)
 collide_stream_persistent(R* fa, R* fb, const __grid_constant__ KParams<R> P, int nsteps, int first_local, long long coef_stride,
-                          unsigned int* bar) {
+                          unsigned int* flags, int rounds) {
     constexpr int NCs = MMS ? MmsNC<Sys>::value : 4;
     __shared__ __align__(16) R coef_s[NCs];
     const long long nseg = (P.n + BLOCK - 1) / BLOCK;
-    const bool staged = MMS && (P.nx % BLOCK == 0);
+    const bool staged = MMS && NCs >= STAGE_MIN_NC && (P.nx % BLOCK == 0);
+    const long long seg0 = (long long)blockIdx.x * rounds, seg1 = seg0 + rounds < nseg ? seg0 + rounds : nseg;
+    // dependency run: the blocks owning the nodes [first - reach, last + reach] (cyclic)
+    const long long npb = (long long)rounds * BLOCK, reach = Sys::D == 3 ? (long long)P.nx * P.ny : (long long)P.nx;
+    const long long first = seg0 * BLOCK, last = (seg1 * BLOCK < P.n ? seg1 * BLOCK : P.n) - 1;
+    int dep0 = 0, ndep = (int)gridDim.x;
+    if (last - first + 1 + 2 * reach < P.n) {
+        long long lo = first - reach, hi = last + reach;
+        if (lo < 0) lo += P.n;
+        if (hi >= P.n) hi -= P.n;
+        dep0 = (int)(lo / npb);
+        const int dep1 = (int)(hi / npb);
+        ndep = (lo > hi && dep0 == dep1) ? (int)gridDim.x : (dep1 - dep0 + (int)gridDim.x) % (int)gridDim.x + 1;
+    }
     R* src = fa;
     R* dst = fb;
     const R* coef = P.coef;
     for (int s = 0; s < nsteps; ++s) {
-        for (long long seg = blockIdx.x; seg < nseg; seg += gridDim.x) {
+        for (long long seg = seg0; seg < seg1; ++seg) {
             if (s == 0 && first_local) node_step<Sys, R, MODE_LOCAL, MMS, BLOCK, true>(src, dst, P, coef, seg * BLOCK, coef_s);
             else node_step<Sys, R, MODE_PULL2, MMS, BLOCK, true>(src, dst, P, coef, seg * BLOCK, coef_s);
             if (staged) __syncthreads();          // coef_s is overwritten by the next segment
         }
         R* t = src; src = dst; dst = t;
         coef += coef_stride;
-        if (s + 1 < nsteps) grid_barrier(bar, (unsigned)(s + 1) * gridDim.x);
+        if (s + 1 < nsteps) {
+            flags_publish(flags + (size_t)blockIdx.x * FLAG_STRIDE, (unsigned)(s + 1));
+            flags_wait(flags, dep0, ndep, (int)gridDim.x, (unsigned)(s + 1));
+        }
     }
 }
 

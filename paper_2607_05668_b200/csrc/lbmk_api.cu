@@ -356,7 +356,7 @@ static void layout(lbmk_grid* g) {
         g->off_coef = off; off += align_up(2 * (size_t)c.coef_B * per_step, 256);
     }
     g->off_feq0 = off; off += align_up((size_t)o->M * (2 * o->D + 1) * 8, 256);
-    g->off_red = off; off += 256;          // [0..3] reductions, [8] grid-barrier counter
+    g->off_red = off; off += 256 + (size_t)PERSISTENT_MAX_BLOCKS * FLAG_STRIDE * sizeof(unsigned int);   // [0..3] reductions; then one step flag per block of the persistent kernel
     c.aux_stride = (long long)(ntiles * TILE);
     g->off_aux = off; off += align_up((size_t)(o->n_aux > 0 ? o->n_aux : 0) * ntiles * TILE * esz, 256);
     g->ws_bytes = off;
@@ -597,7 +597,7 @@ lbmk_status lbmk_grid_bind_workspace(lbmk_grid* g, void* device_ptr, size_t byte
     c.coef = base + g->off_coef;
     c.feq0 = (double*)(base + g->off_feq0);
     c.red = (unsigned long long*)(base + g->off_red);
-    c.bar = (unsigned int*)(base + g->off_red + 64);
+    c.bar = (unsigned int*)(base + g->off_red + 256);
     c.aux_buf = g->ops->n_aux > 0 ? base + g->off_aux : nullptr;
     c.aux_set = false;
     c.cur = 0;

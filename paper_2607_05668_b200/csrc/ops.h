@@ -33,7 +33,7 @@ struct GridCore {
     bool coef_used[2];
     double* feq0;         // [M*Q] reference equilibrium (fp64)
     unsigned long long* red;   // [4] reduction scratch
-    unsigned int* bar;    // grid-barrier counter of the persistent kernel (zeroed before each launch)
+    unsigned int* bar;    // PERSISTENT_MAX_BLOCKS "steps done" flags of the persistent kernel, one per block (zeroed before each launch)
     void* aux_buf;        // prescribed coefficient fields in R, [n_aux][aux_stride]
     long long aux_stride;
     bool aux_set;

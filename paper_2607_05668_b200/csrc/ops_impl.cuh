@@ -1,6 +1,7 @@
 // ops_impl.cuh -- launches of the templated kernels for one system; included by each sys_*.cu.
 #pragma once
 #include <algorithm>
+#include <climits>
 #include <cstring>
 #include <vector>
 
@@ -211,28 +212,31 @@ struct Ops {
     }
     // ---- persistent stepping: `cnt` steps of the two-lattice pull pattern in ONE cooperative launch (kernels.cuh)
     template <class R, bool MMS>
-    static int persistent_grid(GridCore& g) {
+    static int persistent_grid(GridCore& g, int* rounds_out = nullptr) {
         constexpr int BLOCK = TuneP<S, R>::BLOCK, MINB = TuneP<S, R>::MINB;
         int per_sm = 0;
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, collide_stream_persistent<S<R>, R, MMS, BLOCK, MINB>, BLOCK, 0) != cudaSuccess) return 0;
-        const long long cap = (long long)per_sm * g.num_sms, nseg = (g.n + BLOCK - 1) / BLOCK;
+        const long long cap = std::min<long long>((long long)per_sm * g.num_sms, PERSISTENT_MAX_BLOCKS), nseg = (g.n + BLOCK - 1) / BLOCK;
         if (cap <= 0) return 0;
         const long long rounds = (nseg + cap - 1) / cap;          // segments per block and step
-        return (int)((nseg + rounds - 1) / rounds);               // balanced: every block takes `rounds` (or rounds-1) segments
+        if (rounds > INT_MAX) return 0;
+        if (rounds_out) *rounds_out = (int)rounds;
+        return (int)((nseg + rounds - 1) / rounds);               // balanced: every block owns `rounds` consecutive segments (the last one fewer)
     }
     template <class R, bool MMS>
     static cudaError_t launch_persistent(GridCore& g, int cnt, long long coef_stride) {
         constexpr int BLOCK = TuneP<S, R>::BLOCK, MINB = TuneP<S, R>::MINB;
-        const int grid = persistent_grid<R, MMS>(g);
+        int rounds = 0;
+        const int grid = persistent_grid<R, MMS>(g, &rounds);
         if (grid <= 0) return cudaErrorLaunchOutOfResources;
-        cudaError_t e = cudaMemsetAsync(g.bar, 0, sizeof(unsigned int), g.stream);
+        cudaError_t e = cudaMemsetAsync(g.bar, 0, (size_t)grid * FLAG_STRIDE * sizeof(unsigned int), g.stream);     // one "steps done" flag per block
         if (e != cudaSuccess) return e;
         R* fa = (R*)g.f[g.cur];
         R* fb = (R*)g.f[g.cur ^ 1];
         KParams<R> P = kp<R>(g);
         int first_local = g.pending ? 0 : 1;
         unsigned int* bar = g.bar;
-        void* args[] = {&fa, &fb, &P, &cnt, &first_local, &coef_stride, &bar};
+        void* args[] = {&fa, &fb, &P, &cnt, &first_local, &coef_stride, &bar, &rounds};
         e = cudaLaunchCooperativeKernel((const void*)collide_stream_persistent<S<R>, R, MMS, BLOCK, MINB>, dim3(grid), dim3(BLOCK), args, 0, g.stream);
         if (e != cudaSuccess) return e;
         g.launches++;
