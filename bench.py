@@ -514,7 +514,9 @@ def run_ours(args):
     bytes_per_launch = w.n_nodes * w.bytes_per_node
     ms_launch = ms_local / steps
     achieved = bytes_per_launch / (ms_launch * 1e-3) / 1e9
-    traffic = NCU_TRAFFIC_BYTES.get(f"{args.config}:{pattern}:{kernel}") if args.n is None else None    # captured at the full size only
+    mode = getattr(g, "stepping", "launch")                  # persistent / cluster launches have their own captures (per step)
+    key = f"{args.config}:{pattern}:{kernel}" + ("" if mode == "launch" else f":{mode}")
+    traffic = NCU_TRAFFIC_BYTES.get(key) if args.n is None else None    # captured at the full size only
     line = {
         "metric": METRIC, "value": mlups, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warm,
         "ms_per_step": ms / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -532,7 +534,11 @@ def run_ours(args):
                                         "`ncu --set full` capture of this kernel and launch configuration (profiles/), NOT measured by this run")
                                        if traffic is not None else None,
                      "peak_source": peak_src, "frac_of_nominal_8TBps": achieved / 8000.0,
-                     "kernel": "collide_stream (one launch per step)", "algorithmic_bytes_per_launch": bytes_per_launch,
+                     "kernel": {"launch": "collide_stream_node (one launch per step)",
+                                "persistent": "collide_stream_persistent (one cooperative launch per lbmk_step call; figures per step)",
+                                "cluster": "collide_stream_cluster (one cluster launch per lbmk_step call; figures per step)"}.get(
+                                    getattr(g, "stepping", "launch"), "collide_stream"),
+                     "stepping": getattr(g, "stepping", "launch"), "algorithmic_bytes_per_launch": bytes_per_launch,
                      "lbmk_copy_probe_GBps": probe,
                      "frac_of_max_measured_copy": achieved / max(peak, probe) if isinstance(probe, float) else None},
         "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
