@@ -70,7 +70,7 @@ def parse_args():
     ap.add_argument("--kernel", default="auto", choices=["auto", "node", "twopass"])
     ap.add_argument("--n", "--edge", dest="n", type=int, default=None, help="override the grid edge (debug; the line then says so; --edge under torchrun, whose parser claims --n)")
     ap.add_argument("--no-mms", action="store_true", help="without manufactured forcing (the paper's Table 3 kernels carry none)")
-    ap.add_argument("--stepping", default="auto", choices=["auto", "launch", "persistent", "cluster"])
+    ap.add_argument("--stepping", default="auto", choices=["auto", "launch", "persistent", "cluster", "resident"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-all-configs", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -265,14 +265,14 @@ class SlabRunner:
 def short_run(P, torch, name, pattern):
     """MLUPS / GB/s of one of the other configs (its full step count, 5% warm-up, median of 3).  L2-resident configs run
     launch-free (one cooperative launch per batch of steps, lbmk.h LBMK_STEPPING_PERSISTENT); the one-launch-per-step
-    figure is reported beside it."""
+    figure and, where one population copy fits the shared memory of all SMs, the SM-resident figure are reported beside it."""
     w = make_workload(name)
     out = None
-    for stepping in ("auto", "launch"):
-        g = P.Grid.from_workload(w, pattern=pattern, stepping=stepping)
-        if stepping == "launch" and out["stepping"] == "launch":
+    for stepping in ("auto", "launch", "resident"):
+        g = P.Grid.from_workload(w, pattern=pattern if stepping != "resident" else "auto", stepping=stepping)
+        if stepping != "auto" and (out["stepping"] == "launch" or g.stepping != stepping):      # large grids: one launch per step is all there is
             g.close()
-            break
+            continue
         g.init_from_U(torch.from_numpy(w.initial_U()).cuda())
         g.step(max(10, w.steps // 20))
         reps, launches = [], 0
@@ -286,7 +286,8 @@ def short_run(P, torch, name, pattern):
                    "stepping": g.stepping, "steps": w.steps, "launches": launches, "ms_per_step": ms / w.steps, "MLUPS": mlups,
                    "GBps_algorithmic": mlups * w.bytes_per_node / 1e3, "state_MB": w.n_nodes * w.bytes_per_node / 2 / 1e6}
         else:
-            out["one_launch_per_step"] = {"ms_per_step": ms / w.steps, "MLUPS": mlups, "launches": launches}
+            # "resident": LBMK_STEPPING_RESIDENT, one population copy in the shared memory of all SMs (AA pattern; opt-in)
+            out["one_launch_per_step" if stepping == "launch" else "sm_resident"] = {"ms_per_step": ms / w.steps, "MLUPS": mlups, "launches": launches, "pattern": g.pattern}
         g.close()
     return out
 
@@ -490,7 +491,7 @@ def run_ours(args):
                "d2h_bytes_per_step": nbytes / steps, "ms_total": e_ms,
                "what": f"lbmk_init_from_U(pinned host U, {nbytes / 1e6:.0f} MB) -> {steps} steps -> lbmk_read_U(pinned host)"}
         del U_host, out_host
-    pattern, kernel = g.pattern, g.kernel
+    pattern, kernel, mode = g.pattern, g.kernel, getattr(g, "stepping", "launch")
     g.close()
     del g, U0_dev
     torch.cuda.empty_cache()
@@ -514,7 +515,7 @@ def run_ours(args):
     bytes_per_launch = w.n_nodes * w.bytes_per_node
     ms_launch = ms_local / steps
     achieved = bytes_per_launch / (ms_launch * 1e-3) / 1e9
-    mode = getattr(g, "stepping", "launch")                  # persistent / cluster launches have their own captures (per step)
+    # persistent / cluster / resident launches have their own captures (per step)
     key = f"{args.config}:{pattern}:{kernel}" + ("" if mode == "launch" else f":{mode}")
     traffic = NCU_TRAFFIC_BYTES.get(key) if args.n is None else None    # captured at the full size only
     line = {
@@ -536,9 +537,10 @@ def run_ours(args):
                      "peak_source": peak_src, "frac_of_nominal_8TBps": achieved / 8000.0,
                      "kernel": {"launch": "collide_stream_node (one launch per step)",
                                 "persistent": "collide_stream_persistent (one cooperative launch per lbmk_step call; figures per step)",
-                                "cluster": "collide_stream_cluster (one cluster launch per lbmk_step call; figures per step)"}.get(
-                                    getattr(g, "stepping", "launch"), "collide_stream"),
-                     "stepping": getattr(g, "stepping", "launch"), "algorithmic_bytes_per_launch": bytes_per_launch,
+                                "cluster": "collide_stream_cluster (one cluster launch per lbmk_step call; figures per step)",
+                                "resident": "collide_stream_resident (state in the shared memory of all SMs, one cooperative launch per lbmk_step call; figures per step)"}.get(
+                                    mode, "collide_stream"),
+                     "stepping": mode, "algorithmic_bytes_per_launch": bytes_per_launch,
                      "lbmk_copy_probe_GBps": probe,
                      "frac_of_max_measured_copy": achieved / max(peak, probe) if isinstance(probe, float) else None},
         "e2e": e2e, "gpu_launches": launches, "clocks": clocks,

@@ -96,7 +96,7 @@ typedef enum {
     LBMK_OPT_STEPPING = 2   /* how lbmk_step(n) issues its n steps: LBMK_STEPPING_* */
 } lbmk_option;
 /* LBMK_STEPPING_LAUNCH: one kernel launch per step.  LBMK_STEPPING_PERSISTENT: one cooperative launch advances a whole batch
- * of steps (all blocks co-resident, a grid-wide barrier between steps) -- for grids whose populations live in L2 and whose
+ * of steps (all blocks co-resident, point-to-point step flags between neighbouring blocks) -- for grids whose populations live in L2 and whose
  * step is therefore launch-latency bound (SURVEY.md section 7 "Small configs"); two-lattice pull, periodic, node kernel only,
  * bit-identical to the per-launch path.  LBMK_STEPPING_CLUSTER: grids of at most 8192 nodes of a small tracker-free system
  * without forcing or prescribed fields (configs[0]): ONE thread-block cluster of 8 CTAs keeps the populations in distributed
@@ -104,8 +104,14 @@ typedef enum {
  * paths to rounding (nvcc decides FMA contraction per kernel; bit-identical for linear systems such as configs[0]'s).
  * AUTO never changes bits: it picks CLUSTER only when the grid qualifies AND the system is linear (configs[0]), else PERSISTENT
  * when both population copies fit in 96 MB, else LAUNCH; CLUSTER for a nonlinear system must be asked for explicitly; a mode
- * the grid does not qualify for falls back to the next one (lbmk_grid_get_option returns the resolved mode). */
-enum { LBMK_STEPPING_AUTO = 0, LBMK_STEPPING_LAUNCH = 1, LBMK_STEPPING_PERSISTENT = 2, LBMK_STEPPING_CLUSTER = 3 };
+ * the grid does not qualify for falls back to the next one (lbmk_grid_get_option returns the resolved mode).
+ * LBMK_STEPPING_RESIDENT (never picked by AUTO): grids whose ONE population copy fits in the shared memory of all SMs together
+ * (148 x 227 KB = 33 MB; configs[1] in fp64 is 31 MB): one cooperative launch with one block per SM, every block keeps its
+ * contiguous run of 128-node tiles in shared memory and steps it in place with the AA pattern; only the populations that cross a
+ * block boundary stay in global memory (L2).  Implies LBMK_PATTERN_AA unless a pattern was set; periodic, node kernel, BGK;
+ * any system, forcing and prescribed fields included.  Same arithmetic (collide_core), equal to the other paths to rounding.
+ * Resolved at lbmk_grid_bind_workspace (the SM count is a property of the device): a grid that does not fit steps per launch. */
+enum { LBMK_STEPPING_AUTO = 0, LBMK_STEPPING_LAUNCH = 1, LBMK_STEPPING_PERSISTENT = 2, LBMK_STEPPING_CLUSTER = 3, LBMK_STEPPING_RESIDENT = 4 };
 enum { LBMK_PATTERN_AUTO = 0, LBMK_PATTERN_PULL2 = 1 /* two-lattice pull */, LBMK_PATTERN_AA = 2 /* in-place */ };
 enum { LBMK_KERNEL_AUTO = 0, LBMK_KERNEL_NODE = 1 /* one node per thread, direct loads */,
        LBMK_KERNEL_ROW = 2 /* reserved: shared-memory / TMA staged x-rows; not built (direct loads already move exactly the

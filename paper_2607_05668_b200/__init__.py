@@ -30,7 +30,7 @@ LBMK_D2Q5, LBMK_D3Q7 = 0, 1
 LBMK_F64, LBMK_F32_SHIFTED, LBMK_F64_SHIFTED = 0, 1, 2
 LBMK_PERIODIC, LBMK_DIRICHLET_MMS = 0, 1
 LBMK_OPT_PATTERN, LBMK_OPT_KERNEL, LBMK_OPT_STEPPING = 0, 1, 2
-LBMK_STEPPING_AUTO, LBMK_STEPPING_LAUNCH, LBMK_STEPPING_PERSISTENT, LBMK_STEPPING_CLUSTER = 0, 1, 2, 3
+LBMK_STEPPING_AUTO, LBMK_STEPPING_LAUNCH, LBMK_STEPPING_PERSISTENT, LBMK_STEPPING_CLUSTER, LBMK_STEPPING_RESIDENT = 0, 1, 2, 3, 4
 LBMK_PATTERN_AUTO, LBMK_PATTERN_PULL2, LBMK_PATTERN_AA = 0, 1, 2
 LBMK_KERNEL_AUTO, LBMK_KERNEL_NODE, LBMK_KERNEL_ROW, LBMK_KERNEL_TWOPASS = 0, 1, 2, 3
 SYSTEM_ID = {"advection2d": 0, "burgers2d": 1, "swe2d": 2, "euler2d": 3, "adr2d": 4, "nsf3d": 5, "mhd3d": 6, "urf2d": 7, "maxwell2d": 8, "allencahn2d": 9, "inse2d": 10, "elasticity2d": 11, "nsf2d": 12,
@@ -38,7 +38,7 @@ SYSTEM_ID = {"advection2d": 0, "burgers2d": 1, "swe2d": 2, "euler2d": 3, "adr2d"
 PRECISION = {"f64": LBMK_F64, "f32s": LBMK_F32_SHIFTED, "f64s": LBMK_F64_SHIFTED}
 PATTERN = {"auto": 0, "pull2": 1, "aa": 2}
 KERNEL = {"auto": 0, "node": 1, "row": 2, "twopass": 3}
-STEPPING = {"auto": 0, "launch": 1, "persistent": 2, "cluster": 3}
+STEPPING = {"auto": 0, "launch": 1, "persistent": 2, "cluster": 3, "resident": 4}
 
 # every symbol include/lbmk.h declares: (restype, argtypes)
 _dp = C.POINTER(C.c_double)
@@ -451,7 +451,7 @@ class Grid:
         lbmk_grid_bind_workspace(self.h, self.workspace.data_ptr(), self.workspace_bytes)
         self.pattern = {1: "pull2", 2: "aa"}[lbmk_grid_get_option(self.h, LBMK_OPT_PATTERN)]
         self.kernel = {1: "node", 2: "row", 3: "twopass"}[lbmk_grid_get_option(self.h, LBMK_OPT_KERNEL)]
-        self.stepping = {1: "launch", 2: "persistent", 3: "cluster"}[lbmk_grid_get_option(self.h, LBMK_OPT_STEPPING)]
+        self.stepping = {1: "launch", 2: "persistent", 3: "cluster", 4: "resident"}[lbmk_grid_get_option(self.h, LBMK_OPT_STEPPING)]
 
     @classmethod
     def from_workload(cls, w, precision: Optional[str] = None, omega=None, declare_bound: bool = True, collision: str = "bgk",

@@ -295,6 +295,20 @@ __device__ __forceinline__ void flags_wait(const unsigned int* flags, int dep0, 
     __syncthreads();
 }
 
+// The blocks owning the nodes [first - reach, last + reach] (cyclic): a cyclic run of `ndep` blocks starting at `dep0`
+// (every block owns `npb` consecutive nodes, the last one fewer).
+__device__ __forceinline__ void dependency_run(long long first, long long last, long long reach, long long npb, long long n, int& dep0, int& ndep) {
+    dep0 = 0; ndep = (int)gridDim.x;
+    if (last - first + 1 + 2 * reach < n) {
+        long long lo = first - reach, hi = last + reach;
+        if (lo < 0) lo += n;
+        if (hi >= n) hi -= n;
+        dep0 = (int)(lo / npb);
+        const int dep1 = (int)(hi / npb);
+        ndep = (lo > hi && dep0 == dep1) ? (int)gridDim.x : (dep1 - dep0 + (int)gridDim.x) % (int)gridDim.x + 1;
+    }
+}
+
 template <class Sys, class R, bool MMS, int BLOCK, int MINB>
 __global__ void __launch_bounds__(BLOCK, MINB)
 collide_stream_persistent(R* fa, R* fb, const __grid_constant__ KParams<R> P, int nsteps, int first_local, long long coef_stride,
@@ -304,18 +318,9 @@ collide_stream_persistent(R* fa, R* fb, const __grid_constant__ KParams<R> P, in
     const long long nseg = (P.n + BLOCK - 1) / BLOCK;
     const bool staged = MMS && NCs >= STAGE_MIN_NC && (P.nx % BLOCK == 0);
     const long long seg0 = (long long)blockIdx.x * rounds, seg1 = seg0 + rounds < nseg ? seg0 + rounds : nseg;
-    // dependency run: the blocks owning the nodes [first - reach, last + reach] (cyclic)
-    const long long npb = (long long)rounds * BLOCK, reach = Sys::D == 3 ? (long long)P.nx * P.ny : (long long)P.nx;
     const long long first = seg0 * BLOCK, last = (seg1 * BLOCK < P.n ? seg1 * BLOCK : P.n) - 1;
-    int dep0 = 0, ndep = (int)gridDim.x;
-    if (last - first + 1 + 2 * reach < P.n) {
-        long long lo = first - reach, hi = last + reach;
-        if (lo < 0) lo += P.n;
-        if (hi >= P.n) hi -= P.n;
-        dep0 = (int)(lo / npb);
-        const int dep1 = (int)(hi / npb);
-        ndep = (lo > hi && dep0 == dep1) ? (int)gridDim.x : (dep1 - dep0 + (int)gridDim.x) % (int)gridDim.x + 1;
-    }
+    int dep0, ndep;
+    dependency_run(first, last, Sys::D == 3 ? (long long)P.nx * P.ny : (long long)P.nx, (long long)rounds * BLOCK, P.n, dep0, ndep);
     R* src = fa;
     R* dst = fb;
     const R* coef = P.coef;
@@ -334,6 +339,108 @@ collide_stream_persistent(R* fa, R* fb, const __grid_constant__ KParams<R> P, in
     }
 }
 
+
+// ------------------------------------------------------------------------------------------------ step, SM-resident
+// Grids whose ONE population copy fits in the shared memory of the whole GPU (148 x 227 KB = 33 MB; c2 in fp64 is 31 MB):
+// one cooperative launch, one block per SM; block b owns a contiguous run of tiles and keeps them in shared memory IN THE
+// GLOBAL LAYOUT (shared element = global element - shift), stepped in place with the AA pattern (even step: a node reads and
+// rewrites its own slots, swapped; odd step: it reads slot opp(i) of x - c_i and writes slot i of x + c_i -- the same slot set,
+// so no staging and no second copy).  Slot (x, s) is touched by node x on even and by node x - c_s on odd steps: when both
+// belong to the block it lives in shared memory, otherwise it STAYS IN GLOBAL MEMORY (L2) and both blocks access it there --
+// the block-boundary populations are the only per-step traffic that leaves the SM.  Steps are separated by the same
+// point-to-point flags as in collide_stream_persistent (every global-homed slot is written in one step by one block and read
+// in the next by the other).  Pointers are generic (shared or global), the arithmetic is collide_core.  Entry: the tiles are
+// copied in; exit: the shared-homed slots are copied back (the global-homed ones are already in place).
+template <class Sys, class R, bool ODD, bool MMS>
+__device__ __forceinline__ void node_step_generic(R* const (&sp)[2 * Sys::D + 1], const KParams<R>& P, const R* coef, long long node, const NodeIdx& p) {
+    constexpr int D = Sys::D, Q = 2 * D + 1, M = Sys::M;
+    R f[M][Q];
+#pragma unroll
+    for (int k = 0; k < M; ++k)
+#pragma unroll
+        for (int i = 0; i < Q; ++i) f[k][i] = sp[i][(k * Q + (ODD ? opposite(i) : i)) * TILE];
+    typename Sys::Ctx ctx;
+    load_aux<Sys, R>(ctx, P, node);
+    R smms[M];
+    if constexpr (MMS) mms_node<Sys, R, false>(P, p, coef, smms);
+    collide_core<Sys, R, MMS>(f, ctx, P, smms, [&](auto K, const R* fk) {
+        constexpr int k = decltype(K)::value;
+#pragma unroll
+        for (int i = 0; i < Q; ++i) {
+            if constexpr (ODD) sp[opposite(i)][(k * Q + i) * TILE] = fk[i];                  // slot i of x + c_i (the pull source of opp(i))
+            else sp[opposite(i)][(k * Q + opposite(i)) * TILE] = fk[i];                      // own slot opp(i)
+        }
+    });
+}
+
+template <class Sys, class R, bool MMS, int BLOCK>
+__global__ void __launch_bounds__(BLOCK, 1)
+collide_stream_resident(R* f, const __grid_constant__ KParams<R> P, int nsteps, int parity0, long long coef_stride, unsigned int* flags, int rounds) {
+    constexpr int D = Sys::D, Q = 2 * D + 1, M = Sys::M, MQ = M * Q, G = BLOCK / TILE;
+    static_assert(BLOCK % TILE == 0, "whole tiles per pass");
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    R* const sm = reinterpret_cast<R*>(smem_raw);
+    const long long ntile = (P.n + TILE - 1) / TILE;
+    const long long t0 = (long long)blockIdx.x * rounds, t1 = t0 + rounds < ntile ? t0 + rounds : ntile;
+    const long long first = t0 * TILE, last = (t1 * TILE < P.n ? t1 * TILE : P.n) - 1;
+    const long long shift = t0 * (long long)MQ * TILE;
+    int dep0, ndep;
+    dependency_run(first, last, D == 3 ? (long long)P.nx * P.ny : (long long)P.nx, (long long)rounds * TILE, P.n, dep0, ndep);
+    {
+        const long long own = (t1 - t0) * (long long)MQ * TILE;
+        for (long long e = threadIdx.x; e < own; e += BLOCK) sm[e] = f[shift + e];
+    }
+    __syncthreads();
+    const int lane = (int)threadIdx.x & (TILE - 1), grp = (int)threadIdx.x >> LOG_TILE;
+    // boundary tiles (some node has a neighbour outside the block: within one reach of either end) go first in every step, then
+    // the flag is published, then the interior tiles (shared memory only) run while the flag travels to the neighbours
+    const long long reach = D == 3 ? (long long)P.nx * P.ny : (long long)P.nx;
+    long long tb0 = (first + reach - 1) / TILE + 1, tb1 = (last - reach + 1) / TILE;
+    if (tb0 > t1) tb0 = t1;
+    if (last - reach + 1 < first || tb1 < tb0) tb1 = tb0;
+    if (dep0 == 0 && ndep == (int)gridDim.x && gridDim.x == 1) { tb0 = t0; tb1 = t1; }        // a single block has no boundary
+    const long long nlo = tb0 - t0, nbd = nlo + (t1 - tb1);
+    auto tile_step = [&](long long t, bool odd, const R* coef) {
+        const long long node = t * TILE + lane;
+        if (node < P.n) {
+            const NodeIdx p = decompose(node, P.nx, P.ny);
+            R* sp[Q];
+#pragma unroll
+            for (int i = 0; i < Q; ++i) {
+                const long long sn = node + pull_offset(i, p, P.nx, P.ny, P.nz);
+                const long long off = tile_off(odd ? sn : node, MQ);
+                sp[i] = (sn >= first && sn <= last) ? sm + (off - shift) : f + off;
+            }
+            if (odd) node_step_generic<Sys, R, true, MMS>(sp, P, coef, node, p);
+            else node_step_generic<Sys, R, false, MMS>(sp, P, coef, node, p);
+        }
+    };
+    const R* coef = P.coef;
+    for (int s = 0; s < nsteps; ++s) {
+        const bool odd = ((parity0 + s) & 1) != 0;
+        if (s > 0) flags_wait(flags, dep0, ndep, (int)gridDim.x, (unsigned)s);      // the neighbours' boundary tiles of step s-1 are done
+        for (long long j = grp; j < nbd; j += G) tile_step(j < nlo ? t0 + j : tb1 + (j - nlo), odd, coef);
+        if (s + 1 < nsteps) flags_publish(flags + (size_t)blockIdx.x * FLAG_STRIDE, (unsigned)(s + 1));
+        for (long long t = tb0 + grp; t < tb1; t += G) tile_step(t, odd, coef);
+        coef += coef_stride;
+    }
+    __syncthreads();
+    for (long long t = t0 + grp; t < t1; t += G) {
+        const long long node = t * TILE + lane;
+        if (node < P.n) {
+            const NodeIdx p = decompose(node, P.nx, P.ny);
+            const long long off = tile_off(node, MQ);
+#pragma unroll
+            for (int i = 0; i < Q; ++i) {
+                const long long sn = node + pull_offset(i, p, P.nx, P.ny, P.nz);
+                if (sn >= first && sn <= last) {
+#pragma unroll
+                    for (int k = 0; k < M; ++k) f[off + (k * Q + i) * TILE] = sm[off - shift + (k * Q + i) * TILE];
+                }
+            }
+        }
+    }
+}
 
 // ------------------------------------------------------------------------------------------------ step, cluster-resident
 // Grids of a few thousand nodes (configs[0]: 64 x 64) do not even fill L2 lines worth a barrier through L2: ONE thread-block

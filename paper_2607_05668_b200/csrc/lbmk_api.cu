@@ -318,7 +318,7 @@ static void derive_params(lbmk_grid* g) {
 
 static void resolve_options(lbmk_grid* g) {
     GridCore& c = g->c;
-    c.pattern = g->opt_pattern == LBMK_PATTERN_AUTO ? PATTERN_PULL2 : (int)g->opt_pattern;
+    c.pattern = g->opt_pattern == LBMK_PATTERN_AUTO ? (g->opt_stepping == LBMK_STEPPING_RESIDENT ? PATTERN_AA : PATTERN_PULL2) : (int)g->opt_pattern;
     if (c.bc == LBMK_DIRICHLET_MMS) c.pattern = PATTERN_PULL2;      // the frame refill needs canonical storage
     c.kernel = g->opt_kernel == LBMK_KERNEL_AUTO ? KERNEL_NODE : (int)g->opt_kernel;
     c.collision = g->sys.collision != LBMK_COLLISION_BGK ? 1 : 0;          // TRT and regularised share the two-rate kernel
@@ -333,7 +333,11 @@ static void resolve_options(lbmk_grid* g) {
     if (g->opt_stepping == LBMK_STEPPING_AUTO)
         c.stepping = (cl && g->ops->linear) ? STEPPING_CLUSTER : (can && state2 <= (size_t(96) << 20)) ? STEPPING_PERSISTENT : STEPPING_LAUNCH;
     else if (g->opt_stepping == LBMK_STEPPING_CLUSTER) c.stepping = cl ? STEPPING_CLUSTER : (can ? STEPPING_PERSISTENT : STEPPING_LAUNCH);
-    else c.stepping = (g->opt_stepping == LBMK_STEPPING_PERSISTENT && can) ? STEPPING_PERSISTENT : STEPPING_LAUNCH;
+    else if (g->opt_stepping == LBMK_STEPPING_RESIDENT) {
+        // one population copy in the shared memory of all SMs, AA pattern; grids that do not qualify step as they would have otherwise
+        const bool res = c.pattern == PATTERN_AA && c.kernel == KERNEL_NODE && c.bc == LBMK_PERIODIC && !c.Pd.ghost && c.collision == 0 && (c.num_sms <= 0 || g->ops->resident_supported(c));   // SM count known at bind
+        c.stepping = res ? STEPPING_RESIDENT : (can && state2 <= (size_t(96) << 20)) ? STEPPING_PERSISTENT : STEPPING_LAUNCH;
+    } else c.stepping = (g->opt_stepping == LBMK_STEPPING_PERSISTENT && can) ? STEPPING_PERSISTENT : STEPPING_LAUNCH;
 }
 
 static void layout(lbmk_grid* g) {
@@ -418,7 +422,7 @@ lbmk_status lbmk_grid_set_option(lbmk_grid* g, lbmk_option key, long long value)
         if (value == LBMK_KERNEL_ROW) return fail(g, LBMK_EUNSUPPORTED, "LBMK_KERNEL_ROW is reserved: no staged-row kernel in this build");
         g->opt_kernel = value;
     } else if (key == LBMK_OPT_STEPPING) {
-        if (value < LBMK_STEPPING_AUTO || value > LBMK_STEPPING_CLUSTER) return fail(g, LBMK_EINVAL, "unknown stepping mode");
+        if (value < LBMK_STEPPING_AUTO || value > LBMK_STEPPING_RESIDENT) return fail(g, LBMK_EINVAL, "unknown stepping mode");
         g->opt_stepping = value;
     } else {
         return fail(g, LBMK_EINVAL, "unknown option");
@@ -606,6 +610,7 @@ lbmk_status lbmk_grid_bind_workspace(lbmk_grid* g, void* device_ptr, size_t byte
         CK(g, cudaGetDevice(&dev), "cudaGetDevice");
         CK(g, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev), "cudaDeviceGetAttribute");
         c.num_sms = sms;
+        if (c.stepping == STEPPING_RESIDENT && !g->ops->resident_supported(c)) c.stepping = STEPPING_LAUNCH;   // does not fit this GPU's shared memory
     }
     CK(g, g->ops->fill_tables(c), "fill_tables");
     CK(g, g->ops->reference_equilibrium(c), "reference_equilibrium");

@@ -10,7 +10,7 @@ namespace lbmk {
 enum { PREC_F64 = 0, PREC_F32 = 1 };
 enum { PATTERN_PULL2 = 1, PATTERN_AA = 2 };
 enum { KERNEL_NODE = 1, KERNEL_ROW = 2, KERNEL_TWOPASS = 3 };
-enum { STEPPING_LAUNCH = 1, STEPPING_PERSISTENT = 2, STEPPING_CLUSTER = 3 };
+enum { STEPPING_LAUNCH = 1, STEPPING_PERSISTENT = 2, STEPPING_CLUSTER = 3, STEPPING_RESIDENT = 4 };
 
 struct GridCore {
     int nx, ny, nz;
@@ -74,7 +74,8 @@ struct SysOps {
     bool (*row_kernel_supported)(const GridCore&);
     bool (*cluster_supported)(const GridCore&);
     bool has_generated;   // gen/cascade.py emits this system: lbmk_flux_selfcheck is available
-    cudaError_t (*flux_selfcheck)(GridCore&, double g_tau, double* out_host);     // the grid fits the cluster-resident kernel (kernels.cuh collide_stream_cluster)
+    cudaError_t (*flux_selfcheck)(GridCore&, double g_tau, double* out_host);
+    bool (*resident_supported)(const GridCore&);     // one population copy fits the shared memory of all SMs (kernels.cuh collide_stream_resident)
 };
 
 const SysOps* ops_advection2d();

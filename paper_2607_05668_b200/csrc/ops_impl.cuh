@@ -246,6 +246,46 @@ struct Ops {
         g.step += cnt;
         return cudaSuccess;
     }
+    // ---- SM-resident stepping: ONE population copy in the shared memory of all SMs, AA pattern in place (kernels.cuh)
+    static constexpr size_t RESIDENT_SMEM_MAX = 227 * 1024;
+    template <class R> struct TuneR { static constexpr int BLOCK = (size_t)M * Q * sizeof(R) <= 160 ? 512 : 256; };
+    template <class R>
+    static int resident_rounds(const GridCore& g) {         // tiles per block, or 0 if the grid does not fit
+        if (g.num_sms <= 0) return 0;
+        const long long ntile = (g.n + TILE - 1) / TILE;
+        const long long rounds = (ntile + g.num_sms - 1) / g.num_sms;
+        const size_t smem = (size_t)rounds * M * Q * TILE * sizeof(R);
+        return (smem <= RESIDENT_SMEM_MAX && rounds <= INT_MAX) ? (int)rounds : 0;
+    }
+    static bool resident_supported(const GridCore& g) { return (g.prec == PREC_F64 ? resident_rounds<double>(g) : resident_rounds<float>(g)) > 0; }
+    template <class R, bool MMS>
+    static cudaError_t launch_resident(GridCore& g, int cnt, long long coef_stride) {
+        constexpr int BLOCK = TuneR<R>::BLOCK;
+        int rounds = resident_rounds<R>(g);
+        if (rounds <= 0) return cudaErrorLaunchOutOfResources;
+        const long long ntile = (g.n + TILE - 1) / TILE;
+        const int grid = (int)((ntile + rounds - 1) / rounds);
+        const size_t smem = (size_t)rounds * M * Q * TILE * sizeof(R);
+        auto kern = collide_stream_resident<S<R>, R, MMS, BLOCK>;
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        e = cudaMemsetAsync(g.bar, 0, (size_t)grid * FLAG_STRIDE * sizeof(unsigned int), g.stream);
+        if (e != cudaSuccess) return e;
+        R* f = (R*)g.f[0];
+        KParams<R> P = kp<R>(g);
+        int parity0 = (int)(g.step & 1);
+        unsigned int* bar = g.bar;
+        void* args[] = {&f, &P, &cnt, &parity0, &coef_stride, &bar, &rounds};
+        e = cudaLaunchCooperativeKernel((const void*)kern, dim3(grid), dim3(BLOCK), args, smem, g.stream);
+        if (e != cudaSuccess) return e;
+        g.launches++;
+        g.persistent_launches++;
+        g.step += cnt;
+        return cudaSuccess;
+    }
+    static bool use_resident(const GridCore& g, int n_steps) {
+        return g.stepping == STEPPING_RESIDENT && g.pattern == PATTERN_AA && g.kernel == KERNEL_NODE && g.bc == 0 && g.collision == 0 && n_steps >= 2;
+    }
     // ---- cluster-resident stepping for tiny grids: state in distributed shared memory of one cluster (kernels.cuh)
     static constexpr int CLUSTER = 8;
     template <class R>
@@ -318,6 +358,15 @@ struct Ops {
     template <class R, bool MMS>
     static cudaError_t step_t(GridCore& g, int n_steps) {
         if constexpr (!MMS) {
+            if (use_resident(g, n_steps)) {
+                for (int done = 0; done < n_steps;) {
+                    const int cnt = std::min(n_steps - done, 1 << 16);
+                    cudaError_t e = launch_resident<R, false>(g, cnt, 0);
+                    if (e != cudaSuccess) return e;
+                    done += cnt;
+                }
+                return cudaGetLastError();
+            }
             if (use_persistent(g, n_steps)) {
                 if (g.stepping == STEPPING_CLUSTER) return launch_cluster<R>(g, n_steps, cluster_npc<R>(g));
                 for (int done = 0; done < n_steps;) {
@@ -352,7 +401,11 @@ struct Ops {
                 }
                 e = cudaStreamWaitEvent(g.stream, g.ev_coef[buf], 0);
                 if (e != cudaSuccess) return e;
-                if (use_persistent(g, cnt)) {          // the whole batch of steps in one cooperative launch
+                if (use_resident(g, cnt)) {
+                    kp<R>(g).coef = (const R*)g.coef + (size_t)buf * B * rows * C::NC;
+                    e = launch_resident<R, true>(g, cnt, rows * C::NC);
+                    if (e != cudaSuccess) return e;
+                } else if (use_persistent(g, cnt)) {          // the whole batch of steps in one cooperative launch
                     kp<R>(g).coef = (const R*)g.coef + (size_t)buf * B * rows * C::NC;
                     e = launch_persistent<R, true>(g, cnt, rows * C::NC);
                     if (e != cudaSuccess) return e;
@@ -495,7 +548,7 @@ struct Ops {
     static const SysOps* get() {
         static const SysOps ops = {Sd::ID, D, M, Sd::MC, HAS_MMS, C::NT, {C::NX, C::NY, C::NZ}, C::NC, NA, IsLinear<Sd>::value,
                                    &fill_tables, &reference_equilibrium, &init_from_U, &set_f, &step, &step_ranges, &set_aux,
-                                   &read_U_with_frame, &read_f, &max_wave_speed, &error_norms, &row_supported, &cluster_supported, HAS_GEN, &flux_selfcheck};
+                                   &read_U_with_frame, &read_f, &max_wave_speed, &error_norms, &row_supported, &cluster_supported, HAS_GEN, &flux_selfcheck, &resident_supported};
         return &ops;
     }
 };

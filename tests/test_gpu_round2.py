@@ -94,6 +94,48 @@ def test_persistent_stepping_is_bit_identical_to_per_launch(P, mk, kw, steps, ch
         assert mode3 == "persistent" and np.array_equal(f1, f3)     # does not qualify: falls back
 
 
+RESIDENT = PERSIST + [
+    (W.c2_swe, dict(n=512, ny=40), 33, [1, 32]),                    # 160 tiles over 148 SMs: 2 tiles per block, every tile a boundary tile
+    (W.c2_swe, dict(n=200, ny=301), 21, [2, 19]),                   # 60 200 nodes: tiles straddle rows, ragged last tile, interior tiles exist
+    (W.hcnsf3d, dict(n=20, ny=18, nz=16), 12, [5, 7]),              # 3D, prescribed fields, reach = nx*ny
+    (W.c4_nsf3d, dict(n=24, ny=20, nz=18), 9, None),                # 3D, 17 fields, forcing on
+]
+
+
+@pytest.mark.parametrize("mk,kw,steps,chunks", RESIDENT)
+def test_sm_resident_stepping_is_bit_identical_to_aa_per_launch(P, mk, kw, steps, chunks):
+    """LBMK_STEPPING_RESIDENT: every block keeps its tiles in shared memory (global layout, AA pattern in place), only block-boundary
+    populations stay in global memory, neighbouring blocks synchronised by step flags.  The arithmetic is collide_core: the
+    populations agree bit for bit with the per-launch AA path -- odd and even step counts, calls starting at either AA parity."""
+    w = mk(**kw)
+    U1, f1, (mode1, l1) = gpu_run(P, w, steps, chunks, pattern="aa", stepping="launch")
+    U2, f2, (mode2, l2) = gpu_run(P, w, steps, chunks, stepping="resident")
+    assert mode1 == "launch" and mode2 == "resident"
+    if w.mms_id and w.system in ("nsf3d", "nsf2d", "inse2d", "mhd2d"):
+        # >= 48 row coefficients: the per-launch kernel may read them from its shared-memory copy, the resident kernel reads global
+        # memory -- two instantiations of the forcing polynomial, equal to rounding
+        d = np.abs(f2 - f1).max() / np.abs(f1).max()
+        assert d <= (1e-6 if w.precision == "f32s" else 1e-13), d
+    else:
+        assert np.array_equal(f1, f2) and np.array_equal(U1, U2)
+    assert l2 < l1
+    Uo, fo = oracle_run(w, steps)
+    gate(U2, Uo, fo, w.precision, f"{w.name}[resident]", U_ref=w.U_ref, steps=steps, strict=False)
+
+
+def test_sm_resident_stepping_falls_back_when_the_grid_does_not_fit(P):
+    w = W.c3_euler(n=1024, precision="f32s")                        # 1M nodes x 80 B = 84 MB: more than all shared memory together
+    g = P.Grid.from_workload(w, stepping="resident")
+    assert g.pattern == "aa" and g.stepping == "launch"
+    g.close()
+    g = P.Grid.from_workload(W.c2_swe(), stepping="resident")       # configs[1]: 31 MB, 14 tiles (215 KB) per SM
+    assert (g.pattern, g.stepping) == ("aa", "resident")
+    g.close()
+    g = P.Grid.from_workload(W.c2_swe(n=64), stepping="resident", pattern="pull2")    # an explicit two-lattice pattern wins
+    assert (g.pattern, g.stepping) == ("pull2", "persistent")
+    g.close()
+
+
 def test_persistent_is_the_default_for_l2_resident_grids_only(P):
     tiny = P.Grid.from_workload(W.c1_advection())                   # configs[0]: 4096 nodes, no forcing -> one cluster, DSMEM-resident
     assert tiny.stepping == "cluster"

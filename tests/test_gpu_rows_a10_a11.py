@@ -154,10 +154,10 @@ def test_degenerate_grids_parity(P, name, kw, pattern):
 @pytest.mark.parametrize("mk,kw", [(W.c1_advection, dict(n=37, ny=23)), (W.c4_nsf3d, dict(n=5, ny=4, nz=3)), (W.c4_nsf3d, dict(n=130, ny=3, nz=2)),
                                    (W.c5_mhd3d, dict(n=9, ny=2, nz=5)), (W.c2_swe, dict(n=257, ny=3)), (W.pin_nsf2d, dict(n=19)),
                                    (W.pin_swe, dict(n=21)), (W.hcnsf3d, dict(n=7, ny=5, nz=3)), (W.pin_mhd2d, dict(n=13))])
-@pytest.mark.parametrize("pattern,stepping", [("pull2", "launch"), ("aa", "launch"), ("pull2", "persistent"), ("pull2", "cluster")])
+@pytest.mark.parametrize("pattern,stepping", [("pull2", "launch"), ("aa", "launch"), ("pull2", "persistent"), ("pull2", "cluster"), ("aa", "resident")])
 def test_workspace_guards_stay_untouched(P, mk, kw, pattern, stepping):
     """The workspace is bound inside a larger buffer filled with a sentinel; after init, steps (ragged last tile, wraps
-    on every axis, forcing tables, prescribed fields; per-launch, persistent and cluster-resident stepping), reductions,
+    on every axis, forcing tables, prescribed fields; per-launch, persistent, cluster-resident and SM-resident stepping), reductions,
     readbacks and the flux self-check the guard bands before and after it are unchanged (compute-sanitizer is closed on this pool)."""
     import torch
     w = mk(**kw)
