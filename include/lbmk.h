@@ -23,7 +23,9 @@
  *     lbmk_grid_workspace_bytes(), allocate, hand it over with lbmk_grid_bind_workspace().  The library
  *     never frees it.  Arrays passed to init/read calls are borrowed for the duration of the call.
  *   - "on_device" arguments say whether a data pointer is a DEVICE pointer (non-zero) or a HOST pointer
- *     (zero).  Host transfers are staged through a transient stream-ordered device allocation.
+ *     (zero).  Host U arrays (lbmk_init_from_U, lbmk_read_U) move in node chunks through two fixed ~32 MB stream-ordered staging
+ *     buffers, the copy of one chunk overlapping the kernel on the other (pinned host memory makes the copies asynchronous);
+ *     the other host transfers are staged through a transient stream-ordered device allocation of their own size.
  *   - All work is enqueued on the cudaStream_t given to lbmk_grid_create (passed as void*; NULL = the
  *     legacy default stream).  lbmk_step is asynchronous; calls that return data to the host synchronise
  *     that stream.

@@ -611,14 +611,15 @@ collide_stream_twopass(typename StepPtr<R, MODE>::Src src, typename StepPtr<R, M
 // ------------------------------------------------------------------------------------------------ init
 // step 0: f*_k,i = w_i (dQ_k + c_i . dF_k / c_s^2),  dQ = U - Q0 (subtracted in fp64), eq 2.23
 template <class Sys, class R>
-__global__ void init_from_U_kernel(const double* __restrict__ U, R* __restrict__ f, const __grid_constant__ KParams<R> P,
-                                   const __grid_constant__ KParams<double> Pd) {
+__global__ void init_from_U_kernel(const double* __restrict__ U, long long ustride, long long node0, long long node1, R* __restrict__ f,
+                                   const __grid_constant__ KParams<R> P, const __grid_constant__ KParams<double> Pd) {
+    // nodes [node0, node1); U holds that node range, component planes `ustride` apart (the whole grid: 0, n, n)
     constexpr int D = Sys::D, Q = 2 * D + 1, M = Sys::M;
-    const long long node = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (node >= P.n) return;
+    const long long node = node0 + (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (node >= node1) return;
     R dQ[M];
 #pragma unroll
-    for (int k = 0; k < M; ++k) dQ[k] = (R)(U[(long long)k * P.n + node] - Pd.ref[k]);
+    for (int k = 0; k < M; ++k) dQ[k] = (R)(U[(long long)k * ustride + (node - node0)] - Pd.ref[k]);
     typename Sys::Ctx ctx;
     load_aux<Sys, R>(ctx, P, node);
     Sys::setup(ctx, dQ, P);
@@ -677,16 +678,17 @@ __device__ __forceinline__ R load_canonical(const R* __restrict__ f, int M, int 
 
 // U_k = Q0_k + sum_i f*_k,i, accumulated and returned in fp64 (eq 2.6; reading A17)
 template <int Q, class R>
-__global__ void read_U_kernel(const R* __restrict__ f, double* __restrict__ U, int M, int nx, int ny, int nz, long long n,
-                              int gather, const __grid_constant__ KParams<double> Pd) {
-    const long long node = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (node >= n) return;
+__global__ void read_U_kernel(const R* __restrict__ f, double* __restrict__ U, long long ustride, long long node0, long long node1, int M,
+                              int nx, int ny, int nz, int gather, const __grid_constant__ KParams<double> Pd) {
+    // nodes [node0, node1) into U, component planes `ustride` apart (the whole grid: n, 0, n)
+    const long long node = node0 + (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (node >= node1) return;
     const NodeIdx p = decompose(node, nx, ny);
     for (int k = 0; k < M; ++k) {
         double s = 0.0;
 #pragma unroll
         for (int i = 0; i < Q; ++i) s += (double)load_canonical<Q, R>(f, M, k, i, node, p, nx, ny, nz, gather);
-        U[(long long)k * n + node] = Pd.ref[k] + s;
+        U[(long long)k * ustride + (node - node0)] = Pd.ref[k] + s;
     }
 }
 

@@ -679,19 +679,86 @@ static lbmk_status need_inited(lbmk_grid* g) {
     return LBMK_OK;
 }
 
+// Host <-> device transfer of U [m_total][n] in NODE CHUNKS through two fixed staging buffers (2 x ~32 MB) on the auxiliary stream:
+// the copy of chunk j+1 overlaps the kernel on chunk j, and no second device copy of U is ever allocated (the 256^3 17-field
+// headline grid has a 2.3 GB fp64 U).  Each chunk is a strided 2D copy: m_total rows of `w` nodes, n apart on the host.
+static long long chunk_nodes(int M, long long n) {
+    long long c = (long long)((size_t(32) << 20) / ((size_t)M * sizeof(double))) / TILE * TILE;
+    if (c < TILE) c = TILE;
+    return c < n ? c : n;
+}
+
+static lbmk_status host_init_chunked(lbmk_grid* g, const double* U) {
+    GridCore& c = g->c;
+    const int M = g->ops->M;
+    const long long C = chunk_nodes(M, c.n);
+    double* stage = nullptr;
+    CK(g, cudaMallocAsync((void**)&stage, 2 * (size_t)M * C * sizeof(double), c.stream), "cudaMallocAsync staging");
+    cudaError_t e = cudaEventRecord(c.ev_entry, c.stream);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(c.aux, c.ev_entry, 0);
+    long long j = 0;
+    for (long long node0 = 0; node0 < c.n && e == cudaSuccess; node0 += C, ++j) {
+        const int b = (int)(j & 1);
+        const long long node1 = node0 + C < c.n ? node0 + C : c.n, w = node1 - node0;
+        double* sb = stage + (size_t)b * M * C;
+        if (j >= 2) e = cudaStreamWaitEvent(c.aux, c.ev_free[b], 0);               // the kernel on chunk j-2 has consumed this buffer
+        if (e == cudaSuccess) e = cudaMemcpy2DAsync(sb, (size_t)C * sizeof(double), U + node0, (size_t)c.n * sizeof(double), (size_t)w * sizeof(double),
+                                                    (size_t)M, cudaMemcpyHostToDevice, c.aux);
+        if (e == cudaSuccess) e = cudaEventRecord(c.ev_coef[b], c.aux);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(c.stream, c.ev_coef[b], 0);
+        if (e == cudaSuccess) e = g->ops->init_range(c, sb, C, node0, node1);
+        if (e == cudaSuccess) e = cudaEventRecord(c.ev_free[b], c.stream);
+    }
+    cudaError_t e2 = cudaFreeAsync(stage, c.stream);
+    cudaError_t e3 = cudaStreamSynchronize(c.stream);                               // the host buffer is only borrowed
+    CK(g, e, "chunked init_from_U");
+    CK(g, e2, "cudaFreeAsync");
+    CK(g, e3, "cudaStreamSynchronize");
+    return LBMK_OK;
+}
+
+static lbmk_status host_read_chunked(lbmk_grid* g, double* U_out) {
+    GridCore& c = g->c;
+    const int M = g->ops->M;
+    const long long C = chunk_nodes(M, c.n);
+    CK(g, g->ops->frame_now(c), "frame refresh");
+    double* stage = nullptr;
+    CK(g, cudaMallocAsync((void**)&stage, 2 * (size_t)M * C * sizeof(double), c.stream), "cudaMallocAsync staging");
+    cudaError_t e = cudaSuccess;
+    long long j = 0;
+    for (long long node0 = 0; node0 < c.n && e == cudaSuccess; node0 += C, ++j) {
+        const int b = (int)(j & 1);
+        const long long node1 = node0 + C < c.n ? node0 + C : c.n, w = node1 - node0;
+        double* sb = stage + (size_t)b * M * C;
+        if (j >= 2) e = cudaStreamWaitEvent(c.stream, c.ev_free[b], 0);            // the copy of chunk j-2 has left this buffer
+        if (e == cudaSuccess) e = g->ops->read_range(c, sb, C, node0, node1);
+        if (e == cudaSuccess) e = cudaEventRecord(c.ev_coef[b], c.stream);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(c.aux, c.ev_coef[b], 0);
+        if (e == cudaSuccess) e = cudaMemcpy2DAsync(U_out + node0, (size_t)c.n * sizeof(double), sb, (size_t)C * sizeof(double), (size_t)w * sizeof(double),
+                                                    (size_t)M, cudaMemcpyDeviceToHost, c.aux);
+        if (e == cudaSuccess) e = cudaEventRecord(c.ev_free[b], c.aux);
+    }
+    for (int b = 0; b < 2 && b < j; ++b) { cudaError_t ew = cudaStreamWaitEvent(c.stream, c.ev_free[b], 0); if (e == cudaSuccess) e = ew; }
+    cudaError_t e2 = cudaFreeAsync(stage, c.stream);
+    cudaError_t e3 = cudaStreamSynchronize(c.stream);
+    CK(g, e, "chunked read_U");
+    CK(g, e2, "cudaFreeAsync");
+    CK(g, e3, "cudaStreamSynchronize");
+    return LBMK_OK;
+}
+
 lbmk_status lbmk_init_from_U(lbmk_grid* g, const double* U, int on_device, double t0) {
     lbmk_status s = need_bound(g);
     if (s != LBMK_OK) return s;
     if (!U) return fail(g, LBMK_EINVAL, "U is NULL");
     GridCore& c = g->c;
     if (g->ops->n_aux > 0 && !c.aux_set) return fail(g, LBMK_ESTATE, "this system has prescribed coefficient fields: call lbmk_set_aux_fields first");
-    const size_t bytes = (size_t)g->ops->M * c.n * sizeof(double);
-    Staging st;
-    CK(g, st.acquire(U, on_device, bytes, true, c.stream), "stage U");
     c.step = 0; c.t0 = t0; c.cur = 0;
-    CK(g, g->ops->init_from_U(c, (const double*)st.dev), "init_from_U kernel");
-    CK(g, st.release(), "cudaFreeAsync");
-    if (!on_device) CK(g, cudaStreamSynchronize(c.stream), "cudaStreamSynchronize");   // the host buffer is only borrowed
+    if (on_device) CK(g, g->ops->init_from_U(c, U), "init_from_U kernel");
+    else {
+        s = host_init_chunked(g, U);
+        if (s != LBMK_OK) return s;
+    }
     g->inited = true;
     return LBMK_OK;
 }
@@ -756,12 +823,8 @@ lbmk_status lbmk_read_U(lbmk_grid* g, double* U_out, int on_device) {
     if (s != LBMK_OK) return s;
     if (!U_out) return fail(g, LBMK_EINVAL, "U_out is NULL");
     GridCore& c = g->c;
-    const size_t bytes = (size_t)g->ops->M * c.n * sizeof(double);
-    Staging st;
-    CK(g, st.acquire(U_out, on_device, bytes, false, c.stream), "stage U_out");
-    CK(g, g->ops->read_U(c, (double*)st.dev), "read_U kernel");
-    if (!on_device) CK(g, cudaMemcpyAsync(U_out, st.dev, bytes, cudaMemcpyDeviceToHost, c.stream), "cudaMemcpyAsync D2H");
-    CK(g, st.release(), "cudaFreeAsync");
+    if (!on_device) return host_read_chunked(g, U_out);
+    CK(g, g->ops->read_U(c, U_out), "read_U kernel");
     CK(g, cudaStreamSynchronize(c.stream), "cudaStreamSynchronize");
     return LBMK_OK;
 }

@@ -75,7 +75,12 @@ struct SysOps {
     bool (*cluster_supported)(const GridCore&);
     bool has_generated;   // gen/cascade.py emits this system: lbmk_flux_selfcheck is available
     cudaError_t (*flux_selfcheck)(GridCore&, double g_tau, double* out_host);
-    bool (*resident_supported)(const GridCore&);     // one population copy fits the shared memory of all SMs (kernels.cuh collide_stream_resident)
+    bool (*resident_supported)(const GridCore&);
+    // node ranges of init_from_U / read_U (host buffers go through fixed-size staging chunks): U holds [node0, node1), planes ustride apart
+    cudaError_t (*init_range)(GridCore&, const double* U, long long ustride, long long node0, long long node1);
+    cudaError_t (*read_range)(GridCore&, double* U, long long ustride, long long node0, long long node1);
+    cudaError_t (*frame_now)(GridCore&);            // Dirichlet frame refresh before a readback
+     // one population copy fits the shared memory of all SMs (kernels.cuh collide_stream_resident)
 };
 
 const SysOps* ops_advection2d();

@@ -103,15 +103,19 @@ struct Ops {
         return cudaGetLastError();
     }
 
+    // nodes [node0, node1) from a buffer holding that range, component planes `ustride` apart; the last range ends the initialisation
     template <class R>
-    static cudaError_t init_t(GridCore& g, const double* U) {
-        init_from_U_kernel<S<R>, R><<<blocks_for(g.n, 256), 256, 0, g.stream>>>(U, (R*)g.f[0], kp<R>(g), g.Pd);
+    static cudaError_t init_t(GridCore& g, const double* U, long long ustride, long long node0, long long node1) {
+        init_from_U_kernel<S<R>, R><<<blocks_for(node1 - node0, 256), 256, 0, g.stream>>>(U, ustride, node0, node1, (R*)g.f[0], kp<R>(g), g.Pd);
         g.launches++;
         g.cur = 0;
         g.pending = 0;
         return cudaGetLastError();
     }
-    static cudaError_t init_from_U(GridCore& g, const double* U) { return g.prec == PREC_F64 ? init_t<double>(g, U) : init_t<float>(g, U); }
+    static cudaError_t init_range(GridCore& g, const double* U, long long ustride, long long node0, long long node1) {
+        return g.prec == PREC_F64 ? init_t<double>(g, U, ustride, node0, node1) : init_t<float>(g, U, ustride, node0, node1);
+    }
+    static cudaError_t init_from_U(GridCore& g, const double* U) { return init_range(g, U, g.n, 0, g.n); }
 
     template <class R>
     static cudaError_t set_f_t(GridCore& g, const double* f) {
@@ -142,12 +146,16 @@ struct Ops {
     }
 
     template <class R>
-    static cudaError_t read_U_t(GridCore& g, double* U) {
-        read_U_kernel<Q, R><<<blocks_for(g.n, 256), 256, 0, g.stream>>>((const R*)g.f[g.cur], U, M, g.nx, g.ny, g.nz, g.n, aa_odd(g), g.Pd);
+    static cudaError_t read_U_t(GridCore& g, double* U, long long ustride, long long node0, long long node1) {
+        read_U_kernel<Q, R><<<blocks_for(node1 - node0, 256), 256, 0, g.stream>>>((const R*)g.f[g.cur], U, ustride, node0, node1, M, g.nx, g.ny, g.nz,
+                                                                                  aa_odd(g), g.Pd);
         g.launches++;
         return cudaGetLastError();
     }
-    static cudaError_t read_U(GridCore& g, double* U) { return g.prec == PREC_F64 ? read_U_t<double>(g, U) : read_U_t<float>(g, U); }
+    static cudaError_t read_range(GridCore& g, double* U, long long ustride, long long node0, long long node1) {
+        return g.prec == PREC_F64 ? read_U_t<double>(g, U, ustride, node0, node1) : read_U_t<float>(g, U, ustride, node0, node1);
+    }
+    static cudaError_t read_U(GridCore& g, double* U) { return read_range(g, U, g.n, 0, g.n); }
 
     template <class R>
     static cudaError_t read_f_t(GridCore& g, double* f) {
@@ -548,7 +556,7 @@ struct Ops {
     static const SysOps* get() {
         static const SysOps ops = {Sd::ID, D, M, Sd::MC, HAS_MMS, C::NT, {C::NX, C::NY, C::NZ}, C::NC, NA, IsLinear<Sd>::value,
                                    &fill_tables, &reference_equilibrium, &init_from_U, &set_f, &step, &step_ranges, &set_aux,
-                                   &read_U_with_frame, &read_f, &max_wave_speed, &error_norms, &row_supported, &cluster_supported, HAS_GEN, &flux_selfcheck, &resident_supported};
+                                   &read_U_with_frame, &read_f, &max_wave_speed, &error_norms, &row_supported, &cluster_supported, HAS_GEN, &flux_selfcheck, &resident_supported, &init_range, &read_range, &frame_now};
         return &ops;
     }
 };

@@ -289,3 +289,22 @@ def test_multi_node_kernel_for_single_field_fp32_is_bit_identical(P):
     assert (m1, m2) == ("launch", "persistent") and np.array_equal(f1, f2)
     Uo, fo = oracle_run(w, 9)
     gate(U1, Uo, fo, "f32s", f"{w.name}[multi]", U_ref=w.U_ref, steps=9, strict=False)
+
+
+def test_host_U_moves_in_chunks_and_equals_the_device_path(P):
+    """lbmk_init_from_U / lbmk_read_U with HOST buffers go through two fixed staging buffers in node chunks (4 chunks here, the last
+    one ragged; pageable and pinned memory): same populations and same U as with device buffers."""
+    import torch
+    w = W.c4_nsf3d(n=96, ny=96, nz=97, mms=False)                    # 893 952 nodes x 17 fields: 121 MB of fp64 U, chunks of 246 656 nodes
+    U0 = w.initial_U()
+    g = P.Grid.from_workload(w); g.init_from_U(torch.from_numpy(U0).cuda()); g.step(3)
+    f_dev = g.read_populations(); U_dev = g.read_U(torch.empty(U0.shape, dtype=torch.float64, device="cuda")).cpu().numpy()
+    g.close()
+    for pinned in (False, True):
+        src = torch.from_numpy(U0).pin_memory() if pinned else torch.from_numpy(U0)
+        g = P.Grid.from_workload(w); g.init_from_U(src); g.step(3)
+        assert np.array_equal(g.read_populations(), f_dev)
+        out = torch.empty(U0.shape, dtype=torch.float64, pin_memory=pinned)
+        U_host = g.read_U(out)
+        g.close()
+        assert np.array_equal(np.asarray(U_host), U_dev)
