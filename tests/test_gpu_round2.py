@@ -308,3 +308,23 @@ def test_host_U_moves_in_chunks_and_equals_the_device_path(P):
         U_host = g.read_U(out)
         g.close()
         assert np.array_equal(np.asarray(U_host), U_dev)
+
+
+@pytest.mark.parametrize("mk,kw,steps", [
+    (W.c5_mhd3d, dict(n=40, ny=36, nz=30), 9),                       # 3D: 338 tiles, stencil reach nx*ny = 11.25 tiles -> dependency runs of ~24 blocks, cyclic wrap in z
+    (lambda **kw: W.relabel(W.c2_swe(**kw), mms_id=0), dict(n=512, ny=301), 11),   # 1204 tiles: several tiles per block, last block short
+    (W.c3_euler, dict(n=130, ny=517), 10),                           # rows straddle tiles and blocks, ragged last tile
+])
+def test_step_flags_between_neighbouring_blocks_many_blocks(P, mk, kw, steps):
+    """The launch-free kernels synchronise neighbouring blocks with point-to-point step flags (kernels.cuh dependency_run): grids with
+    hundreds of co-resident blocks, partial dependency runs, cyclic wrap and a short last block give the per-launch bits -- persistent
+    against two-lattice per-launch, SM-resident against AA per-launch."""
+    w = mk(**kw)
+    U1, f1, (m1, _) = gpu_run(P, w, steps, [1, steps - 1], pattern="pull2", stepping="launch")
+    U2, f2, (m2, _) = gpu_run(P, w, steps, [1, steps - 1], pattern="pull2", stepping="persistent")
+    assert (m1, m2) == ("launch", "persistent") and np.array_equal(f1, f2)
+    U3, f3, (m3, _) = gpu_run(P, w, steps, [1, steps - 1], pattern="aa", stepping="launch")
+    U4, f4, (m4, _) = gpu_run(P, w, steps, [1, steps - 1], stepping="resident")
+    assert (m3, m4) == ("launch", "resident") and np.array_equal(f3, f4)
+    d = np.abs(f3 - f1).max() / np.abs(f1).max()
+    assert d <= (2e-6 if w.precision == "f32s" else 1e-13), d        # AA and two-lattice kernels: same arithmetic, separately compiled
