@@ -16,7 +16,13 @@ template <> __host__ inline KParams<float>& kp<float>(GridCore& g) { return g.Pf
 
 // launch shape of the node kernel per system: threads per block, min blocks per SM (register cap)
 template <template <class> class S, class R> struct Tune { static constexpr int BLOCK = 128, MINB = 1; };
-template <class R> struct Tune<SysNsf3D, R> { static constexpr int BLOCK = 64, MINB = 6; };
+#ifndef LBMK_NSF3D_BLOCK
+#define LBMK_NSF3D_BLOCK 64
+#endif
+#ifndef LBMK_NSF3D_MINB
+#define LBMK_NSF3D_MINB 6
+#endif
+template <class R> struct Tune<SysNsf3D, R> { static constexpr int BLOCK = LBMK_NSF3D_BLOCK, MINB = LBMK_NSF3D_MINB; };
 template <> struct Tune<SysNsf3D, double> { static constexpr int BLOCK = 128, MINB = 1; };
 template <class R> struct Tune<SysMhd3D, R> { static constexpr int BLOCK = 64, MINB = 4; };
 template <class R> struct Tune<SysHcnsf3D, R> { static constexpr int BLOCK = 64, MINB = 6; };
