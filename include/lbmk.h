@@ -282,6 +282,20 @@ lbmk_status lbmk_check_subcharacteristic(lbmk_grid* g, double* out3);
  * L1 = out[0]/out[3], L2 = sqrt(out[1]/out[4]), Linf = out[2]/out[5].  Synchronises. */
 lbmk_status lbmk_error_norms(lbmk_grid* g, double* out);
 
+/* The same norms for callers that must not allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): lbmk_error_norms stages its result through a stream-ordered device allocation, this entry point calls no
+ * cudaMalloc / cudaFree / allocating routine at all.  out_device: DEVICE pointer to [m_total][6] doubles, layout as above.
+ * The work -- a Dirichlet frame refresh on bounded grids, then two kernels -- is enqueued on the grid's stream and NOT synchronised.
+ * The reduction is a fixed two-pass tree: one record [m_total][6] per 4096 consecutive nodes, records combined in index order,
+ * so the result is bit-reproducible and independent of the SM count (lbmk_error_norms accumulates with atomics; the sums of the
+ * two agree to rounding, the maxima exactly).  The records live in a static device array of LBMK_NOALLOC_SCRATCH_BYTES that
+ * every GPU that loads the library holds until exit; a grid that needs more --
+ *     ceil(nx*ny*nz / 4096) * m_total * 48 bytes   (all BASELINE.json configs fit: c4 256^3 needs 3.3 MB)
+ * -- is refused with LBMK_EINVAL and a message naming both sizes (checked before anything else about the grid's state).
+ * ALL calls on one device share that array: two such calls that may overlap on the GPU (different streams) race; serialise them. */
+#define LBMK_NOALLOC_SCRATCH_BYTES (4 * 1024 * 1024)
+lbmk_status lbmk_error_norms_noalloc(lbmk_grid* g, double* out_device);
+
 /* ---- test hooks ------------------------------------------------------------------------------------- */
 
 /* For every node x: linear index of the node whose post-collision population `dir` arrives at x, i.e.

@@ -70,6 +70,7 @@ SYMBOLS = {
     "lbmk_time": (C.c_int, [_vp, C.POINTER(C.c_longlong), _dp]),
     "lbmk_check_subcharacteristic": (C.c_int, [_vp, _dp]),
     "lbmk_error_norms": (C.c_int, [_vp, _dp]),
+    "lbmk_error_norms_noalloc": (C.c_int, [_vp, _vp]),
     "lbmk_grid_set_origin": (C.c_int, [_vp, C.c_int, C.c_int, C.c_int]),
     "lbmk_grid_set_slab": (C.c_int, [_vp, C.c_int]),
     "lbmk_halo_bytes": (C.c_int, [_vp, C.POINTER(C.c_size_t)]),
@@ -326,6 +327,14 @@ def lbmk_error_norms(grid_h, m_total: int) -> np.ndarray:
     out = np.zeros((m_total, 6))
     _check(lib().lbmk_error_norms(grid_h, out.ctypes.data_as(_dp)), grid_h)
     return out
+
+
+LBMK_NOALLOC_SCRATCH_BYTES = 4 * 1024 * 1024
+
+
+def lbmk_error_norms_noalloc(grid_h, out_device_ptr: int):
+    """[m_total][6] doubles into DEVICE memory at out_device_ptr; enqueued on the grid's stream, nothing allocated, not synchronised."""
+    _check(lib().lbmk_error_norms_noalloc(grid_h, _vp(out_device_ptr)), grid_h)
 
 
 def lbmk_stream_index_map(grid_h, direction: int, ptr: int, on_device: bool):

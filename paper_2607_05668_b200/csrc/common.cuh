@@ -12,6 +12,7 @@
 
 namespace lbmk {
 
+constexpr int NORM_RECORD_NODES = 4096;        // nodes per partial record of the two-pass error norms (kernels.cuh, lbmk_error_norms_noalloc)
 constexpr int PERSISTENT_MAX_BLOCKS = 2048;   // "steps done" flags of the persistent kernel: one per block,
 constexpr int FLAG_STRIDE = 32;              // each in its own 128-byte line (32 words apart)
 

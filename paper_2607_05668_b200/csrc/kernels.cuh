@@ -838,6 +838,71 @@ error_norms_kernel(const R* __restrict__ f, double* __restrict__ out, long long 
     }
 }
 
+// ---- the same norms without atomics, through caller-independent scratch (lbmk_error_norms_noalloc): pass 1 writes one RECORD
+// [M][6] per NORM_RECORD_NODES consecutive nodes (one block per record, fixed summation tree), pass 2 combines the records in index
+// order, so the result does not depend on the SM count or on scheduling.  Every record of [0, nrec) is fully written by pass 1:
+// nothing in the scratch has to be cleared.
+
+template <class Sys, class R>
+__global__ void __launch_bounds__(256)
+error_norm_records_kernel(const R* __restrict__ f, double* __restrict__ rec, long long n, int nx, int ny, int nz, int gather, double t,
+                          const __grid_constant__ MmsHostArgs mh, const __grid_constant__ KParams<double> Pd) {
+    if constexpr (has_mms<Sys>()) {
+        constexpr int Q = 2 * Sys::D + 1, M = Sys::M;
+        using G = typename Sys::Mms;
+        double acc[M][6];
+        for (int k = 0; k < M; ++k) for (int j = 0; j < 6; ++j) acc[k][j] = 0.0;
+        double T[8];
+        G::time_scalars(t, mh, T);
+        const long long first = (long long)blockIdx.x * NORM_RECORD_NODES;
+        const long long last = first + NORM_RECORD_NODES < n ? first + NORM_RECORD_NODES : n;
+        for (long long node = first + threadIdx.x; node < last; node += blockDim.x) {
+            const NodeIdx p = decompose(node, nx, ny);
+            double X[8], Y[8], Z[8], q[M];
+            if (Pd.ghost && is_ghost<Sys::D>(p, ny, nz)) continue;
+            G::axis_row(0, (p.ix + Pd.ox) * mh.dx, mh, X);
+            G::axis_row(1, (p.iy + Pd.oy) * mh.dx, mh, Y);
+            if (G::NZ > 0) G::axis_row(2, (p.iz + Pd.oz) * mh.dx, mh, Z);
+            G::template exact<double>(Pd.mms, T, X, Y, Z, q);
+            for (int k = 0; k < M; ++k) {
+                double s = 0.0;
+#pragma unroll
+                for (int i = 0; i < Q; ++i) s += (double)load_canonical<Q, R>(f, M, k, i, node, p, nx, ny, nz, gather);
+                const double e = fabs(Pd.ref[k] + s - q[k]), a = fabs(q[k]);
+                acc[k][0] += e; acc[k][1] += e * e; acc[k][2] = max_nan_inf(acc[k][2], e);
+                acc[k][3] += a; acc[k][4] += a * a; acc[k][5] = max_nan_inf(acc[k][5], a);
+            }
+        }
+        __shared__ double sm[8][M * 6];
+        const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+        for (int k = 0; k < M; ++k)
+            for (int j = 0; j < 6; ++j) {
+                const double v = (j == 2 || j == 5) ? warp_max(acc[k][j]) : warp_sum(acc[k][j]);
+                if (lane == 0) sm[warp][k * 6 + j] = v;
+            }
+        __syncthreads();
+        for (int q = threadIdx.x; q < M * 6; q += blockDim.x) {
+            const bool is_max = (q % 6 == 2 || q % 6 == 5);
+            double v = sm[0][q];
+            for (int w = 1; w < 8; ++w) v = is_max ? max_nan_inf(v, sm[w][q]) : v + sm[w][q];
+            rec[(long long)blockIdx.x * (M * 6) + q] = v;
+        }
+    }
+}
+
+// pass 2: out[q] = records combined in index order; one thread per (component, quantity)
+static __global__ void combine_norm_records_kernel(const double* __restrict__ rec, long long nrec, int MQ6, double* __restrict__ out) {
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= MQ6) return;
+    const bool is_max = (q % 6 == 2 || q % 6 == 5);
+    double v = rec[q];
+    for (long long r = 1; r < nrec; ++r) {
+        const double x = rec[r * MQ6 + q];
+        v = is_max ? max_nan_inf(v, x) : v + x;
+    }
+    out[q] = v;
+}
+
 // ------------------------------------------------------------------------------------------------ flux self-check
 // Every node of the current state: the hand-written delta form (Sys<double>: dF = F(Q0 + dQ) - F(Q0), s(Q0 + dQ)) against the
 // generated plain form (Gen: F(U), s(U); gen/cascade.py), in fp64.  out[0] = max over nodes and components of

@@ -9,6 +9,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 
@@ -881,6 +882,56 @@ lbmk_status lbmk_error_norms(lbmk_grid* g, double* out) {
     CK(g, cudaStreamSynchronize(c.stream), "cudaStreamSynchronize");
     CK(g, st.release(), "cudaFreeAsync");
     return LBMK_OK;
+}
+
+// ---- error norms without any allocation (lbmk.h lbmk_error_norms_noalloc)
+// The scratch of the two-pass reduction lives in this file-scope device array: LBMK_NOALLOC_SCRATCH_BYTES on every GPU that loads
+// the library, until exit.  In host code `noalloc_scratch` is only the host-side stand-in of the symbol, NOT a device address: the
+// device address is looked up once per device with cudaGetSymbolAddress, with that device current, and that pointer is what the
+// kernels get.  All calls on a device share the array (it keeps the last call's contents; pass 1 overwrites every record it will
+// read, so nothing has to be cleared), hence calls that overlap on the GPU race.
+static __device__ __align__(256) unsigned char noalloc_scratch[LBMK_NOALLOC_SCRATCH_BYTES];
+
+static constexpr int NOALLOC_MAX_DEVICES = 64;
+static std::mutex noalloc_mutex;
+static void* noalloc_ptr[NOALLOC_MAX_DEVICES] = {};
+
+static cudaError_t noalloc_scratch_address(void** out) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(noalloc_mutex);
+    if (!noalloc_ptr[dev]) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, noalloc_scratch);       // the current device's instance of the array
+        if (e != cudaSuccess) return e;
+        noalloc_ptr[dev] = p;
+    }
+    *out = noalloc_ptr[dev];
+    return cudaSuccess;
+}
+
+lbmk_status lbmk_error_norms_noalloc(lbmk_grid* g, double* out_device) {
+    if (!g) return sys_fail(LBMK_EINVAL, "grid is NULL");
+    if (!out_device) return fail(g, LBMK_EINVAL, "out_device is NULL");
+    GridCore& c = g->c;
+    if (!g->ops->has_mms || c.mms_id == 0) return fail(g, LBMK_EUNSUPPORTED, "error norms need a manufactured solution (lbmk_system_set_mms)");
+    // size first: it is a property of the grid, known before any workspace is bound
+    const long long nrec = (c.n + NORM_RECORD_NODES - 1) / NORM_RECORD_NODES;
+    const size_t need = (size_t)nrec * g->ops->M * 6 * sizeof(double);
+    if (need > (size_t)LBMK_NOALLOC_SCRATCH_BYTES) {
+        char msg[256];
+        snprintf(msg, sizeof msg, "grid too large for the static scratch of lbmk_error_norms_noalloc: %lld records of %d x 6 doubles = %zu bytes, "
+                 "the array holds %d bytes (use lbmk_error_norms)", nrec, g->ops->M, need, (int)LBMK_NOALLOC_SCRATCH_BYTES);
+        return fail(g, LBMK_EINVAL, msg);
+    }
+    lbmk_status s = need_inited(g);
+    if (s != LBMK_OK) return s;
+    void* scratch = nullptr;
+    CK(g, noalloc_scratch_address(&scratch), "cudaGetSymbolAddress(noalloc_scratch)");
+    CK(g, g->ops->error_norm_records(c, (double*)scratch, out_device), "error_norm_records kernels");
+    return LBMK_OK;                                          // asynchronous on the grid's stream, like lbmk_step
 }
 
 // ---- generated augmented systems (gen/cascade.py -> cascade_generated.cuh)

@@ -80,6 +80,8 @@ struct SysOps {
     cudaError_t (*init_range)(GridCore&, const double* U, long long ustride, long long node0, long long node1);
     cudaError_t (*read_range)(GridCore&, double* U, long long ustride, long long node0, long long node1);
     cudaError_t (*frame_now)(GridCore&);            // Dirichlet frame refresh before a readback
+    // error norms through caller-independent scratch [ceil(n / NORM_RECORD_NODES)][M][6] doubles, into out_dev [M][6]; nothing allocated
+    cudaError_t (*error_norm_records)(GridCore&, double* scratch, double* out_dev);
      // one population copy fits the shared memory of all SMs (kernels.cuh collide_stream_resident)
 };
 

@@ -528,6 +528,24 @@ struct Ops {
         if (e != cudaSuccess) return e;
         return g.prec == PREC_F64 ? norms_t<double>(g, out) : norms_t<float>(g, out);
     }
+    // the same norms through `scratch` ([nrec][M][6] doubles, nrec = ceil(n / NORM_RECORD_NODES)) into out_dev [M][6]; no atomics
+    template <class R>
+    static cudaError_t norm_records_t(GridCore& g, double* scratch, double* out_dev) {
+        const long long nrec = (g.n + NORM_RECORD_NODES - 1) / NORM_RECORD_NODES;
+        error_norm_records_kernel<Sd, R><<<(unsigned)nrec, 256, 0, g.stream>>>((const R*)g.f[g.cur], scratch, g.n, g.nx, g.ny, g.nz, aa_odd(g),
+                                                                              g.t0 + (double)g.step * g.dt, g.mh, g.Pd);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+        combine_norm_records_kernel<<<1, 128, 0, g.stream>>>(scratch, nrec, M * 6, out_dev);
+        g.launches += 2;
+        return cudaGetLastError();
+    }
+    static cudaError_t error_norm_records(GridCore& g, double* scratch, double* out_dev) {
+        if constexpr (!HAS_MMS) return cudaErrorNotSupported;
+        cudaError_t e = frame_now(g);
+        if (e != cudaSuccess) return e;
+        return g.prec == PREC_F64 ? norm_records_t<double>(g, scratch, out_dev) : norm_records_t<float>(g, scratch, out_dev);
+    }
     using Gen = typename GenOf<S>::type;
     static constexpr bool HAS_GEN = !std::is_void<Gen>::value;
     template <class R>
@@ -562,7 +580,7 @@ struct Ops {
     static const SysOps* get() {
         static const SysOps ops = {Sd::ID, D, M, Sd::MC, HAS_MMS, C::NT, {C::NX, C::NY, C::NZ}, C::NC, NA, IsLinear<Sd>::value,
                                    &fill_tables, &reference_equilibrium, &init_from_U, &set_f, &step, &step_ranges, &set_aux,
-                                   &read_U_with_frame, &read_f, &max_wave_speed, &error_norms, &row_supported, &cluster_supported, HAS_GEN, &flux_selfcheck, &resident_supported, &init_range, &read_range, &frame_now};
+                                   &read_U_with_frame, &read_f, &max_wave_speed, &error_norms, &row_supported, &cluster_supported, HAS_GEN, &flux_selfcheck, &resident_supported, &init_range, &read_range, &frame_now, &error_norm_records};
         return &ops;
     }
 };
