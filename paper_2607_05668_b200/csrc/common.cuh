@@ -12,6 +12,10 @@
 
 namespace lbmk {
 
+// Components whose populations the per-launch two-lattice kernel with forcing keeps in a shared-memory park instead of registers
+// (kernels.cuh collide_core); specialised per system in systems.cuh
+template <class Sys> struct ParkCount { static constexpr int value = 0; };
+
 constexpr int NORM_RECORD_NODES = 4096;        // nodes per partial record of the two-pass error norms (kernels.cuh, lbmk_error_norms_noalloc)
 constexpr int PERSISTENT_MAX_BLOCKS = 2048;   // "steps done" flags of the persistent kernel: one per block,
 constexpr int FLAG_STRIDE = 32;              // each in its own 128-byte line (32 words apart)

@@ -58,6 +58,14 @@ __device__ __forceinline__ void cp_async16(R* smem_dst, const R* gmem_src) {
     const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gmem_src) : "memory");
 }
+template <class R>
+__device__ __forceinline__ void cp_async4(R* smem_dst, const R* gmem_src) {
+    static_assert(sizeof(R) == 4, "4-byte copy");
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(sa), "l"(gmem_src) : "memory");
+}
+template <> __device__ __forceinline__ void cp_async4<double>(double*, const double*) {}     // never selected (PARK is fp32 only)
+__device__ __forceinline__ void cp_async_wait_1() { asm volatile("cp.async.wait_group 1;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
@@ -147,23 +155,37 @@ __device__ __forceinline__ void load_aux(typename Sys::Ctx& ctx, const KParams<R
 // a3-a6 of ONE node, in registers: moments, system algebra, equilibrium + BGK relaxation component by component; `store(K, f_k)`
 // is called with the Q post-collision populations of component k as soon as they exist (so their registers die early).
 // Shared by every step kernel -- one definition of the arithmetic, hence identical bits whatever the storage.
-template <class Sys, class R, bool MMS, bool TRT = false, class Store>
+// PARK > 0: the populations of the LAST `PARK` components are not in f[][] but in the thread's slots of a shared-memory park
+// (element (kk*Q + i)*PSTRIDE of `park`, filled by cp.async during the gather): they are read for the moment sum and again
+// right before their relaxation, so they never occupy registers across the collision of the other components.
+template <class Sys, class R, bool MMS, bool TRT = false, int PARK = 0, int PSTRIDE = 1, class Store>
 __device__ __forceinline__ void collide_core(R (&f)[Sys::M][2 * Sys::D + 1], typename Sys::Ctx& ctx, const KParams<R>& P,
-                                             const R (&smms)[Sys::M], Store&& store) {
+                                             const R (&smms)[Sys::M], const volatile R* park, Store&& store) {
     constexpr int D = Sys::D, Q = 2 * D + 1, M = Sys::M;
     R dQ[M];
 #pragma unroll
     for (int k = 0; k < M; ++k) {
-        R s = f[k][0];
+        if (PARK > 0 && k >= M - PARK) {
+            R s = park[((k - (M - PARK)) * Q) * PSTRIDE];
 #pragma unroll
-        for (int i = 1; i < Q; ++i) s += f[k][i];
-        dQ[k] = s;
+            for (int i = 1; i < Q; ++i) s += park[((k - (M - PARK)) * Q + i) * PSTRIDE];
+            dQ[k] = s;
+        } else {
+            R s = f[k][0];
+#pragma unroll
+            for (int i = 1; i < Q; ++i) s += f[k][i];
+            dQ[k] = s;
+        }
     }
     Sys::setup(ctx, dQ, P);
     static_for<0, M>([&](auto K) {
         constexpr int k = decltype(K)::value;
         R F[D], S;
         Sys::template flux<k>(ctx, dQ, P, F, S);
+        if constexpr (PARK > 0 && k >= M - PARK) {
+#pragma unroll
+            for (int i = 0; i < Q; ++i) f[k][i] = park[((k - (M - PARK)) * Q + i) * PSTRIDE];
+        }
         if constexpr (MMS) S += smms[k];
         if constexpr (TRT) relax_trt<D, R>(f[k], P.omega_p[k], P.omega[k], dQ[k], F, S);
         else relax<D, R>(f[k], P.omega[k], dQ[k], F, S);
@@ -176,10 +198,11 @@ __device__ __forceinline__ void collide_core(R (&f)[Sys::M][2 * Sys::D + 1], typ
 // coef_s = the block's shared-memory slot for its row's forcing coefficients, coef = this step's coefficient table.
 // Called by the per-launch kernel (one segment per block) and by the persistent kernel (segments in a loop): the
 // same code, hence the same bits.
-template <class Sys, class R, int MODE, bool MMS, int BLOCK, bool COHERENT, bool TRT = false, bool PEER = false>
+template <class Sys, class R, int MODE, bool MMS, int BLOCK, bool COHERENT, bool TRT = false, bool PEER = false, int PARK = 0>
 __device__ __forceinline__ void node_step(typename StepPtr<R, MODE, COHERENT>::Src src, typename StepPtr<R, MODE, COHERENT>::Dst dst,
-                                          const KParams<R>& P, const R* coef, long long first, R* coef_s) {
+                                          const KParams<R>& P, const R* coef, long long first, R* coef_s, R* park_s = nullptr) {
     constexpr int D = Sys::D, Q = 2 * D + 1, M = Sys::M;
+    static_assert(PARK == 0 || ((MODE == MODE_PULL2 || MODE == MODE_LOCAL) && !COHERENT && sizeof(R) == 4), "parked components: two-lattice fp32 per-launch kernel");
     const long long node = first + threadIdx.x;
     constexpr int NCs = MMS ? MmsNC<Sys>::value : 4;
     // kernel-uniform: a block lies inside one (y, z) row; then every segment is full (n and node0 are multiples of BLOCK)
@@ -217,9 +240,16 @@ __device__ __forceinline__ void node_step(typename StepPtr<R, MODE, COHERENT>::S
 #pragma unroll
         for (int i = 0; i < Q; ++i) {
             const int slot = (MODE == MODE_AA_ODD) ? opposite(i) : i;
+            if constexpr (PARK > 0) {
+                if (k >= M - PARK) {        // no register destination: asynchronous copy into this thread's slot of the park
+                    cp_async4(park_s + ((k - (M - PARK)) * Q + i) * BLOCK + threadIdx.x, sp[i] + (k * Q + slot) * TILE);
+                    continue;
+                }
+            }
             // persistent kernel: the line may sit stale in this SM's L1 from two steps ago -> read at L2 (ld.global.cg)
             f[k][i] = COHERENT ? __ldcg(sp[i] + (k * Q + slot) * TILE) : sp[i][(k * Q + slot) * TILE];
         }
+    if constexpr (PARK > 0) cp_async_commit();
     typename Sys::Ctx ctx;
     load_aux<Sys, R>(ctx, P, node);
     // manufactured forcing while the gather is in flight: after the row/node split it is ~250 instructions on
@@ -227,14 +257,16 @@ __device__ __forceinline__ void node_step(typename StepPtr<R, MODE, COHERENT>::S
     R smms[M];
     if constexpr (MMS) {
         if (staged) {
-            cp_async_wait_all();
+            if constexpr (PARK > 0) cp_async_wait_1();          // the coefficient group only; the parked populations stay in flight
+            else cp_async_wait_all();
             __syncthreads();
             mms_node<Sys, R, true>(P, p, coef_s, smms);
         } else {
             mms_node<Sys, R, false>(P, p, coef, smms);
         }
     }
-    collide_core<Sys, R, MMS, TRT>(f, ctx, P, smms, [&](auto K, const R* fk) {
+    if constexpr (PARK > 0) cp_async_wait_all();       // a thread reads only the slots it copied itself: no block barrier
+    collide_core<Sys, R, MMS, TRT, PARK, BLOCK>(f, ctx, P, smms, PARK > 0 ? park_s + threadIdx.x : nullptr, [&](auto K, const R* fk) {
         constexpr int k = decltype(K)::value;
 #pragma unroll
         for (int i = 0; i < Q; ++i) {
@@ -258,7 +290,9 @@ __global__ void __launch_bounds__(BLOCK, MINB)
 collide_stream_node(typename StepPtr<R, MODE>::Src src, typename StepPtr<R, MODE>::Dst dst, const __grid_constant__ KParams<R> P) {
     constexpr int NCs = MMS ? MmsNC<Sys>::value : 4;
     __shared__ __align__(16) R coef_s[NCs];
-    node_step<Sys, R, MODE, MMS, BLOCK, false, TRT, PEER>(src, dst, P, P.coef, P.node0 + (long long)blockIdx.x * BLOCK, coef_s);
+    constexpr int PARK = (MMS && !TRT && !PEER && sizeof(R) == 4 && (MODE == MODE_PULL2 || MODE == MODE_LOCAL)) ? ParkCount<Sys>::value : 0;
+    __shared__ R park_s[PARK > 0 ? PARK * (2 * Sys::D + 1) * BLOCK : 1];
+    node_step<Sys, R, MODE, MMS, BLOCK, false, TRT, PEER, PARK>(src, dst, P, P.coef, P.node0 + (long long)blockIdx.x * BLOCK, coef_s, park_s);
 }
 
 // ------------------------------------------------------------------------------------------------ step, persistent
@@ -363,7 +397,7 @@ __device__ __forceinline__ void node_step_generic(R* const (&sp)[2 * Sys::D + 1]
     load_aux<Sys, R>(ctx, P, node);
     R smms[M];
     if constexpr (MMS) mms_node<Sys, R, false>(P, p, coef, smms);
-    collide_core<Sys, R, MMS>(f, ctx, P, smms, [&](auto K, const R* fk) {
+    collide_core<Sys, R, MMS>(f, ctx, P, smms, nullptr, [&](auto K, const R* fk) {
         constexpr int k = decltype(K)::value;
 #pragma unroll
         for (int i = 0; i < Q; ++i) {
@@ -493,7 +527,7 @@ collide_stream_cluster(const R* __restrict__ gsrc, R* __restrict__ gdst, const _
             const bool last = s == nsteps - 1;
             R* const wr = sm + (s & 1) * bufsz + threadIdx.x;
             R* const gp = gdst + tile_off(node, M * Q);
-            collide_core<Sys, R, false>(f, ctx, P, smms, [&](auto K, const R* fk) {
+            collide_core<Sys, R, false>(f, ctx, P, smms, nullptr, [&](auto K, const R* fk) {
                 constexpr int k = decltype(K)::value;
 #pragma unroll
                 for (int i = 0; i < Q; ++i) {
@@ -538,7 +572,7 @@ collide_stream_multi(typename StepPtr<R, MODE>::Src src, typename StepPtr<R, MOD
         if (node < P.node1) {
             typename Sys::Ctx ctx;
             R* const dp = dst + tile_off(node, M * Q);
-            collide_core<Sys, R, false>(f[j], ctx, P, smms, [&](auto K, const R* fk) {
+            collide_core<Sys, R, false>(f[j], ctx, P, smms, nullptr, [&](auto K, const R* fk) {
                 constexpr int k = decltype(K)::value;
 #pragma unroll
                 for (int i = 0; i < Q; ++i) dp[(k * Q + i) * TILE] = fk[i];

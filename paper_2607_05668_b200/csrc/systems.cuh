@@ -811,6 +811,13 @@ template <class R> struct SysMhd2D {
 // ------------------------------------------------------------------------------------------ generated counterparts
 // The plain lattice flux/source that gen/cascade.py DERIVES (Alg 2.1 Split/Cascade/Assemble/Emit) for the same system, where one
 // is emitted: what lbmk_flux_selfcheck compares the hand-written delta form against.
+// c4 with forcing: the populations of the last tracker component wait in shared memory (cp.async) instead of registers -- measured
+// 2.42 ms/step against 2.46 (two components: 2.46, three: 2.47)
+#ifndef LBMK_NSF3D_PARK
+#define LBMK_NSF3D_PARK 1
+#endif
+template <> struct ParkCount<SysNsf3D<float>> { static constexpr int value = LBMK_NSF3D_PARK; };
+
 template <template <class> class S> struct GenOf { using type = void; };
 template <> struct GenOf<SysEuler2D> { using type = Gen_euler2d; };
 template <> struct GenOf<SysSwe2DBathy> { using type = Gen_swe2d_bathy; };
