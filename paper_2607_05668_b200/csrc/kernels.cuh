@@ -374,6 +374,53 @@ collide_stream_persistent(R* fa, R* fb, const __grid_constant__ KParams<R> P, in
 }
 
 
+// The same stepping with FAT blocks: GROUPS x BLOCK threads, one block per SM, each group of BLOCK threads takes whole segments.
+// A block then owns enough rows to have an INTERIOR (segments further than one stencil reach from both ends of its range, which
+// touch no other block's nodes): per step it waits for its neighbours' flags, updates its boundary segments, publishes its own
+// flag and only then updates the interior -- the flag's round trip through L2 is hidden behind the interior work.  flag[b] = s+1
+// now means "block b has finished the BOUNDARY segments of step s", which is all its neighbours depend on (they read and, one
+// step later, their reads of b's nodes are what b's next writes must not overtake: both happen in their boundary phase).
+// Only without shared-memory staging of the row coefficients (node_step's staging is per block); same node_step, same bits.
+template <class Sys, class R, bool MMS, int BLOCK, int GROUPS>
+__global__ void __launch_bounds__(BLOCK * GROUPS, 1)
+collide_stream_persistent_fat(R* fa, R* fb, const __grid_constant__ KParams<R> P, int nsteps, int first_local, long long coef_stride,
+                              unsigned int* flags, int rounds) {
+    static_assert(!(MMS && MmsNC<Sys>::value >= STAGE_MIN_NC), "fat blocks: unstaged row coefficients only");
+    const long long nseg = (P.n + BLOCK - 1) / BLOCK;
+    const long long seg0 = (long long)blockIdx.x * rounds, seg1 = seg0 + rounds < nseg ? seg0 + rounds : nseg;
+    const long long first = seg0 * BLOCK, last = (seg1 * BLOCK < P.n ? seg1 * BLOCK : P.n) - 1;
+    const long long reach = Sys::D == 3 ? (long long)P.nx * P.ny : (long long)P.nx;
+    int dep0, ndep;
+    dependency_run(first, last, reach, (long long)rounds * BLOCK, P.n, dep0, ndep);
+    // interior segments [sb0, sb1): every node in [first + reach, last - reach]
+    long long sb0 = (first + reach + BLOCK - 1) / BLOCK, sb1 = (last - reach + 1) / BLOCK;
+    if (sb0 > seg1) sb0 = seg1;
+    if (last - reach + 1 < first || sb1 < sb0) sb1 = sb0;
+    if (gridDim.x == 1) { sb0 = seg0; sb1 = seg1; }                      // a single block has no boundary
+    const long long nlo = sb0 - seg0, nbd = nlo + (seg1 - sb1);
+    const int grp = (int)threadIdx.x / BLOCK;
+    const long long goff = (long long)grp * BLOCK;                          // node_step adds threadIdx.x to `first`
+    R* src = fa;
+    R* dst = fb;
+    const R* coef = P.coef;
+    for (int s = 0; s < nsteps; ++s) {
+        if (s > 0) flags_wait(flags, dep0, ndep, (int)gridDim.x, (unsigned)s);
+        const bool local = s == 0 && first_local;
+        for (long long j = grp; j < nbd; j += GROUPS) {
+            const long long seg = j < nlo ? seg0 + j : sb1 + (j - nlo);
+            if (local) node_step<Sys, R, MODE_LOCAL, MMS, BLOCK, true>(src, dst, P, coef, seg * BLOCK - goff, nullptr);
+            else node_step<Sys, R, MODE_PULL2, MMS, BLOCK, true>(src, dst, P, coef, seg * BLOCK - goff, nullptr);
+        }
+        if (s + 1 < nsteps) flags_publish(flags + (size_t)blockIdx.x * FLAG_STRIDE, (unsigned)(s + 1));
+        for (long long seg = sb0 + grp; seg < sb1; seg += GROUPS) {
+            if (local) node_step<Sys, R, MODE_LOCAL, MMS, BLOCK, true>(src, dst, P, coef, seg * BLOCK - goff, nullptr);
+            else node_step<Sys, R, MODE_PULL2, MMS, BLOCK, true>(src, dst, P, coef, seg * BLOCK - goff, nullptr);
+        }
+        R* t = src; src = dst; dst = t;
+        coef += coef_stride;
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ step, SM-resident
 // Grids whose ONE population copy fits in the shared memory of the whole GPU (148 x 227 KB = 33 MB; c2 in fp64 is 31 MB):
 // one cooperative launch, one block per SM; block b owns a contiguous run of tiles and keeps them in shared memory IN THE

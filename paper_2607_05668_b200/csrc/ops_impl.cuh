@@ -237,11 +237,35 @@ struct Ops {
         if (rounds_out) *rounds_out = (int)rounds;
         return (int)((nseg + rounds - 1) / rounds);               // balanced: every block owns `rounds` consecutive segments (the last one fewer)
     }
+    // fat blocks (kernels.cuh collide_stream_persistent_fat): 4 x 128 threads, one block per SM, when every block then owns at least
+    // FAT_MIN_ROUNDS segments (so that it has an interior to hide the flag round trip behind) and the coefficients are unstaged
+    static constexpr int FAT_GROUPS = 4, FAT_MIN_ROUNDS = 8;
+    template <class R, bool MMS>
+    static constexpr bool fat_capable() {      // <= 160 B of populations per node: fits the 128 registers of a 512-thread block without spilling
+        return TuneP<S, R>::BLOCK == 128 && !(MMS && C::NC >= STAGE_MIN_NC) && (size_t)M * Q * sizeof(R) <= 160;
+    }
+    template <class R, bool MMS>
+    static int persistent_fat_grid(GridCore& g, int* rounds_out) {
+        if constexpr (fat_capable<R, MMS>()) {
+            constexpr int BLOCK = 128;
+            int per_sm = 0;
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, collide_stream_persistent_fat<S<R>, R, MMS, BLOCK, FAT_GROUPS>, BLOCK * FAT_GROUPS, 0) != cudaSuccess) return 0;
+            const long long cap = std::min<long long>((long long)(per_sm > 0 ? 1 : 0) * g.num_sms, PERSISTENT_MAX_BLOCKS), nseg = (g.n + BLOCK - 1) / BLOCK;
+            if (cap <= 0) return 0;
+            const long long rounds = (nseg + cap - 1) / cap;
+            if (rounds < FAT_MIN_ROUNDS || rounds > INT_MAX) return 0;
+            *rounds_out = (int)rounds;
+            return (int)((nseg + rounds - 1) / rounds);
+        }
+        return 0;
+    }
     template <class R, bool MMS>
     static cudaError_t launch_persistent(GridCore& g, int cnt, long long coef_stride) {
         constexpr int BLOCK = TuneP<S, R>::BLOCK, MINB = TuneP<S, R>::MINB;
         int rounds = 0;
-        const int grid = persistent_grid<R, MMS>(g, &rounds);
+        bool fat = true;
+        int grid = persistent_fat_grid<R, MMS>(g, &rounds);
+        if (grid <= 0) { fat = false; grid = persistent_grid<R, MMS>(g, &rounds); }
         if (grid <= 0) return cudaErrorLaunchOutOfResources;
         cudaError_t e = cudaMemsetAsync(g.bar, 0, (size_t)grid * FLAG_STRIDE * sizeof(unsigned int), g.stream);     // one "steps done" flag per block
         if (e != cudaSuccess) return e;
@@ -251,7 +275,10 @@ struct Ops {
         int first_local = g.pending ? 0 : 1;
         unsigned int* bar = g.bar;
         void* args[] = {&fa, &fb, &P, &cnt, &first_local, &coef_stride, &bar, &rounds};
-        e = cudaLaunchCooperativeKernel((const void*)collide_stream_persistent<S<R>, R, MMS, BLOCK, MINB>, dim3(grid), dim3(BLOCK), args, 0, g.stream);
+        if constexpr (fat_capable<R, MMS>()) {
+            if (fat) e = cudaLaunchCooperativeKernel((const void*)collide_stream_persistent_fat<S<R>, R, MMS, 128, FAT_GROUPS>, dim3(grid), dim3(128 * FAT_GROUPS), args, 0, g.stream);
+        }
+        if (!fat) e = cudaLaunchCooperativeKernel((const void*)collide_stream_persistent<S<R>, R, MMS, BLOCK, MINB>, dim3(grid), dim3(BLOCK), args, 0, g.stream);
         if (e != cudaSuccess) return e;
         g.launches++;
         g.persistent_launches++;

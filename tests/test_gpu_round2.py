@@ -314,11 +314,15 @@ def test_host_U_moves_in_chunks_and_equals_the_device_path(P):
     (W.c5_mhd3d, dict(n=40, ny=36, nz=30), 9),                       # 3D: 338 tiles, stencil reach nx*ny = 11.25 tiles -> dependency runs of ~24 blocks, cyclic wrap in z
     (lambda **kw: W.relabel(W.c2_swe(**kw), mms_id=0), dict(n=512, ny=301), 11),   # 1204 tiles: several tiles per block, last block short
     (W.c3_euler, dict(n=130, ny=517), 10),                           # rows straddle tiles and blocks, ragged last tile
+    (W.c2_swe, dict(n=512, ny=300), 13),                             # forcing on, >= 8 segments per SM: FAT persistent blocks (boundary segments first)
+    (W.c2_swe, dict(n=64, ny=2401), 12),                             # narrow rows: reach = half a segment, nearly all segments interior; ragged
+    (W.c3_euler, dict(n=1000, ny=160), 8),                           # fp32, reach = 7.8 segments of the 9 a block owns: no interior
 ])
 def test_step_flags_between_neighbouring_blocks_many_blocks(P, mk, kw, steps):
     """The launch-free kernels synchronise neighbouring blocks with point-to-point step flags (kernels.cuh dependency_run): grids with
     hundreds of co-resident blocks, partial dependency runs, cyclic wrap and a short last block give the per-launch bits -- persistent
-    against two-lattice per-launch, SM-resident against AA per-launch."""
+    (thin 128-thread blocks, and from 8 segments per SM on the fat 512-thread blocks that publish their flag after the boundary
+    segments and hide its round trip behind the interior ones) against two-lattice per-launch, SM-resident against AA per-launch."""
     w = mk(**kw)
     U1, f1, (m1, _) = gpu_run(P, w, steps, [1, steps - 1], pattern="pull2", stepping="launch")
     U2, f2, (m2, _) = gpu_run(P, w, steps, [1, steps - 1], pattern="pull2", stepping="persistent")
