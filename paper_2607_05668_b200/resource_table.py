@@ -29,7 +29,8 @@ HEADLINE = [  # (label, unit, regex on the demangled-ish mangled name)
     ("MHD2D f32, pull, forcing on", "sys_mhd2d", r"collide_stream_nodeINS_8SysMhd2DIfEEfLi0ELb1ELi128ELi3ELb0ELb0E"),
     ("MHD2D f64, pull, forcing off", "sys_mhd2d", r"collide_stream_nodeINS_8SysMhd2DIdEEdLi0ELb0ELi128ELi1ELb0ELb0E"),
     ("c2 SWE f64, pull, forcing on (per launch)", "sys_swe2d", r"collide_stream_nodeINS_8SysSwe2DIdEEdLi0ELb1ELi128ELi1ELb0ELb0E"),
-    ("c2 SWE f64, persistent, forcing on", "sys_swe2d", r"collide_stream_persistentINS_8SysSwe2DIdEEdLb1E"),
+    ("c2 SWE f64, persistent (fat blocks, the one c2 runs), forcing on", "sys_swe2d", r"collide_stream_persistent_fatINS_8SysSwe2DIdEEdLb1E"),
+    ("c2 SWE f64, persistent (thin blocks), forcing on", "sys_swe2d", r"collide_stream_persistentINS_8SysSwe2DIdEEdLb1E"),
     ("c2 SWE f64, SM-resident (AA in shared memory), forcing on", "sys_swe2d", r"collide_stream_residentINS_8SysSwe2DIdEEdLb1ELi512E"),
     ("c1 advection f64, cluster-resident", "sys_advection2d", r"collide_stream_clusterINS_14SysAdvection2DIdEEdEE"),
     ("c1 advection f64, persistent", "sys_advection2d", r"collide_stream_persistentINS_14SysAdvection2DIdEEdLb0E"),
