@@ -51,8 +51,10 @@ UNIT = "MLUPS"
 # captures (profiles/), keyed by (config, pattern); None = not captured for this launch configuration.
 NCU_TRAFFIC_BYTES = {}
 try:
-    with open(os.path.join(ROOT, "profiles", "traffic_per_launch.json")) as _fh:
-        NCU_TRAFFIC_BYTES = json.load(_fh)
+    with open(os.path.join(ROOT, "profiles", "traffic_per_launch.csv")) as _fh:
+        for _ln in _fh.read().splitlines()[1:]:
+            _k, _v = _ln.rsplit(",", 1)
+            NCU_TRAFFIC_BYTES[_k] = int(_v)
 except Exception:
     NCU_TRAFFIC_BYTES = {}
 
@@ -531,7 +533,7 @@ def run_ours(args):
                    "lattice_wave_speed": max(speeds[0], speeds[1]) + speeds[2], "finite": finite},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": traffic,
-                     "traffic_source": ("constant from profiles/traffic_per_launch.json: dram__bytes_read.sum + dram__bytes_write.sum of one "
+                     "traffic_source": ("constant from profiles/traffic_per_launch.csv: dram__bytes_read.sum + dram__bytes_write.sum of one "
                                         "`ncu --set full` capture of this kernel and launch configuration (profiles/), NOT measured by this run")
                                        if traffic is not None else None,
                      "peak_source": peak_src, "frac_of_nominal_8TBps": achieved / 8000.0,
