@@ -239,7 +239,10 @@ struct Ops {
     }
     // fat blocks (kernels.cuh collide_stream_persistent_fat): 4 x 128 threads, one block per SM, when every block then owns at least
     // FAT_MIN_ROUNDS segments (so that it has an interior to hide the flag round trip behind) and the coefficients are unstaged
-    static constexpr int FAT_GROUPS = 4, FAT_MIN_ROUNDS = 8;
+#ifndef LBMK_FAT_GROUPS
+#define LBMK_FAT_GROUPS 4
+#endif
+    static constexpr int FAT_GROUPS = LBMK_FAT_GROUPS, FAT_MIN_ROUNDS = 8;
     template <class R, bool MMS>
     static constexpr bool fat_capable() {      // <= 160 B of populations per node: fits the 128 registers of a 512-thread block without spilling
         return TuneP<S, R>::BLOCK == 128 && !(MMS && C::NC >= STAGE_MIN_NC) && (size_t)M * Q * sizeof(R) <= 160;
