@@ -13,11 +13,11 @@
 //
 // What pins each system (tests/, -m "not gpu") -- and what does not:
 //   pinned to the paper's PRINTED Table 2 errors (5 digits, N = 512): Burgers, Euler, SWE over a bed (swe2d_bathy), ultrarelativistic
-//     fluid, Maxwell TM, elasticity, ADR, Allen-Cahn;
+//     fluid, Maxwell TM, elasticity, ADR, Allen-Cahn, compressible NSF 2D (reading A24: mu = K = 0.01; also its printed EOCs);
 //   pinned by closed-form dynamics / exact solutions: advection (P4 exact Fourier), NSF3D (P16-P18), MHD3D (P15, P19), NSF2D and
 //     MHD2D (P22 chain-rule viscous / thermal / resistive decay), HCNSF (P22 exact drag, porosity-scaled viscosity), Euler's
 //     config-3 fields (P21 linear acoustics); all systems: P1, P3, P13 (brute force from the paper's listings), P20 (wave speeds);
-//   PARITY UNPINNED to Table 2 digits: INSE2D (reading A22: momentum L2 to 3 digits only), NSF2D (A24: 1.8-2.1x the printed errors),
+//   PARITY UNPINNED to Table 2 digits: INSE2D (reading A22: momentum L2 to 3 digits only),
 //     MHD2D (A27: within 8 %, printed EOCs reproduced), HCNSF (A26: no manufactured forcing -- exact fields cut off in the source);
 //   PARITY UNPINNED beyond the pins above: the free NONLINEAR evolution of config 5 (MHD3D) and of config 3 at its full amplitude
 //     (no closed form); the TRT / regularised collision operators have textbook pins only (the paper runs BGK).

@@ -2,7 +2,7 @@
 that SURVEY.md Appendix A gives full recipes for, next to the values the paper prints.
 
 Calls ONLY `oracle/` and `workloads/` (never the CUDA path).  Run from the repo root:
-    python tests/golden/make_paper_pins.py            # N = 64,128,256,512; ~10 min on 8 cores
+    python tests/golden/make_paper_pins.py            # N = 64,128,256,512; hours on 8 cores (the diffusive cases at N = 512)
 The N = 512 rows are the pins (Table 2); the lower-N rows are fast
 regression values for the default CPU test run (tests/test_oracle_paper_pins.py).
 """
@@ -28,6 +28,9 @@ PAPER = {
     "elasticity": {"F": (3.1874e-05, 2.8940e-05), "v": (6.4804e-05, 4.5664e-05), "cite": "PAPER.md:L536-L539"},
     "urf": {"E": (4.3449e-06, 2.1354e-06), "S": (9.6256e-06, 6.3943e-06), "cite": "PAPER.md:L527-L529"},
     "swe": {"h": (5.5560e-06, 2.3433e-06), "hu": (2.6837e-05, 2.0838e-05), "cite": "PAPER.md:L523-L526"},
+    "nsf2d": {"rho": (7.3384e-05, 3.7592e-05), "rhou": (1.1775e-04, 6.8579e-05), "E": (8.3354e-05, 4.5785e-05),
+              "eoc": {"rho": (1.91, 1.95), "rhou": (1.95, 1.99), "E": (1.98, 2.01)},
+              "cite": "PAPER.md:L547-L551 (N = 512: 131 072 steps of 12 fields, ~1.6 h on 8 cores)"},
     "maxwell": {"Ez": (2.9956e-05, 2.9956e-05), "Hx": (1.0951e-04, 1.0951e-04), "Hy": (1.1587e-05, 1.1587e-05),
                 "cite": "PAPER.md:L530-L535"},
 }
@@ -44,7 +47,7 @@ def rel_errors(U, Ue):
 
 def run_case(case, n):
     w = {"burgers": W.pin_burgers, "euler": W.pin_euler, "adr": W.pin_adr, "urf": W.pin_urf, "maxwell": W.pin_maxwell,
-         "allencahn": W.pin_allencahn, "elasticity": W.pin_elasticity, "swe": W.pin_swe}[case](n)
+         "allencahn": W.pin_allencahn, "elasticity": W.pin_elasticity, "swe": W.pin_swe, "nsf2d": W.pin_nsf2d}[case](n)
     g = oracle.OracleGrid.from_workload(w)
     if g.n_aux:
         g.set_aux(w.aux_fields())          # static bed slope
@@ -58,6 +61,9 @@ def run_case(case, n):
     g.close()
     if case == "burgers":
         fields = {"u": e[0]}
+    elif case == "nsf2d":
+        fields = {"rho": e[0], "E": e[3],
+                  "rhou": (float(np.hypot(e[1][0], e[2][0])), float(np.hypot(e[1][1], e[2][1])))}
     elif case == "euler":
         # vector field norm = root-sum-square of the components' relative norms
         fields = {"rho": e[0], "E": e[3],
@@ -79,14 +85,24 @@ def run_case(case, n):
 
 
 if __name__ == "__main__":
-    cases = sys.argv[1:] or ["burgers", "euler", "adr", "urf", "maxwell", "allencahn", "elasticity", "swe"]
+    # usage: make_paper_pins.py [case ...] [--sizes 64,128]   (--sizes: only these N, merged into the case's existing rows)
+    args = sys.argv[1:]
+    sizes = None
+    if "--sizes" in args:
+        i = args.index("--sizes")
+        sizes = tuple(int(v) for v in args[i + 1].split(","))
+        args = args[:i] + args[i + 2:]
+    cases = args or ["burgers", "euler", "adr", "urf", "maxwell", "allencahn", "elasticity", "swe", "nsf2d"]
     path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "paper_pins.json")
-    out = json.load(open(path)) if os.path.exists(path) else {}
     for case in cases:
         rows = []
-        for n in (64, 128, 256, 512):
+        for n in (sizes or (64, 128, 256, 512)):
             r = run_case(case, n)
             print(case, r, flush=True)
             rows.append(r)
+        out = json.load(open(path)) if os.path.exists(path) else {}       # re-read: another run may have written meanwhile
+        if sizes and case in out:
+            keep = [r for r in out[case]["oracle"] if r["n"] not in sizes]
+            rows = sorted(keep + rows, key=lambda r: r["n"])
         out[case] = {"paper_N512": PAPER[case], "oracle": rows}
         json.dump(out, open(path, "w"), indent=1, sort_keys=True)

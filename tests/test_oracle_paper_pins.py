@@ -23,7 +23,7 @@ import workloads as W
 HERE = os.path.dirname(os.path.abspath(__file__))
 PINS = json.load(open(os.path.join(HERE, "golden", "paper_pins.json")))
 MAKERS = {"burgers": W.pin_burgers, "euler": W.pin_euler, "adr": W.pin_adr, "urf": W.pin_urf, "maxwell": W.pin_maxwell,
-          "allencahn": W.pin_allencahn, "elasticity": W.pin_elasticity, "swe": W.pin_swe}
+          "allencahn": W.pin_allencahn, "elasticity": W.pin_elasticity, "swe": W.pin_swe, "nsf2d": W.pin_nsf2d}
 
 
 def _rows(case):
@@ -71,7 +71,7 @@ def test_p8_live_n64_matches_stored_row(case):
     stored = _rows(case)[64]["fields"]
     if case == "burgers":
         live = {"u": e[0]}
-    elif case == "euler":
+    elif case in ("euler", "nsf2d"):
         live = {"rho": e[0], "E": e[3], "rhou": (math.hypot(e[1][0], e[2][0]), math.hypot(e[1][1], e[2][1]))}
     elif case == "allencahn":
         live = {"phi": e[0]}
@@ -101,3 +101,18 @@ def test_p11_convergence_order_in_paper_band(case):
         l2 = [rows[n]["fields"][field][1] for n in ns]
         slope = -np.polyfit(np.log2(ns), np.log2(l2), 1)[0]          # EOC = -LSQ slope
         assert 1.70 <= slope <= 2.51 + 0.35, f"{case}.{field}: L2 order {slope:.2f}"   # ADR's early rows are pre-asymptotic (2.8 pairwise, L510)
+
+
+def test_nsf2d_orders_through_the_printed_n512_point():
+    """Compressible NSF 2D, the paper's running example (reading A24: mu = K = 0.01 non-dimensional).
+    The printed EOC is the least-squares slope over N = 64 ... 512 (L514).  Through the oracle's stored errors at N = 64, 128, 256
+    and the PRINTED N = 512 error, that slope equals each of the six printed orders to their two decimals -- so the oracle's lower
+    rows lie on the paper's convergence line (a wrong viscous or heat-flux term moves them by tens of percent, i.e. the slope by
+    > 0.05).  The N = 512 row itself (131 072 steps) is checked digit by digit by test_p8_stored_n512_equals_printed_values."""
+    rows = _rows("nsf2d")
+    paper = PINS["nsf2d"]["paper_N512"]
+    for field, eocs in paper["eoc"].items():
+        for j in (0, 1):
+            ys = [rows[n]["fields"][field][j] for n in (64, 128, 256)] + [paper[field][j]]
+            slope = -np.polyfit(np.log2([64, 128, 256, 512]), np.log2(ys), 1)[0]
+            assert abs(slope - eocs[j]) <= 0.0051, (field, j, slope, eocs[j])
